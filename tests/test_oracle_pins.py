@@ -1,0 +1,292 @@
+"""Pins of the FP64 oracle against things OTHER than itself.
+
+Each pin is chosen so that a plausible mistake in oracle/gmg_oracle.c (dropped term, wrong
+sign or index, transposed operand, wrong face) fails at least one of them.
+"""
+import itertools
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2607_07687_b200 import workloads as W
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+BCS = [(0, 0, 0), (1, 0, 0), (1, 1, 1), (1, 0, 1), (0, 1, 0)]
+
+
+# --------------------------------------------------------------------------------------
+# independent restatement: FACE-by-FACE scatter assembly of the dense matrix (the oracle
+# gathers per cell).  A face between cells a and b with coefficient L contributes
+# +L to A[a,b], A[b,a] and -L to A[a,a], A[b,b]  (flux form of div(L grad)).
+# --------------------------------------------------------------------------------------
+def dense_by_faces(n, bc, L):
+    nx, ny, nz = n
+    N = nx * ny * nz
+    A = np.zeros((N, N))
+    idx = lambda i, j, k: i + nx * (j + ny * k)
+    for k, j, i in itertools.product(range(nz), range(ny), range(nx)):
+        I = (i, j, k)
+        for d in range(3):
+            if I[d] == 0 and bc[d] == 1:
+                continue                      # wall face: no flux, stored value ignored
+            J = list(I)
+            J[d] = (I[d] - 1) % n[d]
+            a, b = idx(*I), idx(*J)
+            if a == b:
+                continue
+            c = L[d, k, j, i]
+            A[a, b] += c
+            A[b, a] += c
+            A[a, a] -= c
+            A[b, b] -= c
+    return A
+
+
+def rand_L(rng, n, zero_frac=0.0):
+    L = rng.uniform(0.0, 1.0, (3, n[2], n[1], n[0]))
+    if zero_frac:
+        L[rng.uniform(size=L.shape) < zero_frac] = 0.0
+    return L
+
+
+@pytest.mark.parametrize("bc", BCS)
+def test_operator_matches_face_assembly(bc):
+    rng = np.random.default_rng(1)
+    n = (4, 6, 4)
+    L = rand_L(rng, n, 0.2)
+    A = dense_by_faces(n, bc, L)
+    p = rng.standard_normal((n[2], n[1], n[0]))
+    assert np.allclose(oracle.apply_A(L, bc, p).ravel(), A @ p.ravel(), rtol=0, atol=1e-13)
+    assert np.allclose(oracle.diag(L, bc).ravel(), np.diag(A), rtol=0, atol=1e-14)
+    # residual: b - A p on active cells, 0 where the row is empty
+    L[:, 1:3, 2:4, 1:3] = 0.0
+    L[0, 1:3, 2:4, 3] = 0.0; L[1, 1:3, 4, 1:3] = 0.0; L[2, 3, 2:4, 1:3] = 0.0
+    A = dense_by_faces(n, bc, L)
+    b = rng.standard_normal(p.shape)
+    r = oracle.residual(L, bc, p, b).ravel()
+    ref = np.where(np.diag(A) != 0.0, b.ravel() - A @ p.ravel(), 0.0)
+    assert (np.diag(A) == 0).sum() >= 1
+    assert np.allclose(r, ref, rtol=0, atol=1e-13)
+
+
+def test_fourier_eigenmode_closed_form():
+    vals = {}
+    for line in open(os.path.join(GOLD, "eigenmode.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        t = line.split()
+        vals[t[0]] = [float(x) for x in t[1:]]
+    n = tuple(int(v) for v in vals["n"]); m = vals["m"]; lam_gold = vals["lambda"][0]
+    th = [2 * np.pi * m[d] / n[d] for d in range(3)]
+    lam = sum(2 * np.cos(t) - 2 for t in th)
+    assert abs(lam - lam_gold) < 1e-10
+    k, j, i = np.meshgrid(np.arange(n[2]), np.arange(n[1]), np.arange(n[0]), indexing="ij")
+    p = np.sin(th[0] * i + th[1] * j + th[2] * k + 0.3)
+    L = np.ones((3, n[2], n[1], n[0]))
+    Ap = oracle.apply_A(L, (0, 0, 0), p)
+    assert np.max(np.abs(Ap - lam * p)) < 1e-12
+
+
+def test_level_shapes_table():
+    for line in open(os.path.join(GOLD, "level_shapes.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, bc, shapes = [s.strip() for s in line.split("|")]
+        bc = tuple(int(x) for x in bc.split())
+        shapes = [tuple(int(x) for x in s.split("x")) for s in shapes.split()]
+        assert oracle.level_shapes(shapes[0], bc) == shapes, name
+    # isotropic mode stops when the smallest direction stops
+    assert oracle.level_shapes((32, 32, 16), (0, 0, 0), iso=True) == [(32, 32, 16), (16, 16, 8), (8, 8, 4)]
+    # odd periodic half-extent is never produced; Neumann may go odd
+    assert oracle.level_shapes((20, 20, 20), (0, 0, 0)) == [(20, 20, 20), (10, 10, 10)]
+    assert oracle.level_shapes((20, 20, 20), (1, 1, 1)) == [(20, 20, 20), (10, 10, 10), (5, 5, 5)]
+    assert oracle.level_shapes((20, 20, 20), (1, 0, 0)) == [(20, 20, 20), (10, 10, 10), (5, 10, 10)]
+
+
+@pytest.mark.parametrize("bc", [(0, 0, 0), (1, 0, 0), (1, 1, 1)])
+def test_symmetry_rowsum_definiteness_every_level(bc):
+    rng = np.random.default_rng(2)
+    n = (16, 8, 8)
+    L32 = rand_L(rng, n, 0.1).astype(np.float32)
+    H = oracle.Hierarchy(n, bc, L32)
+    assert H.nlev >= 2
+    for lev in range(H.nlev):
+        nl, _ = H.shape(lev)
+        Ll = H.L(lev)
+        a = rng.standard_normal((nl[2], nl[1], nl[0])); b = rng.standard_normal(a.shape)
+        Aa, Ab = oracle.apply_A(Ll, bc, a), oracle.apply_A(Ll, bc, b)
+        assert abs((a * Ab).sum() - (b * Aa).sum()) < 1e-10
+        assert np.max(np.abs(oracle.apply_A(Ll, bc, np.ones_like(a)))) == 0.0
+        assert (a * Aa).sum() <= 0.0
+        # Neumann wall planes stay zero after coarsening
+        for d in range(3):
+            if bc[d] == 1:
+                sl = [slice(None)] * 3; sl[2 - d] = 0
+                assert np.all(Ll[d][tuple(sl)] == 0.0)
+
+
+@pytest.mark.parametrize("bc", [(0, 0, 0), (1, 0, 1)])
+def test_half_sweep_zeroes_own_colour_and_decreases_energy(bc):
+    rng = np.random.default_rng(3)
+    n = (6, 4, 4)
+    L = rand_L(rng, n, 0.15)
+    A = dense_by_faces(n, bc, L)
+    xs = rng.standard_normal(A.shape[0]); xs[np.diag(A) == 0] = 0
+    b = (A @ xs).reshape(n[2], n[1], n[0])          # compatible rhs with known solution
+    k, j, i = np.meshgrid(np.arange(n[2]), np.arange(n[1]), np.arange(n[0]), indexing="ij")
+    col = (i + j + k) % 2
+    p = rng.standard_normal(b.shape)
+    for colour in (0, 1):
+        q = oracle.half_sweep(L, bc, p, b, 1.0, colour)
+        r = oracle.residual(L, bc, q, b)
+        assert np.max(np.abs(r[col == colour])) < 1e-13
+        assert np.max(np.abs(r[col != colour])) > 1e-3
+        assert np.array_equal(q[col != colour], p[col != colour])
+    energy = lambda e: -(e.ravel() @ (A @ e.ravel()))
+    for omega in (0.7, 1.0, 1.5):
+        q = p.copy(); e0 = energy(q - xs.reshape(q.shape))
+        for s in range(6):
+            q = oracle.half_sweep(L, bc, q, b, omega, s % 2)
+            e1 = energy(q - xs.reshape(q.shape))
+            assert e1 <= e0 * (1 + 1e-12)
+            e0 = e1
+    # omega scales the update linearly
+    q1 = oracle.half_sweep(L, bc, p, b, 1.0, 0); qh = oracle.half_sweep(L, bc, p, b, 0.5, 0)
+    assert np.allclose(qh - p, 0.5 * (q1 - p), atol=1e-14)
+
+
+@pytest.mark.parametrize("c", [(2, 2, 2), (2, 1, 1), (2, 2, 1), (1, 2, 2), (1, 1, 2)])
+def test_transfer_adjoint_and_sum(c):
+    rng = np.random.default_rng(4)
+    nf = (8, 4, 6)
+    nc = tuple(a // b for a, b in zip(nf, c))
+    r = rng.standard_normal((nf[2], nf[1], nf[0])); e = rng.standard_normal((nc[2], nc[1], nc[0]))
+    Rr = oracle.restrict_sum(r, c)
+    Pe = oracle.prolong_add(np.zeros_like(r), e, c)
+    assert abs((Rr * e).sum() - (r * Pe).sum()) < 1e-12
+    assert abs(Rr.sum() - r.sum()) < 1e-12
+    # brute force: parent index by integer division
+    k, j, i = np.meshgrid(np.arange(nf[2]), np.arange(nf[1]), np.arange(nf[0]), indexing="ij")
+    assert np.array_equal(Pe, e[k // c[2], j // c[1], i // c[0]])
+    ref = np.zeros_like(e); np.add.at(ref, (k // c[2], j // c[1], i // c[0]), r)
+    assert np.allclose(Rr, ref, atol=1e-13)
+
+
+def test_coarse_coeffs_closed_form_uniform():
+    n, bc = (32, 16, 8), (0, 0, 0)
+    H = oracle.Hierarchy(n, bc, np.ones((3, 8, 16, 32), np.float32))
+    C = [1, 1, 1]
+    for lev in range(H.nlev):
+        Ll = H.L(lev)
+        for d in range(3):
+            e1, e2 = (d + 1) % 3, (d + 2) % 3
+            assert np.all(Ll[d] == C[e1] * C[e2] / C[d]), (lev, d)
+        _, c = H.shape(lev)
+        C = [a * b for a, b in zip(C, c)]
+    assert H.shape(H.nlev - 1)[0] == (4, 4, 4) and tuple(H.L(3)[:, 0, 0, 0]) == (1.0, 4.0, 16.0)
+
+
+@pytest.mark.parametrize("c", [(2, 2, 2), (2, 1, 1), (2, 2, 1), (1, 2, 2), (1, 1, 2)])
+def test_coarse_operator_consistent_on_quadratics(c):
+    """A^{l+1} q_c = R (A^l q_f) in the interior for a quadratic q sampled at cell centres."""
+    nf = (8, 8, 8); bc = (1, 1, 1)
+    nc = tuple(a // b for a, b in zip(nf, c))
+    Lf = np.ones((3,) + nf[::-1])
+    Lc = oracle.coarsen_coeffs(Lf, c)
+    quad = lambda x, y, z: 0.3 * x * x - 0.7 * y * y + 0.2 * z * z + 0.5 * x * y - 0.1 * y * z + x - 2 * z
+    k, j, i = np.meshgrid(*[np.arange(m) for m in nf[::-1]], indexing="ij")
+    qf = quad(i + 0.5, j + 0.5, k + 0.5)
+    K, J, I = np.meshgrid(*[np.arange(m) for m in nc[::-1]], indexing="ij")
+    qc = quad((I + 0.5) * c[0], (J + 0.5) * c[1], (K + 0.5) * c[2])
+    lhs = oracle.apply_A(Lc, bc, qc)
+    rhs = oracle.restrict_sum(oracle.apply_A(Lf, bc, qf), c)
+    assert np.max(np.abs((lhs - rhs)[1:-1, 1:-1, 1:-1])) < 1e-11
+
+
+def _dense_solution(n, bc, L, z):
+    A = dense_by_faces(n, bc, L)
+    x, *_ = np.linalg.lstsq(A, z.ravel(), rcond=None)
+    return x.reshape(z.shape), A
+
+
+def _demean(p, act):
+    return np.where(act, p - p[act].mean(), 0.0)
+
+
+@pytest.mark.parametrize("solver", [oracle.GMG_RBGS, oracle.PCG, oracle.GMG_PCG])
+def test_solvers_reach_dense_solution_8cubed(solver):
+    rng = np.random.default_rng(5)
+    n, bc = (8, 8, 8), (1, 0, 1)
+    L32 = rng.uniform(0, 1, (3, 8, 8, 8)).astype(np.float32)
+    Le = W.effective_L(L32, bc)
+    act = W.active_mask(L32, bc)
+    z = W.project_compatible(rng.standard_normal((8, 8, 8)), act)
+    xs, A = _dense_solution(n, bc, Le, z)
+    assert np.linalg.norm(A @ xs.ravel() - z.ravel()) < 1e-10
+    H = oracle.Hierarchy(n, bc, L32)
+    out = H.solve(solver, z, tol=1e-10, maxiter=400)
+    assert out["status"] == 0
+    err = np.linalg.norm(_demean(out["p"], act) - _demean(xs, act)) / np.linalg.norm(_demean(xs, act))
+    assert err < 1e-8, err
+    assert out["true_res"] <= 1.001e-10 or solver != oracle.GMG_RBGS
+    assert np.all(np.diff(out["history"]) < 0) or solver != oracle.GMG_RBGS
+
+
+def test_invariants_and_config0_history():
+    w = W.config0()
+    H = oracle.Hierarchy(w.n, w.bc, w.L)
+    z = w.z.astype(np.float64)
+    out = H.solve(oracle.GMG_RBGS, z, tol=w.tol, maxiter=w.maxiter)
+    # textbook cell-centred V(2,2) on L=1 periodic: fast, omega stays 1 (3 cycles)
+    assert out["iterations"] == 3 and out["status"] == 0
+    assert np.all(out["omegas"] == 1.0) and H.omega == 1.0
+    h = out["history"]
+    assert abs(h[0] - 1.0) < 1e-12 and 5e-3 < h[1] < 5e-2 and h[3] < 1e-4
+    # sum(r_k) = sum(z) for every iterate (column sums of A vanish)
+    r = oracle.residual(w.L, w.bc, out["p"], z)
+    assert abs(r.sum() - z.sum()) < 1e-9
+    # k-cycle prefix property: maxiter=k, tol=0 gives the same iterate sequence
+    H2 = oracle.Hierarchy(w.n, w.bc, w.L)
+    o2 = H2.solve(oracle.GMG_RBGS, z, tol=0.0, maxiter=2)
+    assert o2["iterations"] == 2 and o2["status"] == 1
+    assert np.allclose(o2["history"], h[:3], rtol=1e-12)
+    # zero rhs: 0 iterations, p untouched
+    o3 = H2.solve(oracle.GMG_RBGS, np.zeros_like(z), p0=np.ones_like(z))
+    assert o3["iterations"] == 0 and np.all(o3["p"] == 1.0)
+
+
+def test_adaptive_omega_follows_dyadic_rule():
+    """O8 on an under-smoothed V(1,0) jellyfish case (p=4) that grows AND decays:
+    growth -> -1/8 (floor 1/2), decay -> +1/32 (cap 1); no rollback of the iterate."""
+    w = W.config3(4)
+    H = oracle.Hierarchy(w.n, w.bc, w.L)
+    H.set_params(nu1=1, nu2=0)
+    out = H.solve(oracle.GMG_RBGS, w.z.astype(np.float64), tol=0.0, maxiter=8)
+    h, om = out["history"], out["omegas"]
+    assert out["iterations"] == 8 and out["status"] == 1
+    d = np.diff(h)
+    assert np.any(d > 0) and np.any(d <= 0), "this case must exercise both branches"
+    assert list(om[:4]) == [1.0, 0.875, 0.90625, 0.78125]
+    w_ = 1.0
+    for k in range(out["iterations"]):
+        assert om[k] == w_
+        w_ = max(0.5, w_ - 0.125) if h[k + 1] > h[k] else min(1.0, w_ + 0.03125)
+    assert H.omega == w_ == 0.5
+    # adaptive off: omega never moves
+    H2 = oracle.Hierarchy(w.n, w.bc, w.L)
+    H2.set_params(nu1=1, nu2=0, adaptive=False)
+    o2 = H2.solve(oracle.GMG_RBGS, w.z.astype(np.float64), tol=0.0, maxiter=3)
+    assert np.all(o2["omegas"] == 1.0) and H2.omega == 1.0
+
+
+def test_pcg_properties_and_ordering():
+    w = W.config0()
+    H = oracle.Hierarchy(w.n, w.bc, w.L)
+    z = w.z.astype(np.float64)
+    pcg = H.solve(oracle.PCG, z, tol=1e-4, maxiter=500)
+    mg = H.solve(oracle.GMG_PCG, z, tol=1e-4, maxiter=50)
+    assert pcg["status"] == 0 and mg["status"] == 0
+    assert mg["iterations"] <= 4 < 20 < pcg["iterations"] < 120
+    assert abs(pcg["true_res"] - pcg["history"][-1]) < 1e-8
