@@ -1,0 +1,177 @@
+/* gmg.h -- C-ABI boundary of the B200-native geometric-multigrid pressure-Poisson solve
+ * of arxiv/paper_2607_07687 ("Scaling WaterLily.jl with MPI and an improved geometric
+ * multigrid solver").  PAPER.md = /root/reference/PAPER.md.
+ *
+ * What is solved (PAPER.md:43 S3.1 "variable-coefficient Poisson equations arising in
+ * multiphase and immersed-boundary flows"; BASELINE.json:north_star):
+ *
+ *     (A p)_I = sum_d [ L_d(I) (p_{I-e_d} - p_I) + L_d(I+e_d) (p_{I+e_d} - p_I) ] = z_I
+ *
+ * on an nx*ny*nz Cartesian grid, L_d(I) >= 0 the coefficient on the LOWER d-face of cell
+ * I (reading O1).  Solvers: GMG V-cycles with the adaptive under-relaxed
+ * red-black Gauss-Seidel smoother (PAPER.md:43 S3.1) on anisotropically coarsened levels
+ * (PAPER.md:47 S3.2); Jacobi-PCG and GMG-preconditioned PCG as comparison solvers
+ * (PAPER.md:31, 39 S3).
+ *
+ * Conventions
+ *  - Layout: cell I=(i,j,k) at linear index i + nx*(j + ny*k) (x fastest), FP32.
+ *    L is component-major, [3][nz][ny][nx]: L[d*N + idx] = lower d-face of cell idx.
+ *  - bc[d]: GMG_BC_PERIODIC (index wrap; extent must be even) or GMG_BC_NEUMANN
+ *    (homogeneous: the wall faces carry coefficient 0; the caller's plane L_d(index 0)
+ *    on that axis is IGNORED and there is no upper wall face).  DESIGN.md reading O2.
+ *  - Pointers named *_dev are CUDA device pointers owned by the CALLER (torch
+ *    allocations); *_host are host pointers.  The library never frees caller memory.
+ *    The big arrays of the level hierarchy live in the caller-provided workspace; the
+ *    library itself allocates only < 4 MB of device scalars / reduction partials /
+ *    history and its pinned host mirror.
+ *  - `stream` is a cudaStream_t passed as void* (0 = legacy default stream).  All work
+ *    is enqueued on it; gmg_solve and the gmg_op_* hooks synchronise it before returning.
+ *  - Return codes: 0 ok; >0 warning (result valid); <0 error (gmg_last_error has text).
+ *    No exceptions, nothing printed.
+ *  - Determinism: all reductions are two-stage, fixed order, FP64 partials; same inputs
+ *    give bit-identical p and identical iteration counts run to run.
+ *  - There is NO CPU fallback: every step runs in CUDA kernels (sm_100a).
+ */
+#ifndef GMG_H_
+#define GMG_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gmg_ctx gmg_ctx;
+
+enum { GMG_BC_PERIODIC = 0, GMG_BC_NEUMANN = 1 };
+enum { GMG_PCG = 0, GMG_GMG_PCG = 1, GMG_GMG_RBGS = 2 };
+enum { GMG_COARSEN_ANISO = 0, GMG_COARSEN_ISO = 1 };
+enum {
+    GMG_OK = 0,
+    GMG_NOT_CONVERGED = 1, /* maxiter reached; p holds the last iterate */
+    GMG_EINVAL = -1,       /* bad argument */
+    GMG_ESTATE = -2,       /* call order: workspace / coefficients not set */
+    GMG_ECUDA = -3,        /* a CUDA call failed */
+    GMG_ENOMEM = -4,       /* workspace too small */
+    GMG_EBREAKDOWN = -5    /* PCG: d.q == 0 */
+};
+
+/* Parameters; defaults (gmg_default_params) are DESIGN.md readings O4, O7, O8. */
+typedef struct {
+    int nu_pre;        /* pre-smoothing RBGS sweeps per level           (2)  O7 */
+    int nu_post;       /* post-smoothing sweeps per level               (2)  O7 */
+    int nu_coarse;     /* sweeps on the coarsest level, even            (32) O7 */
+    float omega0;      /* initial relaxation factor                     (1)  O8 */
+    float omega_min;   /* lower bound of omega                          (1/2) */
+    float omega_down;  /* decrement after a V-cycle that grew the residual (1/8) */
+    float omega_up;    /* increment after a V-cycle that shrank it      (1/32) */
+    int adaptive;      /* 1: adapt omega after each V-cycle */
+    int coarsen_mode;  /* GMG_COARSEN_ANISO or GMG_COARSEN_ISO */
+    int n_min;         /* a direction coarsens only while n_d/2 >= n_min (4) O4 */
+    int fast_path;     /* 1: fused/tiled kernels where shapes allow; 0: generic kernels only */
+    int use_graph;     /* 1: V-cycle captured in a CUDA graph; 0: plain launches */
+} gmg_params_t;
+
+/* Statistics of the last gmg_solve. */
+typedef struct {
+    int solver;
+    int status;             /* the code gmg_solve returned */
+    int iterations;         /* V-cycles (GMG-RBGS) or CG iterations (PCG, GMG-PCG) */
+    int levels;
+    double omega_final;     /* relaxation factor after the solve (persists in the ctx) */
+    double resid_ref;       /* ||z||_2 over active cells */
+    double resid_init_rel;  /* ||z - A p0||_2 / resid_ref */
+    double resid_final_rel; /* TRUE relative residual at exit (recomputed for PCG) */
+    double gpu_ms;          /* CUDA-event time of the enqueued solve on `stream` */
+    double bytes_algorithmic; /* algorithmic HBM bytes of the solve (DESIGN.md table) */
+    long long kernel_launches; /* kernels launched (graph nodes count) by the solve */
+    int history_len;        /* entries available through gmg_history (iterations+1) */
+} gmg_stats_t;
+
+/* -- life cycle ------------------------------------------------------------------------ */
+
+/* Create a context for an nx*ny*nz grid.  Every n_d >= 2; a periodic axis needs an even
+ * extent (red/black colouring, reading O3).  Builds the level-shape table by the
+ * anisotropic rule (reading O4).  Uses the current CUDA device. */
+int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]);
+void gmg_destroy(gmg_ctx* ctx);
+const char* gmg_last_error(const gmg_ctx* ctx);
+
+void gmg_default_params(gmg_params_t* out);
+/* Changes parameters; rebuilds the level table (coefficients must be set again) and
+ * resets omega to omega0.  Must precede gmg_workspace_bytes / gmg_set_workspace. */
+int gmg_set_params(gmg_ctx* ctx, const gmg_params_t* params);
+int gmg_get_params(const gmg_ctx* ctx, gmg_params_t* out);
+
+/* Bytes of device workspace needed (coarse levels: L, p, b; ping-pong buffers; 4 PCG
+ * vectors), and hand-over of a caller-allocated block (256-byte aligned). */
+size_t gmg_workspace_bytes(const gmg_ctx* ctx);
+int gmg_set_workspace(gmg_ctx* ctx, void* ws_dev, size_t bytes);
+
+/* Set the level-0 face coefficients (kept BY POINTER: L_dev must stay valid and
+ * unchanged until the next gmg_set_coeffs / gmg_destroy) and coarsen them to every level
+ * (reading O5: L_d^{l+1}(J) = (1/c_d) * sum of the fine L_d on the faces tiling the coarse
+ * face).  Checks on device that every value is finite and >= 0 (GMG_EINVAL otherwise).
+ * Resets omega to omega0. */
+int gmg_set_coeffs(gmg_ctx* ctx, const float* L_dev, void* stream);
+
+/* Solve A p = z.  p_dev: in = initial guess, out = solution (in place).  Stops when
+ * ||z - A p||_2 <= tol * ||z||_2 (norms over active cells, reading O9) or after maxiter
+ * iterations (tol = 0 runs exactly maxiter).  solver: GMG_PCG, GMG_GMG_PCG, GMG_GMG_RBGS.
+ * The whole iteration runs on the device (a CUDA-graph WHILE loop); the host reads one
+ * status block at the end.  Returns GMG_OK / GMG_NOT_CONVERGED or an error. */
+int gmg_solve(gmg_ctx* ctx, float* p_dev, const float* z_dev, float tol, int maxiter,
+              int solver, void* stream);
+
+/* Same solve with HOST buffers (pinned or pageable): copies z (and the initial guess p)
+ * host->device into library-held staging carved from the workspace, solves, copies p back.
+ * This is the end-to-end entry point bench.py times as `e2e`. */
+int gmg_solve_host(gmg_ctx* ctx, float* p_host, const float* z_host, float tol, int maxiter,
+                   int solver, void* stream);
+
+int gmg_stats(const gmg_ctx* ctx, gmg_stats_t* out);
+/* Relative residual history of the last solve: out[k] = ||r_k|| / ||z||, k = 0..iterations.
+ * Returns the number of entries written (<= cap). */
+int gmg_history(const gmg_ctx* ctx, double* out, int cap);
+/* Relaxation factors used by V-cycle k+1 (k = 0..iterations-1) of the last GMG-RBGS solve. */
+int gmg_omega_history(const gmg_ctx* ctx, double* out, int cap);
+int gmg_set_omega(gmg_ctx* ctx, float omega);
+
+/* -- level table and per-operator hooks (parity tests; BASELINE.json tolerances for
+ *    "single operator applications") --------------------------------------------------- */
+int gmg_num_levels(const gmg_ctx* ctx);
+/* n = extents of level lev, c = coarsening factors from lev to lev+1 ((1,1,1) on the last). */
+int gmg_level_shape(const gmg_ctx* ctx, int lev, int n[3], int c[3]);
+/* Copies the [3][nz][ny][nx] coefficients of level lev to L_out_dev (device). */
+int gmg_level_coeffs(gmg_ctx* ctx, int lev, float* L_out_dev, void* stream);
+/* r = b - A p on active cells, 0 elsewhere (reading O9). */
+int gmg_op_residual(gmg_ctx* ctx, int lev, const float* p_dev, const float* b_dev, float* r_dev,
+                    void* stream);
+/* nsweeps RBGS sweeps in place; each sweep = colour first_colour then the other
+ * (0 = red = (i+j+k) even; reading O3):  p_I += omega (b_I - (A p)_I) / D_I. */
+int gmg_op_smooth(gmg_ctx* ctx, int lev, float* p_dev, const float* b_dev, float omega,
+                  int nsweeps, int first_colour, void* stream);
+/* b_coarse(J) = sum over the children of J of r_fine (reading O6). */
+int gmg_op_restrict(gmg_ctx* ctx, int lev, const float* r_fine_dev, float* b_coarse_dev,
+                    void* stream);
+/* Fused form the V-cycle uses: b_coarse = R (b - A p) without storing the residual. */
+int gmg_op_residual_restrict(gmg_ctx* ctx, int lev, const float* p_dev, const float* b_dev,
+                             float* b_coarse_dev, void* stream);
+/* p_fine(I) += e_coarse(parent(I)) (reading O6). */
+int gmg_op_prolong(gmg_ctx* ctx, int lev, const float* e_coarse_dev, float* p_fine_dev,
+                   void* stream);
+/* One V(nu_pre,nu_post) cycle on level 0 at the given omega (reading O7); symmetric != 0
+ * = the variant used as CG preconditioner (reading O11). */
+int gmg_op_vcycle(gmg_ctx* ctx, float* p_dev, const float* z_dev, float omega, int symmetric,
+                  void* stream);
+/* sqrt(sum r^2) of a level-lev array (deterministic two-stage reduction). */
+int gmg_op_norm2(gmg_ctx* ctx, int lev, const float* r_dev, double* out_host, void* stream);
+
+/* Names of the kernels a V-cycle launches per level, for profiling notes: writes a
+ * NUL-terminated description into buf. */
+int gmg_describe_plan(const gmg_ctx* ctx, char* buf, size_t cap);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GMG_H_ */

@@ -1,0 +1,766 @@
+// gmg_api.cu -- C-ABI boundary (include/gmg.h) and the host-side driver of the solve: level
+// table (reading O4), workspace carving, V-cycle enqueue (reading O7), the solve
+// loops (O9-O11) as CUDA graphs with a device-side WHILE node, statistics.
+// Product path: no CPU fallback, nothing from oracle/.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <vector>
+
+#include "gmg_internal.h"
+
+namespace gmgf {  // fast-path launchers (kernels_fused.cu)
+bool sweep_supported(const LevelGeom& g);
+// nsweeps (even count handled by caller) fused red+black sweeps src -> dst (out of place).
+// first_colour 0: red then black.  If e_c != nullptr the prolonged coarse correction is added
+// to src on the fly (fused prolongation + correction).
+void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
+              const float* omega, int first_colour, const float* e_c, cudaStream_t s);
+bool resrestrict_supported(const LevelGeom& g);
+void residual_restrict(const LevelGeom& g, const float* L, const float* p, const float* b,
+                       float* b_c, float* p_c, cudaStream_t s);
+int configure();
+}  // namespace gmgf
+
+struct GraphSlot {
+    cudaGraphExec_t exec = nullptr;
+    cudaGraph_t graph = nullptr;
+    float* p = nullptr;
+    const float* z = nullptr;
+    int solver = -1;
+    float tol = 0.0f;
+    int maxiter = -1;
+    double* hist = nullptr;
+    long long n_pre = 0, n_body = 0, n_post = 0;  // kernel launches per section
+};
+
+struct gmg_ctx {
+    int n0[3], bc[3];
+    gmg_params_t prm;
+    int nlev;
+    LevelGeom g[GMG_MAX_LEVELS];
+    LevelPtrs lv[GMG_MAX_LEVELS];
+    int tail_start;       // first level run inside the single-CTA tail kernel (nlev = none)
+    size_t tail_smem;
+    bool fast_sweep[GMG_MAX_LEVELS];
+    bool fast_rr[GMG_MAX_LEVELS];
+    // workspace
+    void* ws;
+    size_t ws_bytes;
+    bool ws_set, coeffs_set;
+    float *pcg_r, *pcg_d, *pcg_q, *pcg_s, *stage_p, *stage_z;
+    // small library-owned device state
+    DevScalars* sc;
+    double* partials;
+    unsigned int* counter;
+    double *hist, *omegas;
+    int hist_cap;
+    DevScalars* sc_host;  // pinned mirror
+    std::vector<double> hist_host, omegas_host;
+    gmg_stats_t stats;
+    cudaEvent_t ev0, ev1;
+    cudaStream_t cap_a, cap_b;  // internal streams used only for graph capture
+    GraphSlot slots[3];
+    long long n_launch;   // launch counter of the section being enqueued
+    char err[512];
+};
+
+#define SET_ERR(ctx, ...) snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__)
+#define CUDA_TRY(ctx, call)                                                              \
+    do {                                                                                 \
+        cudaError_t e_ = (call);                                                         \
+        if (e_ != cudaSuccess) {                                                         \
+            SET_ERR(ctx, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, \
+                    __LINE__);                                                           \
+            return GMG_ECUDA;                                                            \
+        }                                                                                \
+    } while (0)
+
+static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+static inline ReduceBuf rbuf(gmg_ctx* c) { return ReduceBuf{c->partials, c->counter, c->sc}; }
+
+// ---- level table: reading O4 ("downsamples every dimension independently") ------
+static void build_levels(gmg_ctx* c) {
+    LevelGeom g0;
+    for (int d = 0; d < 3; ++d) {
+        g0.n[d] = c->n0[d];
+        g0.bc[d] = c->bc[d];
+    }
+    c->nlev = 0;
+    LevelGeom cur = g0;
+    while (true) {
+        cur.N = (long long)cur.n[0] * cur.n[1] * cur.n[2];
+        int any = 0, all = 1;
+        for (int d = 0; d < 3; ++d) {
+            const int h = cur.n[d] / 2;
+            const int ok = (cur.n[d] % 2 == 0) && (h >= c->prm.n_min) &&
+                           (cur.bc[d] == GMG_BC_NEUMANN || h % 2 == 0);
+            cur.c[d] = ok ? 2 : 1;
+            any |= ok;
+            all &= ok;
+        }
+        if (c->prm.coarsen_mode == GMG_COARSEN_ISO && !all) any = 0;
+        if (!any || c->nlev + 1 >= GMG_MAX_LEVELS) cur.c[0] = cur.c[1] = cur.c[2] = 1;
+        c->g[c->nlev++] = cur;
+        if (cur.c[0] * cur.c[1] * cur.c[2] == 1) break;
+        for (int d = 0; d < 3; ++d) cur.n[d] /= cur.c[d];
+    }
+    // tail: the longest suffix of levels that fits one CTA's shared memory
+    const size_t cap = 200 * 1024;
+    c->tail_start = c->nlev;
+    size_t cells = 0;
+    for (int l = c->nlev - 1; l >= 0; --l) {
+        cells += (size_t)c->g[l].N;
+        if (cells * 5 * sizeof(float) > cap || c->nlev - l > GMG_TAIL_MAX_LEVELS) break;
+        c->tail_start = l;
+        c->tail_smem = cells * 5 * sizeof(float);
+    }
+    for (int l = 0; l < c->nlev; ++l) {
+        c->fast_sweep[l] = c->prm.fast_path && gmgf::sweep_supported(c->g[l]);
+        c->fast_rr[l] = c->prm.fast_path && l + 1 < c->nlev && gmgf::resrestrict_supported(c->g[l]);
+    }
+}
+
+static size_t carve(gmg_ctx* c, char* base) {
+    size_t off = 0;
+    auto take = [&](size_t nfloat) -> float* {
+        float* ptr = base ? (float*)(base + off) : nullptr;
+        off += align_up(nfloat * sizeof(float));
+        return ptr;
+    };
+    for (int l = 0; l < c->nlev; ++l) {
+        const size_t N = (size_t)c->g[l].N;
+        if (l > 0) {
+            float* L = take(3 * N);
+            float* p = take(N);
+            float* b = take(N);
+            if (base) {
+                c->lv[l].L = L;
+                c->lv[l].p = p;
+                c->lv[l].b = b;
+            }
+        }
+        float* q = take(N);
+        if (base) c->lv[l].q = q;
+    }
+    const size_t N0 = (size_t)c->g[0].N;
+    float* v[6];
+    for (int i = 0; i < 6; ++i) v[i] = take(N0);
+    if (base) {
+        c->pcg_r = v[0]; c->pcg_d = v[1]; c->pcg_q = v[2]; c->pcg_s = v[3];
+        c->stage_p = v[4]; c->stage_z = v[5];
+    }
+    return off;
+}
+
+static void drop_graphs(gmg_ctx* c) {
+    for (auto& s : c->slots) {
+        if (s.exec) cudaGraphExecDestroy(s.exec);
+        if (s.graph) cudaGraphDestroy(s.graph);
+        s = GraphSlot();
+    }
+}
+
+extern "C" void gmg_default_params(gmg_params_t* p) {
+    p->nu_pre = 2; p->nu_post = 2; p->nu_coarse = 32;
+    p->omega0 = 1.0f; p->omega_min = 0.5f; p->omega_down = 0.125f; p->omega_up = 0.03125f;
+    p->adaptive = 1; p->coarsen_mode = GMG_COARSEN_ANISO; p->n_min = 4;
+    p->fast_path = 1; p->use_graph = 1;
+}
+
+extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]) {
+    if (!out || !bc) return GMG_EINVAL;
+    *out = nullptr;
+    const int n[3] = {nx, ny, nz};
+    for (int d = 0; d < 3; ++d) {
+        if (n[d] < 2) return GMG_EINVAL;
+        if (bc[d] != GMG_BC_PERIODIC && bc[d] != GMG_BC_NEUMANN) return GMG_EINVAL;
+        if (bc[d] == GMG_BC_PERIODIC && (n[d] & 1)) return GMG_EINVAL;  // reading O3
+    }
+    if ((long long)nx * ny * nz > (1LL << 31) - 1) return GMG_EINVAL;
+    gmg_ctx* c = new gmg_ctx();
+    memset(c->err, 0, sizeof(c->err));
+    for (int d = 0; d < 3; ++d) { c->n0[d] = n[d]; c->bc[d] = bc[d]; }
+    gmg_default_params(&c->prm);
+    c->ws = nullptr; c->ws_bytes = 0; c->ws_set = false; c->coeffs_set = false;
+    c->hist = c->omegas = nullptr; c->hist_cap = 0;
+    memset(&c->stats, 0, sizeof(c->stats));
+    memset(c->lv, 0, sizeof(c->lv));
+    c->sc = nullptr; c->partials = nullptr; c->counter = nullptr; c->sc_host = nullptr;
+    c->ev0 = c->ev1 = nullptr;
+    c->cap_a = c->cap_b = nullptr;
+    build_levels(c);
+    cudaError_t e = cudaMalloc(&c->sc, sizeof(DevScalars));
+    if (e == cudaSuccess) e = cudaMalloc(&c->partials, 2 * GMG_REDUCE_MAX_BLOCKS * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&c->counter, sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMemset(c->sc, 0, sizeof(DevScalars));
+    if (e == cudaSuccess) e = cudaMemset(c->counter, 0, sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMallocHost(&c->sc_host, sizeof(DevScalars));
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->cap_a, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->cap_b, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = (cudaError_t)gmgk::tail_configure(200 * 1024);
+    if (e == cudaSuccess) e = (cudaError_t)gmgf::configure();
+    if (e == cudaSuccess) {
+        gmgk::ctl_set_omega(c->sc, (double)c->prm.omega0, 0);
+        e = cudaDeviceSynchronize();
+    }
+    if (e != cudaSuccess) {
+        gmg_destroy(c);
+        return GMG_ECUDA;
+    }
+    *out = c;
+    return GMG_OK;
+}
+
+extern "C" void gmg_destroy(gmg_ctx* c) {
+    if (!c) return;
+    drop_graphs(c);
+    if (c->sc) cudaFree(c->sc);
+    if (c->partials) cudaFree(c->partials);
+    if (c->counter) cudaFree(c->counter);
+    if (c->hist) cudaFree(c->hist);
+    if (c->omegas) cudaFree(c->omegas);
+    if (c->sc_host) cudaFreeHost(c->sc_host);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->cap_a) cudaStreamDestroy(c->cap_a);
+    if (c->cap_b) cudaStreamDestroy(c->cap_b);
+    delete c;
+}
+
+extern "C" const char* gmg_last_error(const gmg_ctx* c) { return c ? c->err : "null context"; }
+
+extern "C" int gmg_set_params(gmg_ctx* c, const gmg_params_t* p) {
+    if (!c || !p) return GMG_EINVAL;
+    if (p->nu_pre < 0 || p->nu_post < 0 || p->nu_coarse < 0 || (p->nu_coarse & 1) || p->n_min < 1 ||
+        !(p->omega0 > 0.0f) || !(p->omega_min > 0.0f) ||
+        (p->coarsen_mode != GMG_COARSEN_ANISO && p->coarsen_mode != GMG_COARSEN_ISO)) {
+        SET_ERR(c, "gmg_set_params: invalid parameter");
+        return GMG_EINVAL;
+    }
+    c->prm = *p;
+    drop_graphs(c);
+    build_levels(c);
+    c->ws_set = false;
+    c->coeffs_set = false;
+    gmgk::ctl_set_omega(c->sc, (double)p->omega0, 0);
+    CUDA_TRY(c, cudaDeviceSynchronize());
+    return GMG_OK;
+}
+
+extern "C" int gmg_get_params(const gmg_ctx* c, gmg_params_t* out) {
+    if (!c || !out) return GMG_EINVAL;
+    *out = c->prm;
+    return GMG_OK;
+}
+
+extern "C" size_t gmg_workspace_bytes(const gmg_ctx* c) {
+    if (!c) return 0;
+    return carve(const_cast<gmg_ctx*>(c), nullptr);
+}
+
+extern "C" int gmg_set_workspace(gmg_ctx* c, void* ws, size_t bytes) {
+    if (!c || !ws) return GMG_EINVAL;
+    if (((uintptr_t)ws) & 255) { SET_ERR(c, "workspace must be 256-byte aligned"); return GMG_EINVAL; }
+    const size_t need = carve(c, nullptr);
+    if (bytes < need) { SET_ERR(c, "workspace too small: %zu < %zu", bytes, need); return GMG_ENOMEM; }
+    drop_graphs(c);
+    carve(c, (char*)ws);
+    c->ws = ws; c->ws_bytes = bytes; c->ws_set = true; c->coeffs_set = false;
+    return GMG_OK;
+}
+
+extern "C" int gmg_num_levels(const gmg_ctx* c) { return c ? c->nlev : GMG_EINVAL; }
+
+extern "C" int gmg_level_shape(const gmg_ctx* c, int lev, int n[3], int cf[3]) {
+    if (!c || lev < 0 || lev >= c->nlev) return GMG_EINVAL;
+    for (int d = 0; d < 3; ++d) {
+        if (n) n[d] = c->g[lev].n[d];
+        if (cf) cf[d] = c->g[lev].c[d];
+    }
+    return GMG_OK;
+}
+
+// ---- coefficients: reading O5 ("anisotropic coarsening operators") ---------------
+extern "C" int gmg_set_coeffs(gmg_ctx* c, const float* L_dev, void* stream) {
+    if (!c || !L_dev) return GMG_EINVAL;
+    if (!c->ws_set) { SET_ERR(c, "gmg_set_coeffs before gmg_set_workspace"); return GMG_ESTATE; }
+    cudaStream_t s = (cudaStream_t)stream;
+    drop_graphs(c);
+    c->lv[0].L = L_dev;
+    gmgk::check_coeffs(c->g[0], L_dev, rbuf(c), s);
+    for (int l = 0; l + 1 < c->nlev; ++l)
+        gmgk::coarsen_coeffs(c->g[l], c->lv[l].L, const_cast<float*>(c->lv[l + 1].L), s);
+    gmgk::ctl_set_omega(c->sc, (double)c->prm.omega0, s);
+    CUDA_TRY(c, cudaGetLastError());
+    CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(c, cudaStreamSynchronize(s));
+    if (c->sc_host->red[RED_CHECK] != 0.0) {
+        SET_ERR(c, "gmg_set_coeffs: %.0f coefficient(s) negative, NaN or infinite",
+                c->sc_host->red[RED_CHECK]);
+        c->coeffs_set = false;
+        return GMG_EINVAL;
+    }
+    c->coeffs_set = true;
+    return GMG_OK;
+}
+
+extern "C" int gmg_level_coeffs(gmg_ctx* c, int lev, float* L_out_dev, void* stream) {
+    if (!c || lev < 0 || lev >= c->nlev || !L_out_dev) return GMG_EINVAL;
+    if (!c->coeffs_set) { SET_ERR(c, "coefficients not set"); return GMG_ESTATE; }
+    cudaStream_t s = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaMemcpyAsync(L_out_dev, c->lv[lev].L, 3 * (size_t)c->g[lev].N * sizeof(float),
+                                cudaMemcpyDeviceToDevice, s));
+    CUDA_TRY(c, cudaStreamSynchronize(s));
+    return GMG_OK;
+}
+
+// ---- smoothing: nsweeps RBGS sweeps, result in p (reading O3) --------------------
+// e_c != nullptr: the coarse correction P e_c is added to p first (fused into the first sweep
+// on the fast path, a separate kernel otherwise).
+static void smooth(gmg_ctx* c, int l, float* p, const float* b, const float* omega, int nsweeps,
+                   int first_colour, const float* e_c, cudaStream_t s) {
+    const LevelGeom& g = c->g[l];
+    int done = 0;
+    if (c->fast_sweep[l] && nsweeps >= 2) {
+        float* q = c->lv[l].q;
+        const int pairs = nsweeps / 2;
+        for (int i = 0; i < pairs; ++i) {
+            gmgf::rb_sweep(g, c->lv[l].L, p, q, b, omega, first_colour, (i == 0) ? e_c : nullptr, s);
+            gmgf::rb_sweep(g, c->lv[l].L, q, p, b, omega, first_colour, nullptr, s);
+            c->n_launch += 2;
+        }
+        done = 2 * pairs;
+        e_c = nullptr;
+    }
+    if (e_c) {
+        gmgk::prolong_add(g, e_c, p, s);
+        c->n_launch += 1;
+    }
+    for (int i = done; i < nsweeps; ++i) {
+        gmgk::half_sweep(g, c->lv[l].L, p, b, omega, first_colour, s);
+        gmgk::half_sweep(g, c->lv[l].L, p, b, omega, 1 - first_colour, s);
+        c->n_launch += 2;
+    }
+}
+
+// ---- V-cycle: reading O7 (PAPER.md:39 smoother + coarse-grid correction; 51 "V-cycle") -------
+static void enqueue_vcycle(gmg_ctx* c, float* p0, const float* b0, const float* omega, int sym,
+                           cudaStream_t s) {
+    const int nlev = c->nlev, ts = c->tail_start;
+    auto P = [&](int l) { return l == 0 ? p0 : c->lv[l].p; };
+    auto B = [&](int l) { return l == 0 ? b0 : (const float*)c->lv[l].b; };
+    const int post_first = sym ? 1 : 0;
+    int l = 0;
+    for (; l < ts && l < nlev - 1; ++l) {
+        smooth(c, l, P(l), B(l), omega, c->prm.nu_pre, 0, nullptr, s);
+        if (c->fast_rr[l])
+            gmgf::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, s);
+        else
+            gmgk::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, s);
+        c->n_launch += 1;
+    }
+    if (ts < nlev) {
+        // l == ts: the rest of the hierarchy is one single-CTA kernel
+        TailArgs a;
+        memset(&a, 0, sizeof(a));
+        a.nlev = nlev - ts;
+        for (int t = 0; t < a.nlev; ++t) {
+            a.g[t] = c->g[ts + t];
+            a.L[t] = c->lv[ts + t].L;
+        }
+        a.b_in = B(ts);
+        a.p_in = (ts == 0) ? p0 : nullptr;
+        a.p_out = P(ts);
+        a.omega = omega;
+        a.nu1 = c->prm.nu_pre; a.nu2 = c->prm.nu_post; a.nuc = c->prm.nu_coarse; a.sym = sym;
+        gmgk::tail_vcycle(a, c->tail_smem, s);
+        c->n_launch += 1;
+    } else {
+        // coarsest level too large for shared memory: plain half-sweep launches
+        const int cl = nlev - 1;
+        if (!sym) {
+            smooth(c, cl, P(cl), B(cl), omega, c->prm.nu_coarse, 0, nullptr, s);
+        } else {
+            smooth(c, cl, P(cl), B(cl), omega, c->prm.nu_coarse / 2, 0, nullptr, s);
+            smooth(c, cl, P(cl), B(cl), omega, c->prm.nu_coarse / 2, 1, nullptr, s);
+        }
+    }
+    for (l = (ts < nlev ? ts : nlev - 1) - 1; l >= 0; --l)
+        smooth(c, l, P(l), B(l), omega, c->prm.nu_post, post_first, c->lv[l + 1].p, s);
+}
+
+// Algorithmic HBM bytes of one V-cycle + its stopping-test norm.
+static double vcycle_bytes(const gmg_ctx* c, bool with_norm) {
+    double total = 0.0;
+    for (int l = 0; l < c->nlev; ++l) {
+        const double N = (double)c->g[l].N;
+        const double m = (double)(c->g[l].c[0] * c->g[l].c[1] * c->g[l].c[2]);
+        if (l == c->nlev - 1) {
+            total += N * 24.0 * c->prm.nu_coarse;
+        } else {
+            total += N * 24.0 * (c->prm.nu_pre + c->prm.nu_post);  // fused red+black sweeps
+            total += N * (20.0 + 4.0 / m);                          // residual + restriction
+            total += N * (4.0 / m);                                 // prolongation fused in a sweep
+        }
+    }
+    if (with_norm) total += 20.0 * (double)c->g[0].N;
+    return total;
+}
+
+// ---- solve sections (enqueue only; capturable) -------------------------------------------------
+struct LoopCtl {
+    cudaGraphConditionalHandle cond;
+    int use_cond;
+};
+
+// GMG-RBGS (readings O8, O9): pre = reference norm + initial residual norm + loop entry test.
+static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
+    gmgk::active_norm2(c->g[0], c->lv[0].L, z, rbuf(c), RED_RREF, s);
+    gmgk::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, s);
+    gmgk::ctl_begin(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
+    c->n_launch += 3;
+}
+static void rbgs_body(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
+    enqueue_vcycle(c, p, z, &c->sc->omega_f, 0, s);
+    gmgk::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, s);
+    gmgk::ctl_rbgs_cycle_end(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
+    c->n_launch += 2;
+}
+
+// PCG / GMG-PCG (readings O10, O11).
+static void pcg_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
+    gmgk::active_norm2(c->g[0], c->lv[0].L, z, rbuf(c), RED_RREF, s);
+    gmgk::residual(c->g[0], c->lv[0].L, p, z, c->pcg_r, s);
+    gmgk::norm2(c->g[0].N, c->pcg_r, rbuf(c), RED_RR, s);
+    gmgk::fill(c->pcg_d, c->g[0].N, 0.0f, s);
+    gmgk::ctl_begin(c->sc, c->hist, nullptr, lc.cond, lc.use_cond, s);
+    c->n_launch += 5;
+}
+static void pcg_body(gmg_ctx* c, float* p, int gmg_precond, LoopCtl lc, cudaStream_t s) {
+    const long long N = c->g[0].N;
+    if (!gmg_precond) {
+        gmgk::jacobi_apply(c->g[0], c->lv[0].L, c->pcg_r, c->pcg_s, rbuf(c), RED_RS, s);
+        c->n_launch += 1;
+    } else {
+        gmgk::fill(c->pcg_s, N, 0.0f, s);
+        enqueue_vcycle(c, c->pcg_s, c->pcg_r, &c->sc->omega_one, 1, s);
+        gmgk::dot(N, c->pcg_r, c->pcg_s, rbuf(c), RED_RS, s);
+        c->n_launch += 2;
+    }
+    gmgk::ctl_pcg_beta(c->sc, s);
+    gmgk::pcg_update_d(N, c->pcg_d, c->pcg_s, c->sc, 0, s);
+    gmgk::matvec_dot(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rbuf(c), RED_DQ, s);
+    gmgk::ctl_pcg_alpha(c->sc, s);
+    gmgk::pcg_update_pr(c->g[0], c->lv[0].L, p, c->pcg_r, c->pcg_d, c->pcg_q, nullptr, 0, rbuf(c), s);
+    gmgk::ctl_pcg_check(c->sc, c->hist, lc.cond, lc.use_cond, s);
+    c->n_launch += 6;
+}
+static void pcg_post(gmg_ctx* c, float* p, const float* z, cudaStream_t s) {
+    // true residual at exit (the recursive one drove the test)
+    gmgk::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, s);
+    c->n_launch += 1;
+}
+
+static void enqueue_init(gmg_ctx* c, float tol, int maxiter, cudaStream_t s) {
+    gmgk::ctl_init(c->sc, (double)tol, maxiter, c->prm.adaptive, (double)c->prm.omega_min,
+                   (double)c->prm.omega_down, (double)c->prm.omega_up, s);
+    c->n_launch += 1;
+}
+
+static void enqueue_pre(gmg_ctx* c, int solver, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
+    if (solver == GMG_GMG_RBGS) rbgs_pre(c, p, z, lc, s); else pcg_pre(c, p, z, lc, s);
+}
+static void enqueue_body(gmg_ctx* c, int solver, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
+    if (solver == GMG_GMG_RBGS) rbgs_body(c, p, z, lc, s);
+    else pcg_body(c, p, solver == GMG_GMG_PCG, lc, s);
+}
+static void enqueue_post(gmg_ctx* c, int solver, float* p, const float* z, cudaStream_t s) {
+    if (solver != GMG_GMG_RBGS) pcg_post(c, p, z, s);
+}
+
+// Whole solve as ONE graph: init, pre, WHILE(cond){body}, post.
+static int build_graph(gmg_ctx* c, GraphSlot& slot, int solver, float* p, const float* z, float tol,
+                       int maxiter) {
+    if (slot.exec) { cudaGraphExecDestroy(slot.exec); slot.exec = nullptr; }
+    if (slot.graph) { cudaGraphDestroy(slot.graph); slot.graph = nullptr; }
+    cudaGraph_t graph = nullptr;
+    CUDA_TRY(c, cudaGraphCreate(&graph, 0));
+    slot.graph = graph;
+    LoopCtl lc;
+    lc.use_cond = 1;
+    CUDA_TRY(c, cudaGraphConditionalHandleCreate(&lc.cond, graph, 0, cudaGraphCondAssignDefault));
+    CUDA_TRY(c, cudaStreamBeginCaptureToGraph(c->cap_a, graph, nullptr, nullptr, 0,
+                                              cudaStreamCaptureModeRelaxed));
+    c->n_launch = 0;
+    enqueue_init(c, tol, maxiter, c->cap_a);
+    enqueue_pre(c, solver, p, z, lc, c->cap_a);
+    slot.n_pre = c->n_launch;
+    // conditional WHILE node after everything captured so far
+    cudaStreamCaptureStatus st;
+    const cudaGraphNode_t* deps = nullptr;
+    size_t ndeps = 0;
+    cudaGraph_t gcap = nullptr;
+    CUDA_TRY(c, cudaStreamGetCaptureInfo(c->cap_a, &st, nullptr, &gcap, &deps, &ndeps));
+    cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+    np.type = cudaGraphNodeTypeConditional;
+    np.conditional.handle = lc.cond;
+    np.conditional.type = cudaGraphCondTypeWhile;
+    np.conditional.size = 1;
+    cudaGraphNode_t wnode = nullptr;
+    CUDA_TRY(c, cudaGraphAddNode(&wnode, graph, deps, ndeps, &np));
+    cudaGraph_t body = np.conditional.phGraph_out[0];
+    CUDA_TRY(c, cudaStreamBeginCaptureToGraph(c->cap_b, body, nullptr, nullptr, 0,
+                                              cudaStreamCaptureModeRelaxed));
+    c->n_launch = 0;
+    enqueue_body(c, solver, p, z, lc, c->cap_b);
+    slot.n_body = c->n_launch;
+    cudaGraph_t body_out = nullptr;
+    CUDA_TRY(c, cudaStreamEndCapture(c->cap_b, &body_out));
+    CUDA_TRY(c, cudaStreamUpdateCaptureDependencies(c->cap_a, &wnode, 1,
+                                                    cudaStreamSetCaptureDependencies));
+    c->n_launch = 0;
+    enqueue_post(c, solver, p, z, c->cap_a);
+    slot.n_post = c->n_launch;
+    cudaGraph_t gout = nullptr;
+    CUDA_TRY(c, cudaStreamEndCapture(c->cap_a, &gout));
+    CUDA_TRY(c, cudaGetLastError());
+    CUDA_TRY(c, cudaGraphInstantiate(&slot.exec, graph, 0));
+    slot.p = p; slot.z = z; slot.solver = solver; slot.tol = tol; slot.maxiter = maxiter;
+    slot.hist = c->hist;
+    return GMG_OK;
+}
+
+static int ensure_history(gmg_ctx* c, int maxiter) {
+    const int need = maxiter + 2;
+    if (need <= c->hist_cap) return GMG_OK;
+    drop_graphs(c);
+    if (c->hist) cudaFree(c->hist);
+    if (c->omegas) cudaFree(c->omegas);
+    c->hist = c->omegas = nullptr;
+    c->hist_cap = 0;
+    const int cap = need < 64 ? 64 : need;
+    CUDA_TRY(c, cudaMalloc(&c->hist, sizeof(double) * cap));
+    CUDA_TRY(c, cudaMalloc(&c->omegas, sizeof(double) * cap));
+    c->hist_cap = cap;
+    return GMG_OK;
+}
+
+extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int maxiter, int solver,
+                         void* stream) {
+    if (!c) return GMG_EINVAL;
+    if (!p || !z || !(tol >= 0.0f) || maxiter < 0 || solver < GMG_PCG || solver > GMG_GMG_RBGS) {
+        SET_ERR(c, "gmg_solve: invalid argument");
+        return GMG_EINVAL;
+    }
+    if (!c->ws_set || !c->coeffs_set) {
+        SET_ERR(c, "gmg_solve before gmg_set_workspace / gmg_set_coeffs");
+        return GMG_ESTATE;
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_history(c, maxiter);
+    if (rc != GMG_OK) return rc;
+    long long launches = 0;
+    CUDA_TRY(c, cudaEventRecord(c->ev0, s));
+    if (c->prm.use_graph) {
+        GraphSlot& slot = c->slots[solver];
+        if (!slot.exec || slot.p != p || slot.z != z || slot.tol != tol || slot.maxiter != maxiter ||
+            slot.hist != c->hist) {
+            rc = build_graph(c, slot, solver, p, z, tol, maxiter);
+            if (rc != GMG_OK) {
+                // leave no stream in capture mode behind
+                cudaGraph_t junk = nullptr;
+                cudaStreamEndCapture(c->cap_b, &junk);
+                cudaStreamEndCapture(c->cap_a, &junk);
+                cudaGetLastError();
+                return rc;
+            }
+            CUDA_TRY(c, cudaEventRecord(c->ev0, s));
+        }
+        CUDA_TRY(c, cudaGraphLaunch(slot.exec, s));
+        CUDA_TRY(c, cudaEventRecord(c->ev1, s));
+        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
+        CUDA_TRY(c, cudaStreamSynchronize(s));
+        launches = slot.n_pre + slot.n_post + slot.n_body * (long long)c->sc_host->iter;
+    } else {
+        LoopCtl lc;
+        lc.cond = 0;
+        lc.use_cond = 0;
+        c->n_launch = 0;
+        enqueue_init(c, tol, maxiter, s);
+        enqueue_pre(c, solver, p, z, lc, s);
+        while (true) {
+            CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
+            CUDA_TRY(c, cudaStreamSynchronize(s));
+            if (c->sc_host->done) break;
+            enqueue_body(c, solver, p, z, lc, s);
+            CUDA_TRY(c, cudaGetLastError());
+        }
+        enqueue_post(c, solver, p, z, s);
+        CUDA_TRY(c, cudaEventRecord(c->ev1, s));
+        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
+        CUDA_TRY(c, cudaStreamSynchronize(s));
+        launches = c->n_launch;
+    }
+    CUDA_TRY(c, cudaGetLastError());
+    const DevScalars& h = *c->sc_host;
+    const int it = h.iter;
+    c->hist_host.assign((size_t)it + 1, 0.0);
+    c->omegas_host.assign((size_t)it, 0.0);
+    CUDA_TRY(c, cudaMemcpy(c->hist_host.data(), c->hist, sizeof(double) * (it + 1), cudaMemcpyDeviceToHost));
+    if (solver == GMG_GMG_RBGS && it > 0)
+        CUDA_TRY(c, cudaMemcpy(c->omegas_host.data(), c->omegas, sizeof(double) * it, cudaMemcpyDeviceToHost));
+    float ms = 0.0f;
+    CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+    gmg_stats_t& st = c->stats;
+    st.solver = solver;
+    st.status = h.status;
+    st.iterations = it;
+    st.levels = c->nlev;
+    st.omega_final = h.omega;
+    st.resid_ref = h.r_ref;
+    st.resid_init_rel = c->hist_host[0];
+    if (solver == GMG_GMG_RBGS) st.resid_final_rel = c->hist_host[it];
+    else st.resid_final_rel = (h.r_ref > 0.0) ? sqrt(h.red[RED_RR]) / h.r_ref : 0.0;
+    st.gpu_ms = ms;
+    st.kernel_launches = launches;
+    st.history_len = it + 1;
+    const double N0 = (double)c->g[0].N;
+    if (solver == GMG_GMG_RBGS) st.bytes_algorithmic = 36.0 * N0 + it * vcycle_bytes(c, true);
+    else if (solver == GMG_PCG) st.bytes_algorithmic = 60.0 * N0 + it * 64.0 * N0;
+    else st.bytes_algorithmic = 60.0 * N0 + it * (vcycle_bytes(c, false) + 52.0 * N0);
+    if (h.status == GMG_EBREAKDOWN) SET_ERR(c, "PCG breakdown: d.q == 0 at iteration %d", it);
+    return h.status;
+}
+
+extern "C" int gmg_solve_host(gmg_ctx* c, float* p_host, const float* z_host, float tol, int maxiter,
+                              int solver, void* stream) {
+    if (!c || !p_host || !z_host) return GMG_EINVAL;
+    if (!c->ws_set || !c->coeffs_set) { SET_ERR(c, "gmg_solve_host before setup"); return GMG_ESTATE; }
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t bytes = (size_t)c->g[0].N * sizeof(float);
+    CUDA_TRY(c, cudaMemcpyAsync(c->stage_z, z_host, bytes, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(c, cudaMemcpyAsync(c->stage_p, p_host, bytes, cudaMemcpyHostToDevice, s));
+    const int rc = gmg_solve(c, c->stage_p, c->stage_z, tol, maxiter, solver, stream);
+    if (rc < 0) return rc;
+    CUDA_TRY(c, cudaMemcpyAsync(p_host, c->stage_p, bytes, cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(c, cudaStreamSynchronize(s));
+    return rc;
+}
+
+extern "C" int gmg_stats(const gmg_ctx* c, gmg_stats_t* out) {
+    if (!c || !out) return GMG_EINVAL;
+    *out = c->stats;
+    return GMG_OK;
+}
+
+extern "C" int gmg_history(const gmg_ctx* c, double* out, int cap) {
+    if (!c || !out || cap < 0) return GMG_EINVAL;
+    int n = (int)c->hist_host.size();
+    if (n > cap) n = cap;
+    for (int i = 0; i < n; ++i) out[i] = c->hist_host[i];
+    return n;
+}
+
+extern "C" int gmg_omega_history(const gmg_ctx* c, double* out, int cap) {
+    if (!c || !out || cap < 0) return GMG_EINVAL;
+    int n = (int)c->omegas_host.size();
+    if (n > cap) n = cap;
+    for (int i = 0; i < n; ++i) out[i] = c->omegas_host[i];
+    return n;
+}
+
+extern "C" int gmg_set_omega(gmg_ctx* c, float omega) {
+    if (!c || !(omega > 0.0f)) return GMG_EINVAL;
+    gmgk::ctl_set_omega(c->sc, (double)omega, 0);
+    CUDA_TRY(c, cudaDeviceSynchronize());
+    return GMG_OK;
+}
+
+// ---- per-operator hooks (parity tests) -----------------------------------------------------------
+#define HOOK_PROLOGUE(cond_)                                                        \
+    if (!c) return GMG_EINVAL;                                                      \
+    if (!(cond_)) { SET_ERR(c, "%s: invalid argument", __func__); return GMG_EINVAL; } \
+    if (!c->ws_set || !c->coeffs_set) { SET_ERR(c, "%s before setup", __func__); return GMG_ESTATE; } \
+    cudaStream_t s = (cudaStream_t)stream;
+
+#define HOOK_EPILOGUE()                       \
+    CUDA_TRY(c, cudaGetLastError());          \
+    CUDA_TRY(c, cudaStreamSynchronize(s));    \
+    return GMG_OK;
+
+extern "C" int gmg_op_residual(gmg_ctx* c, int lev, const float* p, const float* b, float* r,
+                               void* stream) {
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && p && b && r)
+    gmgk::residual(c->g[lev], c->lv[lev].L, p, b, r, s);
+    HOOK_EPILOGUE()
+}
+
+extern "C" int gmg_op_smooth(gmg_ctx* c, int lev, float* p, const float* b, float omega, int nsweeps,
+                             int first_colour, void* stream) {
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && p && b && nsweeps >= 0 &&
+                  (first_colour == 0 || first_colour == 1))
+    gmgk::ctl_set_hook_omega(c->sc, omega, s);
+    smooth(c, lev, p, b, &c->sc->omega_hook, nsweeps, first_colour, nullptr, s);
+    HOOK_EPILOGUE()
+}
+
+extern "C" int gmg_op_restrict(gmg_ctx* c, int lev, const float* r_fine, float* b_coarse, void* stream) {
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev - 1 && r_fine && b_coarse)
+    gmgk::restrict_sum(c->g[lev], r_fine, b_coarse, s);
+    HOOK_EPILOGUE()
+}
+
+extern "C" int gmg_op_residual_restrict(gmg_ctx* c, int lev, const float* p, const float* b,
+                                        float* b_coarse, void* stream) {
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev - 1 && p && b && b_coarse)
+    if (c->fast_rr[lev]) gmgf::residual_restrict(c->g[lev], c->lv[lev].L, p, b, b_coarse, nullptr, s);
+    else gmgk::residual_restrict(c->g[lev], c->lv[lev].L, p, b, b_coarse, nullptr, s);
+    HOOK_EPILOGUE()
+}
+
+extern "C" int gmg_op_prolong(gmg_ctx* c, int lev, const float* e_coarse, float* p_fine, void* stream) {
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev - 1 && e_coarse && p_fine)
+    gmgk::prolong_add(c->g[lev], e_coarse, p_fine, s);
+    HOOK_EPILOGUE()
+}
+
+extern "C" int gmg_op_vcycle(gmg_ctx* c, float* p, const float* z, float omega, int symmetric,
+                             void* stream) {
+    HOOK_PROLOGUE(p && z)
+    gmgk::ctl_set_hook_omega(c->sc, omega, s);
+    enqueue_vcycle(c, p, z, &c->sc->omega_hook, symmetric ? 1 : 0, s);
+    HOOK_EPILOGUE()
+}
+
+extern "C" int gmg_op_norm2(gmg_ctx* c, int lev, const float* r, double* out_host, void* stream) {
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && r && out_host)
+    gmgk::norm2(c->g[lev].N, r, rbuf(c), RED_HOOK, s);
+    CUDA_TRY(c, cudaGetLastError());
+    CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(c, cudaStreamSynchronize(s));
+    *out_host = sqrt(c->sc_host->red[RED_HOOK]);
+    return GMG_OK;
+}
+
+extern "C" int gmg_describe_plan(const gmg_ctx* c, char* buf, size_t cap) {
+    if (!c || !buf || cap == 0) return GMG_EINVAL;
+    size_t off = 0;
+    buf[0] = 0;
+    for (int l = 0; l < c->nlev; ++l) {
+        const char* how = (l >= c->tail_start) ? "tail(single-CTA smem)"
+                          : (c->fast_sweep[l] ? "fused-rb-sweep" : "generic-half-sweeps");
+        const char* rr = (l >= c->tail_start || l == c->nlev - 1) ? "-"
+                         : (c->fast_rr[l] ? "tiled" : "generic");
+        int w = snprintf(buf + off, cap - off, "L%d %dx%dx%d c=%d%d%d sweep=%s resrestrict=%s\n", l,
+                         c->g[l].n[0], c->g[l].n[1], c->g[l].n[2], c->g[l].c[0], c->g[l].c[1],
+                         c->g[l].c[2], how, rr);
+        if (w < 0 || (size_t)w >= cap - off) break;
+        off += (size_t)w;
+    }
+    return GMG_OK;
+}

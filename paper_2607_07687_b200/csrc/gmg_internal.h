@@ -1,0 +1,131 @@
+// gmg_internal.h -- host/device shared PODs and kernel-launcher prototypes of the CUDA path.
+// Part of the product path; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/gmg.h"
+
+#define GMG_MAX_LEVELS 24
+#define GMG_TAIL_MAX_LEVELS 8
+
+// Geometry of one multigrid level (passed to kernels by value).
+struct LevelGeom {
+    int n[3];     // extents (nx, ny, nz), x fastest
+    int bc[3];    // 0 periodic, 1 Neumann
+    int c[3];     // coarsening factors to the next level (1 or 2)
+    long long N;  // nx*ny*nz
+};
+
+// Device pointers of one level.
+struct LevelPtrs {
+    const float* L;  // [3][N] component-major; level 0: the caller's array
+    float* p;        // level >= 1 unknown (level 0: caller's p, set per call)
+    float* b;        // level >= 1 right-hand side
+    float* q;        // ping-pong partner of p for the fused sweep
+};
+
+// Device scalar block: everything the on-device iteration control needs.
+struct DevScalars {
+    double red[16];    // results of the two-stage reductions (slot per use)
+    double r_ref;      // ||z||_2 over active cells
+    double rho;        // current residual norm
+    double rho_prev;
+    double omega;      // relaxation factor (dyadic, exact in float)
+    double tol;
+    double alpha, beta, rho_cg, rho_cg_new;
+    double omega_min, omega_down, omega_up;
+    float omega_f;     // omega as the kernels read it
+    float omega_one;   // constant 1.0f (GMG-PCG preconditioner runs at omega = 1)
+    float omega_hook;  // omega of the gmg_op_* hooks
+    int iter;
+    int maxiter;
+    int status;        // GMG_OK, GMG_NOT_CONVERGED, GMG_EBREAKDOWN
+    int done;          // 1: loop finished
+    int adaptive;
+    int pad;
+};
+
+enum {
+    RED_RREF = 0,  // sum z^2 over active cells
+    RED_RR = 1,    // sum r^2
+    RED_DQ = 2,    // d.q
+    RED_RS = 3,    // r.s
+    RED_HOOK = 4,  // gmg_op_norm2
+    RED_CHECK = 5  // coefficient check: count of bad values
+};
+
+// Tail: levels small enough to live in one CTA's shared memory, run as ONE kernel.
+struct TailArgs {
+    int nlev;                            // number of tail levels (>= 1)
+    LevelGeom g[GMG_TAIL_MAX_LEVELS];
+    const float* L[GMG_TAIL_MAX_LEVELS]; // global coefficients of each tail level
+    const float* b_in;                   // right-hand side of the first tail level (global)
+    const float* p_in;                   // initial guess of the first tail level; nullptr = zero
+    float* p_out;                        // solution of the first tail level (global; may alias p_in)
+    const float* omega;                  // device scalar
+    int nu1, nu2, nuc, sym;
+};
+
+// Reduction workspace: FP64 block partials.
+struct ReduceBuf {
+    double* partials;       // [2][GMG_REDUCE_MAX_BLOCKS] (a kernel reduces at most two sums)
+    unsigned int* counter;  // ticket of the "last block finishes the sum" stage, self-resetting
+    DevScalars* sc;
+};
+#define GMG_REDUCE_MAX_BLOCKS 4096
+
+// ---- launchers (kernels_generic.cu) --------------------------------------------------------
+namespace gmgk {
+
+void half_sweep(const LevelGeom& g, const float* L, float* p, const float* b, const float* omega,
+                int colour, cudaStream_t s);
+void residual(const LevelGeom& g, const float* L, const float* p, const float* b, float* r,
+              cudaStream_t s);
+void restrict_sum(const LevelGeom& gf, const float* rf, float* bc, cudaStream_t s);
+// b_c = R(b - A p); also zeroes p_c (the coarse initial guess) when p_c != nullptr.
+void residual_restrict(const LevelGeom& gf, const float* L, const float* p, const float* b,
+                       float* b_c, float* p_c, cudaStream_t s);
+void fill(float* x, long long N, float v, cudaStream_t s);
+void prolong_add(const LevelGeom& gf, const float* e_c, float* p_f, cudaStream_t s);
+void coarsen_coeffs(const LevelGeom& gf, const float* Lf, float* Lc, cudaStream_t s);
+void check_coeffs(const LevelGeom& g, const float* L, ReduceBuf rb, cudaStream_t s);
+void tail_vcycle(const TailArgs& a, size_t smem_bytes, cudaStream_t s);
+size_t tail_smem_bytes(const TailArgs& a);
+int tail_configure(size_t max_bytes);  // sets the dynamic-smem attribute; returns cudaError
+
+// reductions: result lands in rb.sc->red[slot]
+void residual_norm2(const LevelGeom& g, const float* L, const float* p, const float* b,
+                    ReduceBuf rb, int slot, cudaStream_t s);
+void active_norm2(const LevelGeom& g, const float* L, const float* z, ReduceBuf rb, int slot,
+                  cudaStream_t s);
+void norm2(long long N, const float* r, ReduceBuf rb, int slot, cudaStream_t s);
+void dot(long long N, const float* a, const float* b, ReduceBuf rb, int slot, cudaStream_t s);
+
+// PCG pieces
+void matvec_dot(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb,
+                int slot, cudaStream_t s);              // q = A d ; red[slot] = d.q
+void pcg_update_pr(const LevelGeom& g, const float* L, float* p, float* r, const float* d,
+                   const float* q, float* s_out, int jacobi, ReduceBuf rb, cudaStream_t st);
+// p += alpha d; r -= alpha q; red[RR] = r.r; if jacobi: s = r/D, red[RS] = r.s
+void pcg_update_d(long long N, float* d, const float* s_in, const DevScalars* sc, int first,
+                  cudaStream_t st);                      // d = s + beta d   (first: d = s)
+void jacobi_apply(const LevelGeom& g, const float* L, const float* r, float* s_out, ReduceBuf rb,
+                  int slot, cudaStream_t st);            // s = r/D ; red[slot] = r.s
+
+// on-device iteration control (single-thread kernels, kernels_ctl.cu).  `cond` is the WHILE
+// node's conditional handle; use_cond = 0 outside a graph.
+void ctl_init(DevScalars* sc, double tol, int maxiter, int adaptive, double omega_min,
+              double omega_down, double omega_up, cudaStream_t s);
+void ctl_begin(DevScalars* sc, double* hist, double* omegas, cudaGraphConditionalHandle cond,
+               int use_cond, cudaStream_t s);
+void ctl_rbgs_cycle_end(DevScalars* sc, double* hist, double* omegas,
+                        cudaGraphConditionalHandle cond, int use_cond, cudaStream_t s);
+void ctl_pcg_beta(DevScalars* sc, cudaStream_t s);
+void ctl_pcg_alpha(DevScalars* sc, cudaStream_t s);
+void ctl_pcg_check(DevScalars* sc, double* hist, cudaGraphConditionalHandle cond, int use_cond,
+                   cudaStream_t s);
+void ctl_set_hook_omega(DevScalars* sc, float omega, cudaStream_t s);
+void ctl_set_omega(DevScalars* sc, double omega, cudaStream_t s);
+
+}  // namespace gmgk

@@ -1,0 +1,109 @@
+// stencil.cuh -- device helpers shared by every kernel of the CUDA path, so that the generic,
+// fused and single-CTA kernels produce bit-identical cell updates.
+//
+// Operator (reading O1; PAPER.md:43 S3.1 "variable-coefficient Poisson"):
+//   (A p)_I = sum_d [ L_d(I)(p_{I-e_d} - p_I) + L_d(I+e_d)(p_{I+e_d} - p_I) ]
+//   D_I     = - sum_d [ L_d(I) + L_d(I+e_d) ]          cell active  <=>  D_I != 0
+// Boundary handling (reading O2): periodic = index wrap; Neumann = coefficient 0 on the wall
+// faces (the stored plane L_d(index 0) is ignored; there is no upper wall face).
+#pragma once
+#include "gmg_internal.h"
+
+namespace gmgd {
+
+// The one arithmetic order used everywhere: x-lo, x-hi, y-lo, y-hi, z-lo, z-hi.
+__device__ __forceinline__ float apply7(float pc, float wxl, float wxh, float wyl, float wyh,
+                                        float wzl, float wzh, float pxl, float pxh, float pyl,
+                                        float pyh, float pzl, float pzh) {
+    float s = wxl * (pxl - pc);
+    s = fmaf(wxh, pxh - pc, s);
+    s = fmaf(wyl, pyl - pc, s);
+    s = fmaf(wyh, pyh - pc, s);
+    s = fmaf(wzl, pzl - pc, s);
+    s = fmaf(wzh, pzh - pc, s);
+    return s;
+}
+
+__device__ __forceinline__ float diag6(float wxl, float wxh, float wyl, float wyh, float wzl,
+                                       float wzh) {
+    return -(((wxl + wxh) + (wyl + wyh)) + (wzl + wzh));
+}
+
+// RBGS cell update (readings O3, O8):  p_I += omega (b_I - (A p)_I) / D_I  on active cells.
+__device__ __forceinline__ float relax(float pc, float b, float Ap, float D, float omega) {
+    return (D != 0.0f) ? pc + __fdividef(omega * (b - Ap), D) : pc;
+}
+
+// Gathers the seven p values and six face coefficients of cell (i,j,k) with plain loads.
+// Works on global or shared pointers.  Out-of-range neighbours on a Neumann axis read a
+// wrapped (valid, finite) value that is multiplied by a zero coefficient.
+struct Cell {
+    float pc, Ap, D;
+};
+
+__device__ __forceinline__ void face_coeffs(const LevelGeom& g, const float* __restrict__ L, int i,
+                                            int j, int k, long long c, float w[6]) {
+    const long long N = g.N;
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const long long sy = nx, sz = (long long)nx * ny;
+    const float* Lx = L;
+    const float* Ly = L + N;
+    const float* Lz = L + 2 * N;
+    w[0] = (i == 0 && g.bc[0]) ? 0.0f : Lx[c];
+    w[1] = (i == nx - 1) ? (g.bc[0] ? 0.0f : Lx[c - (nx - 1)]) : Lx[c + 1];
+    w[2] = (j == 0 && g.bc[1]) ? 0.0f : Ly[c];
+    w[3] = (j == ny - 1) ? (g.bc[1] ? 0.0f : Ly[c - sy * (ny - 1)]) : Ly[c + sy];
+    w[4] = (k == 0 && g.bc[2]) ? 0.0f : Lz[c];
+    w[5] = (k == nz - 1) ? (g.bc[2] ? 0.0f : Lz[c - sz * (nz - 1)]) : Lz[c + sz];
+}
+
+__device__ __forceinline__ Cell cell_stencil(const LevelGeom& g, const float* __restrict__ L,
+                                             const float* __restrict__ p, int i, int j, int k) {
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const long long sy = nx, sz = (long long)nx * ny;
+    const long long c = i + sy * j + sz * k;
+    float w[6];
+    face_coeffs(g, L, i, j, k, c, w);
+    const float pc = p[c];
+    const float pxl = p[(i == 0) ? c + (nx - 1) : c - 1];
+    const float pxh = p[(i == nx - 1) ? c - (nx - 1) : c + 1];
+    const float pyl = p[(j == 0) ? c + sy * (ny - 1) : c - sy];
+    const float pyh = p[(j == ny - 1) ? c - sy * (ny - 1) : c + sy];
+    const float pzl = p[(k == 0) ? c + sz * (nz - 1) : c - sz];
+    const float pzh = p[(k == nz - 1) ? c - sz * (nz - 1) : c + sz];
+    Cell r;
+    r.pc = pc;
+    r.Ap = apply7(pc, w[0], w[1], w[2], w[3], w[4], w[5], pxl, pxh, pyl, pyh, pzl, pzh);
+    r.D = diag6(w[0], w[1], w[2], w[3], w[4], w[5]);
+    return r;
+}
+
+__device__ __forceinline__ float cell_diag(const LevelGeom& g, const float* __restrict__ L, int i,
+                                           int j, int k) {
+    const long long c = i + (long long)g.n[0] * (j + (long long)g.n[1] * k);
+    float w[6];
+    face_coeffs(g, L, i, j, k, c, w);
+    return diag6(w[0], w[1], w[2], w[3], w[4], w[5]);
+}
+
+// Deterministic block reduction of one double per thread; result valid in thread 0.
+// blockDim.x must be a multiple of 32 and <= 1024.
+__device__ __forceinline__ double block_sum(double v) {
+    __shared__ double warp_part[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    __syncthreads();  // protects warp_part across successive calls
+    if (lane == 0) warp_part[wid] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (wid == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        t = (lane < nw) ? warp_part[lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+    }
+    return t;
+}
+
+}  // namespace gmgd
