@@ -1,0 +1,82 @@
+"""CPU-side checks of the boundary: the C-ABI library builds, loads and exports every symbol
+include/gmg.h declares; the Python binding names match; argument validation that needs no
+GPU.  No compute calls here."""
+import ctypes as C
+import os
+import re
+import subprocess
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "gmg.h")
+
+
+def _declared_symbols():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(gmg_[a-z0-9_]+)\s*\(", src)))
+
+
+@pytest.fixture(scope="module")
+def libpath():
+    from paper_2607_07687_b200 import build
+    return build.build()
+
+
+def test_header_declares_the_north_star_entry_points():
+    syms = _declared_symbols()
+    for name in ("gmg_create", "gmg_set_coeffs", "gmg_solve", "gmg_stats"):
+        assert name in syms
+
+
+def test_library_exports_every_declared_symbol(libpath):
+    dll = C.CDLL(libpath)
+    for name in _declared_symbols():
+        assert hasattr(dll, name), f"{name} declared in gmg.h but not exported"
+    out = subprocess.check_output(["nm", "-D", "--defined-only", libpath]).decode()
+    exported = set(re.findall(r" T (gmg_[a-z0-9_]+)", out))
+    assert exported == set(_declared_symbols())
+
+
+def test_binding_covers_every_symbol(libpath):
+    from paper_2607_07687_b200 import gmg
+    assert sorted(gmg.SIGNATURES) == _declared_symbols()
+
+
+def test_library_contains_sm100a_code(libpath):
+    out = subprocess.run(["cuobjdump", "-lelf", libpath], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+
+
+def test_struct_sizes_match_header(libpath):
+    """Params / Stats mirror the C structs (12 x 4 bytes; Stats has 8-byte alignment)."""
+    from paper_2607_07687_b200 import gmg
+    assert C.sizeof(gmg.Params) == 48
+    assert C.sizeof(gmg.Stats) == 4 * 4 + 6 * 8 + 8 + 8
+    p = gmg.Params()
+    gmg.lib.gmg_default_params(C.byref(p))
+    assert (p.nu_pre, p.nu_post, p.nu_coarse, p.n_min) == (2, 2, 32, 4)
+    assert (p.omega0, p.omega_min, p.omega_down, p.omega_up) == (1.0, 0.5, 0.125, 0.03125)
+
+
+def test_null_arguments_are_rejected_without_a_gpu(libpath):
+    from paper_2607_07687_b200 import gmg
+    I3 = C.c_int * 3
+    assert gmg.lib.gmg_create(None, 8, 8, 8, I3(0, 0, 0)) == gmg.EINVAL
+    h = C.c_void_p()
+    assert gmg.lib.gmg_create(C.byref(h), 7, 8, 8, I3(0, 0, 0)) == gmg.EINVAL   # odd periodic
+    assert gmg.lib.gmg_create(C.byref(h), 1, 8, 8, I3(1, 0, 0)) == gmg.EINVAL   # extent < 2
+    assert gmg.lib.gmg_create(C.byref(h), 8, 8, 8, I3(0, 2, 0)) == gmg.EINVAL   # bad bc
+    assert gmg.lib.gmg_num_levels(None) == gmg.EINVAL
+    assert gmg.lib.gmg_workspace_bytes(None) == 0
+
+
+def test_product_path_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2607_07687_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import oracle|from oracle)", txt, flags=re.M), f
+                assert "gmg_oracle" not in txt and "libgmg_oracle" not in txt, f

@@ -1,0 +1,138 @@
+"""-m gpu: per-operator parity of the CUDA path (through the C-ABI) against the FP64 oracle.
+
+Bar (BASELINE.json:north_star): relative L-infinity <= 1e-5 for single operator applications
+(residual, one smoothing sweep, restrict, prolong); level shapes exact; coarse coefficients to
+FP32 rounding."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2607_07687_b200 import workloads as W
+from gpu_util import TOL_OP, dev, host, make_gpu, make_oracle, random_workload, rel_linf
+
+pytestmark = pytest.mark.gpu
+
+CASES = {
+    "c0": lambda: W.config0(),
+    "rand_PPP": lambda: random_workload((24, 16, 12), (0, 0, 0), 11),
+    "rand_NPN": lambda: random_workload((20, 24, 10), (1, 0, 1), 12),
+    "rand_NNN_odd": lambda: random_workload((15, 9, 7), (1, 1, 1), 13),
+    "rand_ragged": lambda: random_workload((36, 20, 6), (0, 1, 0), 14),
+    "c3p5": lambda: W.config3(5),
+    "c4_64": lambda: W.config4(n=64, nspheres=8, diameter=8),
+    "sphere_D4": lambda: W.config2(D=4),
+}
+
+
+@pytest.fixture(scope="module", params=sorted(CASES), ids=sorted(CASES))
+def case(request):
+    wl = CASES[request.param]()
+    g = make_gpu(wl)
+    h = make_oracle(wl)
+    yield wl, g, h
+    g.close()
+
+
+def _fields(n, seed):
+    rng = np.random.default_rng(seed)
+    shp = (n[2], n[1], n[0])
+    return (rng.standard_normal(shp).astype(np.float32), rng.standard_normal(shp).astype(np.float32))
+
+
+def test_level_shapes_match_oracle(case):
+    wl, g, h = case
+    assert g.num_levels() == h.nlev
+    for l in range(h.nlev):
+        assert g.level_shape(l) == h.shape(l)
+
+
+def test_coarse_coefficients(case):
+    wl, g, h = case
+    for l in range(h.nlev):
+        Lg = host(g.level_coeffs(l))
+        Lo = h.L(l)
+        if l == 0:
+            # level 0 is the caller's array; the library ignores the Neumann wall plane
+            Lg = W.effective_L(Lg, wl.bc)
+        assert rel_linf(Lg, Lo) <= 1e-6, l
+        assert np.array_equal(Lg == 0.0, Lo == 0.0), l      # activity pattern is exact
+
+
+def test_residual_every_level(case):
+    wl, g, h = case
+    for l in range(h.nlev):
+        n, _ = h.shape(l)
+        p, b = _fields(n, 100 + l)
+        r = host(g.op_residual(l, dev(p), dev(b)))
+        ro = h.level_residual(l, p, b)
+        assert rel_linf(r, ro) <= TOL_OP, (l, rel_linf(r, ro))
+        assert np.array_equal(r == 0.0, ro == 0.0) or np.count_nonzero((r == 0) != (ro == 0)) < 3
+
+
+@pytest.mark.parametrize("omega,first", [(1.0, 0), (0.8125, 0), (1.0, 1)])
+def test_one_sweep_every_level(case, omega, first):
+    wl, g, h = case
+    for l in range(h.nlev):
+        n, _ = h.shape(l)
+        p, b = _fields(n, 200 + l)
+        out = host(g.op_smooth(l, dev(p), dev(b), omega=omega, nsweeps=1, first_colour=first))
+        ref = h.level_sweeps(l, p, b, omega=omega, count=1, first_colour=first)
+        assert rel_linf(out, ref) <= TOL_OP, (l, rel_linf(out, ref))
+
+
+def test_two_and_three_sweeps(case):
+    """Even counts take the ping-pong fused path where the level supports it; odd counts mix
+    it with the generic half-sweeps."""
+    wl, g, h = case
+    for l in range(min(h.nlev, 3)):
+        n, _ = h.shape(l)
+        p, b = _fields(n, 300 + l)
+        for cnt in (2, 3):
+            out = host(g.op_smooth(l, dev(p), dev(b), omega=1.0, nsweeps=cnt, first_colour=0))
+            ref = h.level_sweeps(l, p, b, omega=1.0, count=cnt, first_colour=0)
+            assert rel_linf(out, ref) <= 3 * TOL_OP, (l, cnt, rel_linf(out, ref))
+
+
+def test_restrict_and_fused_residual_restrict(case):
+    wl, g, h = case
+    for l in range(h.nlev - 1):
+        n, c = h.shape(l)
+        p, b = _fields(n, 400 + l)
+        ro = h.level_residual(l, p, b)
+        bc_o = oracle.restrict_sum(ro, c)
+        bc_g = host(g.op_restrict(l, dev(ro)))
+        assert rel_linf(bc_g, bc_o) <= TOL_OP, l
+        fused = host(g.op_residual_restrict(l, dev(p), dev(b)))
+        assert rel_linf(fused, bc_o) <= TOL_OP, (l, rel_linf(fused, bc_o))
+
+
+def test_prolong_every_level(case):
+    wl, g, h = case
+    for l in range(h.nlev - 1):
+        n, c = h.shape(l)
+        nc, _ = h.shape(l + 1)
+        p, _ = _fields(n, 500 + l)
+        e, _ = _fields(nc, 600 + l)
+        out = host(g.op_prolong(l, dev(e), dev(p)))
+        ref = oracle.prolong_add(p, e, c)
+        assert rel_linf(out, ref) <= 1e-6, l
+
+
+@pytest.mark.parametrize("sym", [False, True])
+def test_one_vcycle(case, sym):
+    """One V(2,2) cycle from a zero guess; the tolerance allows for the accumulated rounding of
+    ~20 operator applications (derived in DESIGN.md)."""
+    wl, g, h = case
+    p = torch.zeros(wl.z.shape, dtype=torch.float32, device="cuda")
+    out = host(g.op_vcycle(p, dev(wl.z), omega=1.0, symmetric=sym))
+    ref = h.vcycle(np.zeros_like(wl.z, dtype=np.float64), wl.z, omega=1.0, sym=sym)
+    act = W.active_mask(wl.L, wl.bc)
+    assert rel_linf(np.where(act, out, 0), np.where(act, ref, 0)) <= 1e-4, rel_linf(out, ref)
+
+
+def test_norm2(case):
+    wl, g, h = case
+    r = np.random.default_rng(7).standard_normal(wl.z.shape).astype(np.float32)
+    got = g.op_norm2(0, dev(r))
+    assert abs(got - np.linalg.norm(r.astype(np.float64))) <= 1e-12 * np.linalg.norm(r)

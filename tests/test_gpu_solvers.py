@@ -1,0 +1,275 @@
+"""-m gpu: solver parity of the CUDA path against the FP64 oracle on the BASELINE.json configs.
+
+Bar (BASELINE.json:north_star): V-cycle / iteration counts within +-1; final pressure relative
+L2 <= 1e-4 (compared at EQUAL iteration count, mean over active cells removed);
+residual below the stated tolerance."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2607_07687_b200 import gmg
+from paper_2607_07687_b200 import workloads as W
+from gpu_util import TOL_P, dev, host, make_gpu, make_oracle, random_workload, rel_l2_demeaned
+
+pytestmark = pytest.mark.gpu
+
+SOLVERS = {"rbgs": (gmg.GMG_RBGS, oracle.GMG_RBGS), "gmgpcg": (gmg.GMG_PCG, oracle.GMG_PCG),
+           "pcg": (gmg.PCG, oracle.PCG)}
+
+CONFIGS = {
+    "c0": (lambda: W.config0(), ("rbgs", "gmgpcg", "pcg"), 2000),
+    "c1": (lambda: W.config1(), ("rbgs", "gmgpcg", "pcg"), 2000),
+    "c2": (lambda: W.config2(), ("rbgs", "gmgpcg"), 2000),
+    "c3p5": (lambda: W.config3(5), ("rbgs", "gmgpcg", "pcg"), 2000),
+    "c3p6": (lambda: W.config3(6), ("rbgs", "gmgpcg"), 2000),
+    "c4_128": (lambda: W.by_name("c4_128"), ("rbgs", "gmgpcg"), 2000),
+}
+
+
+def _solve_gpu(g, wl, solver, tol, maxiter, p0=None):
+    p = torch.zeros(wl.z.shape, dtype=torch.float32, device="cuda") if p0 is None else dev(p0)
+    rc = g.solve(p, dev(wl.z), tol=tol, maxiter=maxiter, solver=solver)
+    st = g.stats()
+    return rc, host(p), st, g.history()
+
+
+@pytest.mark.parametrize("name", sorted(CONFIGS))
+def test_solver_parity(name):
+    mk, solvers, pcg_cap = CONFIGS[name]
+    wl = mk()
+    act = W.active_mask(wl.L, wl.bc)
+    g = make_gpu(wl)
+    h = make_oracle(wl)
+    try:
+        for sname in solvers:
+            sg, so = SOLVERS[sname]
+            maxiter = wl.maxiter if sname != "pcg" else pcg_cap
+            g.set_omega(1.0)
+            rc, p, st, hist = _solve_gpu(g, wl, sg, wl.tol, maxiter)
+            assert rc == gmg.OK, (name, sname, st)
+            h.omega = 1.0
+            ref = h.solve(so, wl.z, tol=wl.tol, maxiter=maxiter)
+            assert ref["status"] == 0
+            k, ko = st["iterations"], ref["iterations"]
+            assert abs(k - ko) <= 1, (name, sname, k, ko)
+            assert st["resid_final_rel"] <= wl.tol * (1.0 + 1e-6), (name, sname, st)
+            assert len(hist) == k + 1
+            # compare the iterate at EQUAL iteration count
+            if ko != k:
+                h.omega = 1.0
+                ref = h.solve(so, wl.z, tol=0.0, maxiter=k)
+            err = rel_l2_demeaned(p, ref["p"], act)
+            assert err <= TOL_P, (name, sname, err)
+            # residual histories agree to a few percent per entry (FP32 vs FP64)
+            m = min(k, ko)
+            ho = ref["history"][: m + 1]
+            hg = np.array(hist[: m + 1])
+            tol_h = 0.05 if sname != "pcg" else 0.5
+            assert np.all(np.abs(hg - ho) <= tol_h * ho + 1e-7), (name, sname, hg, ho)
+            # true residual of the returned p, recomputed by the oracle in FP64
+            r = oracle.residual(W.effective_L(wl.L, wl.bc), wl.bc, p, wl.z)
+            true_rel = oracle.norm2(r) / ref.get("r_ref", np.linalg.norm(np.where(act, wl.z, 0.0)))
+            assert true_rel <= wl.tol * 1.02, (name, sname, true_rel)
+    finally:
+        g.close()
+
+
+def test_adaptive_omega_sequence_matches_oracle():
+    """Reading O8 exercised on the case the oracle pin uses (tests/test_oracle_pins.py):
+    an under-smoothed V(1,0) jellyfish p=4 problem whose residual grows AND decays, so omega
+    takes both branches; the dyadic sequence must be IDENTICAL on GPU and oracle (P12)."""
+    wl = W.config3(4)
+    g = make_gpu(wl, nu_pre=1, nu_post=0)
+    h = make_oracle(wl, nu1=1, nu2=0)
+    try:
+        rc, p, st, hist = _solve_gpu(g, wl, gmg.GMG_RBGS, 0.0, 8)
+        ref = h.solve(oracle.GMG_RBGS, wl.z, tol=0.0, maxiter=8)
+        assert rc == gmg.NOT_CONVERGED and st["iterations"] == 8 == ref["iterations"]
+        om_g = g.omega_history()
+        assert list(om_g) == list(ref["omegas"])
+        assert list(om_g[:4]) == [1.0, 0.875, 0.90625, 0.78125]
+        assert st["omega_final"] == h.omega == 0.5
+        assert np.allclose(hist, ref["history"], rtol=2e-3)
+        act = W.active_mask(wl.L, wl.bc)
+        assert rel_l2_demeaned(p, ref["p"], act) <= TOL_P
+        # omega persists across solves on one context (time stepping) ...
+        rc, p, st, hist = _solve_gpu(g, wl, gmg.GMG_RBGS, 0.0, 1)
+        assert g.omega_history()[0] == 0.5
+        # ... and set_coeffs resets it
+        g.set_coeffs(dev(wl.L))
+        rc, p, st, hist = _solve_gpu(g, wl, gmg.GMG_RBGS, 0.0, 1)
+        assert g.omega_history()[0] == 1.0
+    finally:
+        g.close()
+
+
+def test_v11_cycle_parity():
+    wl = W.config3(5)
+    act = W.active_mask(wl.L, wl.bc)
+    g = make_gpu(wl, nu_pre=1, nu_post=1)
+    h = make_oracle(wl, nu1=1, nu2=1)
+    try:
+        rc, p, st, hist = _solve_gpu(g, wl, gmg.GMG_RBGS, wl.tol, 60)
+        ref = h.solve(oracle.GMG_RBGS, wl.z, tol=wl.tol, maxiter=60)
+        assert rc == gmg.OK and ref["status"] == 0
+        assert abs(st["iterations"] - ref["iterations"]) <= 1
+        if st["iterations"] != ref["iterations"]:
+            h.omega = 1.0
+            ref = h.solve(oracle.GMG_RBGS, wl.z, tol=0.0, maxiter=st["iterations"])
+        assert rel_l2_demeaned(p, ref["p"], act) <= TOL_P
+    finally:
+        g.close()
+
+
+def test_fixed_cycles_tol_zero_and_not_converged_code():
+    wl = W.config0()
+    g = make_gpu(wl)
+    h = make_oracle(wl)
+    try:
+        rc, p, st, hist = _solve_gpu(g, wl, gmg.GMG_RBGS, 0.0, 2)
+        assert rc == gmg.NOT_CONVERGED and st["iterations"] == 2 and len(hist) == 3
+        ref = h.solve(oracle.GMG_RBGS, wl.z, tol=0.0, maxiter=2)
+        act = np.ones(wl.z.shape, dtype=bool)
+        assert rel_l2_demeaned(p, ref["p"], act) <= TOL_P
+        assert np.allclose(hist, ref["history"], rtol=1e-3)
+        # maxiter = 0: nothing runs, p unchanged
+        rc, p, st, hist = _solve_gpu(g, wl, gmg.GMG_RBGS, 1e-4, 0)
+        assert rc == gmg.NOT_CONVERGED and st["iterations"] == 0 and np.all(p == 0)
+    finally:
+        g.close()
+
+
+def test_zero_rhs_and_converged_initial_guess():
+    wl = W.config0()
+    g = make_gpu(wl)
+    try:
+        wl0 = W.Workload("zero", wl.n, wl.bc, wl.L, np.zeros_like(wl.z))
+        p0 = np.random.default_rng(3).standard_normal(wl.z.shape).astype(np.float32)
+        for s in (gmg.GMG_RBGS, gmg.GMG_PCG, gmg.PCG):
+            rc, p, st, hist = _solve_gpu(g, wl0, s, 1e-4, 10, p0=p0)
+            assert rc == gmg.OK and st["iterations"] == 0
+            assert np.array_equal(p.astype(np.float32), p0)
+        # a converged initial guess: solve once, then call again with the result
+        rc, p, st, _ = _solve_gpu(g, wl, gmg.GMG_RBGS, 1e-4, 50)
+        k1 = st["iterations"]
+        rc, p2, st, _ = _solve_gpu(g, wl, gmg.GMG_RBGS, 1e-4, 50, p0=p)
+        assert rc == gmg.OK and st["iterations"] == 0 and k1 >= 1
+        assert np.array_equal(p2, p)
+    finally:
+        g.close()
+
+
+def test_nonzero_initial_guess_parity():
+    wl = W.config3(5)
+    act = W.active_mask(wl.L, wl.bc)
+    g = make_gpu(wl)
+    h = make_oracle(wl)
+    try:
+        p0 = (0.1 * np.random.default_rng(5).standard_normal(wl.z.shape)).astype(np.float32)
+        rc, p, st, hist = _solve_gpu(g, wl, gmg.GMG_RBGS, 1e-4, 50, p0=p0)
+        ref = h.solve(oracle.GMG_RBGS, wl.z, p0=p0, tol=0.0, maxiter=st["iterations"])
+        assert rc == gmg.OK
+        assert rel_l2_demeaned(p, ref["p"], act) <= TOL_P
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("n,bc", [((4, 4, 4), (0, 0, 0)), ((2, 2, 2), (1, 1, 1)),
+                                  ((5, 7, 3), (1, 1, 1)), ((6, 10, 4), (0, 0, 1)),
+                                  ((64, 4, 4), (1, 0, 0)), ((40, 24, 8), (0, 1, 0))])
+def test_degenerate_and_ragged_shapes(n, bc):
+    """Single-level grids (the tail kernel is the whole cycle), odd Neumann extents, strongly
+    anisotropic boxes, extents that are not multiples of the tile sizes."""
+    wl = random_workload(n, bc, seed=sum(n), zero_frac=0.0, blob=False)
+    act = W.active_mask(wl.L, wl.bc)
+    g = make_gpu(wl)
+    h = make_oracle(wl)
+    try:
+        rc, p, st, hist = _solve_gpu(g, wl, gmg.GMG_RBGS, 1e-4, 200)
+        ref = h.solve(oracle.GMG_RBGS, wl.z, tol=1e-4, maxiter=200)
+        assert rc == gmg.OK and ref["status"] == 0
+        assert abs(st["iterations"] - ref["iterations"]) <= 1
+        if st["iterations"] != ref["iterations"]:
+            h.omega = 1.0
+            ref = h.solve(oracle.GMG_RBGS, wl.z, tol=0.0, maxiter=st["iterations"])
+        assert rel_l2_demeaned(p, ref["p"], act) <= TOL_P
+    finally:
+        g.close()
+
+
+def test_runs_are_bit_reproducible_and_graph_equals_plain_launches():
+    wl = W.config3(5)
+    g = make_gpu(wl)
+    g2 = make_gpu(wl, use_graph=0)
+    try:
+        outs = []
+        for ctx in (g, g, g2):
+            ctx.set_omega(1.0)
+            for s in (gmg.GMG_RBGS, gmg.GMG_PCG, gmg.PCG):
+                rc, p, st, hist = _solve_gpu(ctx, wl, s, 1e-4, 1000)
+                outs.append((rc, st["iterations"], p.tobytes(), tuple(hist)))
+        assert outs[0:3] == outs[3:6]
+        assert outs[0:3] == outs[6:9]
+    finally:
+        g.close()
+        g2.close()
+
+
+def test_fast_path_equals_generic_path():
+    """The tiled/fused kernels use the same per-cell arithmetic as the generic ones."""
+    wl = W.by_name("c4_128")
+    act = W.active_mask(wl.L, wl.bc)
+    a = make_gpu(wl)
+    b = make_gpu(wl, fast_path=0)
+    try:
+        ra = _solve_gpu(a, wl, gmg.GMG_RBGS, 1e-4, 50)
+        rb = _solve_gpu(b, wl, gmg.GMG_RBGS, 1e-4, 50)
+        assert ra[2]["iterations"] == rb[2]["iterations"]
+        assert rel_l2_demeaned(ra[1], rb[1], act) <= 1e-5
+    finally:
+        a.close()
+        b.close()
+
+
+def test_error_paths():
+    wl = W.config0()
+    g = gmg.GMG(wl.n, wl.bc)
+    try:
+        p = torch.zeros(wl.z.shape, dtype=torch.float32, device="cuda")
+        with pytest.raises(gmg.GMGError) as e:
+            g.solve(p, dev(wl.z))
+        assert e.value.code == gmg.ESTATE                   # solve before set_coeffs
+        bad = wl.L.copy()
+        bad[1, 3, 4, 5] = -0.25
+        with pytest.raises(gmg.GMGError) as e:
+            g.set_coeffs(dev(bad))
+        assert e.value.code == gmg.EINVAL
+        bad[1, 3, 4, 5] = np.nan
+        with pytest.raises(gmg.GMGError) as e:
+            g.set_coeffs(dev(bad))
+        assert e.value.code == gmg.EINVAL
+        g.set_coeffs(dev(wl.L))
+        with pytest.raises(gmg.GMGError) as e:
+            g.solve(p, dev(wl.z), tol=-1.0)
+        assert e.value.code == gmg.EINVAL
+        assert g.solve(p, dev(wl.z)) == gmg.OK
+    finally:
+        g.close()
+    with pytest.raises(gmg.GMGError):
+        gmg.GMG((31, 32, 16), (0, 0, 0))                    # odd periodic extent (reading O3)
+
+
+def test_solve_host_matches_device_solve():
+    wl = W.config3(5)
+    g = make_gpu(wl)
+    try:
+        rc, p, st, hist = _solve_gpu(g, wl, gmg.GMG_RBGS, 1e-4, 50)
+        ph = torch.zeros(wl.z.shape, dtype=torch.float32).pin_memory()
+        zh = torch.from_numpy(wl.z).pin_memory()
+        g.set_omega(1.0)
+        rc2 = g.solve_host(ph, zh, tol=1e-4, maxiter=50)
+        assert rc2 == rc and g.stats()["iterations"] == st["iterations"]
+        assert np.array_equal(ph.numpy().astype(np.float64), p)
+    finally:
+        g.close()
