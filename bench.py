@@ -1,0 +1,322 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of the GMG pressure-Poisson solve on B200.
+
+A "step" is one pass of the whole hot path: one GMG-RBGS Poisson solve (V(2,2) cycles with the
+adaptive red-black Gauss-Seidel smoother on anisotropically coarsened levels, to relative
+residual 1e-4 from a zero initial guess) on one seeded synthetic workload.  Default workload:
+BASELINE.json configs[4], the 1024^3 periodic cube with 64 BDIM-ramped solid spheres -- the
+configuration the north_star's HBM-roofline target is stated on (the other configs fit in L2
+and are reported under "other_workloads").  Metric: ns per cell per Poisson solve (lower is
+better).  Multi-GPU: replicas only (the north_star excludes sharding): every rank solves its
+own copy, value = time / (N * cells).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c4_512|c1|...]
+    python bench.py --impl reference      # the FP64 CPU oracle on a bounded sample
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "poisson_solve_ns_per_cell_gmg_rbgs_tol1e-4"
+UNIT = "ns/cell"
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index = index
+        self.samples = []
+        self._stop = threading.Event()
+        self._t = None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True,
+                                     text=True, timeout=5).stdout.strip()
+                if out:
+                    self.samples.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            try:
+                sm.append(float(s[0]))
+                mx.append(float(s[1]))
+                for nm, v in zip(names, s[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_solve_time(wl, threads=None):
+    """One GMG-RBGS solve of workload wl with the FP64 oracle, as it stands; returns seconds,
+    iterations, threads used."""
+    import oracle
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    h = oracle.Hierarchy(wl.n, wl.bc, wl.L)
+    t0 = time.perf_counter()
+    out = h.solve(oracle.GMG_RBGS, wl.z, tol=wl.tol, maxiter=wl.maxiter)
+    dt = time.perf_counter() - t0
+    return dt, out["iterations"], cores, out["status"]
+
+
+def run_reference(args):
+    """--impl reference: the oracle (plain FP64 C, OpenMP over k) on the host cores, each step
+    one solve of a bounded sample of the workload (same generator, shrunk grid)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2607_07687_b200 import workloads as W
+    sample = args.reference_sample
+    wl = W.by_name(sample)
+    for _ in range(min(args.warmup, 1)):
+        oracle_solve_time(wl)
+    times, its = [], []
+    for _ in range(args.steps):
+        dt, it, cores, status = oracle_solve_time(wl)
+        times.append(dt)
+        its.append(it)
+    ms = 1e3 * sum(times) / len(times)
+    val = ms * 1e6 / wl.cells
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": ms,
+        "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": f"configs[4] recipe shrunk to {sample} ({wl.n[0]}x{wl.n[1]}x{wl.n[2]}), "
+                               "GMG-RBGS V(2,2) to tol 1e-4", "iterations": its[-1]},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"{sample}: one full solve per step"},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def time_kernel_loop(fn, reps, stream):
+    import torch
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    fn()
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(reps):
+        fn()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    from paper_2607_07687_b200 import gmg
+    from paper_2607_07687_b200 import workloads as W
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    device = torch.device(f"cuda:{local}")
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    t_gen = time.perf_counter()
+    wl = W.by_name(args.workload)
+    t_gen = time.perf_counter() - t_gen
+    N = wl.cells
+    g = gmg.GMG(wl.n, wl.bc, device=str(device))
+    L = torch.from_numpy(wl.L).to(device)
+    z = torch.from_numpy(wl.z).to(device)
+    p = torch.zeros_like(z)
+    g.set_coeffs(L)
+    stream = torch.cuda.current_stream(device)
+    tol, maxiter = wl.tol, wl.maxiter
+
+    # ---- device-resident timing: W warm-up + exactly K timed steps ---------------------------
+    for _ in range(args.warmup):
+        p.zero_()
+        g.set_omega(1.0)
+        g.solve(p, z, tol=tol, maxiter=maxiter, solver=gmg.GMG_RBGS)
+    launches = 0
+    iters = []
+    barrier()
+    sampler = ClockSampler(local)
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    with sampler:
+        e0.record(stream)
+        for _ in range(args.steps):
+            p.zero_()
+            g.set_omega(1.0)
+            rc = g.solve(p, z, tol=tol, maxiter=maxiter, solver=gmg.GMG_RBGS)
+            st = g.stats()
+            launches += st["kernel_launches"] + 1
+            iters.append(st["iterations"])
+        e1.record(stream)
+        barrier()
+    ms_total = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms_total], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    final = g.stats()
+    value = ms_step * 1e6 / (N * world)
+    ns_per_cell_vcycle = (final["gpu_ms"] * 1e6 / N) / max(final["iterations"], 1)
+
+    # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the region -----
+    zh = torch.from_numpy(wl.z).pin_memory()
+    ph = torch.zeros(wl.z.shape, dtype=torch.float32).pin_memory()
+    ph.zero_()
+    g.set_omega(1.0)
+    g.solve_host(ph, zh, tol=tol, maxiter=maxiter, solver=gmg.GMG_RBGS)
+    barrier()
+    t0 = time.perf_counter()
+    e2e_steps = max(1, min(args.steps, 3))
+    for _ in range(e2e_steps):
+        ph.zero_()
+        g.set_omega(1.0)
+        g.solve_host(ph, zh, tol=tol, maxiter=maxiter, solver=gmg.GMG_RBGS)
+    barrier()
+    e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_val = e2e_ms * 1e6 / (N * world)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel: the level-0 red+black sweep ------------------------
+    peak, peak_src = measured_peak()
+    b0 = z
+    q = torch.zeros_like(z)
+    reps = 4 if N > (1 << 28) else 20
+    t_pair = time_kernel_loop(lambda: g.op_smooth(0, q, b0, omega=1.0, nsweeps=2), reps, stream)
+    t_sweep = t_pair / 2.0
+    sweep_gbs = 24.0 * N / (t_sweep * 1e-3) / 1e9
+    t_rr = time_kernel_loop(lambda: g.op_residual_restrict(0, q, b0), reps, stream)
+    _, c0 = g.level_shape(0)
+    m = c0[0] * c0[1] * c0[2]
+    rr_gbs = (20.0 + 4.0 / m) * N / (t_rr * 1e-3) / 1e9
+    vc_bytes = (final["bytes_algorithmic"] - 36.0 * N) / max(final["iterations"], 1)
+    vc_ms = (final["gpu_ms"]) / max(final["iterations"], 1)
+    vcycle_gbs = vc_bytes / (vc_ms * 1e-3) / 1e9
+
+    # ---- cpu_baseline: the oracle, as it stands, on a bounded sample -------------------------
+    cpu = None
+    if not args.no_cpu_baseline:
+        swl = W.by_name(args.reference_sample)
+        dt, it, cores, status = oracle_solve_time(swl)
+        cpu = {"value": dt * 1e9 / swl.cells, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"{args.reference_sample} ({swl.n[0]}^3, same recipe as the workload): "
+                         f"one full solve, {it} V-cycles, {dt:.1f} s"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{wl.name} {wl.n[0]}x{wl.n[1]}x{wl.n[2]} bc={wl.bc} "
+                               "GMG-RBGS V(2,2) nu_coarse=32 tol=1e-4 zero initial guess",
+                   "cells": N, "levels": final["levels"], "iterations": iters[-1],
+                   "resid_final_rel": final["resid_final_rel"],
+                   "l2_policy": "inputs larger than L2" if 20 * N > 2 * 126e6 else
+                                "inputs fit in L2 (no flush; DRAM roofline not meaningful)",
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "input_generation_s": round(t_gen, 1)},
+        "ns_per_cell_per_vcycle": ns_per_cell_vcycle,
+        "vcycle": {"ms": vc_ms, "algorithmic_GBs": vcycle_gbs, "frac_of_peak": vcycle_gbs / peak,
+                   "bytes_per_fine_cell": vc_bytes / N},
+        "roofline": {"bound": "hbm", "kernel": "level-0 red+black Gauss-Seidel sweep",
+                     "achieved": sweep_gbs, "peak": peak, "unit": "GB/s", "frac": sweep_gbs / peak,
+                     "traffic": None, "peak_source": peak_src, "ms_per_launch": t_sweep,
+                     "algorithmic_bytes_per_cell": 24.0,
+                     "frac_of_nominal_8TBs": sweep_gbs / 8000.0},
+        "roofline_residual_restrict": {"achieved": rr_gbs, "peak": peak, "unit": "GB/s",
+                                       "frac": rr_gbs / peak, "ms_per_launch": t_rr,
+                                       "algorithmic_bytes_per_cell": 20.0 + 4.0 / m},
+        "cpu_baseline": cpu,
+        "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": 8 * N, "d2h_bytes_per_step": 4 * N},
+        "gpu_launches": int(launches),
+        "clocks": sampler.summary(),
+        "plan": g.describe_plan().strip().split("\n"),
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4")
+    ap.add_argument("--reference-sample", default="c4_256")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -21,6 +21,8 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
 bool resrestrict_supported(const LevelGeom& g);
 void residual_restrict(const LevelGeom& g, const float* L, const float* p, const float* b,
                        float* b_c, float* p_c, cudaStream_t s);
+void residual_norm2(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
+                    int slot, cudaStream_t s);
 int configure();
 }  // namespace gmgf
 
@@ -418,16 +420,23 @@ struct LoopCtl {
     int use_cond;
 };
 
+static void level0_residual_norm2(gmg_ctx* c, const float* p, const float* z, cudaStream_t s) {
+    if (c->prm.fast_path && gmgf::resrestrict_supported(c->g[0]))
+        gmgf::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, s);
+    else
+        gmgk::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, s);
+}
+
 // GMG-RBGS (readings O8, O9): pre = reference norm + initial residual norm + loop entry test.
 static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
     gmgk::active_norm2(c->g[0], c->lv[0].L, z, rbuf(c), RED_RREF, s);
-    gmgk::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, s);
+    level0_residual_norm2(c, p, z, s);
     gmgk::ctl_begin(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
     c->n_launch += 3;
 }
 static void rbgs_body(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
     enqueue_vcycle(c, p, z, &c->sc->omega_f, 0, s);
-    gmgk::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, s);
+    level0_residual_norm2(c, p, z, s);
     gmgk::ctl_rbgs_cycle_end(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
     c->n_launch += 2;
 }
@@ -462,7 +471,7 @@ static void pcg_body(gmg_ctx* c, float* p, int gmg_precond, LoopCtl lc, cudaStre
 }
 static void pcg_post(gmg_ctx* c, float* p, const float* z, cudaStream_t s) {
     // true residual at exit (the recursive one drove the test)
-    gmgk::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, s);
+    level0_residual_norm2(c, p, z, s);
     c->n_launch += 1;
 }
 

@@ -106,4 +106,35 @@ __device__ __forceinline__ double block_sum(double v) {
     return t;
 }
 
+// Finishes up to two sums: every block deposits its partial(s); the last block adds them in
+// index order and writes red[slot0] (and red[slot1]).
+__device__ __forceinline__ void finish_reduction(double v0, double v1, bool two, ReduceBuf rb,
+                                                 int slot0, int slot1) {
+    __shared__ bool is_last;
+    const double t0 = block_sum(v0);
+    const double t1 = two ? block_sum(v1) : 0.0;
+    if (threadIdx.x == 0) {
+        rb.partials[blockIdx.x] = t0;
+        if (two) rb.partials[GMG_REDUCE_MAX_BLOCKS + blockIdx.x] = t1;
+        __threadfence();
+        const unsigned int ticket = atomicAdd(rb.counter, 1u);
+        is_last = (ticket == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    double a0 = 0.0, a1 = 0.0;
+    for (unsigned int i = threadIdx.x; i < gridDim.x; i += blockDim.x) {
+        a0 += ((volatile double*)rb.partials)[i];
+        if (two) a1 += ((volatile double*)rb.partials)[GMG_REDUCE_MAX_BLOCKS + i];
+    }
+    const double s0 = block_sum(a0);
+    const double s1 = two ? block_sum(a1) : 0.0;
+    if (threadIdx.x == 0) {
+        rb.sc->red[slot0] = s0;
+        if (two) rb.sc->red[slot1] = s1;
+        *rb.counter = 0u;
+    }
+}
+
 }  // namespace gmgd

@@ -94,6 +94,17 @@ def test_two_and_three_sweeps(case):
             assert rel_linf(out, ref) <= 3 * TOL_OP, (l, cnt, rel_linf(out, ref))
 
 
+def test_fused_pair_black_first_underrelaxed(case):
+    """The symmetric V-cycle's post-smoothing order (black then red) through the fused kernel."""
+    wl, g, h = case
+    for l in range(min(h.nlev, 3)):
+        n, _ = h.shape(l)
+        p, b = _fields(n, 350 + l)
+        out = host(g.op_smooth(l, dev(p), dev(b), omega=0.8125, nsweeps=2, first_colour=1))
+        ref = h.level_sweeps(l, p, b, omega=0.8125, count=2, first_colour=1)
+        assert rel_linf(out, ref) <= 3 * TOL_OP, (l, rel_linf(out, ref))
+
+
 def test_restrict_and_fused_residual_restrict(case):
     wl, g, h = case
     for l in range(h.nlev - 1):
