@@ -46,6 +46,9 @@ __device__ __forceinline__ float4 ldg4(const float* p) {
 }
 __device__ __forceinline__ float4 lds4(const float* p) { return *reinterpret_cast<const float4*>(p); }
 __device__ __forceinline__ float4 zero4() { return make_float4(0.f, 0.f, 0.f, 0.f); }
+__device__ __forceinline__ void prefetch_l2(const void* p) {
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
 __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "memory"); }
 
 template <int TX_, int TY_>
@@ -76,6 +79,7 @@ struct SweepArgs {
     int first_colour;
     int zchunk;        // planes per CTA
     int tiles_x, tiles_y;
+    int pf;            // L2 prefetch distance in planes (0 = off)
 };
 
 // Coefficients of the four own cells in one plane: lower x faces (+ the face above the 4th
@@ -166,6 +170,12 @@ __global__ void __launch_bounds__(C::THREADS, MINB) k_rb_sweep(const SweepArgs a
             }
         }
     };
+    auto prefetch_plane = [&](int u) {   // L2 prefetch of a source plane a few steps ahead
+        const float* base = a.src + (size_t)wrap1(u, nz) * plane;
+#pragma unroll
+        for (int i = 0; i < C::APER; ++i)
+            if (a_goff[i] >= 0) prefetch_l2(base + a_goff[i]);
+    };
     auto slot_of = [&](int u) -> float* { return sm + ((u - (z0 - 2)) % C::NSLOT) * C::PLANE; };
     auto store_plane = [&](int u, const float4 (&v)[C::APER]) {
         float* s = slot_of(u);
@@ -209,6 +219,14 @@ __global__ void __launch_bounds__(C::THREADS, MINB) k_rb_sweep(const SweepArgs a
             s.b = ldg4(a.b + pz + o_row);
             if (last_lane) s.lxh = __ldg(Lx + pz + o_xh);
         };
+        auto prefetch_set = [&](int u) {  // L2 prefetch of a coefficient set a few steps ahead
+            const int gz = wrap1(u, nz), gzp = wrap1(u + 1, nz);
+            const size_t pz = (size_t)gz * plane, pzp = (size_t)gzp * plane;
+            prefetch_l2(Lx + pz + o_row);
+            prefetch_l2(Ly + pz + o_row);
+            prefetch_l2(Lz + pzp + o_row);
+            prefetch_l2(a.b + pz + o_row);
+        };
         auto finish = [&](int u, CSet& s) {  // first use of a set: neighbour face + wall faces
             const float t = __shfl_down_sync(0xffffffffu, s.lx.x, 1);
             if (!last_lane) s.lxh = t;
@@ -237,6 +255,8 @@ __global__ void __launch_bounds__(C::THREADS, MINB) k_rb_sweep(const SweepArgs a
             const bool do_a = (u + 2 <= z1 + 1);
             if (u + 1 <= z1) fetch(u + 1, Sn);
             if (do_a) load_plane(u + 2, va);
+            if (a.pf > 0 && u + 1 + a.pf <= z1) prefetch_set(u + 1 + a.pf);
+            if (a.pf > 0 && u + 2 + a.pf <= z1 + 1) prefetch_plane(u + 2 + a.pf);
             finish(u, Sc);
             {   // B(u): first colour on tile + ring 1, in place in shared memory
                 const float4 nw = phase(u, fc, Sc, Sp.lzh);
@@ -303,6 +323,7 @@ __global__ void __launch_bounds__(C::THREADS, MINB) k_rb_sweep(const SweepArgs a
             const bool do_a = (u + 2 <= z1 + 1);
             if (u + 1 <= z1) fetch_e(u + 1, En);
             if (do_a) load_plane(u + 2, va);
+            if (a.pf > 0 && u + 2 + a.pf <= z1 + 1) prefetch_plane(u + 2 + a.pf);
             if (e_act && ((xs + eyl + u) & 1) == fc) {
                 float* P = slot_of(u);
                 const float pc = P[e_off];
@@ -462,7 +483,7 @@ bool sweep_supported(const LevelGeom& g) {
            (long long)g.n[0] * g.n[1] < (1LL << 30);
 }
 
-template <class C>
+template <class C, int MB = kSweepMinBlocks>
 static void launch_sweep(SweepArgs& a, cudaStream_t s) {
     const LevelGeom& g = a.g;
     a.tiles_x = (g.n[0] + C::TX - 1) / C::TX;
@@ -474,9 +495,11 @@ static void launch_sweep(SweepArgs& a, cudaStream_t s) {
     while (zchunk > 16 && (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) < 148 * 4)
         zchunk = (zchunk + 1) / 2;
     a.zchunk = zchunk;
+    static const int pf_env = env_int("GMG_PF", 3);
+    a.pf = pf_env;
     const int nzc = (g.n[2] + zchunk - 1) / zchunk;
     const unsigned int grid = (unsigned int)(a.tiles_x * a.tiles_y * nzc);
-    k_rb_sweep<C, kSweepMinBlocks><<<grid, C::THREADS, C::SMEM, s>>>(a);
+    k_rb_sweep<C, MB><<<grid, C::THREADS, C::SMEM, s>>>(a);
 }
 
 void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
