@@ -29,27 +29,9 @@
 // kernels, so fast and generic paths agree bit for bit on every cell.
 #include <stdlib.h>
 
-#include "stencil.cuh"
+#include "fused_common.cuh"
 
 namespace gmgf {
-using namespace gmgd;
-
-__device__ __forceinline__ int wrapi(int v, int n) {
-    v %= n;
-    return v < 0 ? v + n : v;
-}
-// wrap for v in [-n, 2n)
-__device__ __forceinline__ int wrap1(int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); }
-
-__device__ __forceinline__ float4 ldg4(const float* p) {
-    return __ldg(reinterpret_cast<const float4*>(p));
-}
-__device__ __forceinline__ float4 lds4(const float* p) { return *reinterpret_cast<const float4*>(p); }
-__device__ __forceinline__ float4 zero4() { return make_float4(0.f, 0.f, 0.f, 0.f); }
-__device__ __forceinline__ void prefetch_l2(const void* p) {
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-}
-__device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "memory"); }
 
 template <int TX_, int TY_>
 struct SweepCfg {
@@ -81,34 +63,6 @@ struct SweepArgs {
     int tiles_x, tiles_y;
     int pf;            // L2 prefetch distance in planes (0 = off)
 };
-
-// Coefficients of the four own cells in one plane: lower x faces (+ the face above the 4th
-// cell), lower / upper y faces, UPPER z faces (the lower z faces are the previous plane's
-// upper ones), and the right-hand side.
-struct CSet {
-    float4 lx, ly, lyh, lzh, b;
-    float lxh;
-};
-
-// Updates cells S and S+2 of the own group (S = 0 or 1, compile time).
-template <int S>
-__device__ __forceinline__ float4 update_pair(float xm, float4 own, float xp, float4 ym, float4 yp,
-                                              float4 zm, float4 zp, const CSet& c, float4 lz,
-                                              float omega) {
-    float4 out = own;
-    if (S == 0) {
-        const float a1 = apply7(own.x, c.lx.x, c.lx.y, c.ly.x, c.lyh.x, lz.x, c.lzh.x, xm, own.y, ym.x, yp.x, zm.x, zp.x);
-        const float a2 = apply7(own.z, c.lx.z, c.lx.w, c.ly.z, c.lyh.z, lz.z, c.lzh.z, own.y, own.w, ym.z, yp.z, zm.z, zp.z);
-        out.x = relax(own.x, c.b.x, a1, diag6(c.lx.x, c.lx.y, c.ly.x, c.lyh.x, lz.x, c.lzh.x), omega);
-        out.z = relax(own.z, c.b.z, a2, diag6(c.lx.z, c.lx.w, c.ly.z, c.lyh.z, lz.z, c.lzh.z), omega);
-    } else {
-        const float a1 = apply7(own.y, c.lx.y, c.lx.z, c.ly.y, c.lyh.y, lz.y, c.lzh.y, own.x, own.z, ym.y, yp.y, zm.y, zp.y);
-        const float a2 = apply7(own.w, c.lx.w, c.lxh, c.ly.w, c.lyh.w, lz.w, c.lzh.w, own.z, xp, ym.w, yp.w, zm.w, zp.w);
-        out.y = relax(own.y, c.b.y, a1, diag6(c.lx.y, c.lx.z, c.ly.y, c.lyh.y, lz.y, c.lzh.y), omega);
-        out.w = relax(own.w, c.b.w, a2, diag6(c.lx.w, c.lxh, c.ly.w, c.lyh.w, lz.w, c.lzh.w), omega);
-    }
-    return out;
-}
 
 template <class C, int MINB>
 __global__ void __launch_bounds__(C::THREADS, MINB) k_rb_sweep(const SweepArgs a) {
@@ -478,7 +432,7 @@ static int env_int(const char* name, int dflt) {
     return v ? atoi(v) : dflt;
 }
 
-bool sweep_supported(const LevelGeom& g) {
+bool sweep_v2_supported(const LevelGeom& g) {
     return g.n[0] % 4 == 0 && g.n[0] >= 16 && g.n[1] >= 2 && g.n[2] >= 4 &&
            (long long)g.n[0] * g.n[1] < (1LL << 30);
 }
@@ -502,8 +456,8 @@ static void launch_sweep(SweepArgs& a, cudaStream_t s) {
     k_rb_sweep<C, MB><<<grid, C::THREADS, C::SMEM, s>>>(a);
 }
 
-void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
-              const float* omega, int first_colour, const float* e_c, cudaStream_t s) {
+void rb_sweep_v2(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
+                 const float* omega, int first_colour, const float* e_c, cudaStream_t s) {
     SweepArgs a;
     a.g = g; a.L = L; a.src = src; a.dst = dst; a.b = b; a.omega = omega; a.e_c = e_c;
     a.first_colour = first_colour;
@@ -549,7 +503,7 @@ void residual_norm2(const LevelGeom& g, const float* L, const float* p, const fl
     else launch_res<Res32, 1>(a, s);
 }
 
-int configure() {
+int configure_v2() {
     cudaError_t e = cudaFuncSetAttribute(k_rb_sweep<Sweep128, kSweepMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Sweep128::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep<Sweep64, kSweepMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Sweep64::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep<Sweep32, kSweepMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Sweep32::SMEM);

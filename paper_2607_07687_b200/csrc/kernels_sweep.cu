@@ -1,0 +1,552 @@
+// kernels_sweep.cu -- k_rb_sweep_bulk: the fused red+black Gauss-Seidel sweep of the big levels
+// (PAPER.md:43 S3.1; readings O3, O8; prolongation O6 fused on request), fed by the
+// Tensor Memory Accelerator (cp.async.bulk.tensor + mbarrier, SASS UTMALDG) instead of register
+// loads.
+//
+// Same schedule as k_rb_sweep (kernels_fused.cu): a CTA owns a 128 x TY tile and marches along
+// z; per step u:  wait for the data of step u;  B(u) first-colour update of plane u on tile +
+// ring 1, in place in shared memory;  barrier;  issue the copies of step u+PD;  C(u-1)
+// second-colour update of plane u-1, whole plane streamed to the destination array.
+//
+// What changed: EVERY input stream (source iterate p, right-hand side b, the three
+// face-coefficient arrays) arrives in shared memory as one TMA box per stream and plane
+// (128 x rows floats, 5.6-6.6 KB; plus two 4-float-wide halo boxes for p), issued PD steps
+// ahead of use: 7 TMA operations per step.  No registers are tied up by loads in flight, so the
+// DRAM latency is covered by shared-memory capacity (PD planes x 30 KB per SM) rather than by
+// occupancy.  Phase B reads its coefficient set from shared memory once and hands it to phase C
+// (one step later) in registers, so no coefficient is read twice.
+// Periodic wrap in x = the halo boxes are fetched at wrapped coordinates; in z = a wrapped plane
+// coordinate; tiles touching the y boundary (2 tile rows of ~114 at 1024^3) take a row-by-row
+// bulk-copy path (cp.async.bulk, UBLKCP) with wrapped row addresses.  Neumann walls = zeroed
+// coefficients.  Every shared-memory cell holds the periodic image of its cell, as in k_rb_sweep.
+#include <cuda.h>
+#include <stdlib.h>
+
+#include <map>
+#include <tuple>
+
+#include "fused_common.cuh"
+
+namespace gmgf {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) {
+    }
+}
+__device__ __forceinline__ void bulk_g2s(float* dst_smem, const float* src_gmem, uint32_t bytes,
+                                         uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+            smem_u32(dst_smem)),
+        "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void fence_async_smem() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+__device__ __forceinline__ void tma_load_3d(float* dst_smem, const CUtensorMap* tm, int c0, int c1, int c2,
+                                            uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(
+            smem_u32(dst_smem)),
+        "l"(reinterpret_cast<uint64_t>(tm)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+        : "memory");
+}
+
+template <int TY_, int PD_>
+struct BulkCfg {
+    static constexpr int TX = 128, TY = TY_, PD = PD_;
+    static constexpr int LPR = 32;
+    static constexpr int ROWS = TY + 2;          // rows running phase B (tile + ring 1)
+    static constexpr int MAIN = LPR * ROWS;
+    static constexpr int THREADS = MAIN + 32;    // + one edge warp
+    static constexpr int SH = TY + 4;            // rows of a p plane (halo 2)
+    static constexpr int NP = PD + 4;            // ring depths (slot-reuse argument: DESIGN.md S6)
+    static constexpr int NZ = PD + 1;
+    static constexpr int NC = PD;
+    static constexpr int NB = PD + 1;            // mbarriers of the step groups
+    static constexpr int HPAD = (SH * 4 + 31) / 32 * 32;  // one halo column group, padded to 128 B
+    static constexpr int P_HL = SH * TX;                   // p slot: main | left halo | right halo
+    static constexpr int P_HR = P_HL + HPAD;
+    static constexpr int P_PLANE = P_HR + HPAD;
+    static constexpr int C_PLANE = ROWS * TX;        // Lx, Lz, b
+    static constexpr int Y_PLANE = (ROWS + 1) * TX;  // Ly (needs the row above too)
+    static constexpr int OFF_P = 0;
+    static constexpr int OFF_LZ = OFF_P + NP * P_PLANE;
+    static constexpr int OFF_LX = OFF_LZ + NZ * C_PLANE;
+    static constexpr int OFF_LY = OFF_LX + NC * C_PLANE;
+    static constexpr int OFF_B = OFF_LY + NC * Y_PLANE;
+    static constexpr int FLOATS = OFF_B + NC * C_PLANE;
+    static constexpr size_t SMEM = (size_t)FLOATS * sizeof(float) + 16 * sizeof(uint64_t) + 128;
+    static constexpr uint32_t STEP_BYTES =
+        (uint32_t)(SH * TX + 2 * SH * 4 + 3 * ROWS * TX + (ROWS + 1) * TX) * 4u;
+    static constexpr uint32_t PRO_BYTES = (uint32_t)(2 * (SH * TX + 2 * SH * 4) + ROWS * TX) * 4u;
+    static constexpr int AGROUPS = (LPR + 2) * SH;      // float4 groups of a p plane (prolong fix-up)
+    static constexpr int APER = (AGROUPS + THREADS - 1) / THREADS;
+    static constexpr int NROWCOPY = SH + 4 * ROWS + 1;  // rows per step on the row-copy path
+    static_assert(2 * ROWS <= 32 && NB <= 8 && THREADS / 32 >= 7, "tile shape");
+};
+
+struct BulkArgs {
+    LevelGeom g;
+    const float* L;
+    const float* src;
+    float* dst;
+    const float* b;
+    const float* omega;
+    const float* e_c;
+    int first_colour;
+    int zchunk;
+    int tiles_x, tiles_y;
+};
+
+struct alignas(64) BulkMaps {
+    CUtensorMap p_main, p_halo, lz, lx, ly, b;
+};
+
+struct CFull {  // coefficient set of the four own cells in one plane, carried from B to C
+    float4 lx, ly, lyh, lz, lzh, b;
+    float lxh;
+};
+
+template <int S>
+__device__ __forceinline__ float4 update_pair_full(float xm, float4 own, float xp, float4 ym, float4 yp,
+                                                   float4 zm, float4 zp, const CFull& c, float omega) {
+    CSet s;
+    s.lx = c.lx; s.ly = c.ly; s.lyh = c.lyh; s.lzh = c.lzh; s.b = c.b; s.lxh = c.lxh;
+    return update_pair<S>(xm, own, xp, ym, yp, zm, zp, s, c.lz, omega);
+}
+
+template <class C, bool PROLONG>
+__global__ void __launch_bounds__(C::THREADS, 1)
+k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
+    extern __shared__ float sm_raw[];
+    float* const sm = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(sm_raw) + 127) & ~(uintptr_t)127);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..NB) step groups, [NB] prologue
+    const LevelGeom& g = a.g;
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const size_t N = (size_t)g.N;
+    const int plane = nx * ny;
+    const int tid = threadIdx.x;
+    const int warp_id = tid >> 5, lane_id = tid & 31;
+    constexpr int NWARP = C::THREADS / 32;
+    int bid = blockIdx.x;
+    const int tx = bid % a.tiles_x;
+    bid /= a.tiles_x;
+    const int ty = bid % a.tiles_y;
+    const int zc = bid / a.tiles_y;
+    const int x0 = tx * C::TX, y0 = ty * C::TY;
+    const int z0 = zc * a.zchunk;
+    const int z1 = min(nz, z0 + a.zchunk);
+    const float omega = *a.omega;
+    const int fc = a.first_colour;
+    const int xL = wrapi(x0 - 4, nx), xR = wrapi(x0 + C::TX, nx);  // halo column groups
+    const bool y_inside = (y0 >= 2) && (y0 + C::TY + 2 <= ny);     // TMA boxes stay in the domain
+    const float* Lx = a.L;
+    const float* Ly = a.L + N;
+    const float* Lz = a.L + 2 * N;
+
+    // ring slots: plane v of each stream
+    auto slotP = [&](int v) -> float* { return sm + C::OFF_P + ((v - (z0 - 2)) % C::NP) * C::P_PLANE; };
+    auto slotLz = [&](int v) -> float* { return sm + C::OFF_LZ + ((v - (z0 - 1)) % C::NZ) * C::C_PLANE; };
+    auto slotLx = [&](int v) -> float* { return sm + C::OFF_LX + ((v - (z0 - 1)) % C::NC) * C::C_PLANE; };
+    auto slotLy = [&](int v) -> float* { return sm + C::OFF_LY + ((v - (z0 - 1)) % C::NC) * C::Y_PLANE; };
+    auto slotB = [&](int v) -> float* { return sm + C::OFF_B + ((v - (z0 - 1)) % C::NC) * C::C_PLANE; };
+
+    // ---- copy issue ------------------------------------------------------------------------------
+    // Interior tiles: 7 TMA boxes per step, one per warp 0..6 (lane 0).  Tiles touching the y
+    // boundary: row-by-row bulk copies with wrapped row addresses, dealt round-robin to the warps.
+    // kind 0: p(v+1) rows y0-2..   1: Lz(v+1)   2: Lx(v)   3: Ly(v) (one more row)   4: b(v)
+    __shared__ const float* row_base[C::NROWCOPY];
+    __shared__ int row_kind[C::NROWCOPY], row_idx[C::NROWCOPY];
+    if (!y_inside && tid < C::NROWCOPY) {
+        int t = tid, ck, crow;
+        if (t < C::SH) { ck = 0; crow = t; }
+        else if ((t -= C::SH) < C::ROWS) { ck = 1; crow = t; }
+        else if ((t -= C::ROWS) < C::ROWS) { ck = 2; crow = t; }
+        else if ((t -= C::ROWS) < C::ROWS + 1) { ck = 3; crow = t; }
+        else { t -= C::ROWS + 1; ck = 4; crow = t; }
+        const int y = wrapi(ck == 0 ? y0 - 2 + crow : y0 - 1 + crow, ny);
+        const float* arr = ck == 0 ? a.src : ck == 1 ? Lz : ck == 2 ? Lx : ck == 3 ? Ly : a.b;
+        row_base[tid] = arr + (size_t)y * nx;
+        row_kind[tid] = ck;
+        row_idx[tid] = crow;
+    }
+    auto copy_p_rows = [&](int v, uint64_t* bar) {  // row path: the SH rows of p plane v
+        float* d = slotP(v);
+        const size_t pz = (size_t)wrap1(v, nz) * plane;
+        for (int j = warp_id; j < C::SH; j += NWARP) {
+            const float* rb = row_base[j] + pz;
+            bulk_g2s(d + j * C::TX, rb + x0, C::TX * 4u, bar);
+            bulk_g2s(d + C::P_HL + j * 4, rb + xL, 16u, bar);
+            bulk_g2s(d + C::P_HR + j * 4, rb + xR, 16u, bar);
+        }
+    };
+    auto copy_c_rows = [&](int kind, float* d, size_t pz, uint64_t* bar) {  // row path: one coefficient plane
+        const int first = kind == 1 ? C::SH : kind == 2 ? C::SH + C::ROWS : kind == 3 ? C::SH + 2 * C::ROWS
+                                                                          : C::SH + 3 * C::ROWS + 1;
+        const int cnt = kind == 3 ? C::ROWS + 1 : C::ROWS;
+        for (int j = warp_id; j < cnt; j += NWARP)
+            bulk_g2s(d + j * C::TX, row_base[first + j] + pz + x0, C::TX * 4u, bar);
+    };
+    auto issue_step = [&](int v) {  // the data B(v) newly needs: p(v+1), Lz(v+1), Lx(v), Ly(v), b(v)
+        if (lane_id != 0) return;
+        uint64_t* bar = bars + ((v - (z0 - 1)) % C::NB);
+        if (tid == 0) mbar_expect_tx(bar, C::STEP_BYTES);
+        const int gz0 = wrap1(v, nz), gz1 = wrap1(v + 1, nz);
+        if (y_inside) {
+            switch (warp_id) {
+                case 0: tma_load_3d(slotP(v + 1), &maps.p_main, x0, y0 - 2, gz1, bar); break;
+                case 1: tma_load_3d(slotP(v + 1) + C::P_HL, &maps.p_halo, xL, y0 - 2, gz1, bar); break;
+                case 2: tma_load_3d(slotP(v + 1) + C::P_HR, &maps.p_halo, xR, y0 - 2, gz1, bar); break;
+                case 3: tma_load_3d(slotLz(v + 1), &maps.lz, x0, y0 - 1, gz1, bar); break;
+                case 4: tma_load_3d(slotLx(v), &maps.lx, x0, y0 - 1, gz0, bar); break;
+                case 5: tma_load_3d(slotLy(v), &maps.ly, x0, y0 - 1, gz0, bar); break;
+                case 6: tma_load_3d(slotB(v), &maps.b, x0, y0 - 1, gz0, bar); break;
+                default: break;
+            }
+        } else {
+            copy_p_rows(v + 1, bar);
+            copy_c_rows(1, slotLz(v + 1), (size_t)gz1 * plane, bar);
+            copy_c_rows(2, slotLx(v), (size_t)gz0 * plane, bar);
+            copy_c_rows(3, slotLy(v), (size_t)gz0 * plane, bar);
+            copy_c_rows(4, slotB(v), (size_t)gz0 * plane, bar);
+        }
+    };
+
+    // ---- prolongation fix-up (PROLONG): p += P e_c on a freshly landed plane --------------------
+    int f_soff[C::APER], f_coff[C::APER];
+    const int ncx = nx / g.c[0], ncy = ny / g.c[1];
+    if (PROLONG) {
+#pragma unroll
+        for (int i = 0; i < C::APER; ++i) {
+            const int e = tid + i * C::THREADS;
+            if (e < C::AGROUPS) {
+                const int r = e / (C::LPR + 2), gc = e % (C::LPR + 2);
+                const int x = wrapi(x0 - 4 + 4 * gc, nx), y = wrapi(y0 + r - 2, ny);
+                f_soff[i] = gc == 0 ? C::P_HL + r * 4 : gc == C::LPR + 1 ? C::P_HR + r * 4 : r * C::TX + 4 * (gc - 1);
+                f_coff[i] = (y / g.c[1]) * ncx + x / g.c[0];
+            } else {
+                f_soff[i] = -1;
+                f_coff[i] = 0;
+            }
+        }
+    }
+    auto fix_plane = [&](int v) {
+        float* P = slotP(v);
+        const float* eb = a.e_c + (size_t)(wrap1(v, nz) / g.c[2]) * (ncx * ncy);
+#pragma unroll
+        for (int i = 0; i < C::APER; ++i) {
+            if (f_soff[i] >= 0) {
+                float4 val = lds4(P + f_soff[i]);
+                if (g.c[0] == 2) {
+                    const float2 e2 = __ldg(reinterpret_cast<const float2*>(eb + f_coff[i]));
+                    val.x += e2.x; val.y += e2.x; val.z += e2.y; val.w += e2.y;
+                } else {
+                    const float4 e4 = ldg4(eb + f_coff[i]);
+                    val.x += e4.x; val.y += e4.y; val.z += e4.z; val.w += e4.w;
+                }
+                *reinterpret_cast<float4*>(P + f_soff[i]) = val;
+            }
+        }
+    };
+
+    // ---- prologue: barriers; p(z0-2), p(z0-1), Lz(z0-1); the first PD step groups --------------
+    if (tid == 0) {
+        for (int i = 0; i <= C::NB; ++i) mbar_init(bars + i, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    fence_async_smem();
+    __syncthreads();
+    {
+        uint64_t* bar = bars + C::NB;
+        if (lane_id == 0) {
+            if (tid == 0) mbar_expect_tx(bar, C::PRO_BYTES);
+            const int ga = wrap1(z0 - 2, nz), gb = wrap1(z0 - 1, nz);
+            if (y_inside) {
+                switch (warp_id) {
+                    case 0: tma_load_3d(slotP(z0 - 2), &maps.p_main, x0, y0 - 2, ga, bar); break;
+                    case 1: tma_load_3d(slotP(z0 - 2) + C::P_HL, &maps.p_halo, xL, y0 - 2, ga, bar); break;
+                    case 2: tma_load_3d(slotP(z0 - 2) + C::P_HR, &maps.p_halo, xR, y0 - 2, ga, bar); break;
+                    case 3: tma_load_3d(slotP(z0 - 1), &maps.p_main, x0, y0 - 2, gb, bar); break;
+                    case 4: tma_load_3d(slotP(z0 - 1) + C::P_HL, &maps.p_halo, xL, y0 - 2, gb, bar); break;
+                    case 5: tma_load_3d(slotP(z0 - 1) + C::P_HR, &maps.p_halo, xR, y0 - 2, gb, bar); break;
+                    case 6: tma_load_3d(slotLz(z0 - 1), &maps.lz, x0, y0 - 1, gb, bar); break;
+                    default: break;
+                }
+            } else {
+                copy_p_rows(z0 - 2, bar);
+                copy_p_rows(z0 - 1, bar);
+                copy_c_rows(1, slotLz(z0 - 1), (size_t)gb * plane, bar);
+            }
+        }
+        for (int v = z0 - 1; v < z0 - 1 + C::PD && v <= z1; ++v) issue_step(v);
+        mbar_wait(bar, 0);
+        if (PROLONG) {
+            fix_plane(z0 - 2);
+            fix_plane(z0 - 1);
+        }
+    }
+
+    if (tid < C::MAIN) {
+        // ---- main threads: one float4 group of one row ---------------------------------------
+        const int lx = lane_id, ry = warp_id;
+        const int xl = x0 + 4 * lx;
+        const int yl = y0 + ry - 1;
+        const int gx = xl, gy = wrapi(yl, ny), gyp = wrapi(yl + 1, ny);
+        const int gxh = wrapi(xl + 4, nx);
+        const bool row_c = (ry >= 1) && (ry <= C::TY) && (yl < ny);
+        const bool zx_lo = g.bc[0] && gx == 0, zx_hi = g.bc[0] && gxh == 0;
+        const bool zy_lo = g.bc[1] && gy == 0, zy_hi = g.bc[1] && gyp == 0;
+        const bool last_lane = (lx == C::LPR - 1);
+        const int p_off = (ry + 1) * C::TX + 4 * lx;        // own float4 in a p plane
+        const int h_off = (lx == 0 ? C::P_HL + 3 : C::P_HR) + (ry + 1) * 4;  // x-halo cell of the edge lanes
+        const int c_off = ry * C::TX + 4 * lx;              // own float4 in a coefficient plane
+        float* const dst_row = a.dst + (size_t)gy * nx + gx;
+        const float* const lxh_row = Lx + (size_t)gy * nx + gxh;  // face above the tile's last cell
+
+        auto phase = [&](int u, int colour, const CFull& s) -> float4 {
+            const float* P = slotP(u);
+            const float4 own = lds4(P + p_off);
+            const float4 ym = lds4(P + p_off - C::TX);
+            const float4 yp = lds4(P + p_off + C::TX);
+            const float4 zm = lds4(slotP(u - 1) + p_off);
+            const float4 zp = lds4(slotP(u + 1) + p_off);
+            float xm = __shfl_up_sync(0xffffffffu, own.w, 1);
+            float xp = __shfl_down_sync(0xffffffffu, own.x, 1);
+            if (lx == 0) xm = P[h_off];
+            if (last_lane) xp = P[h_off];
+            return ((yl + u + colour) & 1) ? update_pair_full<1>(xm, own, xp, ym, yp, zm, zp, s, omega)
+                                           : update_pair_full<0>(xm, own, xp, ym, yp, zm, zp, s, omega);
+        };
+        CFull Sp;  // set of plane u-1, handed from B(u-1) to C(u-1)
+        Sp.lx = Sp.ly = Sp.lyh = Sp.lz = Sp.lzh = Sp.b = zero4();
+        Sp.lxh = 0.0f;
+        float lxh_pf = last_lane ? __ldg(lxh_row + (size_t)wrap1(z0 - 1, nz) * plane) : 0.0f;
+        for (int u = z0 - 1; u <= z1; ++u) {
+            const int k = u - (z0 - 1);
+            mbar_wait(bars + (k % C::NB), (uint32_t)(k / C::NB) & 1u);
+            if (PROLONG) {
+                fix_plane(u + 1);
+                cta_sync();
+            }
+            CFull Sc;
+            {   // coefficient set of plane u: shared memory -> registers, wall faces zeroed
+                Sc.lx = lds4(slotLx(u) + c_off);
+                const float* Y = slotLy(u) + c_off;
+                Sc.ly = lds4(Y);
+                Sc.lyh = lds4(Y + C::TX);
+                Sc.lz = lds4(slotLz(u) + c_off);
+                Sc.lzh = lds4(slotLz(u + 1) + c_off);
+                Sc.b = lds4(slotB(u) + c_off);
+                const float t = __shfl_down_sync(0xffffffffu, Sc.lx.x, 1);
+                Sc.lxh = last_lane ? lxh_pf : t;
+                if (last_lane && u + 1 <= z1) lxh_pf = __ldg(lxh_row + (size_t)wrap1(u + 1, nz) * plane);
+                if (zx_lo) Sc.lx.x = 0.0f;
+                if (zx_hi) Sc.lxh = 0.0f;
+                if (zy_lo) Sc.ly = zero4();
+                if (zy_hi) Sc.lyh = zero4();
+                if (g.bc[2]) {
+                    if (wrap1(u, nz) == 0) Sc.lz = zero4();
+                    if (wrap1(u + 1, nz) == 0) Sc.lzh = zero4();
+                }
+            }
+            {   // B(u): first colour on tile + ring 1, in place in shared memory
+                const float4 nw = phase(u, fc, Sc);
+                *reinterpret_cast<float4*>(slotP(u) + p_off) = nw;
+            }
+            cta_sync();
+            if (u + C::PD <= z1) {
+                fence_async_smem();
+                issue_step(u + C::PD);
+            }
+            if (u - 1 >= z0 && row_c) {  // C(u-1): second colour, tile rows only (warp-uniform)
+                const float4 nw = phase(u - 1, fc ^ 1, Sp);
+                *reinterpret_cast<float4*>(dst_row + (size_t)(u - 1) * plane) = nw;
+            }
+            Sp = Sc;
+        }
+    } else {
+        // ---- edge warp: ring-1 cells x0-1 and x0+TX of every row, phase B only ----------------
+        const int el = lane_id;
+        const bool e_act = el < 2 * C::ROWS;
+        const int side = el & 1, ery = e_act ? (el >> 1) : 0;
+        const int xs = side ? x0 + C::TX : x0 - 1;
+        const int eyl = y0 + ery - 1;
+        const int gxs = wrapi(xs, nx), gxs1 = wrapi(xs + 1, nx);
+        const int egy = wrapi(eyl, ny), egyp = wrapi(eyl + 1, ny);
+        const int r = ery + 1;
+        const int pc_off = side ? C::P_HR + r * 4 : C::P_HL + r * 4 + 3;   // the edge cell
+        const int xm_off = side ? r * C::TX + C::TX - 1 : pc_off - 1;      // its x neighbours
+        const int xp_off = side ? pc_off + 1 : r * C::TX;
+        const int o_c = egy * nx + gxs, o_x1 = egy * nx + gxs1, o_yp = egyp * nx + gxs;
+        const bool ex_lo = g.bc[0] && gxs == 0, ex_hi = g.bc[0] && gxs1 == 0;
+        const bool ey_lo = g.bc[1] && egy == 0, ey_hi = g.bc[1] && egyp == 0;
+        struct ESet { float wxl, wxh, wyl, wyh, wzl, wzh, b; };
+        auto fetch_e = [&](int u, ESet& s) {  // global loads, issued one step ahead
+            const int gz = wrap1(u, nz), gzp = wrap1(u + 1, nz);
+            const size_t pz = (size_t)gz * plane, pzp = (size_t)gzp * plane;
+            s.wxl = ex_lo ? 0.0f : __ldg(Lx + pz + o_c);
+            s.wxh = ex_hi ? 0.0f : __ldg(Lx + pz + o_x1);
+            s.wyl = ey_lo ? 0.0f : __ldg(Ly + pz + o_c);
+            s.wyh = ey_hi ? 0.0f : __ldg(Ly + pz + o_yp);
+            s.wzl = (g.bc[2] && gz == 0) ? 0.0f : __ldg(Lz + pz + o_c);
+            s.wzh = (g.bc[2] && gzp == 0) ? 0.0f : __ldg(Lz + pzp + o_c);
+            s.b = __ldg(a.b + pz + o_c);
+        };
+        ESet Ec, En;
+        fetch_e(z0 - 1, Ec);
+        En = Ec;
+        for (int u = z0 - 1; u <= z1; ++u) {
+            const int k = u - (z0 - 1);
+            if (u + 1 <= z1) fetch_e(u + 1, En);
+            mbar_wait(bars + (k % C::NB), (uint32_t)(k / C::NB) & 1u);
+            if (PROLONG) {
+                fix_plane(u + 1);
+                cta_sync();
+            }
+            if (e_act && ((xs + eyl + u) & 1) == fc) {
+                float* P = slotP(u);
+                const float pc = P[pc_off];
+                const float Ap = apply7(pc, Ec.wxl, Ec.wxh, Ec.wyl, Ec.wyh, Ec.wzl, Ec.wzh, P[xm_off],
+                                        P[xp_off], P[pc_off - 4], P[pc_off + 4], slotP(u - 1)[pc_off],
+                                        slotP(u + 1)[pc_off]);
+                P[pc_off] = relax(pc, Ec.b, Ap,
+                                  diag6(Ec.wxl, Ec.wxh, Ec.wyl, Ec.wyh, Ec.wzl, Ec.wzh), omega);
+            }
+            cta_sync();
+            if (u + C::PD <= z1) {
+                fence_async_smem();
+                issue_step(u + C::PD);
+            }
+            Ec = En;
+        }
+    }
+}
+
+// ---- launchers ------------------------------------------------------------------------------
+bool sweep_v2_supported(const LevelGeom& g);
+void rb_sweep_v2(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
+                 const float* omega, int first_colour, const float* e_c, cudaStream_t s);
+int configure_v2();
+
+using Bulk = BulkCfg<9, 3>;
+
+static int env_int2(const char* name, int dflt) {
+    const char* v = getenv(name);
+    return v ? atoi(v) : dflt;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+static EncodeTiledFn g_encode = nullptr;
+
+// 3-D tiled tensor map over an [nz][ny][nx] FP32 array with a bw x bh x 1 box.  Cached per
+// (pointer, extents, box): encoding costs a few microseconds on the host.
+static bool tensor_map(const float* ptr, const LevelGeom& g, int bw, int bh, CUtensorMap* out) {
+    typedef std::tuple<const float*, int, int, int, int, int> Key;
+    static std::map<Key, CUtensorMap> cache;
+    const Key key(ptr, g.n[0], g.n[1], g.n[2], bw, bh);
+    auto it = cache.find(key);
+    if (it != cache.end()) {
+        *out = it->second;
+        return true;
+    }
+    if (!g_encode) return false;
+    const cuuint64_t dims[3] = {(cuuint64_t)g.n[0], (cuuint64_t)g.n[1], (cuuint64_t)g.n[2]};
+    const cuuint64_t strides[2] = {(cuuint64_t)g.n[0] * 4, (cuuint64_t)g.n[0] * g.n[1] * 4};
+    const cuuint32_t box[3] = {(cuuint32_t)bw, (cuuint32_t)bh, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    alignas(64) CUtensorMap tm;
+    const CUresult r = g_encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(ptr), dims, strides,
+                                box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return false;
+    if (cache.size() > 4096) cache.clear();
+    cache[key] = tm;
+    *out = tm;
+    return true;
+}
+
+bool sweep_supported(const LevelGeom& g) { return sweep_v2_supported(g); }
+
+static bool bulk_supported(const LevelGeom& g) {
+    return g_encode && g.n[0] >= 128 && g.n[0] % 128 == 0 && g.n[1] >= 4 && g.n[2] >= 8;
+}
+
+void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
+              const float* omega, int first_colour, const float* e_c, cudaStream_t s) {
+    static const int use_bulk = env_int2("GMG_BULK", 1);
+    BulkMaps maps;
+    const size_t N = (size_t)g.N;
+    bool ok = use_bulk && bulk_supported(g);
+    ok = ok && tensor_map(src, g, Bulk::TX, Bulk::SH, &maps.p_main);
+    ok = ok && tensor_map(src, g, 4, Bulk::SH, &maps.p_halo);
+    ok = ok && tensor_map(L + 2 * N, g, Bulk::TX, Bulk::ROWS, &maps.lz);
+    ok = ok && tensor_map(L, g, Bulk::TX, Bulk::ROWS, &maps.lx);
+    ok = ok && tensor_map(L + N, g, Bulk::TX, Bulk::ROWS + 1, &maps.ly);
+    ok = ok && tensor_map(b, g, Bulk::TX, Bulk::ROWS, &maps.b);
+    if (!ok) {
+        rb_sweep_v2(g, L, src, dst, b, omega, first_colour, e_c, s);
+        return;
+    }
+    BulkArgs a;
+    a.g = g; a.L = L; a.src = src; a.dst = dst; a.b = b; a.omega = omega; a.e_c = e_c;
+    a.first_colour = first_colour;
+    a.tiles_x = g.n[0] / Bulk::TX;
+    a.tiles_y = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
+    static const int zc_env = env_int2("GMG_ZCHUNK", 64);
+    int zchunk = zc_env;
+    if (g.n[2] < 2 * zchunk) zchunk = g.n[2];
+    while (zchunk > 16 && (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) < 148 * 2)
+        zchunk = (zchunk + 1) / 2;
+    a.zchunk = zchunk;
+    const int nzc = (g.n[2] + zchunk - 1) / zchunk;
+    const unsigned int grid = (unsigned int)(a.tiles_x * a.tiles_y * nzc);
+    if (e_c) k_rb_sweep_bulk<Bulk, true><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+    else k_rb_sweep_bulk<Bulk, false><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+}
+
+int configure() {
+    cudaError_t e = (cudaError_t)configure_v2();
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+    if (e == cudaSuccess && !g_encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            g_encode = (EncodeTiledFn)fn;
+        else
+            cudaGetLastError();  // the TMA path is simply not used
+    }
+    return (int)e;
+}
+
+}  // namespace gmgf

@@ -22,6 +22,10 @@ CASES = {
     "c3p5": lambda: W.config3(5),
     "c4_64": lambda: W.config4(n=64, nspheres=8, diameter=8),
     "sphere_D4": lambda: W.config2(D=4),
+    # wide enough (nx % 128 == 0) for the TMA-fed sweep: interior and boundary tiles, all BC mixes
+    "rand_128_NPP": lambda: random_workload((128, 20, 12), (1, 0, 0), 15),
+    "rand_256_PNN": lambda: random_workload((256, 12, 10), (0, 1, 1), 16),
+    "rand_128_PPP": lambda: random_workload((128, 40, 8), (0, 0, 0), 17),
 }
 
 
