@@ -101,13 +101,13 @@ struct BulkCfg {
     static constexpr int OFF_LY = OFF_LX + NC * C_PLANE;
     static constexpr int OFF_B = OFF_LY + NC * Y_PLANE;
     static constexpr int FLOATS = OFF_B + NC * C_PLANE;
-    static constexpr size_t SMEM = (size_t)FLOATS * sizeof(float) + 16 * sizeof(uint64_t) + 128;
+    static constexpr int NROWCOPY = SH + 4 * ROWS + 1;  // rows per step on the row-copy path
+    static constexpr size_t SMEM = (size_t)FLOATS * sizeof(float) + 16 * sizeof(uint64_t) + (size_t)NROWCOPY * 16;
     static constexpr uint32_t STEP_BYTES =
         (uint32_t)(SH * TX + 2 * SH * 4 + 3 * ROWS * TX + (ROWS + 1) * TX) * 4u;
     static constexpr uint32_t PRO_BYTES = (uint32_t)(2 * (SH * TX + 2 * SH * 4) + ROWS * TX) * 4u;
     static constexpr int AGROUPS = (LPR + 2) * SH;      // float4 groups of a p plane (prolong fix-up)
     static constexpr int APER = (AGROUPS + THREADS - 1) / THREADS;
-    static constexpr int NROWCOPY = SH + 4 * ROWS + 1;  // rows per step on the row-copy path
     static_assert(2 * ROWS <= 32 && NB <= 8 && THREADS / 32 >= 7, "tile shape");
 };
 
@@ -144,9 +144,11 @@ __device__ __forceinline__ float4 update_pair_full(float xm, float4 own, float x
 template <class C, bool PROLONG>
 __global__ void __launch_bounds__(C::THREADS, 1)
 k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
-    extern __shared__ float sm_raw[];
-    float* const sm = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(sm_raw) + 127) & ~(uintptr_t)127);
+    extern __shared__ __align__(1024) float sm[];  // no static shared memory: base is 1 KB aligned
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..NB) step groups, [NB] prologue
+    const float** row_base = reinterpret_cast<const float**>(bars + 16);  // row-copy path tables
+    int* row_kind = reinterpret_cast<int*>(row_base + C::NROWCOPY);
+    int* row_idx = row_kind + C::NROWCOPY;
     const LevelGeom& g = a.g;
     const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
     const size_t N = (size_t)g.N;
@@ -181,8 +183,6 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     // Interior tiles: 7 TMA boxes per step, one per warp 0..6 (lane 0).  Tiles touching the y
     // boundary: row-by-row bulk copies with wrapped row addresses, dealt round-robin to the warps.
     // kind 0: p(v+1) rows y0-2..   1: Lz(v+1)   2: Lx(v)   3: Ly(v) (one more row)   4: b(v)
-    __shared__ const float* row_base[C::NROWCOPY];
-    __shared__ int row_kind[C::NROWCOPY], row_idx[C::NROWCOPY];
     if (!y_inside && tid < C::NROWCOPY) {
         int t = tid, ck, crow;
         if (t < C::SH) { ck = 0; crow = t; }
@@ -312,6 +312,31 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         }
     }
 
+    // ring cursors of step u (advanced once per step; no modulo in the loop)
+    float* const P_beg = sm + C::OFF_P;
+    float* const Z_beg = sm + C::OFF_LZ;
+    float* Pm2 = P_beg + (C::NP - 1) * C::P_PLANE;  // plane u-2 (u = z0-1: not loaded, not read)
+    float* Pm1 = P_beg;                             // plane u-1
+    float* P0 = P_beg + C::P_PLANE;                 // plane u
+    float* Pp1 = P_beg + 2 * C::P_PLANE;            // plane u+1
+    const float* Z0 = Z_beg;                        // Lz plane u
+    const float* Z1 = Z_beg + C::C_PLANE;           // Lz plane u+1
+    int ic = 0;                                     // slot of Lx / Ly / b plane u
+    int kb = 0;                                     // mbarrier of step u and its phase parity
+    uint32_t kpar = 0;
+    int gz = wrap1(z0 - 1, nz);                     // wrapped plane index of u
+    auto advance = [&]() {
+        Pm2 = Pm1; Pm1 = P0; P0 = Pp1;
+        Pp1 += C::P_PLANE;
+        if (Pp1 == P_beg + C::NP * C::P_PLANE) Pp1 = P_beg;
+        Z0 = Z1;
+        Z1 += C::C_PLANE;
+        if (Z1 == Z_beg + C::NZ * C::C_PLANE) Z1 = Z_beg;
+        if (++ic == C::NC) ic = 0;
+        if (++kb == C::NB) { kb = 0; kpar ^= 1u; }
+        if (++gz == nz) gz = 0;
+    };
+
     if (tid < C::MAIN) {
         // ---- main threads: one float4 group of one row ---------------------------------------
         const int lx = lane_id, ry = warp_id;
@@ -326,58 +351,59 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         const int p_off = (ry + 1) * C::TX + 4 * lx;        // own float4 in a p plane
         const int h_off = (lx == 0 ? C::P_HL + 3 : C::P_HR) + (ry + 1) * 4;  // x-halo cell of the edge lanes
         const int c_off = ry * C::TX + 4 * lx;              // own float4 in a coefficient plane
-        float* const dst_row = a.dst + (size_t)gy * nx + gx;
+        float* dst_ptr = a.dst + ((long long)gy * nx + gx + (long long)(z0 - 2) * plane);  // plane u-1
         const float* const lxh_row = Lx + (size_t)gy * nx + gxh;  // face above the tile's last cell
 
-        auto phase = [&](int u, int colour, const CFull& s) -> float4 {
-            const float* P = slotP(u);
+        auto phase = [&](const float* Pm, const float* P, const float* Pp, int sel, const CFull& s) -> float4 {
             const float4 own = lds4(P + p_off);
             const float4 ym = lds4(P + p_off - C::TX);
             const float4 yp = lds4(P + p_off + C::TX);
-            const float4 zm = lds4(slotP(u - 1) + p_off);
-            const float4 zp = lds4(slotP(u + 1) + p_off);
+            const float4 zm = lds4(Pm + p_off);
+            const float4 zp = lds4(Pp + p_off);
             float xm = __shfl_up_sync(0xffffffffu, own.w, 1);
             float xp = __shfl_down_sync(0xffffffffu, own.x, 1);
             if (lx == 0) xm = P[h_off];
             if (last_lane) xp = P[h_off];
-            return ((yl + u + colour) & 1) ? update_pair_full<1>(xm, own, xp, ym, yp, zm, zp, s, omega)
-                                           : update_pair_full<0>(xm, own, xp, ym, yp, zm, zp, s, omega);
+            return sel ? update_pair_full<1>(xm, own, xp, ym, yp, zm, zp, s, omega)
+                       : update_pair_full<0>(xm, own, xp, ym, yp, zm, zp, s, omega);
         };
         CFull Sp;  // set of plane u-1, handed from B(u-1) to C(u-1)
         Sp.lx = Sp.ly = Sp.lyh = Sp.lz = Sp.lzh = Sp.b = zero4();
         Sp.lxh = 0.0f;
-        float lxh_pf = last_lane ? __ldg(lxh_row + (size_t)wrap1(z0 - 1, nz) * plane) : 0.0f;
+        float lxh_pf = last_lane ? __ldg(lxh_row + (size_t)gz * plane) : 0.0f;
+        // cells (sel, sel+2) of the group are updated: same parity for B(u) and C(u-1)
+        int sel = (yl + (z0 - 1) + fc) & 1;
         for (int u = z0 - 1; u <= z1; ++u) {
-            const int k = u - (z0 - 1);
-            mbar_wait(bars + (k % C::NB), (uint32_t)(k / C::NB) & 1u);
+            mbar_wait(bars + kb, kpar);
             if (PROLONG) {
                 fix_plane(u + 1);
                 cta_sync();
             }
+            const int gzp = (gz + 1 == nz) ? 0 : gz + 1;
             CFull Sc;
             {   // coefficient set of plane u: shared memory -> registers, wall faces zeroed
-                Sc.lx = lds4(slotLx(u) + c_off);
-                const float* Y = slotLy(u) + c_off;
+                Sc.lx = lds4(sm + C::OFF_LX + ic * C::C_PLANE + c_off);
+                const float* Y = sm + C::OFF_LY + ic * C::Y_PLANE + c_off;
                 Sc.ly = lds4(Y);
                 Sc.lyh = lds4(Y + C::TX);
-                Sc.lz = lds4(slotLz(u) + c_off);
-                Sc.lzh = lds4(slotLz(u + 1) + c_off);
-                Sc.b = lds4(slotB(u) + c_off);
+                Sc.lz = lds4(Z0 + c_off);
+                Sc.lzh = lds4(Z1 + c_off);
+                Sc.b = lds4(sm + C::OFF_B + ic * C::C_PLANE + c_off);
                 const float t = __shfl_down_sync(0xffffffffu, Sc.lx.x, 1);
                 Sc.lxh = last_lane ? lxh_pf : t;
-                if (last_lane && u + 1 <= z1) lxh_pf = __ldg(lxh_row + (size_t)wrap1(u + 1, nz) * plane);
+                if (last_lane && u + 1 <= z1) lxh_pf = __ldg(lxh_row + (size_t)gzp * plane);
                 if (zx_lo) Sc.lx.x = 0.0f;
                 if (zx_hi) Sc.lxh = 0.0f;
                 if (zy_lo) Sc.ly = zero4();
                 if (zy_hi) Sc.lyh = zero4();
                 if (g.bc[2]) {
-                    if (wrap1(u, nz) == 0) Sc.lz = zero4();
-                    if (wrap1(u + 1, nz) == 0) Sc.lzh = zero4();
+                    if (gz == 0) Sc.lz = zero4();
+                    if (gzp == 0) Sc.lzh = zero4();
                 }
             }
             {   // B(u): first colour on tile + ring 1, in place in shared memory
-                const float4 nw = phase(u, fc, Sc);
-                *reinterpret_cast<float4*>(slotP(u) + p_off) = nw;
+                const float4 nw = phase(Pm1, P0, Pp1, sel, Sc);
+                *reinterpret_cast<float4*>(P0 + p_off) = nw;
             }
             cta_sync();
             if (u + C::PD <= z1) {
@@ -385,10 +411,13 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
                 issue_step(u + C::PD);
             }
             if (u - 1 >= z0 && row_c) {  // C(u-1): second colour, tile rows only (warp-uniform)
-                const float4 nw = phase(u - 1, fc ^ 1, Sp);
-                *reinterpret_cast<float4*>(dst_row + (size_t)(u - 1) * plane) = nw;
+                const float4 nw = phase(Pm2, Pm1, P0, sel, Sp);
+                *reinterpret_cast<float4*>(dst_ptr) = nw;
             }
             Sp = Sc;
+            sel ^= 1;
+            dst_ptr += plane;
+            advance();
         }
     } else {
         // ---- edge warp: ring-1 cells x0-1 and x0+TX of every row, phase B only ----------------
@@ -407,36 +436,35 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         const bool ex_lo = g.bc[0] && gxs == 0, ex_hi = g.bc[0] && gxs1 == 0;
         const bool ey_lo = g.bc[1] && egy == 0, ey_hi = g.bc[1] && egyp == 0;
         struct ESet { float wxl, wxh, wyl, wyh, wzl, wzh, b; };
-        auto fetch_e = [&](int u, ESet& s) {  // global loads, issued one step ahead
-            const int gz = wrap1(u, nz), gzp = wrap1(u + 1, nz);
-            const size_t pz = (size_t)gz * plane, pzp = (size_t)gzp * plane;
+        auto fetch_e = [&](int gzc, ESet& s) {  // global loads, issued one step ahead
+            const int gzn = (gzc + 1 == nz) ? 0 : gzc + 1;
+            const size_t pz = (size_t)gzc * plane, pzp = (size_t)gzn * plane;
             s.wxl = ex_lo ? 0.0f : __ldg(Lx + pz + o_c);
             s.wxh = ex_hi ? 0.0f : __ldg(Lx + pz + o_x1);
             s.wyl = ey_lo ? 0.0f : __ldg(Ly + pz + o_c);
             s.wyh = ey_hi ? 0.0f : __ldg(Ly + pz + o_yp);
-            s.wzl = (g.bc[2] && gz == 0) ? 0.0f : __ldg(Lz + pz + o_c);
-            s.wzh = (g.bc[2] && gzp == 0) ? 0.0f : __ldg(Lz + pzp + o_c);
+            s.wzl = (g.bc[2] && gzc == 0) ? 0.0f : __ldg(Lz + pz + o_c);
+            s.wzh = (g.bc[2] && gzn == 0) ? 0.0f : __ldg(Lz + pzp + o_c);
             s.b = __ldg(a.b + pz + o_c);
         };
         ESet Ec, En;
-        fetch_e(z0 - 1, Ec);
+        fetch_e(gz, Ec);
         En = Ec;
+        int ecol = (xs + eyl + (z0 - 1)) & 1;  // colour of the edge cell in plane u
         for (int u = z0 - 1; u <= z1; ++u) {
-            const int k = u - (z0 - 1);
-            if (u + 1 <= z1) fetch_e(u + 1, En);
-            mbar_wait(bars + (k % C::NB), (uint32_t)(k / C::NB) & 1u);
+            if (u + 1 <= z1) fetch_e((gz + 1 == nz) ? 0 : gz + 1, En);
+            mbar_wait(bars + kb, kpar);
             if (PROLONG) {
                 fix_plane(u + 1);
                 cta_sync();
             }
-            if (e_act && ((xs + eyl + u) & 1) == fc) {
-                float* P = slotP(u);
-                const float pc = P[pc_off];
-                const float Ap = apply7(pc, Ec.wxl, Ec.wxh, Ec.wyl, Ec.wyh, Ec.wzl, Ec.wzh, P[xm_off],
-                                        P[xp_off], P[pc_off - 4], P[pc_off + 4], slotP(u - 1)[pc_off],
-                                        slotP(u + 1)[pc_off]);
-                P[pc_off] = relax(pc, Ec.b, Ap,
-                                  diag6(Ec.wxl, Ec.wxh, Ec.wyl, Ec.wyh, Ec.wzl, Ec.wzh), omega);
+            if (e_act && ecol == fc) {
+                const float pc = P0[pc_off];
+                const float Ap = apply7(pc, Ec.wxl, Ec.wxh, Ec.wyl, Ec.wyh, Ec.wzl, Ec.wzh, P0[xm_off],
+                                        P0[xp_off], P0[pc_off - 4], P0[pc_off + 4], Pm1[pc_off],
+                                        Pp1[pc_off]);
+                P0[pc_off] = relax(pc, Ec.b, Ap,
+                                   diag6(Ec.wxl, Ec.wxh, Ec.wyl, Ec.wyh, Ec.wzl, Ec.wzh), omega);
             }
             cta_sync();
             if (u + C::PD <= z1) {
@@ -444,6 +472,8 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
                 issue_step(u + C::PD);
             }
             Ec = En;
+            ecol ^= 1;
+            advance();
         }
     }
 }
