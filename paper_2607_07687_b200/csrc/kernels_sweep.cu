@@ -367,20 +367,20 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
             return sel ? update_pair_full<1>(xm, own, xp, ym, yp, zm, zp, s, omega)
                        : update_pair_full<0>(xm, own, xp, ym, yp, zm, zp, s, omega);
         };
-        CFull Sp;  // set of plane u-1, handed from B(u-1) to C(u-1)
-        Sp.lx = Sp.ly = Sp.lyh = Sp.lz = Sp.lzh = Sp.b = zero4();
-        Sp.lxh = 0.0f;
         float lxh_pf = last_lane ? __ldg(lxh_row + (size_t)gz * plane) : 0.0f;
         // cells (sel, sel+2) of the group are updated: same parity for B(u) and C(u-1)
         int sel = (yl + (z0 - 1) + fc) & 1;
-        for (int u = z0 - 1; u <= z1; ++u) {
+        const bool any_wall = zx_lo || zx_hi || zy_lo || zy_hi || g.bc[2];
+        // One step.  Sp = coefficient set of plane u-1 (made by B(u-1), used by C(u-1));
+        // Sc = set of plane u, read from shared memory here.  The caller alternates the two
+        // register sets, so nothing is copied between steps.
+        auto step = [&](int u, const CFull& Sp, CFull& Sc) {
             mbar_wait(bars + kb, kpar);
             if (PROLONG) {
                 fix_plane(u + 1);
                 cta_sync();
             }
             const int gzp = (gz + 1 == nz) ? 0 : gz + 1;
-            CFull Sc;
             {   // coefficient set of plane u: shared memory -> registers, wall faces zeroed
                 Sc.lx = lds4(sm + C::OFF_LX + ic * C::C_PLANE + c_off);
                 const float* Y = sm + C::OFF_LY + ic * C::Y_PLANE + c_off;
@@ -392,32 +392,39 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
                 const float t = __shfl_down_sync(0xffffffffu, Sc.lx.x, 1);
                 Sc.lxh = last_lane ? lxh_pf : t;
                 if (last_lane && u + 1 <= z1) lxh_pf = __ldg(lxh_row + (size_t)gzp * plane);
-                if (zx_lo) Sc.lx.x = 0.0f;
-                if (zx_hi) Sc.lxh = 0.0f;
-                if (zy_lo) Sc.ly = zero4();
-                if (zy_hi) Sc.lyh = zero4();
-                if (g.bc[2]) {
-                    if (gz == 0) Sc.lz = zero4();
-                    if (gzp == 0) Sc.lzh = zero4();
+                if (any_wall) {
+                    if (zx_lo) Sc.lx.x = 0.0f;
+                    if (zx_hi) Sc.lxh = 0.0f;
+                    if (zy_lo) Sc.ly = zero4();
+                    if (zy_hi) Sc.lyh = zero4();
+                    if (g.bc[2]) {
+                        if (gz == 0) Sc.lz = zero4();
+                        if (gzp == 0) Sc.lzh = zero4();
+                    }
                 }
             }
             {   // B(u): first colour on tile + ring 1, in place in shared memory
                 const float4 nw = phase(Pm1, P0, Pp1, sel, Sc);
                 *reinterpret_cast<float4*>(P0 + p_off) = nw;
             }
+            fence_async_smem();  // order this thread's smem writes before later TMA overwrites
             cta_sync();
-            if (u + C::PD <= z1) {
-                fence_async_smem();
-                issue_step(u + C::PD);
-            }
+            if (u + C::PD <= z1) issue_step(u + C::PD);
             if (u - 1 >= z0 && row_c) {  // C(u-1): second colour, tile rows only (warp-uniform)
                 const float4 nw = phase(Pm2, Pm1, P0, sel, Sp);
                 *reinterpret_cast<float4*>(dst_ptr) = nw;
             }
-            Sp = Sc;
             sel ^= 1;
             dst_ptr += plane;
             advance();
+        };
+        CFull SA, SB;
+        SA.lx = SA.ly = SA.lyh = SA.lz = SA.lzh = SA.b = zero4();
+        SA.lxh = 0.0f;
+        SB = SA;
+        for (int u = z0 - 1; u <= z1; u += 2) {
+            step(u, SA, SB);
+            if (u + 1 <= z1) step(u + 1, SB, SA);
         }
     } else {
         // ---- edge warp: ring-1 cells x0-1 and x0+TX of every row, phase B only ----------------
@@ -466,11 +473,9 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
                 P0[pc_off] = relax(pc, Ec.b, Ap,
                                    diag6(Ec.wxl, Ec.wxh, Ec.wyl, Ec.wyh, Ec.wzl, Ec.wzh), omega);
             }
+            fence_async_smem();
             cta_sync();
-            if (u + C::PD <= z1) {
-                fence_async_smem();
-                issue_step(u + C::PD);
-            }
+            if (u + C::PD <= z1) issue_step(u + C::PD);
             Ec = En;
             ecol ^= 1;
             advance();
