@@ -122,6 +122,7 @@ struct BulkArgs {
     int first_colour;
     int zchunk;
     int tiles_x, tiles_y;
+    int dbg;
 };
 
 struct alignas(64) BulkMaps {
@@ -214,7 +215,7 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
             bulk_g2s(d + j * C::TX, row_base[first + j] + pz + x0, C::TX * 4u, bar);
     };
     auto issue_step = [&](int v) {  // the data B(v) newly needs: p(v+1), Lz(v+1), Lx(v), Ly(v), b(v)
-        if (lane_id != 0) return;
+        if (lane_id != 0 || (y_inside && warp_id >= 7)) return;
         uint64_t* bar = bars + ((v - (z0 - 1)) % C::NB);
         if (tid == 0) mbar_expect_tx(bar, C::STEP_BYTES);
         const int gz0 = wrap1(v, nz), gz1 = wrap1(v + 1, nz);
@@ -403,14 +404,14 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
                     }
                 }
             }
-            {   // B(u): first colour on tile + ring 1, in place in shared memory
+            if (!(a.dbg & 1)) {   // B(u): first colour on tile + ring 1, in place in shared memory
                 const float4 nw = phase(Pm1, P0, Pp1, sel, Sc);
                 *reinterpret_cast<float4*>(P0 + p_off) = nw;
             }
             fence_async_smem();  // order this thread's smem writes before later TMA overwrites
             cta_sync();
             if (u + C::PD <= z1) issue_step(u + C::PD);
-            if (u - 1 >= z0 && row_c) {  // C(u-1): second colour, tile rows only (warp-uniform)
+            if (u - 1 >= z0 && row_c && !(a.dbg & 2)) {  // C(u-1): second colour, tile rows only (warp-uniform)
                 const float4 nw = phase(Pm2, Pm1, P0, sel, Sp);
                 *reinterpret_cast<float4*>(dst_ptr) = nw;
             }
@@ -489,7 +490,7 @@ void rb_sweep_v2(const LevelGeom& g, const float* L, const float* src, float* ds
                  const float* omega, int first_colour, const float* e_c, cudaStream_t s);
 int configure_v2();
 
-using Bulk = BulkCfg<9, 3>;
+using Bulk = BulkCfg<13, 3>;
 
 static int env_int2(const char* name, int dflt) {
     const char* v = getenv(name);
@@ -554,6 +555,8 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
     BulkArgs a;
     a.g = g; a.L = L; a.src = src; a.dst = dst; a.b = b; a.omega = omega; a.e_c = e_c;
     a.first_colour = first_colour;
+    static const int dbg_env = env_int2("GMG_DBG", 0);
+    a.dbg = dbg_env;
     a.tiles_x = g.n[0] / Bulk::TX;
     a.tiles_y = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
     static const int zc_env = env_int2("GMG_ZCHUNK", 64);
