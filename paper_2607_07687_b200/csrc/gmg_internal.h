@@ -73,7 +73,7 @@ struct ReduceBuf {
     unsigned int* counter;  // ticket of the "last block finishes the sum" stage, self-resetting
     DevScalars* sc;
 };
-#define GMG_REDUCE_MAX_BLOCKS 4096
+#define GMG_REDUCE_MAX_BLOCKS 16384
 
 // ---- launchers (kernels_generic.cu) --------------------------------------------------------
 namespace gmgk {

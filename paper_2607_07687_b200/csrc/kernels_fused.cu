@@ -402,11 +402,9 @@ __global__ void __launch_bounds__(C::THREADS) k_residual_tiled(const ResArgs a) 
                 const int I = u % tcx, J = (u / tcx) % tcy, K = u / (tcx * tcy);
                 const int GI = x0 / cx + I, GJ = y0 / cy + J, GK = z0 / cz + K;
                 if (GI < ncx && GJ < ncy && GK < ncz) {
-                    float s = 0.0f;
-                    for (int aa = 0; aa < cz; ++aa)
-                        for (int bq = 0; bq < cy; ++bq)
-                            for (int e = 0; e < cx; ++e)
-                                s += rs[((cz * K + aa) * C::RY + (cy * J + bq)) * C::TX + cx * I + e];
+                    const float s = restrict_tree(cx, cy, cz, [&](int e, int bq, int aa) {
+                        return rs[((cz * K + aa) * C::RY + (cy * J + bq)) * C::TX + cx * I + e];
+                    });
                     const long long o = GI + (long long)ncx * (GJ + (long long)ncy * GK);
                     a.b_c[o] = s;
                     if (a.p_c) a.p_c[o] = 0.0f;
@@ -481,8 +479,15 @@ static void launch_res(ResArgs& a, cudaStream_t s) {
     k_residual_tiled<C, MODE><<<(unsigned int)nt, C::THREADS, 0, s>>>(a);
 }
 
+bool residual_restrict_bulk(const LevelGeom& g, const float* L, const float* p, const float* b, float* b_c,
+                            float* p_c, cudaStream_t s);
+bool residual_norm2_bulk(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
+                         int slot, cudaStream_t s);
+int configure_residual_bulk();
+
 void residual_restrict(const LevelGeom& g, const float* L, const float* p, const float* b,
                        float* b_c, float* p_c, cudaStream_t s) {
+    if (residual_restrict_bulk(g, L, p, b, b_c, p_c, s)) return;
     ResArgs a;
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = b_c; a.p_c = p_c;
     a.rb = ReduceBuf{nullptr, nullptr, nullptr};
@@ -494,6 +499,7 @@ void residual_restrict(const LevelGeom& g, const float* L, const float* p, const
 
 void residual_norm2(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
                     int slot, cudaStream_t s) {
+    if (residual_norm2_bulk(g, L, p, b, rb, slot, s)) return;
     ResArgs a;
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = nullptr; a.p_c = nullptr;
     a.rb = rb;
@@ -504,6 +510,7 @@ void residual_norm2(const LevelGeom& g, const float* L, const float* p, const fl
 }
 
 int configure_v2() {
+    if (configure_residual_bulk() != 0) return 1;
     cudaError_t e = cudaFuncSetAttribute(k_rb_sweep<Sweep128, kSweepMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Sweep128::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep<Sweep64, kSweepMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Sweep64::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep<Sweep32, kSweepMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Sweep32::SMEM);

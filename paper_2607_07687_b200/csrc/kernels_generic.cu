@@ -68,16 +68,11 @@ k_restrict_sum(LevelGeom gf, const float* __restrict__ rf, float* __restrict__ b
     if (t >= Nc) return;
     const long long row = t / ncx;
     const int I = (int)(t - row * ncx), K = (int)(row / ncy), J = (int)(row - (long long)K * ncy);
-    float s = 0.0f;
-    for (int a = 0; a < gf.c[2]; ++a)
-        for (int bb = 0; bb < gf.c[1]; ++bb)
-            for (int e = 0; e < gf.c[0]; ++e) {
-                const long long f = (gf.c[0] * I + e) +
-                                    (long long)gf.n[0] * ((gf.c[1] * J + bb) +
-                                                          (long long)gf.n[1] * (gf.c[2] * K + a));
-                s += rf[f];
-            }
-    bc[t] = s;
+    bc[t] = restrict_tree(gf.c[0], gf.c[1], gf.c[2], [&](int e, int bb, int a) {
+        const long long f = (gf.c[0] * I + e) +
+                            (long long)gf.n[0] * ((gf.c[1] * J + bb) + (long long)gf.n[1] * (gf.c[2] * K + a));
+        return rf[f];
+    });
 }
 
 void restrict_sum(const LevelGeom& gf, const float* rf, float* bc, cudaStream_t s) {
@@ -86,8 +81,8 @@ void restrict_sum(const LevelGeom& gf, const float* rf, float* bc, cudaStream_t 
 }
 
 // ---- residual fused with restriction (BASELINE.json:north_star) -----------------------------
-// One thread per coarse cell; children summed in the order z, y, x (x innermost), the same
-// order as k_restrict_sum, so fused == unfused bit for bit.
+// One thread per coarse cell; children summed in stencil.cuh's canonical tree order, the same
+// as k_restrict_sum, so fused == unfused bit for bit.
 __global__ void __launch_bounds__(kThreads)
 k_residual_restrict(LevelGeom gf, const float* __restrict__ L, const float* __restrict__ p,
                     const float* __restrict__ b, float* __restrict__ b_c, float* __restrict__ p_c) {
@@ -97,16 +92,12 @@ k_residual_restrict(LevelGeom gf, const float* __restrict__ L, const float* __re
     if (t >= Nc) return;
     const long long row = t / ncx;
     const int I = (int)(t - row * ncx), K = (int)(row / ncy), J = (int)(row - (long long)K * ncy);
-    float s = 0.0f;
-    for (int a = 0; a < gf.c[2]; ++a)
-        for (int bb = 0; bb < gf.c[1]; ++bb)
-            for (int e = 0; e < gf.c[0]; ++e) {
-                const int i = gf.c[0] * I + e, j = gf.c[1] * J + bb, k = gf.c[2] * K + a;
-                const long long f = i + (long long)gf.n[0] * (j + (long long)gf.n[1] * k);
-                const Cell c = cell_stencil(gf, L, p, i, j, k);
-                s += (c.D != 0.0f) ? b[f] - c.Ap : 0.0f;
-            }
-    b_c[t] = s;
+    b_c[t] = restrict_tree(gf.c[0], gf.c[1], gf.c[2], [&](int e, int bb, int a) {
+        const int i = gf.c[0] * I + e, j = gf.c[1] * J + bb, k = gf.c[2] * K + a;
+        const long long f = i + (long long)gf.n[0] * (j + (long long)gf.n[1] * k);
+        const Cell c = cell_stencil(gf, L, p, i, j, k);
+        return (c.D != 0.0f) ? b[f] - c.Ap : 0.0f;
+    });
     if (p_c) p_c[t] = 0.0f;
 }
 

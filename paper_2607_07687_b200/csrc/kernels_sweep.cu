@@ -29,54 +29,6 @@
 
 namespace gmgf {
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-    return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
-    uint32_t ok;
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t"
-        "}"
-        : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-    return ok != 0;
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    while (!mbar_try_wait(bar, parity)) {
-    }
-}
-__device__ __forceinline__ void bulk_g2s(float* dst_smem, const float* src_gmem, uint32_t bytes,
-                                         uint64_t* bar) {
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-            smem_u32(dst_smem)),
-        "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
-        : "memory");
-}
-__device__ __forceinline__ void fence_async_smem() {
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-}
-
-__device__ __forceinline__ void tma_load_3d(float* dst_smem, const CUtensorMap* tm, int c0, int c1, int c2,
-                                            uint64_t* bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(
-            smem_u32(dst_smem)),
-        "l"(reinterpret_cast<uint64_t>(tm)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
-        : "memory");
-}
-
 template <int TY_, int PD_>
 struct BulkCfg {
     static constexpr int TX = 128, TY = TY_, PD = PD_;
@@ -501,11 +453,11 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
                                   CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
                                   CUtensorMapFloatOOBfill);
-static EncodeTiledFn g_encode = nullptr;
+EncodeTiledFn g_encode = nullptr;
 
 // 3-D tiled tensor map over an [nz][ny][nx] FP32 array with a bw x bh x 1 box.  Cached per
 // (pointer, extents, box): encoding costs a few microseconds on the host.
-static bool tensor_map(const float* ptr, const LevelGeom& g, int bw, int bh, CUtensorMap* out) {
+bool tensor_map(const float* ptr, const LevelGeom& g, int bw, int bh, CUtensorMap* out) {
     typedef std::tuple<const float*, int, int, int, int, int> Key;
     static std::map<Key, CUtensorMap> cache;
     const Key key(ptr, g.n[0], g.n[1], g.n[2], bw, bh);
@@ -532,7 +484,7 @@ static bool tensor_map(const float* ptr, const LevelGeom& g, int bw, int bh, CUt
 
 bool sweep_supported(const LevelGeom& g) { return sweep_v2_supported(g); }
 
-static bool bulk_supported(const LevelGeom& g) {
+bool bulk_supported(const LevelGeom& g) {
     return g_encode && g.n[0] >= 128 && g.n[0] % 128 == 0 && g.n[1] >= 4 && g.n[2] >= 8;
 }
 

@@ -86,16 +86,12 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_tail_vcycle(TailArgs a) {
         for (int u = threadIdx.x; u < Nc; u += blockDim.x) {
             const int row = u / ncx;
             const int I = u - row * ncx, K = row / ncy, J = row - K * ncy;
-            float s = 0.0f;
-            for (int aa = 0; aa < g.c[2]; ++aa)
-                for (int bb = 0; bb < g.c[1]; ++bb)
-                    for (int e = 0; e < g.c[0]; ++e) {
-                        const int i = g.c[0] * I + e, j = g.c[1] * J + bb, k = g.c[2] * K + aa;
-                        const int f = i + g.n[0] * (j + g.n[1] * k);
-                        const Cell c = cell_stencil(g, S.L[t], S.p[t], i, j, k);
-                        s += (c.D != 0.0f) ? S.b[t][f] - c.Ap : 0.0f;
-                    }
-            S.b[t + 1][u] = s;
+            S.b[t + 1][u] = restrict_tree(g.c[0], g.c[1], g.c[2], [&](int e, int bb, int aa) {
+                const int i = g.c[0] * I + e, j = g.c[1] * J + bb, k = g.c[2] * K + aa;
+                const int f = i + g.n[0] * (j + g.n[1] * k);
+                const Cell c = cell_stencil(g, S.L[t], S.p[t], i, j, k);
+                return (c.D != 0.0f) ? S.b[t][f] - c.Ap : 0.0f;
+            });
             S.p[t + 1][u] = 0.0f;
         }
         __syncthreads();

@@ -86,6 +86,20 @@ __device__ __forceinline__ float cell_diag(const LevelGeom& g, const float* __re
     return diag6(w[0], w[1], w[2], w[3], w[4], w[5]);
 }
 
+// Canonical child order of the restriction (reading O6: sum over the children): x pairs first,
+// then y pairs, then z pairs -- a tree every kernel (generic, tiled, TMA-fed, single-CTA) can
+// reproduce, so all paths give identical bits.  r(e, b, a) = residual of child (x+e, y+b, z+a).
+template <class F>
+__device__ __forceinline__ float restrict_tree(int cx, int cy, int cz, F r) {
+    float zs[2] = {0.0f, 0.0f};
+    for (int a = 0; a < cz; ++a) {
+        float ys[2] = {0.0f, 0.0f};
+        for (int b = 0; b < cy; ++b) ys[b] = (cx == 2) ? r(0, b, a) + r(1, b, a) : r(0, b, a);
+        zs[a] = (cy == 2) ? ys[0] + ys[1] : ys[0];
+    }
+    return (cz == 2) ? zs[0] + zs[1] : zs[0];
+}
+
 // Deterministic block reduction of one double per thread; result valid in thread 0.
 // blockDim.x must be a multiple of 32 and <= 1024.
 __device__ __forceinline__ double block_sum(double v) {

@@ -26,6 +26,8 @@ CASES = {
     "rand_128_NPP": lambda: random_workload((128, 20, 12), (1, 0, 0), 15),
     "rand_256_PNN": lambda: random_workload((256, 12, 10), (0, 1, 1), 16),
     "rand_128_PPP": lambda: random_workload((128, 40, 8), (0, 0, 0), 17),
+    "rand_256_aniso": lambda: random_workload((256, 6, 12), (0, 0, 0), 18),      # c = (2,1,2)
+    "rand_128_xonly": lambda: random_workload((128, 36, 10), (1, 0, 0), 19, blob=False),
 }
 
 
