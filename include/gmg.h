@@ -70,6 +70,9 @@ typedef struct {
     int n_min;         /* a direction coarsens only while n_d/2 >= n_min (4) O4 */
     int fast_path;     /* 1: fused/tiled kernels where shapes allow; 0: generic kernels only */
     int use_graph;     /* 1: V-cycle captured in a CUDA graph; 0: plain launches */
+    int tma_min_cells; /* levels with at least this many cells (and nx % 128 == 0) use the TMA-fed
+                          z-marching kernels; smaller ones the register-fed tiles (4194304);
+                          0 = whenever the shape allows, -1 = never */
 } gmg_params_t;
 
 /* Statistics of the last gmg_solve. */

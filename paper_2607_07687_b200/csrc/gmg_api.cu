@@ -17,12 +17,12 @@ bool sweep_supported(const LevelGeom& g);
 // first_colour 0: red then black.  If e_c != nullptr the prolonged coarse correction is added
 // to src on the fly (fused prolongation + correction).
 void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
-              const float* omega, int first_colour, const float* e_c, cudaStream_t s);
+              const float* omega, int first_colour, const float* e_c, int allow_tma, cudaStream_t s);
 bool resrestrict_supported(const LevelGeom& g);
 void residual_restrict(const LevelGeom& g, const float* L, const float* p, const float* b,
-                       float* b_c, float* p_c, cudaStream_t s);
+                       float* b_c, float* p_c, int allow_tma, cudaStream_t s);
 void residual_norm2(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
-                    int slot, cudaStream_t s);
+                    int slot, int allow_tma, cudaStream_t s);
 int configure();
 }  // namespace gmgf
 
@@ -48,6 +48,7 @@ struct gmg_ctx {
     size_t tail_smem;
     bool fast_sweep[GMG_MAX_LEVELS];
     bool fast_rr[GMG_MAX_LEVELS];
+    int tma_ok[GMG_MAX_LEVELS];  // level large enough for the TMA-fed kernels
     // workspace
     void* ws;
     size_t ws_bytes;
@@ -122,6 +123,7 @@ static void build_levels(gmg_ctx* c) {
     for (int l = 0; l < c->nlev; ++l) {
         c->fast_sweep[l] = c->prm.fast_path && gmgf::sweep_supported(c->g[l]);
         c->fast_rr[l] = c->prm.fast_path && l + 1 < c->nlev && gmgf::resrestrict_supported(c->g[l]);
+        c->tma_ok[l] = c->prm.tma_min_cells >= 0 && c->g[l].N >= (long long)c->prm.tma_min_cells;
     }
 }
 
@@ -169,7 +171,7 @@ extern "C" void gmg_default_params(gmg_params_t* p) {
     p->nu_pre = 2; p->nu_post = 2; p->nu_coarse = 32;
     p->omega0 = 1.0f; p->omega_min = 0.5f; p->omega_down = 0.125f; p->omega_up = 0.03125f;
     p->adaptive = 1; p->coarsen_mode = GMG_COARSEN_ANISO; p->n_min = 4;
-    p->fast_path = 1; p->use_graph = 1;
+    p->fast_path = 1; p->use_graph = 1; p->tma_min_cells = 4 << 20;
 }
 
 extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]) {
@@ -332,8 +334,8 @@ static void smooth(gmg_ctx* c, int l, float* p, const float* b, const float* ome
         float* q = c->lv[l].q;
         const int pairs = nsweeps / 2;
         for (int i = 0; i < pairs; ++i) {
-            gmgf::rb_sweep(g, c->lv[l].L, p, q, b, omega, first_colour, (i == 0) ? e_c : nullptr, s);
-            gmgf::rb_sweep(g, c->lv[l].L, q, p, b, omega, first_colour, nullptr, s);
+            gmgf::rb_sweep(g, c->lv[l].L, p, q, b, omega, first_colour, (i == 0) ? e_c : nullptr, c->tma_ok[l], s);
+            gmgf::rb_sweep(g, c->lv[l].L, q, p, b, omega, first_colour, nullptr, c->tma_ok[l], s);
             c->n_launch += 2;
         }
         done = 2 * pairs;
@@ -361,7 +363,7 @@ static void enqueue_vcycle(gmg_ctx* c, float* p0, const float* b0, const float* 
     for (; l < ts && l < nlev - 1; ++l) {
         smooth(c, l, P(l), B(l), omega, c->prm.nu_pre, 0, nullptr, s);
         if (c->fast_rr[l])
-            gmgf::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, s);
+            gmgf::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, c->tma_ok[l], s);
         else
             gmgk::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, s);
         c->n_launch += 1;
@@ -422,7 +424,7 @@ struct LoopCtl {
 
 static void level0_residual_norm2(gmg_ctx* c, const float* p, const float* z, cudaStream_t s) {
     if (c->prm.fast_path && gmgf::resrestrict_supported(c->g[0]))
-        gmgf::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, s);
+        gmgf::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, c->tma_ok[0], s);
     else
         gmgk::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, s);
 }
@@ -727,7 +729,7 @@ extern "C" int gmg_op_restrict(gmg_ctx* c, int lev, const float* r_fine, float* 
 extern "C" int gmg_op_residual_restrict(gmg_ctx* c, int lev, const float* p, const float* b,
                                         float* b_coarse, void* stream) {
     HOOK_PROLOGUE(lev >= 0 && lev < c->nlev - 1 && p && b && b_coarse)
-    if (c->fast_rr[lev]) gmgf::residual_restrict(c->g[lev], c->lv[lev].L, p, b, b_coarse, nullptr, s);
+    if (c->fast_rr[lev]) gmgf::residual_restrict(c->g[lev], c->lv[lev].L, p, b, b_coarse, nullptr, c->tma_ok[lev], s);
     else gmgk::residual_restrict(c->g[lev], c->lv[lev].L, p, b, b_coarse, nullptr, s);
     HOOK_EPILOGUE()
 }
@@ -761,8 +763,9 @@ extern "C" int gmg_describe_plan(const gmg_ctx* c, char* buf, size_t cap) {
     size_t off = 0;
     buf[0] = 0;
     for (int l = 0; l < c->nlev; ++l) {
+        const bool tma = c->tma_ok[l] && c->g[l].n[0] % 128 == 0 && c->g[l].n[1] >= 4 && c->g[l].n[2] >= 8;
         const char* how = (l >= c->tail_start) ? "tail(single-CTA smem)"
-                          : (c->fast_sweep[l] ? "fused-rb-sweep" : "generic-half-sweeps");
+                          : (c->fast_sweep[l] ? (tma ? "fused-rb-sweep(TMA)" : "fused-rb-sweep") : "generic-half-sweeps");
         const char* rr = (l >= c->tail_start || l == c->nlev - 1) ? "-"
                          : (c->fast_rr[l] ? "tiled" : "generic");
         int w = snprintf(buf + off, cap - off, "L%d %dx%dx%d c=%d%d%d sweep=%s resrestrict=%s\n", l,

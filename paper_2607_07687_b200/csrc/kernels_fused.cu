@@ -32,6 +32,10 @@
 #include "fused_common.cuh"
 
 namespace gmgf {
+static int zmin_env() {
+    static const int v = getenv("GMG_ZMIN") ? atoi(getenv("GMG_ZMIN")) : 4;
+    return v;
+}
 
 template <int TX_, int TY_>
 struct SweepCfg {
@@ -444,7 +448,7 @@ static void launch_sweep(SweepArgs& a, cudaStream_t s) {
     int zchunk = zc_env;
     if (g.n[2] < 2 * zchunk) zchunk = g.n[2];
     // keep at least ~4 CTAs per SM in flight on mid-size levels
-    while (zchunk > 16 && (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) < 148 * 4)
+    while (zchunk > zmin_env() && (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) < 148 * 4)
         zchunk = (zchunk + 1) / 2;
     a.zchunk = zchunk;
     static const int pf_env = env_int("GMG_PF", 3);
@@ -486,8 +490,8 @@ bool residual_norm2_bulk(const LevelGeom& g, const float* L, const float* p, con
 int configure_residual_bulk();
 
 void residual_restrict(const LevelGeom& g, const float* L, const float* p, const float* b,
-                       float* b_c, float* p_c, cudaStream_t s) {
-    if (residual_restrict_bulk(g, L, p, b, b_c, p_c, s)) return;
+                       float* b_c, float* p_c, int allow_tma, cudaStream_t s) {
+    if (allow_tma && residual_restrict_bulk(g, L, p, b, b_c, p_c, s)) return;
     ResArgs a;
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = b_c; a.p_c = p_c;
     a.rb = ReduceBuf{nullptr, nullptr, nullptr};
@@ -498,8 +502,8 @@ void residual_restrict(const LevelGeom& g, const float* L, const float* p, const
 }
 
 void residual_norm2(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
-                    int slot, cudaStream_t s) {
-    if (residual_norm2_bulk(g, L, p, b, rb, slot, s)) return;
+                    int slot, int allow_tma, cudaStream_t s) {
+    if (allow_tma && residual_norm2_bulk(g, L, p, b, rb, slot, s)) return;
     ResArgs a;
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = nullptr; a.p_c = nullptr;
     a.rb = rb;

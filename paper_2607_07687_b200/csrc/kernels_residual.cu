@@ -16,6 +16,10 @@
 #include "fused_common.cuh"
 
 namespace gmgf {
+static int zmin_env() {
+    static const int v = getenv("GMG_ZMIN") ? atoi(getenv("GMG_ZMIN")) : 4;
+    return v;
+}
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
@@ -359,7 +363,7 @@ static bool launch_res_bulk(ResBulkArgs& a, cudaStream_t s) {
     a.tiles_y = (g.n[1] + C::RY - 1) / C::RY;
     int zchunk = 64;
     if (g.n[2] < 2 * zchunk) zchunk = g.n[2];
-    while (zchunk > 16 && zchunk % 4 == 0 &&
+    while (zchunk > zmin_env() && zchunk % 4 == 0 &&
            (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) < 148 * 4)
         zchunk /= 2;
     // the deterministic reduction has a bounded number of block partials

@@ -28,6 +28,10 @@
 #include "fused_common.cuh"
 
 namespace gmgf {
+static int zmin_env() {
+    static const int v = getenv("GMG_ZMIN") ? atoi(getenv("GMG_ZMIN")) : 4;
+    return v;
+}
 
 template <int TY_, int PD_>
 struct BulkCfg {
@@ -489,11 +493,11 @@ bool bulk_supported(const LevelGeom& g) {
 }
 
 void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
-              const float* omega, int first_colour, const float* e_c, cudaStream_t s) {
+              const float* omega, int first_colour, const float* e_c, int allow_tma, cudaStream_t s) {
     static const int use_bulk = env_int2("GMG_BULK", 1);
     BulkMaps maps;
     const size_t N = (size_t)g.N;
-    bool ok = use_bulk && bulk_supported(g);
+    bool ok = use_bulk && allow_tma && bulk_supported(g);
     ok = ok && tensor_map(src, g, Bulk::TX, Bulk::SH, &maps.p_main);
     ok = ok && tensor_map(src, g, 4, Bulk::SH, &maps.p_halo);
     ok = ok && tensor_map(L + 2 * N, g, Bulk::TX, Bulk::ROWS, &maps.lz);
@@ -514,7 +518,7 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
     static const int zc_env = env_int2("GMG_ZCHUNK", 64);
     int zchunk = zc_env;
     if (g.n[2] < 2 * zchunk) zchunk = g.n[2];
-    while (zchunk > 16 && (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) < 148 * 2)
+    while (zchunk > zmin_env() && (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) < 148 * 2)
         zchunk = (zchunk + 1) / 2;
     a.zchunk = zchunk;
     const int nzc = (g.n[2] + zchunk - 1) / zchunk;

@@ -50,9 +50,9 @@ def test_library_contains_sm100a_code(libpath):
 
 
 def test_struct_sizes_match_header(libpath):
-    """Params / Stats mirror the C structs (12 x 4 bytes; Stats has 8-byte alignment)."""
+    """Params / Stats mirror the C structs (13 x 4 bytes; Stats has 8-byte alignment)."""
     from paper_2607_07687_b200 import gmg
-    assert C.sizeof(gmg.Params) == 48
+    assert C.sizeof(gmg.Params) == 52
     assert C.sizeof(gmg.Stats) == 4 * 4 + 6 * 8 + 8 + 8
     p = gmg.Params()
     gmg.lib.gmg_default_params(C.byref(p))

@@ -34,7 +34,7 @@ CASES = {
 @pytest.fixture(scope="module", params=sorted(CASES), ids=sorted(CASES))
 def case(request):
     wl = CASES[request.param]()
-    g = make_gpu(wl)
+    g = make_gpu(wl, tma_min_cells=0)      # TMA-fed kernels wherever the shape allows
     h = make_oracle(wl)
     yield wl, g, h
     g.close()
