@@ -29,6 +29,16 @@ METRIC = "poisson_solve_ns_per_cell_gmg_rbgs_tol1e-4"
 UNIT = "ns/cell"
 
 
+def profiled_traffic(workload, kernel):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of `kernel` from the
+    committed `ncu --set full` capture of this workload (profiles/traffic.json), else None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return float(json.load(f)[workload][kernel]["dram_bytes_per_launch"])
+    except Exception:
+        return None
+
+
 def measured_peak():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -154,7 +164,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
 
-    from paper_2607_07687_b200 import gmg
+    from paper_2607_07687_b200 import gmg, replicas
     from paper_2607_07687_b200 import workloads as W
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -168,15 +178,14 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=device)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        replicas.barrier()
         torch.cuda.synchronize()
 
     t_gen = time.perf_counter()
     wl = W.by_name(args.workload)
     t_gen = time.perf_counter() - t_gen
     N = wl.cells
-    g = gmg.GMG(wl.n, wl.bc, device=str(device))
+    g = gmg.GMG(wl.n, wl.bc, device=str(device), **({"use_graph": 0} if args.no_graph else {}))
     L = torch.from_numpy(wl.L).to(device)
     z = torch.from_numpy(wl.z).to(device)
     p = torch.zeros_like(z)
@@ -206,14 +215,10 @@ def run_ours(args):
             iters.append(st["iterations"])
         e1.record(stream)
         barrier()
-    ms_total = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms_total], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = replicas.max_over_ranks(e0.elapsed_time(e1), device)
     ms_step = ms_total / args.steps
     final = g.stats()
-    value = ms_step * 1e6 / (N * world)
+    value = replicas.ns_per_cell(ms_step, N, world)
     ns_per_cell_vcycle = (final["gpu_ms"] * 1e6 / N) / max(final["iterations"], 1)
 
     # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the region -----
@@ -230,12 +235,8 @@ def run_ours(args):
         g.set_omega(1.0)
         g.solve_host(ph, zh, tol=tol, maxiter=maxiter, solver=gmg.GMG_RBGS)
     barrier()
-    e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_ms], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-    e2e_val = e2e_ms * 1e6 / (N * world)
+    e2e_ms = replicas.max_over_ranks(1e3 * (time.perf_counter() - t0) / e2e_steps, device)
+    e2e_val = replicas.ns_per_cell(e2e_ms, N, world)
 
     if rank != 0:
         if world > 1:
@@ -284,11 +285,13 @@ def run_ours(args):
                    "bytes_per_fine_cell": vc_bytes / N},
         "roofline": {"bound": "hbm", "kernel": "level-0 red+black Gauss-Seidel sweep",
                      "achieved": sweep_gbs, "peak": peak, "unit": "GB/s", "frac": sweep_gbs / peak,
-                     "traffic": None, "peak_source": peak_src, "ms_per_launch": t_sweep,
+                     "traffic": profiled_traffic(args.workload, "sweep"), "peak_source": peak_src,
+                     "ms_per_launch": t_sweep,
                      "algorithmic_bytes_per_cell": 24.0,
                      "frac_of_nominal_8TBs": sweep_gbs / 8000.0},
         "roofline_residual_restrict": {"achieved": rr_gbs, "peak": peak, "unit": "GB/s",
                                        "frac": rr_gbs / peak, "ms_per_launch": t_rr,
+                                       "traffic": profiled_traffic(args.workload, "residual_restrict"),
                                        "algorithmic_bytes_per_cell": 20.0 + 4.0 / m},
         "cpu_baseline": cpu,
         "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": e2e_ms,
@@ -312,6 +315,9 @@ def main():
     ap.add_argument("--workload", default="c4")
     ap.add_argument("--reference-sample", default="c4_256")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-graph", action="store_true",
+                    help="plain kernel launches instead of the CUDA-graph WHILE loop (so that ncu "
+                         "lists every kernel of the solve)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
