@@ -33,15 +33,16 @@ static int zmin_env() {
     return v;
 }
 
-template <int TY_, int PD_>
+template <int TY_, int PD_, int PL_>
 struct BulkCfg {
     static constexpr int TX = 128, TY = TY_, PD = PD_;
+    static constexpr int PL = PL_;               // extra lead of the p planes (prolongation fix-up)
     static constexpr int LPR = 32;
     static constexpr int ROWS = TY + 2;          // rows running phase B (tile + ring 1)
     static constexpr int MAIN = LPR * ROWS;
     static constexpr int THREADS = MAIN + 32;    // + one edge warp
     static constexpr int SH = TY + 4;            // rows of a p plane (halo 2)
-    static constexpr int NP = PD + 4;            // ring depths (slot-reuse argument: DESIGN.md S6)
+    static constexpr int NP = PD + 4 + PL;       // ring depths (slot-reuse argument: DESIGN.md S6)
     static constexpr int NZ = PD + 1;
     static constexpr int NC = PD;
     static constexpr int NB = PD + 1;            // mbarriers of the step groups
@@ -61,7 +62,7 @@ struct BulkCfg {
     static constexpr size_t SMEM = (size_t)FLOATS * sizeof(float) + 16 * sizeof(uint64_t) + (size_t)NROWCOPY * 16;
     static constexpr uint32_t STEP_BYTES =
         (uint32_t)(SH * TX + 2 * SH * 4 + 3 * ROWS * TX + (ROWS + 1) * TX) * 4u;
-    static constexpr uint32_t PRO_BYTES = (uint32_t)(2 * (SH * TX + 2 * SH * 4) + ROWS * TX) * 4u;
+    static constexpr uint32_t PRO_BYTES = (uint32_t)((2 + PL) * (SH * TX + 2 * SH * 4) + ROWS * TX) * 4u;
     static constexpr int AGROUPS = (LPR + 2) * SH;      // float4 groups of a p plane (prolong fix-up)
     static constexpr int APER = (AGROUPS + THREADS - 1) / THREADS;
     static_assert(2 * ROWS <= 32 && NB <= 8 && THREADS / 32 >= 7, "tile shape");
@@ -155,7 +156,7 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     }
     auto copy_p_rows = [&](int v, uint64_t* bar) {  // row path: the SH rows of p plane v
         float* d = slotP(v);
-        const size_t pz = (size_t)wrap1(v, nz) * plane;
+        const size_t pz = (size_t)wrapi(v, nz) * plane;
         for (int j = warp_id; j < C::SH; j += NWARP) {
             const float* rb = row_base[j] + pz;
             bulk_g2s(d + j * C::TX, rb + x0, C::TX * 4u, bar);
@@ -175,11 +176,12 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         uint64_t* bar = bars + ((v - (z0 - 1)) % C::NB);
         if (tid == 0) mbar_expect_tx(bar, C::STEP_BYTES);
         const int gz0 = wrap1(v, nz), gz1 = wrap1(v + 1, nz);
+        const int vp = v + 1 + C::PL, gzv = wrapi(vp, nz);   // the p plane of this group
         if (y_inside) {
             switch (warp_id) {
-                case 0: tma_load_3d(slotP(v + 1), &maps.p_main, x0, y0 - 2, gz1, bar); break;
-                case 1: tma_load_3d(slotP(v + 1) + C::P_HL, &maps.p_halo, xL, y0 - 2, gz1, bar); break;
-                case 2: tma_load_3d(slotP(v + 1) + C::P_HR, &maps.p_halo, xR, y0 - 2, gz1, bar); break;
+                case 0: tma_load_3d(slotP(vp), &maps.p_main, x0, y0 - 2, gzv, bar); break;
+                case 1: tma_load_3d(slotP(vp) + C::P_HL, &maps.p_halo, xL, y0 - 2, gzv, bar); break;
+                case 2: tma_load_3d(slotP(vp) + C::P_HR, &maps.p_halo, xR, y0 - 2, gzv, bar); break;
                 case 3: tma_load_3d(slotLz(v + 1), &maps.lz, x0, y0 - 1, gz1, bar); break;
                 case 4: tma_load_3d(slotLx(v), &maps.lx, x0, y0 - 1, gz0, bar); break;
                 case 5: tma_load_3d(slotLy(v), &maps.ly, x0, y0 - 1, gz0, bar); break;
@@ -187,7 +189,7 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
                 default: break;
             }
         } else {
-            copy_p_rows(v + 1, bar);
+            copy_p_rows(vp, bar);
             copy_c_rows(1, slotLz(v + 1), (size_t)gz1 * plane, bar);
             copy_c_rows(2, slotLx(v), (size_t)gz0 * plane, bar);
             copy_c_rows(3, slotLy(v), (size_t)gz0 * plane, bar);
@@ -215,7 +217,7 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     }
     auto fix_plane = [&](int v) {
         float* P = slotP(v);
-        const float* eb = a.e_c + (size_t)(wrap1(v, nz) / g.c[2]) * (ncx * ncy);
+        const float* eb = a.e_c + (size_t)(wrapi(v, nz) / g.c[2]) * (ncx * ncy);
 #pragma unroll
         for (int i = 0; i < C::APER; ++i) {
             if (f_soff[i] >= 0) {
@@ -243,29 +245,28 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         uint64_t* bar = bars + C::NB;
         if (lane_id == 0) {
             if (tid == 0) mbar_expect_tx(bar, C::PRO_BYTES);
-            const int ga = wrap1(z0 - 2, nz), gb = wrap1(z0 - 1, nz);
+            const int gb = wrap1(z0 - 1, nz);
             if (y_inside) {
-                switch (warp_id) {
-                    case 0: tma_load_3d(slotP(z0 - 2), &maps.p_main, x0, y0 - 2, ga, bar); break;
-                    case 1: tma_load_3d(slotP(z0 - 2) + C::P_HL, &maps.p_halo, xL, y0 - 2, ga, bar); break;
-                    case 2: tma_load_3d(slotP(z0 - 2) + C::P_HR, &maps.p_halo, xR, y0 - 2, ga, bar); break;
-                    case 3: tma_load_3d(slotP(z0 - 1), &maps.p_main, x0, y0 - 2, gb, bar); break;
-                    case 4: tma_load_3d(slotP(z0 - 1) + C::P_HL, &maps.p_halo, xL, y0 - 2, gb, bar); break;
-                    case 5: tma_load_3d(slotP(z0 - 1) + C::P_HR, &maps.p_halo, xR, y0 - 2, gb, bar); break;
-                    case 6: tma_load_3d(slotLz(z0 - 1), &maps.lz, x0, y0 - 1, gb, bar); break;
-                    default: break;
+                // planes z0-2 .. z0-1+PL: three boxes each, one per warp; then Lz(z0-1)
+                const int pl = warp_id / 3, k = warp_id % 3;
+                if (pl < 2 + C::PL) {
+                    const int v = z0 - 2 + pl, gv = wrapi(v, nz);
+                    if (k == 0) tma_load_3d(slotP(v), &maps.p_main, x0, y0 - 2, gv, bar);
+                    else if (k == 1) tma_load_3d(slotP(v) + C::P_HL, &maps.p_halo, xL, y0 - 2, gv, bar);
+                    else tma_load_3d(slotP(v) + C::P_HR, &maps.p_halo, xR, y0 - 2, gv, bar);
+                } else if (warp_id == 3 * (2 + C::PL)) {
+                    tma_load_3d(slotLz(z0 - 1), &maps.lz, x0, y0 - 1, gb, bar);
                 }
             } else {
-                copy_p_rows(z0 - 2, bar);
-                copy_p_rows(z0 - 1, bar);
+                for (int pl = 0; pl < 2 + C::PL; ++pl) copy_p_rows(z0 - 2 + pl, bar);
                 copy_c_rows(1, slotLz(z0 - 1), (size_t)gb * plane, bar);
             }
         }
         for (int v = z0 - 1; v < z0 - 1 + C::PD && v <= z1; ++v) issue_step(v);
         mbar_wait(bar, 0);
         if (PROLONG) {
-            fix_plane(z0 - 2);
-            fix_plane(z0 - 1);
+            for (int pl = 0; pl < 2 + C::PL; ++pl) fix_plane(z0 - 2 + pl);
+            __syncthreads();  // B(z0-1) reads groups other threads fixed
         }
     }
 
@@ -333,10 +334,6 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         // register sets, so nothing is copied between steps.
         auto step = [&](int u, const CFull& Sp, CFull& Sc) {
             mbar_wait(bars + kb, kpar);
-            if (PROLONG) {
-                fix_plane(u + 1);
-                cta_sync();
-            }
             const int gzp = (gz + 1 == nz) ? 0 : gz + 1;
             {   // coefficient set of plane u: shared memory -> registers, wall faces zeroed
                 Sc.lx = lds4(sm + C::OFF_LX + ic * C::C_PLANE + c_off);
@@ -364,6 +361,9 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
                 const float4 nw = phase(Pm1, P0, Pp1, sel, Sc);
                 *reinterpret_cast<float4*>(P0 + p_off) = nw;
             }
+            // prolongation fix-up of the plane that landed with this step's group: it is first read
+            // after the barrier below (by B(u+1), as the plane above)
+            if (PROLONG && u + 1 + C::PL <= z1 + 1) fix_plane(u + 1 + C::PL);
             fence_async_smem();  // order this thread's smem writes before later TMA overwrites
             cta_sync();
             if (u + C::PD <= z1) issue_step(u + C::PD);
@@ -418,10 +418,6 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         for (int u = z0 - 1; u <= z1; ++u) {
             if (u + 1 <= z1) fetch_e((gz + 1 == nz) ? 0 : gz + 1, En);
             mbar_wait(bars + kb, kpar);
-            if (PROLONG) {
-                fix_plane(u + 1);
-                cta_sync();
-            }
             if (e_act && ecol == fc) {
                 const float pc = P0[pc_off];
                 const float Ap = apply7(pc, Ec.wxl, Ec.wxh, Ec.wyl, Ec.wyh, Ec.wzl, Ec.wzh, P0[xm_off],
@@ -430,6 +426,7 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
                 P0[pc_off] = relax(pc, Ec.b, Ap,
                                    diag6(Ec.wxl, Ec.wxh, Ec.wyl, Ec.wyh, Ec.wzl, Ec.wzh), omega);
             }
+            if (PROLONG && u + 1 + C::PL <= z1 + 1) fix_plane(u + 1 + C::PL);
             fence_async_smem();
             cta_sync();
             if (u + C::PD <= z1) issue_step(u + C::PD);
@@ -446,7 +443,8 @@ void rb_sweep_v2(const LevelGeom& g, const float* L, const float* src, float* ds
                  const float* omega, int first_colour, const float* e_c, cudaStream_t s);
 int configure_v2();
 
-using Bulk = BulkCfg<13, 3>;
+using Bulk = BulkCfg<13, 3, 0>;
+using BulkP = BulkCfg<13, 3, 1>;   // prolongation fused: p planes one step further ahead
 
 static int env_int2(const char* name, int dflt) {
     const char* v = getenv(name);
@@ -523,13 +521,13 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
     a.zchunk = zchunk;
     const int nzc = (g.n[2] + zchunk - 1) / zchunk;
     const unsigned int grid = (unsigned int)(a.tiles_x * a.tiles_y * nzc);
-    if (e_c) k_rb_sweep_bulk<Bulk, true><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+    if (e_c) k_rb_sweep_bulk<BulkP, true><<<grid, BulkP::THREADS, BulkP::SMEM, s>>>(a, maps);
     else k_rb_sweep_bulk<Bulk, false><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
 }
 
 int configure() {
     cudaError_t e = (cudaError_t)configure_v2();
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep_bulk<BulkP, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BulkP::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
     if (e == cudaSuccess && !g_encode) {
         void* fn = nullptr;
