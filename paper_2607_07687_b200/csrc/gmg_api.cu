@@ -23,6 +23,8 @@ void residual_restrict(const LevelGeom& g, const float* L, const float* p, const
                        float* b_c, float* p_c, int allow_tma, cudaStream_t s);
 void residual_norm2(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
                     int slot, int allow_tma, cudaStream_t s);
+void prolong_add4(const LevelGeom& g, const float* e_c, float* p_f, cudaStream_t s);
+bool tma_shape_ok(const LevelGeom& g);
 int configure();
 }  // namespace gmgf
 
@@ -330,6 +332,12 @@ static void smooth(gmg_ctx* c, int l, float* p, const float* b, const float* ome
                    int first_colour, const float* e_c, cudaStream_t s) {
     const LevelGeom& g = c->g[l];
     int done = 0;
+    if (e_c && c->fast_sweep[l] && nsweeps >= 2 && c->tma_ok[l] && gmgf::tma_shape_ok(g)) {
+        // in front of the TMA-fed sweep the correction is cheaper as its own streaming pass
+        gmgf::prolong_add4(g, e_c, p, s);
+        c->n_launch += 1;
+        e_c = nullptr;
+    }
     if (c->fast_sweep[l] && nsweeps >= 2) {
         float* q = c->lv[l].q;
         const int pairs = nsweeps / 2;

@@ -420,6 +420,41 @@ __global__ void __launch_bounds__(C::THREADS) k_residual_tiled(const ResArgs a) 
     if (MODE == 1) finish_reduction(acc, 0.0, false, a.rb, a.slot, 0);
 }
 
+
+// ---- prolongation + correction as its own pass (O6): p_f(I) += e_c(parent(I)), one float4 of
+// fine cells per thread.  Used in front of the TMA-fed sweep, where fusing the correction into the
+// sweep's shared-memory planes costs more than this 8.5 B/cell streaming pass.
+__global__ void __launch_bounds__(256)
+k_prolong_add4(LevelGeom g, const float* __restrict__ e_c, float* __restrict__ p_f) {
+    const int nx4 = g.n[0] >> 2;
+    const long long ngroups = g.N >> 2;
+    const int ncx = g.n[0] / g.c[0], ncy = g.n[1] / g.c[1];
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < ngroups;
+         t += (long long)gridDim.x * blockDim.x) {
+        const long long row = t / nx4;
+        const int i4 = (int)(t - row * nx4);
+        const int k = (int)(row / g.n[1]);
+        const int j = (int)(row - (long long)k * g.n[1]);
+        const long long pc = (long long)(k / g.c[2]) * ncy + (j / g.c[1]);
+        float4 v = *reinterpret_cast<const float4*>(p_f + 4 * t);
+        if (g.c[0] == 2) {
+            const float2 e = __ldg(reinterpret_cast<const float2*>(e_c + pc * ncx + 2 * i4));
+            v.x += e.x; v.y += e.x; v.z += e.y; v.w += e.y;
+        } else {
+            const float4 e = ldg4(e_c + pc * ncx + 4 * i4);
+            v.x += e.x; v.y += e.y; v.z += e.z; v.w += e.w;
+        }
+        *reinterpret_cast<float4*>(p_f + 4 * t) = v;
+    }
+}
+
+void prolong_add4(const LevelGeom& g, const float* e_c, float* p_f, cudaStream_t s) {
+    const long long ngroups = g.N >> 2;
+    long long nb = (ngroups + 255) / 256;
+    if (nb > 148LL * 64) nb = 148LL * 64;
+    k_prolong_add4<<<(unsigned int)nb, 256, 0, s>>>(g, e_c, p_f);
+}
+
 // ---- launchers ----------------------------------------------------------------------------------
 using Sweep128 = SweepCfg<128, 9>;
 using Sweep64 = SweepCfg<64, 14>;

@@ -215,23 +215,37 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
             }
         }
     }
-    auto fix_plane = [&](int v) {
-        float* P = slotP(v);
-        const float* eb = a.e_c + (size_t)(wrapi(v, nz) / g.c[2]) * (ncx * ncy);
+    struct EReg { float4 e[C::APER]; };
+    const int czs = g.c[2] - 1;                 // coarse plane = fine plane >> czs
+    const int cplane = ncx * ncy;
+    auto fix_fetch_at = [&](int gzf, EReg& r) {   // coarse values for (wrapped) fine plane gzf
+        const float* eb = a.e_c + (size_t)(gzf >> czs) * cplane;
+#pragma unroll
+        for (int i = 0; i < C::APER; ++i) {
+            if (f_soff[i] >= 0) {
+                if (g.c[0] == 2) {
+                    const float2 e2 = __ldg(reinterpret_cast<const float2*>(eb + f_coff[i]));
+                    r.e[i] = make_float4(e2.x, e2.x, e2.y, e2.y);
+                } else {
+                    r.e[i] = ldg4(eb + f_coff[i]);
+                }
+            }
+        }
+    };
+    auto fix_apply_at = [&](float* P, const EReg& r) {  // p += P e_c in the shared-memory plane P
 #pragma unroll
         for (int i = 0; i < C::APER; ++i) {
             if (f_soff[i] >= 0) {
                 float4 val = lds4(P + f_soff[i]);
-                if (g.c[0] == 2) {
-                    const float2 e2 = __ldg(reinterpret_cast<const float2*>(eb + f_coff[i]));
-                    val.x += e2.x; val.y += e2.x; val.z += e2.y; val.w += e2.y;
-                } else {
-                    const float4 e4 = ldg4(eb + f_coff[i]);
-                    val.x += e4.x; val.y += e4.y; val.z += e4.z; val.w += e4.w;
-                }
+                val.x += r.e[i].x; val.y += r.e[i].y; val.z += r.e[i].z; val.w += r.e[i].w;
                 *reinterpret_cast<float4*>(P + f_soff[i]) = val;
             }
         }
+    };
+    auto fix_plane = [&](int v) {
+        EReg r;
+        fix_fetch_at(wrapi(v, nz), r);
+        fix_apply_at(slotP(v), r);
     };
 
     // ---- prologue: barriers; p(z0-2), p(z0-1), Lz(z0-1); the first PD step groups --------------
@@ -277,6 +291,8 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     float* Pm1 = P_beg;                             // plane u-1
     float* P0 = P_beg + C::P_PLANE;                 // plane u
     float* Pp1 = P_beg + 2 * C::P_PLANE;            // plane u+1
+    float* Pp2 = P_beg + 3 * C::P_PLANE;            // plane u+2 (prolongation fix-up target)
+    int gzf = wrapi(z0 - 1 + 1 + C::PL, nz);        // wrapped index of plane u+1+PL
     const float* Z0 = Z_beg;                        // Lz plane u
     const float* Z1 = Z_beg + C::C_PLANE;           // Lz plane u+1
     int ic = 0;                                     // slot of Lx / Ly / b plane u
@@ -285,8 +301,10 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     int gz = wrap1(z0 - 1, nz);                     // wrapped plane index of u
     auto advance = [&]() {
         Pm2 = Pm1; Pm1 = P0; P0 = Pp1;
-        Pp1 += C::P_PLANE;
-        if (Pp1 == P_beg + C::NP * C::P_PLANE) Pp1 = P_beg;
+        Pp1 = Pp2;
+        Pp2 += C::P_PLANE;
+        if (Pp2 == P_beg + C::NP * C::P_PLANE) Pp2 = P_beg;
+        if (++gzf == nz) gzf = 0;
         Z0 = Z1;
         Z1 += C::C_PLANE;
         if (Z1 == Z_beg + C::NZ * C::C_PLANE) Z1 = Z_beg;
@@ -333,6 +351,9 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         // Sc = set of plane u, read from shared memory here.  The caller alternates the two
         // register sets, so nothing is copied between steps.
         auto step = [&](int u, const CFull& Sp, CFull& Sc) {
+            EReg er;
+            const bool do_fix = PROLONG && (u + 1 + C::PL <= z1 + 1);
+            if (do_fix) fix_fetch_at(gzf, er);   // latency hidden behind the wait and B(u)
             mbar_wait(bars + kb, kpar);
             const int gzp = (gz + 1 == nz) ? 0 : gz + 1;
             {   // coefficient set of plane u: shared memory -> registers, wall faces zeroed
@@ -363,7 +384,7 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
             }
             // prolongation fix-up of the plane that landed with this step's group: it is first read
             // after the barrier below (by B(u+1), as the plane above)
-            if (PROLONG && u + 1 + C::PL <= z1 + 1) fix_plane(u + 1 + C::PL);
+            if (do_fix) fix_apply_at(C::PL ? Pp2 : Pp1, er);
             fence_async_smem();  // order this thread's smem writes before later TMA overwrites
             cta_sync();
             if (u + C::PD <= z1) issue_step(u + C::PD);
@@ -417,6 +438,9 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         int ecol = (xs + eyl + (z0 - 1)) & 1;  // colour of the edge cell in plane u
         for (int u = z0 - 1; u <= z1; ++u) {
             if (u + 1 <= z1) fetch_e((gz + 1 == nz) ? 0 : gz + 1, En);
+            EReg er;
+            const bool do_fix = PROLONG && (u + 1 + C::PL <= z1 + 1);
+            if (do_fix) fix_fetch_at(gzf, er);
             mbar_wait(bars + kb, kpar);
             if (e_act && ecol == fc) {
                 const float pc = P0[pc_off];
@@ -426,7 +450,7 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
                 P0[pc_off] = relax(pc, Ec.b, Ap,
                                    diag6(Ec.wxl, Ec.wxh, Ec.wyl, Ec.wyh, Ec.wzl, Ec.wzh), omega);
             }
-            if (PROLONG && u + 1 + C::PL <= z1 + 1) fix_plane(u + 1 + C::PL);
+            if (do_fix) fix_apply_at(C::PL ? Pp2 : Pp1, er);
             fence_async_smem();
             cta_sync();
             if (u + C::PD <= z1) issue_step(u + C::PD);
@@ -485,6 +509,12 @@ bool tensor_map(const float* ptr, const LevelGeom& g, int bw, int bh, CUtensorMa
 }
 
 bool sweep_supported(const LevelGeom& g) { return sweep_v2_supported(g); }
+
+bool bulk_supported(const LevelGeom& g);
+bool tma_shape_ok(const LevelGeom& g) {
+    static const int use_bulk = env_int2("GMG_BULK", 1);
+    return use_bulk && bulk_supported(g);
+}
 
 bool bulk_supported(const LevelGeom& g) {
     return g_encode && g.n[0] >= 128 && g.n[0] % 128 == 0 && g.n[1] >= 4 && g.n[2] >= 8;
