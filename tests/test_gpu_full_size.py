@@ -1,0 +1,114 @@
+"""-m gpu: parity at the sizes and in the launch configuration bench.py times (BASELINE.json
+configs[4], 1024^3; its 512^3 shrink always runs), where the oracle cannot hold the whole problem in
+the test's time budget.  Checked: (a) SAMPLED outputs the oracle computes one by one -- for a
+sampled cell the oracle runs on the 9^3 neighbourhood cut out of the real
+arrays, which determines that cell's result exactly; (b) properties that hold at any size --
+sum(r) = sum(z) (zero column sums), the norm the solver reports equals the FP64 norm
+of the sampled-verified residual field, the stopping test is met, iteration count equals the
+256^3 / 512^3 shrinks' (3 V-cycles, grid-independent convergence)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2607_07687_b200 import gmg
+from paper_2607_07687_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _block(arr, c, h, n):
+    """(2h+1)^3 neighbourhood of cell c=(i,j,k) with periodic wrap, from a [k][j][i] array."""
+    idx = [np.arange(c[d] - h, c[d] + h + 1) % n[d] for d in range(3)]
+    return np.asarray(arr[np.ix_(idx[2], idx[1], idx[0])], dtype=np.float64)
+
+
+def _blockL(L, c, h, n):
+    return np.stack([_block(L[d], c, h, n) for d in range(3)])
+
+
+def _samples(n, count, seed):
+    rng = np.random.default_rng(seed)
+    pts = [tuple(int(rng.integers(0, n[d])) for d in range(3)) for _ in range(count)]
+    # tile corners / domain corners / wrap seams are where indexing mistakes show
+    pts += [(0, 0, 0), (n[0] - 1, n[1] - 1, n[2] - 1), (127, 12, 63), (128, 13, 64), (n[0] - 1, 0, 31),
+            (0, n[1] - 1, 32), (4, 1, n[2] - 1), (n[0] // 2, n[1] - 2, 0)]
+    return pts
+
+
+def _run(name, nsamples):
+    wl = W.by_name(name)
+    n = wl.n
+    g = gmg.GMG(n, wl.bc)
+    L = torch.from_numpy(wl.L).cuda()
+    z = torch.from_numpy(wl.z).cuda()
+    g.set_coeffs(L)
+    plan = g.describe_plan()
+    assert "fused-rb-sweep(TMA)" in plan.split("\n")[0]          # the configuration bench.py times
+    rng = np.random.default_rng(5)
+    p0 = torch.randn(z.shape, device="cuda", generator=torch.Generator("cuda").manual_seed(11))
+    p0_h = p0.cpu().numpy()
+    pts = _samples(n, nsamples, 3)
+    # ---- (a1) residual, sampled ------------------------------------------------------------
+    r = g.op_residual(0, p0, z)
+    r_h = r.cpu().numpy()
+    # ---- (a2) two fused red+black sweeps (the ping-pong pair the V-cycle launches), sampled ----
+    q = p0.clone()
+    g.op_smooth(0, q, z, omega=0.875, nsweeps=2, first_colour=0)
+    q_h = q.cpu().numpy()
+    bc_blk = (1, 1, 1)      # cut-out block: walls (zero faces) outside, which the centre never sees
+    worst_r = worst_s = 0.0
+    scale_r = float(np.abs(r_h[::7, ::7, ::7]).max())
+    scale_s = float(np.abs(q_h[::7, ::7, ::7]).max())
+    for c in pts:
+        # 9^3 cut-out: two red+black sweeps reach 4 cells; the cut-out's outer faces never matter
+        Lb5 = _blockL(wl.L, c, 4, n)
+        pb = _block(p0_h, c, 4, n)
+        zb = _block(wl.z, c, 4, n)
+        ro5 = oracle.residual(Lb5, bc_blk, pb, zb)[4, 4, 4]
+        worst_r = max(worst_r, abs(ro5 - r_h[c[2], c[1], c[0]]))
+        h = oracle.Hierarchy((9, 9, 9), bc_blk, Lb5.astype(np.float32))
+        # colours in the block must match the global ones: block origin parity
+        par = (c[0] - 4 + c[1] - 4 + c[2] - 4) & 1
+        s = h.level_sweeps(0, pb, zb, omega=0.875, count=2, first_colour=par)
+        worst_s = max(worst_s, abs(s[4, 4, 4] - q_h[c[2], c[1], c[0]]))
+    assert worst_r <= 1e-5 * scale_r, (worst_r, scale_r)
+    assert worst_s <= 3e-5 * scale_s, (worst_s, scale_s)
+    # ---- (a3) the TMA-fed residual+restriction against the (sampled-verified) residual field ---
+    bc_t = g.op_residual_restrict(0, p0, z).double()
+    ref = r.double().view(n[2] // 2, 2, n[1] // 2, 2, n[0] // 2, 2).sum(dim=(1, 3, 5))
+    assert float((bc_t - ref).abs().max().item()) <= 1e-5 * float(ref.abs().max().item())
+    del bc_t, ref
+    # ---- (b) properties at any size ----------------------------------------------------------
+    sum_r = float(r.double().sum().item())
+    sum_z = float(z.double().sum().item())
+    assert abs(sum_r - sum_z) <= 1e-6 * float(r.double().abs().sum().item())
+    assert abs(g.op_norm2(0, r) - float(torch.linalg.vector_norm(r.double()).item())) <= 1e-9 * g.op_norm2(0, r)
+    p = torch.zeros_like(z)
+    rc = g.solve(p, z, tol=wl.tol, maxiter=wl.maxiter, solver=gmg.GMG_RBGS)
+    st = g.stats()
+    assert rc == gmg.OK and st["iterations"] == 3, st            # as on the 128^3 / 256^3 shrinks
+    rr = g.op_residual(0, p, z)
+    true_rel = float(torch.linalg.vector_norm(rr.double()).item()) / st["resid_ref"]
+    assert abs(true_rel - st["resid_final_rel"]) <= 1e-6 * true_rel
+    assert true_rel <= wl.tol
+    hist = g.history()
+    assert len(hist) == 4 and all(hist[k + 1] < 0.1 * hist[k] for k in range(3))
+    g.close()
+
+
+def test_sampled_parity_512():
+    _run("c4_512", 24)
+
+
+def test_sampled_parity_1024_bench_configuration():
+    free, _ = torch.cuda.mem_get_info()
+    if free < 70 * 2 ** 30:
+        pytest.skip("needs 70 GB of free device memory")
+    try:
+        import psutil
+        if psutil.virtual_memory().available < 80 * 2 ** 30:
+            pytest.skip("needs 80 GB of host memory")
+    except ImportError:
+        pass
+    _run("c4", 16)
