@@ -118,9 +118,10 @@ static void build_levels(gmg_ctx* c) {
     size_t cells = 0;
     for (int l = c->nlev - 1; l >= 0; --l) {
         cells += (size_t)c->g[l].N;
-        if (cells * 5 * sizeof(float) > cap || c->nlev - l > GMG_TAIL_MAX_LEVELS) break;
+        // 8 floats per cell (six face weights, p, b); at most 6 cells of a level per thread
+        if (cells * 8 * sizeof(float) > cap || c->g[l].N > 6144 || c->nlev - l > GMG_TAIL_MAX_LEVELS) break;
         c->tail_start = l;
-        c->tail_smem = cells * 5 * sizeof(float);
+        c->tail_smem = cells * 8 * sizeof(float);
     }
     for (int l = 0; l < c->nlev; ++l) {
         c->fast_sweep[l] = c->prm.fast_path && gmgf::sweep_supported(c->g[l]);
