@@ -1,5 +1,5 @@
 // kernels_sweep.cu -- k_rb_sweep_bulk: the fused red+black Gauss-Seidel sweep of the big levels
-// (PAPER.md:43 S3.1; readings O3, O8; prolongation O6 fused on request), fed by the
+// (PAPER.md:43 S3.1; readings O3, O8), fed by the
 // Tensor Memory Accelerator (cp.async.bulk.tensor + mbarrier, SASS UTMALDG) instead of register
 // loads.
 //
@@ -33,16 +33,15 @@ static int zmin_env() {
     return v;
 }
 
-template <int TY_, int PD_, int PL_>
+template <int TY_, int PD_>
 struct BulkCfg {
     static constexpr int TX = 128, TY = TY_, PD = PD_;
-    static constexpr int PL = PL_;               // extra lead of the p planes (prolongation fix-up)
     static constexpr int LPR = 32;
     static constexpr int ROWS = TY + 2;          // rows running phase B (tile + ring 1)
     static constexpr int MAIN = LPR * ROWS;
     static constexpr int THREADS = MAIN + 32;    // + one edge warp
     static constexpr int SH = TY + 4;            // rows of a p plane (halo 2)
-    static constexpr int NP = PD + 4 + PL;       // ring depths (slot-reuse argument: DESIGN.md S6)
+    static constexpr int NP = PD + 4;            // ring depths (slot-reuse argument: DESIGN.md S6)
     static constexpr int NZ = PD + 1;
     static constexpr int NC = PD;
     static constexpr int NB = PD + 1;            // mbarriers of the step groups
@@ -62,9 +61,7 @@ struct BulkCfg {
     static constexpr size_t SMEM = (size_t)FLOATS * sizeof(float) + 16 * sizeof(uint64_t) + (size_t)NROWCOPY * 16;
     static constexpr uint32_t STEP_BYTES =
         (uint32_t)(SH * TX + 2 * SH * 4 + 3 * ROWS * TX + (ROWS + 1) * TX) * 4u;
-    static constexpr uint32_t PRO_BYTES = (uint32_t)((2 + PL) * (SH * TX + 2 * SH * 4) + ROWS * TX) * 4u;
-    static constexpr int AGROUPS = (LPR + 2) * SH;      // float4 groups of a p plane (prolong fix-up)
-    static constexpr int APER = (AGROUPS + THREADS - 1) / THREADS;
+    static constexpr uint32_t PRO_BYTES = (uint32_t)(2 * (SH * TX + 2 * SH * 4) + ROWS * TX) * 4u;
     static_assert(2 * ROWS <= 32 && NB <= 8 && THREADS / 32 >= 7, "tile shape");
 };
 
@@ -75,7 +72,6 @@ struct BulkArgs {
     float* dst;
     const float* b;
     const float* omega;
-    const float* e_c;
     int first_colour;
     int zchunk;
     int tiles_x, tiles_y;
@@ -99,7 +95,7 @@ __device__ __forceinline__ float4 update_pair_full(float xm, float4 own, float x
     return update_pair<S>(xm, own, xp, ym, yp, zm, zp, s, c.lz, omega);
 }
 
-template <class C, bool PROLONG>
+template <class C>
 __global__ void __launch_bounds__(C::THREADS, 1)
 k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     extern __shared__ __align__(1024) float sm[];  // no static shared memory: base is 1 KB aligned
@@ -176,7 +172,7 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         uint64_t* bar = bars + ((v - (z0 - 1)) % C::NB);
         if (tid == 0) mbar_expect_tx(bar, C::STEP_BYTES);
         const int gz0 = wrap1(v, nz), gz1 = wrap1(v + 1, nz);
-        const int vp = v + 1 + C::PL, gzv = wrapi(vp, nz);   // the p plane of this group
+        const int vp = v + 1, gzv = gz1;                     // the p plane of this group
         if (y_inside) {
             switch (warp_id) {
                 case 0: tma_load_3d(slotP(vp), &maps.p_main, x0, y0 - 2, gzv, bar); break;
@@ -197,57 +193,6 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         }
     };
 
-    // ---- prolongation fix-up (PROLONG): p += P e_c on a freshly landed plane --------------------
-    int f_soff[C::APER], f_coff[C::APER];
-    const int ncx = nx / g.c[0], ncy = ny / g.c[1];
-    if (PROLONG) {
-#pragma unroll
-        for (int i = 0; i < C::APER; ++i) {
-            const int e = tid + i * C::THREADS;
-            if (e < C::AGROUPS) {
-                const int r = e / (C::LPR + 2), gc = e % (C::LPR + 2);
-                const int x = wrapi(x0 - 4 + 4 * gc, nx), y = wrapi(y0 + r - 2, ny);
-                f_soff[i] = gc == 0 ? C::P_HL + r * 4 : gc == C::LPR + 1 ? C::P_HR + r * 4 : r * C::TX + 4 * (gc - 1);
-                f_coff[i] = (y / g.c[1]) * ncx + x / g.c[0];
-            } else {
-                f_soff[i] = -1;
-                f_coff[i] = 0;
-            }
-        }
-    }
-    struct EReg { float4 e[C::APER]; };
-    const int czs = g.c[2] - 1;                 // coarse plane = fine plane >> czs
-    const int cplane = ncx * ncy;
-    auto fix_fetch_at = [&](int gzf, EReg& r) {   // coarse values for (wrapped) fine plane gzf
-        const float* eb = a.e_c + (size_t)(gzf >> czs) * cplane;
-#pragma unroll
-        for (int i = 0; i < C::APER; ++i) {
-            if (f_soff[i] >= 0) {
-                if (g.c[0] == 2) {
-                    const float2 e2 = __ldg(reinterpret_cast<const float2*>(eb + f_coff[i]));
-                    r.e[i] = make_float4(e2.x, e2.x, e2.y, e2.y);
-                } else {
-                    r.e[i] = ldg4(eb + f_coff[i]);
-                }
-            }
-        }
-    };
-    auto fix_apply_at = [&](float* P, const EReg& r) {  // p += P e_c in the shared-memory plane P
-#pragma unroll
-        for (int i = 0; i < C::APER; ++i) {
-            if (f_soff[i] >= 0) {
-                float4 val = lds4(P + f_soff[i]);
-                val.x += r.e[i].x; val.y += r.e[i].y; val.z += r.e[i].z; val.w += r.e[i].w;
-                *reinterpret_cast<float4*>(P + f_soff[i]) = val;
-            }
-        }
-    };
-    auto fix_plane = [&](int v) {
-        EReg r;
-        fix_fetch_at(wrapi(v, nz), r);
-        fix_apply_at(slotP(v), r);
-    };
-
     // ---- prologue: barriers; p(z0-2), p(z0-1), Lz(z0-1); the first PD step groups --------------
     if (tid == 0) {
         for (int i = 0; i <= C::NB; ++i) mbar_init(bars + i, 1);
@@ -263,25 +208,21 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
             if (y_inside) {
                 // planes z0-2 .. z0-1+PL: three boxes each, one per warp; then Lz(z0-1)
                 const int pl = warp_id / 3, k = warp_id % 3;
-                if (pl < 2 + C::PL) {
+                if (pl < 2) {
                     const int v = z0 - 2 + pl, gv = wrapi(v, nz);
                     if (k == 0) tma_load_3d(slotP(v), &maps.p_main, x0, y0 - 2, gv, bar);
                     else if (k == 1) tma_load_3d(slotP(v) + C::P_HL, &maps.p_halo, xL, y0 - 2, gv, bar);
                     else tma_load_3d(slotP(v) + C::P_HR, &maps.p_halo, xR, y0 - 2, gv, bar);
-                } else if (warp_id == 3 * (2 + C::PL)) {
+                } else if (warp_id == 6) {
                     tma_load_3d(slotLz(z0 - 1), &maps.lz, x0, y0 - 1, gb, bar);
                 }
             } else {
-                for (int pl = 0; pl < 2 + C::PL; ++pl) copy_p_rows(z0 - 2 + pl, bar);
+                for (int pl = 0; pl < 2; ++pl) copy_p_rows(z0 - 2 + pl, bar);
                 copy_c_rows(1, slotLz(z0 - 1), (size_t)gb * plane, bar);
             }
         }
         for (int v = z0 - 1; v < z0 - 1 + C::PD && v <= z1; ++v) issue_step(v);
         mbar_wait(bar, 0);
-        if (PROLONG) {
-            for (int pl = 0; pl < 2 + C::PL; ++pl) fix_plane(z0 - 2 + pl);
-            __syncthreads();  // B(z0-1) reads groups other threads fixed
-        }
     }
 
     // ring cursors of step u (advanced once per step; no modulo in the loop)
@@ -291,8 +232,6 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     float* Pm1 = P_beg;                             // plane u-1
     float* P0 = P_beg + C::P_PLANE;                 // plane u
     float* Pp1 = P_beg + 2 * C::P_PLANE;            // plane u+1
-    float* Pp2 = P_beg + 3 * C::P_PLANE;            // plane u+2 (prolongation fix-up target)
-    int gzf = wrapi(z0 - 1 + 1 + C::PL, nz);        // wrapped index of plane u+1+PL
     const float* Z0 = Z_beg;                        // Lz plane u
     const float* Z1 = Z_beg + C::C_PLANE;           // Lz plane u+1
     int ic = 0;                                     // slot of Lx / Ly / b plane u
@@ -301,10 +240,8 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     int gz = wrap1(z0 - 1, nz);                     // wrapped plane index of u
     auto advance = [&]() {
         Pm2 = Pm1; Pm1 = P0; P0 = Pp1;
-        Pp1 = Pp2;
-        Pp2 += C::P_PLANE;
-        if (Pp2 == P_beg + C::NP * C::P_PLANE) Pp2 = P_beg;
-        if (++gzf == nz) gzf = 0;
+        Pp1 += C::P_PLANE;
+        if (Pp1 == P_beg + C::NP * C::P_PLANE) Pp1 = P_beg;
         Z0 = Z1;
         Z1 += C::C_PLANE;
         if (Z1 == Z_beg + C::NZ * C::C_PLANE) Z1 = Z_beg;
@@ -351,9 +288,6 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         // Sc = set of plane u, read from shared memory here.  The caller alternates the two
         // register sets, so nothing is copied between steps.
         auto step = [&](int u, const CFull& Sp, CFull& Sc) {
-            EReg er;
-            const bool do_fix = PROLONG && (u + 1 + C::PL <= z1 + 1);
-            if (do_fix) fix_fetch_at(gzf, er);   // latency hidden behind the wait and B(u)
             mbar_wait(bars + kb, kpar);
             const int gzp = (gz + 1 == nz) ? 0 : gz + 1;
             {   // coefficient set of plane u: shared memory -> registers, wall faces zeroed
@@ -382,9 +316,6 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
                 const float4 nw = phase(Pm1, P0, Pp1, sel, Sc);
                 *reinterpret_cast<float4*>(P0 + p_off) = nw;
             }
-            // prolongation fix-up of the plane that landed with this step's group: it is first read
-            // after the barrier below (by B(u+1), as the plane above)
-            if (do_fix) fix_apply_at(C::PL ? Pp2 : Pp1, er);
             fence_async_smem();  // order this thread's smem writes before later TMA overwrites
             cta_sync();
             if (u + C::PD <= z1) issue_step(u + C::PD);
@@ -438,9 +369,6 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         int ecol = (xs + eyl + (z0 - 1)) & 1;  // colour of the edge cell in plane u
         for (int u = z0 - 1; u <= z1; ++u) {
             if (u + 1 <= z1) fetch_e((gz + 1 == nz) ? 0 : gz + 1, En);
-            EReg er;
-            const bool do_fix = PROLONG && (u + 1 + C::PL <= z1 + 1);
-            if (do_fix) fix_fetch_at(gzf, er);
             mbar_wait(bars + kb, kpar);
             if (e_act && ecol == fc) {
                 const float pc = P0[pc_off];
@@ -450,7 +378,6 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
                 P0[pc_off] = relax(pc, Ec.b, Ap,
                                    diag6(Ec.wxl, Ec.wxh, Ec.wyl, Ec.wyh, Ec.wzl, Ec.wzh), omega);
             }
-            if (do_fix) fix_apply_at(C::PL ? Pp2 : Pp1, er);
             fence_async_smem();
             cta_sync();
             if (u + C::PD <= z1) issue_step(u + C::PD);
@@ -467,8 +394,7 @@ void rb_sweep_v2(const LevelGeom& g, const float* L, const float* src, float* ds
                  const float* omega, int first_colour, const float* e_c, cudaStream_t s);
 int configure_v2();
 
-using Bulk = BulkCfg<13, 3, 0>;
-using BulkP = BulkCfg<13, 3, 1>;   // prolongation fused: p planes one step further ahead
+using Bulk = BulkCfg<13, 3>;
 
 static int env_int2(const char* name, int dflt) {
     const char* v = getenv(name);
@@ -525,7 +451,8 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
     static const int use_bulk = env_int2("GMG_BULK", 1);
     BulkMaps maps;
     const size_t N = (size_t)g.N;
-    bool ok = use_bulk && allow_tma && bulk_supported(g);
+    // the caller applies the prolongation as its own pass in front of this kernel (e_c == nullptr)
+    bool ok = use_bulk && allow_tma && !e_c && bulk_supported(g);
     ok = ok && tensor_map(src, g, Bulk::TX, Bulk::SH, &maps.p_main);
     ok = ok && tensor_map(src, g, 4, Bulk::SH, &maps.p_halo);
     ok = ok && tensor_map(L + 2 * N, g, Bulk::TX, Bulk::ROWS, &maps.lz);
@@ -537,7 +464,7 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
         return;
     }
     BulkArgs a;
-    a.g = g; a.L = L; a.src = src; a.dst = dst; a.b = b; a.omega = omega; a.e_c = e_c;
+    a.g = g; a.L = L; a.src = src; a.dst = dst; a.b = b; a.omega = omega;
     a.first_colour = first_colour;
     static const int dbg_env = env_int2("GMG_DBG", 0);
     a.dbg = dbg_env;
@@ -551,14 +478,12 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
     a.zchunk = zchunk;
     const int nzc = (g.n[2] + zchunk - 1) / zchunk;
     const unsigned int grid = (unsigned int)(a.tiles_x * a.tiles_y * nzc);
-    if (e_c) k_rb_sweep_bulk<BulkP, true><<<grid, BulkP::THREADS, BulkP::SMEM, s>>>(a, maps);
-    else k_rb_sweep_bulk<Bulk, false><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+    k_rb_sweep_bulk<Bulk><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
 }
 
 int configure() {
     cudaError_t e = (cudaError_t)configure_v2();
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep_bulk<BulkP, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BulkP::SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
     if (e == cudaSuccess && !g_encode) {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult qres;
