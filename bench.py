@@ -145,6 +145,34 @@ def run_reference(args):
     return 0
 
 
+def solver_table(gmg, W, torch, device, names):
+    """#iterations, final residual, ms and ns/cell of PCG, GMG-PCG and GMG-RBGS per workload
+    (the columns of the paper's Table 1; device-resident, best of 3)."""
+    out = {}
+    for name in names:
+        wl = W.by_name(name)
+        g = gmg.GMG(wl.n, wl.bc, device=str(device))
+        L = torch.from_numpy(wl.L).to(device)
+        z = torch.from_numpy(wl.z).to(device)
+        g.set_coeffs(L)
+        p = torch.zeros_like(z)
+        row = {}
+        for label, solver, cap in (("PCG", gmg.PCG, 5000), ("GMG-PCG", gmg.GMG_PCG, wl.maxiter),
+                                   ("GMG-RBGS", gmg.GMG_RBGS, wl.maxiter)):
+            best = None
+            for _ in range(3):
+                p.zero_()
+                g.set_omega(1.0)
+                g.solve(p, z, tol=wl.tol, maxiter=cap, solver=solver)
+                st = g.stats()
+                best = st["gpu_ms"] if best is None else min(best, st["gpu_ms"])
+            row[label] = {"iterations": st["iterations"], "resid": st["resid_final_rel"], "ms": best,
+                          "ns_per_cell": best * 1e6 / wl.cells}
+        out[name] = row
+        g.close()
+    return out
+
+
 def time_kernel_loop(fn, reps, stream):
     import torch
     e0 = torch.cuda.Event(enable_timing=True)
@@ -268,6 +296,22 @@ def run_ours(args):
                "sample": f"{args.reference_sample} ({swl.n[0]}^3, same recipe as the workload): "
                          f"one full solve, {it} V-cycles, {dt:.1f} s"}
 
+    # ---- the paper's three-way comparison (Table 1's columns) on the small configs ----------
+    table = None
+    if not args.no_table:
+        table = solver_table(gmg, W, torch, device,
+                             ["c0", "c1", "c2", "c3p5", "c3p6"] if N > (1 << 22) else [args.workload])
+        # the big workload itself: GMG-RBGS is the timed step above; GMG-PCG beside it
+        if N > (1 << 22):
+            p.zero_()
+            rc = g.solve(p, z, tol=tol, maxiter=maxiter, solver=gmg.GMG_PCG)
+            st2 = g.stats()
+            table[args.workload] = {
+                "GMG-RBGS": {"iterations": iters[-1], "resid": final["resid_final_rel"],
+                             "ms": final["gpu_ms"], "ns_per_cell": final["gpu_ms"] * 1e6 / N},
+                "GMG-PCG": {"iterations": st2["iterations"], "resid": st2["resid_final_rel"],
+                            "ms": st2["gpu_ms"], "ns_per_cell": st2["gpu_ms"] * 1e6 / N}}
+
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False,
@@ -298,6 +342,7 @@ def run_ours(args):
                 "h2d_bytes_per_step": 8 * N, "d2h_bytes_per_step": 4 * N},
         "gpu_launches": int(launches),
         "clocks": sampler.summary(),
+        "solvers": table,
         "plan": g.describe_plan().strip().split("\n"),
     }
     print(json.dumps(line))
@@ -315,6 +360,7 @@ def main():
     ap.add_argument("--workload", default="c4")
     ap.add_argument("--reference-sample", default="c4_256")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-table", action="store_true", help="skip the three-solver comparison table")
     ap.add_argument("--no-graph", action="store_true",
                     help="plain kernel launches instead of the CUDA-graph WHILE loop (so that ncu "
                          "lists every kernel of the solve)")
