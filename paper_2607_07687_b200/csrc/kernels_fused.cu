@@ -143,12 +143,17 @@ __global__ void __launch_bounds__(C::THREADS, MINB) k_rb_sweep(const SweepArgs a
     };
 
     // ---- prologue: planes z0-2, z0-1, z0 -------------------------------------------------------
+    float4 va[C::APER];  // source plane in flight: loaded during one step, stored during the next
     {
-        float4 v[C::APER];
-        for (int u = z0 - 2; u <= z0; ++u) {
-            load_plane(u, v);
-            store_plane(u, v);
-        }
+        // all four loads are issued before the first store: one memory latency, not four
+        float4 v0[C::APER], v1[C::APER], v2[C::APER];
+        load_plane(z0 - 2, v0);
+        load_plane(z0 - 1, v1);
+        load_plane(z0, v2);
+        if (z0 + 1 <= z1 + 1) load_plane(z0 + 1, va);
+        store_plane(z0 - 2, v0);
+        store_plane(z0 - 1, v1);
+        store_plane(z0, v2);
     }
     cta_sync();
 
@@ -209,18 +214,17 @@ __global__ void __launch_bounds__(C::THREADS, MINB) k_rb_sweep(const SweepArgs a
                                            : update_pair<0>(xm, own, xp, ym, yp, zm, zp, s, lz, omega);
         };
         auto step = [&](int u, CSet& Sp, CSet& Sc, CSet& Sn, float4& lzpp) {
-            float4 va[C::APER];
-            const bool do_a = (u + 2 <= z1 + 1);
             if (u + 1 <= z1) fetch(u + 1, Sn);
-            if (do_a) load_plane(u + 2, va);
             if (a.pf > 0 && u + 1 + a.pf <= z1) prefetch_set(u + 1 + a.pf);
-            if (a.pf > 0 && u + 2 + a.pf <= z1 + 1) prefetch_plane(u + 2 + a.pf);
+            if (a.pf > 0 && u + 3 + a.pf <= z1 + 1) prefetch_plane(u + 3 + a.pf);
             finish(u, Sc);
             {   // B(u): first colour on tile + ring 1, in place in shared memory
                 const float4 nw = phase(u, fc, Sc, Sp.lzh);
                 *reinterpret_cast<float4*>(slot_of(u) + own_off) = nw;
             }
-            if (do_a) store_plane(u + 2, va);
+            // plane u+2 was requested a step ago; plane u+3 has until the next step to arrive
+            if (u + 2 <= z1 + 1) store_plane(u + 2, va);
+            if (u + 3 <= z1 + 1) load_plane(u + 3, va);
             cta_sync();
             if (u - 1 >= z0 && __any_sync(0xffffffffu, row_c)) {  // C(u-1): second colour, tile only
                 const float4 nw = phase(u - 1, fc ^ 1, Sp, lzpp);
@@ -277,11 +281,8 @@ __global__ void __launch_bounds__(C::THREADS, MINB) k_rb_sweep(const SweepArgs a
         fetch_e(z0 - 1, Ec);
         En = Ec;
         for (int u = z0 - 1; u <= z1; ++u) {
-            float4 va[C::APER];
-            const bool do_a = (u + 2 <= z1 + 1);
             if (u + 1 <= z1) fetch_e(u + 1, En);
-            if (do_a) load_plane(u + 2, va);
-            if (a.pf > 0 && u + 2 + a.pf <= z1 + 1) prefetch_plane(u + 2 + a.pf);
+            if (a.pf > 0 && u + 3 + a.pf <= z1 + 1) prefetch_plane(u + 3 + a.pf);
             if (e_act && ((xs + eyl + u) & 1) == fc) {
                 float* P = slot_of(u);
                 const float pc = P[e_off];
@@ -291,7 +292,8 @@ __global__ void __launch_bounds__(C::THREADS, MINB) k_rb_sweep(const SweepArgs a
                 P[e_off] = relax(pc, Ec.b, Ap,
                                  diag6(Ec.wxl, Ec.wxh, Ec.wyl, Ec.wyh, Ec.wzl, Ec.wzh), omega);
             }
-            if (do_a) store_plane(u + 2, va);
+            if (u + 2 <= z1 + 1) store_plane(u + 2, va);
+            if (u + 3 <= z1 + 1) load_plane(u + 3, va);
             cta_sync();
             Ec = En;
         }
