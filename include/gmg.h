@@ -170,6 +170,17 @@ int gmg_op_vcycle(gmg_ctx* ctx, float* p_dev, const float* z_dev, float omega, i
 /* sqrt(sum r^2) of a level-lev array (deterministic two-stage reduction). */
 int gmg_op_norm2(gmg_ctx* ctx, int lev, const float* r_dev, double* out_host, void* stream);
 
+/* -- the steps either side of the solve in a staggered projection step ("predictor +
+ *    corrector steps", one Poisson solve each) -----------------------
+ * u_dev: [3][nz][ny][nx], u[d*N + idx] = velocity on the LOWER d-face of cell idx (like L).
+ * gmg_divergence:  z_I = sum_d [ u_d(I+e_d) - u_d(I) ].  Upper face of the last cell of an axis:
+ *   periodic -> u_d(index 0); Neumann -> wall_hi[d] (host array of 3 floats, NULL = zeros); on a
+ *   Neumann axis u_d(index 0) is the lower-wall value.
+ * gmg_project:  u_d(I) -= L_d(I) * (p_I - p_{I-e_d}) with the coefficients of gmg_set_coeffs
+ *   (Neumann wall faces carry 0 and stay untouched), so that div(u_new) = div(u_old) - A p. */
+int gmg_divergence(gmg_ctx* ctx, const float* u_dev, const float wall_hi[3], float* z_dev, void* stream);
+int gmg_project(gmg_ctx* ctx, float* u_dev, const float* p_dev, void* stream);
+
 /* Names of the kernels a V-cycle launches per level, for profiling notes: writes a
  * NUL-terminated description into buf. */
 int gmg_describe_plan(const gmg_ctx* ctx, char* buf, size_t cap);

@@ -38,6 +38,8 @@ _rule = _sig("gmgo_coarsen_rule", C.c_int, _I3, _I3, C.c_int, C.c_int, _I3)
 _ccoef = _sig("gmgo_coarsen_coeffs", None, _I3, _I3, _dp, _dp)
 _rsum = _sig("gmgo_restrict_sum", None, _I3, _I3, _dp, _dp)
 _padd = _sig("gmgo_prolong_add", None, _I3, _I3, _dp, _dp)
+_div = _sig("gmgo_divergence", None, _I3, _I3, _dp, C.c_double * 3, _dp)
+_proj = _sig("gmgo_project", None, _I3, _I3, _dp, _dp, _dp)
 _hcreate = _sig("gmgo_hier_create", C.c_void_p, _I3, _I3, _fp, C.c_int, C.c_int)
 _hdestroy = _sig("gmgo_hier_destroy", None, C.c_void_p)
 _hnlev = _sig("gmgo_hier_nlev", C.c_int, C.c_void_p)
@@ -139,6 +141,23 @@ def prolong_add(pf, ec, c):
     q = _f64(pf).copy()
     n3, _ = _n_of(q)
     _padd(n3, _I3(*c), _f64(ec), q)
+    return q
+
+
+def divergence(u, bc, wall_hi=(0.0, 0.0, 0.0)):
+    """z_I = sum_d u_d(upper face) - u_d(lower face); u: (3,nz,ny,nx) lower-face velocities."""
+    u = _f64(u)
+    n3, _ = _n_of(u)
+    z = np.empty(u.shape[1:], dtype=np.float64)
+    _div(n3, _I3(*bc), u, (C.c_double * 3)(*[float(v) for v in wall_hi]), z)
+    return z
+
+
+def project(L, bc, p, u):
+    """Returns u - L grad p (new array)."""
+    q = _f64(u).copy()
+    n3, _ = _n_of(q)
+    _proj(n3, _I3(*bc), _f64(L), _f64(p), q)
     return q
 
 

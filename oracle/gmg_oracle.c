@@ -527,3 +527,60 @@ int gmgo_solve_pcg(gmgo_hier *h, int precond, double *p, const double *z, double
     free(r); free(s); free(d); free(q);
     return k;
 }
+
+/* ------------------------------------------------------------------------------------
+ * N1: the two steps either side of the Poisson solve in a
+ * staggered projection step (Fig. 2 "predictor + corrector steps", one solve
+ * each; PAPER.md:9 staggered finite volume).  u is component-major like L: u[d*N + idx] is
+ * the velocity on the LOWER d-face of cell idx.
+ *
+ *   divergence:  z_I = sum_d [ u_d(I+e_d) - u_d(I) ]     (what configs[1..3] hand to the solver)
+ *       upper face of the last cell: periodic -> u_d(index 0); Neumann -> the prescribed
+ *       upper-wall value wall_hi[d].  On a Neumann axis u_d(index 0) is the lower-wall value.
+ *   projection:  u_d(I) -= L_d(I) * (p_I - p_{I-e_d})     (unit spacing; reading O1's face)
+ *       Neumann wall faces carry coefficient 0 (reading O2): untouched.
+ * Identity that ties both to the operator:  div(project(u, p)) = div(u) - A p.
+ * ---------------------------------------------------------------------------------- */
+void gmgo_divergence(const int n[3], const int bc[3], const double *u, const double wall_hi[3],
+                     double *z) {
+    i64 N = ncells(n);
+    for (int k = 0; k < n[2]; ++k)
+        for (int j = 0; j < n[1]; ++j)
+            for (int i = 0; i < n[0]; ++i) {
+                int I[3] = {i, j, k};
+                double s = 0.0;
+                for (int d = 0; d < 3; ++d) {
+                    double lo = u[(i64)d * N + lin(n, i, j, k)];
+                    double hi;
+                    if (I[d] == n[d] - 1) {
+                        if (bc[d] == GMGO_NEUMANN) {
+                            hi = wall_hi[d];
+                        } else {
+                            int J[3] = {i, j, k};
+                            J[d] = 0;
+                            hi = u[(i64)d * N + lin(n, J[0], J[1], J[2])];
+                        }
+                    } else {
+                        int J[3] = {i, j, k};
+                        J[d] = I[d] + 1;
+                        hi = u[(i64)d * N + lin(n, J[0], J[1], J[2])];
+                    }
+                    s += hi - lo;
+                }
+                z[lin(n, i, j, k)] = s;
+            }
+}
+
+void gmgo_project(const int n[3], const int bc[3], const double *L, const double *p, double *u) {
+    i64 N = ncells(n);
+    for (int d = 0; d < 3; ++d)
+        for (int k = 0; k < n[2]; ++k)
+            for (int j = 0; j < n[1]; ++j)
+                for (int i = 0; i < n[0]; ++i) {
+                    int I[3] = {i, j, k};
+                    double w = face_lo(n, bc, L, d, I); /* 0 on a Neumann wall face */
+                    double pm = nb_lo(n, bc, p, d, I);
+                    i64 c = lin(n, i, j, k);
+                    u[(i64)d * N + c] -= w * (p[c] - pm);
+                }
+}

@@ -767,6 +767,30 @@ extern "C" int gmg_op_norm2(gmg_ctx* c, int lev, const float* r, double* out_hos
     return GMG_OK;
 }
 
+// ---- N1: the steps either side of the solve ------------------------------
+extern "C" int gmg_divergence(gmg_ctx* c, const float* u_dev, const float wall_hi[3], float* z_dev,
+                              void* stream) {
+    if (!c) return GMG_EINVAL;
+    if (!u_dev || !z_dev) { SET_ERR(c, "gmg_divergence: null pointer"); return GMG_EINVAL; }
+    cudaStream_t s = (cudaStream_t)stream;
+    const float zero[3] = {0.0f, 0.0f, 0.0f};
+    gmgk::divergence(c->g[0], u_dev, wall_hi ? wall_hi : zero, z_dev, s);
+    CUDA_TRY(c, cudaGetLastError());
+    CUDA_TRY(c, cudaStreamSynchronize(s));
+    return GMG_OK;
+}
+
+extern "C" int gmg_project(gmg_ctx* c, float* u_dev, const float* p_dev, void* stream) {
+    if (!c) return GMG_EINVAL;
+    if (!u_dev || !p_dev) { SET_ERR(c, "gmg_project: null pointer"); return GMG_EINVAL; }
+    if (!c->coeffs_set) { SET_ERR(c, "gmg_project before gmg_set_coeffs"); return GMG_ESTATE; }
+    cudaStream_t s = (cudaStream_t)stream;
+    gmgk::project(c->g[0], c->lv[0].L, p_dev, u_dev, s);
+    CUDA_TRY(c, cudaGetLastError());
+    CUDA_TRY(c, cudaStreamSynchronize(s));
+    return GMG_OK;
+}
+
 extern "C" int gmg_describe_plan(const gmg_ctx* c, char* buf, size_t cap) {
     if (!c || !buf || cap == 0) return GMG_EINVAL;
     size_t off = 0;

@@ -87,6 +87,8 @@ void restrict_sum(const LevelGeom& gf, const float* rf, float* bc, cudaStream_t 
 void residual_restrict(const LevelGeom& gf, const float* L, const float* p, const float* b,
                        float* b_c, float* p_c, cudaStream_t s);
 void fill(float* x, long long N, float v, cudaStream_t s);
+void divergence(const LevelGeom& g, const float* u, const float wall_hi[3], float* z, cudaStream_t s);
+void project(const LevelGeom& g, const float* L, const float* p, float* u, cudaStream_t s);
 void prolong_add(const LevelGeom& gf, const float* e_c, float* p_f, cudaStream_t s);
 void coarsen_coeffs(const LevelGeom& gf, const float* Lf, float* Lc, cudaStream_t s);
 void check_coeffs(const LevelGeom& g, const float* L, ReduceBuf rb, cudaStream_t s);

@@ -135,6 +135,59 @@ void fill(float* x, long long N, float v, cudaStream_t s) {
     k_fill<<<nb, kThreads, 0, s>>>(x, N, v);
 }
 
+
+// ---- N1: the two steps either side of the solve in a staggered projection step
+// ("predictor + corrector steps", one Poisson solve each).  u is component-major like
+// L: u[d*N + idx] = velocity on the LOWER d-face of cell idx.
+// z_I = sum_d [ u_d(I+e_d) - u_d(I) ]; upper face of the last cell: periodic -> u_d(index 0),
+// Neumann -> the prescribed upper-wall value wall_hi[d].
+__global__ void __launch_bounds__(kThreads)
+k_divergence(LevelGeom g, const float* __restrict__ u, float whx, float why, float whz,
+             float* __restrict__ z) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= g.N) return;
+    int i, j, k;
+    unflatten(g, t, i, j, k);
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const long long N = g.N, sy = nx, sz = (long long)nx * ny;
+    const float xh = (i == nx - 1) ? (g.bc[0] ? whx : u[t - (nx - 1)]) : u[t + 1];
+    const float yh = (j == ny - 1) ? (g.bc[1] ? why : u[N + t - sy * (ny - 1)]) : u[N + t + sy];
+    const float zh = (k == nz - 1) ? (g.bc[2] ? whz : u[2 * N + t - sz * (nz - 1)]) : u[2 * N + t + sz];
+    float s = xh - u[t];
+    s += yh - u[N + t];
+    s += zh - u[2 * N + t];
+    z[t] = s;
+}
+
+void divergence(const LevelGeom& g, const float* u, const float wall_hi[3], float* z, cudaStream_t s) {
+    k_divergence<<<blocks_for(g.N), kThreads, 0, s>>>(g, u, wall_hi[0], wall_hi[1], wall_hi[2], z);
+}
+
+// u_d(I) -= L_d(I) * (p_I - p_{I-e_d}); Neumann wall faces carry coefficient 0 (reading O2).
+__global__ void __launch_bounds__(kThreads)
+k_project(LevelGeom g, const float* __restrict__ L, const float* __restrict__ p, float* __restrict__ u) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= g.N) return;
+    int i, j, k;
+    unflatten(g, t, i, j, k);
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const long long N = g.N, sy = nx, sz = (long long)nx * ny;
+    const float pc = p[t];
+    const float wx = (i == 0 && g.bc[0]) ? 0.0f : L[t];
+    const float wy = (j == 0 && g.bc[1]) ? 0.0f : L[N + t];
+    const float wz = (k == 0 && g.bc[2]) ? 0.0f : L[2 * N + t];
+    const float px = p[(i == 0) ? t + (nx - 1) : t - 1];
+    const float py = p[(j == 0) ? t + sy * (ny - 1) : t - sy];
+    const float pz = p[(k == 0) ? t + sz * (nz - 1) : t - sz];
+    u[t] = fmaf(-wx, pc - px, u[t]);
+    u[N + t] = fmaf(-wy, pc - py, u[N + t]);
+    u[2 * N + t] = fmaf(-wz, pc - pz, u[2 * N + t]);
+}
+
+void project(const LevelGeom& g, const float* L, const float* p, float* u, cudaStream_t s) {
+    k_project<<<blocks_for(g.N), kThreads, 0, s>>>(g, L, p, u);
+}
+
 // ---- O5: coefficient coarsening ("anisotropic coarsening operators") -----------
 // L_d^{l+1}(J) = (1/c_d) * sum of the fine L_d over the prod_{e != d} c_e fine lower-d faces
 // tiling the coarse face.  The fine wall plane of a Neumann axis counts as 0 (reading O2).

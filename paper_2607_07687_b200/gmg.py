@@ -76,6 +76,8 @@ SIGNATURES = {
     "gmg_op_prolong": (C.c_int, [_vp, C.c_int, _vp, _vp, _vp]),
     "gmg_op_vcycle": (C.c_int, [_vp, _vp, _vp, C.c_float, C.c_int, _vp]),
     "gmg_op_norm2": (C.c_int, [_vp, C.c_int, _vp, C.POINTER(C.c_double), _vp]),
+    "gmg_divergence": (C.c_int, [_vp, _vp, C.POINTER(C.c_float), _vp, _vp]),
+    "gmg_project": (C.c_int, [_vp, _vp, _vp, _vp]),
     "gmg_describe_plan": (C.c_int, [_vp, C.c_char_p, C.c_size_t]),
 }
 
@@ -288,6 +290,22 @@ class GMG:
         self._check(lib.gmg_op_norm2(self._h, lev, self._vec(r, lev), C.byref(out),
                                      self._stream()))
         return out.value
+
+    def divergence(self, u: torch.Tensor, wall_hi=(0.0, 0.0, 0.0)) -> torch.Tensor:
+        """z = div u; u: (3, nz, ny, nx) lower-face velocities."""
+        assert u.is_cuda and u.dtype == torch.float32 and u.is_contiguous()
+        assert tuple(u.shape) == (3, self.n[2], self.n[1], self.n[0])
+        z = self._new(0)
+        wh = (C.c_float * 3)(*[float(v) for v in wall_hi])
+        self._check(lib.gmg_divergence(self._h, _vp(_ptr(u)), wh, _vp(_ptr(z)), self._stream()))
+        return z
+
+    def project(self, u: torch.Tensor, p: torch.Tensor) -> torch.Tensor:
+        """In place on u: u -= L grad p."""
+        assert u.is_cuda and u.dtype == torch.float32 and u.is_contiguous()
+        assert tuple(u.shape) == (3, self.n[2], self.n[1], self.n[0])
+        self._check(lib.gmg_project(self._h, _vp(_ptr(u)), self._vec(p), self._stream()))
+        return u
 
     def describe_plan(self) -> str:
         buf = C.create_string_buffer(4096)

@@ -273,3 +273,34 @@ def test_solve_host_matches_device_solve():
         assert np.array_equal(ph.numpy().astype(np.float64), p)
     finally:
         g.close()
+
+
+@pytest.mark.parametrize("n,bc", [((128, 16, 16), (0, 0, 0)), ((64, 64, 8), (1, 0, 1))])
+def test_isotropic_vs_anisotropic_coarsening(n, bc):
+    """PAPER.md:47 (S3.2, Fig. 2): with classical isotropic coarsening "the smallest domain
+    dimension limits the number of multigrid levels"; the anisotropic rule keeps coarsening the
+    long directions and needs fewer V-cycles.  Both modes: level shapes and cycle counts match the
+    oracle, and anisotropic never needs more cycles than isotropic."""
+    wl = random_workload(n, bc, seed=77, zero_frac=0.0, blob=False)
+    act = W.active_mask(wl.L, wl.bc)
+    counts = {}
+    for mode, iso in (("aniso", False), ("iso", True)):
+        g = make_gpu(wl, coarsen_mode=gmg.COARSEN_ISO if iso else gmg.COARSEN_ANISO)
+        h = make_oracle(wl, iso=iso)
+        try:
+            assert g.num_levels() == h.nlev
+            for l in range(h.nlev):
+                assert g.level_shape(l) == h.shape(l)
+            rc, p, st, hist = _solve_gpu(g, wl, gmg.GMG_RBGS, 1e-4, 200)
+            ref = h.solve(oracle.GMG_RBGS, wl.z, tol=1e-4, maxiter=200)
+            assert rc == gmg.OK and ref["status"] == 0
+            assert abs(st["iterations"] - ref["iterations"]) <= 1, (mode, st["iterations"], ref["iterations"])
+            if st["iterations"] != ref["iterations"]:
+                h.omega = 1.0
+                ref = h.solve(oracle.GMG_RBGS, wl.z, tol=0.0, maxiter=st["iterations"])
+            assert rel_l2_demeaned(p, ref["p"], act) <= TOL_P
+            counts[mode] = (st["iterations"], g.num_levels())
+        finally:
+            g.close()
+    assert counts["aniso"][1] > counts["iso"][1]          # more levels ...
+    assert counts["aniso"][0] <= counts["iso"][0]         # ... and no more cycles

@@ -290,3 +290,78 @@ def test_pcg_properties_and_ordering():
     assert pcg["status"] == 0 and mg["status"] == 0
     assert mg["iterations"] <= 4 < 20 < pcg["iterations"] < 120
     assert abs(pcg["true_res"] - pcg["history"][-1]) < 1e-8
+
+
+# --------------------------------------------------------------------------------------
+# N1: divergence / projection either side of the solve
+# --------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", BCS)
+def test_projection_identity_ties_to_the_pinned_operator(bc):
+    """div(u - L grad p) = div(u) - A p for any u, p, L, boundary mix (A is pinned above)."""
+    rng = np.random.default_rng(21)
+    n = (6, 4, 8)
+    L = rand_L(rng, n, 0.2)
+    p = rng.standard_normal((n[2], n[1], n[0]))
+    u = rng.standard_normal((3, n[2], n[1], n[0]))
+    wall = (0.3, -0.7, 1.1)
+    lhs = oracle.divergence(oracle.project(L, bc, p, u), bc, wall)
+    rhs = oracle.divergence(u, bc, wall) - oracle.apply_A(L, bc, p)
+    assert np.max(np.abs(lhs - rhs)) < 1e-13
+
+
+def test_divergence_closed_forms():
+    n = (5, 6, 4)
+    bc = (1, 1, 1)
+    # u_d = a_d * (lower-face coordinate): exact divergence a_x + a_y + a_z in every cell, the
+    # upper wall carrying a_d * n_d
+    a = (0.5, -1.25, 2.0)
+    u = np.zeros((3, n[2], n[1], n[0]))
+    u[0] += a[0] * np.arange(n[0])[None, None, :]
+    u[1] += a[1] * np.arange(n[1])[None, :, None]
+    u[2] += a[2] * np.arange(n[2])[:, None, None]
+    z = oracle.divergence(u, bc, tuple(a[d] * n[d] for d in range(3)))
+    assert np.allclose(z, sum(a), atol=1e-14)
+    # discrete Gauss theorem: sum(z) = net outflow through the walls; periodic axes contribute 0
+    rng = np.random.default_rng(2)
+    u = rng.standard_normal((3, n[2], n[1], n[0]))
+    wall = (0.2, 0.4, -0.1)
+    for bcm in [(1, 1, 1), (0 if n[0] % 2 == 0 else 1, 1, 0)]:
+        z = oracle.divergence(u, bcm, wall)
+        flux = 0.0
+        if bcm[0] == 1:
+            flux += wall[0] * n[1] * n[2] - u[0][:, :, 0].sum()
+        if bcm[1] == 1:
+            flux += wall[1] * n[0] * n[2] - u[1][:, 0, :].sum()
+        if bcm[2] == 1:
+            flux += wall[2] * n[0] * n[1] - u[2][0, :, :].sum()
+        assert abs(z.sum() - flux) < 1e-12
+
+
+def test_projection_closed_form_and_wall_faces():
+    n = (6, 4, 4)
+    L = np.ones((3, n[2], n[1], n[0]))
+    p = 0.75 * (np.arange(n[0]) + 0.5)[None, None, :] * np.ones((n[2], n[1], 1))   # slope 0.75 in x
+    u = np.zeros((3, n[2], n[1], n[0]))
+    out = oracle.project(L, (1, 0, 0), p, u)
+    assert np.allclose(out[0][:, :, 1:], -0.75) and np.all(out[0][:, :, 0] == 0.0)   # wall untouched
+    assert np.all(out[1] == 0.0) and np.all(out[2] == 0.0)
+    out = oracle.project(L, (0, 0, 0), p, u)                                          # periodic seam
+    assert np.allclose(out[0][:, :, 0], -(p[0, 0, 0] - p[0, 0, -1]))
+
+
+def test_projected_field_is_divergence_free_after_an_exact_solve():
+    rng = np.random.default_rng(8)
+    n, bc = (8, 8, 8), (1, 0, 1)
+    L = rand_L(rng, n, 0.1)
+    u = rng.standard_normal((3, n[2], n[1], n[0])) * W.effective_L(L, bc)
+    for d in range(3):
+        if bc[d] == 1:
+            sl = [slice(None)] * 3
+            sl[2 - d] = 0
+            u[d][tuple(sl)] = 0.0
+    z = oracle.divergence(u, bc)
+    A = dense_by_faces(n, bc, L)
+    p = np.linalg.lstsq(A, z.ravel(), rcond=None)[0].reshape(z.shape)
+    assert np.linalg.norm(A @ p.ravel() - z.ravel()) < 1e-9 * np.linalg.norm(z)      # z compatible
+    div_after = oracle.divergence(oracle.project(L, bc, p, u), bc)
+    assert np.max(np.abs(div_after)) < 1e-9
