@@ -91,6 +91,18 @@ typedef struct {
     int history_len;        /* entries available through gmg_history (iterations+1) */
 } gmg_stats_t;
 
+/* Level table and workspace size for a grid WITHOUT creating a context (host-only: no CUDA call).
+ * Same rule gmg_create applies (reading O4).  params == NULL: defaults. */
+#define GMG_PLAN_MAX_LEVELS 24
+typedef struct {
+    int levels;
+    int n[GMG_PLAN_MAX_LEVELS][3];  /* extents of each level */
+    int c[GMG_PLAN_MAX_LEVELS][3];  /* coarsening factors to the next level */
+    int tail_start;                 /* first level run inside the single-CTA tail kernel */
+    size_t workspace_bytes;         /* what gmg_workspace_bytes will report */
+} gmg_plan_t;
+int gmg_plan(int nx, int ny, int nz, const int bc[3], const gmg_params_t* params, gmg_plan_t* out);
+
 /* -- life cycle ------------------------------------------------------------------------ */
 
 /* Create a context for an nx*ny*nz grid.  Every n_d >= 2; a periodic axis needs an even

@@ -281,6 +281,31 @@ extern "C" int gmg_set_workspace(gmg_ctx* c, void* ws, size_t bytes) {
     return GMG_OK;
 }
 
+// Host-only planning: no CUDA call, usable (and tested) on a machine without a GPU.
+extern "C" int gmg_plan(int nx, int ny, int nz, const int bc[3], const gmg_params_t* params, gmg_plan_t* out) {
+    if (!bc || !out) return GMG_EINVAL;
+    const int n[3] = {nx, ny, nz};
+    for (int d = 0; d < 3; ++d) {
+        if (n[d] < 2) return GMG_EINVAL;
+        if (bc[d] != GMG_BC_PERIODIC && bc[d] != GMG_BC_NEUMANN) return GMG_EINVAL;
+        if (bc[d] == GMG_BC_PERIODIC && (n[d] & 1)) return GMG_EINVAL;
+    }
+    if ((long long)nx * ny * nz > (1LL << 31) - 1) return GMG_EINVAL;
+    gmg_ctx tmp;
+    for (int d = 0; d < 3; ++d) { tmp.n0[d] = n[d]; tmp.bc[d] = bc[d]; }
+    if (params) tmp.prm = *params; else gmg_default_params(&tmp.prm);
+    if (tmp.prm.n_min < 1) return GMG_EINVAL;
+    memset(tmp.lv, 0, sizeof(tmp.lv));
+    build_levels(&tmp);
+    memset(out, 0, sizeof(*out));
+    out->levels = tmp.nlev;
+    for (int l = 0; l < tmp.nlev; ++l)
+        for (int d = 0; d < 3; ++d) { out->n[l][d] = tmp.g[l].n[d]; out->c[l][d] = tmp.g[l].c[d]; }
+    out->tail_start = tmp.tail_start;
+    out->workspace_bytes = carve(&tmp, nullptr);
+    return GMG_OK;
+}
+
 extern "C" int gmg_num_levels(const gmg_ctx* c) { return c ? c->nlev : GMG_EINVAL; }
 
 extern "C" int gmg_level_shape(const gmg_ctx* c, int lev, int n[3], int cf[3]) {

@@ -49,8 +49,14 @@ class Stats(C.Structure):
 _I3 = C.c_int * 3
 _vp = C.c_void_p
 
+
+class Plan(C.Structure):
+    _fields_ = [("levels", C.c_int), ("n", (C.c_int * 3) * 24), ("c", (C.c_int * 3) * 24),
+                ("tail_start", C.c_int), ("workspace_bytes", C.c_size_t)]
+
 # name -> (restype, argtypes); every symbol include/gmg.h declares
 SIGNATURES = {
+    "gmg_plan": (C.c_int, [C.c_int, C.c_int, C.c_int, _I3, C.POINTER(Params), C.POINTER(Plan)]),
     "gmg_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, _I3]),
     "gmg_destroy": (None, [_vp]),
     "gmg_last_error": (C.c_char_p, [_vp]),
@@ -96,6 +102,21 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
 
 
 lib = load_library()
+
+
+def plan(n, bc, **params):
+    """Host-only level table: (shapes, factors, tail_start, workspace_bytes).  No GPU needed."""
+    prm = Params()
+    lib.gmg_default_params(C.byref(prm))
+    for k, v in params.items():
+        setattr(prm, k, v)
+    out = Plan()
+    rc = lib.gmg_plan(int(n[0]), int(n[1]), int(n[2]), _I3(*[int(b) for b in bc]), C.byref(prm), C.byref(out))
+    if rc != OK:
+        raise ValueError(f"gmg_plan rejected n={tuple(n)} bc={tuple(bc)} (code {rc})")
+    shapes = [tuple(out.n[l]) for l in range(out.levels)]
+    factors = [tuple(out.c[l]) for l in range(out.levels)]
+    return shapes, factors, out.tail_start, out.workspace_bytes
 
 
 class GMGError(RuntimeError):

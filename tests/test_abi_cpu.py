@@ -80,3 +80,36 @@ def test_product_path_never_imports_the_oracle():
                 txt = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import oracle|from oracle)", txt, flags=re.M), f
                 assert "gmg_oracle" not in txt and "libgmg_oracle" not in txt, f
+
+
+# ---- host logic of the library, no GPU: level table (reading O4), tail choice, workspace size ----
+def test_library_level_table_matches_golden_and_oracle(libpath):
+    import oracle
+    from paper_2607_07687_b200 import gmg
+    gold = os.path.join(ROOT, "tests", "golden", "level_shapes.txt")
+    for line in open(gold):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, bc, shapes = [s.strip() for s in line.split("|")]
+        bc = tuple(int(x) for x in bc.split())
+        shapes = [tuple(int(x) for x in s.split("x")) for s in shapes.split()]
+        got, factors, tail, ws = gmg.plan(shapes[0], bc)
+        assert got == shapes, name
+        assert factors[-1] == (1, 1, 1)
+        for l in range(len(shapes) - 1):
+            assert tuple(a // f for a, f in zip(shapes[l], factors[l])) == shapes[l + 1]
+        # the tail is a suffix whose 8 floats per cell fit 200 KB of shared memory
+        cells = sum(s[0] * s[1] * s[2] for s in shapes[tail:])
+        assert tail < len(shapes) and cells * 32 <= 200 * 1024
+        assert tail == 0 or (cells + shapes[tail - 1][0] * shapes[tail - 1][1] * shapes[tail - 1][2]) * 32 > 200 * 1024
+        # workspace: coarse levels (L, p, b, q) + level-0 q + 6 fine vectors, each 256-byte aligned
+        N = [s[0] * s[1] * s[2] for s in shapes]
+        lower = 4 * (N[0] + 6 * N[0] + sum(6 * v for v in N[1:]))
+        assert lower <= ws <= lower + 256 * (6 * len(N) + 8)
+    # agreement with the oracle's rule on odd / mixed cases, both coarsening modes
+    for n, bc in [((20, 20, 20), (1, 0, 0)), ((36, 20, 6), (0, 1, 0)), ((64, 4, 4), (1, 0, 0)), ((15, 9, 7), (1, 1, 1))]:
+        for iso in (False, True):
+            got = gmg.plan(n, bc, coarsen_mode=gmg.COARSEN_ISO if iso else gmg.COARSEN_ANISO)[0]
+            assert got == oracle.level_shapes(n, bc, iso=iso), (n, bc, iso)
+    with pytest.raises(ValueError):
+        gmg.plan((31, 32, 16), (0, 0, 0))

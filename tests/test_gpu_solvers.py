@@ -304,3 +304,47 @@ def test_isotropic_vs_anisotropic_coarsening(n, bc):
             g.close()
     assert counts["aniso"][1] > counts["iso"][1]          # more levels ...
     assert counts["aniso"][0] <= counts["iso"][0]         # ... and no more cycles
+
+
+def test_non_default_stream_and_two_contexts():
+    """Work is enqueued on the caller's stream; contexts are independent."""
+    wl_a, wl_b = W.config3(5), W.config0()
+    ga, gb = make_gpu(wl_a), make_gpu(wl_b)
+    try:
+        ref_a = _solve_gpu(ga, wl_a, gmg.GMG_RBGS, 1e-4, 50)
+        ref_b = _solve_gpu(gb, wl_b, gmg.GMG_RBGS, 1e-4, 50)
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            za, zb = dev(wl_a.z), dev(wl_b.z)
+            pa = torch.zeros_like(za)
+            pb = torch.zeros_like(zb)
+            ga.set_omega(1.0)
+            gb.set_omega(1.0)
+            # interleave the two contexts on a side stream
+            rc_b = gb.solve(pb, zb, tol=1e-4, maxiter=50)
+            rc_a = ga.solve(pa, za, tol=1e-4, maxiter=50)
+        s.synchronize()
+        assert rc_a == gmg.OK and rc_b == gmg.OK
+        assert np.array_equal(host(pa), ref_a[1]) and np.array_equal(host(pb), ref_b[1])
+        assert ga.stats()["iterations"] == ref_a[2]["iterations"]
+    finally:
+        ga.close()
+        gb.close()
+
+
+def test_workspace_too_small_and_misaligned_are_rejected():
+    import ctypes as C
+    wl = W.config0()
+    h = C.c_void_p()
+    I3 = C.c_int * 3
+    assert gmg.lib.gmg_create(C.byref(h), *wl.n, I3(*wl.bc)) == gmg.OK
+    try:
+        need = gmg.lib.gmg_workspace_bytes(h)
+        buf = torch.empty(need + 512, dtype=torch.uint8, device="cuda")
+        base = (buf.data_ptr() + 255) // 256 * 256
+        assert gmg.lib.gmg_set_workspace(h, C.c_void_p(base), need - 1) == gmg.ENOMEM
+        assert gmg.lib.gmg_set_workspace(h, C.c_void_p(base + 4), need) == gmg.EINVAL
+        assert gmg.lib.gmg_set_workspace(h, C.c_void_p(base), need) == gmg.OK
+        assert need == gmg.plan(wl.n, wl.bc)[3]
+    finally:
+        gmg.lib.gmg_destroy(h)
