@@ -23,6 +23,8 @@ void residual_restrict(const LevelGeom& g, const float* L, const float* p, const
                        float* b_c, float* p_c, int allow_tma, cudaStream_t s);
 void residual_norm2(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
                     int slot, int allow_tma, cudaStream_t s);
+bool residual_and_ref_norm2_bulk(const LevelGeom& g, const float* L, const float* p, const float* b,
+                                 ReduceBuf rb, int slot_rr, int slot_ref, cudaStream_t s);
 void prolong_add4(const LevelGeom& g, const float* e_c, float* p_f, cudaStream_t s);
 bool tma_shape_ok(const LevelGeom& g);
 int configure();
@@ -465,10 +467,17 @@ static void level0_residual_norm2(gmg_ctx* c, const float* p, const float* z, cu
 
 // GMG-RBGS (readings O8, O9): pre = reference norm + initial residual norm + loop entry test.
 static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
-    gmgk::active_norm2(c->g[0], c->lv[0].L, z, rbuf(c), RED_RREF, s);
-    level0_residual_norm2(c, p, z, s);
+    // reference norm ||z|| over active cells and initial residual norm: one fused pass on big levels
+    if (c->prm.fast_path && c->tma_ok[0] &&
+        gmgf::residual_and_ref_norm2_bulk(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, RED_RREF, s)) {
+        c->n_launch += 1;
+    } else {
+        gmgk::active_norm2(c->g[0], c->lv[0].L, z, rbuf(c), RED_RREF, s);
+        level0_residual_norm2(c, p, z, s);
+        c->n_launch += 2;
+    }
     gmgk::ctl_begin(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
-    c->n_launch += 3;
+    c->n_launch += 1;
 }
 static void rbgs_body(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
     enqueue_vcycle(c, p, z, &c->sc->omega_f, 0, s);
@@ -675,7 +684,7 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
     st.kernel_launches = launches;
     st.history_len = it + 1;
     const double N0 = (double)c->g[0].N;
-    if (solver == GMG_GMG_RBGS) st.bytes_algorithmic = 36.0 * N0 + it * vcycle_bytes(c, true);
+    if (solver == GMG_GMG_RBGS) st.bytes_algorithmic = 20.0 * N0 + it * vcycle_bytes(c, true);  // loop entry: one pass over p, z, L
     else if (solver == GMG_PCG) st.bytes_algorithmic = 60.0 * N0 + it * 64.0 * N0;
     else st.bytes_algorithmic = 60.0 * N0 + it * (vcycle_bytes(c, false) + 52.0 * N0);
     if (h.status == GMG_EBREAKDOWN) SET_ERR(c, "PCG breakdown: d.q == 0 at iteration %d", it);

@@ -58,7 +58,7 @@ struct ResBulkArgs {
     float* b_c;
     float* p_c;
     ReduceBuf rb;
-    int slot;
+    int slot, slot2;
     int zchunk;
     int tiles_x, tiles_y;
 };
@@ -209,7 +209,7 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
         lxhA_pf = __ldg(lxhA_row + (size_t)gz * plane);
         lxhB_pf = __ldg(lxhB_row + (size_t)gz * plane);
     }
-    double acc = 0.0;                               // MODE 1
+    double acc = 0.0, acc_b = 0.0;                  // MODE 1, 2: sum r^2 (and sum b^2 over active cells)
     float zacc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};  // MODE 0: even-plane partial sums
 
     auto store_coarse = [&](const float* v, int cyi, int czi) {  // one coarse row segment of this thread
@@ -286,9 +286,21 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
             rB[2] = (diag6(lxB.z, lxB.w, lyB.z, lyC.z, lzB.z, lzhB.z) != 0.0f) ? bB.z - B2 : 0.0f;
             rB[3] = (diag6(lxB.w, lxhB, lyB.w, lyC.w, lzB.w, lzhB.w) != 0.0f) ? bB.w - B3 : 0.0f;
         }
-        if (MODE == 1) {
+        if (MODE >= 1) {
             if (vA) acc += ((double)rA[0] * rA[0] + (double)rA[1] * rA[1]) + ((double)rA[2] * rA[2] + (double)rA[3] * rA[3]);
             if (vB) acc += ((double)rB[0] * rB[0] + (double)rB[1] * rB[1]) + ((double)rB[2] * rB[2] + (double)rB[3] * rB[3]);
+            if (MODE == 2) {  // reference norm of the solve loop: b^2 over ACTIVE cells (reading O9)
+                const float a0 = (diag6(lxA.x, lxA.y, lyA.x, lyB.x, lzA.x, lzhA.x) != 0.0f) ? bA.x : 0.0f;
+                const float a1 = (diag6(lxA.y, lxA.z, lyA.y, lyB.y, lzA.y, lzhA.y) != 0.0f) ? bA.y : 0.0f;
+                const float a2 = (diag6(lxA.z, lxA.w, lyA.z, lyB.z, lzA.z, lzhA.z) != 0.0f) ? bA.z : 0.0f;
+                const float a3 = (diag6(lxA.w, lxhA, lyA.w, lyB.w, lzA.w, lzhA.w) != 0.0f) ? bA.w : 0.0f;
+                const float b0 = (diag6(lxB.x, lxB.y, lyB.x, lyC.x, lzB.x, lzhB.x) != 0.0f) ? bB.x : 0.0f;
+                const float b1 = (diag6(lxB.y, lxB.z, lyB.y, lyC.y, lzB.y, lzhB.y) != 0.0f) ? bB.y : 0.0f;
+                const float b2 = (diag6(lxB.z, lxB.w, lyB.z, lyC.z, lzB.z, lzhB.z) != 0.0f) ? bB.z : 0.0f;
+                const float b3 = (diag6(lxB.w, lxhB, lyB.w, lyC.w, lzB.w, lzhB.w) != 0.0f) ? bB.w : 0.0f;
+                if (vA) acc_b += ((double)a0 * a0 + (double)a1 * a1) + ((double)a2 * a2 + (double)a3 * a3);
+                if (vB) acc_b += ((double)b0 * b0 + (double)b1 * b1) + ((double)b2 * b2 + (double)b3 * b3);
+            }
         } else {
             // x pairs, then y pairs, then z pairs (stencil.cuh restrict_tree order)
             float cur[8];
@@ -340,6 +352,7 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
         if (++gz == nz) gz = 0;
     }
     if (MODE == 1) finish_reduction(acc, 0.0, false, a.rb, a.slot, 0);
+    if (MODE == 2) finish_reduction(acc, acc_b, true, a.rb, a.slot, a.slot2);
 }
 
 // ---- launchers ------------------------------------------------------------------------------
@@ -367,7 +380,7 @@ static bool launch_res_bulk(ResBulkArgs& a, cudaStream_t s) {
            (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) < 148 * 4)
         zchunk /= 2;
     // the deterministic reduction has a bounded number of block partials
-    while (MODE == 1 && (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) > GMG_REDUCE_MAX_BLOCKS)
+    while (MODE >= 1 && (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) > GMG_REDUCE_MAX_BLOCKS)
         zchunk *= 2;
     a.zchunk = zchunk;
     const int nzc = (g.n[2] + zchunk - 1) / zchunk;
@@ -382,6 +395,7 @@ bool residual_restrict_bulk(const LevelGeom& g, const float* L, const float* p, 
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = b_c; a.p_c = p_c;
     a.rb = ReduceBuf{nullptr, nullptr, nullptr};
     a.slot = 0;
+    a.slot2 = 0;
     return launch_res_bulk<0>(a, s);
 }
 
@@ -391,12 +405,25 @@ bool residual_norm2_bulk(const LevelGeom& g, const float* L, const float* p, con
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = nullptr; a.p_c = nullptr;
     a.rb = rb;
     a.slot = slot;
+    a.slot2 = 0;
     return launch_res_bulk<1>(a, s);
+}
+
+// sum r^2 -> red[slot_rr] and sum b^2 over active cells -> red[slot_ref] in ONE pass (loop entry)
+bool residual_and_ref_norm2_bulk(const LevelGeom& g, const float* L, const float* p, const float* b,
+                                 ReduceBuf rb, int slot_rr, int slot_ref, cudaStream_t s) {
+    ResBulkArgs a;
+    a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = nullptr; a.p_c = nullptr;
+    a.rb = rb;
+    a.slot = slot_rr;
+    a.slot2 = slot_ref;
+    return launch_res_bulk<2>(a, s);
 }
 
 int configure_residual_bulk() {
     cudaError_t e = cudaFuncSetAttribute(k_residual_bulk<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ResBulkCfg::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_residual_bulk<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ResBulkCfg::SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_residual_bulk<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ResBulkCfg::SMEM);
     return (int)e;
 }
 
