@@ -7,6 +7,28 @@
 namespace gmgf {
 using namespace gmgd;
 
+// Planes per CTA of a z-marching kernel.  Big levels: `zpref` planes (the redundant halo planes
+// cost little and many CTAs smooth the tail of the grid).  Small, L2-resident levels are
+// latency-bound: the kernel takes (waves of CTAs) x (planes per CTA + fixed start-up steps), so
+// the chunk count is chosen to minimise that -- in particular never a few CTAs over a wave.
+static inline int choose_zchunk(long long tiles, int nz, int zpref, int zmin, int slots, int even) {
+    if (nz <= zmin) return nz;
+    if (tiles * ((nz + zpref - 1) / zpref) >= 4LL * slots) return zpref;
+    const int overhead = 5;  // prologue + drain, in steps
+    long long best_t = -1;
+    int best = nz;
+    for (int nchunks = 1; nchunks <= nz / zmin; ++nchunks) {
+        int zc = (nz + nchunks - 1) / nchunks;
+        if (even && (zc & 1)) ++zc;
+        if (zc > zpref * 4) continue;
+        const long long ctas = tiles * ((nz + zc - 1) / zc);
+        const long long waves = (ctas + slots - 1) / slots;
+        const long long t = waves * (zc + overhead);
+        if (best_t < 0 || t < best_t) { best_t = t; best = zc; }
+    }
+    return best;
+}
+
 __device__ __forceinline__ int wrapi(int v, int n) {
     v %= n;
     return v < 0 ? v + n : v;

@@ -482,11 +482,7 @@ static void launch_sweep(SweepArgs& a, cudaStream_t s) {
     a.tiles_x = (g.n[0] + C::TX - 1) / C::TX;
     a.tiles_y = (g.n[1] + C::TY - 1) / C::TY;
     static const int zc_env = env_int("GMG_ZCHUNK", 64);
-    int zchunk = zc_env;
-    if (g.n[2] < 2 * zchunk) zchunk = g.n[2];
-    // keep at least ~4 CTAs per SM in flight on mid-size levels
-    while (zchunk > zmin_env() && (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) < 148 * 4)
-        zchunk = (zchunk + 1) / 2;
+    const int zchunk = choose_zchunk((long long)a.tiles_x * a.tiles_y, g.n[2], zc_env, zmin_env(), 148, 0);
     a.zchunk = zchunk;
     static const int pf_env = env_int("GMG_PF", 3);
     a.pf = pf_env;

@@ -374,11 +374,8 @@ static bool launch_res_bulk(ResBulkArgs& a, cudaStream_t s) {
     if (!res_maps(g, a.L, a.p, a.b, &maps)) return false;
     a.tiles_x = g.n[0] / C::TX;
     a.tiles_y = (g.n[1] + C::RY - 1) / C::RY;
-    int zchunk = 64;
-    if (g.n[2] < 2 * zchunk) zchunk = g.n[2];
-    while (zchunk > zmin_env() && zchunk % 4 == 0 &&
-           (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) < 148 * 4)
-        zchunk /= 2;
+    // two CTAs per SM; chunks start on even planes (the z pair of the restriction)
+    int zchunk = choose_zchunk((long long)a.tiles_x * a.tiles_y, g.n[2], 64, zmin_env(), 296, 1);
     // the deterministic reduction has a bounded number of block partials
     while (MODE >= 1 && (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) > GMG_REDUCE_MAX_BLOCKS)
         zchunk *= 2;

@@ -471,10 +471,7 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
     a.tiles_x = g.n[0] / Bulk::TX;
     a.tiles_y = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
     static const int zc_env = env_int2("GMG_ZCHUNK", 64);
-    int zchunk = zc_env;
-    if (g.n[2] < 2 * zchunk) zchunk = g.n[2];
-    while (zchunk > zmin_env() && (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) < 148 * 2)
-        zchunk = (zchunk + 1) / 2;
+    const int zchunk = choose_zchunk((long long)a.tiles_x * a.tiles_y, g.n[2], zc_env, zmin_env(), 148, 0);
     a.zchunk = zchunk;
     const int nzc = (g.n[2] + zchunk - 1) / zchunk;
     const unsigned int grid = (unsigned int)(a.tiles_x * a.tiles_y * nzc);
