@@ -58,6 +58,7 @@ struct gmg_ctx {
     size_t ws_bytes;
     bool ws_set, coeffs_set;
     float *pcg_r, *pcg_d, *pcg_q, *pcg_s, *stage_p, *stage_z;
+    float* tail_W[GMG_MAX_LEVELS];  // [6][N] face weights of the tail levels
     // small library-owned device state
     DevScalars* sc;
     double* partials;
@@ -153,6 +154,10 @@ static size_t carve(gmg_ctx* c, char* base) {
         }
         float* q = take(N);
         if (base) c->lv[l].q = q;
+        if (l >= c->tail_start) {
+            float* w = take(6 * N);
+            if (base) c->tail_W[l] = w;
+        }
     }
     const size_t N0 = (size_t)c->g[0].N;
     float* v[6];
@@ -329,6 +334,7 @@ extern "C" int gmg_set_coeffs(gmg_ctx* c, const float* L_dev, void* stream) {
     gmgk::check_coeffs(c->g[0], L_dev, rbuf(c), s);
     for (int l = 0; l + 1 < c->nlev; ++l)
         gmgk::coarsen_coeffs(c->g[l], c->lv[l].L, const_cast<float*>(c->lv[l + 1].L), s);
+    for (int l = c->tail_start; l < c->nlev; ++l) gmgk::tail_weights(c->g[l], c->lv[l].L, c->tail_W[l], s);
     gmgk::ctl_set_omega(c->sc, (double)c->prm.omega0, s);
     CUDA_TRY(c, cudaGetLastError());
     CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
@@ -411,7 +417,7 @@ static void enqueue_vcycle(gmg_ctx* c, float* p0, const float* b0, const float* 
         a.nlev = nlev - ts;
         for (int t = 0; t < a.nlev; ++t) {
             a.g[t] = c->g[ts + t];
-            a.L[t] = c->lv[ts + t].L;
+            a.W[t] = c->tail_W[ts + t];
         }
         a.b_in = B(ts);
         a.p_in = (ts == 0) ? p0 : nullptr;

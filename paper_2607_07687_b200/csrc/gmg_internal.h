@@ -59,7 +59,7 @@ enum {
 struct TailArgs {
     int nlev;                            // number of tail levels (>= 1)
     LevelGeom g[GMG_TAIL_MAX_LEVELS];
-    const float* L[GMG_TAIL_MAX_LEVELS]; // global coefficients of each tail level
+    const float* W[GMG_TAIL_MAX_LEVELS]; // [6][N] face weights of each tail level (tail_weights)
     const float* b_in;                   // right-hand side of the first tail level (global)
     const float* p_in;                   // initial guess of the first tail level; nullptr = zero
     float* p_out;                        // solution of the first tail level (global; may alias p_in)
@@ -93,6 +93,8 @@ void prolong_add(const LevelGeom& gf, const float* e_c, float* p_f, cudaStream_t
 void coarsen_coeffs(const LevelGeom& gf, const float* Lf, float* Lc, cudaStream_t s);
 void check_coeffs(const LevelGeom& g, const float* L, ReduceBuf rb, cudaStream_t s);
 void tail_vcycle(const TailArgs& a, size_t smem_bytes, cudaStream_t s);
+// W[f*N + c] = weight of face f (x-lo, x-hi, y-lo, y-hi, z-lo, z-hi) of cell c, wall faces zeroed
+void tail_weights(const LevelGeom& g, const float* L, float* W, cudaStream_t s);
 size_t tail_smem_bytes(const TailArgs& a);
 int tail_configure(size_t max_bytes);  // sets the dynamic-smem attribute; returns cudaError
 

@@ -128,17 +128,10 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_tail_vcycle(TailArgs a) {
     }
     __syncthreads();
     const float omega = *a.omega;
-    // ---- face weights of every tail level (wall faces zeroed by face_coeffs) ------------------
+    // ---- face weights of every tail level: precomputed by gmg_set_coeffs (tail_weights) ---------
     for (int t = 0; t < a.nlev; ++t) {
-        const LevelGeom& g = a.g[t];
-        const int N = (int)g.N, nx = g.n[0], ny = g.n[1];
-        for (int c = tid; c < N; c += kTailThreads) {
-            const int row = c / nx, i = c - row * nx, k = row / ny, j = row - k * ny;
-            float w[6];
-            face_coeffs(g, a.L[t], i, j, k, c, w);
-#pragma unroll
-            for (int f = 0; f < 6; ++f) S.W[t][f * N + c] = w[f];
-        }
+        const int N6 = 6 * (int)a.g[t].N;
+        for (int u = tid; u < N6; u += kTailThreads) S.W[t][u] = a.W[t][u];
     }
     {
         const int N = (int)a.g[0].N;
@@ -198,6 +191,21 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_tail_vcycle(TailArgs a) {
         const int N = (int)a.g[0].N;
         for (int u = tid; u < N; u += kTailThreads) a.p_out[u] = S.p[0][u];
     }
+}
+
+__global__ void __launch_bounds__(256) k_tail_weights(LevelGeom g, const float* __restrict__ L, float* __restrict__ W) {
+    const int N = (int)g.N, nx = g.n[0], ny = g.n[1];
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= N) return;
+    const int row = c / nx, i = c - row * nx, k = row / ny, j = row - k * ny;
+    float w[6];
+    face_coeffs(g, L, i, j, k, c, w);
+#pragma unroll
+    for (int f = 0; f < 6; ++f) W[f * N + c] = w[f];
+}
+
+void tail_weights(const LevelGeom& g, const float* L, float* W, cudaStream_t s) {
+    k_tail_weights<<<(unsigned int)((g.N + 255) / 256), 256, 0, s>>>(g, L, W);
 }
 
 size_t tail_smem_bytes(const TailArgs& a) {

@@ -102,10 +102,11 @@ def test_library_level_table_matches_golden_and_oracle(libpath):
         cells = sum(s[0] * s[1] * s[2] for s in shapes[tail:])
         assert tail < len(shapes) and cells * 32 <= 200 * 1024
         assert tail == 0 or (cells + shapes[tail - 1][0] * shapes[tail - 1][1] * shapes[tail - 1][2]) * 32 > 200 * 1024
-        # workspace: coarse levels (L, p, b, q) + level-0 q + 6 fine vectors, each 256-byte aligned
+        # workspace: coarse levels (L, p, b, q) + level-0 q + 6 fine vectors + the six face weights
+        # of the tail levels, each array 256-byte aligned
         N = [s[0] * s[1] * s[2] for s in shapes]
-        lower = 4 * (N[0] + 6 * N[0] + sum(6 * v for v in N[1:]))
-        assert lower <= ws <= lower + 256 * (6 * len(N) + 8)
+        lower = 4 * (N[0] + 6 * N[0] + sum(6 * v for v in N[1:]) + sum(6 * v for v in N[tail:]))
+        assert lower <= ws <= lower + 256 * (7 * len(N) + 8)
     # agreement with the oracle's rule on odd / mixed cases, both coarsening modes
     for n, bc in [((20, 20, 20), (1, 0, 0)), ((36, 20, 6), (0, 1, 0)), ((64, 4, 4), (1, 0, 0)), ((15, 9, 7), (1, 1, 1))]:
         for iso in (False, True):
