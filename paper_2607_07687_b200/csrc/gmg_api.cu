@@ -331,9 +331,16 @@ extern "C" int gmg_set_coeffs(gmg_ctx* c, const float* L_dev, void* stream) {
     cudaStream_t s = (cudaStream_t)stream;
     drop_graphs(c);
     c->lv[0].L = L_dev;
-    gmgk::check_coeffs(c->g[0], L_dev, rbuf(c), s);
-    for (int l = 0; l + 1 < c->nlev; ++l)
-        gmgk::coarsen_coeffs(c->g[l], c->lv[l].L, const_cast<float*>(c->lv[l + 1].L), s);
+    // finest level: validation rides on the coarsening pass when the float4 kernel takes it
+    const bool fused_check = c->prm.fast_path && c->nlev > 1 && gmgk::coarsen4_supported(c->g[0]);
+    if (!fused_check) gmgk::check_coeffs(c->g[0], L_dev, rbuf(c), s);
+    for (int l = 0; l + 1 < c->nlev; ++l) {
+        float* Lc = const_cast<float*>(c->lv[l + 1].L);
+        if (c->prm.fast_path && gmgk::coarsen4_supported(c->g[l]))
+            gmgk::coarsen_coeffs4(c->g[l], c->lv[l].L, Lc, l == 0, rbuf(c), s);
+        else
+            gmgk::coarsen_coeffs(c->g[l], c->lv[l].L, Lc, s);
+    }
     for (int l = c->tail_start; l < c->nlev; ++l) gmgk::tail_weights(c->g[l], c->lv[l].L, c->tail_W[l], s);
     gmgk::ctl_set_omega(c->sc, (double)c->prm.omega0, s);
     CUDA_TRY(c, cudaGetLastError());
@@ -814,7 +821,8 @@ extern "C" int gmg_divergence(gmg_ctx* c, const float* u_dev, const float wall_h
     if (!u_dev || !z_dev) { SET_ERR(c, "gmg_divergence: null pointer"); return GMG_EINVAL; }
     cudaStream_t s = (cudaStream_t)stream;
     const float zero[3] = {0.0f, 0.0f, 0.0f};
-    gmgk::divergence(c->g[0], u_dev, wall_hi ? wall_hi : zero, z_dev, s);
+    if (c->prm.fast_path && c->g[0].n[0] % 4 == 0) gmgk::divergence4(c->g[0], u_dev, wall_hi ? wall_hi : zero, z_dev, s);
+    else gmgk::divergence(c->g[0], u_dev, wall_hi ? wall_hi : zero, z_dev, s);
     CUDA_TRY(c, cudaGetLastError());
     CUDA_TRY(c, cudaStreamSynchronize(s));
     return GMG_OK;
@@ -825,7 +833,8 @@ extern "C" int gmg_project(gmg_ctx* c, float* u_dev, const float* p_dev, void* s
     if (!u_dev || !p_dev) { SET_ERR(c, "gmg_project: null pointer"); return GMG_EINVAL; }
     if (!c->coeffs_set) { SET_ERR(c, "gmg_project before gmg_set_coeffs"); return GMG_ESTATE; }
     cudaStream_t s = (cudaStream_t)stream;
-    gmgk::project(c->g[0], c->lv[0].L, p_dev, u_dev, s);
+    if (c->prm.fast_path && c->g[0].n[0] % 4 == 0) gmgk::project4(c->g[0], c->lv[0].L, p_dev, u_dev, s);
+    else gmgk::project(c->g[0], c->lv[0].L, p_dev, u_dev, s);
     CUDA_TRY(c, cudaGetLastError());
     CUDA_TRY(c, cudaStreamSynchronize(s));
     return GMG_OK;
