@@ -1,22 +1,23 @@
 // kernels_sweep.cu -- k_rb_sweep_bulk: the fused red+black Gauss-Seidel sweep of the big levels
-// (PAPER.md:43 S3.1; readings O3, O8), fed by the
-// Tensor Memory Accelerator (cp.async.bulk.tensor + mbarrier, SASS UTMALDG) instead of register
-// loads.
+// (PAPER.md:43 S3.1; readings O3, O8), fed by the Tensor Memory Accelerator
+// (cp.async.bulk.tensor + mbarrier, SASS UTMALDG) instead of register loads.
 //
-// Same schedule as k_rb_sweep (kernels_fused.cu): a CTA owns a 128 x TY tile and marches along
-// z; per step u:  wait for the data of step u;  B(u) first-colour update of plane u on tile +
-// ring 1, in place in shared memory;  barrier;  issue the copies of step u+PD;  C(u-1)
-// second-colour update of plane u-1, whole plane streamed to the destination array.
-//
-// What changed: EVERY input stream (source iterate p, right-hand side b, the three
-// face-coefficient arrays) arrives in shared memory as one TMA box per stream and plane
-// (128 x rows floats, 5.6-6.6 KB; plus two 4-float-wide halo boxes for p), issued PD steps
-// ahead of use: 7 TMA operations per step.  No registers are tied up by loads in flight, so the
-// DRAM latency is covered by shared-memory capacity (PD planes x 30 KB per SM) rather than by
-// occupancy.  Phase B reads its coefficient set from shared memory once and hands it to phase C
-// (one step later) in registers, so no coefficient is read twice.
+// A CTA owns a 128 x TY tile and marches along z.  EVERY input stream (source iterate p,
+// right-hand side b, the three face-coefficient arrays) arrives in shared memory as one TMA box
+// per stream and plane (128 x rows floats, 5.6-6.6 KB; plus two 4-float-wide halo boxes for p),
+// issued PD steps ahead of use: 7 TMA operations per step, no registers tied up by loads in
+// flight.  Step u, per thread (one float4 of one row):
+//     B(u)    first-colour update of plane u on tile + ring 1, in place in shared memory;
+//     C(u-1)  second-colour update of plane u-1, streamed to the destination array;
+//     loads of B(u+1)'s operands;  barrier;  issue the copies of step u+PD.
+// B and C sit between the same two barriers because of what each one reads.  A first-colour
+// cell has only second-colour neighbours, and those keep their SOURCE value in shared memory
+// (phase C writes to the destination array only): B(u) depends on no other thread's update,
+// so its operands can be loaded ahead of the barrier.  C(u-1) needs the B(u-1) results of the
+// rows above and below (other warps: behind the barrier of step u-1) and, at its own position,
+// the planes u-2, u-1, u this thread itself produced -- kept in registers.
 // Periodic wrap in x = the halo boxes are fetched at wrapped coordinates; in z = a wrapped plane
-// coordinate; tiles touching the y boundary (2 tile rows of ~114 at 1024^3) take a row-by-row
+// coordinate; tiles touching the y boundary (2 tile rows of ~80 at 1024^3) take a row-by-row
 // bulk-copy path (cp.async.bulk, UBLKCP) with wrapped row addresses.  Neumann walls = zeroed
 // coefficients.  Every shared-memory cell holds the periodic image of its cell, as in k_rb_sweep.
 #include <cuda.h>
@@ -28,9 +29,9 @@
 #include "fused_common.cuh"
 
 namespace gmgf {
-static int zmin_env() {
-    static const int v = getenv("GMG_ZMIN") ? atoi(getenv("GMG_ZMIN")) : 4;
-    return v;
+static int env_int2(const char* name, int dflt) {
+    const char* v = getenv(name);
+    return v ? atoi(v) : dflt;
 }
 
 template <int TY_, int PD_>
@@ -41,7 +42,10 @@ struct BulkCfg {
     static constexpr int MAIN = LPR * ROWS;
     static constexpr int THREADS = MAIN + 32;    // + one edge warp
     static constexpr int SH = TY + 4;            // rows of a p plane (halo 2)
-    static constexpr int NP = PD + 4;            // ring depths (slot-reuse argument: DESIGN.md S6)
+    // Ring depths.  G(u+PD) is issued behind the barrier of step u and may overwrite what step u
+    // was the last to read AND to use: p plane u-1 (rows above/below for C(u-1)), Lz plane u,
+    // Lx/Ly/b plane u.  Still to come are planes u..u+PD (+1 for p, whose group runs one ahead).
+    static constexpr int NP = PD + 2;
     static constexpr int NZ = PD + 1;
     static constexpr int NC = PD;
     static constexpr int NB = PD + 1;            // mbarriers of the step groups
@@ -63,6 +67,7 @@ struct BulkCfg {
         (uint32_t)(SH * TX + 2 * SH * 4 + 3 * ROWS * TX + (ROWS + 1) * TX) * 4u;
     static constexpr uint32_t PRO_BYTES = (uint32_t)(2 * (SH * TX + 2 * SH * 4) + ROWS * TX) * 4u;
     static_assert(2 * ROWS <= 32 && NB <= 8 && THREADS / 32 >= 7, "tile shape");
+    static_assert(SMEM <= 227 * 1024, "shared memory");
 };
 
 struct BulkArgs {
@@ -75,17 +80,56 @@ struct BulkArgs {
     int first_colour;
     int zchunk;
     int tiles_x, tiles_y;
-    int dbg;
 };
 
 struct alignas(64) BulkMaps {
     CUtensorMap p_main, p_halo, lz, lx, ly, b;
 };
 
-struct CFull {  // coefficient set of the four own cells in one plane, carried from B to C
+struct CFull {  // coefficients of the four own cells in one plane (lower faces, the y/z faces above, b)
     float4 lx, ly, lyh, lz, lzh, b;
-    float lxh;
+    float lxh;  // the x face above the fourth cell
 };
+
+struct CPair {  // coefficients of the two cells (a, b) = (S, S+2) phase C updates, carried one step
+    float lxa0, lxa1, lxb0, lxb1, lya, lyb, lyha, lyhb, lza, lzb, lzha, lzhb, ba, bb;
+};
+
+template <int S>
+__device__ __forceinline__ void pick_pair(const CFull& c, CPair& k) {
+    if (S == 0) {
+        k.lxa0 = c.lx.x; k.lxa1 = c.lx.y; k.lxb0 = c.lx.z; k.lxb1 = c.lx.w;
+        k.lya = c.ly.x; k.lyb = c.ly.z; k.lyha = c.lyh.x; k.lyhb = c.lyh.z;
+        k.lza = c.lz.x; k.lzb = c.lz.z; k.lzha = c.lzh.x; k.lzhb = c.lzh.z;
+        k.ba = c.b.x; k.bb = c.b.z;
+    } else {
+        k.lxa0 = c.lx.y; k.lxa1 = c.lx.z; k.lxb0 = c.lx.w; k.lxb1 = c.lxh;
+        k.lya = c.ly.y; k.lyb = c.ly.w; k.lyha = c.lyh.y; k.lyhb = c.lyh.w;
+        k.lza = c.lz.y; k.lzb = c.lz.w; k.lzha = c.lzh.y; k.lzhb = c.lzh.w;
+        k.ba = c.b.y; k.bb = c.b.w;
+    }
+}
+
+// Phase C on cells S and S+2 of `own` (plane v); zm_a/zm_b = plane v-1 and zp = plane v+1 at the
+// own position.  Same operations in the same order as update_pair.
+template <int S>
+__device__ __forceinline__ float4 update_pair_carried(float xm, float4 own, float xp, float4 ym, float4 yp,
+                                                      float zm_a, float zm_b, float4 zp, const CPair& k,
+                                                      float omega) {
+    float4 out = own;
+    if (S == 0) {
+        const float a1 = apply7(own.x, k.lxa0, k.lxa1, k.lya, k.lyha, k.lza, k.lzha, xm, own.y, ym.x, yp.x, zm_a, zp.x);
+        const float a2 = apply7(own.z, k.lxb0, k.lxb1, k.lyb, k.lyhb, k.lzb, k.lzhb, own.y, own.w, ym.z, yp.z, zm_b, zp.z);
+        out.x = relax(own.x, k.ba, a1, diag6(k.lxa0, k.lxa1, k.lya, k.lyha, k.lza, k.lzha), omega);
+        out.z = relax(own.z, k.bb, a2, diag6(k.lxb0, k.lxb1, k.lyb, k.lyhb, k.lzb, k.lzhb), omega);
+    } else {
+        const float a1 = apply7(own.y, k.lxa0, k.lxa1, k.lya, k.lyha, k.lza, k.lzha, own.x, own.z, ym.y, yp.y, zm_a, zp.y);
+        const float a2 = apply7(own.w, k.lxb0, k.lxb1, k.lyb, k.lyhb, k.lzb, k.lzhb, own.z, xp, ym.w, yp.w, zm_b, zp.w);
+        out.y = relax(own.y, k.ba, a1, diag6(k.lxa0, k.lxa1, k.lya, k.lyha, k.lza, k.lzha), omega);
+        out.w = relax(own.w, k.bb, a2, diag6(k.lxb0, k.lxb1, k.lyb, k.lyhb, k.lzb, k.lzhb), omega);
+    }
+    return out;
+}
 
 template <int S>
 __device__ __forceinline__ float4 update_pair_full(float xm, float4 own, float xp, float4 ym, float4 yp,
@@ -95,9 +139,10 @@ __device__ __forceinline__ float4 update_pair_full(float xm, float4 own, float x
     return update_pair<S>(xm, own, xp, ym, yp, zm, zp, s, c.lz, omega);
 }
 
-template <class C>
-__global__ void __launch_bounds__(C::THREADS, 1)
-k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
+// YIN: the tile's TMA boxes stay inside the domain in y (every tile but the first and last
+// tile rows); the other instantiation carries the row-copy path, so the common one stays small.
+template <class C, bool YIN>
+__device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& maps) {
     extern __shared__ __align__(1024) float sm[];  // no static shared memory: base is 1 KB aligned
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..NB) step groups, [NB] prologue
     const float** row_base = reinterpret_cast<const float**>(bars + 16);  // row-copy path tables
@@ -121,7 +166,7 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     const float omega = *a.omega;
     const int fc = a.first_colour;
     const int xL = wrapi(x0 - 4, nx), xR = wrapi(x0 + C::TX, nx);  // halo column groups
-    const bool y_inside = (y0 >= 2) && (y0 + C::TY + 2 <= ny);     // TMA boxes stay in the domain
+    constexpr bool y_inside = YIN;
     const float* Lx = a.L;
     const float* Ly = a.L + N;
     const float* Lz = a.L + 2 * N;
@@ -206,7 +251,7 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
             if (tid == 0) mbar_expect_tx(bar, C::PRO_BYTES);
             const int gb = wrap1(z0 - 1, nz);
             if (y_inside) {
-                // planes z0-2 .. z0-1+PL: three boxes each, one per warp; then Lz(z0-1)
+                // planes z0-2, z0-1: three boxes each, one per warp; then Lz(z0-1)
                 const int pl = warp_id / 3, k = warp_id % 3;
                 if (pl < 2) {
                     const int v = z0 - 2 + pl, gv = wrapi(v, nz);
@@ -228,7 +273,6 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     // ring cursors of step u (advanced once per step; no modulo in the loop)
     float* const P_beg = sm + C::OFF_P;
     float* const Z_beg = sm + C::OFF_LZ;
-    float* Pm2 = P_beg + (C::NP - 1) * C::P_PLANE;  // plane u-2 (u = z0-1: not loaded, not read)
     float* Pm1 = P_beg;                             // plane u-1
     float* P0 = P_beg + C::P_PLANE;                 // plane u
     float* Pp1 = P_beg + 2 * C::P_PLANE;            // plane u+1
@@ -239,7 +283,7 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     uint32_t kpar = 0;
     int gz = wrap1(z0 - 1, nz);                     // wrapped plane index of u
     auto advance = [&]() {
-        Pm2 = Pm1; Pm1 = P0; P0 = Pp1;
+        Pm1 = P0; P0 = Pp1;
         Pp1 += C::P_PLANE;
         if (Pp1 == P_beg + C::NP * C::P_PLANE) Pp1 = P_beg;
         Z0 = Z1;
@@ -262,78 +306,92 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
         const bool zy_lo = g.bc[1] && gy == 0, zy_hi = g.bc[1] && gyp == 0;
         const bool last_lane = (lx == C::LPR - 1);
         const int p_off = (ry + 1) * C::TX + 4 * lx;        // own float4 in a p plane
-        const int h_off = (lx == 0 ? C::P_HL + 3 : C::P_HR) + (ry + 1) * 4;  // x-halo cell of the edge lanes
+        const int h_off = (lx == 0 ? C::P_HL + 3 : C::P_HR) + (ry + 1) * 4;  // x-halo cell (first / last lane)
         const int c_off = ry * C::TX + 4 * lx;              // own float4 in a coefficient plane
         float* dst_ptr = a.dst + ((long long)gy * nx + gx + (long long)(z0 - 2) * plane);  // plane u-1
         const float* const lxh_row = Lx + (size_t)gy * nx + gxh;  // face above the tile's last cell
-
-        auto phase = [&](const float* Pm, const float* P, const float* Pp, int sel, const CFull& s) -> float4 {
-            const float4 own = lds4(P + p_off);
-            const float4 ym = lds4(P + p_off - C::TX);
-            const float4 yp = lds4(P + p_off + C::TX);
-            const float4 zm = lds4(Pm + p_off);
-            const float4 zp = lds4(Pp + p_off);
-            float xm = __shfl_up_sync(0xffffffffu, own.w, 1);
-            float xp = __shfl_down_sync(0xffffffffu, own.x, 1);
-            if (lx == 0) xm = P[h_off];
-            if (last_lane) xp = P[h_off];
-            return sel ? update_pair_full<1>(xm, own, xp, ym, yp, zm, zp, s, omega)
-                       : update_pair_full<0>(xm, own, xp, ym, yp, zm, zp, s, omega);
-        };
-        float lxh_pf = last_lane ? __ldg(lxh_row + (size_t)gz * plane) : 0.0f;
-        // cells (sel, sel+2) of the group are updated: same parity for B(u) and C(u-1)
+        // cells (sel, sel+2) of the group are updated: same parity for B(u) and C(u-1); sel is
+        // warp-uniform and alternates every step
         int sel = (yl + (z0 - 1) + fc) & 1;
+        float lxh_pf = last_lane ? __ldg(lxh_row + (size_t)gz * plane) : 0.0f;
         const bool any_wall = zx_lo || zx_hi || zy_lo || zy_hi || g.bc[2];
-        // One step.  Sp = coefficient set of plane u-1 (made by B(u-1), used by C(u-1));
-        // Sc = set of plane u, read from shared memory here.  The caller alternates the two
-        // register sets, so nothing is copied between steps.
-        auto step = [&](int u, const CFull& Sp, CFull& Sc) {
+        // K = the coefficients of the two cells C updates next step, picked out of this step's
+        // set (14 floats, not a second full set); q1 / z2 = planes u-1 / u-2 at the own position
+        CPair K;
+        K.lxa0 = K.lxa1 = K.lxb0 = K.lxb1 = K.lya = K.lyb = K.lyha = K.lyhb = 0.0f;
+        K.lza = K.lzb = K.lzha = K.lzhb = K.ba = K.bb = 0.0f;
+        float4 q1 = lds4(Pm1 + p_off);   // u = z0-1: source values
+        float z2a = 0.0f, z2b = 0.0f;
+        CFull Sc;
+        float4 own, ym, yp, zp;
+        float hvB;
+        // Operands of B(u) -- TMA data and source values no other thread changes.  Loaded at the
+        // end of step u-1, in front of the barrier: behind it only the two rows phase C needs
+        // are still to be read, so the 16 warps do not all queue on the shared-memory pipe at once.
+        auto load_step = [&]() {
             mbar_wait(bars + kb, kpar);
+            Sc.lx = lds4(sm + C::OFF_LX + ic * C::C_PLANE + c_off);
+            const float* Y = sm + C::OFF_LY + ic * C::Y_PLANE + c_off;
+            Sc.ly = lds4(Y);
+            Sc.lyh = lds4(Y + C::TX);
+            Sc.lz = lds4(Z0 + c_off);
+            Sc.lzh = lds4(Z1 + c_off);
+            Sc.b = lds4(sm + C::OFF_B + ic * C::C_PLANE + c_off);
+            own = lds4(P0 + p_off);
+            ym = lds4(P0 + p_off - C::TX);
+            yp = lds4(P0 + p_off + C::TX);
+            zp = lds4(Pp1 + p_off);
+            hvB = P0[h_off];
+        };
+        load_step();
+        for (int u = z0 - 1; u <= z1; ++u) {
             const int gzp = (gz + 1 == nz) ? 0 : gz + 1;
-            {   // coefficient set of plane u: shared memory -> registers, wall faces zeroed
-                Sc.lx = lds4(sm + C::OFF_LX + ic * C::C_PLANE + c_off);
-                const float* Y = sm + C::OFF_LY + ic * C::Y_PLANE + c_off;
-                Sc.ly = lds4(Y);
-                Sc.lyh = lds4(Y + C::TX);
-                Sc.lz = lds4(Z0 + c_off);
-                Sc.lzh = lds4(Z1 + c_off);
-                Sc.b = lds4(sm + C::OFF_B + ic * C::C_PLANE + c_off);
-                const float t = __shfl_down_sync(0xffffffffu, Sc.lx.x, 1);
-                Sc.lxh = last_lane ? lxh_pf : t;
-                if (last_lane && u + 1 <= z1) lxh_pf = __ldg(lxh_row + (size_t)gzp * plane);
-                if (any_wall) {
-                    if (zx_lo) Sc.lx.x = 0.0f;
-                    if (zx_hi) Sc.lxh = 0.0f;
-                    if (zy_lo) Sc.ly = zero4();
-                    if (zy_hi) Sc.lyh = zero4();
-                    if (g.bc[2]) {
-                        if (gz == 0) Sc.lz = zero4();
-                        if (gzp == 0) Sc.lzh = zero4();
-                    }
+            const float4 cym = lds4(Pm1 + p_off - C::TX);   // plane u-1, B-updated rows above / below
+            const float4 cyp = lds4(Pm1 + p_off + C::TX);
+            const float hvC = Pm1[h_off];
+            const float t = __shfl_down_sync(0xffffffffu, Sc.lx.x, 1);
+            Sc.lxh = last_lane ? lxh_pf : t;
+            if (last_lane && u + 1 <= z1) lxh_pf = __ldg(lxh_row + (size_t)gzp * plane);
+            if (any_wall) {   // Neumann wall faces carry coefficient 0 (reading O2)
+                if (zx_lo) Sc.lx.x = 0.0f;
+                if (zx_hi) Sc.lxh = 0.0f;
+                if (zy_lo) Sc.ly = zero4();
+                if (zy_hi) Sc.lyh = zero4();
+                if (g.bc[2]) {
+                    if (gz == 0) Sc.lz = zero4();
+                    if (gzp == 0) Sc.lzh = zero4();
                 }
             }
-            if (!(a.dbg & 1)) {   // B(u): first colour on tile + ring 1, in place in shared memory
-                const float4 nw = phase(Pm1, P0, Pp1, sel, Sc);
-                *reinterpret_cast<float4*>(P0 + p_off) = nw;
+            float xm = __shfl_up_sync(0xffffffffu, own.w, 1);
+            float xp = __shfl_down_sync(0xffffffffu, own.x, 1);
+            float cxm = __shfl_up_sync(0xffffffffu, q1.w, 1);
+            float cxp = __shfl_down_sync(0xffffffffu, q1.x, 1);
+            xm = (lx == 0) ? hvB : xm;
+            xp = last_lane ? hvB : xp;
+            cxm = (lx == 0) ? hvC : cxm;
+            cxp = last_lane ? hvC : cxp;
+            float4 nw, nc;   // B(u) and C(u-1) results
+            if (sel) {
+                nw = update_pair_full<1>(xm, own, xp, ym, yp, q1, zp, Sc, omega);
+                nc = update_pair_carried<1>(cxm, q1, cxp, cym, cyp, z2a, z2b, nw, K, omega);
+                pick_pair<0>(Sc, K);     // the next step's C works on cells 0 and 2 of plane u
+                z2a = q1.x; z2b = q1.z;
+            } else {
+                nw = update_pair_full<0>(xm, own, xp, ym, yp, q1, zp, Sc, omega);
+                nc = update_pair_carried<0>(cxm, q1, cxp, cym, cyp, z2a, z2b, nw, K, omega);
+                pick_pair<1>(Sc, K);
+                z2a = q1.y; z2b = q1.w;
             }
-            fence_async_smem();  // order this thread's smem writes before later TMA overwrites
-            cta_sync();
-            if (u + C::PD <= z1) issue_step(u + C::PD);
-            if (u - 1 >= z0 && row_c && !(a.dbg & 2)) {  // C(u-1): second colour, tile rows only (warp-uniform)
-                const float4 nw = phase(Pm2, Pm1, P0, sel, Sp);
-                *reinterpret_cast<float4*>(dst_ptr) = nw;
-            }
+            *reinterpret_cast<float4*>(P0 + p_off) = nw;
+            if (u - 1 >= z0 && row_c) *reinterpret_cast<float4*>(dst_ptr) = nc;
+            q1 = nw;
             sel ^= 1;
             dst_ptr += plane;
             advance();
-        };
-        CFull SA, SB;
-        SA.lx = SA.ly = SA.lyh = SA.lz = SA.lzh = SA.b = zero4();
-        SA.lxh = 0.0f;
-        SB = SA;
-        for (int u = z0 - 1; u <= z1; u += 2) {
-            step(u, SA, SB);
-            if (u + 1 <= z1) step(u + 1, SB, SA);
+            if (u + 1 <= z1) load_step();
+            fence_async_smem();  // order this thread's smem writes before later TMA overwrites
+            cta_sync();
+            if (u + C::PD <= z1) issue_step(u + C::PD);
         }
     } else {
         // ---- edge warp: ring-1 cells x0-1 and x0+TX of every row, phase B only ----------------
@@ -388,18 +446,22 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     }
 }
 
+template <class C>
+__global__ void __launch_bounds__(C::THREADS, 1)
+k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
+    const int ty = (blockIdx.x / a.tiles_x) % a.tiles_y;
+    const int y0 = ty * C::TY;
+    if ((y0 >= 2) && (y0 + C::TY + 2 <= a.g.n[1])) sweep_body<C, true>(a, maps);
+    else sweep_body<C, false>(a, maps);
+}
+
 // ---- launchers ------------------------------------------------------------------------------
 bool sweep_v2_supported(const LevelGeom& g);
 void rb_sweep_v2(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
                  const float* omega, int first_colour, const float* e_c, cudaStream_t s);
 int configure_v2();
 
-using Bulk = BulkCfg<13, 3>;
-
-static int env_int2(const char* name, int dflt) {
-    const char* v = getenv(name);
-    return v ? atoi(v) : dflt;
-}
+using Bulk = BulkCfg<13, 4>;
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
@@ -436,23 +498,21 @@ bool tensor_map(const float* ptr, const LevelGeom& g, int bw, int bh, CUtensorMa
 
 bool sweep_supported(const LevelGeom& g) { return sweep_v2_supported(g); }
 
-bool bulk_supported(const LevelGeom& g);
+bool bulk_supported(const LevelGeom& g) {
+    return g_encode && g.n[0] >= 128 && g.n[0] % 128 == 0 && g.n[1] >= 4 && g.n[2] >= 8;
+}
+
 bool tma_shape_ok(const LevelGeom& g) {
     static const int use_bulk = env_int2("GMG_BULK", 1);
     return use_bulk && bulk_supported(g);
 }
 
-bool bulk_supported(const LevelGeom& g) {
-    return g_encode && g.n[0] >= 128 && g.n[0] % 128 == 0 && g.n[1] >= 4 && g.n[2] >= 8;
-}
-
 void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
               const float* omega, int first_colour, const float* e_c, int allow_tma, cudaStream_t s) {
-    static const int use_bulk = env_int2("GMG_BULK", 1);
     BulkMaps maps;
     const size_t N = (size_t)g.N;
     // the caller applies the prolongation as its own pass in front of this kernel (e_c == nullptr)
-    bool ok = use_bulk && allow_tma && !e_c && bulk_supported(g);
+    bool ok = allow_tma && !e_c && tma_shape_ok(g);
     ok = ok && tensor_map(src, g, Bulk::TX, Bulk::SH, &maps.p_main);
     ok = ok && tensor_map(src, g, 4, Bulk::SH, &maps.p_halo);
     ok = ok && tensor_map(L + 2 * N, g, Bulk::TX, Bulk::ROWS, &maps.lz);
@@ -466,12 +526,11 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
     BulkArgs a;
     a.g = g; a.L = L; a.src = src; a.dst = dst; a.b = b; a.omega = omega;
     a.first_colour = first_colour;
-    static const int dbg_env = env_int2("GMG_DBG", 0);
-    a.dbg = dbg_env;
     a.tiles_x = g.n[0] / Bulk::TX;
     a.tiles_y = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
     static const int zc_env = env_int2("GMG_ZCHUNK", 64);
-    const int zchunk = choose_zchunk((long long)a.tiles_x * a.tiles_y, g.n[2], zc_env, zmin_env(), 148, 0);
+    static const int zmin_env = env_int2("GMG_ZMIN", 4);
+    const int zchunk = choose_zchunk((long long)a.tiles_x * a.tiles_y, g.n[2], zc_env, zmin_env, 148, 0);
     a.zchunk = zchunk;
     const int nzc = (g.n[2] + zchunk - 1) / zchunk;
     const unsigned int grid = (unsigned int)(a.tiles_x * a.tiles_y * nzc);
@@ -480,7 +539,8 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
 
 int configure() {
     cudaError_t e = (cudaError_t)configure_v2();
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
     if (e == cudaSuccess && !g_encode) {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult qres;

@@ -31,7 +31,9 @@ __device__ __forceinline__ float diag6(float wxl, float wxh, float wyl, float wy
 
 // RBGS cell update (readings O3, O8):  p_I += omega (b_I - (A p)_I) / D_I  on active cells.
 __device__ __forceinline__ float relax(float pc, float b, float Ap, float D, float omega) {
-    return (D != 0.0f) ? pc + __fdividef(omega * (b - Ap), D) : pc;
+    // branch-free: an inactive cell (D == 0) adds 0/1
+    const bool act = D != 0.0f;
+    return pc + __fdividef(act ? omega * (b - Ap) : 0.0f, act ? D : 1.0f);
 }
 
 // Gathers the seven p values and six face coefficients of cell (i,j,k) with plain loads.
