@@ -325,6 +325,34 @@ def config4(n=1024, nspheres=64, diameter=32, seed=76874):
                           "diameter": diameter})
 
 
+# --------------------------------------------------------------------------
+# Aspect-ratio study (Fig. 2 right): impulsive start of a uniform flow past a
+# sphere in an (N b) x b x b box -- x Neumann (inflow / outflow faces carry the free stream),
+# y/z periodic.  Synthetic stand-in for the paper's case: same structure, our own sizes.
+# --------------------------------------------------------------------------
+def impulsive_sphere(N=4, base=32, D=None):
+    D = base / 4.0 if D is None else float(D)
+    n = (int(N) * base, base, base)
+    nx, ny, nz = n
+    bc = (NEUMANN, PERIODIC, PERIODIC)
+    c = (min(1.0, 0.5 * N) * base, 0.5 * base, 0.5 * base)
+    L = np.empty((3, nz, ny, nx), dtype=np.float64)
+    for d in range(3):
+        X, Y, Z = face_coords(n, d)
+        L[d] = ramp(np.sqrt((X - c[0]) ** 2 + (Y - c[1]) ** 2 + (Z - c[2]) ** 2) - 0.5 * D)
+    L32 = L.astype(np.float32)
+    Lq = L32.astype(np.float64)
+    u = np.zeros_like(Lq)
+    u[0] = Lq[0]                             # u* = the free stream (1, 0, 0), masked by the body
+    u[0][:, :, 0] = 1.0                      # inflow face
+    z = divergence(u, bc, wall_hi=(1.0, 0.0, 0.0))
+    act = active_mask(L32, bc)
+    z = project_compatible(z, act)
+    return Workload(f"impulsive_sphere_N{N}", n, bc, L32, z.astype(np.float32),
+                    tol=1e-4, maxiter=200, seed=0,
+                    meta={"active_fraction": float(act.mean()), "aspect": int(N)})
+
+
 def by_name(name: str) -> Workload:
     """configs by short name: c0, c1, c2, c3p5, c3p6, c4 (1024^3), c4_128, c4_256, c4_512."""
     if name == "c0":

@@ -306,6 +306,28 @@ def test_isotropic_vs_anisotropic_coarsening(n, bc):
     assert counts["aniso"][0] <= counts["iso"][0]         # ... and no more cycles
 
 
+def test_aspect_ratio_study_matches_oracle_and_shows_the_papers_trend():
+    """SURVEY.md S8(f) N3, PAPER.md:47-51 (Fig. 2, right): impulsive start past a sphere in an
+    (N b) x b x b box.  V-cycle counts of both coarsening modes match the oracle within one cycle
+    for N = 1, 4, 8 (b = 16), anisotropic never needs more cycles, and for N >= 4 it has more
+    levels and needs at least 1.4x fewer cycles (oracle: 13 -> 8 and 34 -> 21 at b = 16; the paper's
+    order of magnitude is for its own cases, smoother settings and a count over four time steps)."""
+    from paper_2607_07687_b200 import aspect_study
+    rows = aspect_study.run(aspects=(1, 4, 8), base=16)
+    for r in rows:
+        wl = W.impulsive_sphere(r["aspect"], 16)
+        for name, iso in (("iso", True), ("aniso", False)):
+            h = make_oracle(wl, iso=iso)
+            ref = h.solve(oracle.GMG_RBGS, wl.z, tol=1e-4, maxiter=200)
+            assert r[name]["levels"] == h.nlev
+            assert r[name]["converged"] == (ref["status"] == 0), (r["aspect"], name)
+            assert abs(r[name]["vcycles"] - ref["iterations"]) <= 1, (r["aspect"], name, r[name], ref["iterations"])
+        assert r["aniso"]["vcycles"] <= r["iso"]["vcycles"]
+        if r["aspect"] >= 4:
+            assert r["aniso"]["levels"] > r["iso"]["levels"]
+            assert 1.4 * r["aniso"]["vcycles"] <= r["iso"]["vcycles"], r
+
+
 def test_non_default_stream_and_two_contexts():
     """Work is enqueued on the caller's stream; contexts are independent."""
     wl_a, wl_b = W.config3(5), W.config0()
