@@ -73,6 +73,9 @@ typedef struct {
     int tma_min_cells; /* levels with at least this many cells (and nx % 128 == 0) use the TMA-fed
                           z-marching kernels; smaller ones the register-fed tiles (4194304);
                           0 = whenever the shape allows, -1 = never */
+    int cluster_tail;  /* 1: the coarse levels that fit the shared memory of a cluster of 8 CTAs
+                          (each at most 32768 cells) run as ONE thread-block-cluster kernel;
+                          0: only what fits a single CTA does (1) */
 } gmg_params_t;
 
 /* Statistics of the last gmg_solve. */

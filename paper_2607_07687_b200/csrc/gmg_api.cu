@@ -50,6 +50,10 @@ struct gmg_ctx {
     LevelPtrs lv[GMG_MAX_LEVELS];
     int tail_start;       // first level run inside the single-CTA tail kernel (nlev = none)
     size_t tail_smem;
+    int ctail_start;      // first level run inside the cluster tail kernel (nlev = none); < tail_start
+    size_t ctail_smem;
+    gmgk::CLevelPlan ctail_lv[GMG_TAIL_MAX_LEVELS];
+    bool cluster_ok;      // the device can hold a cluster of 8 CTAs with 200 KB each
     bool fast_sweep[GMG_MAX_LEVELS];
     bool fast_rr[GMG_MAX_LEVELS];
     int tma_ok[GMG_MAX_LEVELS];  // level large enough for the TMA-fed kernels
@@ -126,6 +130,21 @@ static void build_levels(gmg_ctx* c) {
         c->tail_start = l;
         c->tail_smem = cells * 8 * sizeof(float);
     }
+    // cluster tail: the longest suffix (beyond the single-CTA tail) a cluster of 8 CTAs can hold
+    c->ctail_start = c->nlev;
+    c->ctail_smem = 0;
+    if (c->prm.fast_path && c->prm.cluster_tail && c->cluster_ok) {
+        const int lo = c->nlev > GMG_TAIL_MAX_LEVELS ? c->nlev - GMG_TAIL_MAX_LEVELS : 0;
+        for (int l = lo; l < c->tail_start; ++l) {
+            gmgk::CLevelPlan lv[GMG_TAIL_MAX_LEVELS];
+            const size_t bytes = gmgk::ctail_plan(c->g + l, c->nlev - l, lv);
+            if (bytes == 0) continue;
+            c->ctail_start = l;
+            c->ctail_smem = bytes;
+            memcpy(c->ctail_lv, lv, sizeof(lv));
+            break;
+        }
+    }
     for (int l = 0; l < c->nlev; ++l) {
         c->fast_sweep[l] = c->prm.fast_path && gmgf::sweep_supported(c->g[l]);
         c->fast_rr[l] = c->prm.fast_path && l + 1 < c->nlev && gmgf::resrestrict_supported(c->g[l]);
@@ -154,7 +173,7 @@ static size_t carve(gmg_ctx* c, char* base) {
         }
         float* q = take(N);
         if (base) c->lv[l].q = q;
-        if (l >= c->tail_start) {
+        if (l >= c->tail_start || l >= c->ctail_start) {
             float* w = take(6 * N);
             if (base) c->tail_W[l] = w;
         }
@@ -181,7 +200,7 @@ extern "C" void gmg_default_params(gmg_params_t* p) {
     p->nu_pre = 2; p->nu_post = 2; p->nu_coarse = 32;
     p->omega0 = 1.0f; p->omega_min = 0.5f; p->omega_down = 0.125f; p->omega_up = 0.03125f;
     p->adaptive = 1; p->coarsen_mode = GMG_COARSEN_ANISO; p->n_min = 4;
-    p->fast_path = 1; p->use_graph = 1; p->tma_min_cells = 4 << 20;
+    p->fast_path = 1; p->use_graph = 1; p->tma_min_cells = 4 << 20; p->cluster_tail = 1;
 }
 
 extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]) {
@@ -205,6 +224,9 @@ extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]
     c->sc = nullptr; c->partials = nullptr; c->counter = nullptr; c->sc_host = nullptr;
     c->ev0 = c->ev1 = nullptr;
     c->cap_a = c->cap_b = nullptr;
+    c->cluster_ok = false;
+    if (gmgk::ctail_configure(200 * 1024) == (int)cudaSuccess) c->cluster_ok = gmgk::ctail_launchable(200 * 1024);
+    cudaGetLastError();
     build_levels(c);
     cudaError_t e = cudaMalloc(&c->sc, sizeof(DevScalars));
     if (e == cudaSuccess) e = cudaMalloc(&c->partials, 2 * GMG_REDUCE_MAX_BLOCKS * sizeof(double));
@@ -299,6 +321,7 @@ extern "C" int gmg_plan(int nx, int ny, int nz, const int bc[3], const gmg_param
     }
     if ((long long)nx * ny * nz > (1LL << 31) - 1) return GMG_EINVAL;
     gmg_ctx tmp;
+    tmp.cluster_ok = true;   // host-side plan: assume a device that can hold the cluster
     for (int d = 0; d < 3; ++d) { tmp.n0[d] = n[d]; tmp.bc[d] = bc[d]; }
     if (params) tmp.prm = *params; else gmg_default_params(&tmp.prm);
     if (tmp.prm.n_min < 1) return GMG_EINVAL;
@@ -341,7 +364,8 @@ extern "C" int gmg_set_coeffs(gmg_ctx* c, const float* L_dev, void* stream) {
         else
             gmgk::coarsen_coeffs(c->g[l], c->lv[l].L, Lc, s);
     }
-    for (int l = c->tail_start; l < c->nlev; ++l) gmgk::tail_weights(c->g[l], c->lv[l].L, c->tail_W[l], s);
+    for (int l = (c->ctail_start < c->tail_start ? c->ctail_start : c->tail_start); l < c->nlev; ++l)
+        gmgk::tail_weights(c->g[l], c->lv[l].L, c->tail_W[l], s);
     gmgk::ctl_set_omega(c->sc, (double)c->prm.omega0, s);
     CUDA_TRY(c, cudaGetLastError());
     CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
@@ -404,7 +428,8 @@ static void smooth(gmg_ctx* c, int l, float* p, const float* b, const float* ome
 // ---- V-cycle: reading O7 (PAPER.md:39 smoother + coarse-grid correction; 51 "V-cycle") -------
 static void enqueue_vcycle(gmg_ctx* c, float* p0, const float* b0, const float* omega, int sym,
                            cudaStream_t s) {
-    const int nlev = c->nlev, ts = c->tail_start;
+    const bool cluster = c->ctail_start < c->nlev;
+    const int nlev = c->nlev, ts = cluster ? c->ctail_start : c->tail_start;
     auto P = [&](int l) { return l == 0 ? p0 : c->lv[l].p; };
     auto B = [&](int l) { return l == 0 ? b0 : (const float*)c->lv[l].b; };
     const int post_first = sym ? 1 : 0;
@@ -418,7 +443,7 @@ static void enqueue_vcycle(gmg_ctx* c, float* p0, const float* b0, const float* 
         c->n_launch += 1;
     }
     if (ts < nlev) {
-        // l == ts: the rest of the hierarchy is one single-CTA kernel
+        // l == ts: the rest of the hierarchy is one kernel (a cluster of 8 CTAs, or a single CTA)
         TailArgs a;
         memset(&a, 0, sizeof(a));
         a.nlev = nlev - ts;
@@ -431,7 +456,8 @@ static void enqueue_vcycle(gmg_ctx* c, float* p0, const float* b0, const float* 
         a.p_out = P(ts);
         a.omega = omega;
         a.nu1 = c->prm.nu_pre; a.nu2 = c->prm.nu_post; a.nuc = c->prm.nu_coarse; a.sym = sym;
-        gmgk::tail_vcycle(a, c->tail_smem, s);
+        if (cluster) gmgk::ctail_vcycle(a, c->ctail_lv, c->ctail_smem, s);
+        else gmgk::tail_vcycle(a, c->tail_smem, s);
         c->n_launch += 1;
     } else {
         // coarsest level too large for shared memory: plain half-sweep launches
@@ -846,9 +872,11 @@ extern "C" int gmg_describe_plan(const gmg_ctx* c, char* buf, size_t cap) {
     buf[0] = 0;
     for (int l = 0; l < c->nlev; ++l) {
         const bool tma = c->tma_ok[l] && c->g[l].n[0] % 128 == 0 && c->g[l].n[1] >= 4 && c->g[l].n[2] >= 8;
-        const char* how = (l >= c->tail_start) ? "tail(single-CTA smem)"
+        const bool in_cluster = c->ctail_start < c->nlev && l >= c->ctail_start;
+        const bool in_tail = in_cluster || l >= c->tail_start;
+        const char* how = in_cluster ? "tail(8-CTA cluster smem)" : in_tail ? "tail(single-CTA smem)"
                           : (c->fast_sweep[l] ? (tma ? "fused-rb-sweep(TMA)" : "fused-rb-sweep") : "generic-half-sweeps");
-        const char* rr = (l >= c->tail_start || l == c->nlev - 1) ? "-"
+        const char* rr = (in_tail || l == c->nlev - 1) ? "-"
                          : (c->fast_rr[l] ? "tiled" : "generic");
         int w = snprintf(buf + off, cap - off, "L%d %dx%dx%d c=%d%d%d sweep=%s resrestrict=%s\n", l,
                          c->g[l].n[0], c->g[l].n[1], c->g[l].n[2], c->g[l].c[0], c->g[l].c[1],

@@ -101,6 +101,17 @@ void tail_vcycle(const TailArgs& a, size_t smem_bytes, cudaStream_t s);
 // W[f*N + c] = weight of face f (x-lo, x-hi, y-lo, y-hi, z-lo, z-hi) of cell c, wall faces zeroed
 void tail_weights(const LevelGeom& g, const float* L, float* W, cudaStream_t s);
 size_t tail_smem_bytes(const TailArgs& a);
+// Cluster tail (kernels_ctail.cu): layout of a level in the shared memory of the 8 CTAs.
+struct CLevelPlan {
+    int dist;  // 1: cut into 8 z-slabs, one per CTA; 0: whole level in CTA 0
+    int per;   // cells held per CTA
+    int off;   // float offset of this level's block in every CTA: W[6][per] p[per] b[per] r[per]
+};
+// Returns the dynamic shared memory per CTA, or 0 when these levels cannot run on the cluster.
+size_t ctail_plan(const LevelGeom* g, int nlev, CLevelPlan* lv);
+int ctail_configure(size_t max_bytes);
+bool ctail_launchable(size_t smem_bytes);
+void ctail_vcycle(const TailArgs& t, const CLevelPlan* lv, size_t smem_bytes, cudaStream_t s);
 int tail_configure(size_t max_bytes);  // sets the dynamic-smem attribute; returns cudaError
 
 // reductions: result lands in rb.sc->red[slot]

@@ -32,7 +32,7 @@ class Params(C.Structure):
                 ("omega0", C.c_float), ("omega_min", C.c_float), ("omega_down", C.c_float),
                 ("omega_up", C.c_float), ("adaptive", C.c_int), ("coarsen_mode", C.c_int),
                 ("n_min", C.c_int), ("fast_path", C.c_int), ("use_graph", C.c_int),
-                ("tma_min_cells", C.c_int)]
+                ("tma_min_cells", C.c_int), ("cluster_tail", C.c_int)]
 
 
 class Stats(C.Structure):

@@ -50,9 +50,9 @@ def test_library_contains_sm100a_code(libpath):
 
 
 def test_struct_sizes_match_header(libpath):
-    """Params / Stats mirror the C structs (13 x 4 bytes; Stats has 8-byte alignment)."""
+    """Params / Stats mirror the C structs (14 x 4 bytes; Stats has 8-byte alignment)."""
     from paper_2607_07687_b200 import gmg
-    assert C.sizeof(gmg.Params) == 52
+    assert C.sizeof(gmg.Params) == 56
     assert C.sizeof(gmg.Stats) == 4 * 4 + 6 * 8 + 8 + 8
     p = gmg.Params()
     gmg.lib.gmg_default_params(C.byref(p))
@@ -103,10 +103,12 @@ def test_library_level_table_matches_golden_and_oracle(libpath):
         assert tail < len(shapes) and cells * 32 <= 200 * 1024
         assert tail == 0 or (cells + shapes[tail - 1][0] * shapes[tail - 1][1] * shapes[tail - 1][2]) * 32 > 200 * 1024
         # workspace: coarse levels (L, p, b, q) + level-0 q + 6 fine vectors + the six face weights
-        # of the tail levels, each array 256-byte aligned
+        # of the tail levels, each array 256-byte aligned; the cluster tail may take the weights of
+        # levels above the single-CTA tail too (at most 32768 cells each)
         N = [s[0] * s[1] * s[2] for s in shapes]
         lower = 4 * (N[0] + 6 * N[0] + sum(6 * v for v in N[1:]) + sum(6 * v for v in N[tail:]))
-        assert lower <= ws <= lower + 256 * (7 * len(N) + 8)
+        cluster_extra = 4 * sum(6 * v for v in N[:tail] if v <= 32768)
+        assert lower <= ws <= lower + cluster_extra + 256 * (7 * len(N) + 8)
     # agreement with the oracle's rule on odd / mixed cases, both coarsening modes
     for n, bc in [((20, 20, 20), (1, 0, 0)), ((36, 20, 6), (0, 1, 0)), ((64, 4, 4), (1, 0, 0)), ((15, 9, 7), (1, 1, 1))]:
         for iso in (False, True):

@@ -328,6 +328,37 @@ def test_aspect_ratio_study_matches_oracle_and_shows_the_papers_trend():
             assert 1.4 * r["aniso"]["vcycles"] <= r["iso"]["vcycles"], r
 
 
+@pytest.mark.parametrize("n,bc", [((64, 64, 64), (0, 0, 0)), ((64, 64, 32), (1, 0, 1)),
+                                  ((48, 32, 64), (1, 1, 1)), ((128, 32, 32), (0, 1, 0))])
+def test_cluster_tail_is_bit_identical_to_single_cta_tail(n, bc):
+    """The 8-CTA thread-block-cluster tail (kernels_ctail.cu; z-slabs in distributed shared memory)
+    and the single-CTA tail + per-level kernels it replaces run the same arithmetic in the same
+    order: same iterates bit for bit, for a V-cycle from a non-zero guess, a full solve, and the
+    symmetric V-cycle of GMG-PCG.  Parity of either with the oracle is in the config tests."""
+    wl = random_workload(n, bc, seed=91)
+    a = make_gpu(wl, cluster_tail=1)
+    b = make_gpu(wl, cluster_tail=0)
+    try:
+        assert "cluster" in a.describe_plan() and "cluster" not in b.describe_plan()
+        rng = np.random.default_rng(92)
+        p0 = rng.standard_normal(wl.z.shape).astype(np.float32)
+        for om, sym in ((1.0, False), (0.8125, False), (1.0, True)):
+            assert torch.equal(a.op_vcycle(dev(p0), dev(wl.z), omega=om, symmetric=sym),
+                               b.op_vcycle(dev(p0), dev(wl.z), omega=om, symmetric=sym))
+        for solver in (gmg.GMG_RBGS, gmg.GMG_PCG):
+            pa = torch.zeros(wl.z.shape, dtype=torch.float32, device="cuda")
+            pb = torch.zeros_like(pa)
+            a.set_omega(1.0)
+            b.set_omega(1.0)
+            ra = a.solve(pa, dev(wl.z), tol=1e-5, maxiter=30, solver=solver)
+            rb = b.solve(pb, dev(wl.z), tol=1e-5, maxiter=30, solver=solver)
+            assert ra == rb and a.stats()["iterations"] == b.stats()["iterations"]
+            assert torch.equal(pa, pb)
+    finally:
+        a.close()
+        b.close()
+
+
 def test_non_default_stream_and_two_contexts():
     """Work is enqueued on the caller's stream; contexts are independent."""
     wl_a, wl_b = W.config3(5), W.config0()
