@@ -428,32 +428,52 @@ __global__ void __launch_bounds__(C::THREADS) k_residual_tiled(const ResArgs a) 
 // sweep's shared-memory planes costs more than this 8.5 B/cell streaming pass.
 __global__ void __launch_bounds__(256)
 k_prolong_add4(LevelGeom g, const float* __restrict__ e_c, float* __restrict__ p_f) {
+    // one work item = the (up to four) fine rows under one coarse row segment: the parent values
+    // are fetched once and up to four float4 of p are in flight per thread
     const int nx4 = g.n[0] >> 2;
-    const long long ngroups = g.N >> 2;
-    const int ncx = g.n[0] / g.c[0], ncy = g.n[1] / g.c[1];
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < ngroups;
+    const int cy = g.c[1], cz = g.c[2];
+    const int ncx = g.n[0] / g.c[0], ncy = g.n[1] / cy, ncz = g.n[2] / cz;
+    const long long items = (long long)nx4 * ncy * ncz;
+    const long long srow = nx4, splane = (long long)nx4 * g.n[1];   // in float4 units
+    float4* p4 = reinterpret_cast<float4*>(p_f);
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < items;
          t += (long long)gridDim.x * blockDim.x) {
         const long long row = t / nx4;
         const int i4 = (int)(t - row * nx4);
-        const int k = (int)(row / g.n[1]);
-        const int j = (int)(row - (long long)k * g.n[1]);
-        const long long pc = (long long)(k / g.c[2]) * ncy + (j / g.c[1]);
-        float4 v = *reinterpret_cast<const float4*>(p_f + 4 * t);
+        const int K = (int)(row / ncy);
+        const int J = (int)(row - (long long)K * ncy);
+        const long long pc = (long long)K * ncy + J;
+        float4 e;
         if (g.c[0] == 2) {
-            const float2 e = __ldg(reinterpret_cast<const float2*>(e_c + pc * ncx + 2 * i4));
-            v.x += e.x; v.y += e.x; v.z += e.y; v.w += e.y;
+            const float2 h = __ldg(reinterpret_cast<const float2*>(e_c + pc * ncx + 2 * i4));
+            e = make_float4(h.x, h.x, h.y, h.y);
         } else {
-            const float4 e = ldg4(e_c + pc * ncx + 4 * i4);
-            v.x += e.x; v.y += e.y; v.z += e.z; v.w += e.w;
+            e = ldg4(e_c + pc * ncx + 4 * i4);
         }
-        *reinterpret_cast<float4*>(p_f + 4 * t) = v;
+        const long long base = (long long)(K * cz) * splane + (long long)(J * cy) * srow + i4;
+        float4 v[2][2];
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int b = 0; b < 2; ++b)
+                if (a < cz && b < cy) v[a][b] = p4[base + a * splane + b * srow];
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int b = 0; b < 2; ++b)
+                if (a < cz && b < cy) {
+                    float4 w = v[a][b];
+                    w.x += e.x; w.y += e.y; w.z += e.z; w.w += e.w;
+                    p4[base + a * splane + b * srow] = w;
+                }
     }
 }
 
 void prolong_add4(const LevelGeom& g, const float* e_c, float* p_f, cudaStream_t s) {
-    const long long ngroups = g.N >> 2;
-    long long nb = (ngroups + 255) / 256;
+    const long long items = (g.N >> 2) / ((long long)g.c[1] * g.c[2]);
+    long long nb = (items + 255) / 256;
     if (nb > 148LL * 64) nb = 148LL * 64;
+    if (nb < 1) nb = 1;
     k_prolong_add4<<<(unsigned int)nb, 256, 0, s>>>(g, e_c, p_f);
 }
 
