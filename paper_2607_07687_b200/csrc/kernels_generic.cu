@@ -129,7 +129,20 @@ __global__ void __launch_bounds__(kThreads) k_fill(float* __restrict__ x, long l
         x[t] = v;
 }
 
+__global__ void __launch_bounds__(kThreads) k_fill4(float4* __restrict__ x, long long groups, float v) {
+    const float4 w = make_float4(v, v, v, v);
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < groups;
+         t += (long long)gridDim.x * blockDim.x)
+        x[t] = w;
+}
+
 void fill(float* x, long long N, float v, cudaStream_t s) {
+    if (N % 4 == 0 && (reinterpret_cast<size_t>(x) & 15) == 0) {
+        unsigned int nb = blocks_for(N >> 2);
+        if (nb > 148u * 16u) nb = 148u * 16u;
+        k_fill4<<<nb, kThreads, 0, s>>>(reinterpret_cast<float4*>(x), N >> 2, v);
+        return;
+    }
     unsigned int nb = blocks_for(N);
     if (nb > 148u * 16u) nb = 148u * 16u;
     k_fill<<<nb, kThreads, 0, s>>>(x, N, v);

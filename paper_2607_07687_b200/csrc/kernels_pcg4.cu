@@ -1,0 +1,200 @@
+// kernels_pcg4.cu -- the vector work of the (GMG-)PCG iteration (reading
+// O10), four x-adjacent cells (one float4) per thread and grid-stride loops sized
+// to the machine.  Per-cell arithmetic is that of the one-cell kernels in kernels_reduce.cu
+// (same apply7 / diag6 argument order); only the order in which the FP64 partial sums are
+// accumulated differs.  The launchers there dispatch here when nx % 4 == 0.
+#include "stencil.cuh"
+
+namespace gmgk {
+using namespace gmgd;
+
+static constexpr int kPT = 256;
+
+static inline unsigned int blocks4(long long groups) {
+    long long b = (groups + kPT - 1) / kPT;
+    if (b < 1) b = 1;
+    if (b > 148LL * 32) b = 148LL * 32;
+    return (unsigned int)b;
+}
+
+__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+__device__ __forceinline__ float4 splat4(float v) { return make_float4(v, v, v, v); }
+
+// Face weights of the four cells of group (i..i+3, j, k), wall faces zeroed (face_coeffs x 4).
+struct W4 {
+    float4 xl, xh, yl, yh, zl, zh;
+};
+__device__ __forceinline__ W4 weights4(const LevelGeom& g, const float* __restrict__ L, int i, int j, int k,
+                                       long long c) {
+    const long long N = g.N;
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const long long sy = nx, sz = (long long)nx * ny;
+    const float* Lx = L;
+    const float* Ly = L + N;
+    const float* Lz = L + 2 * N;
+    W4 w;
+    w.xl = ldg4(Lx + c);
+    float x4;  // lower x face of the cell after the group
+    if (i + 4 == nx) x4 = g.bc[0] ? 0.0f : __ldg(Lx + c - (nx - 4));
+    else x4 = __ldg(Lx + c + 4);
+    w.xh = make_float4(w.xl.y, w.xl.z, w.xl.w, x4);
+    if (i == 0 && g.bc[0]) w.xl.x = 0.0f;
+    w.yl = (j == 0 && g.bc[1]) ? splat4(0.0f) : ldg4(Ly + c);
+    w.yh = (j == ny - 1) ? (g.bc[1] ? splat4(0.0f) : ldg4(Ly + c - sy * (ny - 1))) : ldg4(Ly + c + sy);
+    w.zl = (k == 0 && g.bc[2]) ? splat4(0.0f) : ldg4(Lz + c);
+    w.zh = (k == nz - 1) ? (g.bc[2] ? splat4(0.0f) : ldg4(Lz + c - sz * (nz - 1))) : ldg4(Lz + c + sz);
+    return w;
+}
+
+__device__ __forceinline__ void unflat4(const LevelGeom& g, long long t, int& i, int& j, int& k) {
+    const int nx4 = g.n[0] >> 2;
+    const long long row = t / nx4;
+    i = 4 * (int)(t - row * nx4);
+    k = (int)(row / g.n[1]);
+    j = (int)(row - (long long)k * g.n[1]);
+}
+
+// q = A d on every cell ; red[slot] = d.q
+__global__ void __launch_bounds__(kPT)
+k_matvec_dot4(LevelGeom g, const float* __restrict__ L, const float* __restrict__ d, float* __restrict__ q,
+              ReduceBuf rb, int slot) {
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const long long sy = nx, sz = (long long)nx * ny;
+    const long long groups = g.N >> 2;
+    double acc = 0.0;
+    for (long long t = (long long)blockIdx.x * kPT + threadIdx.x; t < groups; t += (long long)gridDim.x * kPT) {
+        int i, j, k;
+        unflat4(g, t, i, j, k);
+        const long long c = 4 * t;
+        const W4 w = weights4(g, L, i, j, k, c);
+        const float4 dc = ldg4(d + c);
+        const float dxm = __ldg(d + ((i == 0) ? c + (nx - 1) : c - 1));
+        const float dxp = __ldg(d + ((i + 4 == nx) ? c - (nx - 4) : c + 4));
+        const float4 dyl = ldg4(d + ((j == 0) ? c + sy * (ny - 1) : c - sy));
+        const float4 dyh = ldg4(d + ((j == ny - 1) ? c - sy * (ny - 1) : c + sy));
+        const float4 dzl = ldg4(d + ((k == 0) ? c + sz * (nz - 1) : c - sz));
+        const float4 dzh = ldg4(d + ((k == nz - 1) ? c - sz * (nz - 1) : c + sz));
+        float4 o;
+        o.x = apply7(dc.x, w.xl.x, w.xh.x, w.yl.x, w.yh.x, w.zl.x, w.zh.x, dxm, dc.y, dyl.x, dyh.x, dzl.x, dzh.x);
+        o.y = apply7(dc.y, w.xl.y, w.xh.y, w.yl.y, w.yh.y, w.zl.y, w.zh.y, dc.x, dc.z, dyl.y, dyh.y, dzl.y, dzh.y);
+        o.z = apply7(dc.z, w.xl.z, w.xh.z, w.yl.z, w.yh.z, w.zl.z, w.zh.z, dc.y, dc.w, dyl.z, dyh.z, dzl.z, dzh.z);
+        o.w = apply7(dc.w, w.xl.w, w.xh.w, w.yl.w, w.yh.w, w.zl.w, w.zh.w, dc.z, dxp, dyl.w, dyh.w, dzl.w, dzh.w);
+        *reinterpret_cast<float4*>(q + c) = o;
+        acc += (double)dc.x * (double)o.x + (double)dc.y * (double)o.y + (double)dc.z * (double)o.z +
+               (double)dc.w * (double)o.w;
+    }
+    finish_reduction(acc, 0.0, false, rb, slot, 0);
+}
+
+// s = r / D on active cells, 0 elsewhere (Jacobi) ; red[slot] = r.s
+__global__ void __launch_bounds__(kPT)
+k_jacobi_apply4(LevelGeom g, const float* __restrict__ L, const float* __restrict__ r, float* __restrict__ s_out,
+                ReduceBuf rb, int slot) {
+    const long long groups = g.N >> 2;
+    double acc = 0.0;
+    for (long long t = (long long)blockIdx.x * kPT + threadIdx.x; t < groups; t += (long long)gridDim.x * kPT) {
+        int i, j, k;
+        unflat4(g, t, i, j, k);
+        const long long c = 4 * t;
+        const W4 w = weights4(g, L, i, j, k, c);
+        const float4 rv = ldg4(r + c);
+        const float Dx = diag6(w.xl.x, w.xh.x, w.yl.x, w.yh.x, w.zl.x, w.zh.x);
+        const float Dy = diag6(w.xl.y, w.xh.y, w.yl.y, w.yh.y, w.zl.y, w.zh.y);
+        const float Dz = diag6(w.xl.z, w.xh.z, w.yl.z, w.yh.z, w.zl.z, w.zh.z);
+        const float Dw = diag6(w.xl.w, w.xh.w, w.yl.w, w.yh.w, w.zl.w, w.zh.w);
+        float4 sv;
+        sv.x = (Dx != 0.0f) ? rv.x / Dx : 0.0f;
+        sv.y = (Dy != 0.0f) ? rv.y / Dy : 0.0f;
+        sv.z = (Dz != 0.0f) ? rv.z / Dz : 0.0f;
+        sv.w = (Dw != 0.0f) ? rv.w / Dw : 0.0f;
+        *reinterpret_cast<float4*>(s_out + c) = sv;
+        acc += (double)rv.x * (double)sv.x + (double)rv.y * (double)sv.y + (double)rv.z * (double)sv.z +
+               (double)rv.w * (double)sv.w;
+    }
+    finish_reduction(acc, 0.0, false, rb, slot, 0);
+}
+
+// p += alpha d ; r -= alpha q ; red[RED_RR] = r.r
+__global__ void __launch_bounds__(kPT)
+k_pcg_update_pr4(long long groups, float4* __restrict__ p, float4* __restrict__ r, const float4* __restrict__ d,
+                 const float4* __restrict__ q, ReduceBuf rb) {
+    const float alpha = (float)rb.sc->alpha;
+    double acc = 0.0;
+    for (long long t = (long long)blockIdx.x * kPT + threadIdx.x; t < groups; t += (long long)gridDim.x * kPT) {
+        const float4 dv = __ldg(d + t), qv = __ldg(q + t);
+        float4 pv = p[t], rv = r[t];
+        pv.x = fmaf(alpha, dv.x, pv.x); pv.y = fmaf(alpha, dv.y, pv.y);
+        pv.z = fmaf(alpha, dv.z, pv.z); pv.w = fmaf(alpha, dv.w, pv.w);
+        rv.x = fmaf(-alpha, qv.x, rv.x); rv.y = fmaf(-alpha, qv.y, rv.y);
+        rv.z = fmaf(-alpha, qv.z, rv.z); rv.w = fmaf(-alpha, qv.w, rv.w);
+        p[t] = pv;
+        r[t] = rv;
+        acc += (double)rv.x * (double)rv.x + (double)rv.y * (double)rv.y + (double)rv.z * (double)rv.z +
+               (double)rv.w * (double)rv.w;
+    }
+    finish_reduction(acc, 0.0, false, rb, RED_RR, 0);
+}
+
+// d = s + beta d
+__global__ void __launch_bounds__(kPT)
+k_pcg_update_d4(long long groups, float4* __restrict__ d, const float4* __restrict__ s_in,
+                const DevScalars* __restrict__ sc) {
+    const float beta = (float)sc->beta;
+    for (long long t = (long long)blockIdx.x * kPT + threadIdx.x; t < groups; t += (long long)gridDim.x * kPT) {
+        const float4 sv = __ldg(s_in + t);
+        float4 dv = d[t];
+        dv.x = fmaf(beta, dv.x, sv.x); dv.y = fmaf(beta, dv.y, sv.y);
+        dv.z = fmaf(beta, dv.z, sv.z); dv.w = fmaf(beta, dv.w, sv.w);
+        d[t] = dv;
+    }
+}
+
+// red[slot] = a.b
+__global__ void __launch_bounds__(kPT)
+k_dot4(long long groups, const float4* __restrict__ a, const float4* __restrict__ b, ReduceBuf rb, int slot) {
+    double acc = 0.0;
+    for (long long t = (long long)blockIdx.x * kPT + threadIdx.x; t < groups; t += (long long)gridDim.x * kPT) {
+        const float4 x = __ldg(a + t), y = __ldg(b + t);
+        acc += (double)x.x * (double)y.x + (double)x.y * (double)y.y + (double)x.z * (double)y.z +
+               (double)x.w * (double)y.w;
+    }
+    finish_reduction(acc, 0.0, false, rb, slot, 0);
+}
+
+static inline bool al16(const void* p) { return (reinterpret_cast<size_t>(p) & 15) == 0; }
+
+bool matvec_dot4(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot,
+                 cudaStream_t s) {
+    if (g.n[0] % 4 != 0 || !al16(L) || !al16(d) || !al16(q)) return false;
+    k_matvec_dot4<<<blocks4(g.N >> 2), kPT, 0, s>>>(g, L, d, q, rb, slot);
+    return true;
+}
+bool jacobi_apply4(const LevelGeom& g, const float* L, const float* r, float* s_out, ReduceBuf rb, int slot,
+                   cudaStream_t st) {
+    if (g.n[0] % 4 != 0 || !al16(L) || !al16(r) || !al16(s_out)) return false;
+    k_jacobi_apply4<<<blocks4(g.N >> 2), kPT, 0, st>>>(g, L, r, s_out, rb, slot);
+    return true;
+}
+bool pcg_update_pr4(long long N, float* p, float* r, const float* d, const float* q, ReduceBuf rb,
+                    cudaStream_t st) {
+    if (N % 4 != 0 || !al16(p) || !al16(r) || !al16(d) || !al16(q)) return false;
+    k_pcg_update_pr4<<<blocks4(N >> 2), kPT, 0, st>>>(N >> 2, reinterpret_cast<float4*>(p),
+                                                    reinterpret_cast<float4*>(r),
+                                                    reinterpret_cast<const float4*>(d),
+                                                    reinterpret_cast<const float4*>(q), rb);
+    return true;
+}
+bool pcg_update_d4(long long N, float* d, const float* s_in, const DevScalars* sc, cudaStream_t st) {
+    if (N % 4 != 0 || !al16(d) || !al16(s_in)) return false;
+    k_pcg_update_d4<<<blocks4(N >> 2), kPT, 0, st>>>(N >> 2, reinterpret_cast<float4*>(d),
+                                                   reinterpret_cast<const float4*>(s_in), sc);
+    return true;
+}
+bool dot4(long long N, const float* a, const float* b, ReduceBuf rb, int slot, cudaStream_t s) {
+    if (N % 4 != 0 || !al16(a) || !al16(b)) return false;
+    k_dot4<<<blocks4(N >> 2), kPT, 0, s>>>(N >> 2, reinterpret_cast<const float4*>(a),
+                                          reinterpret_cast<const float4*>(b), rb, slot);
+    return true;
+}
+
+}  // namespace gmgk

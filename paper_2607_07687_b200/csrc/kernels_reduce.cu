@@ -15,6 +15,13 @@ using namespace gmgd;
 
 static constexpr int kRT = 256;  // threads per reduction block
 
+// float4 versions (kernels_pcg4.cu); false = shape or alignment not eligible
+bool matvec_dot4(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot, cudaStream_t s);
+bool jacobi_apply4(const LevelGeom& g, const float* L, const float* r, float* s_out, ReduceBuf rb, int slot, cudaStream_t st);
+bool pcg_update_pr4(long long N, float* p, float* r, const float* d, const float* q, ReduceBuf rb, cudaStream_t st);
+bool pcg_update_d4(long long N, float* d, const float* s_in, const DevScalars* sc, cudaStream_t st);
+bool dot4(long long N, const float* a, const float* b, ReduceBuf rb, int slot, cudaStream_t s);
+
 static inline unsigned int reduce_blocks(long long N) {
     long long b = (N + (long long)kRT * 8 - 1) / ((long long)kRT * 8);
     if (b < 1) b = 1;
@@ -82,9 +89,11 @@ k_dot(long long N, const float* __restrict__ a, const float* __restrict__ b, Red
 }
 
 void norm2(long long N, const float* r, ReduceBuf rb, int slot, cudaStream_t s) {
+    if (dot4(N, r, r, rb, slot, s)) return;
     k_dot<<<reduce_blocks(N), kRT, 0, s>>>(N, r, r, rb, slot);
 }
 void dot(long long N, const float* a, const float* b, ReduceBuf rb, int slot, cudaStream_t s) {
+    if (dot4(N, a, b, rb, slot, s)) return;
     k_dot<<<reduce_blocks(N), kRT, 0, s>>>(N, a, b, rb, slot);
 }
 
@@ -123,6 +132,7 @@ k_matvec_dot(LevelGeom g, const float* __restrict__ L, const float* __restrict__
 
 void matvec_dot(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb,
                 int slot, cudaStream_t s) {
+    if (matvec_dot4(g, L, d, q, rb, slot, s)) return;
     k_matvec_dot<<<reduce_blocks(g.N), kRT, 0, s>>>(g, L, d, q, rb, slot);
 }
 
@@ -145,6 +155,7 @@ k_pcg_update_pr(long long N, float* __restrict__ p, float* __restrict__ r,
 void pcg_update_pr(const LevelGeom& g, const float* L, float* p, float* r, const float* d,
                    const float* q, float* s_out, int jacobi, ReduceBuf rb, cudaStream_t st) {
     (void)L; (void)s_out; (void)jacobi;
+    if (pcg_update_pr4(g.N, p, r, d, q, rb, st)) return;
     k_pcg_update_pr<<<reduce_blocks(g.N), kRT, 0, st>>>(g.N, p, r, d, q, rb);
 }
 
@@ -161,6 +172,7 @@ k_pcg_update_d(long long N, float* __restrict__ d, const float* __restrict__ s_i
 void pcg_update_d(long long N, float* d, const float* s_in, const DevScalars* sc, int first,
                   cudaStream_t st) {
     (void)first;
+    if (pcg_update_d4(N, d, s_in, sc, st)) return;
     k_pcg_update_d<<<reduce_blocks(N), kRT, 0, st>>>(N, d, s_in, sc);
 }
 
@@ -184,6 +196,7 @@ k_jacobi_apply(LevelGeom g, const float* __restrict__ L, const float* __restrict
 
 void jacobi_apply(const LevelGeom& g, const float* L, const float* r, float* s_out, ReduceBuf rb,
                   int slot, cudaStream_t st) {
+    if (jacobi_apply4(g, L, r, s_out, rb, slot, st)) return;
     k_jacobi_apply<<<reduce_blocks(g.N), kRT, 0, st>>>(g, L, r, s_out, rb, slot);
 }
 
