@@ -147,6 +147,12 @@ int gmg_solve(gmg_ctx* ctx, float* p_dev, const float* z_dev, float tol, int max
 int gmg_solve_host(gmg_ctx* ctx, float* p_host, const float* z_host, float tol, int maxiter,
                    int solver, void* stream);
 
+/* Cold-start variant: the initial guess is zero (the first pressure solve of a run; PAPER.md:51
+ * "impulsive" starts), so no guess crosses the bus -- the staging buffer is zeroed on the device.
+ * p_host is written only (the solution).  Otherwise as gmg_solve_host. */
+int gmg_solve_host_cold(gmg_ctx* ctx, float* p_host_out, const float* z_host, float tol, int maxiter,
+                        int solver, void* stream);
+
 int gmg_stats(const gmg_ctx* ctx, gmg_stats_t* out);
 /* Relative residual history of the last solve: out[k] = ||r_k|| / ||z||, k = 0..iterations.
  * Returns the number of entries written (<= cap). */

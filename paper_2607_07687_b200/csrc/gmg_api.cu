@@ -745,6 +745,21 @@ extern "C" int gmg_solve_host(gmg_ctx* c, float* p_host, const float* z_host, fl
     return rc;
 }
 
+extern "C" int gmg_solve_host_cold(gmg_ctx* c, float* p_host_out, const float* z_host, float tol, int maxiter,
+                                   int solver, void* stream) {
+    if (!c || !p_host_out || !z_host) return GMG_EINVAL;
+    if (!c->ws_set || !c->coeffs_set) { SET_ERR(c, "gmg_solve_host_cold before setup"); return GMG_ESTATE; }
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t bytes = (size_t)c->g[0].N * sizeof(float);
+    CUDA_TRY(c, cudaMemcpyAsync(c->stage_z, z_host, bytes, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(c, cudaMemsetAsync(c->stage_p, 0, bytes, s));
+    const int rc = gmg_solve(c, c->stage_p, c->stage_z, tol, maxiter, solver, stream);
+    if (rc < 0) return rc;
+    CUDA_TRY(c, cudaMemcpyAsync(p_host_out, c->stage_p, bytes, cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(c, cudaStreamSynchronize(s));
+    return rc;
+}
+
 extern "C" int gmg_stats(const gmg_ctx* c, gmg_stats_t* out) {
     if (!c || !out) return GMG_EINVAL;
     *out = c->stats;

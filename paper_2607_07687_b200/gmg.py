@@ -68,6 +68,7 @@ SIGNATURES = {
     "gmg_set_coeffs": (C.c_int, [_vp, _vp, _vp]),
     "gmg_solve": (C.c_int, [_vp, _vp, _vp, C.c_float, C.c_int, C.c_int, _vp]),
     "gmg_solve_host": (C.c_int, [_vp, _vp, _vp, C.c_float, C.c_int, C.c_int, _vp]),
+    "gmg_solve_host_cold": (C.c_int, [_vp, _vp, _vp, C.c_float, C.c_int, C.c_int, _vp]),
     "gmg_stats": (C.c_int, [_vp, C.POINTER(Stats)]),
     "gmg_history": (C.c_int, [_vp, C.POINTER(C.c_double), C.c_int]),
     "gmg_omega_history": (C.c_int, [_vp, C.POINTER(C.c_double), C.c_int]),
@@ -228,6 +229,16 @@ class GMG:
         return self._check(lib.gmg_solve_host(self._h, _vp(_ptr(p_host)), _vp(_ptr(z_host)),
                                               float(tol), int(maxiter), int(solver),
                                               self._stream()), allow_warning=True)
+
+    def solve_host_cold(self, p_host_out: torch.Tensor, z_host: torch.Tensor, tol=1e-4, maxiter=50,
+                        solver=GMG_RBGS):
+        """Zero initial guess (made on the device); p_host_out receives the solution."""
+        for t in (p_host_out, z_host):
+            assert (not t.is_cuda) and t.dtype == torch.float32 and t.is_contiguous()
+            assert t.numel() == self.n[0] * self.n[1] * self.n[2]
+        return self._check(lib.gmg_solve_host_cold(self._h, _vp(_ptr(p_host_out)), _vp(_ptr(z_host)),
+                                                   float(tol), int(maxiter), int(solver),
+                                                   self._stream()), allow_warning=True)
 
     def stats(self) -> dict:
         s = Stats()

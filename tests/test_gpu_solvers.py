@@ -271,6 +271,12 @@ def test_solve_host_matches_device_solve():
         rc2 = g.solve_host(ph, zh, tol=1e-4, maxiter=50)
         assert rc2 == rc and g.stats()["iterations"] == st["iterations"]
         assert np.array_equal(ph.numpy().astype(np.float64), p)
+        # cold start: the zero guess is made on the device, the host buffer is output only
+        pc = torch.full(wl.z.shape, 7.0, dtype=torch.float32).pin_memory()
+        g.set_omega(1.0)
+        rc3 = g.solve_host_cold(pc, zh, tol=1e-4, maxiter=50)
+        assert rc3 == rc and g.stats()["iterations"] == st["iterations"]
+        assert torch.equal(pc, ph)
     finally:
         g.close()
 
