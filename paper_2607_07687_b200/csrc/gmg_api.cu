@@ -26,6 +26,8 @@ void residual_norm2(const LevelGeom& g, const float* L, const float* p, const fl
 bool residual_and_ref_norm2_bulk(const LevelGeom& g, const float* L, const float* p, const float* b,
                                  ReduceBuf rb, int slot_rr, int slot_ref, cudaStream_t s);
 void prolong_add4(const LevelGeom& g, const float* e_c, float* p_f, cudaStream_t s);
+bool matvec_dot_bulk(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot,
+                     cudaStream_t s);
 bool tma_shape_ok(const LevelGeom& g);
 int configure();
 }  // namespace gmgf
@@ -547,7 +549,9 @@ static void pcg_body(gmg_ctx* c, float* p, int gmg_precond, LoopCtl lc, cudaStre
     }
     gmgk::ctl_pcg_beta(c->sc, s);
     gmgk::pcg_update_d(N, c->pcg_d, c->pcg_s, c->sc, 0, s);
-    gmgk::matvec_dot(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rbuf(c), RED_DQ, s);
+    if (!(c->prm.fast_path && c->tma_ok[0] &&
+          gmgf::matvec_dot_bulk(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rbuf(c), RED_DQ, s)))
+        gmgk::matvec_dot(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rbuf(c), RED_DQ, s);
     gmgk::ctl_pcg_alpha(c->sc, s);
     gmgk::pcg_update_pr(c->g[0], c->lv[0].L, p, c->pcg_r, c->pcg_d, c->pcg_q, nullptr, 0, rbuf(c), s);
     gmgk::ctl_pcg_check(c->sc, c->hist, lc.cond, lc.use_cond, s);

@@ -17,6 +17,20 @@ static inline unsigned int blocks4(long long groups) {
     return (unsigned int)b;
 }
 
+// Grid for the stencil kernels: one grid-stride "wave" covers about one z plane, so the z +- 1
+// neighbours a wave reads are the planes the previous and the next wave stream -- a few planes of
+// five arrays, which stay in L2 -- instead of a window several planes deep whose edges are
+// fetched twice from DRAM (measured 1.75x the algorithmic traffic with 148 x 32 blocks at 1024^3).
+static inline unsigned int blocks_plane(const LevelGeom& g) {
+    const long long plane_groups = ((long long)g.n[0] * g.n[1]) >> 2;
+    long long b = (plane_groups + kPT - 1) / kPT;
+    if (b < 148LL * 4) b = 148LL * 4;
+    if (b > 148LL * 32) b = 148LL * 32;
+    const long long all = ((g.N >> 2) + kPT - 1) / kPT;
+    if (b > all) b = all < 1 ? 1 : all;
+    return (unsigned int)b;
+}
+
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 __device__ __forceinline__ float4 splat4(float v) { return make_float4(v, v, v, v); }
 
@@ -46,12 +60,14 @@ __device__ __forceinline__ W4 weights4(const LevelGeom& g, const float* __restri
     return w;
 }
 
-__device__ __forceinline__ void unflat4(const LevelGeom& g, long long t, int& i, int& j, int& k) {
-    const int nx4 = g.n[0] >> 2;
-    const long long row = t / nx4;
+// group index -> (i, j, k); 32-bit arithmetic (a level has fewer than 2^31 cells)
+__device__ __forceinline__ void unflat4(const LevelGeom& g, unsigned int t, int& i, int& j, int& k) {
+    const unsigned int nx4 = (unsigned int)g.n[0] >> 2, ny = (unsigned int)g.n[1];
+    const unsigned int row = t / nx4;
     i = 4 * (int)(t - row * nx4);
-    k = (int)(row / g.n[1]);
-    j = (int)(row - (long long)k * g.n[1]);
+    const unsigned int kk = row / ny;
+    k = (int)kk;
+    j = (int)(row - kk * ny);
 }
 
 // q = A d on every cell ; red[slot] = d.q
@@ -60,12 +76,12 @@ k_matvec_dot4(LevelGeom g, const float* __restrict__ L, const float* __restrict_
               ReduceBuf rb, int slot) {
     const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
     const long long sy = nx, sz = (long long)nx * ny;
-    const long long groups = g.N >> 2;
+    const unsigned int groups = (unsigned int)(g.N >> 2);
     double acc = 0.0;
-    for (long long t = (long long)blockIdx.x * kPT + threadIdx.x; t < groups; t += (long long)gridDim.x * kPT) {
+    for (unsigned int t = blockIdx.x * kPT + threadIdx.x; t < groups; t += gridDim.x * kPT) {
         int i, j, k;
         unflat4(g, t, i, j, k);
-        const long long c = 4 * t;
+        const long long c = 4LL * t;
         const W4 w = weights4(g, L, i, j, k, c);
         const float4 dc = ldg4(d + c);
         const float dxm = __ldg(d + ((i == 0) ? c + (nx - 1) : c - 1));
@@ -90,12 +106,12 @@ k_matvec_dot4(LevelGeom g, const float* __restrict__ L, const float* __restrict_
 __global__ void __launch_bounds__(kPT)
 k_jacobi_apply4(LevelGeom g, const float* __restrict__ L, const float* __restrict__ r, float* __restrict__ s_out,
                 ReduceBuf rb, int slot) {
-    const long long groups = g.N >> 2;
+    const unsigned int groups = (unsigned int)(g.N >> 2);
     double acc = 0.0;
-    for (long long t = (long long)blockIdx.x * kPT + threadIdx.x; t < groups; t += (long long)gridDim.x * kPT) {
+    for (unsigned int t = blockIdx.x * kPT + threadIdx.x; t < groups; t += gridDim.x * kPT) {
         int i, j, k;
         unflat4(g, t, i, j, k);
-        const long long c = 4 * t;
+        const long long c = 4LL * t;
         const W4 w = weights4(g, L, i, j, k, c);
         const float4 rv = ldg4(r + c);
         const float Dx = diag6(w.xl.x, w.xh.x, w.yl.x, w.yh.x, w.zl.x, w.zh.x);
@@ -166,13 +182,13 @@ static inline bool al16(const void* p) { return (reinterpret_cast<size_t>(p) & 1
 bool matvec_dot4(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot,
                  cudaStream_t s) {
     if (g.n[0] % 4 != 0 || !al16(L) || !al16(d) || !al16(q)) return false;
-    k_matvec_dot4<<<blocks4(g.N >> 2), kPT, 0, s>>>(g, L, d, q, rb, slot);
+    k_matvec_dot4<<<blocks_plane(g), kPT, 0, s>>>(g, L, d, q, rb, slot);
     return true;
 }
 bool jacobi_apply4(const LevelGeom& g, const float* L, const float* r, float* s_out, ReduceBuf rb, int slot,
                    cudaStream_t st) {
     if (g.n[0] % 4 != 0 || !al16(L) || !al16(r) || !al16(s_out)) return false;
-    k_jacobi_apply4<<<blocks4(g.N >> 2), kPT, 0, st>>>(g, L, r, s_out, rb, slot);
+    k_jacobi_apply4<<<blocks_plane(g), kPT, 0, st>>>(g, L, r, s_out, rb, slot);
     return true;
 }
 bool pcg_update_pr4(long long N, float* p, float* r, const float* d, const float* q, ReduceBuf rb,

@@ -1,5 +1,5 @@
 // kernels_residual.cu -- k_residual_bulk: residual fused with the restriction (MODE 0) or with the
-// squared-norm reduction (MODE 1) on the big levels, fed by TMA (cp.async.bulk.tensor + mbarrier)
+// squared-norm reduction (MODE 1, 2), or the CG mat-vec q = A d with d.q (MODE 3), on the big levels, fed by TMA (cp.async.bulk.tensor + mbarrier)
 // like the sweep.  r = b - A p on active cells, 0 elsewhere (readings O1, O9);
 // restriction = sum over the children (O6; PAPER.md:39 coarse-grid correction, 47 anisotropic
 // coarsening: any factor pattern c in {1,2}^3); BASELINE.json:north_star "a residual kernel fused
@@ -273,6 +273,12 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
             const float A1 = apply7(oA.y, lxA.y, lxA.z, lyA.y, lyB.y, lzA.y, lzhA.y, oA.x, oA.z, ym.y, oB.y, zmA.y, zpA.y);
             const float A2 = apply7(oA.z, lxA.z, lxA.w, lyA.z, lyB.z, lzA.z, lzhA.z, oA.y, oA.w, ym.z, oB.z, zmA.z, zpA.z);
             const float A3 = apply7(oA.w, lxA.w, lxhA, lyA.w, lyB.w, lzA.w, lzhA.w, oA.z, xpA, ym.w, oB.w, zmA.w, zpA.w);
+            if (MODE == 3) {  // mat-vec: q = A d on every cell (inactive rows are all-zero), d.q
+                if (vA) {
+                    *reinterpret_cast<float4*>(a.b_c + (size_t)gz * plane + (size_t)gyA * nx + xl) = make_float4(A0, A1, A2, A3);
+                    acc += ((double)oA.x * A0 + (double)oA.y * A1) + ((double)oA.z * A2 + (double)oA.w * A3);
+                }
+            }
             rA[0] = (diag6(lxA.x, lxA.y, lyA.x, lyB.x, lzA.x, lzhA.x) != 0.0f) ? bA.x - A0 : 0.0f;
             rA[1] = (diag6(lxA.y, lxA.z, lyA.y, lyB.y, lzA.y, lzhA.y) != 0.0f) ? bA.y - A1 : 0.0f;
             rA[2] = (diag6(lxA.z, lxA.w, lyA.z, lyB.z, lzA.z, lzhA.z) != 0.0f) ? bA.z - A2 : 0.0f;
@@ -281,12 +287,20 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
             const float B1 = apply7(oB.y, lxB.y, lxB.z, lyB.y, lyC.y, lzB.y, lzhB.y, oB.x, oB.z, oA.y, yp.y, zmB.y, zpB.y);
             const float B2 = apply7(oB.z, lxB.z, lxB.w, lyB.z, lyC.z, lzB.z, lzhB.z, oB.y, oB.w, oA.z, yp.z, zmB.z, zpB.z);
             const float B3 = apply7(oB.w, lxB.w, lxhB, lyB.w, lyC.w, lzB.w, lzhB.w, oB.z, xpB, oA.w, yp.w, zmB.w, zpB.w);
+            if (MODE == 3) {
+                if (vB) {
+                    *reinterpret_cast<float4*>(a.b_c + (size_t)gz * plane + (size_t)gyB * nx + xl) = make_float4(B0, B1, B2, B3);
+                    acc += ((double)oB.x * B0 + (double)oB.y * B1) + ((double)oB.z * B2 + (double)oB.w * B3);
+                }
+            }
             rB[0] = (diag6(lxB.x, lxB.y, lyB.x, lyC.x, lzB.x, lzhB.x) != 0.0f) ? bB.x - B0 : 0.0f;
             rB[1] = (diag6(lxB.y, lxB.z, lyB.y, lyC.y, lzB.y, lzhB.y) != 0.0f) ? bB.y - B1 : 0.0f;
             rB[2] = (diag6(lxB.z, lxB.w, lyB.z, lyC.z, lzB.z, lzhB.z) != 0.0f) ? bB.z - B2 : 0.0f;
             rB[3] = (diag6(lxB.w, lxhB, lyB.w, lyC.w, lzB.w, lzhB.w) != 0.0f) ? bB.w - B3 : 0.0f;
         }
-        if (MODE >= 1) {
+        if (MODE == 3) {
+            // stored above; rA / rB are unused (dead code)
+        } else if (MODE >= 1) {
             if (vA) acc += ((double)rA[0] * rA[0] + (double)rA[1] * rA[1]) + ((double)rA[2] * rA[2] + (double)rA[3] * rA[3]);
             if (vB) acc += ((double)rB[0] * rB[0] + (double)rB[1] * rB[1]) + ((double)rB[2] * rB[2] + (double)rB[3] * rB[3]);
             if (MODE == 2) {  // reference norm of the solve loop: b^2 over ACTIVE cells (reading O9)
@@ -351,7 +365,7 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
         if (++kb == C::NB) { kb = 0; kpar ^= 1u; }
         if (++gz == nz) gz = 0;
     }
-    if (MODE == 1) finish_reduction(acc, 0.0, false, a.rb, a.slot, 0);
+    if (MODE == 1 || MODE == 3) finish_reduction(acc, 0.0, false, a.rb, a.slot, 0);
     if (MODE == 2) finish_reduction(acc, acc_b, true, a.rb, a.slot, a.slot2);
 }
 
@@ -417,10 +431,23 @@ bool residual_and_ref_norm2_bulk(const LevelGeom& g, const float* L, const float
     return launch_res_bulk<2>(a, s);
 }
 
+// q = A d and red[slot] = d.q in one TMA-fed pass (the CG mat-vec, reading O10); the b stream of
+// the kernel is pointed at d and ignored.
+bool matvec_dot_bulk(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot,
+                     cudaStream_t s) {
+    ResBulkArgs a;
+    a.g = g; a.L = L; a.p = d; a.b = d; a.b_c = q; a.p_c = nullptr;
+    a.rb = rb;
+    a.slot = slot;
+    a.slot2 = 0;
+    return launch_res_bulk<3>(a, s);
+}
+
 int configure_residual_bulk() {
     cudaError_t e = cudaFuncSetAttribute(k_residual_bulk<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ResBulkCfg::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_residual_bulk<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ResBulkCfg::SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_residual_bulk<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ResBulkCfg::SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_residual_bulk<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ResBulkCfg::SMEM);
     return (int)e;
 }
 

@@ -365,6 +365,35 @@ def test_cluster_tail_is_bit_identical_to_single_cta_tail(n, bc):
         b.close()
 
 
+@pytest.mark.parametrize("n,bc", [((128, 40, 16), (0, 0, 0)), ((256, 20, 12), (1, 0, 1))])
+def test_pcg_with_tma_matvec_matches_oracle_and_plain_kernels(n, bc):
+    """The CG mat-vec of the big levels is a mode of the TMA-fed residual kernel (q = A d, d.q in one
+    pass).  Forced on here (tma_min_cells=0): same iteration counts as the oracle (+-1) and as the
+    float4 kernels, and the same pressure to rounding (the mat-vec arithmetic per cell is identical;
+    only the order of the FP64 partial sums of d.q differs)."""
+    wl = random_workload(n, bc, seed=95)
+    act = W.active_mask(wl.L, wl.bc)
+    a = make_gpu(wl, tma_min_cells=0)
+    b = make_gpu(wl, tma_min_cells=-1)
+    h = make_oracle(wl)
+    try:
+        for solver, osolver in ((gmg.PCG, oracle.PCG), (gmg.GMG_PCG, oracle.GMG_PCG)):
+            ref = h.solve(osolver, wl.z, tol=1e-4, maxiter=800)
+            out = []
+            for g in (a, b):
+                p = torch.zeros(wl.z.shape, dtype=torch.float32, device="cuda")
+                rc = g.solve(p, dev(wl.z), tol=1e-4, maxiter=800, solver=solver)
+                assert rc == gmg.OK and ref["status"] == 0, (solver, rc, ref["status"], ref["iterations"])
+                assert abs(g.stats()["iterations"] - ref["iterations"]) <= 1
+                out.append((g.stats()["iterations"], host(p)))
+            assert abs(out[0][0] - out[1][0]) <= 1
+            if out[0][0] == out[1][0]:
+                assert rel_l2_demeaned(out[0][1], out[1][1], act) <= TOL_P
+    finally:
+        a.close()
+        b.close()
+
+
 def test_non_default_stream_and_two_contexts():
     """Work is enqueued on the caller's stream; contexts are independent."""
     wl_a, wl_b = W.config3(5), W.config0()
