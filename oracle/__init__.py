@@ -5,7 +5,7 @@ bench.py's cpu_baseline / --impl reference legs.  The product package
 (paper_2607_07687_b200) never imports this module and this module never imports it.
 
 Arrays: numpy float64, C-ordered [k][j][i]; L float64 (3,nz,ny,nx) for the single-operator
-calls, float32 for Hierarchy (the same FP32 bits the GPU gets).  Readings O1..O11 are
+calls, float32 for Hierarchy (the same FP32 bits the GPU gets).  Readings O1..O12 are
 documented in gmg_oracle.c and DESIGN.md.
 """
 import ctypes as C
@@ -57,7 +57,13 @@ _solve_rbgs = _sig("gmgo_solve_gmg_rbgs", C.c_int, C.c_void_p, _dp, _dp, C.c_dou
 _solve_pcg = _sig("gmgo_solve_pcg", C.c_int, C.c_void_p, C.c_int, _dp, _dp, C.c_double, C.c_int, _dp,
                   C.POINTER(C.c_int), C.POINTER(C.c_double))
 
-PCG, GMG_PCG, GMG_RBGS = 0, 1, 2
+_cgsmooth = _sig("gmgo_level_cg_smooth", None, C.c_void_p, C.c_int, _dp, _dp, C.c_int)
+_vcycle_cgs = _sig("gmgo_vcycle_cgs", None, C.c_void_p, _dp, _dp)
+_solve_cgs = _sig("gmgo_solve_gmg_cgs", C.c_int, C.c_void_p, _dp, _dp, C.c_double, C.c_int, _dp,
+                  C.POINTER(C.c_int), C.POINTER(C.c_double))
+
+# GMG_CGS = the paper's own "GMG-PCG": GMG whose smoother is Jacobi-PCG (reading O12)
+PCG, GMG_PCG, GMG_RBGS, GMG_CGS = 0, 1, 2, 3
 
 
 def _n_of(a):
@@ -214,6 +220,17 @@ class Hierarchy:
         _lsweeps(self._h, lev, q, _f64(b), float(omega), int(count), int(first_colour))
         return q
 
+    def level_cg_smooth(self, lev, x, b, iters):
+        """m Jacobi-PCG iterations restarted from x on level lev (reading O12a)."""
+        q = _f64(x).copy()
+        _cgsmooth(self._h, lev, q, _f64(b), int(iters))
+        return q
+
+    def vcycle_cgs(self, x, b):
+        q = _f64(x).copy()
+        _vcycle_cgs(self._h, q, _f64(b))
+        return q
+
     def solve(self, solver, z, p0=None, tol=1e-4, maxiter=50):
         """Returns dict(p, iterations, status, history, omegas, true_res)."""
         z = _f64(z)
@@ -227,6 +244,11 @@ class Hierarchy:
                             C.byref(rref))
             return dict(p=p, iterations=k, status=status.value, history=hist[:k + 1].copy(),
                         omegas=om[:k].copy(), r_ref=rref.value, true_res=float(hist[k]))
+        if solver == GMG_CGS:
+            rref = C.c_double(0.0)
+            k = _solve_cgs(self._h, p, z, float(tol), int(maxiter), hist, C.byref(status), C.byref(rref))
+            return dict(p=p, iterations=k, status=status.value, history=hist[:k + 1].copy(),
+                        r_ref=rref.value, true_res=float(hist[k]))
         tr = C.c_double(0.0)
         k = _solve_pcg(self._h, 0 if solver == PCG else 1, p, z, float(tol), int(maxiter), hist,
                        C.byref(status), C.byref(tr))

@@ -584,3 +584,111 @@ void gmgo_project(const int n[3], const int bc[3], const double *L, const double
                     u[(i64)d * N + c] -= w * (p[c] - pm);
                 }
 }
+
+/* ------------------------------------------------------------------------------------
+ * N2 (PAPER.md:43 S3.1 "PCG can be used as a smoother", Table 1's
+ * middle row "GMG-PCG" at PAPER.md:37): the SAME V(nu1,nu2) cycle as O7 with every group of
+ * RBGS sweeps replaced by as many Jacobi-preconditioned CG iterations, restarted from the
+ * current iterate of that level.  The paper gives no parameter for it: reading O12.
+ *
+ * O12a, the smoother: m CG iterations on A^l x = b from the given x (A is negative
+ * semi-definite, so r.s and d.q are negative and alpha positive):
+ *     r = b - A x (0 on inactive cells, O9);  s = r/D (0 on inactive);  d = s;  rho = r.s; rho0 = rho
+ *     repeat m times:  q = A d;  alpha = rho/(d.q);  x += alpha d;  r -= alpha q;
+ *                      s = r/D;  rho' = r.s;  d = s + (rho'/rho) d;  rho = rho'
+ * Every level is singular (periodic axes and homogeneous Neumann walls only: constants span the
+ * null space), and CG -- unlike Gauss-Seidel -- amplifies any component of the right-hand side
+ * along the null vector without bound (d.q -> 0 there).  Restricted residuals carry such a
+ * component at rounding level, so the initial residual is made compatible first:
+ *     r -= mean of r over the active cells.
+ * Guards: the iteration stops early when rho is not < 0 at entry, when d.q is not < 0, or once
+ * |rho| <= 1e-8 |rho0| (preconditioned residual reduced by 1e-4, far more than a smoother or a
+ * coarsest-level solve needs; below that an FP32 run approaches its own rounding noise).
+ * ---------------------------------------------------------------------------------- */
+#define GMGO_CGS_FREEZE 1e-8
+
+void gmgo_level_cg_smooth(gmgo_hier *h, int l, double *x, const double *b, int m) {
+    const int *n = h->n[l];
+    i64 N = ncells(n);
+    if (m <= 0) return;
+    double *r = (double *)malloc(sizeof(double) * (size_t)N);
+    double *s = (double *)malloc(sizeof(double) * (size_t)N);
+    double *d = (double *)malloc(sizeof(double) * (size_t)N);
+    double *q = (double *)malloc(sizeof(double) * (size_t)N);
+    double *D = (double *)malloc(sizeof(double) * (size_t)N);
+    gmgo_diag(n, h->bc, h->L[l], D);
+    gmgo_residual(n, h->bc, h->L[l], x, b, r);
+    double sum = 0.0, cnt = 0.0;
+    for (i64 c = 0; c < N; ++c)
+        if (D[c] != 0.0) { sum += r[c]; cnt += 1.0; }
+    if (cnt > 0.0)
+        for (i64 c = 0; c < N; ++c)
+            if (D[c] != 0.0) r[c] -= sum / cnt;
+    for (i64 c = 0; c < N; ++c) s[c] = (D[c] != 0.0) ? r[c] / D[c] : 0.0;
+    memcpy(d, s, sizeof(double) * (size_t)N);
+    double rho = gmgo_dot(n, r, s);
+    const double rho0 = rho;
+    int frozen = !(rho < 0.0);
+    for (int it = 0; it < m && !frozen; ++it) {
+        gmgo_apply(n, h->bc, h->L[l], d, q);
+        double dq = gmgo_dot(n, d, q);
+        if (!(dq < 0.0)) break;
+        double alpha = rho / dq;
+        for (i64 c = 0; c < N; ++c) { x[c] += alpha * d[c]; r[c] -= alpha * q[c]; }
+        if (it == m - 1) break;
+        for (i64 c = 0; c < N; ++c) s[c] = (D[c] != 0.0) ? r[c] / D[c] : 0.0;
+        double rho_new = gmgo_dot(n, r, s);
+        double beta = rho_new / rho;
+        for (i64 c = 0; c < N; ++c) d[c] = s[c] + beta * d[c];
+        rho = rho_new;
+        if (!(fabs(rho) > GMGO_CGS_FREEZE * fabs(rho0))) frozen = 1;
+    }
+    free(r); free(s); free(d); free(q); free(D);
+}
+
+/* O12b: the cycle.  Coarsest level: nuc CG iterations from the zero guess. */
+static void vcycle_cgs_rec(gmgo_hier *h, int l, double *x, const double *b) {
+    if (l == h->nlev - 1) {
+        gmgo_level_cg_smooth(h, l, x, b, h->nuc);
+        return;
+    }
+    gmgo_level_cg_smooth(h, l, x, b, h->nu1);
+    i64 Nf = ncells(h->n[l]);
+    double *r = (l == 0) ? h->r : (double *)malloc(sizeof(double) * (size_t)Nf);
+    gmgo_residual(h->n[l], h->bc, h->L[l], x, b, r);
+    gmgo_restrict_sum(h->n[l], h->c[l], r, h->b[l + 1]);
+    if (l != 0) free(r);
+    memset(h->x[l + 1], 0, sizeof(double) * (size_t)ncells(h->n[l + 1]));
+    vcycle_cgs_rec(h, l + 1, h->x[l + 1], h->b[l + 1]);
+    gmgo_prolong_add(h->n[l], h->c[l], h->x[l + 1], x);
+    gmgo_level_cg_smooth(h, l, x, b, h->nu2);
+}
+
+void gmgo_vcycle_cgs(gmgo_hier *h, double *x, const double *b) { vcycle_cgs_rec(h, 0, x, b); }
+
+/* O12c: the solve loop is O9's, without the relaxation factor: V-cycles until
+ * ||z - A p||_2 <= tol ||z||_2 over active cells or maxiter cycles. */
+int gmgo_solve_gmg_cgs(gmgo_hier *h, double *p, const double *z, double tol, int maxiter,
+                       double *history, int *status, double *r_ref_out) {
+    const int *n = h->n[0];
+    double r_ref = active_norm(h, z);
+    if (r_ref_out) *r_ref_out = r_ref;
+    if (r_ref == 0.0) {
+        if (history) history[0] = 0.0;
+        *status = 0;
+        return 0;
+    }
+    gmgo_residual(n, h->bc, h->L[0], p, z, h->r);
+    double rho = gmgo_norm2(n, h->r);
+    int k = 0;
+    if (history) history[0] = rho / r_ref;
+    while (rho > tol * r_ref && k < maxiter) {
+        vcycle_cgs_rec(h, 0, p, z);
+        ++k;
+        gmgo_residual(n, h->bc, h->L[0], p, z, h->r);
+        rho = gmgo_norm2(n, h->r);
+        if (history) history[k] = rho / r_ref;
+    }
+    *status = (rho <= tol * r_ref) ? 0 : 1;
+    return k;
+}

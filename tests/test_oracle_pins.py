@@ -215,7 +215,7 @@ def _demean(p, act):
     return np.where(act, p - p[act].mean(), 0.0)
 
 
-@pytest.mark.parametrize("solver", [oracle.GMG_RBGS, oracle.PCG, oracle.GMG_PCG])
+@pytest.mark.parametrize("solver", [oracle.GMG_RBGS, oracle.PCG, oracle.GMG_PCG, oracle.GMG_CGS])
 def test_solvers_reach_dense_solution_8cubed(solver):
     rng = np.random.default_rng(5)
     n, bc = (8, 8, 8), (1, 0, 1)
@@ -290,6 +290,107 @@ def test_pcg_properties_and_ordering():
     assert pcg["status"] == 0 and mg["status"] == 0
     assert mg["iterations"] <= 4 < 20 < pcg["iterations"] < 120
     assert abs(pcg["true_res"] - pcg["history"][-1]) < 1e-8
+
+
+# --------------------------------------------------------------------------------------
+# N2: the paper's own "GMG-PCG" = GMG with a Jacobi-PCG smoother (reading O12)
+# --------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [(1, 0, 1), (0, 0, 0), (1, 1, 1)])
+@pytest.mark.parametrize("m", [1, 2, 4])
+def test_cg_smoother_is_the_krylov_energy_minimiser(bc, m):
+    """m preconditioned CG iterations from x0 give THE minimiser of the energy
+    phi(x) = 1/2 x'(-A)x + x'b over x0 + span{v, Tv, .., T^(m-1)v}, v = M^-1 r0, T = M^-1 A
+    (the textbook characterisation of PCG), computed here densely from the face-assembled A."""
+    rng = np.random.default_rng(100 + m)
+    n = (8, 6, 4)
+    L32 = rand_L(rng, n, zero_frac=0.15).astype(np.float32)
+    L32[:, 1:3, 2:4, 3:5] = 0.0                       # a solid block: inactive cells
+    Le = W.effective_L(L32, bc)
+    act = W.active_mask(L32, bc)
+    assert not act.all()
+    A = dense_by_faces(n, bc, Le)
+    Dg = np.diag(A).copy()
+    Minv = np.where(Dg != 0.0, 1.0 / np.where(Dg != 0.0, Dg, 1.0), 0.0)
+    b = W.project_compatible(rng.standard_normal((n[2], n[1], n[0])), act)
+    x0 = rng.standard_normal(b.shape)
+    r0 = np.where(act.ravel(), b.ravel() - A @ x0.ravel(), 0.0)
+    v = Minv * r0
+    K = [v]
+    for _ in range(m - 1):
+        K.append(Minv * (A @ K[-1]))
+    K = np.stack(K, axis=1)
+    y = np.linalg.solve(K.T @ A @ K, K.T @ r0)
+    x_ref = x0.ravel() + K @ y
+    H = oracle.Hierarchy(n, bc, L32, n_min=64)        # one level
+    assert H.nlev == 1
+    x = H.level_cg_smooth(0, x0, b, m)
+    scale = np.abs(x_ref - x0.ravel()).max()
+    assert np.abs(x.ravel() - x_ref).max() < 1e-9 * max(scale, 1.0)
+    assert np.array_equal(x[~act], x0[~act])          # inactive cells untouched
+    # energy of the error never increases with more iterations
+    xs, _ = _dense_solution(n, bc, Le, b)
+    def energy(xx):
+        e = (xx - xs).ravel()
+        return float(-(e @ (A @ e)))
+    e_prev = energy(x0)
+    for mm in range(1, m + 1):
+        e_now = energy(H.level_cg_smooth(0, x0, b, mm))
+        assert e_now <= e_prev * (1 + 1e-12)
+        e_prev = e_now
+
+
+def test_cg_smoother_guards():
+    """Zero residual, zero count, and a long run on a singular 4^3 level stay put / finite."""
+    rng = np.random.default_rng(7)
+    n, bc = (4, 4, 4), (0, 0, 0)
+    L32 = np.ones((3, 4, 4, 4), dtype=np.float32)
+    H = oracle.Hierarchy(n, bc, L32)
+    assert H.nlev == 1
+    x0 = rng.standard_normal((4, 4, 4))
+    b = oracle.apply_A(L32, bc, x0)
+    assert np.array_equal(H.level_cg_smooth(0, x0, b, 5), x0)        # r0 = 0: nothing moves
+    b2 = rng.standard_normal((4, 4, 4))
+    b2 -= b2.mean()
+    assert np.array_equal(H.level_cg_smooth(0, x0, b2, 0), x0)       # m = 0
+    x = H.level_cg_smooth(0, np.zeros_like(b2), b2, 500)             # far past convergence
+    assert np.all(np.isfinite(x))
+    r = oracle.residual(L32, bc, x, b2)
+    assert np.linalg.norm(r) < 1e-4 * np.linalg.norm(b2)
+    # an inconsistent right-hand side (non-zero mean on a singular level) must not blow up either
+    x = H.level_cg_smooth(0, np.zeros_like(b2), b2 + 1e-7, 500)
+    assert np.all(np.isfinite(x)) and np.abs(x).max() < 1e3
+
+
+def test_gmg_cgs_invariants_and_cycle_structure():
+    w = W.config0()
+    H = oracle.Hierarchy(w.n, w.bc, w.L)
+    z = w.z.astype(np.float64)
+    out = H.solve(oracle.GMG_CGS, z, tol=w.tol, maxiter=w.maxiter)
+    assert out["status"] == 0 and 1 <= out["iterations"] <= 12
+    h = out["history"]
+    assert abs(h[0] - 1.0) < 1e-12 and h[-1] <= w.tol
+    r = oracle.residual(w.L, w.bc, out["p"], z)
+    assert abs(r.sum() - z.sum()) < 1e-9
+    # prefix property and the cycle as a composition of its pinned parts (one 2-level case)
+    o2 = oracle.Hierarchy(w.n, w.bc, w.L).solve(oracle.GMG_CGS, z, tol=0.0, maxiter=1)
+    assert np.allclose(o2["history"], h[:2], rtol=1e-12)
+    n, bc = (8, 8, 4), (1, 0, 1)
+    rng = np.random.default_rng(3)
+    L32 = rng.uniform(0, 1, (3, 4, 8, 8)).astype(np.float32)
+    H2 = oracle.Hierarchy(n, bc, L32)
+    assert H2.nlev == 2
+    H2.set_params(nu1=2, nu2=3, nuc=5)
+    b = W.project_compatible(rng.standard_normal((4, 8, 8)), W.active_mask(L32, bc))
+    x0 = rng.standard_normal(b.shape)
+    _, c0 = H2.shape(0)
+    x = H2.level_cg_smooth(0, x0, b, 2)
+    bc_ = oracle.restrict_sum(H2.level_residual(0, x, b), c0)
+    e = H2.level_cg_smooth(1, np.zeros_like(bc_), bc_, 5)
+    x = H2.level_cg_smooth(0, oracle.prolong_add(x, e, c0), b, 3)
+    assert np.allclose(H2.vcycle_cgs(x0, b), x, rtol=0, atol=1e-13)
+    # zero rhs: 0 iterations, p untouched
+    o3 = H.solve(oracle.GMG_CGS, np.zeros_like(z), p0=np.ones_like(z))
+    assert o3["iterations"] == 0 and np.all(o3["p"] == 1.0)
 
 
 # --------------------------------------------------------------------------------------
