@@ -146,8 +146,10 @@ def run_reference(args):
 
 
 def solver_table(gmg, W, torch, device, names):
-    """#iterations, final residual, ms and ns/cell of PCG, GMG-PCG and GMG-RBGS per workload
-    (the columns of the paper's Table 1; device-resident, best of 3)."""
+    """#iterations, final residual, ms and ns/cell of PCG, GMG-PCG, GMG-CGS and GMG-RBGS per workload
+    (the columns of the paper's Table 1; device-resident, best of 3).  GMG-PCG =
+    V-cycle-preconditioned CG (BASELINE.json's meaning); GMG-CGS = the V-cycle with a Jacobi-PCG
+    smoother (the paper's meaning of "GMG-PCG", reading O12)."""
     out = {}
     for name in names:
         wl = W.by_name(name)
@@ -158,6 +160,7 @@ def solver_table(gmg, W, torch, device, names):
         p = torch.zeros_like(z)
         row = {}
         for label, solver, cap in (("PCG", gmg.PCG, 5000), ("GMG-PCG", gmg.GMG_PCG, wl.maxiter),
+                                   ("GMG-CGS", gmg.GMG_CGS, wl.maxiter),
                                    ("GMG-RBGS", gmg.GMG_RBGS, wl.maxiter)):
             best = None
             for _ in range(3):
@@ -335,7 +338,12 @@ def run_ours(args):
             p.zero_()
             rc = g.solve(p, z, tol=tol, maxiter=maxiter, solver=gmg.GMG_PCG)
             st2 = g.stats()
+            p.zero_()
+            rc = g.solve(p, z, tol=tol, maxiter=maxiter, solver=gmg.GMG_CGS)
+            st3 = g.stats()
             table[args.workload] = {
+                "GMG-CGS": {"iterations": st3["iterations"], "resid": st3["resid_final_rel"],
+                            "ms": st3["gpu_ms"], "ns_per_cell": st3["gpu_ms"] * 1e6 / N},
                 "GMG-RBGS": {"iterations": iters[-1], "resid": final["resid_final_rel"],
                              "ms": final["gpu_ms"], "ns_per_cell": final["gpu_ms"] * 1e6 / N},
                 "GMG-PCG": {"iterations": st2["iterations"], "resid": st2["resid_final_rel"],

@@ -44,7 +44,14 @@ extern "C" {
 typedef struct gmg_ctx gmg_ctx;
 
 enum { GMG_BC_PERIODIC = 0, GMG_BC_NEUMANN = 1 };
-enum { GMG_PCG = 0, GMG_GMG_PCG = 1, GMG_GMG_RBGS = 2 };
+/* GMG_GMG_PCG: CG preconditioned by one symmetric V-cycle (BASELINE.json's "GMG-preconditioned PCG",
+ * reading O11).  GMG_GMG_CGS: the paper's own "GMG-PCG" of Table 1 -- the V-cycle
+ * whose smoother is Jacobi-PCG instead of RBGS (reading O12): every group of nu sweeps becomes nu CG
+ * iterations restarted from the level's current iterate, the restart residual made mean-free over
+ * the active cells (every level is singular; CG amplifies a null-space component without bound),
+ * and a smoothing ends early once d.q is not < 0, |r.s| <= 1e-8 |r.s at the restart|, or a step
+ * length above 16 n_max^2 comes out (a direction that drifted into the null space). */
+enum { GMG_PCG = 0, GMG_GMG_PCG = 1, GMG_GMG_RBGS = 2, GMG_GMG_CGS = 3 };
 enum { GMG_COARSEN_ANISO = 0, GMG_COARSEN_ISO = 1 };
 enum {
     GMG_OK = 0,
@@ -82,7 +89,7 @@ typedef struct {
 typedef struct {
     int solver;
     int status;             /* the code gmg_solve returned */
-    int iterations;         /* V-cycles (GMG-RBGS) or CG iterations (PCG, GMG-PCG) */
+    int iterations;         /* V-cycles (GMG-RBGS, GMG-CGS) or CG iterations (PCG, GMG-PCG) */
     int levels;
     double omega_final;     /* relaxation factor after the solve (persists in the ctx) */
     double resid_ref;       /* ||z||_2 over active cells */
@@ -135,7 +142,7 @@ int gmg_set_coeffs(gmg_ctx* ctx, const float* L_dev, void* stream);
 
 /* Solve A p = z.  p_dev: in = initial guess, out = solution (in place).  Stops when
  * ||z - A p||_2 <= tol * ||z||_2 (norms over active cells, reading O9) or after maxiter
- * iterations (tol = 0 runs exactly maxiter).  solver: GMG_PCG, GMG_GMG_PCG, GMG_GMG_RBGS.
+ * iterations (tol = 0 runs exactly maxiter).  solver: GMG_PCG, GMG_GMG_PCG, GMG_GMG_RBGS, GMG_GMG_CGS.
  * The whole iteration runs on the device (a CUDA-graph WHILE loop); the host reads one
  * status block at the end.  Returns GMG_OK / GMG_NOT_CONVERGED or an error. */
 int gmg_solve(gmg_ctx* ctx, float* p_dev, const float* z_dev, float tol, int maxiter,
@@ -188,6 +195,11 @@ int gmg_op_prolong(gmg_ctx* ctx, int lev, const float* e_coarse_dev, float* p_fi
  * = the variant used as CG preconditioner (reading O11). */
 int gmg_op_vcycle(gmg_ctx* ctx, float* p_dev, const float* z_dev, float omega, int symmetric,
                   void* stream);
+/* The smoother of GMG_GMG_CGS (reading O12, "PCG can be used as a smoother"): iters
+ * Jacobi-PCG iterations on A^lev x = b restarted from x (in place), and one whole cycle of it on
+ * level 0 (V(nu_pre, nu_post), nu_coarse iterations on the coarsest level). */
+int gmg_op_cg_smooth(gmg_ctx* ctx, int lev, float* x_dev, const float* b_dev, int iters, void* stream);
+int gmg_op_vcycle_cgs(gmg_ctx* ctx, float* p_dev, const float* z_dev, void* stream);
 /* sqrt(sum r^2) of a level-lev array (deterministic two-stage reduction). */
 int gmg_op_norm2(gmg_ctx* ctx, int lev, const float* r_dev, double* out_host, void* stream);
 

@@ -601,9 +601,13 @@ void gmgo_project(const int n[3], const int bc[3], const double *L, const double
  * along the null vector without bound (d.q -> 0 there).  Restricted residuals carry such a
  * component at rounding level, so the initial residual is made compatible first:
  *     r -= mean of r over the active cells.
- * Guards: the iteration stops early when rho is not < 0 at entry, when d.q is not < 0, or once
+ * Guards: the iteration stops early when rho is not < 0 at entry, when d.q is not < 0, once
  * |rho| <= 1e-8 |rho0| (preconditioned residual reduced by 1e-4, far more than a smoother or a
- * coarsest-level solve needs; below that an FP32 run approaches its own rounding noise).
+ * coarsest-level solve needs; below that an FP32 run approaches its own rounding noise), or when
+ * a step length alpha > 16 n_max^2 comes out (n_max = the level's largest extent).  In exact
+ * arithmetic 1/alpha is bounded below by the smallest non-zero eigenvalue of D^-1 A, which is
+ * about (pi/n_max)^2/6 for uniform coefficients, i.e. alpha <= 0.6 n_max^2: a step 26 times
+ * longer than that is a direction that has drifted into the null space, not a solve.
  * ---------------------------------------------------------------------------------- */
 #define GMGO_CGS_FREEZE 1e-8
 
@@ -628,12 +632,16 @@ void gmgo_level_cg_smooth(gmgo_hier *h, int l, double *x, const double *b, int m
     memcpy(d, s, sizeof(double) * (size_t)N);
     double rho = gmgo_dot(n, r, s);
     const double rho0 = rho;
+    int nmax = n[0] > n[1] ? n[0] : n[1];
+    if (n[2] > nmax) nmax = n[2];
+    const double alpha_cap = 16.0 * (double)nmax * (double)nmax;
     int frozen = !(rho < 0.0);
     for (int it = 0; it < m && !frozen; ++it) {
         gmgo_apply(n, h->bc, h->L[l], d, q);
         double dq = gmgo_dot(n, d, q);
         if (!(dq < 0.0)) break;
         double alpha = rho / dq;
+        if (alpha > alpha_cap) break;
         for (i64 c = 0; c < N; ++c) { x[c] += alpha * d[c]; r[c] -= alpha * q[c]; }
         if (it == m - 1) break;
         for (i64 c = 0; c < N; ++c) s[c] = (D[c] != 0.0) ? r[c] / D[c] : 0.0;

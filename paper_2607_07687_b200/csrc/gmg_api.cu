@@ -76,7 +76,7 @@ struct gmg_ctx {
     gmg_stats_t stats;
     cudaEvent_t ev0, ev1;
     cudaStream_t cap_a, cap_b;  // internal streams used only for graph capture
-    GraphSlot slots[3];
+    GraphSlot slots[4];
     long long n_launch;   // launch counter of the section being enqueued
     char err[512];
 };
@@ -475,6 +475,75 @@ static void enqueue_vcycle(gmg_ctx* c, float* p0, const float* b0, const float* 
         smooth(c, l, P(l), B(l), omega, c->prm.nu_post, post_first, c->lv[l + 1].p, s);
 }
 
+// ---- N2: the paper's own "GMG-PCG" (PAPER.md:43 S3.1, Table 1 at PAPER.md:37; reading O12) -------
+// m Jacobi-PCG iterations on A^l x = b restarted from x.  The four CG vectors are the level-0
+// sized PCG vectors of the workspace on EVERY level: the CG state does not survive the visit to
+// the coarser levels (the post-smoothing restarts), so the levels can share them.
+static void cg_smooth(gmg_ctx* c, int l, float* x, const float* b, int m, cudaStream_t s) {
+    if (m <= 0) return;
+    const LevelGeom& g = c->g[l];
+    const float* L = c->lv[l].L;
+    float *r = c->pcg_r, *d = c->pcg_d, *q = c->pcg_q, *sv = c->pcg_s;
+    gmgk::cgs_residual_sum(g, L, x, b, r, rbuf(c), s);
+    gmgk::cgs_start(g, L, r, d, rbuf(c), s);       // r -= mean; d = r/D; rho = r.d
+    gmgk::ctl_cgs_begin(c->sc, g, s);
+    c->n_launch += 3;
+    for (int it = 0; it < m; ++it) {
+        if (!(c->prm.fast_path && c->tma_ok[l] && gmgf::matvec_dot_bulk(g, L, d, q, rbuf(c), RED_DQ, s)))
+            gmgk::matvec_dot(g, L, d, q, rbuf(c), RED_DQ, s);
+        gmgk::ctl_cgs_alpha(c->sc, s);
+        gmgk::pcg_update_pr(g, L, x, r, d, q, nullptr, 0, rbuf(c), s);
+        c->n_launch += 3;
+        if (it == m - 1) break;
+        gmgk::jacobi_apply(g, L, r, sv, rbuf(c), RED_RS, s);
+        gmgk::ctl_cgs_beta(c->sc, s);
+        gmgk::pcg_update_d(g.N, d, sv, c->sc, 0, s);
+        c->n_launch += 3;
+    }
+}
+
+// The V(nu_pre, nu_post) cycle of reading O7 with every group of sweeps replaced by as many CG
+// iterations (O12b); the coarsest level gets nu_coarse iterations from the zero guess.
+static void enqueue_vcycle_cgs(gmg_ctx* c, float* p0, const float* b0, cudaStream_t s) {
+    const int nlev = c->nlev;
+    auto P = [&](int l) { return l == 0 ? p0 : c->lv[l].p; };
+    auto B = [&](int l) { return l == 0 ? b0 : (const float*)c->lv[l].b; };
+    for (int l = 0; l < nlev - 1; ++l) {
+        cg_smooth(c, l, P(l), B(l), c->prm.nu_pre, s);
+        if (c->fast_rr[l])
+            gmgf::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, c->tma_ok[l], s);
+        else
+            gmgk::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, s);
+        c->n_launch += 1;
+    }
+    if (nlev == 1) {
+        cg_smooth(c, 0, p0, b0, c->prm.nu_coarse, s);
+        return;
+    }
+    cg_smooth(c, nlev - 1, P(nlev - 1), B(nlev - 1), c->prm.nu_coarse, s);
+    for (int l = nlev - 2; l >= 0; --l) {
+        if (c->fast_sweep[l] && c->tma_ok[l] && gmgf::tma_shape_ok(c->g[l])) gmgf::prolong_add4(c->g[l], c->lv[l + 1].p, P(l), s);
+        else gmgk::prolong_add(c->g[l], c->lv[l + 1].p, P(l), s);
+        c->n_launch += 1;
+        cg_smooth(c, l, P(l), B(l), c->prm.nu_post, s);
+    }
+}
+
+// Algorithmic bytes of that cycle: a smoothing of m iterations moves 48 B/cell at the restart
+// (residual + sum 24, mean-free start 24), 44 per iteration (mat-vec 20, x/r update 24) and 32
+// between iterations (Jacobi 20, direction update 12).
+static double vcycle_cgs_bytes(const gmg_ctx* c) {
+    auto sm = [](int m) { return m > 0 ? 48.0 + 44.0 * m + 32.0 * (m - 1) : 0.0; };
+    double total = 0.0;
+    for (int l = 0; l < c->nlev; ++l) {
+        const double N = (double)c->g[l].N;
+        const double m = (double)(c->g[l].c[0] * c->g[l].c[1] * c->g[l].c[2]);
+        if (l == c->nlev - 1) total += N * sm(c->prm.nu_coarse);
+        else total += N * (sm(c->prm.nu_pre) + sm(c->prm.nu_post) + (20.0 + 4.0 / m) + (8.0 + 4.0 / m));
+    }
+    return total + 20.0 * (double)c->g[0].N;
+}
+
 // Algorithmic HBM bytes of one V-cycle + its stopping-test norm.
 static double vcycle_bytes(const gmg_ctx* c, bool with_norm) {
     double total = 0.0;
@@ -520,8 +589,9 @@ static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStrea
     gmgk::ctl_begin(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
     c->n_launch += 1;
 }
-static void rbgs_body(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
-    enqueue_vcycle(c, p, z, &c->sc->omega_f, 0, s);
+static void rbgs_body(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s, bool cgs = false) {
+    if (cgs) enqueue_vcycle_cgs(c, p, z, s);
+    else enqueue_vcycle(c, p, z, &c->sc->omega_f, 0, s);
     level0_residual_norm2(c, p, z, s);
     gmgk::ctl_rbgs_cycle_end(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
     c->n_launch += 2;
@@ -563,21 +633,23 @@ static void pcg_post(gmg_ctx* c, float* p, const float* z, cudaStream_t s) {
     c->n_launch += 1;
 }
 
-static void enqueue_init(gmg_ctx* c, float tol, int maxiter, cudaStream_t s) {
-    gmgk::ctl_init(c->sc, (double)tol, maxiter, c->prm.adaptive, (double)c->prm.omega_min,
+static void enqueue_init(gmg_ctx* c, float tol, int maxiter, int solver, cudaStream_t s) {
+    // the relaxation factor belongs to the RBGS smoother: the CG-smoothed cycle leaves it alone
+    gmgk::ctl_init(c->sc, (double)tol, maxiter, solver == GMG_GMG_CGS ? 0 : c->prm.adaptive, (double)c->prm.omega_min,
                    (double)c->prm.omega_down, (double)c->prm.omega_up, s);
     c->n_launch += 1;
 }
 
 static void enqueue_pre(gmg_ctx* c, int solver, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
-    if (solver == GMG_GMG_RBGS) rbgs_pre(c, p, z, lc, s); else pcg_pre(c, p, z, lc, s);
+    if (solver == GMG_GMG_RBGS || solver == GMG_GMG_CGS) rbgs_pre(c, p, z, lc, s); else pcg_pre(c, p, z, lc, s);
 }
 static void enqueue_body(gmg_ctx* c, int solver, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
     if (solver == GMG_GMG_RBGS) rbgs_body(c, p, z, lc, s);
+    else if (solver == GMG_GMG_CGS) rbgs_body(c, p, z, lc, s, true);
     else pcg_body(c, p, solver == GMG_GMG_PCG, lc, s);
 }
 static void enqueue_post(gmg_ctx* c, int solver, float* p, const float* z, cudaStream_t s) {
-    if (solver != GMG_GMG_RBGS) pcg_post(c, p, z, s);
+    if (solver != GMG_GMG_RBGS && solver != GMG_GMG_CGS) pcg_post(c, p, z, s);
 }
 
 // Whole solve as ONE graph: init, pre, WHILE(cond){body}, post.
@@ -594,7 +666,7 @@ static int build_graph(gmg_ctx* c, GraphSlot& slot, int solver, float* p, const 
     CUDA_TRY(c, cudaStreamBeginCaptureToGraph(c->cap_a, graph, nullptr, nullptr, 0,
                                               cudaStreamCaptureModeRelaxed));
     c->n_launch = 0;
-    enqueue_init(c, tol, maxiter, c->cap_a);
+    enqueue_init(c, tol, maxiter, solver, c->cap_a);
     enqueue_pre(c, solver, p, z, lc, c->cap_a);
     slot.n_pre = c->n_launch;
     // conditional WHILE node after everything captured so far
@@ -650,7 +722,7 @@ static int ensure_history(gmg_ctx* c, int maxiter) {
 extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int maxiter, int solver,
                          void* stream) {
     if (!c) return GMG_EINVAL;
-    if (!p || !z || !(tol >= 0.0f) || maxiter < 0 || solver < GMG_PCG || solver > GMG_GMG_RBGS) {
+    if (!p || !z || !(tol >= 0.0f) || maxiter < 0 || solver < GMG_PCG || solver > GMG_GMG_CGS) {
         SET_ERR(c, "gmg_solve: invalid argument");
         return GMG_EINVAL;
     }
@@ -688,7 +760,7 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
         lc.cond = 0;
         lc.use_cond = 0;
         c->n_launch = 0;
-        enqueue_init(c, tol, maxiter, s);
+        enqueue_init(c, tol, maxiter, solver, s);
         enqueue_pre(c, solver, p, z, lc, s);
         while (true) {
             CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
@@ -709,7 +781,7 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
     c->hist_host.assign((size_t)it + 1, 0.0);
     c->omegas_host.assign((size_t)it, 0.0);
     CUDA_TRY(c, cudaMemcpy(c->hist_host.data(), c->hist, sizeof(double) * (it + 1), cudaMemcpyDeviceToHost));
-    if (solver == GMG_GMG_RBGS && it > 0)
+    if ((solver == GMG_GMG_RBGS || solver == GMG_GMG_CGS) && it > 0)
         CUDA_TRY(c, cudaMemcpy(c->omegas_host.data(), c->omegas, sizeof(double) * it, cudaMemcpyDeviceToHost));
     float ms = 0.0f;
     CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1));
@@ -721,13 +793,14 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
     st.omega_final = h.omega;
     st.resid_ref = h.r_ref;
     st.resid_init_rel = c->hist_host[0];
-    if (solver == GMG_GMG_RBGS) st.resid_final_rel = c->hist_host[it];
+    if (solver == GMG_GMG_RBGS || solver == GMG_GMG_CGS) st.resid_final_rel = c->hist_host[it];
     else st.resid_final_rel = (h.r_ref > 0.0) ? sqrt(h.red[RED_RR]) / h.r_ref : 0.0;
     st.gpu_ms = ms;
     st.kernel_launches = launches;
     st.history_len = it + 1;
     const double N0 = (double)c->g[0].N;
     if (solver == GMG_GMG_RBGS) st.bytes_algorithmic = 20.0 * N0 + it * vcycle_bytes(c, true);  // loop entry: one pass over p, z, L
+    else if (solver == GMG_GMG_CGS) st.bytes_algorithmic = 20.0 * N0 + it * vcycle_cgs_bytes(c);
     else if (solver == GMG_PCG) st.bytes_algorithmic = 60.0 * N0 + it * 64.0 * N0;
     else st.bytes_algorithmic = 60.0 * N0 + it * (vcycle_bytes(c, false) + 52.0 * N0);
     if (h.status == GMG_EBREAKDOWN) SET_ERR(c, "PCG breakdown: d.q == 0 at iteration %d", it);
@@ -846,6 +919,18 @@ extern "C" int gmg_op_vcycle(gmg_ctx* c, float* p, const float* z, float omega, 
     HOOK_PROLOGUE(p && z)
     gmgk::ctl_set_hook_omega(c->sc, omega, s);
     enqueue_vcycle(c, p, z, &c->sc->omega_hook, symmetric ? 1 : 0, s);
+    HOOK_EPILOGUE()
+}
+
+extern "C" int gmg_op_cg_smooth(gmg_ctx* c, int lev, float* x, const float* b, int iters, void* stream) {
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && x && b && iters >= 0)
+    cg_smooth(c, lev, x, b, iters, s);
+    HOOK_EPILOGUE()
+}
+
+extern "C" int gmg_op_vcycle_cgs(gmg_ctx* c, float* p, const float* z, void* stream) {
+    HOOK_PROLOGUE(p && z)
+    enqueue_vcycle_cgs(c, p, z, s);
     HOOK_EPILOGUE()
 }
 

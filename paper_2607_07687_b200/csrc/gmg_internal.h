@@ -43,8 +43,13 @@ struct DevScalars {
     int status;        // GMG_OK, GMG_NOT_CONVERGED, GMG_EBREAKDOWN
     int done;          // 1: loop finished
     int adaptive;
-    int pad;
+    int cgs_frozen;    // CG smoother (reading O12): 1 = the remaining iterations leave x untouched
+    double cgs_rho0;   // r.s at the restart of the CG smoother
+    double cgs_alpha_cap;  // longest step the CG smoother accepts on the current level
 };
+
+// CG smoother: stop once |r.s| <= this * |r.s at the restart| (reading O12)
+#define GMG_CGS_FREEZE 1e-8
 
 enum {
     RED_RREF = 0,  // sum z^2 over active cells
@@ -52,8 +57,18 @@ enum {
     RED_DQ = 2,    // d.q
     RED_RS = 3,    // r.s
     RED_HOOK = 4,  // gmg_op_norm2
-    RED_CHECK = 5  // coefficient check: count of bad values
+    RED_CHECK = 5, // coefficient check: count of bad values
+    RED_CGS_SUM = 6,  // CG smoother: sum of the restart residual over active cells
+    RED_CGS_CNT = 7   // CG smoother: number of active cells
 };
+
+#ifdef __CUDACC__
+// mean of the restart residual over the active cells, as the kernels subtract it
+__device__ __forceinline__ float cgs_mean(const DevScalars* sc) {
+    const double cnt = sc->red[RED_CGS_CNT];
+    return cnt > 0.0 ? (float)(sc->red[RED_CGS_SUM] / cnt) : 0.0f;
+}
+#endif
 
 // Tail: levels small enough to live in one CTA's shared memory, run as ONE kernel.
 struct TailArgs {
@@ -146,6 +161,16 @@ void ctl_pcg_alpha(DevScalars* sc, cudaStream_t s);
 void ctl_pcg_check(DevScalars* sc, double* hist, cudaGraphConditionalHandle cond, int use_cond,
                    cudaStream_t s);
 void ctl_set_hook_omega(DevScalars* sc, float omega, cudaStream_t s);
+
+// CG smoother of the paper's GMG-PCG (kernels_cgs.cu, reading O12)
+// r = b - A x (0 on inactive cells); red[CGS_SUM] = sum r, red[CGS_CNT] = number of active cells
+void cgs_residual_sum(const LevelGeom& g, const float* L, const float* x, const float* b, float* r,
+                      ReduceBuf rb, cudaStream_t s);
+// r -= mean over active cells; d = r/D; red[RS] = r.d
+void cgs_start(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s);
+void ctl_cgs_begin(DevScalars* sc, const LevelGeom& g, cudaStream_t s);
+void ctl_cgs_alpha(DevScalars* sc, cudaStream_t s);
+void ctl_cgs_beta(DevScalars* sc, cudaStream_t s);
 void ctl_set_omega(DevScalars* sc, double omega, cudaStream_t s);
 
 }  // namespace gmgk

@@ -1,0 +1,138 @@
+// kernels_cgs.cu -- the Jacobi-PCG SMOOTHER of the paper's own "GMG-PCG" (
+// PAPER.md:43 S3.1 "PCG can be used as a smoother", Table 1's middle row at PAPER.md:37;
+// DESIGN.md reading O12): m preconditioned CG iterations on A^l x = b restarted from the
+// current iterate of a level.  The iteration itself reuses the PCG vector kernels
+// (kernels_reduce.cu / kernels_pcg4.cu / the TMA-fed mat-vec); this file holds what the restart
+// needs -- the residual with its sum over the active cells, the mean-free start r -= mean,
+// d = r/D, rho = r.d -- and the single-thread control kernels with the smoother's guards.
+// Per-cell arithmetic in the one-cell and the float4 kernels is identical.
+#include "stencil.cuh"
+
+namespace gmgk {
+using namespace gmgd;
+
+static constexpr int kCT = 256;
+
+// float4 versions (kernels_pcg4.cu); false = shape or alignment not eligible
+bool cgs_residual_sum4(const LevelGeom& g, const float* L, const float* x, const float* b, float* r,
+                       ReduceBuf rb, cudaStream_t s);
+bool cgs_start4(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s);
+
+static inline unsigned int cgs_blocks(long long N) {
+    long long b = (N + (long long)kCT * 8 - 1) / ((long long)kCT * 8);
+    if (b < 1) b = 1;
+    if (b > GMG_REDUCE_MAX_BLOCKS) b = GMG_REDUCE_MAX_BLOCKS;
+    return (unsigned int)b;
+}
+
+__device__ __forceinline__ void cgs_unflat(const LevelGeom& g, long long t, int& i, int& j, int& k) {
+    const int nx = g.n[0], ny = g.n[1];
+    const long long row = t / nx;
+    i = (int)(t - row * nx);
+    k = (int)(row / ny);
+    j = (int)(row - (long long)k * ny);
+}
+
+// r = b - A x on active cells, 0 elsewhere ; red[CGS_SUM] = sum r ; red[CGS_CNT] = #active
+__global__ void __launch_bounds__(kCT)
+k_cgs_residual_sum(LevelGeom g, const float* __restrict__ L, const float* __restrict__ x,
+                   const float* __restrict__ b, float* __restrict__ r, ReduceBuf rb) {
+    double sum = 0.0, cnt = 0.0;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < g.N;
+         t += (long long)gridDim.x * blockDim.x) {
+        int i, j, k;
+        cgs_unflat(g, t, i, j, k);
+        const Cell c = cell_stencil(g, L, x, i, j, k);
+        const bool act = c.D != 0.0f;
+        const float rv = act ? b[t] - c.Ap : 0.0f;
+        r[t] = rv;
+        sum += (double)rv;
+        cnt += act ? 1.0 : 0.0;
+    }
+    finish_reduction(sum, cnt, true, rb, RED_CGS_SUM, RED_CGS_CNT);
+}
+
+void cgs_residual_sum(const LevelGeom& g, const float* L, const float* x, const float* b, float* r,
+                      ReduceBuf rb, cudaStream_t s) {
+    if (cgs_residual_sum4(g, L, x, b, r, rb, s)) return;
+    k_cgs_residual_sum<<<cgs_blocks(g.N), kCT, 0, s>>>(g, L, x, b, r, rb);
+}
+
+// active cells: r -= mean ; d = r/D ; inactive: d = 0 ; red[RS] = r.d
+__global__ void __launch_bounds__(kCT)
+k_cgs_start(LevelGeom g, const float* __restrict__ L, float* __restrict__ r, float* __restrict__ d,
+            ReduceBuf rb) {
+    const float mu = cgs_mean(rb.sc);
+    double acc = 0.0;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < g.N;
+         t += (long long)gridDim.x * blockDim.x) {
+        int i, j, k;
+        cgs_unflat(g, t, i, j, k);
+        const float D = cell_diag(g, L, i, j, k);
+        float rv = 0.0f, dv = 0.0f;
+        if (D != 0.0f) {
+            rv = r[t] - mu;
+            dv = rv / D;
+        }
+        r[t] = rv;
+        d[t] = dv;
+        acc += (double)rv * (double)dv;
+    }
+    finish_reduction(acc, 0.0, false, rb, RED_RS, 0);
+}
+
+void cgs_start(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s) {
+    if (cgs_start4(g, L, r, d, rb, s)) return;
+    k_cgs_start<<<cgs_blocks(g.N), kCT, 0, s>>>(g, L, r, d, rb);
+}
+
+// ---- control (single thread).  A is negative semi-definite: r.s and d.q are negative. -----------
+// after cgs_start: rho = rho0 = r.d ; nothing to do when rho is not < 0
+__global__ void k_ctl_cgs_begin(DevScalars* sc, double alpha_cap) {
+    const double rho = sc->red[RED_RS];
+    sc->cgs_alpha_cap = alpha_cap;
+    sc->rho_cg = rho;
+    sc->cgs_rho0 = rho;
+    sc->cgs_frozen = !(rho < 0.0);
+    sc->alpha = 0.0;
+    sc->beta = 0.0;
+}
+void ctl_cgs_begin(DevScalars* sc, const LevelGeom& g, cudaStream_t s) {
+    // a step longer than 16 n_max^2 is a direction that drifted into the null space (reading O12)
+    int nmax = g.n[0] > g.n[1] ? g.n[0] : g.n[1];
+    if (g.n[2] > nmax) nmax = g.n[2];
+    k_ctl_cgs_begin<<<1, 1, 0, s>>>(sc, 16.0 * (double)nmax * (double)nmax);
+}
+
+// after q = A d, red[DQ] = d.q : alpha = rho/(d.q); d.q not < 0 or alpha above the cap ends the
+// smoothing (alpha = 0 leaves x and r untouched for the remaining iterations)
+__global__ void k_ctl_cgs_alpha(DevScalars* sc) {
+    const double dq = sc->red[RED_DQ];
+    double alpha = 0.0;
+    bool stop = sc->cgs_frozen || !(dq < 0.0);
+    if (!stop) {
+        alpha = sc->rho_cg / dq;
+        stop = alpha > sc->cgs_alpha_cap;
+    }
+    if (stop) {
+        sc->cgs_frozen = 1;
+        alpha = 0.0;
+    }
+    sc->alpha = alpha;
+}
+void ctl_cgs_alpha(DevScalars* sc, cudaStream_t s) { k_ctl_cgs_alpha<<<1, 1, 0, s>>>(sc); }
+
+// after s = r/D, red[RS] = r.s : beta = rho'/rho ; freeze once |rho'| <= 1e-8 |rho0|
+__global__ void k_ctl_cgs_beta(DevScalars* sc) {
+    if (sc->cgs_frozen) {
+        sc->beta = 0.0;
+        return;
+    }
+    const double rho_new = sc->red[RED_RS];
+    sc->beta = rho_new / sc->rho_cg;
+    sc->rho_cg = rho_new;
+    if (!(fabs(rho_new) > GMG_CGS_FREEZE * fabs(sc->cgs_rho0))) sc->cgs_frozen = 1;
+}
+void ctl_cgs_beta(DevScalars* sc, cudaStream_t s) { k_ctl_cgs_beta<<<1, 1, 0, s>>>(sc); }
+
+}  // namespace gmgk

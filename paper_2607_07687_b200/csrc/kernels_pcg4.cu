@@ -177,6 +177,78 @@ k_dot4(long long groups, const float4* __restrict__ a, const float4* __restrict_
     finish_reduction(acc, 0.0, false, rb, slot, 0);
 }
 
+// ---- CG smoother restart (reading O12; one-cell versions in kernels_cgs.cu) ------------------------
+// r = b - A x on active cells, 0 elsewhere ; red[CGS_SUM] = sum r ; red[CGS_CNT] = #active
+__global__ void __launch_bounds__(kPT)
+k_cgs_residual_sum4(LevelGeom g, const float* __restrict__ L, const float* __restrict__ x,
+                    const float* __restrict__ b, float* __restrict__ r, ReduceBuf rb) {
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const long long sy = nx, sz = (long long)nx * ny;
+    const unsigned int groups = (unsigned int)(g.N >> 2);
+    double sum = 0.0, cnt = 0.0;
+    for (unsigned int t = blockIdx.x * kPT + threadIdx.x; t < groups; t += gridDim.x * kPT) {
+        int i, j, k;
+        unflat4(g, t, i, j, k);
+        const long long c = 4LL * t;
+        const W4 w = weights4(g, L, i, j, k, c);
+        const float4 xc = ldg4(x + c);
+        const float xm = __ldg(x + ((i == 0) ? c + (nx - 1) : c - 1));
+        const float xp = __ldg(x + ((i + 4 == nx) ? c - (nx - 4) : c + 4));
+        const float4 yl = ldg4(x + ((j == 0) ? c + sy * (ny - 1) : c - sy));
+        const float4 yh = ldg4(x + ((j == ny - 1) ? c - sy * (ny - 1) : c + sy));
+        const float4 zl = ldg4(x + ((k == 0) ? c + sz * (nz - 1) : c - sz));
+        const float4 zh = ldg4(x + ((k == nz - 1) ? c - sz * (nz - 1) : c + sz));
+        const float4 bv = ldg4(b + c);
+        const float Ax = apply7(xc.x, w.xl.x, w.xh.x, w.yl.x, w.yh.x, w.zl.x, w.zh.x, xm, xc.y, yl.x, yh.x, zl.x, zh.x);
+        const float Ay = apply7(xc.y, w.xl.y, w.xh.y, w.yl.y, w.yh.y, w.zl.y, w.zh.y, xc.x, xc.z, yl.y, yh.y, zl.y, zh.y);
+        const float Az = apply7(xc.z, w.xl.z, w.xh.z, w.yl.z, w.yh.z, w.zl.z, w.zh.z, xc.y, xc.w, yl.z, yh.z, zl.z, zh.z);
+        const float Aw = apply7(xc.w, w.xl.w, w.xh.w, w.yl.w, w.yh.w, w.zl.w, w.zh.w, xc.z, xp, yl.w, yh.w, zl.w, zh.w);
+        const bool ax = diag6(w.xl.x, w.xh.x, w.yl.x, w.yh.x, w.zl.x, w.zh.x) != 0.0f;
+        const bool ay = diag6(w.xl.y, w.xh.y, w.yl.y, w.yh.y, w.zl.y, w.zh.y) != 0.0f;
+        const bool az = diag6(w.xl.z, w.xh.z, w.yl.z, w.yh.z, w.zl.z, w.zh.z) != 0.0f;
+        const bool aw = diag6(w.xl.w, w.xh.w, w.yl.w, w.yh.w, w.zl.w, w.zh.w) != 0.0f;
+        float4 rv;
+        rv.x = ax ? bv.x - Ax : 0.0f;
+        rv.y = ay ? bv.y - Ay : 0.0f;
+        rv.z = az ? bv.z - Az : 0.0f;
+        rv.w = aw ? bv.w - Aw : 0.0f;
+        *reinterpret_cast<float4*>(r + c) = rv;
+        sum += (double)rv.x + (double)rv.y + (double)rv.z + (double)rv.w;
+        cnt += (double)((int)ax + (int)ay + (int)az + (int)aw);
+    }
+    finish_reduction(sum, cnt, true, rb, RED_CGS_SUM, RED_CGS_CNT);
+}
+
+// active cells: r -= mean ; d = r/D ; inactive: d = 0 ; red[RS] = r.d
+__global__ void __launch_bounds__(kPT)
+k_cgs_start4(LevelGeom g, const float* __restrict__ L, float* __restrict__ r, float* __restrict__ d,
+             ReduceBuf rb) {
+    const unsigned int groups = (unsigned int)(g.N >> 2);
+    const float mu = cgs_mean(rb.sc);
+    double acc = 0.0;
+    for (unsigned int t = blockIdx.x * kPT + threadIdx.x; t < groups; t += gridDim.x * kPT) {
+        int i, j, k;
+        unflat4(g, t, i, j, k);
+        const long long c = 4LL * t;
+        const W4 w = weights4(g, L, i, j, k, c);
+        const float4 r0 = *reinterpret_cast<const float4*>(r + c);
+        const float Dx = diag6(w.xl.x, w.xh.x, w.yl.x, w.yh.x, w.zl.x, w.zh.x);
+        const float Dy = diag6(w.xl.y, w.xh.y, w.yl.y, w.yh.y, w.zl.y, w.zh.y);
+        const float Dz = diag6(w.xl.z, w.xh.z, w.yl.z, w.yh.z, w.zl.z, w.zh.z);
+        const float Dw = diag6(w.xl.w, w.xh.w, w.yl.w, w.yh.w, w.zl.w, w.zh.w);
+        float4 rv = make_float4(0.0f, 0.0f, 0.0f, 0.0f), dv = rv;
+        if (Dx != 0.0f) { rv.x = r0.x - mu; dv.x = rv.x / Dx; }
+        if (Dy != 0.0f) { rv.y = r0.y - mu; dv.y = rv.y / Dy; }
+        if (Dz != 0.0f) { rv.z = r0.z - mu; dv.z = rv.z / Dz; }
+        if (Dw != 0.0f) { rv.w = r0.w - mu; dv.w = rv.w / Dw; }
+        *reinterpret_cast<float4*>(r + c) = rv;
+        *reinterpret_cast<float4*>(d + c) = dv;
+        acc += (double)rv.x * (double)dv.x + (double)rv.y * (double)dv.y + (double)rv.z * (double)dv.z +
+               (double)rv.w * (double)dv.w;
+    }
+    finish_reduction(acc, 0.0, false, rb, RED_RS, 0);
+}
+
 static inline bool al16(const void* p) { return (reinterpret_cast<size_t>(p) & 15) == 0; }
 
 bool matvec_dot4(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot,
@@ -204,6 +276,17 @@ bool pcg_update_d4(long long N, float* d, const float* s_in, const DevScalars* s
     if (N % 4 != 0 || !al16(d) || !al16(s_in)) return false;
     k_pcg_update_d4<<<blocks4(N >> 2), kPT, 0, st>>>(N >> 2, reinterpret_cast<float4*>(d),
                                                    reinterpret_cast<const float4*>(s_in), sc);
+    return true;
+}
+bool cgs_residual_sum4(const LevelGeom& g, const float* L, const float* x, const float* b, float* r,
+                       ReduceBuf rb, cudaStream_t s) {
+    if (g.n[0] % 4 != 0 || !al16(L) || !al16(x) || !al16(b) || !al16(r)) return false;
+    k_cgs_residual_sum4<<<blocks_plane(g), kPT, 0, s>>>(g, L, x, b, r, rb);
+    return true;
+}
+bool cgs_start4(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s) {
+    if (g.n[0] % 4 != 0 || !al16(L) || !al16(r) || !al16(d)) return false;
+    k_cgs_start4<<<blocks_plane(g), kPT, 0, s>>>(g, L, r, d, rb);
     return true;
 }
 bool dot4(long long N, const float* a, const float* b, ReduceBuf rb, int slot, cudaStream_t s) {

@@ -20,7 +20,8 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgmg.so")
 
-PCG, GMG_PCG, GMG_RBGS = 0, 1, 2
+# GMG_CGS: the paper's own GMG-PCG, the V-cycle with a Jacobi-PCG smoother (include/gmg.h)
+PCG, GMG_PCG, GMG_RBGS, GMG_CGS = 0, 1, 2, 3
 BC_PERIODIC, BC_NEUMANN = 0, 1
 OK, NOT_CONVERGED = 0, 1
 EINVAL, ESTATE, ECUDA, ENOMEM, EBREAKDOWN = -1, -2, -3, -4, -5
@@ -82,6 +83,8 @@ SIGNATURES = {
     "gmg_op_residual_restrict": (C.c_int, [_vp, C.c_int, _vp, _vp, _vp, _vp]),
     "gmg_op_prolong": (C.c_int, [_vp, C.c_int, _vp, _vp, _vp]),
     "gmg_op_vcycle": (C.c_int, [_vp, _vp, _vp, C.c_float, C.c_int, _vp]),
+    "gmg_op_cg_smooth": (C.c_int, [_vp, C.c_int, _vp, _vp, C.c_int, _vp]),
+    "gmg_op_vcycle_cgs": (C.c_int, [_vp, _vp, _vp, _vp]),
     "gmg_op_norm2": (C.c_int, [_vp, C.c_int, _vp, C.POINTER(C.c_double), _vp]),
     "gmg_divergence": (C.c_int, [_vp, _vp, C.POINTER(C.c_float), _vp, _vp]),
     "gmg_project": (C.c_int, [_vp, _vp, _vp, _vp]),
@@ -315,6 +318,17 @@ class GMG:
         """In place on p."""
         self._check(lib.gmg_op_vcycle(self._h, self._vec(p), self._vec(z), float(omega),
                                       int(bool(symmetric)), self._stream()))
+        return p
+
+    def op_cg_smooth(self, lev, x, b, iters):
+        """In place on x."""
+        self._check(lib.gmg_op_cg_smooth(self._h, lev, self._vec(x, lev), self._vec(b, lev),
+                                         int(iters), self._stream()))
+        return x
+
+    def op_vcycle_cgs(self, p, z):
+        """In place on p."""
+        self._check(lib.gmg_op_vcycle_cgs(self._h, self._vec(p), self._vec(z), self._stream()))
         return p
 
     def op_norm2(self, lev, r) -> float:
