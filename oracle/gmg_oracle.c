@@ -13,7 +13,7 @@
  *   - anisotropic coarsening "downsamples every dimension independently"      PAPER.md:47 (S3.2)
  *   - PCG as the general-purpose comparison solver                            PAPER.md:31, 39 (S3)
  * The paper gives these in words only (no equation, constant or stencil), so every
- * formula below is a READING, numbered O1..O11 as in SURVEY.md S8(c) and listed in
+ * formula below is a READING, numbered O1..O12 as in SURVEY.md S8(c) and listed in
  * DESIGN.md "Readings of the paper".
  *
  * PARITY PINS (tests/, -m "not gpu"): operator vs a face-by-face dense assembly and
@@ -21,10 +21,11 @@
  * (O5); half-sweep zeroes the residual of its colour and decreases the error energy (O3);
  * <Rr,e> = <r,Pe> (O6); closed-form coarse coefficients and quadratic consistency (O5);
  * level shapes (O4); dense least-squares solve on 8^3 (O7,O9,O10,O11 solutions);
- * dyadic omega sequence (O8).
+ * dyadic omega sequence (O8); the CG smoother as the Krylov energy minimiser of the dense
+ * face-assembled system, its guards, the CG-smoothed cycle as a composition of its parts (O12).
  * PARITY UNPINNED against the paper itself: the omega rule and its constants (O8), the
- * sweep counts nu1/nu2/nuc (O7) and the meaning of "GMG-PCG" (O11): the paper prints no
- * worked example or constant for them.
+ * sweep counts nu1/nu2/nuc (O7), the meaning of "GMG-PCG" (O11) and the restart, counts and
+ * guards of the PCG-smoothed cycle (O12): the paper prints no worked example or constant for them.
  *
  * Layout: cell I=(i,j,k), linear index i + nx*(j + ny*k) (x fastest).  L is
  * component-major: L[d*N + idx] is the coefficient on the LOWER d-face of cell idx
