@@ -176,6 +176,45 @@ def solver_table(gmg, W, torch, device, names):
     return out
 
 
+def step_table(gmg, W, torch, device, exps=(5, 6), nsteps=16):
+    """Warm-started pressure steps with a moving body (Table 1's shape: average
+    iterations per solve, final residual, cost per cell per step): per step gmg_set_coeffs ->
+    gmg_divergence -> gmg_solve (p from the step before) -> gmg_project, device-resident, CUDA
+    events around the whole step.  The first (cold) step is reported separately."""
+    from paper_2607_07687_b200.pressure_step import PressureStepper
+    out = {}
+    for pe in exps:
+        nx = 2 ** (pe + 1)
+        n, bc = (nx, nx, nx // 2), W.JELLYFISH_BC
+        cells = n[0] * n[1] * n[2]
+        seq = [(torch.from_numpy(L).to(device), torch.from_numpy(u).to(device))
+               for L, u in W.jellyfish_steps(pe, nsteps)]
+        row = {}
+        for label, solver, cap in (("PCG", gmg.PCG, 5000), ("GMG-PCG", gmg.GMG_PCG, 50),
+                                   ("GMG-CGS", gmg.GMG_CGS, 50), ("GMG-RBGS", gmg.GMG_RBGS, 50)):
+            ps = PressureStepper(n, bc, solver=solver, tol=1e-4, maxiter=cap, device=str(device))
+            its, res, ms = [], [], []
+            Lcur = torch.empty_like(seq[0][0])   # the body update rewrites ONE coefficient array
+            for L, u in seq:
+                uu = u.clone()
+                Lcur.copy_(L)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                rc, st = ps.step(Lcur, uu)
+                e1.record()
+                torch.cuda.synchronize()
+                its.append(st["iterations"]); res.append(st["resid_final_rel"]); ms.append(e0.elapsed_time(e1))
+            ps.close()
+            warm = slice(1, None)
+            row[label] = {"iterations_first": its[0],
+                          "iterations_avg": sum(its[warm]) / len(its[warm]),
+                          "resid_avg": sum(res[warm]) / len(res[warm]),
+                          "ms_per_step": sum(ms[warm]) / len(ms[warm]),
+                          "ns_per_cell_per_step": sum(ms[warm]) / len(ms[warm]) * 1e6 / cells}
+        out[f"jellyfish_p{pe}_{n[0]}x{n[1]}x{n[2]}_{nsteps}steps"] = row
+    return out
+
+
 def time_kernel_loop(fn, reps, stream):
     import torch
     e0 = torch.cuda.Event(enable_timing=True)
@@ -349,6 +388,8 @@ def run_ours(args):
                 "GMG-PCG": {"iterations": st2["iterations"], "resid": st2["resid_final_rel"],
                             "ms": st2["gpu_ms"], "ns_per_cell": st2["gpu_ms"] * 1e6 / N}}
 
+    steps_tab = step_table(gmg, W, torch, device) if (not args.no_table and rank == 0) else None
+
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False,
@@ -385,6 +426,7 @@ def run_ours(args):
         "clocks": sampler.summary(),
         "around_solve": around,
         "solvers": table,
+        "pressure_steps": steps_tab,
         "plan": g.describe_plan().strip().split("\n"),
     }
     print(json.dumps(line))

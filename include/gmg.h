@@ -137,7 +137,8 @@ int gmg_set_workspace(gmg_ctx* ctx, void* ws_dev, size_t bytes);
  * unchanged until the next gmg_set_coeffs / gmg_destroy) and coarsen them to every level
  * (reading O5: L_d^{l+1}(J) = (1/c_d) * sum of the fine L_d on the faces tiling the coarse
  * face).  Checks on device that every value is finite and >= 0 (GMG_EINVAL otherwise).
- * Resets omega to omega0. */
+ * Resets omega to omega0.  Calling it again with the SAME pointer after rewriting the array in
+ * place (a moving body) keeps the captured solve graphs; a new pointer drops them. */
 int gmg_set_coeffs(gmg_ctx* ctx, const float* L_dev, void* stream);
 
 /* Solve A p = z.  p_dev: in = initial guess, out = solution (in place).  Stops when

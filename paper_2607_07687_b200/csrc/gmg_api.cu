@@ -354,7 +354,9 @@ extern "C" int gmg_set_coeffs(gmg_ctx* c, const float* L_dev, void* stream) {
     if (!c || !L_dev) return GMG_EINVAL;
     if (!c->ws_set) { SET_ERR(c, "gmg_set_coeffs before gmg_set_workspace"); return GMG_ESTATE; }
     cudaStream_t s = (cudaStream_t)stream;
-    drop_graphs(c);
+    // the captured solve graphs hold pointers only: a moving body that rewrites the SAME array
+    // every step keeps them; a new array drops them
+    if (c->lv[0].L != L_dev) drop_graphs(c);
     c->lv[0].L = L_dev;
     // finest level: validation rides on the coarsening pass when the float4 kernel takes it
     const bool fused_check = c->prm.fast_path && c->nlev > 1 && gmgk::coarsen4_supported(c->g[0]);

@@ -337,11 +337,12 @@ class GMG:
                                      self._stream()))
         return out.value
 
-    def divergence(self, u: torch.Tensor, wall_hi=(0.0, 0.0, 0.0)) -> torch.Tensor:
-        """z = div u; u: (3, nz, ny, nx) lower-face velocities."""
+    def divergence(self, u: torch.Tensor, wall_hi=(0.0, 0.0, 0.0), out=None) -> torch.Tensor:
+        """z = div u; u: (3, nz, ny, nx) lower-face velocities.  out: optional result tensor."""
         assert u.is_cuda and u.dtype == torch.float32 and u.is_contiguous()
         assert tuple(u.shape) == (3, self.n[2], self.n[1], self.n[0])
-        z = self._new(0)
+        z = self._new(0) if out is None else out
+        self._vec(z)
         wh = (C.c_float * 3)(*[float(v) for v in wall_hi])
         self._check(lib.gmg_divergence(self._h, _vp(_ptr(u)), wh, _vp(_ptr(z)), self._stream()))
         return z

@@ -252,6 +252,59 @@ def config3(p=5, seed=None):
                     meta={"active_fraction": float(act.mean()), "p": p})
 
 
+def jellyfish_steps(p=5, nsteps=8, period=64, seed=None):
+    """A swimming-jellyfish-SHAPED sequence of pressure steps ("simplified swimming
+    jellyfish", Table 1; warm starts and a coefficient update every step).
+    The shell of configs[3] heaves along z, c_z(k) = nz/2 + 2 sin(2 pi k / period) cells, and its
+    contraction velocity swings with it, amplitude 0.5 cos(2 pi k / period); the random-Fourier
+    background flow is drawn once and kept.  Yields per step (L32, ustar32): the face
+    coefficients [3][nz][ny][nx] and the predicted velocity u* = L (u_F + u_C) on the lower faces
+    (all wall faces 0, so div u* sums to zero).  A synthetic stand-in: no Navier-Stokes step is
+    taken, the steps are linked only through the warm start of p.  Input conditioning only."""
+    if seed is None:
+        seed = 76880 + p
+    rng = np.random.default_rng(seed)
+    nx = 2 ** (p + 1)
+    n = (nx, nx, nx // 2)
+    nx, ny, nz = n
+    R = 0.25 * nx
+    coords = [face_coords(n, d) for d in range(3)]
+    uF = []
+    for d in range(3):
+        f = np.zeros((nz, ny, nx), dtype=np.float64)
+        for _t in range(8):
+            kk = rng.integers(0, 5, 3)
+            phi = rng.uniform(0.0, 2.0 * np.pi, 3)
+            a = rng.standard_normal()
+            term = a
+            for q in range(3):
+                term = term * np.cos(2.0 * np.pi * kk[q] * coords[d][q] / n[q] + phi[q])
+            f += term
+        uF.append(0.125 * f)
+    for k in range(nsteps):
+        th = 2.0 * np.pi * k / period
+        c = (nx / 2.0, ny / 2.0, nz / 2.0 + 2.0 * np.sin(th))
+        amp = 0.5 * np.cos(th)
+        L = np.empty((3, nz, ny, nx), dtype=np.float64)
+        u = np.empty_like(L)
+        for d in range(3):
+            X, Y, Z = coords[d]
+            sd = _shell_distance(X, Y, Z, c, R)
+            L[d] = np.clip((sd - 1.5) / 4.0, 0.0, 1.0)
+            rel = (X - c[0], Y - c[1], Z - c[2])
+            dist = np.sqrt(rel[0] ** 2 + rel[1] ** 2 + rel[2] ** 2)
+            dist = np.where(dist == 0.0, 1.0, dist)
+            uC = -amp * np.exp(-(sd / 3.0) ** 2) * rel[d] / dist
+            u[d] = L[d].astype(np.float32).astype(np.float64) * (uF[d] + uC)
+            sl = [slice(None)] * 3
+            sl[2 - d] = 0
+            u[d][tuple(sl)] = 0.0                      # wall faces carry 0
+        yield L.astype(np.float32), u.astype(np.float32)
+
+
+JELLYFISH_BC = (NEUMANN,) * 3
+
+
 # --------------------------------------------------------------------------
 # configs[4]: billion-cell stress: periodic cube, seeded random solid spheres
 # --------------------------------------------------------------------------

@@ -116,3 +116,23 @@ def test_library_level_table_matches_golden_and_oracle(libpath):
             assert got == oracle.level_shapes(n, bc, iso=iso), (n, bc, iso)
     with pytest.raises(ValueError):
         gmg.plan((31, 32, 16), (0, 0, 0))
+
+
+def test_jellyfish_step_sequence_is_compatible_and_moves_smoothly():
+    """Input recipe of the warm-started pressure steps (S4): div u* sums to zero, solid
+    cells carry no flux, and consecutive steps differ by a fraction of a cell of body motion."""
+    import numpy as np
+    from paper_2607_07687_b200 import workloads as W
+    steps = list(W.jellyfish_steps(4, 4))
+    assert len(steps) == 4
+    prev = None
+    for L, u in steps:
+        assert L.dtype == np.float32 and u.dtype == np.float32 and L.shape == u.shape == (3, 16, 32, 32)
+        assert L.min() >= 0.0 and L.max() <= 1.0 and (L == 0.0).any()
+        z = W.divergence(u.astype(np.float64), W.JELLYFISH_BC)
+        assert abs(z.sum()) < 1e-9 * np.abs(z).sum()
+        act = W.active_mask(L, W.JELLYFISH_BC)
+        assert np.all(z[~act] == 0.0)
+        if prev is not None:
+            assert 0.0 < np.abs(L - prev).max() < 0.5
+        prev = L
