@@ -115,8 +115,10 @@ int gmg_plan(int nx, int ny, int nz, const int bc[3], const gmg_params_t* params
 
 /* -- life cycle ------------------------------------------------------------------------ */
 
-/* Create a context for an nx*ny*nz grid.  Every n_d >= 2; a periodic axis needs an even
- * extent (red/black colouring, reading O3).  Builds the level-shape table by the
+/* Create a context for an nx*ny*nz grid.  A periodic axis needs an even extent (red/black
+ * colouring, reading O3).  An extent of 1 is allowed on a Neumann axis: nx*ny*1 is the 2-D mode
+ * (Fig. 2 left "2D flow around a circular cylinder"); that axis never coarsens and
+ * its coefficients are ignored.  Builds the level-shape table by the
  * anisotropic rule (reading O4).  Uses the current CUDA device. */
 int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]);
 void gmg_destroy(gmg_ctx* ctx);

@@ -197,7 +197,8 @@ void gmgo_half_sweep(const int n[3], const int bc[3], const double *L, double *p
  * O4 (PAPER.md:47 S3.2 "downsamples every dimension independently"): direction d is
  * halved from one level to the next iff  n_d even  and  n_d/2 >= n_min  and
  * (axis d is Neumann or n_d/2 is even).  iso != 0 = classical isotropic coarsening:
- * coarsen all three directions or stop.  Returns 1 if anything coarsens.
+ * coarsen all directions (of extent > 1: a 2-D grid is nx x ny x 1 with Neumann z) or stop.
+ * Returns 1 if anything coarsens.
  * ---------------------------------------------------------------------------------- */
 int gmgo_coarsen_rule(const int n[3], const int bc[3], int n_min, int iso, int c[3]) {
     int any = 0, all = 1;
@@ -206,7 +207,7 @@ int gmgo_coarsen_rule(const int n[3], const int bc[3], int n_min, int iso, int c
         int ok = (n[d] % 2 == 0) && (h >= n_min) && (bc[d] == GMGO_NEUMANN || h % 2 == 0);
         c[d] = ok ? 2 : 1;
         any |= ok;
-        all &= ok;
+        if (n[d] > 1) all &= ok; /* an extent-1 direction (2-D grid) has nothing to coarsen */
     }
     if (iso && !all) {
         c[0] = c[1] = c[2] = 1;

@@ -2,7 +2,7 @@
 impulsive start of a uniform flow past a sphere in an (N b) x b x b box, with the classical
 isotropic coarsening and with the paper's anisotropic coarsening.
 
-    python -m paper_2607_07687_b200.aspect_study [--base 32] [--aspects 1 2 4 8 16]
+    python -m paper_2607_07687_b200.aspect_study [--base 32] [--aspects 1 2 4 8 16] [--case sphere|cylinder2d]
 
 Needs a CUDA device (the solves run through the C-ABI library).  Inputs are synthetic
 (workloads.impulsive_sphere); the paper's own cases and sizes are not reproduced."""
@@ -15,10 +15,12 @@ from . import gmg
 from . import workloads as W
 
 
-def run(aspects=(1, 2, 4, 8, 16), base=32, tol=1e-4, maxiter=200):
+def run(aspects=(1, 2, 4, 8, 16), base=32, tol=1e-4, maxiter=200, case="sphere"):
+    """case: "sphere" (Fig. 2 right, 3-D) or "cylinder2d" (Fig. 2 left, an (N b) x b x 1 grid)."""
     rows = []
+    make = W.impulsive_sphere if case == "sphere" else W.impulsive_cylinder_2d
     for N in aspects:
-        wl = W.impulsive_sphere(N, base)
+        wl = make(N, base)
         L = torch.from_numpy(wl.L).cuda()
         z = torch.from_numpy(wl.z).cuda()
         row = {"aspect": N, "grid": list(wl.n)}
@@ -42,9 +44,10 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--base", type=int, default=32)
     ap.add_argument("--aspects", type=int, nargs="+", default=[1, 2, 4, 8, 16])
+    ap.add_argument("--case", default="sphere", choices=["sphere", "cylinder2d"])
     ap.add_argument("--json", action="store_true")
     a = ap.parse_args()
-    rows = run(a.aspects, a.base)
+    rows = run(a.aspects, a.base, case=a.case)
     if a.json:
         print(json.dumps(rows))
         return

@@ -113,7 +113,7 @@ static void build_levels(gmg_ctx* c) {
                            (cur.bc[d] == GMG_BC_NEUMANN || h % 2 == 0);
             cur.c[d] = ok ? 2 : 1;
             any |= ok;
-            all &= ok;
+            if (cur.n[d] > 1) all &= ok;  // an extent-1 direction (2-D grid) has nothing to coarsen
         }
         if (c->prm.coarsen_mode == GMG_COARSEN_ISO && !all) any = 0;
         if (!any || c->nlev + 1 >= GMG_MAX_LEVELS) cur.c[0] = cur.c[1] = cur.c[2] = 1;
@@ -210,8 +210,9 @@ extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]
     *out = nullptr;
     const int n[3] = {nx, ny, nz};
     for (int d = 0; d < 3; ++d) {
-        if (n[d] < 2) return GMG_EINVAL;
+        if (n[d] < 1) return GMG_EINVAL;
         if (bc[d] != GMG_BC_PERIODIC && bc[d] != GMG_BC_NEUMANN) return GMG_EINVAL;
+        if (n[d] == 1 && bc[d] != GMG_BC_NEUMANN) return GMG_EINVAL;  // 2-D mode: walls either side
         if (bc[d] == GMG_BC_PERIODIC && (n[d] & 1)) return GMG_EINVAL;  // reading O3
     }
     if ((long long)nx * ny * nz > (1LL << 31) - 1) return GMG_EINVAL;
@@ -317,8 +318,9 @@ extern "C" int gmg_plan(int nx, int ny, int nz, const int bc[3], const gmg_param
     if (!bc || !out) return GMG_EINVAL;
     const int n[3] = {nx, ny, nz};
     for (int d = 0; d < 3; ++d) {
-        if (n[d] < 2) return GMG_EINVAL;
+        if (n[d] < 1) return GMG_EINVAL;
         if (bc[d] != GMG_BC_PERIODIC && bc[d] != GMG_BC_NEUMANN) return GMG_EINVAL;
+        if (n[d] == 1 && bc[d] != GMG_BC_NEUMANN) return GMG_EINVAL;  // 2-D mode: walls either side
         if (bc[d] == GMG_BC_PERIODIC && (n[d] & 1)) return GMG_EINVAL;
     }
     if ((long long)nx * ny * nz > (1LL << 31) - 1) return GMG_EINVAL;

@@ -406,6 +406,32 @@ def impulsive_sphere(N=4, base=32, D=None):
                     meta={"active_fraction": float(act.mean()), "aspect": int(N)})
 
 
+def impulsive_cylinder_2d(N=4, base=32, D=None):
+    """2-D counterpart of impulsive_sphere (Fig. 2 left "2D flow around a circular
+    cylinder"): an (N b) x b x 1 grid, x Neumann with the free stream on the in/outflow faces, y
+    periodic, the single z layer between two walls (its coefficients are ignored)."""
+    D = base / 4.0 if D is None else float(D)
+    n = (int(N) * base, base, 1)
+    nx, ny, nz = n
+    bc = (NEUMANN, PERIODIC, NEUMANN)
+    c = (min(1.0, 0.5 * N) * base, 0.5 * base)
+    L = np.empty((3, nz, ny, nx), dtype=np.float64)
+    for d in range(3):
+        X, Y, Z = face_coords(n, d)
+        L[d] = ramp(np.sqrt((X - c[0]) ** 2 + (Y - c[1]) ** 2) - 0.5 * D)
+    L32 = L.astype(np.float32)
+    Lq = L32.astype(np.float64)
+    u = np.zeros_like(Lq)
+    u[0] = Lq[0]
+    u[0][:, :, 0] = 1.0
+    z = divergence(u, bc, wall_hi=(1.0, 0.0, 0.0))
+    act = active_mask(L32, bc)
+    z = project_compatible(z, act)
+    return Workload(f"impulsive_cylinder2d_N{N}", n, bc, L32, z.astype(np.float32),
+                    tol=1e-4, maxiter=200, seed=0,
+                    meta={"active_fraction": float(act.mean()), "aspect": int(N)})
+
+
 def by_name(name: str) -> Workload:
     """configs by short name: c0, c1, c2, c3p5, c3p6, c4 (1024^3), c4_128, c4_256, c4_512."""
     if name == "c0":

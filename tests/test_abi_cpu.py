@@ -66,7 +66,8 @@ def test_null_arguments_are_rejected_without_a_gpu(libpath):
     assert gmg.lib.gmg_create(None, 8, 8, 8, I3(0, 0, 0)) == gmg.EINVAL
     h = C.c_void_p()
     assert gmg.lib.gmg_create(C.byref(h), 7, 8, 8, I3(0, 0, 0)) == gmg.EINVAL   # odd periodic
-    assert gmg.lib.gmg_create(C.byref(h), 1, 8, 8, I3(1, 0, 0)) == gmg.EINVAL   # extent < 2
+    assert gmg.lib.gmg_create(C.byref(h), 0, 8, 8, I3(1, 0, 0)) == gmg.EINVAL   # extent < 1
+    assert gmg.lib.gmg_create(C.byref(h), 8, 8, 1, I3(0, 0, 0)) == gmg.EINVAL   # extent 1 needs walls
     assert gmg.lib.gmg_create(C.byref(h), 8, 8, 8, I3(0, 2, 0)) == gmg.EINVAL   # bad bc
     assert gmg.lib.gmg_num_levels(None) == gmg.EINVAL
     assert gmg.lib.gmg_workspace_bytes(None) == 0
@@ -110,7 +111,8 @@ def test_library_level_table_matches_golden_and_oracle(libpath):
         cluster_extra = 4 * sum(6 * v for v in N[:tail] if v <= 32768)
         assert lower <= ws <= lower + cluster_extra + 256 * (7 * len(N) + 8)
     # agreement with the oracle's rule on odd / mixed cases, both coarsening modes
-    for n, bc in [((20, 20, 20), (1, 0, 0)), ((36, 20, 6), (0, 1, 0)), ((64, 4, 4), (1, 0, 0)), ((15, 9, 7), (1, 1, 1))]:
+    for n, bc in [((20, 20, 20), (1, 0, 0)), ((36, 20, 6), (0, 1, 0)), ((64, 4, 4), (1, 0, 0)), ((15, 9, 7), (1, 1, 1)),
+                  ((64, 16, 1), (1, 0, 1)), ((128, 32, 1), (0, 0, 1))]:      # 2-D mode
         for iso in (False, True):
             got = gmg.plan(n, bc, coarsen_mode=gmg.COARSEN_ISO if iso else gmg.COARSEN_ANISO)[0]
             assert got == oracle.level_shapes(n, bc, iso=iso), (n, bc, iso)

@@ -177,7 +177,8 @@ def test_nonzero_initial_guess_parity():
 
 @pytest.mark.parametrize("n,bc", [((4, 4, 4), (0, 0, 0)), ((2, 2, 2), (1, 1, 1)),
                                   ((5, 7, 3), (1, 1, 1)), ((6, 10, 4), (0, 0, 1)),
-                                  ((64, 4, 4), (1, 0, 0)), ((40, 24, 8), (0, 1, 0))])
+                                  ((64, 4, 4), (1, 0, 0)), ((40, 24, 8), (0, 1, 0)),
+                                  ((64, 48, 1), (1, 0, 1)), ((256, 64, 1), (0, 0, 1)), ((33, 17, 1), (1, 1, 1))])
 def test_degenerate_and_ragged_shapes(n, bc):
     """Single-level grids (the tail kernel is the whole cycle), odd Neumann extents, strongly
     anisotropic boxes, extents that are not multiples of the tile sizes."""
@@ -332,6 +333,25 @@ def test_aspect_ratio_study_matches_oracle_and_shows_the_papers_trend():
         if r["aspect"] >= 4:
             assert r["aniso"]["levels"] > r["iso"]["levels"]
             assert 1.4 * r["aniso"]["vcycles"] <= r["iso"]["vcycles"], r
+
+
+def test_2d_aspect_ratio_study_matches_oracle():
+    """Fig. 2 (left): impulsive start past a 2-D cylinder on an (N b) x b x 1 grid, both coarsening
+    rules, V-cycle counts against the oracle within one cycle; anisotropic never needs more."""
+    from paper_2607_07687_b200 import aspect_study
+    rows = aspect_study.run(aspects=(1, 4, 8), base=16, case="cylinder2d")
+    for r in rows:
+        wl = W.impulsive_cylinder_2d(r["aspect"], 16)
+        assert wl.n[2] == 1
+        for name, iso in (("iso", True), ("aniso", False)):
+            h = make_oracle(wl, iso=iso)
+            ref = h.solve(oracle.GMG_RBGS, wl.z, tol=1e-4, maxiter=200)
+            assert r[name]["levels"] == h.nlev
+            assert r[name]["converged"] == (ref["status"] == 0), (r["aspect"], name)
+            assert abs(r[name]["vcycles"] - ref["iterations"]) <= 1, (r["aspect"], name, r[name], ref["iterations"])
+        assert r["aniso"]["vcycles"] <= r["iso"]["vcycles"]
+        if r["aspect"] >= 4:
+            assert r["aniso"]["levels"] > r["iso"]["levels"]
 
 
 @pytest.mark.parametrize("n,bc", [((64, 64, 64), (0, 0, 0)), ((64, 64, 32), (1, 0, 1)),

@@ -466,3 +466,41 @@ def test_projected_field_is_divergence_free_after_an_exact_solve():
     assert np.linalg.norm(A @ p.ravel() - z.ravel()) < 1e-9 * np.linalg.norm(z)      # z compatible
     div_after = oracle.divergence(oracle.project(L, bc, p, u), bc)
     assert np.max(np.abs(div_after)) < 1e-9
+
+
+# --------------------------------------------------------------------------------------
+# 2-D mode: an nx x ny x 1 grid with Neumann z (Fig. 2 left)
+# --------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bc", [(1, 0, 1), (0, 0, 1), (1, 1, 1)])
+def test_2d_grid_operator_is_the_five_point_face_assembly(bc):
+    rng = np.random.default_rng(21)
+    n = (8, 6, 1)
+    L = rand_L(rng, n, zero_frac=0.2)
+    A = dense_by_faces(n, bc, L)
+    # the z coefficients must not matter at all: a five-point operator
+    A2 = dense_by_faces(n, bc, np.stack([L[0], L[1], rng.uniform(0, 1, L[2].shape)]))
+    assert np.array_equal(A, A2)
+    assert np.max(np.count_nonzero(A, axis=1)) <= 5
+    p = rng.standard_normal((1, 6, 8))
+    assert np.allclose(oracle.apply_A(L, bc, p).ravel(), A @ p.ravel(), atol=1e-13)
+    assert np.allclose(oracle.diag(L, bc).ravel(), np.diag(A), atol=1e-13)
+
+
+def test_2d_level_shapes_and_dense_solution():
+    assert oracle.level_shapes((64, 16, 1), (1, 0, 1)) == [(64, 16, 1), (32, 8, 1), (16, 4, 1), (8, 4, 1), (4, 4, 1)]
+    # isotropic = both in-plane directions or stop; the extent-1 axis has nothing to coarsen
+    assert oracle.level_shapes((64, 16, 1), (1, 0, 1), iso=True) == [(64, 16, 1), (32, 8, 1), (16, 4, 1)]
+    rng = np.random.default_rng(22)
+    n, bc = (16, 8, 1), (1, 0, 1)
+    L32 = rng.uniform(0.1, 1, (3, 1, 8, 16)).astype(np.float32)
+    Le = W.effective_L(L32, bc)
+    act = W.active_mask(L32, bc)
+    z = W.project_compatible(rng.standard_normal((1, 8, 16)), act)
+    xs, A = _dense_solution(n, bc, Le, z)
+    for solver in (oracle.GMG_RBGS, oracle.PCG, oracle.GMG_PCG, oracle.GMG_CGS):
+        H = oracle.Hierarchy(n, bc, L32)
+        assert H.nlev == 3
+        out = H.solve(solver, z, tol=1e-10, maxiter=400)
+        assert out["status"] == 0, solver
+        err = np.linalg.norm(_demean(out["p"], act) - _demean(xs, act)) / np.linalg.norm(_demean(xs, act))
+        assert err < 1e-8, (solver, err)
