@@ -94,6 +94,29 @@ def _run(name, nsamples):
     assert true_rel <= wl.tol
     hist = g.history()
     assert len(hist) == 4 and all(hist[k + 1] < 0.1 * hist[k] for k in range(3))
+    del rr
+    # ---- (c) the PCG smoother / PCG-smoothed cycle (reading O12) in the same configuration ------
+    # one CG iteration from x0 minimises the energy along d = x1 - x0: the new (mean-free) residual
+    # is orthogonal to the step -- a property of the whole-array inner products at any size
+    x1 = p0.clone()
+    g.op_cg_smooth(0, x1, z, 1)
+    r1 = g.op_residual(0, x1, z).double()
+    act = r1 != 0
+    r1 = torch.where(act, r1 - r1.sum() / act.sum(), r1)
+    step = (x1 - p0).double()
+    cosang = float((r1 * step).sum().item()) / (float(torch.linalg.vector_norm(r1).item()) *
+                                                float(torch.linalg.vector_norm(step).item()))
+    assert abs(cosang) <= 1e-4, cosang
+    r0n = float(torch.linalg.vector_norm(r.double()).item())
+    assert float(torch.linalg.vector_norm(r1).item()) < r0n          # and it made progress
+    del x1, r1, act, step
+    p.zero_()
+    rc = g.solve(p, z, tol=wl.tol, maxiter=wl.maxiter, solver=gmg.GMG_CGS)
+    st = g.stats()
+    assert rc == gmg.OK and st["iterations"] == 4, st            # as on the 128^3 shrink and in the oracle
+    rr = g.op_residual(0, p, z)
+    true_rel = float(torch.linalg.vector_norm(rr.double()).item()) / st["resid_ref"]
+    assert abs(true_rel - st["resid_final_rel"]) <= 1e-6 * true_rel and true_rel <= wl.tol
     g.close()
 
 
