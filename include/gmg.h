@@ -83,6 +83,11 @@ typedef struct {
     int cluster_tail;  /* 1: the coarse levels that fit the shared memory of a cluster of 8 CTAs
                           (each at most 32768 cells) run as ONE thread-block-cluster kernel;
                           0: only what fits a single CTA does (1) */
+    int fused_norm;    /* 1: on a finest level that runs the TMA-fed sweep, the stopping-test norm
+                          ||z - A p_k|| is accumulated by the first pre-smoothing sweep of cycle k+1
+                          (out of place, so p_k survives when the test ends the solve) instead of
+                          by a 20 B/cell pass of its own after every cycle; same iterates, same
+                          test, one sweep wasted at the end of a solve (1) */
 } gmg_params_t;
 
 /* Statistics of the last gmg_solve. */
@@ -201,6 +206,12 @@ int gmg_op_vcycle(gmg_ctx* ctx, float* p_dev, const float* z_dev, float omega, i
 /* The smoother of GMG_GMG_CGS (reading O12, "PCG can be used as a smoother"): iters
  * Jacobi-PCG iterations on A^lev x = b restarted from x (in place), and one whole cycle of it on
  * level 0 (V(nu_pre, nu_post), nu_coarse iterations on the coarsest level). */
+/* ONE fused red+black sweep src -> dst (out of place) of the TMA-fed kernel that also returns
+ * sum r^2, r = b - A src on active cells, and sum b^2 over active cells (the fused_norm path of
+ * gmg_solve).  GMG_EINVAL when level lev cannot run that kernel (nx % 128, small levels). */
+int gmg_op_sweep_with_norm(gmg_ctx* ctx, int lev, const float* src_dev, float* dst_dev, const float* b_dev,
+                           float omega, int first_colour, double* rr_out_host, double* bb_out_host,
+                           void* stream);
 int gmg_op_cg_smooth(gmg_ctx* ctx, int lev, float* x_dev, const float* b_dev, int iters, void* stream);
 int gmg_op_vcycle_cgs(gmg_ctx* ctx, float* p_dev, const float* z_dev, void* stream);
 /* sqrt(sum r^2) of a level-lev array (deterministic two-stage reduction). */

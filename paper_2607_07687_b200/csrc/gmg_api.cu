@@ -29,6 +29,15 @@ void prolong_add4(const LevelGeom& g, const float* e_c, float* p_f, cudaStream_t
 bool matvec_dot_bulk(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot,
                      cudaStream_t s);
 bool tma_shape_ok(const LevelGeom& g);
+// one TMA-fed sweep src -> dst that also leaves sum r^2 (r = b - A src) and sum b^2 over the active
+// cells in red[slot_rr] / red[slot_ref]; false = the level cannot run it (nothing launched)
+bool rb_sweep_with_norm(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
+                        const float* omega, int first_colour, ReduceBuf rb, int slot_rr, int slot_ref,
+                        cudaStream_t s);
+bool sweep_norm_supported(const LevelGeom& g);
+// the same sweep as a no-op unless *run_flag != 0
+bool rb_sweep_if(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
+                 const float* omega, int first_colour, const int* run_flag, cudaStream_t s);
 int configure();
 }  // namespace gmgf
 
@@ -59,6 +68,7 @@ struct gmg_ctx {
     bool fast_sweep[GMG_MAX_LEVELS];
     bool fast_rr[GMG_MAX_LEVELS];
     int tma_ok[GMG_MAX_LEVELS];  // level large enough for the TMA-fed kernels
+    bool fused_norm_on;   // GMG-RBGS: the stopping-test norm rides on the first pre-sweep (prm.fused_norm)
     // workspace
     void* ws;
     size_t ws_bytes;
@@ -152,6 +162,9 @@ static void build_levels(gmg_ctx* c) {
         c->fast_rr[l] = c->prm.fast_path && l + 1 < c->nlev && gmgf::resrestrict_supported(c->g[l]);
         c->tma_ok[l] = c->prm.tma_min_cells >= 0 && c->g[l].N >= (long long)c->prm.tma_min_cells;
     }
+    const int first_tail = c->ctail_start < c->tail_start ? c->ctail_start : c->tail_start;
+    c->fused_norm_on = c->prm.fused_norm && c->prm.fast_path && c->nlev > 1 && first_tail > 0 &&
+                       c->fast_sweep[0] && c->tma_ok[0] && c->prm.nu_pre >= 2;
 }
 
 static size_t carve(gmg_ctx* c, char* base) {
@@ -203,6 +216,7 @@ extern "C" void gmg_default_params(gmg_params_t* p) {
     p->omega0 = 1.0f; p->omega_min = 0.5f; p->omega_down = 0.125f; p->omega_up = 0.03125f;
     p->adaptive = 1; p->coarsen_mode = GMG_COARSEN_ANISO; p->n_min = 4;
     p->fast_path = 1; p->use_graph = 1; p->tma_min_cells = 4 << 20; p->cluster_tail = 1;
+    p->fused_norm = 1;
 }
 
 extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]) {
@@ -399,8 +413,9 @@ extern "C" int gmg_level_coeffs(gmg_ctx* c, int lev, float* L_out_dev, void* str
 // ---- smoothing: nsweeps RBGS sweeps, result in p (reading O3) --------------------
 // e_c != nullptr: the coarse correction P e_c is added to p first (fused into the first sweep
 // on the fast path, a separate kernel otherwise).
+// skip_first: the first fused sweep p -> q of this call has already been run (fused_norm path).
 static void smooth(gmg_ctx* c, int l, float* p, const float* b, const float* omega, int nsweeps,
-                   int first_colour, const float* e_c, cudaStream_t s) {
+                   int first_colour, const float* e_c, cudaStream_t s, int skip_first = 0) {
     const LevelGeom& g = c->g[l];
     int done = 0;
     if (e_c && c->fast_sweep[l] && nsweeps >= 2 && c->tma_ok[l] && gmgf::tma_shape_ok(g)) {
@@ -413,9 +428,12 @@ static void smooth(gmg_ctx* c, int l, float* p, const float* b, const float* ome
         float* q = c->lv[l].q;
         const int pairs = nsweeps / 2;
         for (int i = 0; i < pairs; ++i) {
-            gmgf::rb_sweep(g, c->lv[l].L, p, q, b, omega, first_colour, (i == 0) ? e_c : nullptr, c->tma_ok[l], s);
+            if (!(i == 0 && skip_first)) {
+                gmgf::rb_sweep(g, c->lv[l].L, p, q, b, omega, first_colour, (i == 0) ? e_c : nullptr, c->tma_ok[l], s);
+                c->n_launch += 1;
+            }
             gmgf::rb_sweep(g, c->lv[l].L, q, p, b, omega, first_colour, nullptr, c->tma_ok[l], s);
-            c->n_launch += 2;
+            c->n_launch += 1;
         }
         done = 2 * pairs;
         e_c = nullptr;
@@ -433,7 +451,7 @@ static void smooth(gmg_ctx* c, int l, float* p, const float* b, const float* ome
 
 // ---- V-cycle: reading O7 (PAPER.md:39 smoother + coarse-grid correction; 51 "V-cycle") -------
 static void enqueue_vcycle(gmg_ctx* c, float* p0, const float* b0, const float* omega, int sym,
-                           cudaStream_t s) {
+                           cudaStream_t s, int skip_first = 0) {
     const bool cluster = c->ctail_start < c->nlev;
     const int nlev = c->nlev, ts = cluster ? c->ctail_start : c->tail_start;
     auto P = [&](int l) { return l == 0 ? p0 : c->lv[l].p; };
@@ -441,7 +459,7 @@ static void enqueue_vcycle(gmg_ctx* c, float* p0, const float* b0, const float* 
     const int post_first = sym ? 1 : 0;
     int l = 0;
     for (; l < ts && l < nlev - 1; ++l) {
-        smooth(c, l, P(l), B(l), omega, c->prm.nu_pre, 0, nullptr, s);
+        smooth(c, l, P(l), B(l), omega, c->prm.nu_pre, 0, nullptr, s, l == 0 ? skip_first : 0);
         if (c->fast_rr[l])
             gmgf::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, c->tma_ok[l], s);
         else
@@ -580,7 +598,24 @@ static void level0_residual_norm2(gmg_ctx* c, const float* p, const float* z, cu
 }
 
 // GMG-RBGS (readings O8, O9): pre = reference norm + initial residual norm + loop entry test.
-static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
+// fused_norm path (gmg.h): cycle k+1's first pre-sweep p -> q (out of place) also sums the squared
+// residual of p = p_k and ||z||^2.  It has to run before cycle k's omega update is known, so it
+// runs with the decay-branch omega (omega_spec_f); when the update takes the growth branch
+// instead, k_ctl_rbgs_cycle_end raises redo_first and the sweep is run again with the right omega.
+static bool fused_norm_active(const gmg_ctx* c) {
+    return c->fused_norm_on && gmgf::sweep_norm_supported(c->g[0]);
+}
+static void first_sweep_with_norm(gmg_ctx* c, float* p, const float* z, const float* omega, cudaStream_t s) {
+    gmgf::rb_sweep_with_norm(c->g[0], c->lv[0].L, p, c->lv[0].q, z, omega, 0, rbuf(c), RED_RR, RED_RREF, s);
+}
+
+static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s, bool cgs = false) {
+    if (!cgs && fused_norm_active(c)) {
+        first_sweep_with_norm(c, p, z, &c->sc->omega_f, s);
+        gmgk::ctl_begin(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
+        c->n_launch += 2;
+        return;
+    }
     // reference norm ||z|| over active cells and initial residual norm: one fused pass on big levels
     if (c->prm.fast_path && c->tma_ok[0] &&
         gmgf::residual_and_ref_norm2_bulk(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, RED_RREF, s)) {
@@ -594,6 +629,14 @@ static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStrea
     c->n_launch += 1;
 }
 static void rbgs_body(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s, bool cgs = false) {
+    if (!cgs && fused_norm_active(c)) {
+        enqueue_vcycle(c, p, z, &c->sc->omega_f, 0, s, 1);             // its first sweep already ran
+        first_sweep_with_norm(c, p, z, &c->sc->omega_spec_f, s);       // next cycle's, + ||z - A p_k||
+        gmgk::ctl_rbgs_cycle_end(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
+        gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->redo_first, s);
+        c->n_launch += 3;
+        return;
+    }
     if (cgs) enqueue_vcycle_cgs(c, p, z, s);
     else enqueue_vcycle(c, p, z, &c->sc->omega_f, 0, s);
     level0_residual_norm2(c, p, z, s);
@@ -645,7 +688,8 @@ static void enqueue_init(gmg_ctx* c, float tol, int maxiter, int solver, cudaStr
 }
 
 static void enqueue_pre(gmg_ctx* c, int solver, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
-    if (solver == GMG_GMG_RBGS || solver == GMG_GMG_CGS) rbgs_pre(c, p, z, lc, s); else pcg_pre(c, p, z, lc, s);
+    if (solver == GMG_GMG_RBGS || solver == GMG_GMG_CGS) rbgs_pre(c, p, z, lc, s, solver == GMG_GMG_CGS);
+    else pcg_pre(c, p, z, lc, s);
 }
 static void enqueue_body(gmg_ctx* c, int solver, float* p, const float* z, LoopCtl lc, cudaStream_t s) {
     if (solver == GMG_GMG_RBGS) rbgs_body(c, p, z, lc, s);
@@ -924,6 +968,25 @@ extern "C" int gmg_op_vcycle(gmg_ctx* c, float* p, const float* z, float omega, 
     gmgk::ctl_set_hook_omega(c->sc, omega, s);
     enqueue_vcycle(c, p, z, &c->sc->omega_hook, symmetric ? 1 : 0, s);
     HOOK_EPILOGUE()
+}
+
+extern "C" int gmg_op_sweep_with_norm(gmg_ctx* c, int lev, const float* src, float* dst, const float* b,
+                                      float omega, int first_colour, double* rr_out, double* bb_out,
+                                      void* stream) {
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && src && dst && b && src != dst && rr_out && bb_out &&
+                  (first_colour == 0 || first_colour == 1))
+    gmgk::ctl_set_hook_omega(c->sc, omega, s);
+    if (!gmgf::rb_sweep_with_norm(c->g[lev], c->lv[lev].L, src, dst, b, &c->sc->omega_hook, first_colour,
+                                  rbuf(c), RED_HOOK, RED_HOOK2, s)) {
+        SET_ERR(c, "gmg_op_sweep_with_norm: level %d cannot run the TMA-fed sweep", lev);
+        return GMG_EINVAL;
+    }
+    CUDA_TRY(c, cudaGetLastError());
+    CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(c, cudaStreamSynchronize(s));
+    *rr_out = c->sc_host->red[RED_HOOK];
+    *bb_out = c->sc_host->red[RED_HOOK2];
+    return GMG_OK;
 }
 
 extern "C" int gmg_op_cg_smooth(gmg_ctx* c, int lev, float* x, const float* b, int iters, void* stream) {

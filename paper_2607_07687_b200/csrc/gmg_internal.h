@@ -46,6 +46,9 @@ struct DevScalars {
     int cgs_frozen;    // CG smoother (reading O12): 1 = the remaining iterations leave x untouched
     double cgs_rho0;   // r.s at the restart of the CG smoother
     double cgs_alpha_cap;  // longest step the CG smoother accepts on the current level
+    // fused_norm path: the first sweep of cycle k+1 runs before cycle k's omega update is known
+    float omega_spec_f;    // omega it ran with: the decay branch of reading O8
+    int redo_first;        // 1: the update took the growth branch -- run that sweep again
 };
 
 // CG smoother: stop once |r.s| <= this * |r.s at the restart| (reading O12)
@@ -59,7 +62,8 @@ enum {
     RED_HOOK = 4,  // gmg_op_norm2
     RED_CHECK = 5, // coefficient check: count of bad values
     RED_CGS_SUM = 6,  // CG smoother: sum of the restart residual over active cells
-    RED_CGS_CNT = 7   // CG smoother: number of active cells
+    RED_CGS_CNT = 7,  // CG smoother: number of active cells
+    RED_HOOK2 = 8     // gmg_op_sweep_with_norm: second sum
 };
 
 #ifdef __CUDACC__

@@ -14,6 +14,15 @@ __device__ __forceinline__ void set_cond(cudaGraphConditionalHandle cond, int us
     if (use_cond) cudaGraphSetConditional(cond, go ? 1u : 0u);
 }
 
+// omega of the cycle AFTER the one about to run, if that one shrinks the residual (reading O8's
+// decay branch; the same operations as k_ctl_rbgs_cycle_end, so the values compare equal)
+__device__ __forceinline__ double speculate_omega(const DevScalars* sc) {
+    if (!sc->adaptive) return sc->omega;
+    double w = sc->omega + sc->omega_up;
+    if (!(w < 1.0)) w = 1.0;
+    return w;
+}
+
 __global__ void k_ctl_init(DevScalars* sc, double tol, int maxiter, int adaptive, double omega_min,
                            double omega_down, double omega_up) {
     sc->tol = tol;
@@ -59,6 +68,8 @@ __global__ void k_ctl_begin(DevScalars* sc, double* hist, double* omegas,
     }
     if (omegas) omegas[0] = sc->omega;
     sc->omega_f = (float)sc->omega;
+    sc->omega_spec_f = (float)speculate_omega(sc);
+    sc->redo_first = 0;
     sc->done = done;
     set_cond(cond, use_cond, !done);
 }
@@ -93,6 +104,9 @@ __global__ void k_ctl_rbgs_cycle_end(DevScalars* sc, double* hist, double* omega
     sc->status = conv ? GMG_OK : GMG_NOT_CONVERGED;
     const int done = conv || k >= sc->maxiter;
     if (!done) omegas[k] = sc->omega;
+    // fused_norm path: the next cycle's first sweep already ran with omega_spec_f
+    sc->redo_first = (!done && sc->omega_f != sc->omega_spec_f) ? 1 : 0;
+    sc->omega_spec_f = (float)speculate_omega(sc);
     sc->done = done;
     set_cond(cond, use_cond, !done);
 }

@@ -80,6 +80,11 @@ struct BulkArgs {
     int first_colour;
     int zchunk;
     int tiles_x, tiles_y;
+    // NORM variant: sums over the tile cells of r^2 (r = b - A src on active cells: the residual of
+    // the SOURCE iterate) and of b^2 on active cells, into rb.sc->red[slot_rr / slot_ref]
+    ReduceBuf rb;
+    int slot_rr, slot_ref;
+    const int* run_flag;   // != nullptr: the kernel does nothing unless *run_flag != 0
 };
 
 struct alignas(64) BulkMaps {
@@ -141,7 +146,7 @@ __device__ __forceinline__ float4 update_pair_full(float xm, float4 own, float x
 
 // YIN: the tile's TMA boxes stay inside the domain in y (every tile but the first and last
 // tile rows); the other instantiation carries the row-copy path, so the common one stays small.
-template <class C, bool YIN>
+template <class C, bool YIN, bool NORM>
 __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& maps) {
     extern __shared__ __align__(1024) float sm[];  // no static shared memory: base is 1 KB aligned
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..NB) step groups, [NB] prologue
@@ -294,6 +299,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
         if (++gz == nz) gz = 0;
     };
 
+    float acc_rr_out = 0.0f, acc_bb_out = 0.0f;   // NORM: the thread's partial sums
     if (tid < C::MAIN) {
         // ---- main threads: one float4 group of one row ---------------------------------------
         const int lx = lane_id, ry = warp_id;
@@ -322,6 +328,9 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
         K.lza = K.lzb = K.lzha = K.lzhb = K.ba = K.bb = 0.0f;
         float4 q1 = lds4(Pm1 + p_off);   // u = z0-1: source values
         float z2a = 0.0f, z2b = 0.0f;
+        // NORM: SOURCE values of plane u-1 at the lanes of plane u's second-colour cells (q1 holds
+        // the B-updated ones there), and this thread's partial sums
+        float zs_a = 0.0f, zs_b = 0.0f, acc_rr = 0.0f, acc_bb = 0.0f;
         CFull Sc;
         float4 own, ym, yp, zp;
         float hvB;
@@ -371,6 +380,30 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
             cxm = (lx == 0) ? hvC : cxm;
             cxp = last_lane ? hvC : cxp;
             float4 nw, nc;   // B(u) and C(u-1) results
+            if (NORM) {
+                // residual of the SOURCE iterate on all four cells of plane u: every operand B(u)
+                // has is a source value except plane u-1 under the second-colour cells (zs_a, zs_b)
+                const float s0 = sel ? zs_a : q1.x, s1 = sel ? q1.y : zs_a;
+                const float s2 = sel ? zs_b : q1.z, s3 = sel ? q1.w : zs_b;
+                const float A0 = apply7(own.x, Sc.lx.x, Sc.lx.y, Sc.ly.x, Sc.lyh.x, Sc.lz.x, Sc.lzh.x, xm, own.y, ym.x, yp.x, s0, zp.x);
+                const float A1 = apply7(own.y, Sc.lx.y, Sc.lx.z, Sc.ly.y, Sc.lyh.y, Sc.lz.y, Sc.lzh.y, own.x, own.z, ym.y, yp.y, s1, zp.y);
+                const float A2 = apply7(own.z, Sc.lx.z, Sc.lx.w, Sc.ly.z, Sc.lyh.z, Sc.lz.z, Sc.lzh.z, own.y, own.w, ym.z, yp.z, s2, zp.z);
+                const float A3 = apply7(own.w, Sc.lx.w, Sc.lxh, Sc.ly.w, Sc.lyh.w, Sc.lz.w, Sc.lzh.w, own.z, xp, ym.w, yp.w, s3, zp.w);
+                const bool a0 = diag6(Sc.lx.x, Sc.lx.y, Sc.ly.x, Sc.lyh.x, Sc.lz.x, Sc.lzh.x) != 0.0f;
+                const bool a1 = diag6(Sc.lx.y, Sc.lx.z, Sc.ly.y, Sc.lyh.y, Sc.lz.y, Sc.lzh.y) != 0.0f;
+                const bool a2 = diag6(Sc.lx.z, Sc.lx.w, Sc.ly.z, Sc.lyh.z, Sc.lz.z, Sc.lzh.z) != 0.0f;
+                const bool a3 = diag6(Sc.lx.w, Sc.lxh, Sc.ly.w, Sc.lyh.w, Sc.lz.w, Sc.lzh.w) != 0.0f;
+                if (row_c && u >= z0 && u < z1) {
+                    const float r0 = a0 ? Sc.b.x - A0 : 0.0f, r1 = a1 ? Sc.b.y - A1 : 0.0f;
+                    const float r2 = a2 ? Sc.b.z - A2 : 0.0f, r3 = a3 ? Sc.b.w - A3 : 0.0f;
+                    acc_rr += (r0 * r0 + r1 * r1) + (r2 * r2 + r3 * r3);
+                    const float b0 = a0 ? Sc.b.x : 0.0f, b1 = a1 ? Sc.b.y : 0.0f;
+                    const float b2 = a2 ? Sc.b.z : 0.0f, b3 = a3 ? Sc.b.w : 0.0f;
+                    acc_bb += (b0 * b0 + b1 * b1) + (b2 * b2 + b3 * b3);
+                }
+                zs_a = sel ? own.y : own.x;
+                zs_b = sel ? own.w : own.z;
+            }
             if (sel) {
                 nw = update_pair_full<1>(xm, own, xp, ym, yp, q1, zp, Sc, omega);
                 nc = update_pair_carried<1>(cxm, q1, cxp, cym, cyp, z2a, z2b, nw, K, omega);
@@ -393,6 +426,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
             cta_sync();
             if (u + C::PD <= z1) issue_step(u + C::PD);
         }
+        if (NORM) { acc_rr_out = acc_rr; acc_bb_out = acc_bb; }
     } else {
         // ---- edge warp: ring-1 cells x0-1 and x0+TX of every row, phase B only ----------------
         const int el = lane_id;
@@ -444,15 +478,62 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
             advance();
         }
     }
+    if (NORM) {
+        // deterministic two-stage reduction (FP64 from here on); the plane rings are free now
+        double v0 = 0.0, v1 = 0.0;
+        if (tid < C::MAIN) { v0 = (double)acc_rr_out; v1 = (double)acc_bb_out; }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            v0 += __shfl_down_sync(0xffffffffu, v0, o);
+            v1 += __shfl_down_sync(0xffffffffu, v1, o);
+        }
+        double* scratch = reinterpret_cast<double*>(sm);
+        int* last = reinterpret_cast<int*>(scratch + 2 * NWARP);
+        if (lane_id == 0) { scratch[warp_id] = v0; scratch[NWARP + warp_id] = v1; }
+        __syncthreads();
+        if (tid == 0) {
+            double t0 = 0.0, t1 = 0.0;
+            for (int w = 0; w < NWARP; ++w) { t0 += scratch[w]; t1 += scratch[NWARP + w]; }
+            a.rb.partials[blockIdx.x] = t0;
+            a.rb.partials[GMG_REDUCE_MAX_BLOCKS + blockIdx.x] = t1;
+            __threadfence();
+            *last = (atomicAdd(a.rb.counter, 1u) == gridDim.x - 1) ? 1 : 0;
+        }
+        __syncthreads();
+        if (*last) {
+            __threadfence();
+            double a0 = 0.0, a1 = 0.0;
+            for (unsigned int i = tid; i < gridDim.x; i += C::THREADS) {
+                a0 += ((volatile double*)a.rb.partials)[i];
+                a1 += ((volatile double*)a.rb.partials)[GMG_REDUCE_MAX_BLOCKS + i];
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                a0 += __shfl_down_sync(0xffffffffu, a0, o);
+                a1 += __shfl_down_sync(0xffffffffu, a1, o);
+            }
+            __syncthreads();
+            if (lane_id == 0) { scratch[warp_id] = a0; scratch[NWARP + warp_id] = a1; }
+            __syncthreads();
+            if (tid == 0) {
+                double t0 = 0.0, t1 = 0.0;
+                for (int w = 0; w < NWARP; ++w) { t0 += scratch[w]; t1 += scratch[NWARP + w]; }
+                a.rb.sc->red[a.slot_rr] = t0;
+                a.rb.sc->red[a.slot_ref] = t1;
+                *a.rb.counter = 0u;
+            }
+        }
+    }
 }
 
-template <class C>
+template <class C, bool NORM = false>
 __global__ void __launch_bounds__(C::THREADS, 1)
 k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
+    if (a.run_flag && *a.run_flag == 0) return;   // a re-run that turned out not to be needed
     const int ty = (blockIdx.x / a.tiles_x) % a.tiles_y;
     const int y0 = ty * C::TY;
-    if ((y0 >= 2) && (y0 + C::TY + 2 <= a.g.n[1])) sweep_body<C, true>(a, maps);
-    else sweep_body<C, false>(a, maps);
+    if ((y0 >= 2) && (y0 + C::TY + 2 <= a.g.n[1])) sweep_body<C, true, NORM>(a, maps);
+    else sweep_body<C, false, NORM>(a, maps);
 }
 
 // ---- launchers ------------------------------------------------------------------------------
@@ -507,40 +588,83 @@ bool tma_shape_ok(const LevelGeom& g) {
     return use_bulk && bulk_supported(g);
 }
 
+static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
+                                 const float* omega, int first_colour, const ReduceBuf* norm, int slot_rr,
+                                 int slot_ref, const int* run_flag, cudaStream_t s);
+
+static unsigned int bulk_grid(const LevelGeom& g, int* zchunk_out) {
+    static const int zc_env = env_int2("GMG_ZCHUNK", 64);
+    static const int zmin_env = env_int2("GMG_ZMIN", 4);
+    const int tiles_x = g.n[0] / Bulk::TX, tiles_y = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
+    const int zchunk = choose_zchunk((long long)tiles_x * tiles_y, g.n[2], zc_env, zmin_env, 148, 0);
+    if (zchunk_out) *zchunk_out = zchunk;
+    return (unsigned int)(tiles_x * tiles_y * ((g.n[2] + zchunk - 1) / zchunk));
+}
+
+// rb_sweep_with_norm will run on this level (shape fits the TMA kernel, one partial per CTA fits)
+bool sweep_norm_supported(const LevelGeom& g) {
+    return tma_shape_ok(g) && bulk_grid(g, nullptr) <= GMG_REDUCE_MAX_BLOCKS;
+}
+
 void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
               const float* omega, int first_colour, const float* e_c, int allow_tma, cudaStream_t s) {
+    // the caller applies the prolongation as its own pass in front of the TMA kernel (e_c == nullptr)
+    if (allow_tma && !e_c && rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, nullptr, 0, 0, nullptr, s))
+        return;
+    rb_sweep_v2(g, L, src, dst, b, omega, first_colour, e_c, s);
+}
+
+// The same sweep src -> dst which ALSO leaves sum r^2 (r = b - A src, active cells) in
+// red[slot_rr] and sum b^2 over active cells in red[slot_ref]: the stopping-test norm of the
+// iterate a V-cycle starts from, for the price of two more stencils per thread and step instead
+// of a 20 B/cell pass.  run_flag != nullptr: the launch is a no-op unless *run_flag != 0.
+// false = this level cannot use the TMA kernel (nothing launched).
+bool rb_sweep_with_norm(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
+                        const float* omega, int first_colour, ReduceBuf rb, int slot_rr, int slot_ref,
+                        cudaStream_t s) {
+    return rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, &rb, slot_rr, slot_ref, nullptr, s);
+}
+bool rb_sweep_if(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
+                 const float* omega, int first_colour, const int* run_flag, cudaStream_t s) {
+    return rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, nullptr, 0, 0, run_flag, s);
+}
+
+static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
+                                 const float* omega, int first_colour, const ReduceBuf* norm, int slot_rr,
+                                 int slot_ref, const int* run_flag, cudaStream_t s) {
     BulkMaps maps;
     const size_t N = (size_t)g.N;
-    // the caller applies the prolongation as its own pass in front of this kernel (e_c == nullptr)
-    bool ok = allow_tma && !e_c && tma_shape_ok(g);
+    bool ok = tma_shape_ok(g);
     ok = ok && tensor_map(src, g, Bulk::TX, Bulk::SH, &maps.p_main);
     ok = ok && tensor_map(src, g, 4, Bulk::SH, &maps.p_halo);
     ok = ok && tensor_map(L + 2 * N, g, Bulk::TX, Bulk::ROWS, &maps.lz);
     ok = ok && tensor_map(L, g, Bulk::TX, Bulk::ROWS, &maps.lx);
     ok = ok && tensor_map(L + N, g, Bulk::TX, Bulk::ROWS + 1, &maps.ly);
     ok = ok && tensor_map(b, g, Bulk::TX, Bulk::ROWS, &maps.b);
-    if (!ok) {
-        rb_sweep_v2(g, L, src, dst, b, omega, first_colour, e_c, s);
-        return;
-    }
+    if (!ok) return false;
     BulkArgs a;
     a.g = g; a.L = L; a.src = src; a.dst = dst; a.b = b; a.omega = omega;
     a.first_colour = first_colour;
+    a.rb = norm ? *norm : ReduceBuf{nullptr, nullptr, nullptr};
+    a.slot_rr = slot_rr; a.slot_ref = slot_ref;
+    a.run_flag = run_flag;
     a.tiles_x = g.n[0] / Bulk::TX;
     a.tiles_y = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
-    static const int zc_env = env_int2("GMG_ZCHUNK", 64);
-    static const int zmin_env = env_int2("GMG_ZMIN", 4);
-    const int zchunk = choose_zchunk((long long)a.tiles_x * a.tiles_y, g.n[2], zc_env, zmin_env, 148, 0);
+    int zchunk = 0;
+    const unsigned int grid = bulk_grid(g, &zchunk);
     a.zchunk = zchunk;
-    const int nzc = (g.n[2] + zchunk - 1) / zchunk;
-    const unsigned int grid = (unsigned int)(a.tiles_x * a.tiles_y * nzc);
-    k_rb_sweep_bulk<Bulk><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+    if (grid > GMG_REDUCE_MAX_BLOCKS && norm) return false;
+    if (norm) k_rb_sweep_bulk<Bulk, true><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+    else k_rb_sweep_bulk<Bulk, false><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+    return true;
 }
 
 int configure() {
     cudaError_t e = (cudaError_t)configure_v2();
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
     if (e == cudaSuccess && !g_encode) {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult qres;

@@ -33,7 +33,8 @@ class Params(C.Structure):
                 ("omega0", C.c_float), ("omega_min", C.c_float), ("omega_down", C.c_float),
                 ("omega_up", C.c_float), ("adaptive", C.c_int), ("coarsen_mode", C.c_int),
                 ("n_min", C.c_int), ("fast_path", C.c_int), ("use_graph", C.c_int),
-                ("tma_min_cells", C.c_int), ("cluster_tail", C.c_int)]
+                ("tma_min_cells", C.c_int), ("cluster_tail", C.c_int),
+                ("fused_norm", C.c_int)]
 
 
 class Stats(C.Structure):
@@ -83,6 +84,8 @@ SIGNATURES = {
     "gmg_op_residual_restrict": (C.c_int, [_vp, C.c_int, _vp, _vp, _vp, _vp]),
     "gmg_op_prolong": (C.c_int, [_vp, C.c_int, _vp, _vp, _vp]),
     "gmg_op_vcycle": (C.c_int, [_vp, _vp, _vp, C.c_float, C.c_int, _vp]),
+    "gmg_op_sweep_with_norm": (C.c_int, [_vp, C.c_int, _vp, _vp, _vp, C.c_float, C.c_int,
+                                         C.POINTER(C.c_double), C.POINTER(C.c_double), _vp]),
     "gmg_op_cg_smooth": (C.c_int, [_vp, C.c_int, _vp, _vp, C.c_int, _vp]),
     "gmg_op_vcycle_cgs": (C.c_int, [_vp, _vp, _vp, _vp]),
     "gmg_op_norm2": (C.c_int, [_vp, C.c_int, _vp, C.POINTER(C.c_double), _vp]),
@@ -319,6 +322,15 @@ class GMG:
         self._check(lib.gmg_op_vcycle(self._h, self._vec(p), self._vec(z), float(omega),
                                       int(bool(symmetric)), self._stream()))
         return p
+
+    def op_sweep_with_norm(self, lev, src, b, omega=1.0, first_colour=0):
+        """One fused red+black sweep out of place; returns (dst, sum r^2 of src, sum b^2 active)."""
+        dst = self._new(lev)
+        rr, bb = C.c_double(0.0), C.c_double(0.0)
+        self._check(lib.gmg_op_sweep_with_norm(self._h, lev, self._vec(src, lev), _vp(_ptr(dst)),
+                                               self._vec(b, lev), float(omega), int(first_colour),
+                                               C.byref(rr), C.byref(bb), self._stream()))
+        return dst, rr.value, bb.value
 
     def op_cg_smooth(self, lev, x, b, iters):
         """In place on x."""
