@@ -332,6 +332,10 @@ def run_ours(args):
     t_pair = time_kernel_loop(lambda: g.op_smooth(0, q, b0, omega=1.0, nsweeps=2), reps, stream)
     t_sweep = t_pair / 2.0
     sweep_gbs = 24.0 * N / (t_sweep * 1e-3) / 1e9
+    try:    # the variant of the sweep that also accumulates the stopping-test norm (fused_norm)
+        t_sweep_norm = time_kernel_loop(lambda: g.op_sweep_with_norm(0, q, b0, omega=1.0), reps, stream)
+    except gmg.GMGError:
+        t_sweep_norm = None
     t_rr = time_kernel_loop(lambda: g.op_residual_restrict(0, q, b0), reps, stream)
     _, c0 = g.level_shape(0)
     m = c0[0] * c0[1] * c0[2]
@@ -408,7 +412,7 @@ def run_ours(args):
         "roofline": {"bound": "hbm", "kernel": "level-0 red+black Gauss-Seidel sweep",
                      "achieved": sweep_gbs, "peak": peak, "unit": "GB/s", "frac": sweep_gbs / peak,
                      "traffic": profiled_traffic(args.workload, "sweep"), "peak_source": peak_src,
-                     "ms_per_launch": t_sweep,
+                     "ms_per_launch": t_sweep, "ms_per_launch_with_norm": t_sweep_norm,
                      "algorithmic_bytes_per_cell": 24.0,
                      "frac_of_nominal_8TBs": sweep_gbs / 8000.0},
         "roofline_residual_restrict": {"achieved": rr_gbs, "peak": peak, "unit": "GB/s",

@@ -605,13 +605,16 @@ static void level0_residual_norm2(gmg_ctx* c, const float* p, const float* z, cu
 static bool fused_norm_active(const gmg_ctx* c) {
     return c->fused_norm_on && gmgf::sweep_norm_supported(c->g[0]);
 }
-static void first_sweep_with_norm(gmg_ctx* c, float* p, const float* z, const float* omega, cudaStream_t s) {
-    gmgf::rb_sweep_with_norm(c->g[0], c->lv[0].L, p, c->lv[0].q, z, omega, 0, rbuf(c), RED_RR, RED_RREF, s);
+// with_ref: also ||z||^2 over the active cells (needed once, at loop entry)
+static void first_sweep_with_norm(gmg_ctx* c, float* p, const float* z, const float* omega, bool with_ref,
+                                  cudaStream_t s) {
+    gmgf::rb_sweep_with_norm(c->g[0], c->lv[0].L, p, c->lv[0].q, z, omega, 0, rbuf(c), RED_RR,
+                             with_ref ? RED_RREF : -1, s);
 }
 
 static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s, bool cgs = false) {
     if (!cgs && fused_norm_active(c)) {
-        first_sweep_with_norm(c, p, z, &c->sc->omega_f, s);
+        first_sweep_with_norm(c, p, z, &c->sc->omega_f, true, s);
         gmgk::ctl_begin(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
         c->n_launch += 2;
         return;
@@ -631,7 +634,7 @@ static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStrea
 static void rbgs_body(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s, bool cgs = false) {
     if (!cgs && fused_norm_active(c)) {
         enqueue_vcycle(c, p, z, &c->sc->omega_f, 0, s, 1);             // its first sweep already ran
-        first_sweep_with_norm(c, p, z, &c->sc->omega_spec_f, s);       // next cycle's, + ||z - A p_k||
+        first_sweep_with_norm(c, p, z, &c->sc->omega_spec_f, false, s);       // next cycle's, + ||z - A p_k||
         gmgk::ctl_rbgs_cycle_end(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
         gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->redo_first, s);
         c->n_launch += 3;

@@ -146,7 +146,8 @@ __device__ __forceinline__ float4 update_pair_full(float xm, float4 own, float x
 
 // YIN: the tile's TMA boxes stay inside the domain in y (every tile but the first and last
 // tile rows); the other instantiation carries the row-copy path, so the common one stays small.
-template <class C, bool YIN, bool NORM>
+// NORM: 0 = plain sweep; 1 = also sum r^2 of the source iterate; 2 = also sum b^2 over active cells
+template <class C, bool YIN, int NORM>
 __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& maps) {
     extern __shared__ __align__(1024) float sm[];  // no static shared memory: base is 1 KB aligned
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..NB) step groups, [NB] prologue
@@ -397,9 +398,11 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
                     const float r0 = a0 ? Sc.b.x - A0 : 0.0f, r1 = a1 ? Sc.b.y - A1 : 0.0f;
                     const float r2 = a2 ? Sc.b.z - A2 : 0.0f, r3 = a3 ? Sc.b.w - A3 : 0.0f;
                     acc_rr += (r0 * r0 + r1 * r1) + (r2 * r2 + r3 * r3);
-                    const float b0 = a0 ? Sc.b.x : 0.0f, b1 = a1 ? Sc.b.y : 0.0f;
-                    const float b2 = a2 ? Sc.b.z : 0.0f, b3 = a3 ? Sc.b.w : 0.0f;
-                    acc_bb += (b0 * b0 + b1 * b1) + (b2 * b2 + b3 * b3);
+                    if (NORM == 2) {
+                        const float b0 = a0 ? Sc.b.x : 0.0f, b1 = a1 ? Sc.b.y : 0.0f;
+                        const float b2 = a2 ? Sc.b.z : 0.0f, b3 = a3 ? Sc.b.w : 0.0f;
+                        acc_bb += (b0 * b0 + b1 * b1) + (b2 * b2 + b3 * b3);
+                    }
                 }
                 zs_a = sel ? own.y : own.x;
                 zs_b = sel ? own.w : own.z;
@@ -519,14 +522,14 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
                 double t0 = 0.0, t1 = 0.0;
                 for (int w = 0; w < NWARP; ++w) { t0 += scratch[w]; t1 += scratch[NWARP + w]; }
                 a.rb.sc->red[a.slot_rr] = t0;
-                a.rb.sc->red[a.slot_ref] = t1;
+                if (NORM == 2) a.rb.sc->red[a.slot_ref] = t1;
                 *a.rb.counter = 0u;
             }
         }
     }
 }
 
-template <class C, bool NORM = false>
+template <class C, int NORM = 0>
 __global__ void __launch_bounds__(C::THREADS, 1)
 k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     if (a.run_flag && *a.run_flag == 0) return;   // a re-run that turned out not to be needed
@@ -615,7 +618,7 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
 }
 
 // The same sweep src -> dst which ALSO leaves sum r^2 (r = b - A src, active cells) in
-// red[slot_rr] and sum b^2 over active cells in red[slot_ref]: the stopping-test norm of the
+// red[slot_rr] and (slot_ref >= 0) sum b^2 over active cells in red[slot_ref]: the stopping-test norm of the
 // iterate a V-cycle starts from, for the price of two more stencils per thread and step instead
 // of a 20 B/cell pass.  run_flag != nullptr: the launch is a no-op unless *run_flag != 0.
 // false = this level cannot use the TMA kernel (nothing launched).
@@ -654,17 +657,20 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
     const unsigned int grid = bulk_grid(g, &zchunk);
     a.zchunk = zchunk;
     if (grid > GMG_REDUCE_MAX_BLOCKS && norm) return false;
-    if (norm) k_rb_sweep_bulk<Bulk, true><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
-    else k_rb_sweep_bulk<Bulk, false><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+    if (norm && slot_ref >= 0) k_rb_sweep_bulk<Bulk, 2><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+    else if (norm) k_rb_sweep_bulk<Bulk, 1><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+    else k_rb_sweep_bulk<Bulk, 0><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
     return true;
 }
 
 int configure() {
     cudaError_t e = (cudaError_t)configure_v2();
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
     if (e == cudaSuccess && !g_encode) {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult qres;
