@@ -850,7 +850,11 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
     st.kernel_launches = launches;
     st.history_len = it + 1;
     const double N0 = (double)c->g[0].N;
-    if (solver == GMG_GMG_RBGS) st.bytes_algorithmic = 20.0 * N0 + it * vcycle_bytes(c, true);  // loop entry: one pass over p, z, L
+    // loop entry: one pass over p, z, L -- unless the norms ride on sweeps that run anyway (fused_norm)
+    if (solver == GMG_GMG_RBGS) {
+        const bool fn = fused_norm_active(c);
+        st.bytes_algorithmic = (fn ? 0.0 : 20.0 * N0) + it * vcycle_bytes(c, !fn);
+    }
     else if (solver == GMG_GMG_CGS) st.bytes_algorithmic = 20.0 * N0 + it * vcycle_cgs_bytes(c);
     else if (solver == GMG_PCG) st.bytes_algorithmic = 60.0 * N0 + it * 64.0 * N0;
     else st.bytes_algorithmic = 60.0 * N0 + it * (vcycle_bytes(c, false) + 52.0 * N0);
