@@ -33,7 +33,10 @@ bool tma_shape_ok(const LevelGeom& g);
 // cells in red[slot_rr] / red[slot_ref]; false = the level cannot run it (nothing launched)
 bool rb_sweep_with_norm(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
                         const float* omega, int first_colour, ReduceBuf rb, int slot_rr, int slot_ref,
-                        cudaStream_t s);
+                        const int* run_flag, cudaStream_t s);
+bool residual_norm2_bulk_if(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
+                            int slot, const int* run_flag, cudaStream_t s);
+bool residual_norm_bulk_supported(const LevelGeom& g);
 bool sweep_norm_supported(const LevelGeom& g);
 // the same sweep as a no-op unless *run_flag != 0
 bool rb_sweep_if(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
@@ -606,15 +609,20 @@ static bool fused_norm_active(const gmg_ctx* c) {
     return c->fused_norm_on && gmgf::sweep_norm_supported(c->g[0]);
 }
 // with_ref: also ||z||^2 over the active cells (needed once, at loop entry)
+// The cycle expected to be the last (kernels_ctl.cu) gets the plain norm pass instead of the next
+// cycle's norm-carrying sweep, which would be wasted when the test then ends the solve.
+static bool predict_active(const gmg_ctx* c) {
+    return fused_norm_active(c) && gmgf::residual_norm_bulk_supported(c->g[0]);
+}
 static void first_sweep_with_norm(gmg_ctx* c, float* p, const float* z, const float* omega, bool with_ref,
-                                  cudaStream_t s) {
+                                  const int* run_flag, cudaStream_t s) {
     gmgf::rb_sweep_with_norm(c->g[0], c->lv[0].L, p, c->lv[0].q, z, omega, 0, rbuf(c), RED_RR,
-                             with_ref ? RED_RREF : -1, s);
+                             with_ref ? RED_RREF : -1, run_flag, s);
 }
 
 static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s, bool cgs = false) {
     if (!cgs && fused_norm_active(c)) {
-        first_sweep_with_norm(c, p, z, &c->sc->omega_f, true, s);
+        first_sweep_with_norm(c, p, z, &c->sc->omega_f, true, nullptr, s);
         gmgk::ctl_begin(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
         c->n_launch += 2;
         return;
@@ -633,8 +641,18 @@ static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStrea
 }
 static void rbgs_body(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s, bool cgs = false) {
     if (!cgs && fused_norm_active(c)) {
+        const bool pred = predict_active(c);
+        if (pred) {   // after a failed "last cycle" prediction the first sweep is still to run
+            gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->need_first, s);
+            c->n_launch += 1;
+        }
         enqueue_vcycle(c, p, z, &c->sc->omega_f, 0, s, 1);             // its first sweep already ran
-        first_sweep_with_norm(c, p, z, &c->sc->omega_spec_f, false, s);       // next cycle's, + ||z - A p_k||
+        if (pred) {   // expected to be the last cycle: the plain norm pass
+            gmgf::residual_norm2_bulk_if(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, &c->sc->expect_last, s);
+            c->n_launch += 1;
+        }
+        // otherwise: next cycle's first sweep, + ||z - A p_k||
+        first_sweep_with_norm(c, p, z, &c->sc->omega_spec_f, false, pred ? &c->sc->run_s1n : nullptr, s);
         gmgk::ctl_rbgs_cycle_end(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
         gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->redo_first, s);
         c->n_launch += 3;
@@ -686,7 +704,8 @@ static void pcg_post(gmg_ctx* c, float* p, const float* z, cudaStream_t s) {
 static void enqueue_init(gmg_ctx* c, float tol, int maxiter, int solver, cudaStream_t s) {
     // the relaxation factor belongs to the RBGS smoother: the CG-smoothed cycle leaves it alone
     gmgk::ctl_init(c->sc, (double)tol, maxiter, solver == GMG_GMG_CGS ? 0 : c->prm.adaptive, (double)c->prm.omega_min,
-                   (double)c->prm.omega_down, (double)c->prm.omega_up, s);
+                   (double)c->prm.omega_down, (double)c->prm.omega_up,
+                   (solver == GMG_GMG_RBGS && predict_active(c)) ? 1 : 0, s);
     c->n_launch += 1;
 }
 
@@ -984,7 +1003,7 @@ extern "C" int gmg_op_sweep_with_norm(gmg_ctx* c, int lev, const float* src, flo
                   (first_colour == 0 || first_colour == 1))
     gmgk::ctl_set_hook_omega(c->sc, omega, s);
     if (!gmgf::rb_sweep_with_norm(c->g[lev], c->lv[lev].L, src, dst, b, &c->sc->omega_hook, first_colour,
-                                  rbuf(c), RED_HOOK, RED_HOOK2, s)) {
+                                  rbuf(c), RED_HOOK, RED_HOOK2, nullptr, s)) {
         SET_ERR(c, "gmg_op_sweep_with_norm: level %d cannot run the TMA-fed sweep", lev);
         return GMG_EINVAL;
     }

@@ -49,6 +49,12 @@ struct DevScalars {
     // fused_norm path: the first sweep of cycle k+1 runs before cycle k's omega update is known
     float omega_spec_f;    // omega it ran with: the decay branch of reading O8
     int redo_first;        // 1: the update took the growth branch -- run that sweep again
+    // ... and the cycle expected to be the LAST one (rate-based prediction, or maxiter reached) is
+    // followed by the plain 20 B/cell norm pass instead, so that no sweep is wasted at the exit
+    int predict;           // 1: prediction enabled for this solve
+    int expect_last;       // 1: the cycle now running is expected to meet the stopping test
+    int run_s1n;           // = !expect_last: the norm-carrying first sweep of the next cycle runs
+    int need_first;        // 1: the prediction failed -- the next cycle's first sweep still has to run
 };
 
 // CG smoother: stop once |r.s| <= this * |r.s at the restart| (reading O12)
@@ -155,7 +161,7 @@ void jacobi_apply(const LevelGeom& g, const float* L, const float* r, float* s_o
 // on-device iteration control (single-thread kernels, kernels_ctl.cu).  `cond` is the WHILE
 // node's conditional handle; use_cond = 0 outside a graph.
 void ctl_init(DevScalars* sc, double tol, int maxiter, int adaptive, double omega_min,
-              double omega_down, double omega_up, cudaStream_t s);
+              double omega_down, double omega_up, int predict, cudaStream_t s);
 void ctl_begin(DevScalars* sc, double* hist, double* omegas, cudaGraphConditionalHandle cond,
                int use_cond, cudaStream_t s);
 void ctl_rbgs_cycle_end(DevScalars* sc, double* hist, double* omegas,

@@ -24,7 +24,11 @@ __device__ __forceinline__ double speculate_omega(const DevScalars* sc) {
 }
 
 __global__ void k_ctl_init(DevScalars* sc, double tol, int maxiter, int adaptive, double omega_min,
-                           double omega_down, double omega_up) {
+                           double omega_down, double omega_up, int predict) {
+    sc->predict = predict;
+    sc->expect_last = 0;
+    sc->run_s1n = 1;
+    sc->need_first = 0;
     sc->tol = tol;
     sc->maxiter = maxiter;
     sc->adaptive = adaptive;
@@ -39,8 +43,8 @@ __global__ void k_ctl_init(DevScalars* sc, double tol, int maxiter, int adaptive
 }
 
 void ctl_init(DevScalars* sc, double tol, int maxiter, int adaptive, double omega_min,
-              double omega_down, double omega_up, cudaStream_t s) {
-    k_ctl_init<<<1, 1, 0, s>>>(sc, tol, maxiter, adaptive, omega_min, omega_down, omega_up);
+              double omega_down, double omega_up, int predict, cudaStream_t s) {
+    k_ctl_init<<<1, 1, 0, s>>>(sc, tol, maxiter, adaptive, omega_min, omega_down, omega_up, predict);
 }
 
 // After the reference norm (red[RREF]) and the initial residual norm (red[RR]).
@@ -70,6 +74,9 @@ __global__ void k_ctl_begin(DevScalars* sc, double* hist, double* omegas,
     sc->omega_f = (float)sc->omega;
     sc->omega_spec_f = (float)speculate_omega(sc);
     sc->redo_first = 0;
+    sc->need_first = 0;
+    sc->expect_last = (!done && sc->predict && sc->maxiter <= 1) ? 1 : 0;  // no rate known yet
+    sc->run_s1n = !sc->expect_last;
     sc->done = done;
     set_cond(cond, use_cond, !done);
 }
@@ -104,9 +111,23 @@ __global__ void k_ctl_rbgs_cycle_end(DevScalars* sc, double* hist, double* omega
     sc->status = conv ? GMG_OK : GMG_NOT_CONVERGED;
     const int done = conv || k >= sc->maxiter;
     if (!done) omegas[k] = sc->omega;
-    // fused_norm path: the next cycle's first sweep already ran with omega_spec_f
-    sc->redo_first = (!done && sc->omega_f != sc->omega_spec_f) ? 1 : 0;
+    // fused_norm path.  This cycle's norm came either from the next cycle's first sweep, which then
+    // already ran with omega_spec_f (re-run it if the omega update went the other way), or -- the
+    // cycle was expected to be the last -- from the plain norm pass, and that sweep is still to run.
+    if (sc->expect_last) {
+        sc->need_first = !done;
+        sc->redo_first = 0;
+    } else {
+        sc->need_first = 0;
+        sc->redo_first = (!done && sc->omega_f != sc->omega_spec_f) ? 1 : 0;
+    }
     sc->omega_spec_f = (float)speculate_omega(sc);
+    // expect the NEXT cycle to be the last if it is the maxiter-th, or if one more reduction by the
+    // factor just seen lands a factor two below the tolerance
+    const double rho_old = sc->rho_prev;   // the norm before this cycle
+    const bool rate_says = rho_new < rho_old && 2.0 * rho_new * (rho_new / rho_old) <= sc->tol * sc->r_ref;
+    sc->expect_last = (!done && sc->predict && (k + 1 >= sc->maxiter || rate_says)) ? 1 : 0;
+    sc->run_s1n = !sc->expect_last;
     sc->done = done;
     set_cond(cond, use_cond, !done);
 }

@@ -61,6 +61,7 @@ struct ResBulkArgs {
     int slot, slot2;
     int zchunk;
     int tiles_x, tiles_y;
+    const int* run_flag;   // != nullptr: the kernel does nothing unless *run_flag != 0
 };
 
 struct alignas(64) ResBulkMaps {
@@ -71,6 +72,7 @@ template <int MODE>
 __global__ void __launch_bounds__(ResBulkCfg::THREADS, 2)
 k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
     using C = ResBulkCfg;
+    if (a.run_flag && *a.run_flag == 0) return;
     extern __shared__ __align__(128) float sm[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..NB) steps, [NB] prologue
     const LevelGeom& g = a.g;
@@ -407,6 +409,7 @@ bool residual_restrict_bulk(const LevelGeom& g, const float* L, const float* p, 
     a.rb = ReduceBuf{nullptr, nullptr, nullptr};
     a.slot = 0;
     a.slot2 = 0;
+    a.run_flag = nullptr;
     return launch_res_bulk<0>(a, s);
 }
 
@@ -417,7 +420,24 @@ bool residual_norm2_bulk(const LevelGeom& g, const float* L, const float* p, con
     a.rb = rb;
     a.slot = slot;
     a.slot2 = 0;
+    a.run_flag = nullptr;
     return launch_res_bulk<1>(a, s);
+}
+
+// the same pass as a no-op unless *run_flag != 0 (fused_norm: the cycle expected to be the last)
+bool residual_norm2_bulk_if(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
+                            int slot, const int* run_flag, cudaStream_t s) {
+    ResBulkArgs a;
+    a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = nullptr; a.p_c = nullptr;
+    a.rb = rb;
+    a.slot = slot;
+    a.slot2 = 0;
+    a.run_flag = run_flag;
+    return launch_res_bulk<1>(a, s);
+}
+bool residual_norm_bulk_supported(const LevelGeom& g) {
+    static const int use_bulk = getenv("GMG_BULK") ? atoi(getenv("GMG_BULK")) : 1;
+    return use_bulk && bulk_supported(g) && !(g.n[2] & 1);
 }
 
 // sum r^2 -> red[slot_rr] and sum b^2 over active cells -> red[slot_ref] in ONE pass (loop entry)
@@ -428,6 +448,7 @@ bool residual_and_ref_norm2_bulk(const LevelGeom& g, const float* L, const float
     a.rb = rb;
     a.slot = slot_rr;
     a.slot2 = slot_ref;
+    a.run_flag = nullptr;
     return launch_res_bulk<2>(a, s);
 }
 
@@ -440,6 +461,7 @@ bool matvec_dot_bulk(const LevelGeom& g, const float* L, const float* d, float* 
     a.rb = rb;
     a.slot = slot;
     a.slot2 = 0;
+    a.run_flag = nullptr;
     return launch_res_bulk<3>(a, s);
 }
 

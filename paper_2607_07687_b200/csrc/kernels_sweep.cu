@@ -624,8 +624,8 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
 // false = this level cannot use the TMA kernel (nothing launched).
 bool rb_sweep_with_norm(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
                         const float* omega, int first_colour, ReduceBuf rb, int slot_rr, int slot_ref,
-                        cudaStream_t s) {
-    return rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, &rb, slot_rr, slot_ref, nullptr, s);
+                        const int* run_flag, cudaStream_t s) {
+    return rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, &rb, slot_rr, slot_ref, run_flag, s);
 }
 bool rb_sweep_if(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
                  const float* omega, int first_colour, const int* run_flag, cudaStream_t s) {
