@@ -139,3 +139,22 @@ def test_jellyfish_step_sequence_is_compatible_and_moves_smoothly():
         if prev is not None:
             assert 0.0 < np.abs(L - prev).max() < 0.5
         prev = L
+
+
+def test_maximum_grid_size_is_planned_on_the_host_and_one_more_cell_is_refused(libpath):
+    """The library indexes a level with 32-bit cell counts: 2^31 - 1 cells at most.  The largest
+    grids are planned without a GPU (level table, workspace) and the first one too large is refused
+    by gmg_plan and gmg_create alike."""
+    from paper_2607_07687_b200 import gmg
+    shapes, factors, tail, ws = gmg.plan((2048, 1024, 1022), (0, 0, 0))
+    import oracle
+    # periodic z: 1022 / 2 = 511 is odd, so z never coarsens (reading O4); x and y go down to 4
+    assert shapes[0] == (2048, 1024, 1022) and shapes[1] == (1024, 512, 1022) and shapes[-1] == (4, 4, 1022)
+    assert shapes == oracle.level_shapes((2048, 1024, 1022), (0, 0, 0))
+    N = [s[0] * s[1] * s[2] for s in shapes]
+    assert N[0] < 2 ** 31 and ws > 4 * 7 * N[0]
+    with pytest.raises(ValueError):
+        gmg.plan((2048, 1024, 1024), (0, 0, 0))                                  # 2^31 cells
+    h = C.c_void_p()
+    I3 = C.c_int * 3
+    assert gmg.lib.gmg_create(C.byref(h), 2048, 1024, 1024, I3(0, 0, 0)) == gmg.EINVAL
