@@ -228,6 +228,16 @@ int gmg_op_norm2(gmg_ctx* ctx, int lev, const float* r_dev, double* out_host, vo
 int gmg_divergence(gmg_ctx* ctx, const float* u_dev, const float wall_hi[3], float* z_dev, void* stream);
 int gmg_project(gmg_ctx* ctx, float* u_dev, const float* p_dev, void* stream);
 
+/* One whole pressure step in one call (a moving body): gmg_set_coeffs(L_dev)
+ * -> z = gmg_divergence(u_dev, wall_hi) into a library-held buffer -> gmg_solve(p_dev: in = guess, e.g.
+ * the previous step's pressure, out = solution) -> gmg_project(u_dev, p_dev), enqueued back to back on
+ * `stream` with ONE host synchronisation (the solve's status read) instead of four.  Returns the
+ * solve's code (gmg_stats describes the solve), or GMG_EINVAL when L holds a negative / non-finite value
+ * (u, p are then meaningless).  The projection is stream-ordered behind the return: synchronise
+ * `stream` before reading u on the host. */
+int gmg_pressure_step(gmg_ctx* ctx, const float* L_dev, float* u_dev, const float wall_hi[3], float* p_dev,
+                      float tol, int maxiter, int solver, void* stream);
+
 /* Names of the kernels a V-cycle launches per level, for profiling notes: writes a
  * NUL-terminated description into buf. */
 int gmg_describe_plan(const gmg_ctx* ctx, char* buf, size_t cap);

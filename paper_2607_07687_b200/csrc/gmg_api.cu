@@ -369,10 +369,8 @@ extern "C" int gmg_level_shape(const gmg_ctx* c, int lev, int n[3], int cf[3]) {
 }
 
 // ---- coefficients: reading O5 ("anisotropic coarsening operators") ---------------
-extern "C" int gmg_set_coeffs(gmg_ctx* c, const float* L_dev, void* stream) {
-    if (!c || !L_dev) return GMG_EINVAL;
-    if (!c->ws_set) { SET_ERR(c, "gmg_set_coeffs before gmg_set_workspace"); return GMG_ESTATE; }
-    cudaStream_t s = (cudaStream_t)stream;
+// Enqueues the whole coefficient pass (validation count lands in red[RED_CHECK]); no host sync.
+static void set_coeffs_enqueue(gmg_ctx* c, const float* L_dev, cudaStream_t s) {
     // the captured solve graphs hold pointers only: a moving body that rewrites the SAME array
     // every step keeps them; a new array drops them
     if (c->lv[0].L != L_dev) drop_graphs(c);
@@ -390,6 +388,13 @@ extern "C" int gmg_set_coeffs(gmg_ctx* c, const float* L_dev, void* stream) {
     for (int l = (c->ctail_start < c->tail_start ? c->ctail_start : c->tail_start); l < c->nlev; ++l)
         gmgk::tail_weights(c->g[l], c->lv[l].L, c->tail_W[l], s);
     gmgk::ctl_set_omega(c->sc, (double)c->prm.omega0, s);
+}
+
+extern "C" int gmg_set_coeffs(gmg_ctx* c, const float* L_dev, void* stream) {
+    if (!c || !L_dev) return GMG_EINVAL;
+    if (!c->ws_set) { SET_ERR(c, "gmg_set_coeffs before gmg_set_workspace"); return GMG_ESTATE; }
+    cudaStream_t s = (cudaStream_t)stream;
+    set_coeffs_enqueue(c, L_dev, s);
     CUDA_TRY(c, cudaGetLastError());
     CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
     CUDA_TRY(c, cudaStreamSynchronize(s));
@@ -1061,6 +1066,33 @@ extern "C" int gmg_project(gmg_ctx* c, float* u_dev, const float* p_dev, void* s
     CUDA_TRY(c, cudaGetLastError());
     CUDA_TRY(c, cudaStreamSynchronize(s));
     return GMG_OK;
+}
+
+// One pressure step, enqueued back to back with ONE host synchronisation (the solve's status read):
+// coefficients -> z = div u* (library-held buffer) -> solve (p_dev in/out) -> u* -= L grad p.
+extern "C" int gmg_pressure_step(gmg_ctx* c, const float* L_dev, float* u_dev, const float wall_hi[3],
+                                 float* p_dev, float tol, int maxiter, int solver, void* stream) {
+    if (!c) return GMG_EINVAL;
+    if (!L_dev || !u_dev || !p_dev) { SET_ERR(c, "gmg_pressure_step: null pointer"); return GMG_EINVAL; }
+    if (!c->ws_set) { SET_ERR(c, "gmg_pressure_step before gmg_set_workspace"); return GMG_ESTATE; }
+    cudaStream_t s = (cudaStream_t)stream;
+    const float zero[3] = {0.0f, 0.0f, 0.0f};
+    set_coeffs_enqueue(c, L_dev, s);
+    c->coeffs_set = true;   // provisionally: the validation count is read with the solve's status block
+    if (c->prm.fast_path && c->g[0].n[0] % 4 == 0) gmgk::divergence4(c->g[0], u_dev, wall_hi ? wall_hi : zero, c->stage_z, s);
+    else gmgk::divergence(c->g[0], u_dev, wall_hi ? wall_hi : zero, c->stage_z, s);
+    CUDA_TRY(c, cudaGetLastError());
+    const int rc = gmg_solve(c, p_dev, c->stage_z, tol, maxiter, solver, stream);
+    if (c->sc_host->red[RED_CHECK] != 0.0) {
+        SET_ERR(c, "gmg_pressure_step: %.0f coefficient(s) negative, NaN or infinite", c->sc_host->red[RED_CHECK]);
+        c->coeffs_set = false;
+        return GMG_EINVAL;
+    }
+    if (rc < 0) return rc;
+    if (c->prm.fast_path && c->g[0].n[0] % 4 == 0) gmgk::project4(c->g[0], c->lv[0].L, p_dev, u_dev, s);
+    else gmgk::project(c->g[0], c->lv[0].L, p_dev, u_dev, s);
+    CUDA_TRY(c, cudaGetLastError());
+    return rc;   // the projection is stream-ordered: synchronise `stream` before reading u on the host
 }
 
 extern "C" int gmg_describe_plan(const gmg_ctx* c, char* buf, size_t cap) {

@@ -91,6 +91,7 @@ SIGNATURES = {
     "gmg_op_norm2": (C.c_int, [_vp, C.c_int, _vp, C.POINTER(C.c_double), _vp]),
     "gmg_divergence": (C.c_int, [_vp, _vp, C.POINTER(C.c_float), _vp, _vp]),
     "gmg_project": (C.c_int, [_vp, _vp, _vp, _vp]),
+    "gmg_pressure_step": (C.c_int, [_vp, _vp, _vp, C.POINTER(C.c_float), _vp, C.c_float, C.c_int, C.c_int, _vp]),
     "gmg_describe_plan": (C.c_int, [_vp, C.c_char_p, C.c_size_t]),
 }
 
@@ -365,6 +366,20 @@ class GMG:
         assert tuple(u.shape) == (3, self.n[2], self.n[1], self.n[0])
         self._check(lib.gmg_project(self._h, _vp(_ptr(u)), self._vec(p), self._stream()))
         return u
+
+    def pressure_step(self, L: torch.Tensor, u: torch.Tensor, p: torch.Tensor, wall_hi=(0.0, 0.0, 0.0),
+                      tol=1e-4, maxiter=50, solver=GMG_RBGS):
+        """set_coeffs(L) -> div u -> solve (p in/out) -> u -= L grad p, one host synchronisation.
+        Returns the solve's status code; u is projected in place (stream-ordered)."""
+        shape3 = (3, self.n[2], self.n[1], self.n[0])
+        for t in (L, u):
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == shape3
+        wh = (C.c_float * 3)(*[float(v) for v in wall_hi])
+        rc = lib.gmg_pressure_step(self._h, _vp(_ptr(L)), _vp(_ptr(u)), wh, self._vec(p), float(tol),
+                                   int(maxiter), int(solver), self._stream())
+        self._check(rc, allow_warning=True)
+        self._L = L          # kept by pointer
+        return rc
 
     def describe_plan(self) -> str:
         buf = C.create_string_buffer(4096)

@@ -3,7 +3,8 @@
 
     gmg_set_coeffs(L)  ->  z = gmg_divergence(u*)  ->  gmg_solve(p, z)  ->  gmg_project(u*, p)
 
-with p kept from the previous step as the initial guess (the warm start behind Table 1's ~2
+(one call, gmg_pressure_step: the four are enqueued back to back with a single host
+synchronisation; `fused=False` issues the four calls one by one) with p kept from the previous step as the initial guess (the warm start behind Table 1's ~2
 V-cycles per step).  Argument marshalling only: every step runs in the CUDA
 kernels behind include/gmg.h."""
 import torch
@@ -12,8 +13,10 @@ from . import gmg
 
 
 class PressureStepper:
-    def __init__(self, n, bc, solver=gmg.GMG_RBGS, tol=1e-4, maxiter=50, device="cuda:0", **params):
+    def __init__(self, n, bc, solver=gmg.GMG_RBGS, tol=1e-4, maxiter=50, device="cuda:0", fused=True,
+                 **params):
         self.g = gmg.GMG(n, bc, device=device, **params)
+        self.fused = fused
         self.solver, self.tol, self.maxiter = solver, tol, maxiter
         nx, ny, nz = n
         self.p = torch.zeros((nz, ny, nx), dtype=torch.float32, device=device)
@@ -25,6 +28,10 @@ class PressureStepper:
         L tensor, rewritten in place, every step keeps the captured solve graph.
         Returns (status code, stats dict of the solve)."""
         self._L = L
+        if self.fused:
+            rc = self.g.pressure_step(L, ustar, self.p, wall_hi, tol=self.tol, maxiter=self.maxiter,
+                                      solver=self.solver)
+            return rc, self.g.stats()
         self.g.set_coeffs(L)
         z = self.g.divergence(ustar, wall_hi, out=self.z)
         rc = self.g.solve(self.p, z, tol=self.tol, maxiter=self.maxiter, solver=self.solver)

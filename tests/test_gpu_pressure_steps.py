@@ -100,3 +100,30 @@ def test_rewriting_the_coefficients_in_place_reuses_the_graph_and_changes_nothin
     finally:
         a.close()
         b.close()
+
+
+def test_one_call_pressure_step_equals_the_four_calls_and_rejects_bad_coefficients():
+    import torch
+    p_exp, nsteps = 4, 3
+    nx = 2 ** (p_exp + 1)
+    n, bc = (nx, nx, nx // 2), W.JELLYFISH_BC
+    a = PressureStepper(n, bc, fused=True)
+    b = PressureStepper(n, bc, fused=False)
+    try:
+        for L32, u32 in W.jellyfish_steps(p_exp, nsteps):
+            ua, ub = dev(u32), dev(u32)
+            rca, sta = a.step(dev(L32), ua)
+            rcb, stb = b.step(dev(L32), ub)
+            torch.cuda.synchronize()
+            assert rca == rcb == gmg.OK and sta["iterations"] == stb["iterations"]
+            assert torch.equal(a.p, b.p) and torch.equal(ua, ub)
+        bad = dev(L32)
+        bad[1, 3, 4, 5] = -0.25
+        with pytest.raises(gmg.GMGError):
+            a.step(bad, dev(u32))
+        # and the context recovers with valid coefficients
+        rc, _ = a.step(dev(L32), dev(u32))
+        assert rc == gmg.OK
+    finally:
+        a.close()
+        b.close()
