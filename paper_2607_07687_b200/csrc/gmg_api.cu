@@ -84,6 +84,7 @@ struct gmg_ctx {
     unsigned int* counter;
     double *hist, *omegas;
     int hist_cap;
+    double* hist_pin;     // pinned mirror: [0, cap) history, [cap, 2 cap) omegas -- read with the status block
     DevScalars* sc_host;  // pinned mirror
     std::vector<double> hist_host, omegas_host;
     gmg_stats_t stats;
@@ -238,7 +239,7 @@ extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]
     for (int d = 0; d < 3; ++d) { c->n0[d] = n[d]; c->bc[d] = bc[d]; }
     gmg_default_params(&c->prm);
     c->ws = nullptr; c->ws_bytes = 0; c->ws_set = false; c->coeffs_set = false;
-    c->hist = c->omegas = nullptr; c->hist_cap = 0;
+    c->hist = c->omegas = nullptr; c->hist_cap = 0; c->hist_pin = nullptr;
     memset(&c->stats, 0, sizeof(c->stats));
     memset(c->lv, 0, sizeof(c->lv));
     c->sc = nullptr; c->partials = nullptr; c->counter = nullptr; c->sc_host = nullptr;
@@ -280,6 +281,7 @@ extern "C" void gmg_destroy(gmg_ctx* c) {
     if (c->counter) cudaFree(c->counter);
     if (c->hist) cudaFree(c->hist);
     if (c->omegas) cudaFree(c->omegas);
+    if (c->hist_pin) cudaFreeHost(c->hist_pin);
     if (c->sc_host) cudaFreeHost(c->sc_host);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -785,13 +787,24 @@ static int ensure_history(gmg_ctx* c, int maxiter) {
     drop_graphs(c);
     if (c->hist) cudaFree(c->hist);
     if (c->omegas) cudaFree(c->omegas);
-    c->hist = c->omegas = nullptr;
+    if (c->hist_pin) cudaFreeHost(c->hist_pin);
+    c->hist = c->omegas = c->hist_pin = nullptr;
     c->hist_cap = 0;
     const int cap = need < 64 ? 64 : need;
     CUDA_TRY(c, cudaMalloc(&c->hist, sizeof(double) * cap));
     CUDA_TRY(c, cudaMalloc(&c->omegas, sizeof(double) * cap));
+    CUDA_TRY(c, cudaMallocHost(&c->hist_pin, sizeof(double) * 2 * cap));
     c->hist_cap = cap;
     return GMG_OK;
+}
+
+// history[0..maxiter] and omegas[0..maxiter) into the pinned mirror, behind the solve on `s`
+static cudaError_t read_history_async(gmg_ctx* c, int maxiter, cudaStream_t s) {
+    const size_t n = (size_t)maxiter + 1;
+    cudaError_t e = cudaMemcpyAsync(c->hist_pin, c->hist, sizeof(double) * n, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(c->hist_pin + c->hist_cap, c->omegas, sizeof(double) * n, cudaMemcpyDeviceToHost, s);
+    return e;
 }
 
 extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int maxiter, int solver,
@@ -828,6 +841,7 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
         CUDA_TRY(c, cudaGraphLaunch(slot.exec, s));
         CUDA_TRY(c, cudaEventRecord(c->ev1, s));
         CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
+        CUDA_TRY(c, read_history_async(c, maxiter, s));
         CUDA_TRY(c, cudaStreamSynchronize(s));
         launches = slot.n_pre + slot.n_post + slot.n_body * (long long)c->sc_host->iter;
     } else {
@@ -847,17 +861,19 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
         enqueue_post(c, solver, p, z, s);
         CUDA_TRY(c, cudaEventRecord(c->ev1, s));
         CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
+        CUDA_TRY(c, read_history_async(c, maxiter, s));
         CUDA_TRY(c, cudaStreamSynchronize(s));
         launches = c->n_launch;
     }
     CUDA_TRY(c, cudaGetLastError());
     const DevScalars& h = *c->sc_host;
     const int it = h.iter;
-    c->hist_host.assign((size_t)it + 1, 0.0);
-    c->omegas_host.assign((size_t)it, 0.0);
-    CUDA_TRY(c, cudaMemcpy(c->hist_host.data(), c->hist, sizeof(double) * (it + 1), cudaMemcpyDeviceToHost));
-    if ((solver == GMG_GMG_RBGS || solver == GMG_GMG_CGS) && it > 0)
-        CUDA_TRY(c, cudaMemcpy(c->omegas_host.data(), c->omegas, sizeof(double) * it, cudaMemcpyDeviceToHost));
+    // history and omegas came down with the status block (one synchronisation per solve)
+    c->hist_host.assign(c->hist_pin, c->hist_pin + it + 1);
+    if (solver == GMG_GMG_RBGS || solver == GMG_GMG_CGS)
+        c->omegas_host.assign(c->hist_pin + c->hist_cap, c->hist_pin + c->hist_cap + it);
+    else
+        c->omegas_host.assign((size_t)it, 0.0);
     float ms = 0.0f;
     CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1));
     gmg_stats_t& st = c->stats;
