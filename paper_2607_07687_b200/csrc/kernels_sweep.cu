@@ -87,8 +87,15 @@ struct BulkArgs {
     const int* run_flag;   // != nullptr: the kernel does nothing unless *run_flag != 0
 };
 
-struct alignas(64) BulkMaps {
+struct alignas(64) MapSet {
     CUtensorMap p_main, p_halo, lz, lx, ly, b;
+};
+// [0] full boxes (tiles inside the domain in y; with a Neumann y axis every tile: rows outside
+// arrive as zeros, which is what a wall needs); [1] the FIRST tile row of a periodic y axis: boxes
+// that start at y = 0; [2] its FINAL tile row: boxes that end at y = ny - 1.  The few wrapped rows
+// of [1] and [2] come as row copies (YMODE 2 below).
+struct alignas(64) BulkMaps {
+    MapSet m[3];
 };
 
 struct CFull {  // coefficients of the four own cells in one plane (lower faces, the y/z faces above, b)
@@ -144,11 +151,15 @@ __device__ __forceinline__ float4 update_pair_full(float xm, float4 own, float x
     return update_pair<S>(xm, own, xp, ym, yp, zm, zp, s, c.lz, omega);
 }
 
-// YIN: the tile's TMA boxes stay inside the domain in y (every tile but the first and last
+// YMODE 0: full TMA boxes.  YMODE 1: row-by-row bulk copies with wrapped row addresses (odd cases
+// of a periodic y axis).  YMODE 2: first / final tile row of a periodic y axis -- shorter boxes over
+// the rows inside the domain plus row copies for the two or three wrapped rows of each stream;
+// box and row copies write disjoint rows of a slot and complete on the same mbarrier.
+// (was) YIN: the tile's TMA boxes stay inside the domain in y (every tile but the first and last
 // tile rows); the other instantiation carries the row-copy path, so the common one stays small.
 // NORM: 0 = plain sweep; 1 = also sum r^2 of the source iterate; 2 = also sum b^2 over active cells
-template <class C, bool YIN, int NORM>
-__device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& maps) {
+template <class C, int YMODE, int NORM>
+__device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& allmaps) {
     extern __shared__ __align__(1024) float sm[];  // no static shared memory: base is 1 KB aligned
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..NB) step groups, [NB] prologue
     const float** row_base = reinterpret_cast<const float**>(bars + 16);  // row-copy path tables
@@ -172,7 +183,28 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
     const float omega = *a.omega;
     const int fc = a.first_colour;
     const int xL = wrapi(x0 - 4, nx), xR = wrapi(x0 + C::TX, nx);  // halo column groups
-    constexpr bool y_inside = YIN;
+    constexpr bool y_inside = (YMODE == 0);
+    constexpr bool y_rows = (YMODE == 1);
+    // YMODE 2 geometry (uniform over the CTA): which map set, where the boxes start (global row and
+    // row offset in the slot), the wrapped rows (slot row j <- global row y), the bytes per group
+    const bool y_first = (y0 == 0);
+    const MapSet& maps = allmaps.m[YMODE == 2 ? (y_first ? 1 : 2) : 0];
+    const int hP = ny - y0 + 2, hC = ny - y0 + 1;          // FINAL: rows of the p / coefficient boxes
+    const int e_oP = y_first ? 2 : 0, e_oC = y_first ? 1 : 0;
+    // a tensor box must land on a 128-byte boundary: in a FIRST tile the x-halo columns (16 B per
+    // row) are kept 6 rows further down in their padded area, so that row 2 -- where the box
+    // starts -- sits at byte 128 (HPAD leaves room: (SH + 6) * 4 <= HPAD)
+    static_assert((C::SH + 6) * 4 <= C::HPAD, "halo padding");
+    const int hs = (YMODE == 2 && y_first) ? 24 : 0;
+    const int e_yP = y_first ? 0 : y0 - 2, e_yC = y_first ? 0 : y0 - 1;
+    const int e_pj0 = y_first ? 0 : hP, e_py0 = y_first ? ny - 2 : 0;     // p: rows j0, j0+1 <- y0', y0'+1
+    const int e_cj = y_first ? 0 : hC, e_cy = y_first ? ny - 1 : 0;       // Lz, Lx, b, Ly: row j <- y
+    const bool e_ly2 = !y_first;                                          // Ly FINAL: also row j+1 <- 1
+    const uint32_t e_pbytes = (uint32_t)((y_first ? C::SH : hP + 2) * (C::TX + 8)) * 4u;
+    const uint32_t e_cbytes = (uint32_t)((y_first ? C::ROWS : hC + 1) * C::TX) * 4u;
+    const uint32_t e_lybytes = (uint32_t)((y_first ? C::ROWS + 1 : hC + 2) * C::TX) * 4u;
+    const uint32_t step_bytes = (YMODE == 2) ? e_pbytes + 3u * e_cbytes + e_lybytes : C::STEP_BYTES;
+    const uint32_t pro_bytes = (YMODE == 2) ? 2u * e_pbytes + e_cbytes : C::PRO_BYTES;
     const float* Lx = a.L;
     const float* Ly = a.L + N;
     const float* Lz = a.L + 2 * N;
@@ -188,7 +220,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
     // Interior tiles: 7 TMA boxes per step, one per warp 0..6 (lane 0).  Tiles touching the y
     // boundary: row-by-row bulk copies with wrapped row addresses, dealt round-robin to the warps.
     // kind 0: p(v+1) rows y0-2..   1: Lz(v+1)   2: Lx(v)   3: Ly(v) (one more row)   4: b(v)
-    if (!y_inside && tid < C::NROWCOPY) {
+    if (y_rows && tid < C::NROWCOPY) {
         int t = tid, ck, crow;
         if (t < C::SH) { ck = 0; crow = t; }
         else if ((t -= C::SH) < C::ROWS) { ck = 1; crow = t; }
@@ -221,7 +253,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
     auto issue_step = [&](int v) {  // the data B(v) newly needs: p(v+1), Lz(v+1), Lx(v), Ly(v), b(v)
         if (lane_id != 0 || (y_inside && warp_id >= 7)) return;
         uint64_t* bar = bars + ((v - (z0 - 1)) % C::NB);
-        if (tid == 0) mbar_expect_tx(bar, C::STEP_BYTES);
+        if (tid == 0) mbar_expect_tx(bar, step_bytes);
         const int gz0 = wrap1(v, nz), gz1 = wrap1(v + 1, nz);
         const int vp = v + 1, gzv = gz1;                     // the p plane of this group
         if (y_inside) {
@@ -233,6 +265,33 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
                 case 4: tma_load_3d(slotLx(v), &maps.lx, x0, y0 - 1, gz0, bar); break;
                 case 5: tma_load_3d(slotLy(v), &maps.ly, x0, y0 - 1, gz0, bar); break;
                 case 6: tma_load_3d(slotB(v), &maps.b, x0, y0 - 1, gz0, bar); break;
+                default: break;
+            }
+        } else if (YMODE == 2) {
+            const size_t pz0 = (size_t)gz0 * plane, pz1 = (size_t)gz1 * plane;
+            switch (warp_id) {
+                case 0: tma_load_3d(slotP(vp) + e_oP * C::TX, &maps.p_main, x0, e_yP, gzv, bar); break;
+                case 1: tma_load_3d(slotP(vp) + C::P_HL + hs + e_oP * 4, &maps.p_halo, xL, e_yP, gzv, bar); break;
+                case 2: tma_load_3d(slotP(vp) + C::P_HR + hs + e_oP * 4, &maps.p_halo, xR, e_yP, gzv, bar); break;
+                case 3: tma_load_3d(slotLz(v + 1) + e_oC * C::TX, &maps.lz, x0, e_yC, gz1, bar); break;
+                case 4: tma_load_3d(slotLx(v) + e_oC * C::TX, &maps.lx, x0, e_yC, gz0, bar); break;
+                case 5: tma_load_3d(slotLy(v) + e_oC * C::TX, &maps.ly, x0, e_yC, gz0, bar); break;
+                case 6: tma_load_3d(slotB(v) + e_oC * C::TX, &maps.b, x0, e_yC, gz0, bar); break;
+                case 7: case 8: {   // the two wrapped p rows
+                    const int r = warp_id - 7, j = e_pj0 + r;
+                    const float* rb = a.src + pz1 + (size_t)(e_py0 + r) * nx;
+                    float* d = slotP(vp);
+                    bulk_g2s(d + j * C::TX, rb + x0, C::TX * 4u, bar);
+                    bulk_g2s(d + C::P_HL + hs + j * 4, rb + xL, 16u, bar);
+                    bulk_g2s(d + C::P_HR + hs + j * 4, rb + xR, 16u, bar);
+                } break;
+                case 9: bulk_g2s(slotLz(v + 1) + e_cj * C::TX, Lz + pz1 + (size_t)e_cy * nx + x0, C::TX * 4u, bar); break;
+                case 10: bulk_g2s(slotLx(v) + e_cj * C::TX, Lx + pz0 + (size_t)e_cy * nx + x0, C::TX * 4u, bar); break;
+                case 11:
+                    bulk_g2s(slotLy(v) + e_cj * C::TX, Ly + pz0 + (size_t)e_cy * nx + x0, C::TX * 4u, bar);
+                    if (e_ly2) bulk_g2s(slotLy(v) + (e_cj + 1) * C::TX, Ly + pz0 + (size_t)(e_cy + 1) * nx + x0, C::TX * 4u, bar);
+                    break;
+                case 12: bulk_g2s(slotB(v) + e_cj * C::TX, a.b + pz0 + (size_t)e_cy * nx + x0, C::TX * 4u, bar); break;
                 default: break;
             }
         } else {
@@ -254,7 +313,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
     {
         uint64_t* bar = bars + C::NB;
         if (lane_id == 0) {
-            if (tid == 0) mbar_expect_tx(bar, C::PRO_BYTES);
+            if (tid == 0) mbar_expect_tx(bar, pro_bytes);
             const int gb = wrap1(z0 - 1, nz);
             if (y_inside) {
                 // planes z0-2, z0-1: three boxes each, one per warp; then Lz(z0-1)
@@ -266,6 +325,25 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
                     else tma_load_3d(slotP(v) + C::P_HR, &maps.p_halo, xR, y0 - 2, gv, bar);
                 } else if (warp_id == 6) {
                     tma_load_3d(slotLz(z0 - 1), &maps.lz, x0, y0 - 1, gb, bar);
+                }
+            } else if (YMODE == 2) {
+                const int pl = warp_id / 3, k = warp_id % 3;
+                if (pl < 2) {
+                    const int v = z0 - 2 + pl, gv = wrapi(v, nz);
+                    if (k == 0) tma_load_3d(slotP(v) + e_oP * C::TX, &maps.p_main, x0, e_yP, gv, bar);
+                    else if (k == 1) tma_load_3d(slotP(v) + C::P_HL + hs + e_oP * 4, &maps.p_halo, xL, e_yP, gv, bar);
+                    else tma_load_3d(slotP(v) + C::P_HR + hs + e_oP * 4, &maps.p_halo, xR, e_yP, gv, bar);
+                } else if (warp_id == 6) {
+                    tma_load_3d(slotLz(z0 - 1) + e_oC * C::TX, &maps.lz, x0, e_yC, gb, bar);
+                } else if (warp_id >= 7 && warp_id <= 10) {      // wrapped p rows of the two planes
+                    const int v = z0 - 2 + (warp_id - 7) / 2, r = (warp_id - 7) & 1, j = e_pj0 + r;
+                    const float* rb = a.src + (size_t)wrapi(v, nz) * plane + (size_t)(e_py0 + r) * nx;
+                    float* d = slotP(v);
+                    bulk_g2s(d + j * C::TX, rb + x0, C::TX * 4u, bar);
+                    bulk_g2s(d + C::P_HL + hs + j * 4, rb + xL, 16u, bar);
+                    bulk_g2s(d + C::P_HR + hs + j * 4, rb + xR, 16u, bar);
+                } else if (warp_id == 11) {
+                    bulk_g2s(slotLz(z0 - 1) + e_cj * C::TX, Lz + (size_t)gb * plane + (size_t)e_cy * nx + x0, C::TX * 4u, bar);
                 }
             } else {
                 for (int pl = 0; pl < 2; ++pl) copy_p_rows(z0 - 2 + pl, bar);
@@ -313,7 +391,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
         const bool zy_lo = g.bc[1] && gy == 0, zy_hi = g.bc[1] && gyp == 0;
         const bool last_lane = (lx == C::LPR - 1);
         const int p_off = (ry + 1) * C::TX + 4 * lx;        // own float4 in a p plane
-        const int h_off = (lx == 0 ? C::P_HL + 3 : C::P_HR) + (ry + 1) * 4;  // x-halo cell (first / last lane)
+        const int h_off = (lx == 0 ? C::P_HL + 3 : C::P_HR) + hs + (ry + 1) * 4;  // x-halo cell (first / last lane)
         const int c_off = ry * C::TX + 4 * lx;              // own float4 in a coefficient plane
         float* dst_ptr = a.dst + ((long long)gy * nx + gx + (long long)(z0 - 2) * plane);  // plane u-1
         const float* const lxh_row = Lx + (size_t)gy * nx + gxh;  // face above the tile's last cell
@@ -440,7 +518,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
         const int gxs = wrapi(xs, nx), gxs1 = wrapi(xs + 1, nx);
         const int egy = wrapi(eyl, ny), egyp = wrapi(eyl + 1, ny);
         const int r = ery + 1;
-        const int pc_off = side ? C::P_HR + r * 4 : C::P_HL + r * 4 + 3;   // the edge cell
+        const int pc_off = hs + (side ? C::P_HR + r * 4 : C::P_HL + r * 4 + 3);   // the edge cell
         const int xm_off = side ? r * C::TX + C::TX - 1 : pc_off - 1;      // its x neighbours
         const int xp_off = side ? pc_off + 1 : r * C::TX;
         const int o_c = egy * nx + gxs, o_x1 = egy * nx + gxs1, o_yp = egyp * nx + gxs;
@@ -529,14 +607,27 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& ma
     }
 }
 
-template <class C, int NORM = 0>
+// EDGE: the kernel also carries the YMODE 2 body and sends every tile of a Neumann y axis through
+// the full boxes.  It pays on grids with few tile rows (a 1024 x 384 x 384 channel: -5 % per solve);
+// on a 1024^3 cube the third body costs the interior loop its register allocation (+2.6 % per
+// sweep, measured A/B on one box), so the launcher picks the kernel by the number of tile rows.
+template <class C, int NORM = 0, bool EDGE = false>
 __global__ void __launch_bounds__(C::THREADS, 1)
 k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     if (a.run_flag && *a.run_flag == 0) return;   // a re-run that turned out not to be needed
     const int ty = (blockIdx.x / a.tiles_x) % a.tiles_y;
     const int y0 = ty * C::TY;
-    if ((y0 >= 2) && (y0 + C::TY + 2 <= a.g.n[1])) sweep_body<C, true, NORM>(a, maps);
-    else sweep_body<C, false, NORM>(a, maps);
+    const int ny = a.g.n[1];
+    const bool inside = (y0 >= 2) && (y0 + C::TY + 2 <= ny);
+    if (EDGE) {
+        if (a.g.bc[1] != 0 || inside) sweep_body<C, 0, NORM>(a, maps);
+        else if (a.tiles_y >= 2 && ((ty == 0 && C::TY + 2 <= ny) || (ty == a.tiles_y - 1 && y0 >= 2)))
+            sweep_body<C, 2, NORM>(a, maps);
+        else sweep_body<C, 1, NORM>(a, maps);
+    } else {
+        if (inside) sweep_body<C, 0, NORM>(a, maps);
+        else sweep_body<C, 1, NORM>(a, maps);
+    }
 }
 
 // ---- launchers ------------------------------------------------------------------------------
@@ -638,12 +729,23 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
     BulkMaps maps;
     const size_t N = (size_t)g.N;
     bool ok = tma_shape_ok(g);
-    ok = ok && tensor_map(src, g, Bulk::TX, Bulk::SH, &maps.p_main);
-    ok = ok && tensor_map(src, g, 4, Bulk::SH, &maps.p_halo);
-    ok = ok && tensor_map(L + 2 * N, g, Bulk::TX, Bulk::ROWS, &maps.lz);
-    ok = ok && tensor_map(L, g, Bulk::TX, Bulk::ROWS, &maps.lx);
-    ok = ok && tensor_map(L + N, g, Bulk::TX, Bulk::ROWS + 1, &maps.ly);
-    ok = ok && tensor_map(b, g, Bulk::TX, Bulk::ROWS, &maps.b);
+    auto set = [&](MapSet& m, int hp, int hc, int hly) {
+        return tensor_map(src, g, Bulk::TX, hp, &m.p_main) && tensor_map(src, g, 4, hp, &m.p_halo) &&
+               tensor_map(L + 2 * N, g, Bulk::TX, hc, &m.lz) && tensor_map(L, g, Bulk::TX, hc, &m.lx) &&
+               tensor_map(L + N, g, Bulk::TX, hly, &m.ly) && tensor_map(b, g, Bulk::TX, hc, &m.b);
+    };
+    ok = ok && set(maps.m[0], Bulk::SH, Bulk::ROWS, Bulk::ROWS + 1);
+    const int tiles_y_ = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
+    const int rem = g.n[1] - (tiles_y_ - 1) * Bulk::TY;      // rows of the final tile row
+    // few tile rows, or walls in y: the kernel with the boundary-box body (see k_rb_sweep_bulk)
+    const bool edge = g.bc[1] != 0 || (tiles_y_ >= 2 && tiles_y_ <= 40);
+    if (ok && edge && g.bc[1] == 0 && tiles_y_ >= 2) {
+        ok = ok && set(maps.m[1], Bulk::SH - 2, Bulk::ROWS - 1, Bulk::ROWS);   // FIRST: from y = 0
+        ok = ok && set(maps.m[2], rem + 2, rem + 1, rem + 1);                  // FINAL: up to y = ny - 1
+    } else {
+        maps.m[1] = maps.m[0];
+        maps.m[2] = maps.m[0];
+    }
     if (!ok) return false;
     BulkArgs a;
     a.g = g; a.L = L; a.src = src; a.dst = dst; a.b = b; a.omega = omega;
@@ -657,20 +759,33 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
     const unsigned int grid = bulk_grid(g, &zchunk);
     a.zchunk = zchunk;
     if (grid > GMG_REDUCE_MAX_BLOCKS && norm) return false;
-    if (norm && slot_ref >= 0) k_rb_sweep_bulk<Bulk, 2><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
-    else if (norm) k_rb_sweep_bulk<Bulk, 1><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
-    else k_rb_sweep_bulk<Bulk, 0><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+    const int nv = (norm && slot_ref >= 0) ? 2 : (norm ? 1 : 0);
+    if (edge) {
+        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, true><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, true><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+        else k_rb_sweep_bulk<Bulk, 0, true><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+    } else {
+        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, false><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, false><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+        else k_rb_sweep_bulk<Bulk, 0, false><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+    }
     return true;
 }
 
 int configure() {
     cudaError_t e = (cudaError_t)configure_v2();
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
     if (e == cudaSuccess && !g_encode) {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult qres;
