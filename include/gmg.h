@@ -86,8 +86,9 @@ typedef struct {
     int fused_norm;    /* 1: on a finest level that runs the TMA-fed sweep, the stopping-test norm
                           ||z - A p_k|| is accumulated by the first pre-smoothing sweep of cycle k+1
                           (out of place, so p_k survives when the test ends the solve) instead of
-                          by a 20 B/cell pass of its own after every cycle; same iterates, same
-                          test, one sweep wasted at the end of a solve (1) */
+                          by a 20 B/cell pass of its own after every cycle; the cycle expected to be
+                          the last (rate-based prediction, or the maxiter-th) takes the plain pass
+                          instead, so that no sweep is wasted at the exit; same iterates, same test (1) */
 } gmg_params_t;
 
 /* Statistics of the last gmg_solve. */
