@@ -78,7 +78,7 @@ typedef struct {
     int fast_path;     /* 1: fused/tiled kernels where shapes allow; 0: generic kernels only */
     int use_graph;     /* 1: V-cycle captured in a CUDA graph; 0: plain launches */
     int tma_min_cells; /* levels with at least this many cells (and nx % 128 == 0) use the TMA-fed
-                          z-marching kernels; smaller ones the register-fed tiles (4194304);
+                          z-marching kernels; smaller ones the register-fed tiles (1048576);
                           0 = whenever the shape allows, -1 = never */
     int cluster_tail;  /* 1: the coarse levels that fit the shared memory of a cluster of 8 CTAs
                           (each at most 32768 cells) run as ONE thread-block-cluster kernel;

@@ -106,6 +106,11 @@ struct gmg_ctx {
         }                                                                                \
     } while (0)
 
+// The TMA-fed CG mat-vec pays from 4 Mi cells on; below that the float4 kernel is faster (128^3
+// Jacobi-PCG: 5.2 vs 5.7 ms per solve), whatever tma_min_cells says for the sweeps -- unless it is
+// 0 ("whenever the shape allows": the tests force the TMA path on small grids that way).
+static const long long kBulkMatvecMinCells = 4LL << 20;
+
 static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 static inline ReduceBuf rbuf(gmg_ctx* c) { return ReduceBuf{c->partials, c->counter, c->sc}; }
 
@@ -219,7 +224,7 @@ extern "C" void gmg_default_params(gmg_params_t* p) {
     p->nu_pre = 2; p->nu_post = 2; p->nu_coarse = 32;
     p->omega0 = 1.0f; p->omega_min = 0.5f; p->omega_down = 0.125f; p->omega_up = 0.03125f;
     p->adaptive = 1; p->coarsen_mode = GMG_COARSEN_ANISO; p->n_min = 4;
-    p->fast_path = 1; p->use_graph = 1; p->tma_min_cells = 4 << 20; p->cluster_tail = 1;
+    p->fast_path = 1; p->use_graph = 1; p->tma_min_cells = 1 << 20; p->cluster_tail = 1;
     p->fused_norm = 1;
 }
 
@@ -521,7 +526,8 @@ static void cg_smooth(gmg_ctx* c, int l, float* x, const float* b, int m, cudaSt
     gmgk::ctl_cgs_begin(c->sc, g, s);
     c->n_launch += 3;
     for (int it = 0; it < m; ++it) {
-        if (!(c->prm.fast_path && c->tma_ok[l] && gmgf::matvec_dot_bulk(g, L, d, q, rbuf(c), RED_DQ, s)))
+        if (!(c->prm.fast_path && c->tma_ok[l] && (c->prm.tma_min_cells == 0 || g.N >= kBulkMatvecMinCells) &&
+              gmgf::matvec_dot_bulk(g, L, d, q, rbuf(c), RED_DQ, s)))
             gmgk::matvec_dot(g, L, d, q, rbuf(c), RED_DQ, s);
         gmgk::ctl_cgs_alpha(c->sc, s);
         gmgk::pcg_update_pr(g, L, x, r, d, q, nullptr, 0, rbuf(c), s);
@@ -694,7 +700,7 @@ static void pcg_body(gmg_ctx* c, float* p, int gmg_precond, LoopCtl lc, cudaStre
     }
     gmgk::ctl_pcg_beta(c->sc, s);
     gmgk::pcg_update_d(N, c->pcg_d, c->pcg_s, c->sc, 0, s);
-    if (!(c->prm.fast_path && c->tma_ok[0] &&
+    if (!(c->prm.fast_path && c->tma_ok[0] && (c->prm.tma_min_cells == 0 || c->g[0].N >= kBulkMatvecMinCells) &&
           gmgf::matvec_dot_bulk(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rbuf(c), RED_DQ, s)))
         gmgk::matvec_dot(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rbuf(c), RED_DQ, s);
     gmgk::ctl_pcg_alpha(c->sc, s);
