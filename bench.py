@@ -449,7 +449,7 @@ def main():
     ap.add_argument("--workload", default="c4")
     ap.add_argument("--reference-sample", default="c4_256")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-table", action="store_true", help="skip the three-solver comparison table")
+    ap.add_argument("--no-table", action="store_true", help="skip the solver comparison and pressure-step tables")
     ap.add_argument("--no-graph", action="store_true",
                     help="plain kernel launches instead of the CUDA-graph WHILE loop (so that ncu "
                          "lists every kernel of the solve)")
