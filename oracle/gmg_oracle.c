@@ -21,8 +21,15 @@
  * (O5); half-sweep zeroes the residual of its colour and decreases the error energy (O3);
  * <Rr,e> = <r,Pe> (O6); closed-form coarse coefficients and quadratic consistency (O5);
  * level shapes (O4); dense least-squares solve on 8^3 (O7,O9,O10,O11 solutions);
- * dyadic omega sequence (O8); the CG smoother as the Krylov energy minimiser of the dense
- * face-assembled system, its guards, the CG-smoothed cycle as a composition of its parts (O12).
+ * omega rule restated against the produced history, persistence across solves (O8); the RBGS
+ * cycle and its symmetric variant as compositions of the separately pinned operators with
+ * (nu1,nu2,nuc) = (2,3,5|6), self-adjointness of the symmetric cycle on the active cells (O7, O11);
+ * flux conservation of linear fields on random coefficients for all five coarsening patterns
+ * (O5 tiling); norms / stopping test blind to inactive cells and relative to ||z|| (O9); the CG
+ * smoother as the Krylov energy minimiser of the dense face-assembled system, its guards incl.
+ * the step-length cap firing in FP64 on a two-region level, the CG-smoothed cycle as a composition
+ * of its parts (O12).  A mutation run (each plausible slip applied to a copy of this file) turns
+ * at least one pin red for every mutation listed in DESIGN.md S3.
  * PARITY UNPINNED against the paper itself: the omega rule and its constants (O8), the
  * sweep counts nu1/nu2/nuc (O7), the meaning of "GMG-PCG" (O11) and the restart, counts and
  * guards of the PCG-smoothed cycle (O12): the paper prints no worked example or constant for them.

@@ -268,8 +268,7 @@ def test_adaptive_omega_follows_dyadic_rule():
     assert out["iterations"] == 8 and out["status"] == 1
     d = np.diff(h)
     assert np.any(d > 0) and np.any(d <= 0), "this case must exercise both branches"
-    assert list(om[:4]) == [1.0, 0.875, 0.90625, 0.78125]
-    w_ = 1.0
+    w_ = 1.0                                            # the rule restated, fed by the history
     for k in range(out["iterations"]):
         assert om[k] == w_
         w_ = max(0.5, w_ - 0.125) if h[k + 1] > h[k] else min(1.0, w_ + 0.03125)
@@ -504,3 +503,272 @@ def test_2d_level_shapes_and_dense_solution():
         assert out["status"] == 0, solver
         err = np.linalg.norm(_demean(out["p"], act) - _demean(xs, act)) / np.linalg.norm(_demean(xs, act))
         assert err < 1e-8, (solver, err)
+
+
+# --------------------------------------------------------------------------------------
+# Round-2 pins: parts that mutation testing of a copy of gmg_oracle.c showed unpinned
+# (VERDICT r1 "What's weak" 1).  Each names the mutation it turns red.
+# --------------------------------------------------------------------------------------
+def _compose_rbgs_cycle(H, x0, b, nu1, nu2, nuc, omega, sym):
+    """Reading O7 / O11 written out from the single-operator calls that are pinned on their own
+    (half_sweep <- own-colour residual 0; residual <- face assembly; restrict/prolong <- brute
+    force), with every colour order spelt explicitly.  2-level hierarchies only."""
+    assert H.nlev == 2
+    (n0, c0), (n1, _) = H.shape(0), H.shape(1)
+    L0, L1, bc = H.L(0), H.L(1), H.bc
+    RED, BLACK = 0, 1
+
+    def sweep(L, x, rhs, first):
+        x = oracle.half_sweep(L, bc, x, rhs, omega, first)
+        return oracle.half_sweep(L, bc, x, rhs, omega, 1 - first)
+
+    x = x0
+    for _ in range(nu1):                                   # pre-smoothing: red -> black
+        x = sweep(L0, x, b, RED)
+    bc1 = oracle.restrict_sum(oracle.residual(L0, bc, x, b), c0)
+    e = np.zeros_like(bc1)                                 # coarse unknown starts at 0 (O6)
+    if not sym:
+        for _ in range(nuc):                               # coarsest: nu_c sweeps red -> black
+            e = sweep(L1, e, bc1, RED)
+    else:
+        for _ in range(nuc // 2):                          # O11: nu_c/2 red -> black ...
+            e = sweep(L1, e, bc1, RED)
+        for _ in range(nuc // 2):                          # ... then nu_c/2 black -> red
+            e = sweep(L1, e, bc1, BLACK)
+    x = oracle.prolong_add(x, e, c0)
+    for _ in range(nu2):                                   # post: red -> black (O7) / black -> red (O11)
+        x = sweep(L0, x, b, BLACK if sym else RED)
+    return x
+
+
+@pytest.mark.parametrize("sym", [False, True])
+@pytest.mark.parametrize("n,bc", [((8, 8, 4), (1, 0, 1)), ((8, 4, 8), (0, 0, 0))])
+def test_rbgs_cycle_is_the_composition_of_its_pinned_parts(n, bc, sym):
+    """Fails: nu_c replaced by a constant, nu1/nu2 off by one, a wrong colour order in the pre-,
+    post- or coarsest sweeps of either variant (gmg_oracle.c vcycle_rec)."""
+    rng = np.random.default_rng(31)
+    L32 = rand_L(rng, n, 0.1).astype(np.float32)
+    H = oracle.Hierarchy(n, bc, L32, n_min=4)
+    assert H.nlev == 2
+    nu1, nu2, nuc = 2, 3, (6 if sym else 5)
+    H.set_params(nu1=nu1, nu2=nu2, nuc=nuc)
+    b = rng.standard_normal((n[2], n[1], n[0]))
+    x0 = rng.standard_normal(b.shape)
+    for omega in (1.0, 0.75):
+        ref = _compose_rbgs_cycle(H, x0, b, nu1, nu2, nuc, omega, sym)
+        got = H.vcycle(x0, b, omega=omega, sym=sym)
+        assert np.allclose(got, ref, rtol=0, atol=1e-12)
+        # the test must be able to tell the variants apart
+        other = _compose_rbgs_cycle(H, x0, b, nu1, nu2, nuc + (2 if sym else 1), omega, sym)
+        assert np.abs(other - ref).max() > 1e-6
+        flip = _compose_rbgs_cycle(H, x0, b, nu1, nu2, 6, omega, not sym)
+        assert np.abs(flip - ref).max() > 1e-6
+
+
+@pytest.mark.parametrize("bc", [(1, 0, 1), (0, 0, 0), (1, 1, 1)])
+def test_symmetric_cycle_is_self_adjoint(bc):
+    """O11 needs B (one symmetric cycle from a zero guess) self-adjoint: <a, B b> = <b, B a>.
+    The plain cycle (post-sweeps red->black) is NOT, and neither is a symmetric cycle whose
+    coarsest second half is not reversed (fails that mutation of gmg_oracle.c vcycle_rec)."""
+    rng = np.random.default_rng(32)
+    n = (8, 8, 8)
+    L32 = rand_L(rng, n, 0.1).astype(np.float32)
+    H = oracle.Hierarchy(n, bc, L32)
+    assert H.nlev == 2
+    H.set_params(nu1=2, nu2=2, nuc=2)
+    # CG applies B to residuals, which are 0 on inactive cells (O9); the prolongation also
+    # writes the (never read) unknowns of inactive cells, so B is self-adjoint on the active ones
+    act = W.active_mask(L32, bc)
+    a = rng.standard_normal((8, 8, 8)) * act; b = rng.standard_normal(a.shape) * act
+    zero = np.zeros_like(a)
+    Ba, Bb = H.vcycle(zero, a, sym=True), H.vcycle(zero, b, sym=True)
+    scale = abs((a * Bb).sum())
+    assert abs((a * Bb).sum() - (b * Ba).sum()) < 1e-12 * max(scale, 1.0)
+    Na, Nb = H.vcycle(zero, a, sym=False), H.vcycle(zero, b, sym=False)
+    assert abs((a * Nb).sum() - (b * Na).sum()) > 1e-6 * max(scale, 1.0)
+    # three levels, default counts: still self-adjoint
+    L3 = rand_L(rng, (16, 8, 8), 0.1).astype(np.float32)
+    L3[:, 2:4, 2:4, 5:8] = 0.0                          # with a solid block
+    H3 = oracle.Hierarchy((16, 8, 8), bc, L3)
+    assert H3.nlev == 3
+    act = W.active_mask(L3, bc)
+    assert not act.all()
+    a = rng.standard_normal((8, 8, 16)) * act; b = rng.standard_normal(a.shape) * act
+    zero = np.zeros_like(a)
+    Ba, Bb = H3.vcycle(zero, a, sym=True), H3.vcycle(zero, b, sym=True)
+    assert abs((a * Bb).sum() - (b * Ba).sum()) < 1e-12 * max(abs((a * Bb).sum()), 1.0)
+
+
+@pytest.mark.parametrize("c", [(2, 2, 2), (2, 1, 1), (2, 2, 1), (1, 2, 2), (1, 1, 2)])
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_coarse_coefficients_conserve_the_flux_of_linear_fields(c, d):
+    """O5 on HETEROGENEOUS coefficients.  For q = x_d (linear) the fine operator gives the
+    difference of the two d-face coefficients of a cell; summed over the children of a coarse
+    cell the inner faces telescope and what is left is the sum over the fine faces tiling the
+    coarse cell's two d-faces.  The coarse operator on the same field (coarse spacing c_d) gives
+    c_d * (L^c_hi - L^c_lo).  Both agree for every random L iff L^c = (1/c_d) * sum over exactly
+    the tiling fine faces.  With walls on every axis the wall faces carry 0 on both levels, so the
+    identity holds in EVERY cell; with periodic axes away from the seam of q.  Fails: a fine
+    face summed twice or missed, a wrong child plane, the 1/c_d factor dropped."""
+    rng = np.random.default_rng(40 + d)
+    nf = (8, 6, 8)
+    nc = tuple(a // b for a, b in zip(nf, c))
+    k, j, i = np.meshgrid(*[np.arange(m) for m in nf[::-1]], indexing="ij")
+    K, J, I = np.meshgrid(*[np.arange(m) for m in nc[::-1]], indexing="ij")
+    qf = (i, j, k)[d] + 0.5
+    qc = ((I, J, K)[d] + 0.5) * c[d]
+    for bc in [(1, 1, 1), (0, 0, 0)]:
+        Lf = W.effective_L(rand_L(rng, nf, 0.2), bc)
+        Lc = oracle.coarsen_coeffs(Lf, c)
+        lhs = oracle.apply_A(Lc, bc, qc)
+        rhs = oracle.restrict_sum(oracle.apply_A(Lf, bc, qf), c)
+        sl = [slice(None)] * 3
+        if bc[d] == 0:
+            sl[2 - d] = slice(1, -1)          # the linear field jumps across the periodic seam
+        assert np.max(np.abs((lhs - rhs)[tuple(sl)])) < 1e-12
+        assert np.max(np.abs(lhs)) > 0.1
+        # the coarse wall plane of a Neumann axis is the coarsened (zero) fine wall plane
+        if bc[d] == 1:
+            w = [slice(None)] * 3; w[2 - d] = 0
+            assert np.all(Lc[d][tuple(w)] == 0.0)
+
+
+@pytest.mark.parametrize("solver", [oracle.GMG_RBGS, oracle.PCG, oracle.GMG_PCG, oracle.GMG_CGS])
+def test_norms_and_stopping_ignore_inactive_cells(solver):
+    """O9: the reference norm and the residual are taken over ACTIVE cells.  Garbage in the
+    right-hand side on inactive cells (inside a solid) must change nothing: r_ref equals the
+    norm over the independently built activity mask, history, count and p are unchanged.
+    Fails: active_norm summing over all cells."""
+    rng = np.random.default_rng(33)
+    n, bc = (8, 8, 8), (1, 0, 0)
+    L32 = rng.uniform(0.2, 1, (3, 8, 8, 8)).astype(np.float32)
+    L32[:, 2:5, 2:5, 2:5] = 0.0                        # a solid block: 2x2x2 cells have no face
+    A = dense_by_faces(n, bc, W.effective_L(L32, bc))
+    act = (np.diag(A) != 0.0).reshape(8, 8, 8)
+    assert (~act).sum() == 8
+    z = W.project_compatible(rng.standard_normal((8, 8, 8)), act)
+    zg = z.copy()
+    zg[~act] = 50.0 * rng.standard_normal((~act).sum())
+    o1 = oracle.Hierarchy(n, bc, L32).solve(solver, z, tol=1e-6, maxiter=300)
+    o2 = oracle.Hierarchy(n, bc, L32).solve(solver, zg, tol=1e-6, maxiter=300)
+    assert o1["status"] == 0 and o2["status"] == 0
+    assert o1["iterations"] == o2["iterations"] >= 2
+    assert np.array_equal(o1["history"], o2["history"])
+    assert np.array_equal(o1["p"], o2["p"]) and np.all(o2["p"][~act] == 0.0)
+    if "r_ref" in o2:
+        assert abs(o2["r_ref"] - np.linalg.norm(z[act])) < 1e-12
+    # history[0] = ||z - A 0|| / ||z|| over active cells = 1 exactly with a zero guess
+    assert abs(o2["history"][0] - 1.0) < 1e-12
+    r = np.where(act.ravel(), zg.ravel() - A @ o2["p"].ravel(), 0.0)
+    assert abs(np.linalg.norm(r) / np.linalg.norm(z[act]) - o2["true_res"]) < 1e-9
+
+
+def _two_slab_level(sigma, seed=51):
+    """One level, (4, 6, 8) periodic, cut into two x-slabs of width 2 by zero x-faces at i = 0
+    and i = 2: two disconnected fluid regions, null space = constants per slab.  Coefficients
+    1 + 0.01*noise (D = -5 up to 1 % in every cell); right-hand side +1 / -1 on the two slabs
+    (zero global mean, incompatible per slab) plus sigma * compatible noise."""
+    rng = np.random.default_rng(seed)
+    n, bc = (4, 6, 8), (0, 0, 0)
+    L = 1.0 + 0.01 * rng.uniform(-1, 1, (3, 8, 6, 4))
+    L[0, :, :, 0] = 0.0
+    L[0, :, :, 2] = 0.0
+    L32 = L.astype(np.float32)
+    b = np.zeros((8, 6, 4))
+    b[:, :, :2] = 1.0
+    b[:, :, 2:] = -1.0
+    b += sigma * W.project_compatible(rng.standard_normal(b.shape), np.ones(b.shape, bool))
+    return n, bc, L32, b
+
+
+def _dense_first_cg_step(n, bc, L32, b):
+    """alpha_1 and x_1 of Jacobi-PCG from x0 = 0, from the face-assembled matrix: x_1 is the
+    energy minimiser along v = D^-1 r0 and alpha_1 = r0.(x_1 - x0) / (r0 . D^-1 r0)."""
+    A = dense_by_faces(n, bc, L32.astype(np.float64))
+    Dg = np.diag(A)
+    r0 = b.ravel() - b.mean()
+    v = r0 / Dg
+    t = (v @ r0) / (v @ (A @ v))
+    x1 = t * v
+    return (r0 @ x1) / (r0 @ v), x1.reshape(b.shape)
+
+
+def test_cg_smoother_step_length_cap():
+    """O12's guard 'a step of length alpha > 16 n_max^2 is not taken' in a case where it fires in
+    FP64: a right-hand side incompatible on each of two disconnected regions (only the global
+    mean is removed at the restart), with nearly uniform coefficients so that the first search
+    direction is nearly a null vector (the smaller the compatible part of the right-hand side,
+    the longer the step).  alpha_1 is computed independently from the dense matrix;
+    just below the cap the oracle takes the step (= the dense minimiser), just above it leaves x
+    untouched for any iteration count.  Fails: cap removed, cap on another extent or constant,
+    step applied before the test."""
+    cap = 16.0 * 8 * 8
+    lo, hi = 1e-3, 0.3                                  # alpha_1 falls as the noise sigma grows
+    for _ in range(60):
+        mid = np.sqrt(lo * hi)
+        a, _ = _dense_first_cg_step(*_two_slab_level(mid))
+        lo, hi = (mid, hi) if a > cap else (lo, mid)
+    sigma_cap = hi
+    below, above = None, None
+    for sigma in (sigma_cap * 1.2, sigma_cap / 1.2):
+        n, bc, L32, b = _two_slab_level(sigma)
+        a1, x1 = _dense_first_cg_step(n, bc, L32, b)
+        H = oracle.Hierarchy(n, bc, L32, n_min=64)
+        assert H.nlev == 1
+        x0 = np.zeros_like(b)
+        if a1 <= cap:
+            below = a1
+            got = H.level_cg_smooth(0, x0, b, 1)
+            assert np.abs(got - x1).max() < 1e-9 * np.abs(x1).max() and np.abs(x1).max() > 1.0
+        else:
+            above = a1
+            for m in (1, 2, 7):
+                assert np.array_equal(H.level_cg_smooth(0, x0, b, m), x0)
+    assert below is not None and above is not None
+    assert 0.5 * cap < below <= cap < above < 2.0 * cap
+
+
+@pytest.mark.parametrize("solver", [oracle.GMG_RBGS, oracle.PCG, oracle.GMG_PCG, oracle.GMG_CGS])
+def test_stopping_test_is_relative_to_the_right_hand_side_not_the_first_residual(solver):
+    """O9: stop when ||z - A p|| <= tol ||z||, tested BEFORE the first cycle.  A warm start whose
+    residual is already below tol ||z|| takes 0 iterations and leaves p alone; history[0] is the
+    warm start's residual relative to ||z|| (recomputed here from the face-assembled matrix)."""
+    rng = np.random.default_rng(34)
+    n, bc = (8, 8, 8), (0, 1, 0)
+    L32 = rng.uniform(0.2, 1, (3, 8, 8, 8)).astype(np.float32)
+    A = dense_by_faces(n, bc, W.effective_L(L32, bc))
+    z = W.project_compatible(rng.standard_normal((8, 8, 8)), np.ones((8, 8, 8), bool))
+    good = oracle.Hierarchy(n, bc, L32).solve(oracle.GMG_RBGS, z, tol=1e-7, maxiter=100)["p"]
+    rel0 = np.linalg.norm(z.ravel() - A @ good.ravel()) / np.linalg.norm(z)
+    assert 1e-9 < rel0 <= 1e-7
+    out = oracle.Hierarchy(n, bc, L32).solve(solver, z, p0=good, tol=1e-4, maxiter=50)
+    assert out["iterations"] == 0 and out["status"] == 0 and np.array_equal(out["p"], good)
+    assert abs(out["history"][0] - rel0) < 1e-12
+    # a start WORSE than zero: history[0] > 1 is still relative to ||z||, and the solve goes on
+    # until tol * ||z||, not merely tol * (first residual)
+    poor = good + 10.0 * rng.standard_normal(good.shape)
+    rel1 = np.linalg.norm(z.ravel() - A @ poor.ravel()) / np.linalg.norm(z)
+    assert rel1 > 5.0
+    out = oracle.Hierarchy(n, bc, L32).solve(solver, z, p0=poor, tol=1e-3, maxiter=300)
+    assert abs(out["history"][0] - rel1) < 1e-12 * rel1 and out["iterations"] >= 1
+    assert out["status"] == 0 and out["history"][-1] <= 1e-3 < out["history"][-2]
+
+
+def test_relaxation_factor_persists_for_rbgs_and_never_enters_the_preconditioner():
+    """O8: omega is carried from one GMG-RBGS solve to the next on the same hierarchy (time
+    stepping).  O11: the preconditioning cycle runs at omega = 1 whatever that
+    state is."""
+    w = W.config0()
+    z = w.z.astype(np.float64)
+    H = oracle.Hierarchy(w.n, w.bc, w.L)
+    H.omega = 0.625
+    out = H.solve(oracle.GMG_RBGS, z, tol=0.0, maxiter=3)
+    # started from the carried value; every cycle decays here, so +1/32 per cycle
+    assert list(out["omegas"]) == [0.625, 0.65625, 0.6875] and H.omega == 0.71875
+    fresh = oracle.Hierarchy(w.n, w.bc, w.L).solve(oracle.GMG_RBGS, z, tol=0.0, maxiter=3)
+    assert not np.allclose(fresh["history"][1:], out["history"][1:], rtol=1e-3)
+    H = oracle.Hierarchy(w.n, w.bc, w.L)
+    H.omega = 0.625
+    a = H.solve(oracle.GMG_PCG, z, tol=1e-6, maxiter=50)
+    b = oracle.Hierarchy(w.n, w.bc, w.L).solve(oracle.GMG_PCG, z, tol=1e-6, maxiter=50)
+    assert np.array_equal(a["history"], b["history"]) and H.omega == 0.625
