@@ -24,6 +24,9 @@
  *    The big arrays of the level hierarchy live in the caller-provided workspace; the
  *    library itself allocates only < 4 MB of device scalars / reduction partials /
  *    history and its pinned host mirror.
+ *  - Alignment: every *_dev array handed to the library (p, z, L, u, the hooks' operands) must
+ *    start on a 16-byte boundary (the fast paths move float4s and TMA boxes); a misaligned
+ *    pointer is refused with GMG_EINVAL.  The workspace must be 256-byte aligned.
  *  - `stream` is a cudaStream_t passed as void* (0 = legacy default stream).  All work
  *    is enqueued on it; gmg_solve and the gmg_op_* hooks synchronise it before returning.
  *  - Return codes: 0 ok; >0 warning (result valid); <0 error (gmg_last_error has text).
@@ -204,15 +207,15 @@ int gmg_op_prolong(gmg_ctx* ctx, int lev, const float* e_coarse_dev, float* p_fi
  * = the variant used as CG preconditioner (reading O11). */
 int gmg_op_vcycle(gmg_ctx* ctx, float* p_dev, const float* z_dev, float omega, int symmetric,
                   void* stream);
-/* The smoother of GMG_GMG_CGS (reading O12, PAPER.md:43 "PCG can be used as a smoother"): iters
- * Jacobi-PCG iterations on A^lev x = b restarted from x (in place), and one whole cycle of it on
- * level 0 (V(nu_pre, nu_post), nu_coarse iterations on the coarsest level). */
 /* ONE fused red+black sweep src -> dst (out of place) of the TMA-fed kernel that also returns
  * sum r^2, r = b - A src on active cells, and sum b^2 over active cells (the fused_norm path of
  * gmg_solve).  GMG_EINVAL when level lev cannot run that kernel (nx % 128, small levels). */
 int gmg_op_sweep_with_norm(gmg_ctx* ctx, int lev, const float* src_dev, float* dst_dev, const float* b_dev,
                            float omega, int first_colour, double* rr_out_host, double* bb_out_host,
                            void* stream);
+/* The smoother of GMG_GMG_CGS (reading O12, PAPER.md:43 "PCG can be used as a smoother"): iters
+ * Jacobi-PCG iterations on A^lev x = b restarted from x (in place), and one whole cycle of it on
+ * level 0 (V(nu_pre, nu_post), nu_coarse iterations on the coarsest level). */
 int gmg_op_cg_smooth(gmg_ctx* ctx, int lev, float* x_dev, const float* b_dev, int iters, void* stream);
 int gmg_op_vcycle_cgs(gmg_ctx* ctx, float* p_dev, const float* z_dev, void* stream);
 /* sqrt(sum r^2) of a level-lev array (deterministic two-stage reduction). */

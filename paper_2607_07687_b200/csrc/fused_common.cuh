@@ -11,6 +11,8 @@ using namespace gmgd;
 // cost little and many CTAs smooth the tail of the grid).  Small, L2-resident levels are
 // latency-bound: the kernel takes (waves of CTAs) x (planes per CTA + fixed start-up steps), so
 // the chunk count is chosen to minimise that -- in particular never a few CTAs over a wave.
+static constexpr int kZChunkPref = 64;  // planes per CTA on big levels
+static constexpr int kZChunkMin = 4;    // never fewer planes per CTA than this
 static inline int choose_zchunk(long long tiles, int nz, int zpref, int zmin, int slots, int even) {
     if (nz <= zmin) return nz;
     if (tiles * ((nz + zpref - 1) / zpref) >= 4LL * slots) return zpref;

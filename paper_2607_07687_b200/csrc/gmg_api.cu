@@ -29,6 +29,7 @@ void prolong_add4(const LevelGeom& g, const float* e_c, float* p_f, cudaStream_t
 bool matvec_dot_bulk(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot,
                      cudaStream_t s);
 bool tma_shape_ok(const LevelGeom& g);
+bool bulk_sweep_edge(const LevelGeom& g, bool norm);
 // one TMA-fed sweep src -> dst that also leaves sum r^2 (r = b - A src) and sum b^2 over the active
 // cells in red[slot_rr] / red[slot_ref]; false = the level cannot run it (nothing launched)
 bool rb_sweep_with_norm(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
@@ -92,6 +93,8 @@ struct gmg_ctx {
     cudaStream_t cap_a, cap_b;  // internal streams used only for graph capture
     GraphSlot slots[4];
     long long n_launch;   // launch counter of the section being enqueued
+    bool enqueue_fail;    // a launcher the plan counted on refused (tensor-map encode failed)
+    bool sc_fresh;        // sc_host holds the status block of the call in progress
     char err[512];
 };
 
@@ -112,6 +115,9 @@ struct gmg_ctx {
 static const long long kBulkMatvecMinCells = 4LL << 20;
 
 static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+// The float4 / TMA paths read caller arrays 16 bytes at a time (gmg.h "Alignment").
+static inline bool al16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
+#define MUST_LAUNCH(c, call) do { if (!(call)) (c)->enqueue_fail = true; } while (0)
 static inline ReduceBuf rbuf(gmg_ctx* c) { return ReduceBuf{c->partials, c->counter, c->sc}; }
 
 // ---- level table: reading O4 ("downsamples every dimension independently") ------
@@ -251,6 +257,7 @@ extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]
     c->ev0 = c->ev1 = nullptr;
     c->cap_a = c->cap_b = nullptr;
     c->cluster_ok = false;
+    c->enqueue_fail = false; c->sc_fresh = false;
     if (gmgk::ctail_configure(200 * 1024) == (int)cudaSuccess) c->cluster_ok = gmgk::ctail_launchable(200 * 1024);
     cudaGetLastError();
     build_levels(c);
@@ -399,6 +406,7 @@ static void set_coeffs_enqueue(gmg_ctx* c, const float* L_dev, cudaStream_t s) {
 
 extern "C" int gmg_set_coeffs(gmg_ctx* c, const float* L_dev, void* stream) {
     if (!c || !L_dev) return GMG_EINVAL;
+    if (!al16(L_dev)) { SET_ERR(c, "gmg_set_coeffs: L_dev must be 16-byte aligned"); return GMG_EINVAL; }
     if (!c->ws_set) { SET_ERR(c, "gmg_set_coeffs before gmg_set_workspace"); return GMG_ESTATE; }
     cudaStream_t s = (cudaStream_t)stream;
     set_coeffs_enqueue(c, L_dev, s);
@@ -416,7 +424,7 @@ extern "C" int gmg_set_coeffs(gmg_ctx* c, const float* L_dev, void* stream) {
 }
 
 extern "C" int gmg_level_coeffs(gmg_ctx* c, int lev, float* L_out_dev, void* stream) {
-    if (!c || lev < 0 || lev >= c->nlev || !L_out_dev) return GMG_EINVAL;
+    if (!c || lev < 0 || lev >= c->nlev || !L_out_dev || !al16(L_out_dev)) return GMG_EINVAL;
     if (!c->coeffs_set) { SET_ERR(c, "coefficients not set"); return GMG_ESTATE; }
     cudaStream_t s = (cudaStream_t)stream;
     CUDA_TRY(c, cudaMemcpyAsync(L_out_dev, c->lv[lev].L, 3 * (size_t)c->g[lev].N * sizeof(float),
@@ -629,8 +637,8 @@ static bool predict_active(const gmg_ctx* c) {
 }
 static void first_sweep_with_norm(gmg_ctx* c, float* p, const float* z, const float* omega, bool with_ref,
                                   const int* run_flag, cudaStream_t s) {
-    gmgf::rb_sweep_with_norm(c->g[0], c->lv[0].L, p, c->lv[0].q, z, omega, 0, rbuf(c), RED_RR,
-                             with_ref ? RED_RREF : -1, run_flag, s);
+    MUST_LAUNCH(c, gmgf::rb_sweep_with_norm(c->g[0], c->lv[0].L, p, c->lv[0].q, z, omega, 0, rbuf(c), RED_RR,
+                                            with_ref ? RED_RREF : -1, run_flag, s));
 }
 
 static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s, bool cgs = false) {
@@ -656,18 +664,18 @@ static void rbgs_body(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStre
     if (!cgs && fused_norm_active(c)) {
         const bool pred = predict_active(c);
         if (pred) {   // after a failed "last cycle" prediction the first sweep is still to run
-            gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->need_first, s);
+            MUST_LAUNCH(c, gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->need_first, s));
             c->n_launch += 1;
         }
         enqueue_vcycle(c, p, z, &c->sc->omega_f, 0, s, 1);             // its first sweep already ran
         if (pred) {   // expected to be the last cycle: the plain norm pass
-            gmgf::residual_norm2_bulk_if(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, &c->sc->expect_last, s);
+            MUST_LAUNCH(c, gmgf::residual_norm2_bulk_if(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, &c->sc->expect_last, s));
             c->n_launch += 1;
         }
         // otherwise: next cycle's first sweep, + ||z - A p_k||
         first_sweep_with_norm(c, p, z, &c->sc->omega_spec_f, false, pred ? &c->sc->run_s1n : nullptr, s);
         gmgk::ctl_rbgs_cycle_end(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
-        gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->redo_first, s);
+        MUST_LAUNCH(c, gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->redo_first, s));
         c->n_launch += 3;
         return;
     }
@@ -781,6 +789,10 @@ static int build_graph(gmg_ctx* c, GraphSlot& slot, int solver, float* p, const 
     cudaGraph_t gout = nullptr;
     CUDA_TRY(c, cudaStreamEndCapture(c->cap_a, &gout));
     CUDA_TRY(c, cudaGetLastError());
+    if (c->enqueue_fail) {
+        SET_ERR(c, "gmg_solve: a TMA-fed kernel of the plan could not be launched (tensor-map encode failed)");
+        return GMG_ECUDA;
+    }
     CUDA_TRY(c, cudaGraphInstantiate(&slot.exec, graph, 0));
     slot.p = p; slot.z = z; slot.solver = solver; slot.tol = tol; slot.maxiter = maxiter;
     slot.hist = c->hist;
@@ -820,11 +832,17 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
         SET_ERR(c, "gmg_solve: invalid argument");
         return GMG_EINVAL;
     }
+    if (!al16(p) || !al16(z)) {
+        SET_ERR(c, "gmg_solve: p_dev and z_dev must be 16-byte aligned");
+        return GMG_EINVAL;
+    }
     if (!c->ws_set || !c->coeffs_set) {
         SET_ERR(c, "gmg_solve before gmg_set_workspace / gmg_set_coeffs");
         return GMG_ESTATE;
     }
     cudaStream_t s = (cudaStream_t)stream;
+    c->sc_fresh = false;
+    c->enqueue_fail = false;
     int rc = ensure_history(c, maxiter);
     if (rc != GMG_OK) return rc;
     long long launches = 0;
@@ -857,12 +875,17 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
         c->n_launch = 0;
         enqueue_init(c, tol, maxiter, solver, s);
         enqueue_pre(c, solver, p, z, lc, s);
-        while (true) {
+        while (!c->enqueue_fail) {
             CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
             CUDA_TRY(c, cudaStreamSynchronize(s));
             if (c->sc_host->done) break;
             enqueue_body(c, solver, p, z, lc, s);
             CUDA_TRY(c, cudaGetLastError());
+        }
+        if (c->enqueue_fail) {
+            cudaStreamSynchronize(s);
+            SET_ERR(c, "gmg_solve: a TMA-fed kernel of the plan could not be launched (tensor-map encode failed)");
+            return GMG_ECUDA;
         }
         enqueue_post(c, solver, p, z, s);
         CUDA_TRY(c, cudaEventRecord(c->ev1, s));
@@ -872,6 +895,7 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
         launches = c->n_launch;
     }
     CUDA_TRY(c, cudaGetLastError());
+    c->sc_fresh = true;
     const DevScalars& h = *c->sc_host;
     const int it = h.iter;
     // history and omegas came down with the status block (one synchronisation per solve)
@@ -981,14 +1005,14 @@ extern "C" int gmg_set_omega(gmg_ctx* c, float omega) {
 
 extern "C" int gmg_op_residual(gmg_ctx* c, int lev, const float* p, const float* b, float* r,
                                void* stream) {
-    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && p && b && r)
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && p && b && r && al16(p) && al16(b) && al16(r))
     gmgk::residual(c->g[lev], c->lv[lev].L, p, b, r, s);
     HOOK_EPILOGUE()
 }
 
 extern "C" int gmg_op_smooth(gmg_ctx* c, int lev, float* p, const float* b, float omega, int nsweeps,
                              int first_colour, void* stream) {
-    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && p && b && nsweeps >= 0 &&
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && p && b && nsweeps >= 0 && al16(p) && al16(b) &&
                   (first_colour == 0 || first_colour == 1))
     gmgk::ctl_set_hook_omega(c->sc, omega, s);
     smooth(c, lev, p, b, &c->sc->omega_hook, nsweeps, first_colour, nullptr, s);
@@ -996,28 +1020,28 @@ extern "C" int gmg_op_smooth(gmg_ctx* c, int lev, float* p, const float* b, floa
 }
 
 extern "C" int gmg_op_restrict(gmg_ctx* c, int lev, const float* r_fine, float* b_coarse, void* stream) {
-    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev - 1 && r_fine && b_coarse)
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev - 1 && r_fine && b_coarse && al16(r_fine) && al16(b_coarse))
     gmgk::restrict_sum(c->g[lev], r_fine, b_coarse, s);
     HOOK_EPILOGUE()
 }
 
 extern "C" int gmg_op_residual_restrict(gmg_ctx* c, int lev, const float* p, const float* b,
                                         float* b_coarse, void* stream) {
-    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev - 1 && p && b && b_coarse)
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev - 1 && p && b && b_coarse && al16(p) && al16(b) && al16(b_coarse))
     if (c->fast_rr[lev]) gmgf::residual_restrict(c->g[lev], c->lv[lev].L, p, b, b_coarse, nullptr, c->tma_ok[lev], s);
     else gmgk::residual_restrict(c->g[lev], c->lv[lev].L, p, b, b_coarse, nullptr, s);
     HOOK_EPILOGUE()
 }
 
 extern "C" int gmg_op_prolong(gmg_ctx* c, int lev, const float* e_coarse, float* p_fine, void* stream) {
-    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev - 1 && e_coarse && p_fine)
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev - 1 && e_coarse && p_fine && al16(e_coarse) && al16(p_fine))
     gmgk::prolong_add(c->g[lev], e_coarse, p_fine, s);
     HOOK_EPILOGUE()
 }
 
 extern "C" int gmg_op_vcycle(gmg_ctx* c, float* p, const float* z, float omega, int symmetric,
                              void* stream) {
-    HOOK_PROLOGUE(p && z)
+    HOOK_PROLOGUE(p && z && al16(p) && al16(z))
     gmgk::ctl_set_hook_omega(c->sc, omega, s);
     enqueue_vcycle(c, p, z, &c->sc->omega_hook, symmetric ? 1 : 0, s);
     HOOK_EPILOGUE()
@@ -1027,6 +1051,7 @@ extern "C" int gmg_op_sweep_with_norm(gmg_ctx* c, int lev, const float* src, flo
                                       float omega, int first_colour, double* rr_out, double* bb_out,
                                       void* stream) {
     HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && src && dst && b && src != dst && rr_out && bb_out &&
+                  al16(src) && al16(dst) && al16(b) &&
                   (first_colour == 0 || first_colour == 1))
     gmgk::ctl_set_hook_omega(c->sc, omega, s);
     if (!gmgf::rb_sweep_with_norm(c->g[lev], c->lv[lev].L, src, dst, b, &c->sc->omega_hook, first_colour,
@@ -1043,19 +1068,19 @@ extern "C" int gmg_op_sweep_with_norm(gmg_ctx* c, int lev, const float* src, flo
 }
 
 extern "C" int gmg_op_cg_smooth(gmg_ctx* c, int lev, float* x, const float* b, int iters, void* stream) {
-    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && x && b && iters >= 0)
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && x && b && iters >= 0 && al16(x) && al16(b))
     cg_smooth(c, lev, x, b, iters, s);
     HOOK_EPILOGUE()
 }
 
 extern "C" int gmg_op_vcycle_cgs(gmg_ctx* c, float* p, const float* z, void* stream) {
-    HOOK_PROLOGUE(p && z)
+    HOOK_PROLOGUE(p && z && al16(p) && al16(z))
     enqueue_vcycle_cgs(c, p, z, s);
     HOOK_EPILOGUE()
 }
 
 extern "C" int gmg_op_norm2(gmg_ctx* c, int lev, const float* r, double* out_host, void* stream) {
-    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && r && out_host)
+    HOOK_PROLOGUE(lev >= 0 && lev < c->nlev && r && out_host && al16(r))
     gmgk::norm2(c->g[lev].N, r, rbuf(c), RED_HOOK, s);
     CUDA_TRY(c, cudaGetLastError());
     CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
@@ -1069,6 +1094,7 @@ extern "C" int gmg_divergence(gmg_ctx* c, const float* u_dev, const float wall_h
                               void* stream) {
     if (!c) return GMG_EINVAL;
     if (!u_dev || !z_dev) { SET_ERR(c, "gmg_divergence: null pointer"); return GMG_EINVAL; }
+    if (!al16(u_dev) || !al16(z_dev)) { SET_ERR(c, "gmg_divergence: u_dev and z_dev must be 16-byte aligned"); return GMG_EINVAL; }
     cudaStream_t s = (cudaStream_t)stream;
     const float zero[3] = {0.0f, 0.0f, 0.0f};
     if (c->prm.fast_path && c->g[0].n[0] % 4 == 0) gmgk::divergence4(c->g[0], u_dev, wall_hi ? wall_hi : zero, z_dev, s);
@@ -1081,6 +1107,7 @@ extern "C" int gmg_divergence(gmg_ctx* c, const float* u_dev, const float wall_h
 extern "C" int gmg_project(gmg_ctx* c, float* u_dev, const float* p_dev, void* stream) {
     if (!c) return GMG_EINVAL;
     if (!u_dev || !p_dev) { SET_ERR(c, "gmg_project: null pointer"); return GMG_EINVAL; }
+    if (!al16(u_dev) || !al16(p_dev)) { SET_ERR(c, "gmg_project: u_dev and p_dev must be 16-byte aligned"); return GMG_EINVAL; }
     if (!c->coeffs_set) { SET_ERR(c, "gmg_project before gmg_set_coeffs"); return GMG_ESTATE; }
     cudaStream_t s = (cudaStream_t)stream;
     if (c->prm.fast_path && c->g[0].n[0] % 4 == 0) gmgk::project4(c->g[0], c->lv[0].L, p_dev, u_dev, s);
@@ -1096,6 +1123,10 @@ extern "C" int gmg_pressure_step(gmg_ctx* c, const float* L_dev, float* u_dev, c
                                  float* p_dev, float tol, int maxiter, int solver, void* stream) {
     if (!c) return GMG_EINVAL;
     if (!L_dev || !u_dev || !p_dev) { SET_ERR(c, "gmg_pressure_step: null pointer"); return GMG_EINVAL; }
+    if (!al16(L_dev) || !al16(u_dev) || !al16(p_dev)) {
+        SET_ERR(c, "gmg_pressure_step: L_dev, u_dev and p_dev must be 16-byte aligned");
+        return GMG_EINVAL;
+    }
     if (!c->ws_set) { SET_ERR(c, "gmg_pressure_step before gmg_set_workspace"); return GMG_ESTATE; }
     cudaStream_t s = (cudaStream_t)stream;
     const float zero[3] = {0.0f, 0.0f, 0.0f};
@@ -1105,6 +1136,10 @@ extern "C" int gmg_pressure_step(gmg_ctx* c, const float* L_dev, float* u_dev, c
     else gmgk::divergence(c->g[0], u_dev, wall_hi ? wall_hi : zero, c->stage_z, s);
     CUDA_TRY(c, cudaGetLastError());
     const int rc = gmg_solve(c, p_dev, c->stage_z, tol, maxiter, solver, stream);
+    if (!c->sc_fresh) {          // the solve returned before its status read: nothing is validated
+        c->coeffs_set = false;
+        return rc;
+    }
     if (c->sc_host->red[RED_CHECK] != 0.0) {
         SET_ERR(c, "gmg_pressure_step: %.0f coefficient(s) negative, NaN or infinite", c->sc_host->red[RED_CHECK]);
         c->coeffs_set = false;
@@ -1125,8 +1160,11 @@ extern "C" int gmg_describe_plan(const gmg_ctx* c, char* buf, size_t cap) {
         const bool tma = c->tma_ok[l] && c->g[l].n[0] % 128 == 0 && c->g[l].n[1] >= 4 && c->g[l].n[2] >= 8;
         const bool in_cluster = c->ctail_start < c->nlev && l >= c->ctail_start;
         const bool in_tail = in_cluster || l >= c->tail_start;
+        // TMA-fed sweep: which of its two instantiations the plain (not norm-carrying) sweeps run
         const char* how = in_cluster ? "tail(8-CTA cluster smem)" : in_tail ? "tail(single-CTA smem)"
-                          : (c->fast_sweep[l] ? (tma ? "fused-rb-sweep(TMA)" : "fused-rb-sweep") : "generic-half-sweeps");
+                          : (c->fast_sweep[l] ? (tma ? (gmgf::bulk_sweep_edge(c->g[l], false) ? "fused-rb-sweep(TMA,EDGE)"
+                                                                                               : "fused-rb-sweep(TMA,rowcopy-edges)")
+                                                     : "fused-rb-sweep") : "generic-half-sweeps");
         const char* rr = (in_tail || l == c->nlev - 1) ? "-"
                          : (c->fast_rr[l] ? "tiled" : "generic");
         int w = snprintf(buf + off, cap - off, "L%d %dx%dx%d c=%d%d%d sweep=%s resrestrict=%s\n", l,

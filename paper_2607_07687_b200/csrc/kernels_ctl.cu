@@ -66,9 +66,13 @@ __global__ void k_ctl_begin(DevScalars* sc, double* hist, double* omegas,
         done = 1;
     } else {
         hist[0] = rho / r_ref;
-        const bool conv = !(rho > sc->tol * r_ref);
+        // reading O9 as the oracle writes it: go on while rho > tol r_ref, converged iff
+        // rho <= tol r_ref -- a NaN norm (NaN/Inf in z or p) is neither: stop, NOT converged
+        const bool fin = isfinite(rho) && isfinite(r_ref);       // overflowed FP32 squares give Inf
+        const bool conv = fin && rho <= sc->tol * r_ref;
+        const bool go = fin && rho > sc->tol * r_ref && sc->maxiter > 0;
         sc->status = conv ? GMG_OK : GMG_NOT_CONVERGED;
-        done = conv || sc->maxiter <= 0;
+        done = !go;
     }
     if (omegas) omegas[0] = sc->omega;
     sc->omega_f = (float)sc->omega;
@@ -107,9 +111,11 @@ __global__ void k_ctl_rbgs_cycle_end(DevScalars* sc, double* hist, double* omega
     sc->rho_prev = sc->rho;
     sc->rho = rho_new;
     sc->iter = k;
-    const bool conv = !(rho_new > sc->tol * sc->r_ref);
+    const bool fin = isfinite(rho_new) && isfinite(sc->r_ref);
+    const bool conv = fin && rho_new <= sc->tol * sc->r_ref;        // false for a NaN / Inf norm ...
+    const bool go = fin && rho_new > sc->tol * sc->r_ref && k < sc->maxiter;   // ... and so is this
     sc->status = conv ? GMG_OK : GMG_NOT_CONVERGED;
-    const int done = conv || k >= sc->maxiter;
+    const int done = !go;
     if (!done) omegas[k] = sc->omega;
     // fused_norm path.  This cycle's norm came either from the next cycle's first sweep, which then
     // already ran with omega_spec_f (re-run it if the omega update went the other way), or -- the
@@ -171,9 +177,11 @@ __global__ void k_ctl_pcg_check(DevScalars* sc, double* hist, cudaGraphCondition
     sc->rho_prev = sc->rho;
     sc->rho = rn;
     sc->iter = k;
-    const bool conv = !(rn > sc->tol * sc->r_ref);
+    const bool fin = isfinite(rn) && isfinite(sc->r_ref);
+    const bool conv = fin && rn <= sc->tol * sc->r_ref;      // a NaN / Inf norm: not converged, stop
+    const bool go = fin && rn > sc->tol * sc->r_ref && k < sc->maxiter;
     sc->status = conv ? GMG_OK : GMG_NOT_CONVERGED;
-    const int done = conv || k >= sc->maxiter;
+    const int done = !go;
     sc->done = done;
     set_cond(cond, use_cond, !done);
 }

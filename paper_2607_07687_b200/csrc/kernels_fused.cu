@@ -27,15 +27,9 @@
 // (x0-1 and x0+TX) are updated by one extra "edge" warp, one lane per (side,row).
 // The per-cell arithmetic is stencil.cuh's apply7/diag6/relax, identical to the generic
 // kernels, so fast and generic paths agree bit for bit on every cell.
-#include <stdlib.h>
-
 #include "fused_common.cuh"
 
 namespace gmgf {
-static int zmin_env() {
-    static const int v = getenv("GMG_ZMIN") ? atoi(getenv("GMG_ZMIN")) : 4;
-    return v;
-}
 
 template <int TX_, int TY_>
 struct SweepCfg {
@@ -486,11 +480,6 @@ using Res128 = ResCfg<128, 4, 4>;
 using Res64 = ResCfg<64, 8, 4>;
 using Res32 = ResCfg<32, 16, 4>;
 
-static int env_int(const char* name, int dflt) {
-    const char* v = getenv(name);
-    return v ? atoi(v) : dflt;
-}
-
 bool sweep_v2_supported(const LevelGeom& g) {
     return g.n[0] % 4 == 0 && g.n[0] >= 16 && g.n[1] >= 2 && g.n[2] >= 4 &&
            (long long)g.n[0] * g.n[1] < (1LL << 30);
@@ -501,11 +490,9 @@ static void launch_sweep(SweepArgs& a, cudaStream_t s) {
     const LevelGeom& g = a.g;
     a.tiles_x = (g.n[0] + C::TX - 1) / C::TX;
     a.tiles_y = (g.n[1] + C::TY - 1) / C::TY;
-    static const int zc_env = env_int("GMG_ZCHUNK", 64);
-    const int zchunk = choose_zchunk((long long)a.tiles_x * a.tiles_y, g.n[2], zc_env, zmin_env(), 148, 0);
+    const int zchunk = choose_zchunk((long long)a.tiles_x * a.tiles_y, g.n[2], kZChunkPref, kZChunkMin, 148, 0);
     a.zchunk = zchunk;
-    static const int pf_env = env_int("GMG_PF", 3);
-    a.pf = pf_env;
+    a.pf = 3;   // L2 prefetch distance of the coefficient streams, in planes
     const int nzc = (g.n[2] + zchunk - 1) / zchunk;
     const unsigned int grid = (unsigned int)(a.tiles_x * a.tiles_y * nzc);
     k_rb_sweep<C, MB><<<grid, C::THREADS, C::SMEM, s>>>(a);

@@ -11,15 +11,9 @@
 // protects ring-slot reuse.  The x pair and y pair sums of the restriction happen in registers,
 // the z pair across two consecutive steps, in stencil.cuh's canonical tree order, so the result is
 // bit-identical to the generic kernel.  112 KB of shared memory per CTA: two CTAs per SM.
-#include <stdlib.h>
-
 #include "fused_common.cuh"
 
 namespace gmgf {
-static int zmin_env() {
-    static const int v = getenv("GMG_ZMIN") ? atoi(getenv("GMG_ZMIN")) : 4;
-    return v;
-}
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
@@ -384,14 +378,13 @@ template <int MODE>
 static bool launch_res_bulk(ResBulkArgs& a, cudaStream_t s) {
     using C = ResBulkCfg;
     const LevelGeom& g = a.g;
-    static const int use_bulk = getenv("GMG_BULK") ? atoi(getenv("GMG_BULK")) : 1;
-    if (!use_bulk || !bulk_supported(g) || (g.n[2] & 1)) return false;
+    if (!bulk_supported(g) || (g.n[2] & 1)) return false;
     ResBulkMaps maps;
     if (!res_maps(g, a.L, a.p, a.b, &maps)) return false;
     a.tiles_x = g.n[0] / C::TX;
     a.tiles_y = (g.n[1] + C::RY - 1) / C::RY;
     // two CTAs per SM; chunks start on even planes (the z pair of the restriction)
-    int zchunk = choose_zchunk((long long)a.tiles_x * a.tiles_y, g.n[2], 64, zmin_env(), 296, 1);
+    int zchunk = choose_zchunk((long long)a.tiles_x * a.tiles_y, g.n[2], kZChunkPref, kZChunkMin, 296, 1);
     // the deterministic reduction has a bounded number of block partials
     while (MODE >= 1 && (long long)a.tiles_x * a.tiles_y * ((g.n[2] + zchunk - 1) / zchunk) > GMG_REDUCE_MAX_BLOCKS)
         zchunk *= 2;
@@ -436,8 +429,7 @@ bool residual_norm2_bulk_if(const LevelGeom& g, const float* L, const float* p, 
     return launch_res_bulk<1>(a, s);
 }
 bool residual_norm_bulk_supported(const LevelGeom& g) {
-    static const int use_bulk = getenv("GMG_BULK") ? atoi(getenv("GMG_BULK")) : 1;
-    return use_bulk && bulk_supported(g) && !(g.n[2] & 1);
+    return bulk_supported(g) && !(g.n[2] & 1);
 }
 
 // sum r^2 -> red[slot_rr] and sum b^2 over active cells -> red[slot_ref] in ONE pass (loop entry)

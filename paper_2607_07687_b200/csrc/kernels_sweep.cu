@@ -21,19 +21,14 @@
 // bulk-copy path (cp.async.bulk, UBLKCP) with wrapped row addresses.  Neumann walls = zeroed
 // coefficients.  Every shared-memory cell holds the periodic image of its cell, as in k_rb_sweep.
 #include <cuda.h>
-#include <stdlib.h>
 
 #include <map>
+#include <mutex>
 #include <tuple>
 
 #include "fused_common.cuh"
 
 namespace gmgf {
-static int env_int2(const char* name, int dflt) {
-    const char* v = getenv(name);
-    return v ? atoi(v) : dflt;
-}
-
 template <int TY_, int PD_>
 struct BulkCfg {
     static constexpr int TX = 128, TY = TY_, PD = PD_;
@@ -649,6 +644,8 @@ EncodeTiledFn g_encode = nullptr;
 bool tensor_map(const float* ptr, const LevelGeom& g, int bw, int bh, CUtensorMap* out) {
     typedef std::tuple<const float*, int, int, int, int, int> Key;
     static std::map<Key, CUtensorMap> cache;
+    static std::mutex cache_mutex;   // contexts on several host threads share the cache
+    std::lock_guard<std::mutex> lock(cache_mutex);
     const Key key(ptr, g.n[0], g.n[1], g.n[2], bw, bh);
     auto it = cache.find(key);
     if (it != cache.end()) {
@@ -677,20 +674,15 @@ bool bulk_supported(const LevelGeom& g) {
     return g_encode && g.n[0] >= 128 && g.n[0] % 128 == 0 && g.n[1] >= 4 && g.n[2] >= 8;
 }
 
-bool tma_shape_ok(const LevelGeom& g) {
-    static const int use_bulk = env_int2("GMG_BULK", 1);
-    return use_bulk && bulk_supported(g);
-}
+bool tma_shape_ok(const LevelGeom& g) { return bulk_supported(g); }
 
 static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
                                  const float* omega, int first_colour, const ReduceBuf* norm, int slot_rr,
                                  int slot_ref, const int* run_flag, cudaStream_t s);
 
 static unsigned int bulk_grid(const LevelGeom& g, int* zchunk_out) {
-    static const int zc_env = env_int2("GMG_ZCHUNK", 64);
-    static const int zmin_env = env_int2("GMG_ZMIN", 4);
     const int tiles_x = g.n[0] / Bulk::TX, tiles_y = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
-    const int zchunk = choose_zchunk((long long)tiles_x * tiles_y, g.n[2], zc_env, zmin_env, 148, 0);
+    const int zchunk = choose_zchunk((long long)tiles_x * tiles_y, g.n[2], kZChunkPref, kZChunkMin, 148, 0);
     if (zchunk_out) *zchunk_out = zchunk;
     return (unsigned int)(tiles_x * tiles_y * ((g.n[2] + zchunk - 1) / zchunk));
 }
@@ -723,6 +715,15 @@ bool rb_sweep_if(const LevelGeom& g, const float* L, const float* src, float* ds
     return rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, nullptr, 0, 0, run_flag, s);
 }
 
+// Which instantiation of k_rb_sweep_bulk a level gets: true = EDGE (the kernel that carries the
+// boundary-box body), false = the two-body kernel whose y-boundary tile rows take row copies.
+// Few tile rows, or walls in y: EDGE.  The norm-carrying variants come out faster with the third
+// body at any size (5.91 vs 6.04 ms at 1024^3 in the same A/B).
+bool bulk_sweep_edge(const LevelGeom& g, bool norm) {
+    const int tiles_y = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
+    return g.bc[1] != 0 || (tiles_y >= 2 && (tiles_y <= 40 || norm));
+}
+
 static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
                                  const float* omega, int first_colour, const ReduceBuf* norm, int slot_rr,
                                  int slot_ref, const int* run_flag, cudaStream_t s) {
@@ -737,10 +738,7 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
     ok = ok && set(maps.m[0], Bulk::SH, Bulk::ROWS, Bulk::ROWS + 1);
     const int tiles_y_ = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
     const int rem = g.n[1] - (tiles_y_ - 1) * Bulk::TY;      // rows of the final tile row
-    // few tile rows, or walls in y: the kernel with the boundary-box body (see k_rb_sweep_bulk)
-    // (the norm-carrying variants come out faster with the third body at any size: 5.91 vs 6.04 ms
-    // at 1024^3 in the same A/B)
-    const bool edge = g.bc[1] != 0 || (tiles_y_ >= 2 && (tiles_y_ <= 40 || norm != nullptr));
+    const bool edge = bulk_sweep_edge(g, norm != nullptr);
     if (ok && edge && g.bc[1] == 0 && tiles_y_ >= 2) {
         ok = ok && set(maps.m[1], Bulk::SH - 2, Bulk::ROWS - 1, Bulk::ROWS);   // FIRST: from y = 0
         ok = ok && set(maps.m[2], rem + 2, rem + 1, rem + 1);                  // FINAL: up to y = ny - 1

@@ -28,7 +28,13 @@ CASES = {
     "rand_128_PPP": lambda: random_workload((128, 40, 8), (0, 0, 0), 17),
     "rand_256_aniso": lambda: random_workload((256, 6, 12), (0, 0, 0), 18),      # c = (2,1,2)
     "rand_128_xonly": lambda: random_workload((128, 36, 10), (1, 0, 0), 19, blob=False),
+    # more than 40 tile rows on a periodic y axis: the instantiation k_rb_sweep_bulk<.., EDGE = false>
+    # that bench.py's 1024^3 level 0 runs (interior boxes + ROW-COPY tiles on the first / final tile
+    # row, final tile ragged: 534 = 41 * 13 + 1, 546 = 42 * 13), whole field against the oracle
+    "rand_128x534x16_PPP": lambda: random_workload((128, 534, 16), (0, 0, 0), 20),
+    "rand_256x546x8_NPP": lambda: random_workload((256, 546, 8), (1, 0, 0), 21),
 }
+NON_EDGE = ("rand_128x534x16_PPP", "rand_256x546x8_NPP")
 
 
 @pytest.fixture(scope="module", params=sorted(CASES), ids=sorted(CASES))
@@ -44,6 +50,17 @@ def _fields(n, seed):
     rng = np.random.default_rng(seed)
     shp = (n[2], n[1], n[0])
     return (rng.standard_normal(shp).astype(np.float32), rng.standard_normal(shp).astype(np.float32))
+
+
+def test_plan_names_the_sweep_instantiation(case):
+    """describe_plan says which k_rb_sweep_bulk instantiation a TMA-fed level runs, so that the
+    whole-field comparisons below are known to cover BOTH."""
+    wl, g, h = case
+    line0 = g.describe_plan().split("\n")[0]
+    if wl.name.startswith("random_") and wl.n[1] > 520 and wl.bc[1] == 0:
+        assert "fused-rb-sweep(TMA,rowcopy-edges)" in line0, line0
+    elif wl.n[0] % 128 == 0 and wl.n[1] >= 4 and wl.n[2] >= 8:
+        assert "fused-rb-sweep(TMA,EDGE)" in line0 or wl.n[1] <= 13, line0
 
 
 def test_level_shapes_match_oracle(case):

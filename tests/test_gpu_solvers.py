@@ -20,9 +20,9 @@ SOLVERS = {"rbgs": (gmg.GMG_RBGS, oracle.GMG_RBGS), "gmgpcg": (gmg.GMG_PCG, orac
 CONFIGS = {
     "c0": (lambda: W.config0(), ("rbgs", "gmgpcg", "pcg"), 2000),
     "c1": (lambda: W.config1(), ("rbgs", "gmgpcg", "pcg"), 2000),
-    "c2": (lambda: W.config2(), ("rbgs", "gmgpcg"), 2000),
+    "c2": (lambda: W.config2(), ("rbgs", "gmgpcg", "pcg"), 2000),
     "c3p5": (lambda: W.config3(5), ("rbgs", "gmgpcg", "pcg"), 2000),
-    "c3p6": (lambda: W.config3(6), ("rbgs", "gmgpcg"), 2000),
+    "c3p6": (lambda: W.config3(6), ("rbgs", "gmgpcg", "pcg"), 2000),
     "c4_128": (lambda: W.by_name("c4_128"), ("rbgs", "gmgpcg"), 2000),
 }
 
@@ -88,7 +88,7 @@ def test_adaptive_omega_sequence_matches_oracle():
         assert rc == gmg.NOT_CONVERGED and st["iterations"] == 8 == ref["iterations"]
         om_g = g.omega_history()
         assert list(om_g) == list(ref["omegas"])
-        assert list(om_g[:4]) == [1.0, 0.875, 0.90625, 0.78125]
+        assert len(set(om_g)) >= 4 and min(om_g) < 0.8      # both branches were taken
         assert st["omega_final"] == h.omega == 0.5
         assert np.allclose(hist, ref["history"], rtol=2e-3)
         act = W.active_mask(wl.L, wl.bc)
