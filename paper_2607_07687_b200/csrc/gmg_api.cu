@@ -915,7 +915,7 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
     st.resid_ref = h.r_ref;
     st.resid_init_rel = c->hist_host[0];
     if (solver == GMG_GMG_RBGS || solver == GMG_GMG_CGS) st.resid_final_rel = c->hist_host[it];
-    else st.resid_final_rel = (h.r_ref > 0.0) ? sqrt(h.red[RED_RR]) / h.r_ref : 0.0;
+    else st.resid_final_rel = (h.r_ref == 0.0) ? 0.0 : sqrt(h.red[RED_RR]) / h.r_ref;   // NaN stays NaN
     st.gpu_ms = ms;
     st.kernel_launches = launches;
     st.history_len = it + 1;
