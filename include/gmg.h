@@ -92,6 +92,16 @@ typedef struct {
                           by a 20 B/cell pass of its own after every cycle; the cycle expected to be
                           the last (rate-based prediction, or the maxiter-th) takes the plain pass
                           instead, so that no sweep is wasted at the exit; same iterates, same test (1) */
+    int uniform_tiles; /* 1: gmg_set_coeffs marks the bricks (128 x 8 x 8 cells) of every TMA-fed level
+                          whose stored coefficients all equal the level's constant per direction -- 1 on
+                          the finest level (the BDIM coefficient away from bodies; north_star "L in
+                          [0,1]"), (prod_{e != d} C_e) / C_d on coarser ones (reading O5 applied to ones) --
+                          and a CTA whose footprint holds only such bricks and no wall skips the three
+                          coefficient streams: 12 instead of 24 B/cell per sweep, 8 + 4/m instead of
+                          20 + 4/m for the residual pass.  LOSSLESS: the same operations run on the
+                          constants, every cell gets the same bits (SURVEY.md S8(d) "a lossless 'tile is
+                          all L=1' flag ... honest only if reported as such": gmg_stats.uniform_fraction
+                          and bytes_as_run report it).  0: every CTA loads its coefficients (1) */
 } gmg_params_t;
 
 /* Statistics of the last gmg_solve. */
@@ -108,6 +118,9 @@ typedef struct {
     double bytes_algorithmic; /* algorithmic HBM bytes of the solve (DESIGN.md table) */
     long long kernel_launches; /* kernels launched (graph nodes count) by the solve */
     int history_len;        /* entries available through gmg_history (iterations+1) */
+    double uniform_fraction; /* share of the finest level's cells swept by CTAs on the lean path
+                                (uniform_tiles; 0 when off or when level 0 is not TMA-fed) */
+    double bytes_as_run;    /* bytes_algorithmic minus the coefficient bytes the lean path did not move */
 } gmg_stats_t;
 
 /* Level table and workspace size for a grid WITHOUT creating a context (host-only: no CUDA call).

@@ -10,38 +10,43 @@
 #include <vector>
 
 #include "gmg_internal.h"
+#include "uniform.cuh"
 
 namespace gmgf {  // fast-path launchers (kernels_fused.cu)
 bool sweep_supported(const LevelGeom& g);
 // nsweeps (even count handled by caller) fused red+black sweeps src -> dst (out of place).
 // first_colour 0: red then black.  If e_c != nullptr the prolonged coarse correction is added
 // to src on the fly (fused prolongation + correction).
+// `uni`: the level's uniform bricks (uniform.cuh), brick == nullptr where the lean path is off
 void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
-              const float* omega, int first_colour, const float* e_c, int allow_tma, cudaStream_t s);
+              const float* omega, int first_colour, const float* e_c, int allow_tma, const UniArgs& uni,
+              cudaStream_t s);
 bool resrestrict_supported(const LevelGeom& g);
 void residual_restrict(const LevelGeom& g, const float* L, const float* p, const float* b,
-                       float* b_c, float* p_c, int allow_tma, cudaStream_t s);
+                       float* b_c, float* p_c, int allow_tma, const UniArgs& uni, cudaStream_t s);
 void residual_norm2(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
-                    int slot, int allow_tma, cudaStream_t s);
+                    int slot, int allow_tma, const UniArgs& uni, cudaStream_t s);
 bool residual_and_ref_norm2_bulk(const LevelGeom& g, const float* L, const float* p, const float* b,
-                                 ReduceBuf rb, int slot_rr, int slot_ref, cudaStream_t s);
+                                 ReduceBuf rb, int slot_rr, int slot_ref, const UniArgs& uni, cudaStream_t s);
 void prolong_add4(const LevelGeom& g, const float* e_c, float* p_f, cudaStream_t s);
 bool matvec_dot_bulk(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot,
-                     cudaStream_t s);
+                     const UniArgs& uni, cudaStream_t s);
+double bulk_sweep_uniform_fraction(const LevelGeom& g, const unsigned char* brick_host);
+double res_bulk_uniform_fraction(const LevelGeom& g, const unsigned char* brick_host);
 bool tma_shape_ok(const LevelGeom& g);
 bool bulk_sweep_edge(const LevelGeom& g, bool norm);
 // one TMA-fed sweep src -> dst that also leaves sum r^2 (r = b - A src) and sum b^2 over the active
 // cells in red[slot_rr] / red[slot_ref]; false = the level cannot run it (nothing launched)
 bool rb_sweep_with_norm(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
                         const float* omega, int first_colour, ReduceBuf rb, int slot_rr, int slot_ref,
-                        const int* run_flag, cudaStream_t s);
+                        const int* run_flag, const UniArgs& uni, cudaStream_t s);
 bool residual_norm2_bulk_if(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
-                            int slot, const int* run_flag, cudaStream_t s);
+                            int slot, const int* run_flag, const UniArgs& uni, cudaStream_t s);
 bool residual_norm_bulk_supported(const LevelGeom& g);
 bool sweep_norm_supported(const LevelGeom& g);
 // the same sweep as a no-op unless *run_flag != 0
 bool rb_sweep_if(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
-                 const float* omega, int first_colour, const int* run_flag, cudaStream_t s);
+                 const float* omega, int first_colour, const int* run_flag, const UniArgs& uni, cudaStream_t s);
 int configure();
 }  // namespace gmgf
 
@@ -73,6 +78,15 @@ struct gmg_ctx {
     bool fast_rr[GMG_MAX_LEVELS];
     int tma_ok[GMG_MAX_LEVELS];  // level large enough for the TMA-fed kernels
     bool fused_norm_on;   // GMG-RBGS: the stopping-test norm rides on the first pre-sweep (prm.fused_norm)
+    // uniform bricks (uniform.cuh): levels that run the TMA-fed kernels
+    gmgf::UniArgs uni[GMG_MAX_LEVELS];     // brick == nullptr: level not marked
+    size_t ubrick_n[GMG_MAX_LEVELS];       // bricks of the level
+    unsigned char* ubrick_dev;             // all levels' flags, one allocation
+    unsigned char* ubrick_host;            // pinned mirror
+    size_t ubrick_total;
+    double uni_frac_sweep[GMG_MAX_LEVELS]; // cells whose sweep / residual CTA takes the lean path
+    double uni_frac_res[GMG_MAX_LEVELS];
+    bool uni_stats_pending;                // flags copied down, fractions not yet recomputed
     // workspace
     void* ws;
     size_t ws_bytes;
@@ -115,6 +129,7 @@ struct gmg_ctx {
 static const long long kBulkMatvecMinCells = 4LL << 20;
 
 static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+static inline const gmgf::UniArgs& U(const gmg_ctx* c, int l) { return c->uni[l]; }
 // The float4 / TMA paths read caller arrays 16 bytes at a time (gmg.h "Alignment").
 static inline bool al16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
 #define MUST_LAUNCH(c, call) do { if (!(call)) (c)->enqueue_fail = true; } while (0)
@@ -177,6 +192,20 @@ static void build_levels(gmg_ctx* c) {
         c->fast_rr[l] = c->prm.fast_path && l + 1 < c->nlev && gmgf::resrestrict_supported(c->g[l]);
         c->tma_ok[l] = c->prm.tma_min_cells >= 0 && c->g[l].N >= (long long)c->prm.tma_min_cells;
     }
+    // uniform.cuh: the constant a level's coefficients take where every fine coefficient below is 1
+    // (reading O5 applied to ones): (prod_{e != d} C_e) / C_d with C the cumulative coarsening factors
+    {
+        double C[3] = {1.0, 1.0, 1.0};
+        for (int l = 0; l < c->nlev; ++l) {
+            c->uni[l].ux = (float)(C[1] * C[2] / C[0]);
+            c->uni[l].uy = (float)(C[0] * C[2] / C[1]);
+            c->uni[l].uz = (float)(C[0] * C[1] / C[2]);
+            c->uni[l].brick = nullptr;
+            c->ubrick_n[l] = 0;
+            c->uni_frac_sweep[l] = c->uni_frac_res[l] = 0.0;
+            for (int d = 0; d < 3; ++d) C[d] *= c->g[l].c[d];
+        }
+    }
     const int first_tail = c->ctail_start < c->tail_start ? c->ctail_start : c->tail_start;
     c->fused_norm_on = c->prm.fused_norm && c->prm.fast_path && c->nlev > 1 && first_tail > 0 &&
                        c->fast_sweep[0] && c->tma_ok[0] && c->prm.nu_pre >= 2;
@@ -218,6 +247,38 @@ static size_t carve(gmg_ctx* c, char* base) {
     return off;
 }
 
+// Brick flags of the levels that run the TMA-fed kernels: one small library-owned allocation.
+static void free_uniform(gmg_ctx* c) {
+    if (c->ubrick_dev) cudaFree(c->ubrick_dev);
+    if (c->ubrick_host) cudaFreeHost(c->ubrick_host);
+    c->ubrick_dev = c->ubrick_host = nullptr;
+    c->ubrick_total = 0;
+    for (int l = 0; l < GMG_MAX_LEVELS; ++l) { c->uni[l].brick = nullptr; c->ubrick_n[l] = 0; }
+}
+static cudaError_t alloc_uniform(gmg_ctx* c) {
+    free_uniform(c);
+    if (!c->prm.uniform_tiles || !c->prm.fast_path) return cudaSuccess;
+    const int first_tail = c->ctail_start < c->tail_start ? c->ctail_start : c->tail_start;
+    size_t off[GMG_MAX_LEVELS], total = 0;
+    for (int l = 0; l < c->nlev && l < first_tail; ++l) {
+        off[l] = total;
+        if (!(c->fast_sweep[l] && c->tma_ok[l] && gmgf::tma_shape_ok(c->g[l]))) continue;
+        c->ubrick_n[l] = (size_t)gmgf::ub_count(c->g[l].n[0], gmgf::kUBX) * gmgf::ub_count(c->g[l].n[1], gmgf::kUBY) *
+                         gmgf::ub_count(c->g[l].n[2], gmgf::kUBZ);
+        total += align_up(c->ubrick_n[l], 16);
+    }
+    if (total == 0) return cudaSuccess;
+    // + one counter per level (uniform bricks), behind the flags
+    const size_t bytes = total + sizeof(unsigned int) * GMG_MAX_LEVELS;
+    cudaError_t e = cudaMalloc(&c->ubrick_dev, bytes);
+    if (e == cudaSuccess) e = cudaMallocHost(&c->ubrick_host, bytes);
+    if (e != cudaSuccess) { free_uniform(c); return e; }
+    c->ubrick_total = total;
+    for (int l = 0; l < c->nlev; ++l)
+        if (c->ubrick_n[l]) c->uni[l].brick = c->ubrick_dev + off[l];
+    return cudaSuccess;
+}
+
 static void drop_graphs(gmg_ctx* c) {
     for (auto& s : c->slots) {
         if (s.exec) cudaGraphExecDestroy(s.exec);
@@ -232,6 +293,7 @@ extern "C" void gmg_default_params(gmg_params_t* p) {
     p->adaptive = 1; p->coarsen_mode = GMG_COARSEN_ANISO; p->n_min = 4;
     p->fast_path = 1; p->use_graph = 1; p->tma_min_cells = 1 << 20; p->cluster_tail = 1;
     p->fused_norm = 1;
+    p->uniform_tiles = 1;
 }
 
 extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]) {
@@ -258,6 +320,7 @@ extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]
     c->cap_a = c->cap_b = nullptr;
     c->cluster_ok = false;
     c->enqueue_fail = false; c->sc_fresh = false;
+    c->ubrick_dev = c->ubrick_host = nullptr; c->ubrick_total = 0; c->uni_stats_pending = false;
     if (gmgk::ctail_configure(200 * 1024) == (int)cudaSuccess) c->cluster_ok = gmgk::ctail_launchable(200 * 1024);
     cudaGetLastError();
     build_levels(c);
@@ -288,6 +351,7 @@ extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]
 extern "C" void gmg_destroy(gmg_ctx* c) {
     if (!c) return;
     drop_graphs(c);
+    free_uniform(c);
     if (c->sc) cudaFree(c->sc);
     if (c->partials) cudaFree(c->partials);
     if (c->counter) cudaFree(c->counter);
@@ -314,6 +378,7 @@ extern "C" int gmg_set_params(gmg_ctx* c, const gmg_params_t* p) {
     }
     c->prm = *p;
     drop_graphs(c);
+    free_uniform(c);
     build_levels(c);
     c->ws_set = false;
     c->coeffs_set = false;
@@ -341,6 +406,7 @@ extern "C" int gmg_set_workspace(gmg_ctx* c, void* ws, size_t bytes) {
     drop_graphs(c);
     carve(c, (char*)ws);
     c->ws = ws; c->ws_bytes = bytes; c->ws_set = true; c->coeffs_set = false;
+    CUDA_TRY(c, alloc_uniform(c));
     return GMG_OK;
 }
 
@@ -401,7 +467,33 @@ static void set_coeffs_enqueue(gmg_ctx* c, const float* L_dev, cudaStream_t s) {
     }
     for (int l = (c->ctail_start < c->tail_start ? c->ctail_start : c->tail_start); l < c->nlev; ++l)
         gmgk::tail_weights(c->g[l], c->lv[l].L, c->tail_W[l], s);
+    // uniform bricks of the TMA-fed levels (uniform.cuh); flags and counts come down with the status
+    if (c->ubrick_dev) {
+        unsigned int* cnt = reinterpret_cast<unsigned int*>(c->ubrick_dev + c->ubrick_total);
+        cudaMemsetAsync(cnt, 0, sizeof(unsigned int) * GMG_MAX_LEVELS, s);
+        for (int l = 0; l < c->nlev; ++l)
+            if (c->uni[l].brick)
+                gmgk::uniform_bricks(c->g[l], c->lv[l].L, c->uni[l].ux, c->uni[l].uy, c->uni[l].uz,
+                                     const_cast<unsigned char*>(c->uni[l].brick), cnt + l, s);
+        cudaMemcpyAsync(c->ubrick_host, c->ubrick_dev, c->ubrick_total + sizeof(unsigned int) * GMG_MAX_LEVELS,
+                        cudaMemcpyDeviceToHost, s);
+        c->uni_stats_pending = true;
+    }
     gmgk::ctl_set_omega(c->sc, (double)c->prm.omega0, s);
+}
+
+// After a synchronisation behind set_coeffs_enqueue: which share of each level's cells the lean
+// path covers (the kernels' own footprint test on the host copy of the flags).
+static void refresh_uniform_stats(gmg_ctx* c) {
+    if (!c->uni_stats_pending) return;
+    c->uni_stats_pending = false;
+    for (int l = 0; l < c->nlev; ++l) {
+        c->uni_frac_sweep[l] = c->uni_frac_res[l] = 0.0;
+        if (!c->uni[l].brick) continue;
+        const unsigned char* hb = c->ubrick_host + (c->uni[l].brick - c->ubrick_dev);
+        c->uni_frac_sweep[l] = gmgf::bulk_sweep_uniform_fraction(c->g[l], hb);
+        c->uni_frac_res[l] = gmgf::res_bulk_uniform_fraction(c->g[l], hb);
+    }
 }
 
 extern "C" int gmg_set_coeffs(gmg_ctx* c, const float* L_dev, void* stream) {
@@ -420,6 +512,7 @@ extern "C" int gmg_set_coeffs(gmg_ctx* c, const float* L_dev, void* stream) {
         return GMG_EINVAL;
     }
     c->coeffs_set = true;
+    refresh_uniform_stats(c);
     return GMG_OK;
 }
 
@@ -452,10 +545,10 @@ static void smooth(gmg_ctx* c, int l, float* p, const float* b, const float* ome
         const int pairs = nsweeps / 2;
         for (int i = 0; i < pairs; ++i) {
             if (!(i == 0 && skip_first)) {
-                gmgf::rb_sweep(g, c->lv[l].L, p, q, b, omega, first_colour, (i == 0) ? e_c : nullptr, c->tma_ok[l], s);
+                gmgf::rb_sweep(g, c->lv[l].L, p, q, b, omega, first_colour, (i == 0) ? e_c : nullptr, c->tma_ok[l], U(c, l), s);
                 c->n_launch += 1;
             }
-            gmgf::rb_sweep(g, c->lv[l].L, q, p, b, omega, first_colour, nullptr, c->tma_ok[l], s);
+            gmgf::rb_sweep(g, c->lv[l].L, q, p, b, omega, first_colour, nullptr, c->tma_ok[l], U(c, l), s);
             c->n_launch += 1;
         }
         done = 2 * pairs;
@@ -484,7 +577,7 @@ static void enqueue_vcycle(gmg_ctx* c, float* p0, const float* b0, const float* 
     for (; l < ts && l < nlev - 1; ++l) {
         smooth(c, l, P(l), B(l), omega, c->prm.nu_pre, 0, nullptr, s, l == 0 ? skip_first : 0);
         if (c->fast_rr[l])
-            gmgf::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, c->tma_ok[l], s);
+            gmgf::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, c->tma_ok[l], U(c, l), s);
         else
             gmgk::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, s);
         c->n_launch += 1;
@@ -535,7 +628,7 @@ static void cg_smooth(gmg_ctx* c, int l, float* x, const float* b, int m, cudaSt
     c->n_launch += 3;
     for (int it = 0; it < m; ++it) {
         if (!(c->prm.fast_path && c->tma_ok[l] && (c->prm.tma_min_cells == 0 || g.N >= kBulkMatvecMinCells) &&
-              gmgf::matvec_dot_bulk(g, L, d, q, rbuf(c), RED_DQ, s)))
+              gmgf::matvec_dot_bulk(g, L, d, q, rbuf(c), RED_DQ, U(c, l), s)))
             gmgk::matvec_dot(g, L, d, q, rbuf(c), RED_DQ, s);
         gmgk::ctl_cgs_alpha(c->sc, s);
         gmgk::pcg_update_pr(g, L, x, r, d, q, nullptr, 0, rbuf(c), s);
@@ -557,7 +650,7 @@ static void enqueue_vcycle_cgs(gmg_ctx* c, float* p0, const float* b0, cudaStrea
     for (int l = 0; l < nlev - 1; ++l) {
         cg_smooth(c, l, P(l), B(l), c->prm.nu_pre, s);
         if (c->fast_rr[l])
-            gmgf::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, c->tma_ok[l], s);
+            gmgf::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, c->tma_ok[l], U(c, l), s);
         else
             gmgk::residual_restrict(c->g[l], c->lv[l].L, P(l), B(l), c->lv[l + 1].b, c->lv[l + 1].p, s);
         c->n_launch += 1;
@@ -591,20 +684,22 @@ static double vcycle_cgs_bytes(const gmg_ctx* c) {
 }
 
 // Algorithmic HBM bytes of one V-cycle + its stopping-test norm.
-static double vcycle_bytes(const gmg_ctx* c, bool with_norm) {
+// as_run: minus the 12 B/cell of coefficient streams the lean path (uniform.cuh) does not move
+static double vcycle_bytes(const gmg_ctx* c, bool with_norm, bool as_run = false) {
     double total = 0.0;
     for (int l = 0; l < c->nlev; ++l) {
         const double N = (double)c->g[l].N;
         const double m = (double)(c->g[l].c[0] * c->g[l].c[1] * c->g[l].c[2]);
+        const double fs = as_run ? c->uni_frac_sweep[l] : 0.0, fr = as_run ? c->uni_frac_res[l] : 0.0;
         if (l == c->nlev - 1) {
             total += N * 24.0 * c->prm.nu_coarse;
         } else {
-            total += N * 24.0 * (c->prm.nu_pre + c->prm.nu_post);  // fused red+black sweeps
-            total += N * (20.0 + 4.0 / m);                          // residual + restriction
+            total += N * (24.0 - 12.0 * fs) * (c->prm.nu_pre + c->prm.nu_post);  // fused red+black sweeps
+            total += N * (20.0 - 12.0 * fr + 4.0 / m);                            // residual + restriction
             total += N * (4.0 / m);                                 // prolongation fused in a sweep
         }
     }
-    if (with_norm) total += 20.0 * (double)c->g[0].N;
+    if (with_norm) total += (20.0 - (as_run ? 12.0 * c->uni_frac_res[0] : 0.0)) * (double)c->g[0].N;
     return total;
 }
 
@@ -616,7 +711,7 @@ struct LoopCtl {
 
 static void level0_residual_norm2(gmg_ctx* c, const float* p, const float* z, cudaStream_t s) {
     if (c->prm.fast_path && gmgf::resrestrict_supported(c->g[0]))
-        gmgf::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, c->tma_ok[0], s);
+        gmgf::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, c->tma_ok[0], U(c, 0), s);
     else
         gmgk::residual_norm2(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, s);
 }
@@ -638,7 +733,7 @@ static bool predict_active(const gmg_ctx* c) {
 static void first_sweep_with_norm(gmg_ctx* c, float* p, const float* z, const float* omega, bool with_ref,
                                   const int* run_flag, cudaStream_t s) {
     MUST_LAUNCH(c, gmgf::rb_sweep_with_norm(c->g[0], c->lv[0].L, p, c->lv[0].q, z, omega, 0, rbuf(c), RED_RR,
-                                            with_ref ? RED_RREF : -1, run_flag, s));
+                                            with_ref ? RED_RREF : -1, run_flag, U(c, 0), s));
 }
 
 static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream_t s, bool cgs = false) {
@@ -650,7 +745,7 @@ static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStrea
     }
     // reference norm ||z|| over active cells and initial residual norm: one fused pass on big levels
     if (c->prm.fast_path && c->tma_ok[0] &&
-        gmgf::residual_and_ref_norm2_bulk(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, RED_RREF, s)) {
+        gmgf::residual_and_ref_norm2_bulk(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, RED_RREF, U(c, 0), s)) {
         c->n_launch += 1;
     } else {
         gmgk::active_norm2(c->g[0], c->lv[0].L, z, rbuf(c), RED_RREF, s);
@@ -664,18 +759,18 @@ static void rbgs_body(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStre
     if (!cgs && fused_norm_active(c)) {
         const bool pred = predict_active(c);
         if (pred) {   // after a failed "last cycle" prediction the first sweep is still to run
-            MUST_LAUNCH(c, gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->need_first, s));
+            MUST_LAUNCH(c, gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->need_first, U(c, 0), s));
             c->n_launch += 1;
         }
         enqueue_vcycle(c, p, z, &c->sc->omega_f, 0, s, 1);             // its first sweep already ran
         if (pred) {   // expected to be the last cycle: the plain norm pass
-            MUST_LAUNCH(c, gmgf::residual_norm2_bulk_if(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, &c->sc->expect_last, s));
+            MUST_LAUNCH(c, gmgf::residual_norm2_bulk_if(c->g[0], c->lv[0].L, p, z, rbuf(c), RED_RR, &c->sc->expect_last, U(c, 0), s));
             c->n_launch += 1;
         }
         // otherwise: next cycle's first sweep, + ||z - A p_k||
         first_sweep_with_norm(c, p, z, &c->sc->omega_spec_f, false, pred ? &c->sc->run_s1n : nullptr, s);
         gmgk::ctl_rbgs_cycle_end(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
-        MUST_LAUNCH(c, gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->redo_first, s));
+        MUST_LAUNCH(c, gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->redo_first, U(c, 0), s));
         c->n_launch += 3;
         return;
     }
@@ -709,7 +804,7 @@ static void pcg_body(gmg_ctx* c, float* p, int gmg_precond, LoopCtl lc, cudaStre
     gmgk::ctl_pcg_beta(c->sc, s);
     gmgk::pcg_update_d(N, c->pcg_d, c->pcg_s, c->sc, 0, s);
     if (!(c->prm.fast_path && c->tma_ok[0] && (c->prm.tma_min_cells == 0 || c->g[0].N >= kBulkMatvecMinCells) &&
-          gmgf::matvec_dot_bulk(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rbuf(c), RED_DQ, s)))
+          gmgf::matvec_dot_bulk(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rbuf(c), RED_DQ, U(c, 0), s)))
         gmgk::matvec_dot(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rbuf(c), RED_DQ, s);
     gmgk::ctl_pcg_alpha(c->sc, s);
     gmgk::pcg_update_pr(c->g[0], c->lv[0].L, p, c->pcg_r, c->pcg_d, c->pcg_q, nullptr, 0, rbuf(c), s);
@@ -921,13 +1016,17 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
     st.history_len = it + 1;
     const double N0 = (double)c->g[0].N;
     // loop entry: one pass over p, z, L -- unless the norms ride on sweeps that run anyway (fused_norm)
+    refresh_uniform_stats(c);   // gmg_pressure_step: the flags came down with this solve's status
+    st.uniform_fraction = c->uni_frac_sweep[0];
     if (solver == GMG_GMG_RBGS) {
         const bool fn = fused_norm_active(c);
         st.bytes_algorithmic = (fn ? 0.0 : 20.0 * N0) + it * vcycle_bytes(c, !fn);
+        st.bytes_as_run = (fn ? 0.0 : (20.0 - 12.0 * c->uni_frac_res[0]) * N0) + it * vcycle_bytes(c, !fn, true);
     }
     else if (solver == GMG_GMG_CGS) st.bytes_algorithmic = 20.0 * N0 + it * vcycle_cgs_bytes(c);
     else if (solver == GMG_PCG) st.bytes_algorithmic = 60.0 * N0 + it * 64.0 * N0;
     else st.bytes_algorithmic = 60.0 * N0 + it * (vcycle_bytes(c, false) + 52.0 * N0);
+    if (solver != GMG_GMG_RBGS) st.bytes_as_run = st.bytes_algorithmic;   // not modelled for the comparison solvers
     if (h.status == GMG_EBREAKDOWN) SET_ERR(c, "PCG breakdown: d.q == 0 at iteration %d", it);
     return h.status;
 }
@@ -1028,7 +1127,7 @@ extern "C" int gmg_op_restrict(gmg_ctx* c, int lev, const float* r_fine, float* 
 extern "C" int gmg_op_residual_restrict(gmg_ctx* c, int lev, const float* p, const float* b,
                                         float* b_coarse, void* stream) {
     HOOK_PROLOGUE(lev >= 0 && lev < c->nlev - 1 && p && b && b_coarse && al16(p) && al16(b) && al16(b_coarse))
-    if (c->fast_rr[lev]) gmgf::residual_restrict(c->g[lev], c->lv[lev].L, p, b, b_coarse, nullptr, c->tma_ok[lev], s);
+    if (c->fast_rr[lev]) gmgf::residual_restrict(c->g[lev], c->lv[lev].L, p, b, b_coarse, nullptr, c->tma_ok[lev], U(c, lev), s);
     else gmgk::residual_restrict(c->g[lev], c->lv[lev].L, p, b, b_coarse, nullptr, s);
     HOOK_EPILOGUE()
 }
@@ -1055,7 +1154,7 @@ extern "C" int gmg_op_sweep_with_norm(gmg_ctx* c, int lev, const float* src, flo
                   (first_colour == 0 || first_colour == 1))
     gmgk::ctl_set_hook_omega(c->sc, omega, s);
     if (!gmgf::rb_sweep_with_norm(c->g[lev], c->lv[lev].L, src, dst, b, &c->sc->omega_hook, first_colour,
-                                  rbuf(c), RED_HOOK, RED_HOOK2, nullptr, s)) {
+                                  rbuf(c), RED_HOOK, RED_HOOK2, nullptr, U(c, lev), s)) {
         SET_ERR(c, "gmg_op_sweep_with_norm: level %d cannot run the TMA-fed sweep", lev);
         return GMG_EINVAL;
     }

@@ -28,6 +28,7 @@
 // The per-cell arithmetic is stencil.cuh's apply7/diag6/relax, identical to the generic
 // kernels, so fast and generic paths agree bit for bit on every cell.
 #include "fused_common.cuh"
+#include "uniform.cuh"
 
 namespace gmgf {
 
@@ -524,14 +525,14 @@ static void launch_res(ResArgs& a, cudaStream_t s) {
 }
 
 bool residual_restrict_bulk(const LevelGeom& g, const float* L, const float* p, const float* b, float* b_c,
-                            float* p_c, cudaStream_t s);
+                            float* p_c, const UniArgs& uni, cudaStream_t s);
 bool residual_norm2_bulk(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
-                         int slot, cudaStream_t s);
+                         int slot, const UniArgs& uni, cudaStream_t s);
 int configure_residual_bulk();
 
 void residual_restrict(const LevelGeom& g, const float* L, const float* p, const float* b,
-                       float* b_c, float* p_c, int allow_tma, cudaStream_t s) {
-    if (allow_tma && residual_restrict_bulk(g, L, p, b, b_c, p_c, s)) return;
+                       float* b_c, float* p_c, int allow_tma, const UniArgs& uni, cudaStream_t s) {
+    if (allow_tma && residual_restrict_bulk(g, L, p, b, b_c, p_c, uni, s)) return;
     ResArgs a;
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = b_c; a.p_c = p_c;
     a.rb = ReduceBuf{nullptr, nullptr, nullptr};
@@ -542,8 +543,8 @@ void residual_restrict(const LevelGeom& g, const float* L, const float* p, const
 }
 
 void residual_norm2(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
-                    int slot, int allow_tma, cudaStream_t s) {
-    if (allow_tma && residual_norm2_bulk(g, L, p, b, rb, slot, s)) return;
+                    int slot, int allow_tma, const UniArgs& uni, cudaStream_t s) {
+    if (allow_tma && residual_norm2_bulk(g, L, p, b, rb, slot, uni, s)) return;
     ResArgs a;
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = nullptr; a.p_c = nullptr;
     a.rb = rb;

@@ -12,6 +12,7 @@
 // the z pair across two consecutive steps, in stencil.cuh's canonical tree order, so the result is
 // bit-identical to the generic kernel.  112 KB of shared memory per CTA: two CTAs per SM.
 #include "fused_common.cuh"
+#include "uniform.cuh"
 
 namespace gmgf {
 
@@ -42,6 +43,9 @@ struct ResBulkCfg {
     static constexpr uint32_t P_BYTES = (uint32_t)(PH * TX + 2 * PH * 4) * 4u;
     static constexpr uint32_t STEP_BYTES = P_BYTES + (uint32_t)(3 * RY * TX + (RY + 1) * TX) * 4u;
     static constexpr uint32_t PRO_BYTES = 2 * P_BYTES + (uint32_t)(RY * TX) * 4u;
+    // lean path (uniform.cuh): only the p and b streams are copied
+    static constexpr uint32_t STEP_BYTES_UNI = P_BYTES + (uint32_t)(RY * TX) * 4u;
+    static constexpr uint32_t PRO_BYTES_UNI = 2 * P_BYTES;
 };
 
 struct ResBulkArgs {
@@ -56,17 +60,18 @@ struct ResBulkArgs {
     int zchunk;
     int tiles_x, tiles_y;
     const int* run_flag;   // != nullptr: the kernel does nothing unless *run_flag != 0
+    UniArgs uni;           // uniform bricks of the level (uniform.cuh); brick == nullptr: disabled
 };
 
 struct alignas(64) ResBulkMaps {
     CUtensorMap p_main, p_halo, lz, lx, ly, b;
 };
 
-template <int MODE>
-__global__ void __launch_bounds__(ResBulkCfg::THREADS, 2)
-k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
+// UNI: the lean path of uniform.cuh (interior tiles in y only) -- the coefficient streams are
+// neither copied nor read; the same apply7 / diag6 operations run on the level's constants.
+template <int MODE, bool UNI>
+__device__ __forceinline__ void res_body(const ResBulkArgs& a, const ResBulkMaps& maps) {
     using C = ResBulkCfg;
-    if (a.run_flag && *a.run_flag == 0) return;
     extern __shared__ __align__(128) float sm[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..NB) steps, [NB] prologue
     const LevelGeom& g = a.g;
@@ -114,16 +119,16 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
     auto issue_step = [&](int v) {  // p(v+1), Lz(v+1), Lx(v), Ly(v), b(v)
         if (lane_id != 0 || (y_inside && warp_id >= 7)) return;
         uint64_t* bar = bars + ((v - z0) % C::NB);
-        if (tid == 0) mbar_expect_tx(bar, C::STEP_BYTES);
+        if (tid == 0) mbar_expect_tx(bar, UNI ? C::STEP_BYTES_UNI : C::STEP_BYTES);
         const int gz0 = wrap1(v, nz), gz1 = wrap1(v + 1, nz);
         if (y_inside) {
             switch (warp_id) {
                 case 0: tma_load_3d(slotP(v + 1), &maps.p_main, x0, y0 - 1, gz1, bar); break;
                 case 1: tma_load_3d(slotP(v + 1) + C::P_HL, &maps.p_halo, xL, y0 - 1, gz1, bar); break;
                 case 2: tma_load_3d(slotP(v + 1) + C::P_HR, &maps.p_halo, xR, y0 - 1, gz1, bar); break;
-                case 3: tma_load_3d(slotLz(v + 1), &maps.lz, x0, y0, gz1, bar); break;
-                case 4: tma_load_3d(slotLx(v), &maps.lx, x0, y0, gz0, bar); break;
-                case 5: tma_load_3d(slotLy(v), &maps.ly, x0, y0, gz0, bar); break;
+                case 3: if (!UNI) tma_load_3d(slotLz(v + 1), &maps.lz, x0, y0, gz1, bar); break;
+                case 4: if (!UNI) tma_load_3d(slotLx(v), &maps.lx, x0, y0, gz0, bar); break;
+                case 5: if (!UNI) tma_load_3d(slotLy(v), &maps.ly, x0, y0, gz0, bar); break;
                 case 6: tma_load_3d(slotB(v), &maps.b, x0, y0, gz0, bar); break;
                 default: break;
             }
@@ -146,7 +151,7 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
     {
         uint64_t* bar = bars + C::NB;
         if (lane_id == 0) {
-            if (tid == 0) mbar_expect_tx(bar, C::PRO_BYTES);
+            if (tid == 0) mbar_expect_tx(bar, UNI ? C::PRO_BYTES_UNI : C::PRO_BYTES);
             const int ga = wrap1(z0 - 1, nz), gb = wrap1(z0, nz);
             if (y_inside) {
                 switch (warp_id) {
@@ -156,7 +161,7 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
                     case 3: tma_load_3d(slotP(z0), &maps.p_main, x0, y0 - 1, gb, bar); break;
                     case 4: tma_load_3d(slotP(z0) + C::P_HL, &maps.p_halo, xL, y0 - 1, gb, bar); break;
                     case 5: tma_load_3d(slotP(z0) + C::P_HR, &maps.p_halo, xR, y0 - 1, gb, bar); break;
-                    case 6: tma_load_3d(slotLz(z0), &maps.lz, x0, y0, gb, bar); break;
+                    case 6: if (!UNI) tma_load_3d(slotLz(z0), &maps.lz, x0, y0, gb, bar); break;
                     default: break;
                 }
             } else {
@@ -179,7 +184,7 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
     const int gxh = wrapi(xl + 4, nx);
     const bool zx_lo = g.bc[0] && xl == 0, zx_hi = g.bc[0] && gxh == 0;
     const bool zyA = g.bc[1] && gyA == 0, zyB = g.bc[1] && gyB == 0, zyC = g.bc[1] && gyC == 0;
-    const bool any_wall = zx_lo || zx_hi || zyA || zyB || zyC || g.bc[2];
+    const bool any_wall = !UNI && (zx_lo || zx_hi || zyA || zyB || zyC || g.bc[2]);
     const bool last_lane = (lx == 31);
     const int p_off = (rA + 1) * C::TX + 4 * lx;    // row A in a p plane (row B: +TX)
     const int h_off = (lx == 0 ? C::P_HL + 3 : C::P_HR) + (rA + 1) * 4;
@@ -201,10 +206,13 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
     uint32_t kpar = 0;
     int gz = z0;
     float lxhA_pf = 0.0f, lxhB_pf = 0.0f;
-    if (last_lane) {
+    if (!UNI && last_lane) {
         lxhA_pf = __ldg(lxhA_row + (size_t)gz * plane);
         lxhB_pf = __ldg(lxhB_row + (size_t)gz * plane);
     }
+    const float4 ux4 = make_float4(a.uni.ux, a.uni.ux, a.uni.ux, a.uni.ux);
+    const float4 uy4 = make_float4(a.uni.uy, a.uni.uy, a.uni.uy, a.uni.uy);
+    const float4 uz4 = make_float4(a.uni.uz, a.uni.uz, a.uni.uz, a.uni.uz);
     double acc = 0.0, acc_b = 0.0;                  // MODE 1, 2: sum r^2 (and sum b^2 over active cells)
     float zacc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};  // MODE 0: even-plane partial sums
 
@@ -226,19 +234,26 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
         const float* X = sm + C::OFF_LX + ic * C::C_PLANE + c_off;
         const float* Y = sm + C::OFF_LY + ic * C::Y_PLANE + c_off;
         const float* Bq = sm + C::OFF_B + ic * C::C_PLANE + c_off;
-        float4 lxA = lds4(X), lxB = lds4(X + C::TX);
-        float4 lyA = lds4(Y), lyB = lds4(Y + C::TX), lyC = lds4(Y + 2 * C::TX);
-        float4 lzA = lds4(Z0 + c_off), lzB = lds4(Z0 + c_off + C::TX);
-        float4 lzhA = lds4(Z1 + c_off), lzhB = lds4(Z1 + c_off + C::TX);
-        const float4 bA = lds4(Bq), bB = lds4(Bq + C::TX);
-        const float tA = __shfl_down_sync(0xffffffffu, lxA.x, 1);
-        const float tB = __shfl_down_sync(0xffffffffu, lxB.x, 1);
-        float lxhA = last_lane ? lxhA_pf : tA;
-        float lxhB = last_lane ? lxhB_pf : tB;
-        if (last_lane && v + 1 < z1) {
-            lxhA_pf = __ldg(lxhA_row + (size_t)gzp * plane);
-            lxhB_pf = __ldg(lxhB_row + (size_t)gzp * plane);
+        float4 lxA, lxB, lyA, lyB, lyC, lzA, lzB, lzhA, lzhB;
+        float lxhA, lxhB;
+        if (UNI) {
+            lxA = lxB = ux4; lyA = lyB = lyC = uy4; lzA = lzB = lzhA = lzhB = uz4;
+            lxhA = lxhB = a.uni.ux;
+        } else {
+            lxA = lds4(X); lxB = lds4(X + C::TX);
+            lyA = lds4(Y); lyB = lds4(Y + C::TX); lyC = lds4(Y + 2 * C::TX);
+            lzA = lds4(Z0 + c_off); lzB = lds4(Z0 + c_off + C::TX);
+            lzhA = lds4(Z1 + c_off); lzhB = lds4(Z1 + c_off + C::TX);
+            const float tA = __shfl_down_sync(0xffffffffu, lxA.x, 1);
+            const float tB = __shfl_down_sync(0xffffffffu, lxB.x, 1);
+            lxhA = last_lane ? lxhA_pf : tA;
+            lxhB = last_lane ? lxhB_pf : tB;
+            if (last_lane && v + 1 < z1) {
+                lxhA_pf = __ldg(lxhA_row + (size_t)gzp * plane);
+                lxhB_pf = __ldg(lxhB_row + (size_t)gzp * plane);
+            }
         }
+        const float4 bA = lds4(Bq), bB = lds4(Bq + C::TX);
         if (any_wall) {
             if (zx_lo) { lxA.x = 0.0f; lxB.x = 0.0f; }
             if (zx_hi) { lxhA = 0.0f; lxhB = 0.0f; }
@@ -365,6 +380,28 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
     if (MODE == 2) finish_reduction(acc, acc_b, true, a.rb, a.slot, a.slot2);
 }
 
+template <int MODE>
+__global__ void __launch_bounds__(ResBulkCfg::THREADS, 2)
+k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
+    using C = ResBulkCfg;
+    if (a.run_flag && *a.run_flag == 0) return;
+    // lean path (uniform.cuh)?  Tile + ring 1, planes z0-1 .. z1; box-fed (interior in y) tiles only
+    bool uni = false;
+    if (a.uni.brick) {
+        int bid = blockIdx.x;
+        const int tx = bid % a.tiles_x;
+        bid /= a.tiles_x;
+        const int ty = bid % a.tiles_y;
+        const int zc = bid / a.tiles_y;
+        const int x0 = tx * C::TX, y0 = ty * C::RY, z0 = zc * a.zchunk, z1 = min(a.g.n[2], z0 + a.zchunk);
+        if ((y0 >= 1) && (y0 + C::RY + 1 <= a.g.n[1]))
+            uni = ub_box_uniform_warp(a.g, a.uni.brick, x0 - 2, x0 + C::TX + 1, y0 - 2, y0 + C::RY + 1, z0 - 2, z1 + 1,
+                                      threadIdx.x & 31);
+    }
+    if (uni) res_body<MODE, true>(a, maps);
+    else res_body<MODE, false>(a, maps);
+}
+
 // ---- launchers ------------------------------------------------------------------------------
 static bool res_maps(const LevelGeom& g, const float* L, const float* p, const float* b, ResBulkMaps* m) {
     using C = ResBulkCfg;
@@ -372,6 +409,24 @@ static bool res_maps(const LevelGeom& g, const float* L, const float* p, const f
     return tensor_map(p, g, C::TX, C::PH, &m->p_main) && tensor_map(p, g, 4, C::PH, &m->p_halo) &&
            tensor_map(L + 2 * N, g, C::TX, C::RY, &m->lz) && tensor_map(L, g, C::TX, C::RY, &m->lx) &&
            tensor_map(L + N, g, C::TX, C::RY + 1, &m->ly) && tensor_map(b, g, C::TX, C::RY, &m->b);
+}
+
+// Fraction of the level's cells whose residual CTA takes the lean path (see bulk_sweep_uniform_fraction)
+double res_bulk_uniform_fraction(const LevelGeom& g, const unsigned char* brick_host) {
+    using C = ResBulkCfg;
+    if (!bulk_supported(g) || (g.n[2] & 1)) return 0.0;
+    const int tiles_x = g.n[0] / C::TX, tiles_y = (g.n[1] + C::RY - 1) / C::RY;
+    const int zchunk = choose_zchunk((long long)tiles_x * tiles_y, g.n[2], kZChunkPref, kZChunkMin, 296, 1);
+    double cells = 0.0;
+    for (int z0 = 0; z0 < g.n[2]; z0 += zchunk)
+        for (int ty = 0; ty < tiles_y; ++ty)
+            for (int tx = 0; tx < tiles_x; ++tx) {
+                const int x0 = tx * C::TX, y0 = ty * C::RY, z1 = z0 + zchunk < g.n[2] ? z0 + zchunk : g.n[2];
+                if (!((y0 >= 1) && (y0 + C::RY + 1 <= g.n[1]))) continue;
+                if (!ub_box_uniform(g, brick_host, x0 - 2, x0 + C::TX + 1, y0 - 2, y0 + C::RY + 1, z0 - 2, z1 + 1)) continue;
+                cells += (double)C::TX * C::RY * (z1 - z0);
+            }
+    return cells / (double)g.N;
 }
 
 template <int MODE>
@@ -396,8 +451,9 @@ static bool launch_res_bulk(ResBulkArgs& a, cudaStream_t s) {
 }
 
 bool residual_restrict_bulk(const LevelGeom& g, const float* L, const float* p, const float* b, float* b_c,
-                            float* p_c, cudaStream_t s) {
+                            float* p_c, const UniArgs& uni, cudaStream_t s) {
     ResBulkArgs a;
+    a.uni = uni;
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = b_c; a.p_c = p_c;
     a.rb = ReduceBuf{nullptr, nullptr, nullptr};
     a.slot = 0;
@@ -407,8 +463,9 @@ bool residual_restrict_bulk(const LevelGeom& g, const float* L, const float* p, 
 }
 
 bool residual_norm2_bulk(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
-                         int slot, cudaStream_t s) {
+                         int slot, const UniArgs& uni, cudaStream_t s) {
     ResBulkArgs a;
+    a.uni = uni;
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = nullptr; a.p_c = nullptr;
     a.rb = rb;
     a.slot = slot;
@@ -419,8 +476,9 @@ bool residual_norm2_bulk(const LevelGeom& g, const float* L, const float* p, con
 
 // the same pass as a no-op unless *run_flag != 0 (fused_norm: the cycle expected to be the last)
 bool residual_norm2_bulk_if(const LevelGeom& g, const float* L, const float* p, const float* b, ReduceBuf rb,
-                            int slot, const int* run_flag, cudaStream_t s) {
+                            int slot, const int* run_flag, const UniArgs& uni, cudaStream_t s) {
     ResBulkArgs a;
+    a.uni = uni;
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = nullptr; a.p_c = nullptr;
     a.rb = rb;
     a.slot = slot;
@@ -434,8 +492,9 @@ bool residual_norm_bulk_supported(const LevelGeom& g) {
 
 // sum r^2 -> red[slot_rr] and sum b^2 over active cells -> red[slot_ref] in ONE pass (loop entry)
 bool residual_and_ref_norm2_bulk(const LevelGeom& g, const float* L, const float* p, const float* b,
-                                 ReduceBuf rb, int slot_rr, int slot_ref, cudaStream_t s) {
+                                 ReduceBuf rb, int slot_rr, int slot_ref, const UniArgs& uni, cudaStream_t s) {
     ResBulkArgs a;
+    a.uni = uni;
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = nullptr; a.p_c = nullptr;
     a.rb = rb;
     a.slot = slot_rr;
@@ -447,8 +506,9 @@ bool residual_and_ref_norm2_bulk(const LevelGeom& g, const float* L, const float
 // q = A d and red[slot] = d.q in one TMA-fed pass (the CG mat-vec, reading O10); the b stream of
 // the kernel is pointed at d and ignored.
 bool matvec_dot_bulk(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot,
-                     cudaStream_t s) {
+                     const UniArgs& uni, cudaStream_t s) {
     ResBulkArgs a;
+    a.uni = uni;
     a.g = g; a.L = L; a.p = d; a.b = d; a.b_c = q; a.p_c = nullptr;
     a.rb = rb;
     a.slot = slot;

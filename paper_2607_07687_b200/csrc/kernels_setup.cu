@@ -8,6 +8,7 @@
 // Same per-value arithmetic and summation order as the one-thread-per-value kernels in
 // kernels_generic.cu, so the two paths are bit-identical (tests compare them).
 #include "stencil.cuh"
+#include "uniform.cuh"
 
 namespace gmgk {
 using namespace gmgd;
@@ -209,6 +210,46 @@ k_project4(LevelGeom g, const float* __restrict__ L, const float* __restrict__ p
 void project4(const LevelGeom& g, const float* L, const float* p, float* u, cudaStream_t s) {
     const long long items = g.N >> 2;
     k_project4<<<(unsigned int)((items + kST - 1) / kST), kST, 0, s>>>(g, L, p, u);
+}
+
+// ---- uniform bricks (uniform.cuh): one block per brick of kUBX x kUBY x kUBZ cells; flag = every
+// stored Lx, Ly, Lz value of the brick equals the level's constant of its direction.  nx % 128 == 0
+// (only levels that run the TMA-fed kernels are marked).  count[0] += 1 per uniform brick.
+__global__ void __launch_bounds__(256)
+k_uniform_bricks(LevelGeom g, const float* __restrict__ L, float ux, float uy, float uz,
+                 unsigned char* __restrict__ flag, unsigned int* __restrict__ count) {
+    using namespace gmgf;
+    const int nbx = ub_count(g.n[0], kUBX), nby = ub_count(g.n[1], kUBY);
+    int b = blockIdx.x;
+    const int bx = b % nbx;
+    b /= nbx;
+    const int by = b % nby, bz = b / nby;
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const long long N = g.N;
+    bool ok = true;
+    // kUBY * kUBZ rows of kUBX / 4 float4 groups per array
+    constexpr int GPR = kUBX / 4;
+    for (int t = threadIdx.x; t < GPR * kUBY * kUBZ; t += 256) {
+        const int gx = t % GPR, r = t / GPR;
+        const int y = by * kUBY + r % kUBY, z = bz * kUBZ + r / kUBY;
+        if (y >= ny || z >= nz) continue;
+        const long long o = (long long)bx * kUBX + 4 * gx + (long long)nx * (y + (long long)ny * z);
+        const float4 a = ld4(L + o), c = ld4(L + N + o), d = ld4(L + 2 * N + o);
+        ok = ok && a.x == ux && a.y == ux && a.z == ux && a.w == ux && c.x == uy && c.y == uy && c.z == uy &&
+             c.w == uy && d.x == uz && d.y == uz && d.z == uz && d.w == uz;
+    }
+    const int all = __syncthreads_and(ok ? 1 : 0);
+    if (threadIdx.x == 0) {
+        flag[blockIdx.x] = all ? 1 : 0;
+        if (all) atomicAdd(count, 1u);
+    }
+}
+
+void uniform_bricks(const LevelGeom& g, const float* L, float ux, float uy, float uz, unsigned char* flag,
+                    unsigned int* count, cudaStream_t s) {
+    using namespace gmgf;
+    const unsigned int nb = (unsigned int)(ub_count(g.n[0], kUBX) * ub_count(g.n[1], kUBY) * ub_count(g.n[2], kUBZ));
+    k_uniform_bricks<<<nb, 256, 0, s>>>(g, L, ux, uy, uz, flag, count);
 }
 
 }  // namespace gmgk

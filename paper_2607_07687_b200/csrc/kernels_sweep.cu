@@ -27,6 +27,7 @@
 #include <tuple>
 
 #include "fused_common.cuh"
+#include "uniform.cuh"
 
 namespace gmgf {
 template <int TY_, int PD_>
@@ -61,6 +62,9 @@ struct BulkCfg {
     static constexpr uint32_t STEP_BYTES =
         (uint32_t)(SH * TX + 2 * SH * 4 + 3 * ROWS * TX + (ROWS + 1) * TX) * 4u;
     static constexpr uint32_t PRO_BYTES = (uint32_t)(2 * (SH * TX + 2 * SH * 4) + ROWS * TX) * 4u;
+    // lean path (uniform.cuh): only the p and b streams are copied
+    static constexpr uint32_t STEP_BYTES_UNI = (uint32_t)(SH * TX + 2 * SH * 4 + ROWS * TX) * 4u;
+    static constexpr uint32_t PRO_BYTES_UNI = (uint32_t)(2 * (SH * TX + 2 * SH * 4)) * 4u;
     static_assert(2 * ROWS <= 32 && NB <= 8 && THREADS / 32 >= 7, "tile shape");
     static_assert(SMEM <= 227 * 1024, "shared memory");
 };
@@ -80,6 +84,7 @@ struct BulkArgs {
     ReduceBuf rb;
     int slot_rr, slot_ref;
     const int* run_flag;   // != nullptr: the kernel does nothing unless *run_flag != 0
+    UniArgs uni;           // uniform bricks of the level (uniform.cuh); brick == nullptr: disabled
 };
 
 struct alignas(64) MapSet {
@@ -153,7 +158,11 @@ __device__ __forceinline__ float4 update_pair_full(float xm, float4 own, float x
 // (was) YIN: the tile's TMA boxes stay inside the domain in y (every tile but the first and last
 // tile rows); the other instantiation carries the row-copy path, so the common one stays small.
 // NORM: 0 = plain sweep; 1 = also sum r^2 of the source iterate; 2 = also sum b^2 over active cells
-template <class C, int YMODE, int NORM>
+// UNI: the lean path of uniform.cuh -- every coefficient this CTA would read equals the level's
+// constant of its direction and no wall is near: the Lz / Lx / Ly streams are neither copied nor
+// read, the SAME apply7 / diag6 / relax operations run on the constants (bit-identical results;
+// diag6 and the reciprocal are loop-invariant, every cell is active).
+template <class C, int YMODE, int NORM, bool UNI = false>
 __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& allmaps) {
     extern __shared__ __align__(1024) float sm[];  // no static shared memory: base is 1 KB aligned
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..NB) step groups, [NB] prologue
@@ -198,8 +207,11 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
     const uint32_t e_pbytes = (uint32_t)((y_first ? C::SH : hP + 2) * (C::TX + 8)) * 4u;
     const uint32_t e_cbytes = (uint32_t)((y_first ? C::ROWS : hC + 1) * C::TX) * 4u;
     const uint32_t e_lybytes = (uint32_t)((y_first ? C::ROWS + 1 : hC + 2) * C::TX) * 4u;
-    const uint32_t step_bytes = (YMODE == 2) ? e_pbytes + 3u * e_cbytes + e_lybytes : C::STEP_BYTES;
-    const uint32_t pro_bytes = (YMODE == 2) ? 2u * e_pbytes + e_cbytes : C::PRO_BYTES;
+    const uint32_t step_bytes = UNI ? ((YMODE == 2) ? e_pbytes + e_cbytes : C::STEP_BYTES_UNI)
+                                    : ((YMODE == 2) ? e_pbytes + 3u * e_cbytes + e_lybytes : C::STEP_BYTES);
+    const uint32_t pro_bytes = UNI ? ((YMODE == 2) ? 2u * e_pbytes : C::PRO_BYTES_UNI)
+                                   : ((YMODE == 2) ? 2u * e_pbytes + e_cbytes : C::PRO_BYTES);
+    static_assert(!UNI || YMODE != 1, "the lean path is built for box-fed tiles only");
     const float* Lx = a.L;
     const float* Ly = a.L + N;
     const float* Lz = a.L + 2 * N;
@@ -256,9 +268,9 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                 case 0: tma_load_3d(slotP(vp), &maps.p_main, x0, y0 - 2, gzv, bar); break;
                 case 1: tma_load_3d(slotP(vp) + C::P_HL, &maps.p_halo, xL, y0 - 2, gzv, bar); break;
                 case 2: tma_load_3d(slotP(vp) + C::P_HR, &maps.p_halo, xR, y0 - 2, gzv, bar); break;
-                case 3: tma_load_3d(slotLz(v + 1), &maps.lz, x0, y0 - 1, gz1, bar); break;
-                case 4: tma_load_3d(slotLx(v), &maps.lx, x0, y0 - 1, gz0, bar); break;
-                case 5: tma_load_3d(slotLy(v), &maps.ly, x0, y0 - 1, gz0, bar); break;
+                case 3: if (!UNI) tma_load_3d(slotLz(v + 1), &maps.lz, x0, y0 - 1, gz1, bar); break;
+                case 4: if (!UNI) tma_load_3d(slotLx(v), &maps.lx, x0, y0 - 1, gz0, bar); break;
+                case 5: if (!UNI) tma_load_3d(slotLy(v), &maps.ly, x0, y0 - 1, gz0, bar); break;
                 case 6: tma_load_3d(slotB(v), &maps.b, x0, y0 - 1, gz0, bar); break;
                 default: break;
             }
@@ -268,9 +280,9 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                 case 0: tma_load_3d(slotP(vp) + e_oP * C::TX, &maps.p_main, x0, e_yP, gzv, bar); break;
                 case 1: tma_load_3d(slotP(vp) + C::P_HL + hs + e_oP * 4, &maps.p_halo, xL, e_yP, gzv, bar); break;
                 case 2: tma_load_3d(slotP(vp) + C::P_HR + hs + e_oP * 4, &maps.p_halo, xR, e_yP, gzv, bar); break;
-                case 3: tma_load_3d(slotLz(v + 1) + e_oC * C::TX, &maps.lz, x0, e_yC, gz1, bar); break;
-                case 4: tma_load_3d(slotLx(v) + e_oC * C::TX, &maps.lx, x0, e_yC, gz0, bar); break;
-                case 5: tma_load_3d(slotLy(v) + e_oC * C::TX, &maps.ly, x0, e_yC, gz0, bar); break;
+                case 3: if (!UNI) tma_load_3d(slotLz(v + 1) + e_oC * C::TX, &maps.lz, x0, e_yC, gz1, bar); break;
+                case 4: if (!UNI) tma_load_3d(slotLx(v) + e_oC * C::TX, &maps.lx, x0, e_yC, gz0, bar); break;
+                case 5: if (!UNI) tma_load_3d(slotLy(v) + e_oC * C::TX, &maps.ly, x0, e_yC, gz0, bar); break;
                 case 6: tma_load_3d(slotB(v) + e_oC * C::TX, &maps.b, x0, e_yC, gz0, bar); break;
                 case 7: case 8: {   // the two wrapped p rows
                     const int r = warp_id - 7, j = e_pj0 + r;
@@ -280,9 +292,10 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                     bulk_g2s(d + C::P_HL + hs + j * 4, rb + xL, 16u, bar);
                     bulk_g2s(d + C::P_HR + hs + j * 4, rb + xR, 16u, bar);
                 } break;
-                case 9: bulk_g2s(slotLz(v + 1) + e_cj * C::TX, Lz + pz1 + (size_t)e_cy * nx + x0, C::TX * 4u, bar); break;
-                case 10: bulk_g2s(slotLx(v) + e_cj * C::TX, Lx + pz0 + (size_t)e_cy * nx + x0, C::TX * 4u, bar); break;
+                case 9: if (!UNI) bulk_g2s(slotLz(v + 1) + e_cj * C::TX, Lz + pz1 + (size_t)e_cy * nx + x0, C::TX * 4u, bar); break;
+                case 10: if (!UNI) bulk_g2s(slotLx(v) + e_cj * C::TX, Lx + pz0 + (size_t)e_cy * nx + x0, C::TX * 4u, bar); break;
                 case 11:
+                    if (UNI) break;
                     bulk_g2s(slotLy(v) + e_cj * C::TX, Ly + pz0 + (size_t)e_cy * nx + x0, C::TX * 4u, bar);
                     if (e_ly2) bulk_g2s(slotLy(v) + (e_cj + 1) * C::TX, Ly + pz0 + (size_t)(e_cy + 1) * nx + x0, C::TX * 4u, bar);
                     break;
@@ -319,7 +332,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                     else if (k == 1) tma_load_3d(slotP(v) + C::P_HL, &maps.p_halo, xL, y0 - 2, gv, bar);
                     else tma_load_3d(slotP(v) + C::P_HR, &maps.p_halo, xR, y0 - 2, gv, bar);
                 } else if (warp_id == 6) {
-                    tma_load_3d(slotLz(z0 - 1), &maps.lz, x0, y0 - 1, gb, bar);
+                    if (!UNI) tma_load_3d(slotLz(z0 - 1), &maps.lz, x0, y0 - 1, gb, bar);
                 }
             } else if (YMODE == 2) {
                 const int pl = warp_id / 3, k = warp_id % 3;
@@ -329,7 +342,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                     else if (k == 1) tma_load_3d(slotP(v) + C::P_HL + hs + e_oP * 4, &maps.p_halo, xL, e_yP, gv, bar);
                     else tma_load_3d(slotP(v) + C::P_HR + hs + e_oP * 4, &maps.p_halo, xR, e_yP, gv, bar);
                 } else if (warp_id == 6) {
-                    tma_load_3d(slotLz(z0 - 1) + e_oC * C::TX, &maps.lz, x0, e_yC, gb, bar);
+                    if (!UNI) tma_load_3d(slotLz(z0 - 1) + e_oC * C::TX, &maps.lz, x0, e_yC, gb, bar);
                 } else if (warp_id >= 7 && warp_id <= 10) {      // wrapped p rows of the two planes
                     const int v = z0 - 2 + (warp_id - 7) / 2, r = (warp_id - 7) & 1, j = e_pj0 + r;
                     const float* rb = a.src + (size_t)wrapi(v, nz) * plane + (size_t)(e_py0 + r) * nx;
@@ -338,7 +351,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                     bulk_g2s(d + C::P_HL + hs + j * 4, rb + xL, 16u, bar);
                     bulk_g2s(d + C::P_HR + hs + j * 4, rb + xR, 16u, bar);
                 } else if (warp_id == 11) {
-                    bulk_g2s(slotLz(z0 - 1) + e_cj * C::TX, Lz + (size_t)gb * plane + (size_t)e_cy * nx + x0, C::TX * 4u, bar);
+                    if (!UNI) bulk_g2s(slotLz(z0 - 1) + e_cj * C::TX, Lz + (size_t)gb * plane + (size_t)e_cy * nx + x0, C::TX * 4u, bar);
                 }
             } else {
                 for (int pl = 0; pl < 2; ++pl) copy_p_rows(z0 - 2 + pl, bar);
@@ -393,8 +406,8 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
         // cells (sel, sel+2) of the group are updated: same parity for B(u) and C(u-1); sel is
         // warp-uniform and alternates every step
         int sel = (yl + (z0 - 1) + fc) & 1;
-        float lxh_pf = last_lane ? __ldg(lxh_row + (size_t)gz * plane) : 0.0f;
-        const bool any_wall = zx_lo || zx_hi || zy_lo || zy_hi || g.bc[2];
+        float lxh_pf = (!UNI && last_lane) ? __ldg(lxh_row + (size_t)gz * plane) : 0.0f;
+        const bool any_wall = !UNI && (zx_lo || zx_hi || zy_lo || zy_hi || g.bc[2]);
         // K = the coefficients of the two cells C updates next step, picked out of this step's
         // set (14 floats, not a second full set); q1 / z2 = planes u-1 / u-2 at the own position
         CPair K;
@@ -406,6 +419,12 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
         // the B-updated ones there), and this thread's partial sums
         float zs_a = 0.0f, zs_b = 0.0f, acc_rr = 0.0f, acc_bb = 0.0f;
         CFull Sc;
+        if (UNI) {   // the level's constants; only Sc.b changes from step to step
+            Sc.lx = make_float4(a.uni.ux, a.uni.ux, a.uni.ux, a.uni.ux);
+            Sc.lxh = a.uni.ux;
+            Sc.ly = Sc.lyh = make_float4(a.uni.uy, a.uni.uy, a.uni.uy, a.uni.uy);
+            Sc.lz = Sc.lzh = make_float4(a.uni.uz, a.uni.uz, a.uni.uz, a.uni.uz);
+        }
         float4 own, ym, yp, zp;
         float hvB;
         // Operands of B(u) -- TMA data and source values no other thread changes.  Loaded at the
@@ -413,12 +432,14 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
         // are still to be read, so the 16 warps do not all queue on the shared-memory pipe at once.
         auto load_step = [&]() {
             mbar_wait(bars + kb, kpar);
-            Sc.lx = lds4(sm + C::OFF_LX + ic * C::C_PLANE + c_off);
-            const float* Y = sm + C::OFF_LY + ic * C::Y_PLANE + c_off;
-            Sc.ly = lds4(Y);
-            Sc.lyh = lds4(Y + C::TX);
-            Sc.lz = lds4(Z0 + c_off);
-            Sc.lzh = lds4(Z1 + c_off);
+            if (!UNI) {
+                Sc.lx = lds4(sm + C::OFF_LX + ic * C::C_PLANE + c_off);
+                const float* Y = sm + C::OFF_LY + ic * C::Y_PLANE + c_off;
+                Sc.ly = lds4(Y);
+                Sc.lyh = lds4(Y + C::TX);
+                Sc.lz = lds4(Z0 + c_off);
+                Sc.lzh = lds4(Z1 + c_off);
+            }
             Sc.b = lds4(sm + C::OFF_B + ic * C::C_PLANE + c_off);
             own = lds4(P0 + p_off);
             ym = lds4(P0 + p_off - C::TX);
@@ -432,9 +453,11 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
             const float4 cym = lds4(Pm1 + p_off - C::TX);   // plane u-1, B-updated rows above / below
             const float4 cyp = lds4(Pm1 + p_off + C::TX);
             const float hvC = Pm1[h_off];
-            const float t = __shfl_down_sync(0xffffffffu, Sc.lx.x, 1);
-            Sc.lxh = last_lane ? lxh_pf : t;
-            if (last_lane && u + 1 <= z1) lxh_pf = __ldg(lxh_row + (size_t)gzp * plane);
+            if (!UNI) {
+                const float t = __shfl_down_sync(0xffffffffu, Sc.lx.x, 1);
+                Sc.lxh = last_lane ? lxh_pf : t;
+                if (last_lane && u + 1 <= z1) lxh_pf = __ldg(lxh_row + (size_t)gzp * plane);
+            }
             if (any_wall) {   // Neumann wall faces carry coefficient 0 (reading O2)
                 if (zx_lo) Sc.lx.x = 0.0f;
                 if (zx_hi) Sc.lxh = 0.0f;
@@ -470,11 +493,14 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                 if (row_c && u >= z0 && u < z1) {
                     const float r0 = a0 ? Sc.b.x - A0 : 0.0f, r1 = a1 ? Sc.b.y - A1 : 0.0f;
                     const float r2 = a2 ? Sc.b.z - A2 : 0.0f, r3 = a3 ? Sc.b.w - A3 : 0.0f;
-                    acc_rr += (r0 * r0 + r1 * r1) + (r2 * r2 + r3 * r3);
+                    // explicit roundings (no FMA contraction): general and lean path add the same bits
+                    acc_rr = __fadd_rn(acc_rr, __fadd_rn(__fadd_rn(__fmul_rn(r0, r0), __fmul_rn(r1, r1)),
+                                                         __fadd_rn(__fmul_rn(r2, r2), __fmul_rn(r3, r3))));
                     if (NORM == 2) {
                         const float b0 = a0 ? Sc.b.x : 0.0f, b1 = a1 ? Sc.b.y : 0.0f;
                         const float b2 = a2 ? Sc.b.z : 0.0f, b3 = a3 ? Sc.b.w : 0.0f;
-                        acc_bb += (b0 * b0 + b1 * b1) + (b2 * b2 + b3 * b3);
+                        acc_bb = __fadd_rn(acc_bb, __fadd_rn(__fadd_rn(__fmul_rn(b0, b0), __fmul_rn(b1, b1)),
+                                                             __fadd_rn(__fmul_rn(b2, b2), __fmul_rn(b3, b3))));
                     }
                 }
                 zs_a = sel ? own.y : own.x;
@@ -523,6 +549,11 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
         auto fetch_e = [&](int gzc, ESet& s) {  // global loads, issued one step ahead
             const int gzn = (gzc + 1 == nz) ? 0 : gzc + 1;
             const size_t pz = (size_t)gzc * plane, pzp = (size_t)gzn * plane;
+            if (UNI) {
+                s.wxl = s.wxh = a.uni.ux; s.wyl = s.wyh = a.uni.uy; s.wzl = s.wzh = a.uni.uz;
+                s.b = __ldg(a.b + pz + o_c);
+                return;
+            }
             s.wxl = ex_lo ? 0.0f : __ldg(Lx + pz + o_c);
             s.wxh = ex_hi ? 0.0f : __ldg(Lx + pz + o_x1);
             s.wyl = ey_lo ? 0.0f : __ldg(Ly + pz + o_c);
@@ -614,14 +645,31 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     const int y0 = ty * C::TY;
     const int ny = a.g.n[1];
     const bool inside = (y0 >= 2) && (y0 + C::TY + 2 <= ny);
+    // Lean path (uniform.cuh)?  Every warp evaluates the same few brick flags (CTA-uniform verdict):
+    // all coefficients the CTA would touch -- tile + ring 2, planes z0-2 .. z1+1 -- are the level's
+    // constants and no Neumann wall is in reach.
+    bool uni = false;
+    if (a.uni.brick) {
+        int bid = blockIdx.x;
+        const int tx = bid % a.tiles_x;
+        const int zc = bid / (a.tiles_x * a.tiles_y);
+        const int x0 = tx * C::TX, z0 = zc * a.zchunk, z1 = min(a.g.n[2], z0 + a.zchunk);
+        uni = ub_box_uniform_warp(a.g, a.uni.brick, x0 - 2, x0 + C::TX + 1, y0 - 2, y0 + C::TY + 2, z0 - 2, z1 + 1,
+                                  threadIdx.x & 31);
+    }
     if (EDGE) {
-        if (a.g.bc[1] != 0 || inside) sweep_body<C, 0, NORM>(a, maps);
-        else if (a.tiles_y >= 2 && ((ty == 0 && C::TY + 2 <= ny) || (ty == a.tiles_y - 1 && y0 >= 2)))
-            sweep_body<C, 2, NORM>(a, maps);
-        else sweep_body<C, 1, NORM>(a, maps);
+        if (a.g.bc[1] != 0 || inside) {
+            if (uni) sweep_body<C, 0, NORM, true>(a, maps);
+            else sweep_body<C, 0, NORM>(a, maps);
+        } else if (a.tiles_y >= 2 && ((ty == 0 && C::TY + 2 <= ny) || (ty == a.tiles_y - 1 && y0 >= 2))) {
+            if (uni) sweep_body<C, 2, NORM, true>(a, maps);
+            else sweep_body<C, 2, NORM>(a, maps);
+        } else sweep_body<C, 1, NORM>(a, maps);
     } else {
-        if (inside) sweep_body<C, 0, NORM>(a, maps);
-        else sweep_body<C, 1, NORM>(a, maps);
+        if (inside) {
+            if (uni) sweep_body<C, 0, NORM, true>(a, maps);
+            else sweep_body<C, 0, NORM>(a, maps);
+        } else sweep_body<C, 1, NORM>(a, maps);
     }
 }
 
@@ -678,13 +726,39 @@ bool tma_shape_ok(const LevelGeom& g) { return bulk_supported(g); }
 
 static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
                                  const float* omega, int first_colour, const ReduceBuf* norm, int slot_rr,
-                                 int slot_ref, const int* run_flag, cudaStream_t s);
+                                 int slot_ref, const int* run_flag, const UniArgs& uni, cudaStream_t s);
 
+bool bulk_sweep_edge(const LevelGeom& g, bool norm);
 static unsigned int bulk_grid(const LevelGeom& g, int* zchunk_out) {
     const int tiles_x = g.n[0] / Bulk::TX, tiles_y = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
     const int zchunk = choose_zchunk((long long)tiles_x * tiles_y, g.n[2], kZChunkPref, kZChunkMin, 148, 0);
     if (zchunk_out) *zchunk_out = zchunk;
     return (unsigned int)(tiles_x * tiles_y * ((g.n[2] + zchunk - 1) / zchunk));
+}
+
+// Fraction of the level's cells whose CTA takes the lean path (uniform.cuh), from a HOST copy of
+// the brick flags: the same footprint test the kernel applies, for gmg_stats' as-run byte count.
+double bulk_sweep_uniform_fraction(const LevelGeom& g, const unsigned char* brick_host) {
+    if (!bulk_supported(g)) return 0.0;
+    int zchunk = 0;
+    bulk_grid(g, &zchunk);
+    const int tiles_x = g.n[0] / Bulk::TX, tiles_y = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
+    const bool edge = bulk_sweep_edge(g, false);
+    double cells = 0.0;
+    for (int z0 = 0; z0 < g.n[2]; z0 += zchunk)
+        for (int ty = 0; ty < tiles_y; ++ty)
+            for (int tx = 0; tx < tiles_x; ++tx) {
+                const int x0 = tx * Bulk::TX, y0 = ty * Bulk::TY, z1 = z0 + zchunk < g.n[2] ? z0 + zchunk : g.n[2];
+                const bool inside = (y0 >= 2) && (y0 + Bulk::TY + 2 <= g.n[1]);
+                const bool boxfed = inside || (edge && (g.bc[1] != 0 || (tiles_y >= 2 &&
+                                    ((ty == 0 && Bulk::TY + 2 <= g.n[1]) || (ty == tiles_y - 1 && y0 >= 2)))));
+                if (!boxfed) continue;
+                if (!ub_box_uniform(g, brick_host, x0 - 2, x0 + Bulk::TX + 1, y0 - 2, y0 + Bulk::TY + 2, z0 - 2, z1 + 1))
+                    continue;
+                const int rows = (y0 + Bulk::TY <= g.n[1] ? Bulk::TY : g.n[1] - y0);
+                cells += (double)Bulk::TX * rows * (z1 - z0);
+            }
+    return cells / (double)g.N;
 }
 
 // rb_sweep_with_norm will run on this level (shape fits the TMA kernel, one partial per CTA fits)
@@ -693,9 +767,10 @@ bool sweep_norm_supported(const LevelGeom& g) {
 }
 
 void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
-              const float* omega, int first_colour, const float* e_c, int allow_tma, cudaStream_t s) {
+              const float* omega, int first_colour, const float* e_c, int allow_tma, const UniArgs& uni,
+              cudaStream_t s) {
     // the caller applies the prolongation as its own pass in front of the TMA kernel (e_c == nullptr)
-    if (allow_tma && !e_c && rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, nullptr, 0, 0, nullptr, s))
+    if (allow_tma && !e_c && rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, nullptr, 0, 0, nullptr, uni, s))
         return;
     rb_sweep_v2(g, L, src, dst, b, omega, first_colour, e_c, s);
 }
@@ -707,12 +782,12 @@ void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, 
 // false = this level cannot use the TMA kernel (nothing launched).
 bool rb_sweep_with_norm(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
                         const float* omega, int first_colour, ReduceBuf rb, int slot_rr, int slot_ref,
-                        const int* run_flag, cudaStream_t s) {
-    return rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, &rb, slot_rr, slot_ref, run_flag, s);
+                        const int* run_flag, const UniArgs& uni, cudaStream_t s) {
+    return rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, &rb, slot_rr, slot_ref, run_flag, uni, s);
 }
 bool rb_sweep_if(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
-                 const float* omega, int first_colour, const int* run_flag, cudaStream_t s) {
-    return rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, nullptr, 0, 0, run_flag, s);
+                 const float* omega, int first_colour, const int* run_flag, const UniArgs& uni, cudaStream_t s) {
+    return rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, nullptr, 0, 0, run_flag, uni, s);
 }
 
 // Which instantiation of k_rb_sweep_bulk a level gets: true = EDGE (the kernel that carries the
@@ -726,7 +801,7 @@ bool bulk_sweep_edge(const LevelGeom& g, bool norm) {
 
 static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
                                  const float* omega, int first_colour, const ReduceBuf* norm, int slot_rr,
-                                 int slot_ref, const int* run_flag, cudaStream_t s) {
+                                 int slot_ref, const int* run_flag, const UniArgs& uni, cudaStream_t s) {
     BulkMaps maps;
     const size_t N = (size_t)g.N;
     bool ok = tma_shape_ok(g);
@@ -753,6 +828,7 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
     a.rb = norm ? *norm : ReduceBuf{nullptr, nullptr, nullptr};
     a.slot_rr = slot_rr; a.slot_ref = slot_ref;
     a.run_flag = run_flag;
+    a.uni = uni;
     a.tiles_x = g.n[0] / Bulk::TX;
     a.tiles_y = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
     int zchunk = 0;

@@ -34,7 +34,7 @@ class Params(C.Structure):
                 ("omega_up", C.c_float), ("adaptive", C.c_int), ("coarsen_mode", C.c_int),
                 ("n_min", C.c_int), ("fast_path", C.c_int), ("use_graph", C.c_int),
                 ("tma_min_cells", C.c_int), ("cluster_tail", C.c_int),
-                ("fused_norm", C.c_int)]
+                ("fused_norm", C.c_int), ("uniform_tiles", C.c_int)]
 
 
 class Stats(C.Structure):
@@ -42,7 +42,8 @@ class Stats(C.Structure):
                 ("levels", C.c_int), ("omega_final", C.c_double), ("resid_ref", C.c_double),
                 ("resid_init_rel", C.c_double), ("resid_final_rel", C.c_double),
                 ("gpu_ms", C.c_double), ("bytes_algorithmic", C.c_double),
-                ("kernel_launches", C.c_longlong), ("history_len", C.c_int)]
+                ("kernel_launches", C.c_longlong), ("history_len", C.c_int),
+                ("uniform_fraction", C.c_double), ("bytes_as_run", C.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
