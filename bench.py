@@ -458,6 +458,7 @@ def run_ours(args):
                                "GMG-RBGS V(2,2) nu_coarse=32 tol=1e-4 zero initial guess",
                    "cells": N, "levels": final["levels"], "iterations": iters[-1],
                    "resid_final_rel": final["resid_final_rel"],
+                   "uniform_fraction_level0": final["uniform_fraction"],
                    "l2_policy": "inputs larger than L2" if 20 * N > 2 * 126e6 else
                                 "inputs fit in L2 (no flush; DRAM roofline not meaningful)",
                    "parallelism": "replicas only" if world > 1 else "single GPU",

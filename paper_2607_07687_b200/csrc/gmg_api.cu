@@ -31,8 +31,8 @@ bool residual_and_ref_norm2_bulk(const LevelGeom& g, const float* L, const float
 void prolong_add4(const LevelGeom& g, const float* e_c, float* p_f, cudaStream_t s);
 bool matvec_dot_bulk(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot,
                      const UniArgs& uni, cudaStream_t s);
-double bulk_sweep_uniform_fraction(const LevelGeom& g, const unsigned char* brick_host);
-double res_bulk_uniform_fraction(const LevelGeom& g, const unsigned char* brick_host);
+bool bulk_sweep_tiling(const LevelGeom& g, int* tile_y, int* zchunk);
+bool res_bulk_tiling(const LevelGeom& g, int* tile_y, int* zchunk);
 bool tma_shape_ok(const LevelGeom& g);
 bool bulk_sweep_edge(const LevelGeom& g, bool norm);
 // one TMA-fed sweep src -> dst that also leaves sum r^2 (r = b - A src) and sum b^2 over the active
@@ -81,8 +81,9 @@ struct gmg_ctx {
     // uniform bricks (uniform.cuh): levels that run the TMA-fed kernels
     gmgf::UniArgs uni[GMG_MAX_LEVELS];     // brick == nullptr: level not marked
     size_t ubrick_n[GMG_MAX_LEVELS];       // bricks of the level
-    unsigned char* ubrick_dev;             // all levels' flags, one allocation
-    unsigned char* ubrick_host;            // pinned mirror
+    unsigned char* ubrick_dev;             // all levels' flags, one allocation; behind them
+                                           // [2][GMG_MAX_LEVELS] counts of lean-path cells (sweep, residual)
+    unsigned long long* ucount_host;       // pinned mirror of the counts
     size_t ubrick_total;
     double uni_frac_sweep[GMG_MAX_LEVELS]; // cells whose sweep / residual CTA takes the lean path
     double uni_frac_res[GMG_MAX_LEVELS];
@@ -105,6 +106,11 @@ struct gmg_ctx {
     gmg_stats_t stats;
     cudaEvent_t ev0, ev1;
     cudaStream_t cap_a, cap_b;  // internal streams used only for graph capture
+    // forked beside the enqueuing stream (uniform.cuh: lean + general kernels side by side).  Two
+    // sets: while a solve graph is built two captures are open at once (the outer graph and the WHILE
+    // body), and a stream can belong to one capture only.
+    cudaStream_t side[2];
+    cudaEvent_t ev_fork[2], ev_join[2];
     GraphSlot slots[4];
     long long n_launch;   // launch counter of the section being enqueued
     bool enqueue_fail;    // a launcher the plan counted on refused (tensor-map encode failed)
@@ -201,6 +207,7 @@ static void build_levels(gmg_ctx* c) {
             c->uni[l].uy = (float)(C[0] * C[2] / C[1]);
             c->uni[l].uz = (float)(C[0] * C[1] / C[2]);
             c->uni[l].brick = nullptr;
+            c->uni[l].side_stream = c->uni[l].ev_fork = c->uni[l].ev_join = nullptr;
             c->ubrick_n[l] = 0;
             c->uni_frac_sweep[l] = c->uni_frac_res[l] = 0.0;
             for (int d = 0; d < 3; ++d) C[d] *= c->g[l].c[d];
@@ -250,8 +257,9 @@ static size_t carve(gmg_ctx* c, char* base) {
 // Brick flags of the levels that run the TMA-fed kernels: one small library-owned allocation.
 static void free_uniform(gmg_ctx* c) {
     if (c->ubrick_dev) cudaFree(c->ubrick_dev);
-    if (c->ubrick_host) cudaFreeHost(c->ubrick_host);
-    c->ubrick_dev = c->ubrick_host = nullptr;
+    if (c->ucount_host) cudaFreeHost(c->ucount_host);
+    c->ubrick_dev = nullptr;
+    c->ucount_host = nullptr;
     c->ubrick_total = 0;
     for (int l = 0; l < GMG_MAX_LEVELS; ++l) { c->uni[l].brick = nullptr; c->ubrick_n[l] = 0; }
 }
@@ -265,18 +273,31 @@ static cudaError_t alloc_uniform(gmg_ctx* c) {
         if (!(c->fast_sweep[l] && c->tma_ok[l] && gmgf::tma_shape_ok(c->g[l]))) continue;
         c->ubrick_n[l] = (size_t)gmgf::ub_count(c->g[l].n[0], gmgf::kUBX) * gmgf::ub_count(c->g[l].n[1], gmgf::kUBY) *
                          gmgf::ub_count(c->g[l].n[2], gmgf::kUBZ);
-        total += align_up(c->ubrick_n[l], 16);
+        total += align_up(c->ubrick_n[l], 256);
     }
     if (total == 0) return cudaSuccess;
-    // + one counter per level (uniform bricks), behind the flags
-    const size_t bytes = total + sizeof(unsigned int) * GMG_MAX_LEVELS;
-    cudaError_t e = cudaMalloc(&c->ubrick_dev, bytes);
-    if (e == cudaSuccess) e = cudaMallocHost(&c->ubrick_host, bytes);
+    const size_t cbytes = sizeof(unsigned long long) * 2 * GMG_MAX_LEVELS;
+    cudaError_t e = cudaMalloc(&c->ubrick_dev, total + cbytes);
+    if (e == cudaSuccess) e = cudaMallocHost(&c->ucount_host, cbytes);
     if (e != cudaSuccess) { free_uniform(c); return e; }
     c->ubrick_total = total;
     for (int l = 0; l < c->nlev; ++l)
-        if (c->ubrick_n[l]) c->uni[l].brick = c->ubrick_dev + off[l];
+        if (c->ubrick_n[l]) {
+            c->uni[l].brick = c->ubrick_dev + off[l];
+            c->uni[l].side_stream = c->side[0]; c->uni[l].ev_fork = c->ev_fork[0]; c->uni[l].ev_join = c->ev_join[0];
+        }
     return cudaSuccess;
+}
+
+// Which fork set the launchers use from now on: 0 = plain launches and the outer graph, 1 = the
+// WHILE body (captured while the outer capture is still open).
+static void use_side(gmg_ctx* c, int which) {
+    for (int l = 0; l < c->nlev; ++l)
+        if (c->uni[l].brick) {
+            c->uni[l].side_stream = c->side[which];
+            c->uni[l].ev_fork = c->ev_fork[which];
+            c->uni[l].ev_join = c->ev_join[which];
+        }
 }
 
 static void drop_graphs(gmg_ctx* c) {
@@ -318,9 +339,10 @@ extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]
     c->sc = nullptr; c->partials = nullptr; c->counter = nullptr; c->sc_host = nullptr;
     c->ev0 = c->ev1 = nullptr;
     c->cap_a = c->cap_b = nullptr;
+    for (int i = 0; i < 2; ++i) { c->side[i] = nullptr; c->ev_fork[i] = c->ev_join[i] = nullptr; }
     c->cluster_ok = false;
     c->enqueue_fail = false; c->sc_fresh = false;
-    c->ubrick_dev = c->ubrick_host = nullptr; c->ubrick_total = 0; c->uni_stats_pending = false;
+    c->ubrick_dev = nullptr; c->ucount_host = nullptr; c->ubrick_total = 0; c->uni_stats_pending = false;
     if (gmgk::ctail_configure(200 * 1024) == (int)cudaSuccess) c->cluster_ok = gmgk::ctail_launchable(200 * 1024);
     cudaGetLastError();
     build_levels(c);
@@ -334,6 +356,11 @@ extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->cap_a, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->cap_b, cudaStreamNonBlocking);
+    for (int i = 0; i < 2; ++i) {
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->side[i], cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join[i], cudaEventDisableTiming);
+    }
     if (e == cudaSuccess) e = (cudaError_t)gmgk::tail_configure(200 * 1024);
     if (e == cudaSuccess) e = (cudaError_t)gmgf::configure();
     if (e == cudaSuccess) {
@@ -363,6 +390,11 @@ extern "C" void gmg_destroy(gmg_ctx* c) {
     if (c->ev1) cudaEventDestroy(c->ev1);
     if (c->cap_a) cudaStreamDestroy(c->cap_a);
     if (c->cap_b) cudaStreamDestroy(c->cap_b);
+    for (int i = 0; i < 2; ++i) {
+        if (c->side[i]) cudaStreamDestroy(c->side[i]);
+        if (c->ev_fork[i]) cudaEventDestroy(c->ev_fork[i]);
+        if (c->ev_join[i]) cudaEventDestroy(c->ev_join[i]);
+    }
     delete c;
 }
 
@@ -460,39 +492,43 @@ static void set_coeffs_enqueue(gmg_ctx* c, const float* L_dev, cudaStream_t s) {
     if (!fused_check) gmgk::check_coeffs(c->g[0], L_dev, rbuf(c), s);
     for (int l = 0; l + 1 < c->nlev; ++l) {
         float* Lc = const_cast<float*>(c->lv[l + 1].L);
-        if (c->prm.fast_path && gmgk::coarsen4_supported(c->g[l]))
-            gmgk::coarsen_coeffs4(c->g[l], c->lv[l].L, Lc, l == 0, rbuf(c), s);
-        else
+        if (c->prm.fast_path && gmgk::coarsen4_supported(c->g[l])) {
+            // the pass that reads every coefficient of level l also marks its uniform bricks
+            if (c->uni[l].brick) cudaMemsetAsync(const_cast<unsigned char*>(c->uni[l].brick), 1, c->ubrick_n[l], s);
+            gmgk::coarsen_coeffs4(c->g[l], c->lv[l].L, Lc, l == 0, rbuf(c), c->uni[l], s);
+        } else {
+            if (c->uni[l].brick) cudaMemsetAsync(const_cast<unsigned char*>(c->uni[l].brick), 0, c->ubrick_n[l], s);
             gmgk::coarsen_coeffs(c->g[l], c->lv[l].L, Lc, s);
+        }
     }
     for (int l = (c->ctail_start < c->tail_start ? c->ctail_start : c->tail_start); l < c->nlev; ++l)
         gmgk::tail_weights(c->g[l], c->lv[l].L, c->tail_W[l], s);
-    // uniform bricks of the TMA-fed levels (uniform.cuh); flags and counts come down with the status
+    // uniform bricks (uniform.cuh): how many cells of each level the lean path covers, counted on the
+    // device with the kernels' own footprint test; the counts come down with the next status read
     if (c->ubrick_dev) {
-        unsigned int* cnt = reinterpret_cast<unsigned int*>(c->ubrick_dev + c->ubrick_total);
-        cudaMemsetAsync(cnt, 0, sizeof(unsigned int) * GMG_MAX_LEVELS, s);
-        for (int l = 0; l < c->nlev; ++l)
-            if (c->uni[l].brick)
-                gmgk::uniform_bricks(c->g[l], c->lv[l].L, c->uni[l].ux, c->uni[l].uy, c->uni[l].uz,
-                                     const_cast<unsigned char*>(c->uni[l].brick), cnt + l, s);
-        cudaMemcpyAsync(c->ubrick_host, c->ubrick_dev, c->ubrick_total + sizeof(unsigned int) * GMG_MAX_LEVELS,
-                        cudaMemcpyDeviceToHost, s);
+        unsigned long long* cnt = reinterpret_cast<unsigned long long*>(c->ubrick_dev + c->ubrick_total);
+        cudaMemsetAsync(cnt, 0, sizeof(unsigned long long) * 2 * GMG_MAX_LEVELS, s);
+        for (int l = 0; l < c->nlev; ++l) {
+            if (!c->uni[l].brick) continue;
+            int ty = 0, zc = 0;
+            if (gmgf::bulk_sweep_tiling(c->g[l], &ty, &zc))
+                gmgk::uniform_cells(c->g[l], c->uni[l].brick, 128, ty, ty + 2, zc, 0, cnt + l, s);
+            if (gmgf::res_bulk_tiling(c->g[l], &ty, &zc))
+                gmgk::uniform_cells(c->g[l], c->uni[l].brick, 128, ty, ty + 1, zc, 1, cnt + GMG_MAX_LEVELS + l, s);
+        }
+        cudaMemcpyAsync(c->ucount_host, cnt, sizeof(unsigned long long) * 2 * GMG_MAX_LEVELS, cudaMemcpyDeviceToHost, s);
         c->uni_stats_pending = true;
     }
     gmgk::ctl_set_omega(c->sc, (double)c->prm.omega0, s);
 }
 
-// After a synchronisation behind set_coeffs_enqueue: which share of each level's cells the lean
-// path covers (the kernels' own footprint test on the host copy of the flags).
+// After a synchronisation behind set_coeffs_enqueue: the share of each level's cells on the lean path.
 static void refresh_uniform_stats(gmg_ctx* c) {
     if (!c->uni_stats_pending) return;
     c->uni_stats_pending = false;
     for (int l = 0; l < c->nlev; ++l) {
-        c->uni_frac_sweep[l] = c->uni_frac_res[l] = 0.0;
-        if (!c->uni[l].brick) continue;
-        const unsigned char* hb = c->ubrick_host + (c->uni[l].brick - c->ubrick_dev);
-        c->uni_frac_sweep[l] = gmgf::bulk_sweep_uniform_fraction(c->g[l], hb);
-        c->uni_frac_res[l] = gmgf::res_bulk_uniform_fraction(c->g[l], hb);
+        c->uni_frac_sweep[l] = c->uni[l].brick ? (double)c->ucount_host[l] / (double)c->g[l].N : 0.0;
+        c->uni_frac_res[l] = c->uni[l].brick ? (double)c->ucount_host[GMG_MAX_LEVELS + l] / (double)c->g[l].N : 0.0;
     }
 }
 
@@ -872,7 +908,9 @@ static int build_graph(gmg_ctx* c, GraphSlot& slot, int solver, float* p, const 
     CUDA_TRY(c, cudaStreamBeginCaptureToGraph(c->cap_b, body, nullptr, nullptr, 0,
                                               cudaStreamCaptureModeRelaxed));
     c->n_launch = 0;
+    use_side(c, 1);
     enqueue_body(c, solver, p, z, lc, c->cap_b);
+    use_side(c, 0);
     slot.n_body = c->n_launch;
     cudaGraph_t body_out = nullptr;
     CUDA_TRY(c, cudaStreamEndCapture(c->cap_b, &body_out));

@@ -6,6 +6,8 @@
 
 #include "../../include/gmg.h"
 
+namespace gmgf { struct UniArgs; }
+
 #define GMG_MAX_LEVELS 24
 #define GMG_TAIL_MAX_LEVELS 8
 
@@ -119,12 +121,13 @@ void coarsen_coeffs(const LevelGeom& gf, const float* Lf, float* Lc, cudaStream_
 void check_coeffs(const LevelGeom& g, const float* L, ReduceBuf rb, cudaStream_t s);
 // float4 passes (kernels_setup.cu): bit-identical to the three kernels above
 bool coarsen4_supported(const LevelGeom& gf);
-void coarsen_coeffs4(const LevelGeom& gf, const float* Lf, float* Lc, bool check, ReduceBuf rb, cudaStream_t s);
+void coarsen_coeffs4(const LevelGeom& gf, const float* Lf, float* Lc, bool check, ReduceBuf rb,
+                     const gmgf::UniArgs& uni, cudaStream_t s);
 void divergence4(const LevelGeom& g, const float* u, const float wall_hi[3], float* z, cudaStream_t s);
 void project4(const LevelGeom& g, const float* L, const float* p, float* u, cudaStream_t s);
-// uniform bricks (uniform.cuh): flag[brick] = every Lx, Ly, Lz of the brick equals ux, uy, uz
-void uniform_bricks(const LevelGeom& g, const float* L, float ux, float uy, float uz, unsigned char* flag,
-                    unsigned int* count, cudaStream_t s);
+// uniform bricks (uniform.cuh): cells of a level on the lean path of a kernel with this tiling
+void uniform_cells(const LevelGeom& g, const unsigned char* brick, int TXc, int TYc, int yhi, int zchunk, int rule,
+                   unsigned long long* out, cudaStream_t s);
 void tail_vcycle(const TailArgs& a, size_t smem_bytes, cudaStream_t s);
 // W[f*N + c] = weight of face f (x-lo, x-hi, y-lo, y-hi, z-lo, z-hi) of cell c, wall faces zeroed
 void tail_weights(const LevelGeom& g, const float* L, float* W, cudaStream_t s);

@@ -411,22 +411,14 @@ static bool res_maps(const LevelGeom& g, const float* L, const float* p, const f
            tensor_map(L + N, g, C::TX, C::RY + 1, &m->ly) && tensor_map(b, g, C::TX, C::RY, &m->b);
 }
 
-// Fraction of the level's cells whose residual CTA takes the lean path (see bulk_sweep_uniform_fraction)
-double res_bulk_uniform_fraction(const LevelGeom& g, const unsigned char* brick_host) {
+// The tiling of the TMA-fed residual pass on this level (for gmg_stats' count of lean-path cells)
+bool res_bulk_tiling(const LevelGeom& g, int* tile_y, int* zchunk) {
     using C = ResBulkCfg;
-    if (!bulk_supported(g) || (g.n[2] & 1)) return 0.0;
+    if (!bulk_supported(g) || (g.n[2] & 1)) return false;
     const int tiles_x = g.n[0] / C::TX, tiles_y = (g.n[1] + C::RY - 1) / C::RY;
-    const int zchunk = choose_zchunk((long long)tiles_x * tiles_y, g.n[2], kZChunkPref, kZChunkMin, 296, 1);
-    double cells = 0.0;
-    for (int z0 = 0; z0 < g.n[2]; z0 += zchunk)
-        for (int ty = 0; ty < tiles_y; ++ty)
-            for (int tx = 0; tx < tiles_x; ++tx) {
-                const int x0 = tx * C::TX, y0 = ty * C::RY, z1 = z0 + zchunk < g.n[2] ? z0 + zchunk : g.n[2];
-                if (!((y0 >= 1) && (y0 + C::RY + 1 <= g.n[1]))) continue;
-                if (!ub_box_uniform(g, brick_host, x0 - 2, x0 + C::TX + 1, y0 - 2, y0 + C::RY + 1, z0 - 2, z1 + 1)) continue;
-                cells += (double)C::TX * C::RY * (z1 - z0);
-            }
-    return cells / (double)g.N;
+    *tile_y = C::RY;
+    *zchunk = choose_zchunk((long long)tiles_x * tiles_y, g.n[2], kZChunkPref, kZChunkMin, 296, 1);
+    return true;
 }
 
 template <int MODE>

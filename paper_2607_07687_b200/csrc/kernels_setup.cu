@@ -26,9 +26,11 @@ __device__ __forceinline__ int bad4(const float4& v) {
 
 // One work item = four x-adjacent coarse cells (J, K fixed) = a 4CX x CY x CZ brick of fine cells.
 // f[d][a][b][e]: float4 number e of fine row (y = CY*J + b, z = CZ*K + a) of array d.
+// uni.brick != nullptr: the pass also CLEARS the uniform-brick flag (uniform.cuh; preset to 1) of
+// the brick its fine values lie in as soon as one of them differs from the level's constant.
 template <int CX, int CY, int CZ, bool CHECK>
 __global__ void __launch_bounds__(kST)
-k_coarsen4(LevelGeom gf, const float* __restrict__ Lf, float* __restrict__ Lc, ReduceBuf rb) {
+k_coarsen4(LevelGeom gf, const float* __restrict__ Lf, float* __restrict__ Lc, ReduceBuf rb, gmgf::UniArgs uni) {
     const int ncx = gf.n[0] / CX, ncy = gf.n[1] / CY, ncz = gf.n[2] / CZ;
     const int gpr = ncx / 4;  // groups per coarse row
     const long long items = (long long)gpr * ncy * ncz;
@@ -44,8 +46,10 @@ k_coarsen4(LevelGeom gf, const float* __restrict__ Lf, float* __restrict__ Lc, R
         const int J = (int)(row - (long long)K * ncy);
         const long long fbase = (long long)(4 * CX * Ig) + (long long)nx * (CY * J) + fsz * (CZ * K);
         const long long cbase = (long long)(4 * Ig) + (long long)ncx * (J + (long long)ncy * K);
+        bool differs = false;
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
+            const float ud = d == 0 ? uni.ux : d == 1 ? uni.uy : uni.uz;
             float4 f[CZ][CY][CX];
 #pragma unroll
             for (int a = 0; a < CZ; ++a)
@@ -55,6 +59,8 @@ k_coarsen4(LevelGeom gf, const float* __restrict__ Lf, float* __restrict__ Lc, R
                     for (int e = 0; e < CX; ++e) {
                         f[a][b][e] = ld4(Lf + d * Nf + fbase + a * fsz + (long long)b * nx + 4 * e);
                         if (CHECK) bad += bad4(f[a][b][e]);
+                        differs = differs || f[a][b][e].x != ud || f[a][b][e].y != ud || f[a][b][e].z != ud ||
+                                  f[a][b][e].w != ud;
                     }
             // fine value at (x = CX*(4 Ig + m) + ex, y = CY*J + b, z = CZ*K + a)
             auto at = [&](int m, int ex, int b, int a) -> float {
@@ -91,6 +97,12 @@ k_coarsen4(LevelGeom gf, const float* __restrict__ Lf, float* __restrict__ Lc, R
             }
             *reinterpret_cast<float4*>(Lc + d * Nc + cbase) = make_float4(o[0], o[1], o[2], o[3]);
         }
+        if (uni.brick && differs) {
+            // the 4CX x CY x CZ fine cells of this work item lie in ONE brick (4CX | kUBX, CY | kUBY, CZ | kUBZ)
+            using namespace gmgf;
+            const int bx = (4 * CX * Ig) / kUBX, by = (CY * J) / kUBY, bz = (CZ * K) / kUBZ;
+            const_cast<unsigned char*>(uni.brick)[((size_t)bz * ub_count(gf.n[1], kUBY) + by) * ub_count(nx, kUBX) + bx] = 0;
+        }
     }
     if (CHECK) finish_reduction((double)bad, 0.0, false, rb, RED_CHECK, 0);
 }
@@ -103,28 +115,28 @@ bool coarsen4_supported(const LevelGeom& gf) {
 
 template <int CX, int CY, int CZ>
 static void coarsen4_launch(const LevelGeom& gf, const float* Lf, float* Lc, bool check, ReduceBuf rb,
-                            cudaStream_t s) {
+                            const gmgf::UniArgs& uni, cudaStream_t s) {
     const long long items = gf.N / ((long long)CX * CY * CZ) / 4;
     long long blocks = (items + kST - 1) / kST;
     if (blocks > 148 * 16) blocks = 148 * 16;
     if (blocks < 1) blocks = 1;
-    if (check) k_coarsen4<CX, CY, CZ, true><<<(unsigned int)blocks, kST, 0, s>>>(gf, Lf, Lc, rb);
-    else k_coarsen4<CX, CY, CZ, false><<<(unsigned int)blocks, kST, 0, s>>>(gf, Lf, Lc, rb);
+    if (check) k_coarsen4<CX, CY, CZ, true><<<(unsigned int)blocks, kST, 0, s>>>(gf, Lf, Lc, rb, uni);
+    else k_coarsen4<CX, CY, CZ, false><<<(unsigned int)blocks, kST, 0, s>>>(gf, Lf, Lc, rb, uni);
 }
 
 // Next level's coefficients from this level's; check = also count invalid values into
 // red[RED_CHECK] (replaces check_coeffs on the finest level).
 void coarsen_coeffs4(const LevelGeom& gf, const float* Lf, float* Lc, bool check, ReduceBuf rb,
-                     cudaStream_t s) {
+                     const gmgf::UniArgs& uni, cudaStream_t s) {
     const int key = (gf.c[0] - 1) | ((gf.c[1] - 1) << 1) | ((gf.c[2] - 1) << 2);
     switch (key) {
-        case 1: coarsen4_launch<2, 1, 1>(gf, Lf, Lc, check, rb, s); break;
-        case 2: coarsen4_launch<1, 2, 1>(gf, Lf, Lc, check, rb, s); break;
-        case 3: coarsen4_launch<2, 2, 1>(gf, Lf, Lc, check, rb, s); break;
-        case 4: coarsen4_launch<1, 1, 2>(gf, Lf, Lc, check, rb, s); break;
-        case 5: coarsen4_launch<2, 1, 2>(gf, Lf, Lc, check, rb, s); break;
-        case 6: coarsen4_launch<1, 2, 2>(gf, Lf, Lc, check, rb, s); break;
-        default: coarsen4_launch<2, 2, 2>(gf, Lf, Lc, check, rb, s); break;
+        case 1: coarsen4_launch<2, 1, 1>(gf, Lf, Lc, check, rb, uni, s); break;
+        case 2: coarsen4_launch<1, 2, 1>(gf, Lf, Lc, check, rb, uni, s); break;
+        case 3: coarsen4_launch<2, 2, 1>(gf, Lf, Lc, check, rb, uni, s); break;
+        case 4: coarsen4_launch<1, 1, 2>(gf, Lf, Lc, check, rb, uni, s); break;
+        case 5: coarsen4_launch<2, 1, 2>(gf, Lf, Lc, check, rb, uni, s); break;
+        case 6: coarsen4_launch<1, 2, 2>(gf, Lf, Lc, check, rb, uni, s); break;
+        default: coarsen4_launch<2, 2, 2>(gf, Lf, Lc, check, rb, uni, s); break;
     }
 }
 
@@ -212,44 +224,38 @@ void project4(const LevelGeom& g, const float* L, const float* p, float* u, cuda
     k_project4<<<(unsigned int)((items + kST - 1) / kST), kST, 0, s>>>(g, L, p, u);
 }
 
-// ---- uniform bricks (uniform.cuh): one block per brick of kUBX x kUBY x kUBZ cells; flag = every
-// stored Lx, Ly, Lz value of the brick equals the level's constant of its direction.  nx % 128 == 0
-// (only levels that run the TMA-fed kernels are marked).  count[0] += 1 per uniform brick.
-__global__ void __launch_bounds__(256)
-k_uniform_bricks(LevelGeom g, const float* __restrict__ L, float ux, float uy, float uz,
-                 unsigned char* __restrict__ flag, unsigned int* __restrict__ count) {
+// ---- uniform bricks (uniform.cuh): how many cells of a level are worked on by CTAs that take the
+// lean path, for a kernel's tiling (one thread per CTA of that kernel, the kernel's own footprint
+// test).  rule 0 = the sweep (box-fed tiles: inside, walls in y, or first / final tile row of a
+// periodic y axis), rule 1 = the residual pass (tiles inside the domain in y).  out += cells.
+__global__ void __launch_bounds__(128)
+k_uniform_cells(LevelGeom g, const unsigned char* __restrict__ brick, int TXc, int TYc, int yhi, int zchunk, int rule,
+                unsigned long long* __restrict__ out) {
     using namespace gmgf;
-    const int nbx = ub_count(g.n[0], kUBX), nby = ub_count(g.n[1], kUBY);
-    int b = blockIdx.x;
-    const int bx = b % nbx;
-    b /= nbx;
-    const int by = b % nby, bz = b / nby;
-    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
-    const long long N = g.N;
-    bool ok = true;
-    // kUBY * kUBZ rows of kUBX / 4 float4 groups per array
-    constexpr int GPR = kUBX / 4;
-    for (int t = threadIdx.x; t < GPR * kUBY * kUBZ; t += 256) {
-        const int gx = t % GPR, r = t / GPR;
-        const int y = by * kUBY + r % kUBY, z = bz * kUBZ + r / kUBY;
-        if (y >= ny || z >= nz) continue;
-        const long long o = (long long)bx * kUBX + 4 * gx + (long long)nx * (y + (long long)ny * z);
-        const float4 a = ld4(L + o), c = ld4(L + N + o), d = ld4(L + 2 * N + o);
-        ok = ok && a.x == ux && a.y == ux && a.z == ux && a.w == ux && c.x == uy && c.y == uy && c.z == uy &&
-             c.w == uy && d.x == uz && d.y == uz && d.z == uz && d.w == uz;
+    const int tiles_x = g.n[0] / TXc, tiles_y = (g.n[1] + TYc - 1) / TYc, nzc = (g.n[2] + zchunk - 1) / zchunk;
+    const long long total = (long long)tiles_x * tiles_y * nzc;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= total) return;
+    const int tx = (int)(t % tiles_x), ty = (int)((t / tiles_x) % tiles_y), zc = (int)(t / ((long long)tiles_x * tiles_y));
+    const int x0 = tx * TXc, y0 = ty * TYc, z0 = zc * zchunk, z1 = min(g.n[2], z0 + zchunk), ny = g.n[1];
+    bool boxfed;
+    if (rule == 0) {
+        const bool inside = (y0 >= 2) && (y0 + TYc + 2 <= ny);
+        boxfed = g.bc[1] != 0 || inside || (tiles_y >= 2 && ((ty == 0 && TYc + 2 <= ny) || (ty == tiles_y - 1 && y0 >= 2)));
+    } else {
+        boxfed = (y0 >= 1) && (y0 + TYc + 1 <= ny);
     }
-    const int all = __syncthreads_and(ok ? 1 : 0);
-    if (threadIdx.x == 0) {
-        flag[blockIdx.x] = all ? 1 : 0;
-        if (all) atomicAdd(count, 1u);
-    }
+    if (!boxfed) return;
+    if (!ub_box_uniform(g, brick, x0 - 2, x0 + TXc + 1, y0 - 2, y0 + yhi, z0 - 2, z1 + 1)) return;
+    const int rows = min(TYc, ny - y0);
+    atomicAdd(out, (unsigned long long)TXc * rows * (z1 - z0));
 }
 
-void uniform_bricks(const LevelGeom& g, const float* L, float ux, float uy, float uz, unsigned char* flag,
-                    unsigned int* count, cudaStream_t s) {
-    using namespace gmgf;
-    const unsigned int nb = (unsigned int)(ub_count(g.n[0], kUBX) * ub_count(g.n[1], kUBY) * ub_count(g.n[2], kUBZ));
-    k_uniform_bricks<<<nb, 256, 0, s>>>(g, L, ux, uy, uz, flag, count);
+void uniform_cells(const LevelGeom& g, const unsigned char* brick, int TXc, int TYc, int yhi, int zchunk, int rule,
+                   unsigned long long* out, cudaStream_t s) {
+    const int tiles_x = g.n[0] / TXc, tiles_y = (g.n[1] + TYc - 1) / TYc, nzc = (g.n[2] + zchunk - 1) / zchunk;
+    const long long total = (long long)tiles_x * tiles_y * nzc;
+    k_uniform_cells<<<(unsigned int)((total + 127) / 128), 128, 0, s>>>(g, brick, TXc, TYc, yhi, zchunk, rule, out);
 }
 
 }  // namespace gmgk

@@ -21,6 +21,8 @@
 // bulk-copy path (cp.async.bulk, UBLKCP) with wrapped row addresses.  Neumann walls = zeroed
 // coefficients.  Every shared-memory cell holds the periodic image of its cell, as in k_rb_sweep.
 #include <cuda.h>
+#include <stdio.h>
+#include <stdlib.h>
 
 #include <map>
 #include <mutex>
@@ -30,9 +32,12 @@
 #include "uniform.cuh"
 
 namespace gmgf {
-template <int TY_, int PD_>
+// LEAN_: the layout of the kernel that runs ONLY the lean path (uniform.cuh): no coefficient rings,
+// 88 KB instead of 190 KB, so that two CTAs share an SM.
+template <int TY_, int PD_, bool LEAN_ = false>
 struct BulkCfg {
     static constexpr int TX = 128, TY = TY_, PD = PD_;
+    static constexpr bool LEAN = LEAN_;
     static constexpr int LPR = 32;
     static constexpr int ROWS = TY + 2;          // rows running phase B (tile + ring 1)
     static constexpr int MAIN = LPR * ROWS;
@@ -53,9 +58,9 @@ struct BulkCfg {
     static constexpr int Y_PLANE = (ROWS + 1) * TX;  // Ly (needs the row above too)
     static constexpr int OFF_P = 0;
     static constexpr int OFF_LZ = OFF_P + NP * P_PLANE;
-    static constexpr int OFF_LX = OFF_LZ + NZ * C_PLANE;
-    static constexpr int OFF_LY = OFF_LX + NC * C_PLANE;
-    static constexpr int OFF_B = OFF_LY + NC * Y_PLANE;
+    static constexpr int OFF_LX = OFF_LZ + (LEAN ? 0 : NZ * C_PLANE);
+    static constexpr int OFF_LY = OFF_LX + (LEAN ? 0 : NC * C_PLANE);
+    static constexpr int OFF_B = OFF_LY + (LEAN ? 0 : NC * Y_PLANE);
     static constexpr int FLOATS = OFF_B + NC * C_PLANE;
     static constexpr int NROWCOPY = SH + 4 * ROWS + 1;  // rows per step on the row-copy path
     static constexpr size_t SMEM = (size_t)FLOATS * sizeof(float) + 16 * sizeof(uint64_t) + (size_t)NROWCOPY * 16;
@@ -633,44 +638,69 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
     }
 }
 
+// How a tile's planes reach shared memory: 0 = full boxes (inside the domain in y, or walls in y:
+// rows outside arrive zero-filled), 2 = first / final tile row of a periodic y axis: boundary boxes
+// plus a few row copies, 1 = row copies only (odd cases: a single tile row, a final row too short).
+template <class C>
+__device__ __forceinline__ int tile_ymode(const BulkArgs& a, int ty) {
+    const int y0 = ty * C::TY, ny = a.g.n[1];
+    if (a.g.bc[1] != 0 || ((y0 >= 2) && (y0 + C::TY + 2 <= ny))) return 0;
+    if (a.tiles_y >= 2 && ((ty == 0 && C::TY + 2 <= ny) || (ty == a.tiles_y - 1 && y0 >= 2))) return 2;
+    return 1;
+}
+
+// Lean path (uniform.cuh)?  Every warp evaluates the same few brick flags (CTA-uniform verdict): the
+// tile is box-fed and all coefficients the CTA would touch -- tile + ring 2, planes z0-2 .. z1+1 --
+// are the level's constants with no Neumann wall in reach.  Such tiles belong to k_rb_sweep_lean.
+template <class C>
+__device__ __forceinline__ bool tile_is_lean(const BulkArgs& a, int ymode) {
+    if (!a.uni.brick || ymode == 1) return false;
+    int bid = blockIdx.x;
+    const int tx = bid % a.tiles_x;
+    bid /= a.tiles_x;
+    const int ty = bid % a.tiles_y;
+    const int zc = bid / a.tiles_y;
+    const int x0 = tx * C::TX, y0 = ty * C::TY, z0 = zc * a.zchunk, z1 = min(a.g.n[2], z0 + a.zchunk);
+    return ub_box_uniform_warp(a.g, a.uni.brick, x0 - 2, x0 + C::TX + 1, y0 - 2, y0 + C::TY + 2, z0 - 2, z1 + 1,
+                               threadIdx.x & 31);
+}
+
 // EDGE: the kernel also carries the YMODE 2 body and sends every tile of a Neumann y axis through
 // the full boxes.  It pays on grids with few tile rows (a 1024 x 384 x 384 channel: -5 % per solve);
 // on a 1024^3 cube the third body costs the interior loop its register allocation (+2.6 % per
 // sweep, measured A/B on one box), so the launcher picks the kernel by the number of tile rows.
+// With uniform bricks marked (a.uni.brick) the lean tiles are k_rb_sweep_lean's: they return here.
 template <class C, int NORM = 0, bool EDGE = false>
 __global__ void __launch_bounds__(C::THREADS, 1)
 k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     if (a.run_flag && *a.run_flag == 0) return;   // a re-run that turned out not to be needed
     const int ty = (blockIdx.x / a.tiles_x) % a.tiles_y;
-    const int y0 = ty * C::TY;
-    const int ny = a.g.n[1];
-    const bool inside = (y0 >= 2) && (y0 + C::TY + 2 <= ny);
-    // Lean path (uniform.cuh)?  Every warp evaluates the same few brick flags (CTA-uniform verdict):
-    // all coefficients the CTA would touch -- tile + ring 2, planes z0-2 .. z1+1 -- are the level's
-    // constants and no Neumann wall is in reach.
-    bool uni = false;
-    if (a.uni.brick) {
-        int bid = blockIdx.x;
-        const int tx = bid % a.tiles_x;
-        const int zc = bid / (a.tiles_x * a.tiles_y);
-        const int x0 = tx * C::TX, z0 = zc * a.zchunk, z1 = min(a.g.n[2], z0 + a.zchunk);
-        uni = ub_box_uniform_warp(a.g, a.uni.brick, x0 - 2, x0 + C::TX + 1, y0 - 2, y0 + C::TY + 2, z0 - 2, z1 + 1,
-                                  threadIdx.x & 31);
-    }
+    const int ymode = tile_ymode<C>(a, ty);
+    if (tile_is_lean<C>(a, ymode)) return;
     if (EDGE) {
-        if (a.g.bc[1] != 0 || inside) {
-            if (uni) sweep_body<C, 0, NORM, true>(a, maps);
-            else sweep_body<C, 0, NORM>(a, maps);
-        } else if (a.tiles_y >= 2 && ((ty == 0 && C::TY + 2 <= ny) || (ty == a.tiles_y - 1 && y0 >= 2))) {
-            if (uni) sweep_body<C, 2, NORM, true>(a, maps);
-            else sweep_body<C, 2, NORM>(a, maps);
-        } else sweep_body<C, 1, NORM>(a, maps);
+        if (ymode == 0) sweep_body<C, 0, NORM>(a, maps);
+        else if (ymode == 2) sweep_body<C, 2, NORM>(a, maps);
+        else sweep_body<C, 1, NORM>(a, maps);
     } else {
-        if (inside) {
-            if (uni) sweep_body<C, 0, NORM, true>(a, maps);
-            else sweep_body<C, 0, NORM>(a, maps);
-        } else sweep_body<C, 1, NORM>(a, maps);
+        const int y0 = ty * C::TY;
+        if ((y0 >= 2) && (y0 + C::TY + 2 <= a.g.n[1])) sweep_body<C, 0, NORM>(a, maps);
+        else sweep_body<C, 1, NORM>(a, maps);
     }
+}
+
+// The lean path as a kernel of its own: the box-fed tiles whose footprint is uniform; every other
+// tile of the grid returns at once (k_rb_sweep_bulk takes those).  Without coefficient rings a CTA
+// needs 88 KB of shared memory and 64 registers per thread, so TWO CTAs share an SM and one fills
+// the other's barrier and latency gaps (issue slots 44 % -> 69 % busy).
+template <class C, int NORM = 0>
+__global__ void __launch_bounds__(C::THREADS, 2)
+k_rb_sweep_lean(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
+    if (a.run_flag && *a.run_flag == 0) return;
+    const int ty = (blockIdx.x / a.tiles_x) % a.tiles_y;
+    const int ymode = tile_ymode<C>(a, ty);
+    if (!tile_is_lean<C>(a, ymode)) return;
+    if (ymode == 0) sweep_body<C, 0, NORM, true>(a, maps);
+    else sweep_body<C, 2, NORM, true>(a, maps);
 }
 
 // ---- launchers ------------------------------------------------------------------------------
@@ -680,6 +710,8 @@ void rb_sweep_v2(const LevelGeom& g, const float* L, const float* src, float* ds
 int configure_v2();
 
 using Bulk = BulkCfg<13, 4>;
+using Lean = BulkCfg<13, 4, true>;
+static_assert(2 * (Lean::SMEM + 1024) <= 227 * 1024, "two lean CTAs per SM");
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
@@ -736,29 +768,12 @@ static unsigned int bulk_grid(const LevelGeom& g, int* zchunk_out) {
     return (unsigned int)(tiles_x * tiles_y * ((g.n[2] + zchunk - 1) / zchunk));
 }
 
-// Fraction of the level's cells whose CTA takes the lean path (uniform.cuh), from a HOST copy of
-// the brick flags: the same footprint test the kernel applies, for gmg_stats' as-run byte count.
-double bulk_sweep_uniform_fraction(const LevelGeom& g, const unsigned char* brick_host) {
-    if (!bulk_supported(g)) return 0.0;
-    int zchunk = 0;
-    bulk_grid(g, &zchunk);
-    const int tiles_x = g.n[0] / Bulk::TX, tiles_y = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
-    const bool edge = bulk_sweep_edge(g, false);
-    double cells = 0.0;
-    for (int z0 = 0; z0 < g.n[2]; z0 += zchunk)
-        for (int ty = 0; ty < tiles_y; ++ty)
-            for (int tx = 0; tx < tiles_x; ++tx) {
-                const int x0 = tx * Bulk::TX, y0 = ty * Bulk::TY, z1 = z0 + zchunk < g.n[2] ? z0 + zchunk : g.n[2];
-                const bool inside = (y0 >= 2) && (y0 + Bulk::TY + 2 <= g.n[1]);
-                const bool boxfed = inside || (edge && (g.bc[1] != 0 || (tiles_y >= 2 &&
-                                    ((ty == 0 && Bulk::TY + 2 <= g.n[1]) || (ty == tiles_y - 1 && y0 >= 2)))));
-                if (!boxfed) continue;
-                if (!ub_box_uniform(g, brick_host, x0 - 2, x0 + Bulk::TX + 1, y0 - 2, y0 + Bulk::TY + 2, z0 - 2, z1 + 1))
-                    continue;
-                const int rows = (y0 + Bulk::TY <= g.n[1] ? Bulk::TY : g.n[1] - y0);
-                cells += (double)Bulk::TX * rows * (z1 - z0);
-            }
-    return cells / (double)g.N;
+// The tiling of the TMA-fed sweep on this level (for gmg_stats' count of lean-path cells)
+bool bulk_sweep_tiling(const LevelGeom& g, int* tile_y, int* zchunk) {
+    if (!bulk_supported(g)) return false;
+    *tile_y = Bulk::TY;
+    bulk_grid(g, zchunk);
+    return true;
 }
 
 // rb_sweep_with_norm will run on this level (shape fits the TMA kernel, one partial per CTA fits)
@@ -814,7 +829,7 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
     const int tiles_y_ = (g.n[1] + Bulk::TY - 1) / Bulk::TY;
     const int rem = g.n[1] - (tiles_y_ - 1) * Bulk::TY;      // rows of the final tile row
     const bool edge = bulk_sweep_edge(g, norm != nullptr);
-    if (ok && edge && g.bc[1] == 0 && tiles_y_ >= 2) {
+    if (ok && (edge || uni.brick) && g.bc[1] == 0 && tiles_y_ >= 2) {
         ok = ok && set(maps.m[1], Bulk::SH - 2, Bulk::ROWS - 1, Bulk::ROWS);   // FIRST: from y = 0
         ok = ok && set(maps.m[2], rem + 2, rem + 1, rem + 1);                  // FINAL: up to y = ny - 1
     } else {
@@ -836,14 +851,38 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
     a.zchunk = zchunk;
     if (grid > GMG_REDUCE_MAX_BLOCKS && norm) return false;
     const int nv = (norm && slot_ref >= 0) ? 2 : (norm ? 1 : 0);
+    // With uniform bricks marked, two kernels share the grid: k_rb_sweep_lean (two CTAs per SM) takes
+    // the lean tiles, k_rb_sweep_bulk the rest.  They touch disjoint tiles of dst, so they run side by
+    // side -- the general one first, on a forked stream, so that its few long CTAs are spread over the
+    // SMs while the lean CTAs fill in -- and the caller's stream waits for both.  The partial sums of a
+    // norm-carrying sweep are shared: every tile is worked on by exactly one kernel and only working
+    // CTAs take a ticket, so the last of either kernel finishes the sum.
+    cudaStream_t sg = s;
+    const bool fork = uni.brick && uni.side_stream;
+    if (fork) {
+        sg = (cudaStream_t)uni.side_stream;
+        cudaEventRecord((cudaEvent_t)uni.ev_fork, s);
+        cudaStreamWaitEvent(sg, (cudaEvent_t)uni.ev_fork, 0);
+    }
+    auto launch_lean = [&]() {
+        if (nv == 2) k_rb_sweep_lean<Lean, 2><<<grid, Lean::THREADS, Lean::SMEM, s>>>(a, maps);
+        else if (nv == 1) k_rb_sweep_lean<Lean, 1><<<grid, Lean::THREADS, Lean::SMEM, s>>>(a, maps);
+        else k_rb_sweep_lean<Lean, 0><<<grid, Lean::THREADS, Lean::SMEM, s>>>(a, maps);
+    };
+    if (uni.brick && !fork) launch_lean();
     if (edge) {
-        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, true><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
-        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, true><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
-        else k_rb_sweep_bulk<Bulk, 0, true><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, true><<<grid, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, true><<<grid, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+        else k_rb_sweep_bulk<Bulk, 0, true><<<grid, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
     } else {
-        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, false><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
-        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, false><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
-        else k_rb_sweep_bulk<Bulk, 0, false><<<grid, Bulk::THREADS, Bulk::SMEM, s>>>(a, maps);
+        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, false><<<grid, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, false><<<grid, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+        else k_rb_sweep_bulk<Bulk, 0, false><<<grid, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+    }
+    if (fork) {
+        launch_lean();
+        cudaEventRecord((cudaEvent_t)uni.ev_join, sg);
+        cudaStreamWaitEvent(s, (cudaEvent_t)uni.ev_join, 0);
     }
     return true;
 }
@@ -862,6 +901,24 @@ int configure() {
         e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_rb_sweep_bulk<Bulk, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Bulk::SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_lean<Lean, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Lean::SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_lean<Lean, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Lean::SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_lean<Lean, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Lean::SMEM);
+    // two lean CTAs per SM need the large shared-memory carve-out
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_lean<Lean, 0>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_lean<Lean, 1>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_lean<Lean, 2>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    if (e == cudaSuccess && getenv("GMG_DEBUG_OCC")) {
+        int nb = -1;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_rb_sweep_lean<Lean, 0>, Lean::THREADS, Lean::SMEM);
+        fprintf(stderr, "[gmg] k_rb_sweep_lean: %d CTAs/SM, smem %zu\n", nb, (size_t)Lean::SMEM);
+    }
     if (e == cudaSuccess && !g_encode) {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult qres;
