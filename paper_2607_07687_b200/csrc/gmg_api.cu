@@ -60,6 +60,7 @@ struct GraphSlot {
     int maxiter = -1;
     double* hist = nullptr;
     long long n_pre = 0, n_body = 0, n_post = 0;  // kernel launches per section
+    int left_n[GMG_MAX_LEVELS];   // lengths of the remaining-tile lists the launch grids were sized with
 };
 
 struct gmg_ctx {
@@ -83,7 +84,8 @@ struct gmg_ctx {
     size_t ubrick_n[GMG_MAX_LEVELS];       // bricks of the level
     unsigned char* ubrick_dev;             // all levels' flags, one allocation; behind them
                                            // [2][GMG_MAX_LEVELS] counts of lean-path cells (sweep, residual)
-    unsigned long long* ucount_host;       // pinned mirror of the counts
+                                           // and [GMG_MAX_LEVELS] lengths of the remaining-tile lists, then the lists
+    unsigned long long* ucount_host;       // pinned mirror of the counts and lengths
     size_t ubrick_total;
     double uni_frac_sweep[GMG_MAX_LEVELS]; // cells whose sweep / residual CTA takes the lean path
     double uni_frac_res[GMG_MAX_LEVELS];
@@ -135,6 +137,8 @@ struct gmg_ctx {
 static const long long kBulkMatvecMinCells = 4LL << 20;
 
 static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+// behind the brick flags: [2][levels] u64 lean-cell counts, [levels] u32 remaining-tile list lengths
+static const size_t kUniCountBytes = 256 * ((sizeof(unsigned long long) * 2 * GMG_MAX_LEVELS + sizeof(unsigned int) * GMG_MAX_LEVELS + 255) / 256);
 static inline const gmgf::UniArgs& U(const gmg_ctx* c, int l) { return c->uni[l]; }
 // The float4 / TMA paths read caller arrays 16 bytes at a time (gmg.h "Alignment").
 static inline bool al16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
@@ -208,6 +212,7 @@ static void build_levels(gmg_ctx* c) {
             c->uni[l].uz = (float)(C[0] * C[1] / C[2]);
             c->uni[l].brick = nullptr;
             c->uni[l].side_stream = c->uni[l].ev_fork = c->uni[l].ev_join = nullptr;
+            c->uni[l].left_list = nullptr; c->uni[l].left_count = nullptr; c->uni[l].left_n = -1;
             c->ubrick_n[l] = 0;
             c->uni_frac_sweep[l] = c->uni_frac_res[l] = 0.0;
             for (int d = 0; d < 3; ++d) C[d] *= c->g[l].c[d];
@@ -261,7 +266,10 @@ static void free_uniform(gmg_ctx* c) {
     c->ubrick_dev = nullptr;
     c->ucount_host = nullptr;
     c->ubrick_total = 0;
-    for (int l = 0; l < GMG_MAX_LEVELS; ++l) { c->uni[l].brick = nullptr; c->ubrick_n[l] = 0; }
+    for (int l = 0; l < GMG_MAX_LEVELS; ++l) {
+        c->uni[l].brick = nullptr; c->ubrick_n[l] = 0;
+        c->uni[l].left_list = nullptr; c->uni[l].left_count = nullptr; c->uni[l].left_n = -1;
+    }
 }
 static cudaError_t alloc_uniform(gmg_ctx* c) {
     free_uniform(c);
@@ -276,15 +284,32 @@ static cudaError_t alloc_uniform(gmg_ctx* c) {
         total += align_up(c->ubrick_n[l], 256);
     }
     if (total == 0) return cudaSuccess;
-    const size_t cbytes = sizeof(unsigned long long) * 2 * GMG_MAX_LEVELS;
-    cudaError_t e = cudaMalloc(&c->ubrick_dev, total + cbytes);
+    const size_t cbytes = kUniCountBytes;
+    size_t loff[GMG_MAX_LEVELS], lbytes[GMG_MAX_LEVELS], ltotal = 0;      // remaining-tile lists of the sweep
+    for (int l = 0; l < c->nlev; ++l) {
+        loff[l] = ltotal;
+        lbytes[l] = 0;
+        int ty = 0, zc = 0;
+        if (c->ubrick_n[l] && gmgf::bulk_sweep_tiling(c->g[l], &ty, &zc)) {
+            const size_t tiles = (size_t)(c->g[l].n[0] / 128) * ((c->g[l].n[1] + ty - 1) / ty) * ((c->g[l].n[2] + zc - 1) / zc);
+            lbytes[l] = align_up(tiles * sizeof(int), 256);
+            ltotal += lbytes[l];
+        }
+    }
+    cudaError_t e = cudaMalloc(&c->ubrick_dev, total + cbytes + ltotal);
     if (e == cudaSuccess) e = cudaMallocHost(&c->ucount_host, cbytes);
     if (e != cudaSuccess) { free_uniform(c); return e; }
     c->ubrick_total = total;
+    unsigned int* lcnt = reinterpret_cast<unsigned int*>(c->ubrick_dev + total + sizeof(unsigned long long) * 2 * GMG_MAX_LEVELS);
     for (int l = 0; l < c->nlev; ++l)
         if (c->ubrick_n[l]) {
             c->uni[l].brick = c->ubrick_dev + off[l];
             c->uni[l].side_stream = c->side[0]; c->uni[l].ev_fork = c->ev_fork[0]; c->uni[l].ev_join = c->ev_join[0];
+            if (lbytes[l]) {
+                c->uni[l].left_list = reinterpret_cast<const int*>(c->ubrick_dev + total + cbytes + loff[l]);
+                c->uni[l].left_count = lcnt + l;
+                c->uni[l].left_n = -1;
+            }
         }
     return cudaSuccess;
 }
@@ -507,16 +532,20 @@ static void set_coeffs_enqueue(gmg_ctx* c, const float* L_dev, cudaStream_t s) {
     // device with the kernels' own footprint test; the counts come down with the next status read
     if (c->ubrick_dev) {
         unsigned long long* cnt = reinterpret_cast<unsigned long long*>(c->ubrick_dev + c->ubrick_total);
-        cudaMemsetAsync(cnt, 0, sizeof(unsigned long long) * 2 * GMG_MAX_LEVELS, s);
+        cudaMemsetAsync(cnt, 0, kUniCountBytes, s);
         for (int l = 0; l < c->nlev; ++l) {
             if (!c->uni[l].brick) continue;
             int ty = 0, zc = 0;
+            // the sweep's pass also lists the tiles that are not lean; until the host has read the
+            // list's length back the launchers size the grid for all tiles (left_n = -1)
+            c->uni[l].left_n = -1;
             if (gmgf::bulk_sweep_tiling(c->g[l], &ty, &zc))
-                gmgk::uniform_cells(c->g[l], c->uni[l].brick, 128, ty, ty + 2, zc, 0, cnt + l, s);
+                gmgk::uniform_cells(c->g[l], c->uni[l].brick, 128, ty, ty + 2, zc, 0, cnt + l,
+                                    const_cast<int*>(c->uni[l].left_list), const_cast<unsigned int*>(c->uni[l].left_count), s);
             if (gmgf::res_bulk_tiling(c->g[l], &ty, &zc))
-                gmgk::uniform_cells(c->g[l], c->uni[l].brick, 128, ty, ty + 1, zc, 1, cnt + GMG_MAX_LEVELS + l, s);
+                gmgk::uniform_cells(c->g[l], c->uni[l].brick, 128, ty, ty + 1, zc, 1, cnt + GMG_MAX_LEVELS + l, nullptr, nullptr, s);
         }
-        cudaMemcpyAsync(c->ucount_host, cnt, sizeof(unsigned long long) * 2 * GMG_MAX_LEVELS, cudaMemcpyDeviceToHost, s);
+        cudaMemcpyAsync(c->ucount_host, cnt, kUniCountBytes, cudaMemcpyDeviceToHost, s);
         c->uni_stats_pending = true;
     }
     gmgk::ctl_set_omega(c->sc, (double)c->prm.omega0, s);
@@ -526,9 +555,11 @@ static void set_coeffs_enqueue(gmg_ctx* c, const float* L_dev, cudaStream_t s) {
 static void refresh_uniform_stats(gmg_ctx* c) {
     if (!c->uni_stats_pending) return;
     c->uni_stats_pending = false;
+    const unsigned int* lcnt = reinterpret_cast<const unsigned int*>(c->ucount_host + 2 * GMG_MAX_LEVELS);
     for (int l = 0; l < c->nlev; ++l) {
         c->uni_frac_sweep[l] = c->uni[l].brick ? (double)c->ucount_host[l] / (double)c->g[l].N : 0.0;
         c->uni_frac_res[l] = c->uni[l].brick ? (double)c->ucount_host[GMG_MAX_LEVELS + l] / (double)c->g[l].N : 0.0;
+        if (c->uni[l].left_list) c->uni[l].left_n = (int)lcnt[l];
     }
 }
 
@@ -929,6 +960,7 @@ static int build_graph(gmg_ctx* c, GraphSlot& slot, int solver, float* p, const 
     CUDA_TRY(c, cudaGraphInstantiate(&slot.exec, graph, 0));
     slot.p = p; slot.z = z; slot.solver = solver; slot.tol = tol; slot.maxiter = maxiter;
     slot.hist = c->hist;
+    for (int l = 0; l < GMG_MAX_LEVELS; ++l) slot.left_n[l] = l < c->nlev ? c->uni[l].left_n : -1;
     return GMG_OK;
 }
 
@@ -982,8 +1014,10 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
     CUDA_TRY(c, cudaEventRecord(c->ev0, s));
     if (c->prm.use_graph) {
         GraphSlot& slot = c->slots[solver];
+        bool same_lists = true;   // the launch grids in the graph were sized with these list lengths
+        for (int l = 0; l < c->nlev; ++l) same_lists = same_lists && slot.left_n[l] == c->uni[l].left_n;
         if (!slot.exec || slot.p != p || slot.z != z || slot.tol != tol || slot.maxiter != maxiter ||
-            slot.hist != c->hist) {
+            slot.hist != c->hist || !same_lists) {
             rc = build_graph(c, slot, solver, p, z, tol, maxiter);
             if (rc != GMG_OK) {
                 // leave no stream in capture mode behind

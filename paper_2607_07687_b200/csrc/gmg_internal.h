@@ -126,8 +126,9 @@ void coarsen_coeffs4(const LevelGeom& gf, const float* Lf, float* Lc, bool check
 void divergence4(const LevelGeom& g, const float* u, const float wall_hi[3], float* z, cudaStream_t s);
 void project4(const LevelGeom& g, const float* L, const float* p, float* u, cudaStream_t s);
 // uniform bricks (uniform.cuh): cells of a level on the lean path of a kernel with this tiling
+// left_list / left_count != nullptr: the tiles that are NOT lean are appended to the list
 void uniform_cells(const LevelGeom& g, const unsigned char* brick, int TXc, int TYc, int yhi, int zchunk, int rule,
-                   unsigned long long* out, cudaStream_t s);
+                   unsigned long long* out, int* left_list, unsigned int* left_count, cudaStream_t s);
 void tail_vcycle(const TailArgs& a, size_t smem_bytes, cudaStream_t s);
 // W[f*N + c] = weight of face f (x-lo, x-hi, y-lo, y-hi, z-lo, z-hi) of cell c, wall faces zeroed
 void tail_weights(const LevelGeom& g, const float* L, float* W, cudaStream_t s);

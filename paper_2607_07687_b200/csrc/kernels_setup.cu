@@ -230,7 +230,7 @@ void project4(const LevelGeom& g, const float* L, const float* p, float* u, cuda
 // periodic y axis), rule 1 = the residual pass (tiles inside the domain in y).  out += cells.
 __global__ void __launch_bounds__(128)
 k_uniform_cells(LevelGeom g, const unsigned char* __restrict__ brick, int TXc, int TYc, int yhi, int zchunk, int rule,
-                unsigned long long* __restrict__ out) {
+                unsigned long long* __restrict__ out, int* __restrict__ left_list, unsigned int* __restrict__ left_count) {
     using namespace gmgf;
     const int tiles_x = g.n[0] / TXc, tiles_y = (g.n[1] + TYc - 1) / TYc, nzc = (g.n[2] + zchunk - 1) / zchunk;
     const long long total = (long long)tiles_x * tiles_y * nzc;
@@ -245,17 +245,20 @@ k_uniform_cells(LevelGeom g, const unsigned char* __restrict__ brick, int TXc, i
     } else {
         boxfed = (y0 >= 1) && (y0 + TYc + 1 <= ny);
     }
-    if (!boxfed) return;
-    if (!ub_box_uniform(g, brick, x0 - 2, x0 + TXc + 1, y0 - 2, y0 + yhi, z0 - 2, z1 + 1)) return;
+    if (!boxfed || !ub_box_uniform(g, brick, x0 - 2, x0 + TXc + 1, y0 - 2, y0 + yhi, z0 - 2, z1 + 1)) {
+        // not lean: onto the list of remaining tiles (any order: tiles are independent)
+        if (left_list) left_list[atomicAdd(left_count, 1u)] = (int)t;
+        return;
+    }
     const int rows = min(TYc, ny - y0);
     atomicAdd(out, (unsigned long long)TXc * rows * (z1 - z0));
 }
 
 void uniform_cells(const LevelGeom& g, const unsigned char* brick, int TXc, int TYc, int yhi, int zchunk, int rule,
-                   unsigned long long* out, cudaStream_t s) {
+                   unsigned long long* out, int* left_list, unsigned int* left_count, cudaStream_t s) {
     const int tiles_x = g.n[0] / TXc, tiles_y = (g.n[1] + TYc - 1) / TYc, nzc = (g.n[2] + zchunk - 1) / zchunk;
     const long long total = (long long)tiles_x * tiles_y * nzc;
-    k_uniform_cells<<<(unsigned int)((total + 127) / 128), 128, 0, s>>>(g, brick, TXc, TYc, yhi, zchunk, rule, out);
+    k_uniform_cells<<<(unsigned int)((total + 127) / 128), 128, 0, s>>>(g, brick, TXc, TYc, yhi, zchunk, rule, out, left_list, left_count);
 }
 
 }  // namespace gmgk

@@ -84,6 +84,7 @@ struct BulkArgs {
     int first_colour;
     int zchunk;
     int tiles_x, tiles_y;
+    int ntiles;            // tiles of the level = tickets of a norm-carrying sweep (lean + remaining kernel)
     // NORM variant: sums over the tile cells of r^2 (r = b - A src on active cells: the residual of
     // the SOURCE iterate) and of b^2 on active cells, into rb.sc->red[slot_rr / slot_ref]
     ReduceBuf rb;
@@ -168,7 +169,7 @@ __device__ __forceinline__ float4 update_pair_full(float xm, float4 own, float x
 // read, the SAME apply7 / diag6 / relax operations run on the constants (bit-identical results;
 // diag6 and the reciprocal are loop-invariant, every cell is active).
 template <class C, int YMODE, int NORM, bool UNI = false>
-__device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& allmaps) {
+__device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& allmaps, const int tile) {
     extern __shared__ __align__(1024) float sm[];  // no static shared memory: base is 1 KB aligned
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..NB) step groups, [NB] prologue
     const float** row_base = reinterpret_cast<const float**>(bars + 16);  // row-copy path tables
@@ -181,7 +182,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
     const int tid = threadIdx.x;
     const int warp_id = tid >> 5, lane_id = tid & 31;
     constexpr int NWARP = C::THREADS / 32;
-    int bid = blockIdx.x;
+    int bid = tile;
     const int tx = bid % a.tiles_x;
     bid /= a.tiles_x;
     const int ty = bid % a.tiles_y;
@@ -606,16 +607,16 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
         if (tid == 0) {
             double t0 = 0.0, t1 = 0.0;
             for (int w = 0; w < NWARP; ++w) { t0 += scratch[w]; t1 += scratch[NWARP + w]; }
-            a.rb.partials[blockIdx.x] = t0;
-            a.rb.partials[GMG_REDUCE_MAX_BLOCKS + blockIdx.x] = t1;
+            a.rb.partials[tile] = t0;
+            a.rb.partials[GMG_REDUCE_MAX_BLOCKS + tile] = t1;
             __threadfence();
-            *last = (atomicAdd(a.rb.counter, 1u) == gridDim.x - 1) ? 1 : 0;
+            *last = (atomicAdd(a.rb.counter, 1u) == (unsigned int)a.ntiles - 1u) ? 1 : 0;   // one ticket per TILE
         }
         __syncthreads();
         if (*last) {
             __threadfence();
             double a0 = 0.0, a1 = 0.0;
-            for (unsigned int i = tid; i < gridDim.x; i += C::THREADS) {
+            for (unsigned int i = tid; i < (unsigned int)a.ntiles; i += C::THREADS) {
                 a0 += ((volatile double*)a.rb.partials)[i];
                 a1 += ((volatile double*)a.rb.partials)[GMG_REDUCE_MAX_BLOCKS + i];
             }
@@ -653,9 +654,9 @@ __device__ __forceinline__ int tile_ymode(const BulkArgs& a, int ty) {
 // tile is box-fed and all coefficients the CTA would touch -- tile + ring 2, planes z0-2 .. z1+1 --
 // are the level's constants with no Neumann wall in reach.  Such tiles belong to k_rb_sweep_lean.
 template <class C>
-__device__ __forceinline__ bool tile_is_lean(const BulkArgs& a, int ymode) {
+__device__ __forceinline__ bool tile_is_lean(const BulkArgs& a, int tile, int ymode) {
     if (!a.uni.brick || ymode == 1) return false;
-    int bid = blockIdx.x;
+    int bid = tile;
     const int tx = bid % a.tiles_x;
     bid /= a.tiles_x;
     const int ty = bid % a.tiles_y;
@@ -669,22 +670,29 @@ __device__ __forceinline__ bool tile_is_lean(const BulkArgs& a, int ymode) {
 // the full boxes.  It pays on grids with few tile rows (a 1024 x 384 x 384 channel: -5 % per solve);
 // on a 1024^3 cube the third body costs the interior loop its register allocation (+2.6 % per
 // sweep, measured A/B on one box), so the launcher picks the kernel by the number of tile rows.
-// With uniform bricks marked (a.uni.brick) the lean tiles are k_rb_sweep_lean's: they return here.
+// With uniform bricks marked (a.uni.brick) the lean tiles are k_rb_sweep_lean's; this kernel then
+// runs one CTA per entry of the list of remaining tiles (a.uni.left_list), or -- the list's length
+// not yet known on the host -- over the whole grid, where the lean tiles return at once.
 template <class C, int NORM = 0, bool EDGE = false>
 __global__ void __launch_bounds__(C::THREADS, 1)
 k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     if (a.run_flag && *a.run_flag == 0) return;   // a re-run that turned out not to be needed
-    const int ty = (blockIdx.x / a.tiles_x) % a.tiles_y;
+    int tile = blockIdx.x;
+    if (a.uni.left_list) {
+        if (blockIdx.x >= *a.uni.left_count) return;
+        tile = a.uni.left_list[blockIdx.x];
+    }
+    const int ty = (tile / a.tiles_x) % a.tiles_y;
     const int ymode = tile_ymode<C>(a, ty);
-    if (tile_is_lean<C>(a, ymode)) return;
+    if (!a.uni.left_list && tile_is_lean<C>(a, tile, ymode)) return;
     if (EDGE) {
-        if (ymode == 0) sweep_body<C, 0, NORM>(a, maps);
-        else if (ymode == 2) sweep_body<C, 2, NORM>(a, maps);
-        else sweep_body<C, 1, NORM>(a, maps);
+        if (ymode == 0) sweep_body<C, 0, NORM>(a, maps, tile);
+        else if (ymode == 2) sweep_body<C, 2, NORM>(a, maps, tile);
+        else sweep_body<C, 1, NORM>(a, maps, tile);
     } else {
         const int y0 = ty * C::TY;
-        if ((y0 >= 2) && (y0 + C::TY + 2 <= a.g.n[1])) sweep_body<C, 0, NORM>(a, maps);
-        else sweep_body<C, 1, NORM>(a, maps);
+        if ((y0 >= 2) && (y0 + C::TY + 2 <= a.g.n[1])) sweep_body<C, 0, NORM>(a, maps, tile);
+        else sweep_body<C, 1, NORM>(a, maps, tile);
     }
 }
 
@@ -696,11 +704,12 @@ template <class C, int NORM = 0>
 __global__ void __launch_bounds__(C::THREADS, 2)
 k_rb_sweep_lean(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     if (a.run_flag && *a.run_flag == 0) return;
-    const int ty = (blockIdx.x / a.tiles_x) % a.tiles_y;
+    const int tile = blockIdx.x;
+    const int ty = (tile / a.tiles_x) % a.tiles_y;
     const int ymode = tile_ymode<C>(a, ty);
-    if (!tile_is_lean<C>(a, ymode)) return;
-    if (ymode == 0) sweep_body<C, 0, NORM, true>(a, maps);
-    else sweep_body<C, 2, NORM, true>(a, maps);
+    if (!tile_is_lean<C>(a, tile, ymode)) return;
+    if (ymode == 0) sweep_body<C, 0, NORM, true>(a, maps, tile);
+    else sweep_body<C, 2, NORM, true>(a, maps, tile);
 }
 
 // ---- launchers ------------------------------------------------------------------------------
@@ -849,8 +858,11 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
     int zchunk = 0;
     const unsigned int grid = bulk_grid(g, &zchunk);
     a.zchunk = zchunk;
+    a.ntiles = (int)grid;
     if (grid > GMG_REDUCE_MAX_BLOCKS && norm) return false;
     const int nv = (norm && slot_ref >= 0) ? 2 : (norm ? 1 : 0);
+    // grid of the kernel of the remaining tiles: the list's length where the host knows it
+    const unsigned int gl = (uni.brick && uni.left_list && uni.left_n >= 0) ? (unsigned int)uni.left_n : grid;
     // With uniform bricks marked, two kernels share the grid: k_rb_sweep_lean (two CTAs per SM) takes
     // the lean tiles, k_rb_sweep_bulk the rest.  They touch disjoint tiles of dst, so they run side by
     // side -- the general one first, on a forked stream, so that its few long CTAs are spread over the
@@ -870,14 +882,16 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
         else k_rb_sweep_lean<Lean, 0><<<grid, Lean::THREADS, Lean::SMEM, s>>>(a, maps);
     };
     if (uni.brick && !fork) launch_lean();
-    if (edge) {
-        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, true><<<grid, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
-        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, true><<<grid, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
-        else k_rb_sweep_bulk<Bulk, 0, true><<<grid, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+    if (gl == 0) {
+        // every tile is lean
+    } else if (edge) {
+        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, true><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, true><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+        else k_rb_sweep_bulk<Bulk, 0, true><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
     } else {
-        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, false><<<grid, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
-        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, false><<<grid, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
-        else k_rb_sweep_bulk<Bulk, 0, false><<<grid, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, false><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, false><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+        else k_rb_sweep_bulk<Bulk, 0, false><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
     }
     if (fork) {
         launch_lean();

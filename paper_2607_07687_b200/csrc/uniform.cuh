@@ -25,6 +25,13 @@ static constexpr int kUBX = 32, kUBY = 8, kUBZ = 8;
 struct UniArgs {
     const unsigned char* brick;  // [nbz][nby][nbx] flags of the level; nullptr: lean path disabled
     float ux, uy, uz;            // the level's constants
+    // the tiles of the sweep that are NOT lean, as a compact list (built by gmg_set_coeffs on the
+    // device): the kernel of the remaining tiles launches one CTA per entry instead of a grid full
+    // of CTAs that return at once.  left_n: the count as the host knows it, -1 = not read back yet
+    // (gmg_pressure_step): the kernel then gets the full grid and bounds itself by *left_count.
+    const int* left_list;
+    const unsigned int* left_count;
+    int left_n;
     // host side only: a side stream and two events with which a launcher runs the kernel of the
     // remaining (non-uniform) tiles beside the lean kernel; nullptr = one after the other
     void* side_stream;
