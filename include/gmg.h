@@ -121,6 +121,7 @@ typedef struct {
     double uniform_fraction; /* share of the finest level's cells swept by CTAs on the lean path
                                 (uniform_tiles; 0 when off or when level 0 is not TMA-fed) */
     double bytes_as_run;    /* bytes_algorithmic minus the coefficient bytes the lean path did not move */
+    double uniform_fraction_residual; /* the same share for the residual + restriction pass (its own tiling) */
 } gmg_stats_t;
 
 /* Level table and workspace size for a grid WITHOUT creating a context (host-only: no CUDA call).

@@ -1090,6 +1090,7 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
     // loop entry: one pass over p, z, L -- unless the norms ride on sweeps that run anyway (fused_norm)
     refresh_uniform_stats(c);   // gmg_pressure_step: the flags came down with this solve's status
     st.uniform_fraction = c->uni_frac_sweep[0];
+    st.uniform_fraction_residual = c->uni_frac_res[0];
     if (solver == GMG_GMG_RBGS) {
         const bool fn = fused_norm_active(c);
         st.bytes_algorithmic = (fn ? 0.0 : 20.0 * N0) + it * vcycle_bytes(c, !fn);

@@ -11,6 +11,8 @@
 // protects ring-slot reuse.  The x pair and y pair sums of the restriction happen in registers,
 // the z pair across two consecutive steps, in stencil.cuh's canonical tree order, so the result is
 // bit-identical to the generic kernel.  112 KB of shared memory per CTA: two CTAs per SM.
+#include <type_traits>
+
 #include "fused_common.cuh"
 #include "uniform.cuh"
 
@@ -24,8 +26,12 @@ extern EncodeTiledFn g_encode;
 bool tensor_map(const float* ptr, const LevelGeom& g, int bw, int bh, CUtensorMap* out);
 bool bulk_supported(const LevelGeom& g);
 
-struct ResBulkCfg {
-    static constexpr int TX = 128, RY = 16, PD = 2;
+// LEAN_: ring layout of the lean path (uniform.cuh) -- no coefficient rings, so the same 112 KB hold a
+// deeper pipeline of the two streams that are left (PD = 5 steps of 18 KB in flight instead of 2).
+template <int PD_, bool LEAN_>
+struct ResBulkCfgT {
+    static constexpr int TX = 128, RY = 16, PD = PD_;
+    static constexpr bool LEAN = LEAN_;
     static constexpr int THREADS = 32 * RY / 2;   // 256: a thread owns two rows
     static constexpr int PH = RY + 2;             // rows of a p plane (halo 1)
     static constexpr int NP = PD + 2, NZ = PD + 1, NC = PD, NB = PD + 1;
@@ -35,11 +41,12 @@ struct ResBulkCfg {
     static constexpr int Y_PLANE = (RY + 1) * TX;
     static constexpr int OFF_P = 0;
     static constexpr int OFF_LZ = OFF_P + NP * P_PLANE;
-    static constexpr int OFF_LX = OFF_LZ + NZ * C_PLANE;
-    static constexpr int OFF_LY = OFF_LX + NC * C_PLANE;
-    static constexpr int OFF_B = OFF_LY + NC * Y_PLANE;
+    static constexpr int OFF_LX = OFF_LZ + (LEAN ? 0 : NZ * C_PLANE);
+    static constexpr int OFF_LY = OFF_LX + (LEAN ? 0 : NC * C_PLANE);
+    static constexpr int OFF_B = OFF_LY + (LEAN ? 0 : NC * Y_PLANE);
     static constexpr int FLOATS = OFF_B + NC * C_PLANE;
     static constexpr size_t SMEM = (size_t)FLOATS * sizeof(float) + 16 * sizeof(uint64_t);
+    static_assert(NB + 1 <= 16, "mbarriers");
     static constexpr uint32_t P_BYTES = (uint32_t)(PH * TX + 2 * PH * 4) * 4u;
     static constexpr uint32_t STEP_BYTES = P_BYTES + (uint32_t)(3 * RY * TX + (RY + 1) * TX) * 4u;
     static constexpr uint32_t PRO_BYTES = 2 * P_BYTES + (uint32_t)(RY * TX) * 4u;
@@ -47,6 +54,9 @@ struct ResBulkCfg {
     static constexpr uint32_t STEP_BYTES_UNI = P_BYTES + (uint32_t)(RY * TX) * 4u;
     static constexpr uint32_t PRO_BYTES_UNI = 2 * P_BYTES;
 };
+using ResBulkCfg = ResBulkCfgT<2, false>;
+using ResLeanCfg = ResBulkCfgT<5, true>;
+static_assert(ResLeanCfg::SMEM <= ResBulkCfg::SMEM, "the lean rings live in the general kernel's allocation");
 
 struct ResBulkArgs {
     LevelGeom g;
@@ -71,7 +81,7 @@ struct alignas(64) ResBulkMaps {
 // neither copied nor read; the same apply7 / diag6 operations run on the level's constants.
 template <int MODE, bool UNI>
 __device__ __forceinline__ void res_body(const ResBulkArgs& a, const ResBulkMaps& maps) {
-    using C = ResBulkCfg;
+    using C = typename std::conditional<UNI, ResLeanCfg, ResBulkCfg>::type;
     extern __shared__ __align__(128) float sm[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..NB) steps, [NB] prologue
     const LevelGeom& g = a.g;

@@ -43,7 +43,8 @@ class Stats(C.Structure):
                 ("resid_init_rel", C.c_double), ("resid_final_rel", C.c_double),
                 ("gpu_ms", C.c_double), ("bytes_algorithmic", C.c_double),
                 ("kernel_launches", C.c_longlong), ("history_len", C.c_int),
-                ("uniform_fraction", C.c_double), ("bytes_as_run", C.c_double)]
+                ("uniform_fraction", C.c_double), ("bytes_as_run", C.c_double),
+                ("uniform_fraction_residual", C.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -53,7 +53,7 @@ def test_struct_sizes_match_header(libpath):
     """Params / Stats mirror the C structs (16 x 4 bytes; Stats has 8-byte alignment)."""
     from paper_2607_07687_b200 import gmg
     assert C.sizeof(gmg.Params) == 64
-    assert C.sizeof(gmg.Stats) == 4 * 4 + 6 * 8 + 8 + 8 + 2 * 8
+    assert C.sizeof(gmg.Stats) == 4 * 4 + 6 * 8 + 8 + 8 + 3 * 8
     p = gmg.Params()
     gmg.lib.gmg_default_params(C.byref(p))
     assert (p.nu_pre, p.nu_post, p.nu_coarse, p.n_min) == (2, 2, 32, 4)
