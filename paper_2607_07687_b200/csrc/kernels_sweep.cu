@@ -27,6 +27,7 @@
 #include <map>
 #include <mutex>
 #include <tuple>
+#include <type_traits>
 
 #include "fused_common.cuh"
 #include "uniform.cuh"
@@ -48,8 +49,9 @@ struct BulkCfg {
     // Lx/Ly/b plane u.  Still to come are planes u..u+PD (+1 for p, whose group runs one ahead).
     static constexpr int NP = PD + 2;
     static constexpr int NZ = PD + 1;
-    static constexpr int NC = PD;
-    static constexpr int NB = PD + 1;            // mbarriers of the step groups
+    // (the lean layout gives every ring the period of the p ring: sweep_lean.cuh unrolls over it)
+    static constexpr int NC = LEAN ? PD + 2 : PD;
+    static constexpr int NB = LEAN ? PD + 2 : PD + 1;   // mbarriers of the step groups
     static constexpr int HPAD = (SH * 4 + 31) / 32 * 32;  // one halo column group, padded to 128 B
     static constexpr int P_HL = SH * TX;                   // p slot: main | left halo | right halo
     static constexpr int P_HR = P_HL + HPAD;
@@ -639,6 +641,10 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
     }
 }
 
+}  // namespace gmgf
+#include "sweep_lean.cuh"
+namespace gmgf {
+
 // How a tile's planes reach shared memory: 0 = full boxes (inside the domain in y, or walls in y:
 // rows outside arrive zero-filled), 2 = first / final tile row of a periodic y axis: boundary boxes
 // plus a few row copies, 1 = row copies only (odd cases: a single tile row, a final row too short).
@@ -708,8 +714,8 @@ k_rb_sweep_lean(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     const int ty = (tile / a.tiles_x) % a.tiles_y;
     const int ymode = tile_ymode<C>(a, ty);
     if (!tile_is_lean<C>(a, tile, ymode)) return;
-    if (ymode == 0) sweep_body<C, 0, NORM, true>(a, maps, tile);
-    else sweep_body<C, 2, NORM, true>(a, maps, tile);
+    if (ymode == 0) lean_body<C, 0, NORM>(a, maps, tile);
+    else lean_body<C, 2, NORM>(a, maps, tile);
 }
 
 // ---- launchers ------------------------------------------------------------------------------
