@@ -166,11 +166,8 @@ __device__ __forceinline__ float4 update_pair_full(float xm, float4 own, float x
 // (was) YIN: the tile's TMA boxes stay inside the domain in y (every tile but the first and last
 // tile rows); the other instantiation carries the row-copy path, so the common one stays small.
 // NORM: 0 = plain sweep; 1 = also sum r^2 of the source iterate; 2 = also sum b^2 over active cells
-// UNI: the lean path of uniform.cuh -- every coefficient this CTA would read equals the level's
-// constant of its direction and no wall is near: the Lz / Lx / Ly streams are neither copied nor
-// read, the SAME apply7 / diag6 / relax operations run on the constants (bit-identical results;
-// diag6 and the reciprocal are loop-invariant, every cell is active).
-template <class C, int YMODE, int NORM, bool UNI = false>
+// (Tiles whose coefficients are the level's constants take lean_body, sweep_lean.cuh, instead.)
+template <class C, int YMODE, int NORM>
 __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& allmaps, const int tile) {
     extern __shared__ __align__(1024) float sm[];  // no static shared memory: base is 1 KB aligned
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..NB) step groups, [NB] prologue
@@ -215,11 +212,8 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
     const uint32_t e_pbytes = (uint32_t)((y_first ? C::SH : hP + 2) * (C::TX + 8)) * 4u;
     const uint32_t e_cbytes = (uint32_t)((y_first ? C::ROWS : hC + 1) * C::TX) * 4u;
     const uint32_t e_lybytes = (uint32_t)((y_first ? C::ROWS + 1 : hC + 2) * C::TX) * 4u;
-    const uint32_t step_bytes = UNI ? ((YMODE == 2) ? e_pbytes + e_cbytes : C::STEP_BYTES_UNI)
-                                    : ((YMODE == 2) ? e_pbytes + 3u * e_cbytes + e_lybytes : C::STEP_BYTES);
-    const uint32_t pro_bytes = UNI ? ((YMODE == 2) ? 2u * e_pbytes : C::PRO_BYTES_UNI)
-                                   : ((YMODE == 2) ? 2u * e_pbytes + e_cbytes : C::PRO_BYTES);
-    static_assert(!UNI || YMODE != 1, "the lean path is built for box-fed tiles only");
+    const uint32_t step_bytes = (YMODE == 2) ? e_pbytes + 3u * e_cbytes + e_lybytes : C::STEP_BYTES;
+    const uint32_t pro_bytes = (YMODE == 2) ? 2u * e_pbytes + e_cbytes : C::PRO_BYTES;
     const float* Lx = a.L;
     const float* Ly = a.L + N;
     const float* Lz = a.L + 2 * N;
@@ -276,9 +270,9 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                 case 0: tma_load_3d(slotP(vp), &maps.p_main, x0, y0 - 2, gzv, bar); break;
                 case 1: tma_load_3d(slotP(vp) + C::P_HL, &maps.p_halo, xL, y0 - 2, gzv, bar); break;
                 case 2: tma_load_3d(slotP(vp) + C::P_HR, &maps.p_halo, xR, y0 - 2, gzv, bar); break;
-                case 3: if (!UNI) tma_load_3d(slotLz(v + 1), &maps.lz, x0, y0 - 1, gz1, bar); break;
-                case 4: if (!UNI) tma_load_3d(slotLx(v), &maps.lx, x0, y0 - 1, gz0, bar); break;
-                case 5: if (!UNI) tma_load_3d(slotLy(v), &maps.ly, x0, y0 - 1, gz0, bar); break;
+                case 3: tma_load_3d(slotLz(v + 1), &maps.lz, x0, y0 - 1, gz1, bar); break;
+                case 4: tma_load_3d(slotLx(v), &maps.lx, x0, y0 - 1, gz0, bar); break;
+                case 5: tma_load_3d(slotLy(v), &maps.ly, x0, y0 - 1, gz0, bar); break;
                 case 6: tma_load_3d(slotB(v), &maps.b, x0, y0 - 1, gz0, bar); break;
                 default: break;
             }
@@ -288,9 +282,9 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                 case 0: tma_load_3d(slotP(vp) + e_oP * C::TX, &maps.p_main, x0, e_yP, gzv, bar); break;
                 case 1: tma_load_3d(slotP(vp) + C::P_HL + hs + e_oP * 4, &maps.p_halo, xL, e_yP, gzv, bar); break;
                 case 2: tma_load_3d(slotP(vp) + C::P_HR + hs + e_oP * 4, &maps.p_halo, xR, e_yP, gzv, bar); break;
-                case 3: if (!UNI) tma_load_3d(slotLz(v + 1) + e_oC * C::TX, &maps.lz, x0, e_yC, gz1, bar); break;
-                case 4: if (!UNI) tma_load_3d(slotLx(v) + e_oC * C::TX, &maps.lx, x0, e_yC, gz0, bar); break;
-                case 5: if (!UNI) tma_load_3d(slotLy(v) + e_oC * C::TX, &maps.ly, x0, e_yC, gz0, bar); break;
+                case 3: tma_load_3d(slotLz(v + 1) + e_oC * C::TX, &maps.lz, x0, e_yC, gz1, bar); break;
+                case 4: tma_load_3d(slotLx(v) + e_oC * C::TX, &maps.lx, x0, e_yC, gz0, bar); break;
+                case 5: tma_load_3d(slotLy(v) + e_oC * C::TX, &maps.ly, x0, e_yC, gz0, bar); break;
                 case 6: tma_load_3d(slotB(v) + e_oC * C::TX, &maps.b, x0, e_yC, gz0, bar); break;
                 case 7: case 8: {   // the two wrapped p rows
                     const int r = warp_id - 7, j = e_pj0 + r;
@@ -300,10 +294,9 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                     bulk_g2s(d + C::P_HL + hs + j * 4, rb + xL, 16u, bar);
                     bulk_g2s(d + C::P_HR + hs + j * 4, rb + xR, 16u, bar);
                 } break;
-                case 9: if (!UNI) bulk_g2s(slotLz(v + 1) + e_cj * C::TX, Lz + pz1 + (size_t)e_cy * nx + x0, C::TX * 4u, bar); break;
-                case 10: if (!UNI) bulk_g2s(slotLx(v) + e_cj * C::TX, Lx + pz0 + (size_t)e_cy * nx + x0, C::TX * 4u, bar); break;
+                case 9: bulk_g2s(slotLz(v + 1) + e_cj * C::TX, Lz + pz1 + (size_t)e_cy * nx + x0, C::TX * 4u, bar); break;
+                case 10: bulk_g2s(slotLx(v) + e_cj * C::TX, Lx + pz0 + (size_t)e_cy * nx + x0, C::TX * 4u, bar); break;
                 case 11:
-                    if (UNI) break;
                     bulk_g2s(slotLy(v) + e_cj * C::TX, Ly + pz0 + (size_t)e_cy * nx + x0, C::TX * 4u, bar);
                     if (e_ly2) bulk_g2s(slotLy(v) + (e_cj + 1) * C::TX, Ly + pz0 + (size_t)(e_cy + 1) * nx + x0, C::TX * 4u, bar);
                     break;
@@ -340,7 +333,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                     else if (k == 1) tma_load_3d(slotP(v) + C::P_HL, &maps.p_halo, xL, y0 - 2, gv, bar);
                     else tma_load_3d(slotP(v) + C::P_HR, &maps.p_halo, xR, y0 - 2, gv, bar);
                 } else if (warp_id == 6) {
-                    if (!UNI) tma_load_3d(slotLz(z0 - 1), &maps.lz, x0, y0 - 1, gb, bar);
+                    tma_load_3d(slotLz(z0 - 1), &maps.lz, x0, y0 - 1, gb, bar);
                 }
             } else if (YMODE == 2) {
                 const int pl = warp_id / 3, k = warp_id % 3;
@@ -350,7 +343,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                     else if (k == 1) tma_load_3d(slotP(v) + C::P_HL + hs + e_oP * 4, &maps.p_halo, xL, e_yP, gv, bar);
                     else tma_load_3d(slotP(v) + C::P_HR + hs + e_oP * 4, &maps.p_halo, xR, e_yP, gv, bar);
                 } else if (warp_id == 6) {
-                    if (!UNI) tma_load_3d(slotLz(z0 - 1) + e_oC * C::TX, &maps.lz, x0, e_yC, gb, bar);
+                    tma_load_3d(slotLz(z0 - 1) + e_oC * C::TX, &maps.lz, x0, e_yC, gb, bar);
                 } else if (warp_id >= 7 && warp_id <= 10) {      // wrapped p rows of the two planes
                     const int v = z0 - 2 + (warp_id - 7) / 2, r = (warp_id - 7) & 1, j = e_pj0 + r;
                     const float* rb = a.src + (size_t)wrapi(v, nz) * plane + (size_t)(e_py0 + r) * nx;
@@ -359,7 +352,7 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
                     bulk_g2s(d + C::P_HL + hs + j * 4, rb + xL, 16u, bar);
                     bulk_g2s(d + C::P_HR + hs + j * 4, rb + xR, 16u, bar);
                 } else if (warp_id == 11) {
-                    if (!UNI) bulk_g2s(slotLz(z0 - 1) + e_cj * C::TX, Lz + (size_t)gb * plane + (size_t)e_cy * nx + x0, C::TX * 4u, bar);
+                    bulk_g2s(slotLz(z0 - 1) + e_cj * C::TX, Lz + (size_t)gb * plane + (size_t)e_cy * nx + x0, C::TX * 4u, bar);
                 }
             } else {
                 for (int pl = 0; pl < 2; ++pl) copy_p_rows(z0 - 2 + pl, bar);
@@ -414,8 +407,8 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
         // cells (sel, sel+2) of the group are updated: same parity for B(u) and C(u-1); sel is
         // warp-uniform and alternates every step
         int sel = (yl + (z0 - 1) + fc) & 1;
-        float lxh_pf = (!UNI && last_lane) ? __ldg(lxh_row + (size_t)gz * plane) : 0.0f;
-        const bool any_wall = !UNI && (zx_lo || zx_hi || zy_lo || zy_hi || g.bc[2]);
+        float lxh_pf = last_lane ? __ldg(lxh_row + (size_t)gz * plane) : 0.0f;
+        const bool any_wall = zx_lo || zx_hi || zy_lo || zy_hi || g.bc[2];
         // K = the coefficients of the two cells C updates next step, picked out of this step's
         // set (14 floats, not a second full set); q1 / z2 = planes u-1 / u-2 at the own position
         CPair K;
@@ -427,12 +420,6 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
         // the B-updated ones there), and this thread's partial sums
         float zs_a = 0.0f, zs_b = 0.0f, acc_rr = 0.0f, acc_bb = 0.0f;
         CFull Sc;
-        if (UNI) {   // the level's constants; only Sc.b changes from step to step
-            Sc.lx = make_float4(a.uni.ux, a.uni.ux, a.uni.ux, a.uni.ux);
-            Sc.lxh = a.uni.ux;
-            Sc.ly = Sc.lyh = make_float4(a.uni.uy, a.uni.uy, a.uni.uy, a.uni.uy);
-            Sc.lz = Sc.lzh = make_float4(a.uni.uz, a.uni.uz, a.uni.uz, a.uni.uz);
-        }
         float4 own, ym, yp, zp;
         float hvB;
         // Operands of B(u) -- TMA data and source values no other thread changes.  Loaded at the
@@ -440,14 +427,12 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
         // are still to be read, so the 16 warps do not all queue on the shared-memory pipe at once.
         auto load_step = [&]() {
             mbar_wait(bars + kb, kpar);
-            if (!UNI) {
-                Sc.lx = lds4(sm + C::OFF_LX + ic * C::C_PLANE + c_off);
-                const float* Y = sm + C::OFF_LY + ic * C::Y_PLANE + c_off;
-                Sc.ly = lds4(Y);
-                Sc.lyh = lds4(Y + C::TX);
-                Sc.lz = lds4(Z0 + c_off);
-                Sc.lzh = lds4(Z1 + c_off);
-            }
+            Sc.lx = lds4(sm + C::OFF_LX + ic * C::C_PLANE + c_off);
+            const float* Y = sm + C::OFF_LY + ic * C::Y_PLANE + c_off;
+            Sc.ly = lds4(Y);
+            Sc.lyh = lds4(Y + C::TX);
+            Sc.lz = lds4(Z0 + c_off);
+            Sc.lzh = lds4(Z1 + c_off);
             Sc.b = lds4(sm + C::OFF_B + ic * C::C_PLANE + c_off);
             own = lds4(P0 + p_off);
             ym = lds4(P0 + p_off - C::TX);
@@ -461,11 +446,9 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
             const float4 cym = lds4(Pm1 + p_off - C::TX);   // plane u-1, B-updated rows above / below
             const float4 cyp = lds4(Pm1 + p_off + C::TX);
             const float hvC = Pm1[h_off];
-            if (!UNI) {
-                const float t = __shfl_down_sync(0xffffffffu, Sc.lx.x, 1);
-                Sc.lxh = last_lane ? lxh_pf : t;
-                if (last_lane && u + 1 <= z1) lxh_pf = __ldg(lxh_row + (size_t)gzp * plane);
-            }
+            const float t = __shfl_down_sync(0xffffffffu, Sc.lx.x, 1);
+            Sc.lxh = last_lane ? lxh_pf : t;
+            if (last_lane && u + 1 <= z1) lxh_pf = __ldg(lxh_row + (size_t)gzp * plane);
             if (any_wall) {   // Neumann wall faces carry coefficient 0 (reading O2)
                 if (zx_lo) Sc.lx.x = 0.0f;
                 if (zx_hi) Sc.lxh = 0.0f;
@@ -557,11 +540,6 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
         auto fetch_e = [&](int gzc, ESet& s) {  // global loads, issued one step ahead
             const int gzn = (gzc + 1 == nz) ? 0 : gzc + 1;
             const size_t pz = (size_t)gzc * plane, pzp = (size_t)gzn * plane;
-            if (UNI) {
-                s.wxl = s.wxh = a.uni.ux; s.wyl = s.wyh = a.uni.uy; s.wzl = s.wzh = a.uni.uz;
-                s.b = __ldg(a.b + pz + o_c);
-                return;
-            }
             s.wxl = ex_lo ? 0.0f : __ldg(Lx + pz + o_c);
             s.wxh = ex_hi ? 0.0f : __ldg(Lx + pz + o_x1);
             s.wyl = ey_lo ? 0.0f : __ldg(Ly + pz + o_c);
