@@ -21,8 +21,6 @@
 // bulk-copy path (cp.async.bulk, UBLKCP) with wrapped row addresses.  Neumann walls = zeroed
 // coefficients.  Every shared-memory cell holds the periodic image of its cell, as in k_rb_sweep.
 #include <cuda.h>
-#include <stdio.h>
-#include <stdlib.h>
 
 #include <map>
 #include <mutex>
@@ -912,11 +910,6 @@ int configure() {
         e = cudaFuncSetAttribute(k_rb_sweep_lean<Lean, 1>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_rb_sweep_lean<Lean, 2>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    if (e == cudaSuccess && getenv("GMG_DEBUG_OCC")) {
-        int nb = -1;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_rb_sweep_lean<Lean, 0>, Lean::THREADS, Lean::SMEM);
-        fprintf(stderr, "[gmg] k_rb_sweep_lean: %d CTAs/SM, smem %zu\n", nb, (size_t)Lean::SMEM);
-    }
     if (e == cudaSuccess && !g_encode) {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult qres;
