@@ -157,6 +157,74 @@ __device__ __forceinline__ float4 update_pair_full(float xm, float4 own, float x
     return update_pair<S>(xm, own, xp, ym, yp, zm, zp, s, c.lz, omega);
 }
 
+// Finish of a norm-carrying sweep: deterministic two-stage reduction, FP64 from the warp on, the
+// same for every kernel that contributes (sweep_body with one row per warp, lean_body2 with two rows
+// per warp, whatever their CTA sizes), so that the sums do not depend on which kernel a tile ran in
+// or which CTA comes last.  Per tile: one partial per phase-B ROW (16 slots; a warp fills the slot(s)
+// of its row(s)), added in row order.  Across tiles: the first 256 threads of the last CTA add the
+// tile partials with stride 256.  Callers have passed a CTA barrier since their last ring access.
+template <int NORM>
+__device__ __forceinline__ void norm_finish(const BulkArgs& a, const int tile, float rr0, float bb0, float rr1,
+                                            float bb1, const bool two_rows, float* sm) {
+    const int tid = threadIdx.x, warp_id = tid >> 5, lane_id = tid & 31;
+    double v0 = (double)rr0, w0 = (double)bb0, v1 = (double)rr1, w1 = (double)bb1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        v0 += __shfl_down_sync(0xffffffffu, v0, o);
+        w0 += __shfl_down_sync(0xffffffffu, w0, o);
+        if (two_rows) {
+            v1 += __shfl_down_sync(0xffffffffu, v1, o);
+            w1 += __shfl_down_sync(0xffffffffu, w1, o);
+        }
+    }
+    double* scratch = reinterpret_cast<double*>(sm);   // [0..16) sum r^2 per row, [16..32) sum b^2 per row
+    int* last = reinterpret_cast<int*>(scratch + 32);
+    if (lane_id == 0) {
+        if (two_rows) {
+            if (2 * warp_id + 1 < 16) {
+                scratch[2 * warp_id] = v0; scratch[16 + 2 * warp_id] = w0;
+                scratch[2 * warp_id + 1] = v1; scratch[16 + 2 * warp_id + 1] = w1;
+            }
+        } else if (warp_id < 16) {
+            scratch[warp_id] = v0; scratch[16 + warp_id] = w0;
+        }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        double t0 = 0.0, t1 = 0.0;
+        for (int r = 0; r < 16; ++r) { t0 += scratch[r]; t1 += scratch[16 + r]; }
+        a.rb.partials[tile] = t0;
+        a.rb.partials[GMG_REDUCE_MAX_BLOCKS + tile] = t1;
+        __threadfence();
+        *last = (atomicAdd(a.rb.counter, 1u) == (unsigned int)a.ntiles - 1u) ? 1 : 0;   // one ticket per TILE
+    }
+    __syncthreads();
+    if (*last) {
+        __threadfence();
+        double a0 = 0.0, a1 = 0.0;
+        if (tid < 256)
+            for (unsigned int i = tid; i < (unsigned int)a.ntiles; i += 256u) {
+                a0 += ((volatile double*)a.rb.partials)[i];
+                a1 += ((volatile double*)a.rb.partials)[GMG_REDUCE_MAX_BLOCKS + i];
+            }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a0 += __shfl_down_sync(0xffffffffu, a0, o);
+            a1 += __shfl_down_sync(0xffffffffu, a1, o);
+        }
+        __syncthreads();
+        if (lane_id == 0 && warp_id < 8) { scratch[warp_id] = a0; scratch[16 + warp_id] = a1; }
+        __syncthreads();
+        if (tid == 0) {
+            double t0 = 0.0, t1 = 0.0;
+            for (int w = 0; w < 8; ++w) { t0 += scratch[w]; t1 += scratch[16 + w]; }
+            a.rb.sc->red[a.slot_rr] = t0;
+            if (NORM == 2) a.rb.sc->red[a.slot_ref] = t1;
+            *a.rb.counter = 0u;
+        }
+    }
+}
+
 // YMODE 0: full TMA boxes.  YMODE 1: row-by-row bulk copies with wrapped row addresses (odd cases
 // of a periodic y axis).  YMODE 2: first / final tile row of a periodic y axis -- shorter boxes over
 // the rows inside the domain plus row copies for the two or three wrapped rows of each stream;
@@ -569,56 +637,12 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
             advance();
         }
     }
-    if (NORM) {
-        // deterministic two-stage reduction (FP64 from here on); the plane rings are free now
-        double v0 = 0.0, v1 = 0.0;
-        if (tid < C::MAIN) { v0 = (double)acc_rr_out; v1 = (double)acc_bb_out; }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            v0 += __shfl_down_sync(0xffffffffu, v0, o);
-            v1 += __shfl_down_sync(0xffffffffu, v1, o);
-        }
-        double* scratch = reinterpret_cast<double*>(sm);
-        int* last = reinterpret_cast<int*>(scratch + 2 * NWARP);
-        if (lane_id == 0) { scratch[warp_id] = v0; scratch[NWARP + warp_id] = v1; }
-        __syncthreads();
-        if (tid == 0) {
-            double t0 = 0.0, t1 = 0.0;
-            for (int w = 0; w < NWARP; ++w) { t0 += scratch[w]; t1 += scratch[NWARP + w]; }
-            a.rb.partials[tile] = t0;
-            a.rb.partials[GMG_REDUCE_MAX_BLOCKS + tile] = t1;
-            __threadfence();
-            *last = (atomicAdd(a.rb.counter, 1u) == (unsigned int)a.ntiles - 1u) ? 1 : 0;   // one ticket per TILE
-        }
-        __syncthreads();
-        if (*last) {
-            __threadfence();
-            double a0 = 0.0, a1 = 0.0;
-            for (unsigned int i = tid; i < (unsigned int)a.ntiles; i += C::THREADS) {
-                a0 += ((volatile double*)a.rb.partials)[i];
-                a1 += ((volatile double*)a.rb.partials)[GMG_REDUCE_MAX_BLOCKS + i];
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                a0 += __shfl_down_sync(0xffffffffu, a0, o);
-                a1 += __shfl_down_sync(0xffffffffu, a1, o);
-            }
-            __syncthreads();
-            if (lane_id == 0) { scratch[warp_id] = a0; scratch[NWARP + warp_id] = a1; }
-            __syncthreads();
-            if (tid == 0) {
-                double t0 = 0.0, t1 = 0.0;
-                for (int w = 0; w < NWARP; ++w) { t0 += scratch[w]; t1 += scratch[NWARP + w]; }
-                a.rb.sc->red[a.slot_rr] = t0;
-                if (NORM == 2) a.rb.sc->red[a.slot_ref] = t1;
-                *a.rb.counter = 0u;
-            }
-        }
-    }
+    if (NORM) norm_finish<NORM>(a, tile, acc_rr_out, acc_bb_out, 0.0f, 0.0f, false, sm);
 }
 
 }  // namespace gmgf
 #include "sweep_lean.cuh"
+#include "sweep_lean2.cuh"
 namespace gmgf {
 
 // How a tile's planes reach shared memory: 0 = full boxes (inside the domain in y, or walls in y:
@@ -683,15 +707,15 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
 // needs 88 KB of shared memory and 64 registers per thread, so TWO CTAs share an SM and one fills
 // the other's barrier and latency gaps (issue slots 44 % -> 69 % busy).
 template <class C, int NORM = 0>
-__global__ void __launch_bounds__(C::THREADS, 2)
+__global__ void __launch_bounds__(kLean2Threads, 2)
 k_rb_sweep_lean(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     if (a.run_flag && *a.run_flag == 0) return;
     const int tile = blockIdx.x;
     const int ty = (tile / a.tiles_x) % a.tiles_y;
     const int ymode = tile_ymode<C>(a, ty);
     if (!tile_is_lean<C>(a, tile, ymode)) return;
-    if (ymode == 0) lean_body<C, 0, NORM>(a, maps, tile);
-    else lean_body<C, 2, NORM>(a, maps, tile);
+    if (ymode == 0) lean_body2<C, 0, NORM>(a, maps, tile);
+    else lean_body2<C, 2, NORM>(a, maps, tile);
 }
 
 // ---- launchers ------------------------------------------------------------------------------
@@ -859,9 +883,9 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
         cudaStreamWaitEvent(sg, (cudaEvent_t)uni.ev_fork, 0);
     }
     auto launch_lean = [&]() {
-        if (nv == 2) k_rb_sweep_lean<Lean, 2><<<grid, Lean::THREADS, Lean::SMEM, s>>>(a, maps);
-        else if (nv == 1) k_rb_sweep_lean<Lean, 1><<<grid, Lean::THREADS, Lean::SMEM, s>>>(a, maps);
-        else k_rb_sweep_lean<Lean, 0><<<grid, Lean::THREADS, Lean::SMEM, s>>>(a, maps);
+        if (nv == 2) k_rb_sweep_lean<Lean, 2><<<grid, kLean2Threads, Lean::SMEM, s>>>(a, maps);
+        else if (nv == 1) k_rb_sweep_lean<Lean, 1><<<grid, kLean2Threads, Lean::SMEM, s>>>(a, maps);
+        else k_rb_sweep_lean<Lean, 0><<<grid, kLean2Threads, Lean::SMEM, s>>>(a, maps);
     };
     if (uni.brick && !fork) launch_lean();
     if (gl == 0) {

@@ -27,7 +27,6 @@ __device__ __forceinline__ void lean_body(const BulkArgs& a, const BulkMaps& all
     const int plane = nx * ny;
     const int tid = threadIdx.x;
     const int warp_id = tid >> 5, lane_id = tid & 31;
-    constexpr int NWARP = C::THREADS / 32;
     int bid = tile;
     const int tx = bid % a.tiles_x;
     bid /= a.tiles_x;
@@ -293,53 +292,7 @@ __device__ __forceinline__ void lean_body(const BulkArgs& a, const BulkMaps& all
             if (++jb == R) { jb = 0; kpar ^= 1u; }
         }
     }
-    if (NORM) {
-        // deterministic two-stage reduction (FP64 from here on), as in sweep_body: the two kernels
-        // share the partial sums and the ticket counter
-        double v0 = 0.0, v1 = 0.0;
-        if (tid < C::MAIN) { v0 = (double)acc_rr_out; v1 = (double)acc_bb_out; }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            v0 += __shfl_down_sync(0xffffffffu, v0, o);
-            v1 += __shfl_down_sync(0xffffffffu, v1, o);
-        }
-        double* scratch = reinterpret_cast<double*>(sm);
-        int* last = reinterpret_cast<int*>(scratch + 2 * NWARP);
-        if (lane_id == 0) { scratch[warp_id] = v0; scratch[NWARP + warp_id] = v1; }
-        __syncthreads();
-        if (tid == 0) {
-            double t0 = 0.0, t1 = 0.0;
-            for (int w = 0; w < NWARP; ++w) { t0 += scratch[w]; t1 += scratch[NWARP + w]; }
-            a.rb.partials[tile] = t0;
-            a.rb.partials[GMG_REDUCE_MAX_BLOCKS + tile] = t1;
-            __threadfence();
-            *last = (atomicAdd(a.rb.counter, 1u) == (unsigned int)a.ntiles - 1u) ? 1 : 0;   // one ticket per TILE
-        }
-        __syncthreads();
-        if (*last) {
-            __threadfence();
-            double a0 = 0.0, a1 = 0.0;
-            for (unsigned int i = tid; i < (unsigned int)a.ntiles; i += C::THREADS) {
-                a0 += ((volatile double*)a.rb.partials)[i];
-                a1 += ((volatile double*)a.rb.partials)[GMG_REDUCE_MAX_BLOCKS + i];
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                a0 += __shfl_down_sync(0xffffffffu, a0, o);
-                a1 += __shfl_down_sync(0xffffffffu, a1, o);
-            }
-            __syncthreads();
-            if (lane_id == 0) { scratch[warp_id] = a0; scratch[NWARP + warp_id] = a1; }
-            __syncthreads();
-            if (tid == 0) {
-                double t0 = 0.0, t1 = 0.0;
-                for (int w = 0; w < NWARP; ++w) { t0 += scratch[w]; t1 += scratch[NWARP + w]; }
-                a.rb.sc->red[a.slot_rr] = t0;
-                if (NORM == 2) a.rb.sc->red[a.slot_ref] = t1;
-                *a.rb.counter = 0u;
-            }
-        }
-    }
+    if (NORM) norm_finish<NORM>(a, tile, acc_rr_out, acc_bb_out, 0.0f, 0.0f, false, sm);
 }
 
 }  // namespace gmgf
