@@ -47,7 +47,7 @@ struct BulkCfg {
     // Lx/Ly/b plane u.  Still to come are planes u..u+PD (+1 for p, whose group runs one ahead).
     static constexpr int NP = PD + 2;
     static constexpr int NZ = PD + 1;
-    // (the lean layout gives every ring the period of the p ring: sweep_lean.cuh unrolls over it)
+    // (the lean layout gives every ring the period of the p ring: one cursor rotation serves all, sweep_lean2.cuh)
     static constexpr int NC = LEAN ? PD + 2 : PD;
     static constexpr int NB = LEAN ? PD + 2 : PD + 1;   // mbarriers of the step groups
     static constexpr int HPAD = (SH * 4 + 31) / 32 * 32;  // one halo column group, padded to 128 B
@@ -232,7 +232,7 @@ __device__ __forceinline__ void norm_finish(const BulkArgs& a, const int tile, f
 // (was) YIN: the tile's TMA boxes stay inside the domain in y (every tile but the first and last
 // tile rows); the other instantiation carries the row-copy path, so the common one stays small.
 // NORM: 0 = plain sweep; 1 = also sum r^2 of the source iterate; 2 = also sum b^2 over active cells
-// (Tiles whose coefficients are the level's constants take lean_body, sweep_lean.cuh, instead.)
+// (Tiles whose coefficients are the level's constants take lean_body2, sweep_lean2.cuh, instead.)
 template <class C, int YMODE, int NORM>
 __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& allmaps, const int tile) {
     extern __shared__ __align__(1024) float sm[];  // no static shared memory: base is 1 KB aligned
@@ -641,7 +641,6 @@ __device__ __forceinline__ void sweep_body(const BulkArgs& a, const BulkMaps& al
 }
 
 }  // namespace gmgf
-#include "sweep_lean.cuh"
 #include "sweep_lean2.cuh"
 namespace gmgf {
 
@@ -707,15 +706,15 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
 // needs 88 KB of shared memory and 64 registers per thread, so TWO CTAs share an SM and one fills
 // the other's barrier and latency gaps (issue slots 44 % -> 69 % busy).
 template <class C, int NORM = 0>
-__global__ void __launch_bounds__(kLean2Threads, 2)
+__global__ void __launch_bounds__(Lean2Threads<(NORM != 0)>::value, 2)
 k_rb_sweep_lean(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     if (a.run_flag && *a.run_flag == 0) return;
     const int tile = blockIdx.x;
     const int ty = (tile / a.tiles_x) % a.tiles_y;
     const int ymode = tile_ymode<C>(a, ty);
     if (!tile_is_lean<C>(a, tile, ymode)) return;
-    if (ymode == 0) lean_body2<C, 0, NORM>(a, maps, tile);
-    else lean_body2<C, 2, NORM>(a, maps, tile);
+    if (ymode == 0) lean_body2<C, 0, NORM, (NORM != 0)>(a, maps, tile);
+    else lean_body2<C, 2, NORM, (NORM != 0)>(a, maps, tile);
 }
 
 // ---- launchers ------------------------------------------------------------------------------
@@ -883,9 +882,9 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
         cudaStreamWaitEvent(sg, (cudaEvent_t)uni.ev_fork, 0);
     }
     auto launch_lean = [&]() {
-        if (nv == 2) k_rb_sweep_lean<Lean, 2><<<grid, kLean2Threads, Lean::SMEM, s>>>(a, maps);
-        else if (nv == 1) k_rb_sweep_lean<Lean, 1><<<grid, kLean2Threads, Lean::SMEM, s>>>(a, maps);
-        else k_rb_sweep_lean<Lean, 0><<<grid, kLean2Threads, Lean::SMEM, s>>>(a, maps);
+        if (nv == 2) k_rb_sweep_lean<Lean, 2><<<grid, Lean2Threads<true>::value, Lean::SMEM, s>>>(a, maps);
+        else if (nv == 1) k_rb_sweep_lean<Lean, 1><<<grid, Lean2Threads<true>::value, Lean::SMEM, s>>>(a, maps);
+        else k_rb_sweep_lean<Lean, 0><<<grid, Lean2Threads<false>::value, Lean::SMEM, s>>>(a, maps);
     };
     if (uni.brick && !fork) launch_lean();
     if (gl == 0) {

@@ -1,5 +1,8 @@
-// sweep_lean2.cuh -- lean_body2: the lean sweep (see sweep_lean.cuh, uniform.cuh) with TWO vertically
-// adjacent rows per thread.  The lean sweep is bound by the shared-memory pipe (every cell is read six
+// sweep_lean2.cuh -- lean_body2: the fused red+black sweep of a tile whose coefficients are the level's
+// constants (uniform.cuh), for the kernel that runs ONLY such tiles (k_rb_sweep_lean, two CTAs per SM),
+// with TWO vertically adjacent rows per thread.  Same schedule as sweep_body: per z step B(u) on tile +
+// ring 1 in shared memory, C(u-1) streamed to the destination, one CTA barrier, TMA boxes PD steps ahead;
+// the z loop is unrolled twice so that the colour parity of a step is a compile-time constant.  The lean sweep is bound by the shared-memory pipe (every cell is read six
 // times per sweep and the x-neighbour shuffles share the queue: profiles/r02_top_kernels_c4.md); a
 // thread that owns rows r and r+1 has each row's vertical neighbour in its own registers -- in plane u
 // (source values) for phase B, in plane u-1 (its own phase-B results of the step before) for phase C --
@@ -7,14 +10,18 @@
 // main warps cover the 15 phase-B rows of a 128 x 13 tile (the last thread row has one row only), one
 // edge warp the two ring-1 columns: 288 threads, two CTAs per SM, up to 112 registers, operands of
 // the next step loaded in front of the barrier as in sweep_body.  Same update_pair_* calls on the same
-// operands: bit-identical to sweep_body and lean_body (tests).  Included by kernels_sweep.cu.
+// operands: bit-identical to sweep_body (tests).  Included by kernels_sweep.cu.
 #pragma once
 
 namespace gmgf {
 
-static constexpr int kLean2Threads = 288;
+// RIM = false: 8 main warps + an edge warp (288 threads; 96 registers at two CTAs per SM, a few
+// spills -- the faster shape for the plain sweep: 2.98 vs 3.16 ms at 1024^3); RIM = true: the last
+// main warp, which owns one row only, also updates the ring-1 cells (256 threads, up to 128
+// registers: the norm-carrying variants need them -- 3.66 vs 3.93 ms).
+template <bool RIM> struct Lean2Threads { static constexpr int value = RIM ? 256 : 288; };
 
-template <class C, int YMODE, int NORM>
+template <class C, int YMODE, int NORM, bool RIM>
 __device__ __forceinline__ void lean_body2(const BulkArgs& a, const BulkMaps& allmaps, const int tile) {
     static_assert(C::LEAN && C::PD == 4 && C::NP == 6 && C::NC == 6 && C::NB == 6, "rings of period 6");
     static_assert(YMODE == 0 || YMODE == 2, "box-fed tiles only");
@@ -26,7 +33,7 @@ __device__ __forceinline__ void lean_body2(const BulkArgs& a, const BulkMaps& al
     const int plane = nx * ny;
     const int tid = threadIdx.x;
     const int warp_id = tid >> 5, lane_id = tid & 31;
-    constexpr int NWARP = kLean2Threads / 32;   // 8 main warps (two rows per thread) + the edge warp
+    constexpr int NMAIN = 8;   // main warps, two rows per thread; the last one has ONE row (and, RIM, the edge cells)
     int bid = tile;
     const int tx = bid % a.tiles_x;
     bid /= a.tiles_x;
@@ -138,7 +145,7 @@ __device__ __forceinline__ void lean_body2(const BulkArgs& a, const BulkMaps& al
 
     const float wx = a.uni.ux, wy = a.uni.uy, wz = a.uni.uz;
     float acc_rr_out = 0.0f, acc_bb_out = 0.0f, acc_rr_out2 = 0.0f, acc_bb_out2 = 0.0f;   // NORM: per row
-    if (warp_id < NWARP - 1) {
+    if (warp_id < NMAIN) {
         // ---- main threads: one float4 group of TWO rows, a = 2 warp_id and b = a + 1 (phase-B row
         // indices 0 .. ROWS-1; the last warp's row b does not exist) -----------------------------
         const int lx = lane_id, ra = 2 * warp_id;
@@ -194,6 +201,23 @@ __device__ __forceinline__ void lean_body2(const BulkArgs& a, const BulkMaps& al
         ownb = lds4(pp + o0 + C::TX);
         load_step();
 
+        // The last warp owns one row only (phase-B row 14, the ring row) and also updates the ring-1
+        // CELLS x0-1 and x0+TX of all 15 rows (phase B only; lane = 2 row + side), as sweep_body's edge
+        // warp does: its neighbours are second-colour cells, which phase B leaves alone.
+        const bool rim = RIM && (warp_id == NMAIN - 1);
+        const bool e_act = rim && lane_id < 2 * C::ROWS;
+        const int e_side = lane_id & 1, e_r = (e_act ? (lane_id >> 1) : 0) + 1;
+        const int e_xs = e_side ? x0 + C::TX : x0 - 1, e_yl = y0 + e_r - 2;
+        const int e_pc = hs + (e_side ? C::P_HR + e_r * 4 : C::P_HL + e_r * 4 + 3);   // the edge cell
+        const int e_xm = e_side ? e_r * C::TX + C::TX - 1 : e_pc - 1;               // its x neighbours
+        const int e_xp = e_side ? e_pc + 1 : e_r * C::TX;
+        const float* const e_bptr = a.b + (size_t)wrapi(e_yl, ny) * nx + wrapi(e_xs, nx);
+        int e_gz = wrap1(z0 - 1, nz);
+        float e_b = rim ? __ldg(e_bptr + (size_t)e_gz * plane) : 0.0f, e_bn = e_b;
+        const int e_col0 = (e_xs + e_yl + (z0 - 1)) & 1;   // colour of the edge cell in plane u at t = 0
+        const float e_D = diag6(wx, wx, wy, wy, wz, wz);
+        float* const Pbase = sm + C::OFF_P;
+
         auto step = [&](auto Sc_, const int t) {
             constexpr int SA = decltype(Sc_)::value, SB = SA ^ 1;
             const float4 cym = lds4(pp + oM - C::TX);       // plane u-1, B-updated: row above a
@@ -248,12 +272,15 @@ __device__ __forceinline__ void lean_body2(const BulkArgs& a, const BulkMaps& al
             // phase B on plane u: row a's lower y neighbour is row b and vice versa (source values)
             Sc.b = ba;
             const float4 nwa = update_pair_full<SA>(xma, owna, xpa, ym, ownb, q1a, zpa, Sc, omega);
-            Sc.b = bb;
-            const float4 nwb = update_pair_full<SB>(xmb, ownb, xpb, owna, yp, q1b, zpb, Sc, omega);
+            float4 nwb = ownb, ncb = q1b;
+            if (vb) {   // (warp-uniform: only the last warp has no row b)
+                Sc.b = bb;
+                nwb = update_pair_full<SB>(xmb, ownb, xpb, owna, yp, q1b, zpb, Sc, omega);
+            }
             // phase C on plane u-1: the neighbouring row of the pair is q1 of the other row (phase-B
             // results of the step before, in registers)
             const float4 nca = update_pair_carried<SA>(cxma, q1a, cxpa, cym, q1b, z2a0, z2a1, nwa, Ka, omega);
-            const float4 ncb = update_pair_carried<SB>(cxmb, q1b, cxpb, q1a, cyp, z2b0, z2b1, nwb, Kb, omega);
+            if (vb) ncb = update_pair_carried<SB>(cxmb, q1b, cxpb, q1a, cyp, z2b0, z2b1, nwb, Kb, omega);
             // the next step's C works on the other two cells of plane u
             if (SA) { Ka.ba = ba.x; Ka.bb = ba.z; z2a0 = q1a.x; z2a1 = q1a.z; Kb.ba = bb.y; Kb.bb = bb.w; z2b0 = q1b.y; z2b1 = q1b.w; }
             else { Ka.ba = ba.y; Ka.bb = ba.w; z2a0 = q1a.y; z2a1 = q1a.w; Kb.ba = bb.x; Kb.bb = bb.z; z2b0 = q1b.x; z2b1 = q1b.z; }
@@ -266,6 +293,20 @@ __device__ __forceinline__ void lean_body2(const BulkArgs& a, const BulkMaps& al
             q1a = nwa; q1b = nwb;
             owna = zpa; ownb = zpb;
             dsta += plane; dstb += plane;
+            if (rim) {   // the ring-1 cells of plane u
+                if (t + 1 < T) {   // the next plane's right-hand side, one step ahead
+                    e_gz = (e_gz + 1 == nz) ? 0 : e_gz + 1;
+                    e_bn = __ldg(e_bptr + (size_t)e_gz * plane);
+                }
+                if (e_act && ((e_col0 ^ t) & 1) == fc) {
+                    float* P0 = Pbase + o0;
+                    const float pc = P0[e_pc];
+                    const float Ap = apply7(pc, wx, wx, wy, wy, wz, wz, P0[e_xm], P0[e_xp], P0[e_pc - 4],
+                                            P0[e_pc + 4], Pbase[oM + e_pc], Pbase[oP + e_pc]);
+                    P0[e_pc] = relax(pc, e_b, Ap, e_D, omega);
+                }
+                e_b = e_bn;
+            }
             // rotate the cursors to step t+1 and load its operands in front of the barrier
             const int jb_issue = jb + PD >= R ? jb + PD - R : jb + PD;
             oM = o0; o0 = oP;
@@ -287,7 +328,7 @@ __device__ __forceinline__ void lean_body2(const BulkArgs& a, const BulkMaps& al
         if (par) run(std::integral_constant<int, 1>());
         else run(std::integral_constant<int, 0>());
         if (NORM) { acc_rr_out = acc_rr; acc_bb_out = acc_bb; acc_rr_out2 = acc_rr2; acc_bb_out2 = acc_bb2; }
-    } else {
+    } else {   // (RIM == false only)
         // ---- edge warp: ring-1 cells x0-1 and x0+TX of every row, phase B only ----------------
         const int el = lane_id;
         const bool e_act = el < 2 * C::ROWS;
