@@ -79,7 +79,9 @@ struct alignas(64) ResBulkMaps {
 
 // UNI: the lean path of uniform.cuh (interior tiles in y only) -- the coefficient streams are
 // neither copied nor read; the same apply7 / diag6 operations run on the level's constants.
-template <int MODE, bool UNI>
+// C222: the level coarsens by two in every direction (compile-time factors: no integer divisions
+// in the store of the coarse right-hand side).
+template <int MODE, bool UNI, bool C222 = false>
 __device__ __forceinline__ void res_body(const ResBulkArgs& a, const ResBulkMaps& maps) {
     using C = typename std::conditional<UNI, ResLeanCfg, ResBulkCfg>::type;
     extern __shared__ __align__(128) float sm[];
@@ -99,7 +101,7 @@ __device__ __forceinline__ void res_body(const ResBulkArgs& a, const ResBulkMaps
     const int z0 = zc * a.zchunk;
     const int z1 = min(nz, z0 + a.zchunk);
     const int xL = wrapi(x0 - 4, nx), xR = wrapi(x0 + C::TX, nx);
-    const bool y_inside = (y0 >= 1) && (y0 + C::RY + 1 <= ny);
+    const bool y_inside = UNI || ((y0 >= 1) && (y0 + C::RY + 1 <= ny));   // lean tiles are box-fed by construction
     const float* Lx = a.L;
     const float* Ly = a.L + N;
     const float* Lz = a.L + 2 * N;
@@ -201,7 +203,7 @@ __device__ __forceinline__ void res_body(const ResBulkArgs& a, const ResBulkMaps
     const int c_off = rA * C::TX + 4 * lx;
     const float* const lxhA_row = Lx + (size_t)gyA * nx + gxh;
     const float* const lxhB_row = Lx + (size_t)gyB * nx + gxh;
-    const int cx = g.c[0], cy = g.c[1], cz = g.c[2];
+    const int cx = C222 ? 2 : g.c[0], cy = C222 ? 2 : g.c[1], cz = C222 ? 2 : g.c[2];
     const int ncx = nx / cx, ncy = ny / cy;
 
     // ring cursors
@@ -408,8 +410,12 @@ k_residual_bulk(const ResBulkArgs a, const __grid_constant__ ResBulkMaps maps) {
             uni = ub_box_uniform_warp(a.g, a.uni.brick, x0 - 2, x0 + C::TX + 1, y0 - 2, y0 + C::RY + 1, z0 - 2, z1 + 1,
                                       threadIdx.x & 31);
     }
-    if (uni) res_body<MODE, true>(a, maps);
-    else res_body<MODE, false>(a, maps);
+    if (uni) {
+        if (MODE == 0 && a.g.c[0] == 2 && a.g.c[1] == 2 && a.g.c[2] == 2) res_body<MODE, true, (MODE == 0)>(a, maps);
+        else res_body<MODE, true, false>(a, maps);
+    } else {
+        res_body<MODE, false, false>(a, maps);
+    }
 }
 
 // ---- launchers ------------------------------------------------------------------------------
