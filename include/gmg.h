@@ -256,6 +256,27 @@ int gmg_project(gmg_ctx* ctx, float* u_dev, const float* p_dev, void* stream);
 int gmg_pressure_step(gmg_ctx* ctx, const float* L_dev, float* u_dev, const float wall_hi[3], float* p_dev,
                       float tol, int maxiter, int solver, void* stream);
 
+/* -- one entry point that allocates nothing ---------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid it): out_dev[0] = ||b - A p||_2 over the active cells of an nx*ny*nz grid
+ * with the operator and boundary handling at the top of this file (readings O1, O2; the norm of the
+ * stopping test, reading O9, PAPER.md:39 S3) -- what gmg_op_residual + gmg_op_norm2 compute on level 0,
+ * without a context or a workspace.  L_dev [3][N], p_dev [N], b_dev [N] (float, 4-byte aligned) and
+ * out_dev (one double, 8-byte aligned) are the caller's device memory on the CURRENT device.  The
+ * reduction scratch (one FP64 partial per 2048 cells and a ticket) is a static device array of
+ * 65,792 bytes that every GPU loading the library holds until exit; hence the limit
+ * nx*ny*nz <= GMG_NOALLOC_MAX_CELLS (256^3), larger grids are refused with GMG_EINVAL.
+ * Nothing is allocated or freed and the host is not synchronised: the result is stream-ordered on
+ * `stream`.  The first call on each device looks the array's address up (make that call outside a
+ * capture).  All calls share the array: calls that overlap on the GPU (two streams, two host
+ * threads) race -- serialise them; calls on one stream are safe back to back.  Deterministic (two
+ * stages, fixed order).  err (may be NULL) receives a NUL-terminated message of at most err_cap
+ * bytes when the return code is < 0: GMG_EINVAL bad argument / too large, GMG_ECUDA enqueue failed. */
+#define GMG_NOALLOC_MAX_CELLS 16777216LL
+int gmg_residual_norm2_noalloc(int nx, int ny, int nz, const int bc[3], const float* L_dev,
+                               const float* p_dev, const float* b_dev, double* out_dev, void* stream,
+                               char* err, size_t err_cap);
+
 /* Names of the kernels a V-cycle launches per level, for profiling notes: writes a
  * NUL-terminated description into buf. */
 int gmg_describe_plan(const gmg_ctx* ctx, char* buf, size_t cap);

@@ -12,7 +12,7 @@ LIB = os.path.join(HERE, "libgmg.so")
 SOURCES = ["gmg_api.cu", "kernels_generic.cu", "kernels_reduce.cu", "kernels_ctl.cu",
            "kernels_tail.cu", "kernels_fused.cu", "kernels_sweep.cu", "kernels_residual.cu",
            "kernels_setup.cu", "kernels_ctail.cu",
-           "kernels_pcg4.cu", "kernels_cgs.cu"]
+           "kernels_pcg4.cu", "kernels_cgs.cu", "noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC"]

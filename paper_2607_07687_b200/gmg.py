@@ -95,6 +95,8 @@ SIGNATURES = {
     "gmg_project": (C.c_int, [_vp, _vp, _vp, _vp]),
     "gmg_pressure_step": (C.c_int, [_vp, _vp, _vp, C.POINTER(C.c_float), _vp, C.c_float, C.c_int, C.c_int, _vp]),
     "gmg_describe_plan": (C.c_int, [_vp, C.c_char_p, C.c_size_t]),
+    "gmg_residual_norm2_noalloc": (C.c_int, [C.c_int, C.c_int, C.c_int, _I3, _vp, _vp, _vp, _vp, _vp,
+                                             C.c_char_p, C.c_size_t]),
 }
 
 
@@ -127,6 +129,24 @@ def plan(n, bc, **params):
     shapes = [tuple(out.n[l]) for l in range(out.levels)]
     factors = [tuple(out.c[l]) for l in range(out.levels)]
     return shapes, factors, out.tail_start, out.workspace_bytes
+
+
+NOALLOC_MAX_CELLS = 1 << 24
+
+
+def residual_norm2_noalloc(n, bc, L, p, b, out, stream=None):
+    """out[0] = ||b - A p||_2 over the active cells, through the entry point that allocates nothing
+    (static device scratch; at most NOALLOC_MAX_CELLS cells).  L, p, b: float32 CUDA tensors; out: a
+    float64 CUDA tensor the caller made beforehand.  Stream-ordered, no host synchronisation."""
+    if stream is None:
+        stream = torch.cuda.current_stream(out.device).cuda_stream
+    err = C.create_string_buffer(512)
+    rc = lib.gmg_residual_norm2_noalloc(int(n[0]), int(n[1]), int(n[2]), _I3(*[int(v) for v in bc]),
+                                        _vp(L.data_ptr()), _vp(p.data_ptr()), _vp(b.data_ptr()),
+                                        _vp(out.data_ptr()), _vp(stream), err, 512)
+    if rc != OK:
+        raise GMGError(rc, err.value.decode())
+    return out
 
 
 class GMGError(RuntimeError):
