@@ -34,6 +34,7 @@ bool matvec_dot_bulk(const LevelGeom& g, const float* L, const float* d, float* 
 bool bulk_sweep_tiling(const LevelGeom& g, int* tile_y, int* zchunk);
 bool res_bulk_tiling(const LevelGeom& g, int* tile_y, int* zchunk);
 bool tma_shape_ok(const LevelGeom& g);
+bool sweep_fuses_prolong(const LevelGeom& g, const UniArgs& uni);
 bool bulk_sweep_edge(const LevelGeom& g, bool norm);
 // one TMA-fed sweep src -> dst that also leaves sum r^2 (r = b - A src) and sum b^2 over the active
 // cells in red[slot_rr] / red[slot_ref]; false = the level cannot run it (nothing launched)
@@ -95,6 +96,7 @@ struct gmg_ctx {
     size_t ws_bytes;
     bool ws_set, coeffs_set;
     float *pcg_r, *pcg_d, *pcg_q, *pcg_s, *stage_p, *stage_z;
+    float* uni_scratch;   // level-0-sized: corrected iterate over the non-lean tiles (uniform.cuh, PRO)
     float* tail_W[GMG_MAX_LEVELS];  // [6][N] face weights of the tail levels
     // small library-owned device state
     DevScalars* sc;
@@ -213,6 +215,7 @@ static void build_levels(gmg_ctx* c) {
             c->uni[l].brick = nullptr;
             c->uni[l].side_stream = c->uni[l].ev_fork = c->uni[l].ev_join = nullptr;
             c->uni[l].left_list = nullptr; c->uni[l].left_count = nullptr; c->uni[l].left_n = -1;
+            c->uni[l].scratch = nullptr;
             c->ubrick_n[l] = 0;
             c->uni_frac_sweep[l] = c->uni_frac_res[l] = 0.0;
             for (int d = 0; d < 3; ++d) C[d] *= c->g[l].c[d];
@@ -256,6 +259,19 @@ static size_t carve(gmg_ctx* c, char* base) {
         c->pcg_r = v[0]; c->pcg_d = v[1]; c->pcg_q = v[2]; c->pcg_s = v[3];
         c->stage_p = v[4]; c->stage_z = v[5];
     }
+    // the sweep that folds the prolongation in (gmgf::sweep_fuses_prolong) leaves p + P e_c of the
+    // non-lean tiles here: as large as the largest level that can take that path (host-side test of
+    // the shape the TMA kernels accept, so that gmg_plan gives the same size without a GPU)
+    size_t nscr = 0;
+    if (c->prm.uniform_tiles && c->prm.fast_path)
+        for (int l = 0; l + 1 < c->nlev && l < c->tail_start && l < c->ctail_start; ++l) {
+            const LevelGeom& g = c->g[l];
+            const bool shape = g.n[0] >= 128 && g.n[0] % 128 == 0 && g.n[1] >= 4 && g.n[2] >= 8;
+            if (shape && c->tma_ok[l] && g.c[0] == 2 && g.c[1] == 2 && g.c[2] == 2 && (size_t)g.N > nscr)
+                nscr = (size_t)g.N;
+        }
+    float* scr = nscr ? take(nscr) : nullptr;
+    if (base) c->uni_scratch = scr;
     return off;
 }
 
@@ -269,6 +285,7 @@ static void free_uniform(gmg_ctx* c) {
     for (int l = 0; l < GMG_MAX_LEVELS; ++l) {
         c->uni[l].brick = nullptr; c->ubrick_n[l] = 0;
         c->uni[l].left_list = nullptr; c->uni[l].left_count = nullptr; c->uni[l].left_n = -1;
+        c->uni[l].scratch = nullptr;
     }
 }
 static cudaError_t alloc_uniform(gmg_ctx* c) {
@@ -305,6 +322,7 @@ static cudaError_t alloc_uniform(gmg_ctx* c) {
         if (c->ubrick_n[l]) {
             c->uni[l].brick = c->ubrick_dev + off[l];
             c->uni[l].side_stream = c->side[0]; c->uni[l].ev_fork = c->ev_fork[0]; c->uni[l].ev_join = c->ev_join[0];
+            c->uni[l].scratch = c->uni_scratch;
             if (lbytes[l]) {
                 c->uni[l].left_list = reinterpret_cast<const int*>(c->ubrick_dev + total + cbytes + loff[l]);
                 c->uni[l].left_count = lcnt + l;
@@ -358,6 +376,7 @@ extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]
     for (int d = 0; d < 3; ++d) { c->n0[d] = n[d]; c->bc[d] = bc[d]; }
     gmg_default_params(&c->prm);
     c->ws = nullptr; c->ws_bytes = 0; c->ws_set = false; c->coeffs_set = false;
+    c->uni_scratch = nullptr;
     c->hist = c->omegas = nullptr; c->hist_cap = 0; c->hist_pin = nullptr;
     memset(&c->stats, 0, sizeof(c->stats));
     memset(c->lv, 0, sizeof(c->lv));
@@ -480,6 +499,7 @@ extern "C" int gmg_plan(int nx, int ny, int nz, const int bc[3], const gmg_param
     if ((long long)nx * ny * nz > (1LL << 31) - 1) return GMG_EINVAL;
     gmg_ctx tmp;
     tmp.cluster_ok = true;   // host-side plan: assume a device that can hold the cluster
+    tmp.uni_scratch = nullptr;
     for (int d = 0; d < 3; ++d) { tmp.n0[d] = n[d]; tmp.bc[d] = bc[d]; }
     if (params) tmp.prm = *params; else gmg_default_params(&tmp.prm);
     if (tmp.prm.n_min < 1) return GMG_EINVAL;
@@ -602,10 +622,16 @@ static void smooth(gmg_ctx* c, int l, float* p, const float* b, const float* ome
     const LevelGeom& g = c->g[l];
     int done = 0;
     if (e_c && c->fast_sweep[l] && nsweeps >= 2 && c->tma_ok[l] && gmgf::tma_shape_ok(g)) {
-        // in front of the TMA-fed sweep the correction is cheaper as its own streaming pass
-        gmgf::prolong_add4(g, e_c, p, s);
-        c->n_launch += 1;
-        e_c = nullptr;
+        if (gmgf::sweep_fuses_prolong(g, U(c, l))) {
+            // uniform bricks: the first sweep takes the correction along (lean tiles on the fly, the
+            // others through a corrected copy of their footprints): e_c stays
+            c->n_launch += 1;
+        } else {
+            // in front of the general TMA-fed sweep the correction is cheaper as its own streaming pass
+            gmgf::prolong_add4(g, e_c, p, s);
+            c->n_launch += 1;
+            e_c = nullptr;
+        }
     }
     if (c->fast_sweep[l] && nsweeps >= 2) {
         float* q = c->lv[l].q;
@@ -1339,9 +1365,13 @@ extern "C" int gmg_describe_plan(const gmg_ctx* c, char* buf, size_t cap) {
                                                      : "fused-rb-sweep") : "generic-half-sweeps");
         const char* rr = (in_tail || l == c->nlev - 1) ? "-"
                          : (c->fast_rr[l] ? "tiled" : "generic");
-        int w = snprintf(buf + off, cap - off, "L%d %dx%dx%d c=%d%d%d sweep=%s resrestrict=%s\n", l,
+        // prolongation + correction on the way up: its own pass, or folded into the first post-sweep
+        const char* pro = (in_tail || l == c->nlev - 1) ? "-"
+                          : (tma && c->fast_sweep[l] && c->prm.nu_post >= 2 && gmgf::sweep_fuses_prolong(c->g[l], c->uni[l]))
+                                ? "in-sweep" : "pass";
+        int w = snprintf(buf + off, cap - off, "L%d %dx%dx%d c=%d%d%d sweep=%s resrestrict=%s prolong=%s\n", l,
                          c->g[l].n[0], c->g[l].n[1], c->g[l].n[2], c->g[l].c[0], c->g[l].c[1],
-                         c->g[l].c[2], how, rr);
+                         c->g[l].c[2], how, rr, pro);
         if (w < 0 || (size_t)w >= cap - off) break;
         off += (size_t)w;
     }

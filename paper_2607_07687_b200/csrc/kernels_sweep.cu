@@ -91,6 +91,7 @@ struct BulkArgs {
     int slot_rr, slot_ref;
     const int* run_flag;   // != nullptr: the kernel does nothing unless *run_flag != 0
     UniArgs uni;           // uniform bricks of the level (uniform.cuh); brick == nullptr: disabled
+    const float* e_c;      // lean kernel, PRO: the coarse correction to be added to src on the fly
 };
 
 struct alignas(64) MapSet {
@@ -717,6 +718,60 @@ k_rb_sweep_lean(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
     else lean_body2<C, 2, NORM, (NORM != 0)>(a, maps, tile);
 }
 
+// ... with the prolongation + correction folded in (lean_body2<PRO>): 288 threads, two CTAs per SM
+// (96 registers: warps are allocated in pairs, 2 x 10 x 32 x 96 = 61,440 of the 65,536; at 112
+// registers only one CTA fits and the kernel takes 4.2 instead of 2.4 ms at 1024^3)
+template <class C>
+__global__ void __launch_bounds__(Lean2Threads<false>::value, 2)
+k_rb_sweep_lean_pro(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
+    if (a.run_flag && *a.run_flag == 0) return;
+    const int tile = blockIdx.x;
+    const int ty = (tile / a.tiles_x) % a.tiles_y;
+    const int ymode = tile_ymode<C>(a, ty);
+    if (!tile_is_lean<C>(a, tile, ymode)) return;
+    if (ymode == 0) lean_body2<C, 0, 0, false, true>(a, maps, tile);
+    else lean_body2<C, 2, 0, false, true>(a, maps, tile);
+}
+
+// Prolongation + correction for the tiles that are NOT lean, when the first post-sweep folds it in
+// (lean tiles: lean_body2<PRO>): scratch = src + P e_c over the footprint of each such tile (tile +
+// the halo the TMA boxes of k_rb_sweep_bulk fetch, wrapped on periodic axes), one CTA per entry of
+// the remaining-tile list.  k_rb_sweep_bulk then sweeps scratch -> dst on those tiles.  Footprints
+// of neighbouring tiles overlap; they write the same values.  2x2x2 coarsening.
+template <class C>
+__global__ void __launch_bounds__(256)
+k_prolong_tiles(const BulkArgs a, float* __restrict__ scratch) {
+    int tile = blockIdx.x;
+    if (a.uni.left_list) {
+        if (blockIdx.x >= *a.uni.left_count) return;
+        tile = a.uni.left_list[blockIdx.x];
+    } else {
+        const int ty_ = (tile / a.tiles_x) % a.tiles_y;
+        if (tile_is_lean<C>(a, tile, tile_ymode<C>(a, ty_))) return;
+    }
+    const LevelGeom& g = a.g;
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const int tx = tile % a.tiles_x, ty = (tile / a.tiles_x) % a.tiles_y, zc = tile / (a.tiles_x * a.tiles_y);
+    const int x0 = tx * C::TX, y0 = ty * C::TY, z0 = zc * a.zchunk, z1 = min(nz, z0 + a.zchunk);
+    constexpr int GX = C::TX / 4 + 2, GY = C::TY + 4;      // float4 groups x0-4 .. x0+TX+3, rows y0-2 .. y0+TY+1
+    const int GZ = z1 - z0 + 4;                            // planes z0-2 .. z1+1
+    const int ncx = nx >> 1, ncy = ny >> 1;
+    for (int t = threadIdx.x; t < GX * GY * GZ; t += 256) {
+        const int gxi = t % GX, r = t / GX;
+        const int y = y0 - 2 + r % GY, z = z0 - 2 + r / GY;
+        int x = x0 - 4 + 4 * gxi;
+        // out of the domain: wrapped on every axis -- behind a wall the boxes fill zeros, but the row
+        // copies of a tile row at a y wall read the wrapped rows (times a zero coefficient)
+        x = wrapi(x, nx);
+        const int gy = wrapi(y, ny), gz = wrapi(z, nz);
+        const size_t o = ((size_t)gz * ny + gy) * nx + x;
+        float4 v = ldg4(a.src + o);
+        const float2 e = __ldg(reinterpret_cast<const float2*>(a.e_c + ((size_t)(gz >> 1) * ncy + (gy >> 1)) * ncx + (x >> 1)));
+        v.x += e.x; v.y += e.x; v.z += e.y; v.w += e.y;
+        *reinterpret_cast<float4*>(scratch + o) = v;
+    }
+}
+
 // ---- launchers ------------------------------------------------------------------------------
 bool sweep_v2_supported(const LevelGeom& g);
 void rb_sweep_v2(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
@@ -772,7 +827,8 @@ bool tma_shape_ok(const LevelGeom& g) { return bulk_supported(g); }
 
 static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
                                  const float* omega, int first_colour, const ReduceBuf* norm, int slot_rr,
-                                 int slot_ref, const int* run_flag, const UniArgs& uni, cudaStream_t s);
+                                 int slot_ref, const int* run_flag, const UniArgs& uni, cudaStream_t s,
+                                 const float* e_c = nullptr);
 
 bool bulk_sweep_edge(const LevelGeom& g, bool norm);
 static unsigned int bulk_grid(const LevelGeom& g, int* zchunk_out) {
@@ -795,10 +851,20 @@ bool sweep_norm_supported(const LevelGeom& g) {
     return tma_shape_ok(g) && bulk_grid(g, nullptr) <= GMG_REDUCE_MAX_BLOCKS;
 }
 
+// The TMA-fed sweep of this level takes the prolongation + correction along (lean tiles on the fly,
+// the others through the scratch copy): uniform bricks marked, 2x2x2 coarsening, scratch at hand.
+bool sweep_fuses_prolong(const LevelGeom& g, const UniArgs& uni) {
+    return tma_shape_ok(g) && uni.brick && uni.left_list && uni.scratch && g.c[0] == 2 && g.c[1] == 2 && g.c[2] == 2;
+}
+
 void rb_sweep(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
               const float* omega, int first_colour, const float* e_c, int allow_tma, const UniArgs& uni,
               cudaStream_t s) {
-    // the caller applies the prolongation as its own pass in front of the TMA kernel (e_c == nullptr)
+    // in front of the TMA kernel the caller applies the prolongation as its own pass (e_c == nullptr)
+    // unless sweep_fuses_prolong
+    if (allow_tma && e_c && sweep_fuses_prolong(g, uni) &&
+        rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, nullptr, 0, 0, nullptr, uni, s, e_c))
+        return;
     if (allow_tma && !e_c && rb_sweep_bulk_launch(g, L, src, dst, b, omega, first_colour, nullptr, 0, 0, nullptr, uni, s))
         return;
     rb_sweep_v2(g, L, src, dst, b, omega, first_colour, e_c, s);
@@ -830,12 +896,14 @@ bool bulk_sweep_edge(const LevelGeom& g, bool norm) {
 
 static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float* src, float* dst, const float* b,
                                  const float* omega, int first_colour, const ReduceBuf* norm, int slot_rr,
-                                 int slot_ref, const int* run_flag, const UniArgs& uni, cudaStream_t s) {
+                                 int slot_ref, const int* run_flag, const UniArgs& uni, cudaStream_t s,
+                                 const float* e_c) {
     BulkMaps maps;
     const size_t N = (size_t)g.N;
     bool ok = tma_shape_ok(g);
+    const float* psrc = src;   // the array the p boxes are cut from
     auto set = [&](MapSet& m, int hp, int hc, int hly) {
-        return tensor_map(src, g, Bulk::TX, hp, &m.p_main) && tensor_map(src, g, 4, hp, &m.p_halo) &&
+        return tensor_map(psrc, g, Bulk::TX, hp, &m.p_main) && tensor_map(psrc, g, 4, hp, &m.p_halo) &&
                tensor_map(L + 2 * N, g, Bulk::TX, hc, &m.lz) && tensor_map(L, g, Bulk::TX, hc, &m.lx) &&
                tensor_map(L + N, g, Bulk::TX, hly, &m.ly) && tensor_map(b, g, Bulk::TX, hc, &m.b);
     };
@@ -850,8 +918,25 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
         maps.m[1] = maps.m[0];
         maps.m[2] = maps.m[0];
     }
+    // e_c: the sweep folds the prolongation in (sweep_fuses_prolong).  The lean kernel corrects src on
+    // the fly; the kernel of the remaining tiles reads the corrected copy k_prolong_tiles leaves in
+    // uni.scratch, through a second set of p boxes.
+    BulkMaps gmaps = maps;
+    if (ok && e_c) {
+        psrc = uni.scratch;
+        ok = set(gmaps.m[0], Bulk::SH, Bulk::ROWS, Bulk::ROWS + 1);
+        if (ok && g.bc[1] == 0 && tiles_y_ >= 2) {
+            ok = ok && set(gmaps.m[1], Bulk::SH - 2, Bulk::ROWS - 1, Bulk::ROWS);
+            ok = ok && set(gmaps.m[2], rem + 2, rem + 1, rem + 1);
+        } else {
+            gmaps.m[1] = gmaps.m[0];
+            gmaps.m[2] = gmaps.m[0];
+        }
+        psrc = src;
+    }
     if (!ok) return false;
     BulkArgs a;
+    a.e_c = e_c;
     a.g = g; a.L = L; a.src = src; a.dst = dst; a.b = b; a.omega = omega;
     a.first_colour = first_colour;
     a.rb = norm ? *norm : ReduceBuf{nullptr, nullptr, nullptr};
@@ -882,21 +967,28 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
         cudaStreamWaitEvent(sg, (cudaEvent_t)uni.ev_fork, 0);
     }
     auto launch_lean = [&]() {
-        if (nv == 2) k_rb_sweep_lean<Lean, 2><<<grid, Lean2Threads<true>::value, Lean::SMEM, s>>>(a, maps);
+        if (e_c) k_rb_sweep_lean_pro<Lean><<<grid, Lean2Threads<false>::value, Lean::SMEM, s>>>(a, maps);
+        else if (nv == 2) k_rb_sweep_lean<Lean, 2><<<grid, Lean2Threads<true>::value, Lean::SMEM, s>>>(a, maps);
         else if (nv == 1) k_rb_sweep_lean<Lean, 1><<<grid, Lean2Threads<true>::value, Lean::SMEM, s>>>(a, maps);
         else k_rb_sweep_lean<Lean, 0><<<grid, Lean2Threads<false>::value, Lean::SMEM, s>>>(a, maps);
     };
     if (uni.brick && !fork) launch_lean();
+    BulkArgs ga = a;   // the kernel of the remaining tiles
+    if (e_c && gl != 0) {
+        k_prolong_tiles<Bulk><<<gl, 256, 0, sg>>>(a, uni.scratch);
+        ga.src = uni.scratch;
+    }
+    const BulkMaps& bm = e_c ? gmaps : maps;
     if (gl == 0) {
         // every tile is lean
     } else if (edge) {
-        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, true><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
-        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, true><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
-        else k_rb_sweep_bulk<Bulk, 0, true><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, true><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(ga, bm);
+        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, true><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(ga, bm);
+        else k_rb_sweep_bulk<Bulk, 0, true><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(ga, bm);
     } else {
-        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, false><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
-        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, false><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
-        else k_rb_sweep_bulk<Bulk, 0, false><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(a, maps);
+        if (nv == 2) k_rb_sweep_bulk<Bulk, 2, false><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(ga, bm);
+        else if (nv == 1) k_rb_sweep_bulk<Bulk, 1, false><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(ga, bm);
+        else k_rb_sweep_bulk<Bulk, 0, false><<<gl, Bulk::THREADS, Bulk::SMEM, sg>>>(ga, bm);
     }
     if (fork) {
         launch_lean();
@@ -927,6 +1019,10 @@ int configure() {
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_rb_sweep_lean<Lean, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Lean::SMEM);
     // two lean CTAs per SM need the large shared-memory carve-out
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_lean_pro<Lean>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Lean::SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_rb_sweep_lean_pro<Lean>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_rb_sweep_lean<Lean, 0>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e == cudaSuccess)

@@ -21,10 +21,22 @@ namespace gmgf {
 // registers: the norm-carrying variants need them -- 3.66 vs 3.93 ms).
 template <bool RIM> struct Lean2Threads { static constexpr int value = RIM ? 256 : 288; };
 
-template <class C, int YMODE, int NORM, bool RIM>
+// PRO: the sweep starts from p + P e_c (prolongation + correction, reading O6: each fine cell gets its
+// parent's value) without p having been rewritten: every SOURCE value is corrected where it enters a
+// register, with the same single addition k_prolong_add4 performs, so the result equals "correction
+// pass, then sweep" bit for bit.  Phase B stores whole float4s of corrected values, so the operands
+// other threads store to during a step are loaded in front of the barrier (main threads: as always;
+// the edge warp: its one in-tile neighbour) -- and one more CTA barrier separates the loads in front
+// of step 0 from step 0's stores.  The parents change every second plane: a thread keeps the float2
+// parents of its four operand rows (and of the x-halo cell) for the current coarse plane in registers
+// and fetches the next coarse plane's right in front of the loads that use them (fetched at the top
+// of the step, a step body ahead, they are live across the step and spill: 3.20 vs 2.94 ms at
+// 1024^3; the plain lean sweep takes 2.38 ms).  2x2x2 coarsening, plain sweep only.
+template <class C, int YMODE, int NORM, bool RIM, bool PRO = false>
 __device__ __forceinline__ void lean_body2(const BulkArgs& a, const BulkMaps& allmaps, const int tile) {
     static_assert(C::LEAN && C::PD == 4 && C::NP == 6 && C::NC == 6 && C::NB == 6, "rings of period 6");
     static_assert(YMODE == 0 || YMODE == 2, "box-fed tiles only");
+    static_assert(!PRO || (NORM == 0 && !RIM), "prolongation rides on the plain sweep");
     constexpr int R = 6, PD = C::PD;
     extern __shared__ __align__(1024) float sm[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + C::FLOATS);  // [0..6) step groups, [6] prologue
@@ -173,8 +185,40 @@ __device__ __forceinline__ void lean_body2(const BulkArgs& a, const BulkMaps& al
         Ka.lza = Ka.lzb = Ka.lzha = Ka.lzhb = wz;
         Ka.ba = Ka.bb = 0.0f;
         Kb = Ka;
+        // PRO: parents of the own float4 (two coarse cells) in coarse row gy/2 of coarse plane gz/2, and of
+        // the x-halo cell (first / last lane)
+        const int ncx = nx >> 1, cplane = ncx * (ny >> 1);
+        const int xc = xl >> 1;
+        // float offsets (coarse plane 0) of the parents of rows a-1, a, b, b+1 at the own float4
+        const int em_o = (wrapi(yla - 1, ny) >> 1) * ncx + xc, ea_o = (gya >> 1) * ncx + xc;
+        const int eb_o = (gyb >> 1) * ncx + xc, ep_o = (wrapi(ylb + 1, ny) >> 1) * ncx + xc;
+        const int eh_d = ((first_lane ? wrapi(x0 - 1, nx) : wrapi(x0 + C::TX, nx)) >> 1) - xc;   // x-halo cell's parent
+        const bool has_h = first_lane || last_lane;
+        auto ld2 = [&](int o) { return __ldg(reinterpret_cast<const float2*>(a.e_c + o)); };
+        auto add2 = [](float4& v, const float2 e) { v.x += e.x; v.y += e.x; v.z += e.y; v.w += e.y; };
+        float2 Em = make_float2(0.f, 0.f), Ea = Em, Eb = Em, Ep = Em;   // parents in coarse plane gzs/2
+        float2 Aa = Em, Ab = Em;                                        // rows a, b one coarse plane on
+        float Ha = 0.0f, Hb = 0.0f;
+        int gzs = wrap1(z0 - 1, nz);    // PRO: wrapped plane index of the step whose operands load_step fetches
+        // what load_step will need for plane gzs: all of coarse plane gzs/2 (fetched when gzs is even:
+        // the plane before was the last of its pair) or, gzs odd, rows a and b of the next coarse plane
+        auto fetch_parents = [&](bool all) {
+            if (all || !(gzs & 1)) {
+                const int o = (gzs >> 1) * cplane;
+                Em = ld2(o + em_o); Ea = ld2(o + ea_o); Eb = ld2(o + eb_o); Ep = ld2(o + ep_o);
+                if (has_h) { Ha = __ldg(a.e_c + o + ea_o + eh_d); Hb = __ldg(a.e_c + o + eb_o + eh_d); }
+            }
+            if (gzs & 1) {
+                const int o = (wrap1(gzs + 1, nz) >> 1) * cplane;
+                Aa = ld2(o + ea_o); Ab = ld2(o + eb_o);
+            }
+        };
         // plane u-1 at the own positions (t = 0: source values), plane u-2 under the cells C updates
         float4 q1a = lds4(pp), q1b = lds4(pp + C::TX);
+        if (PRO) {
+            const int o = (wrapi(z0 - 2, nz) >> 1) * cplane;
+            add2(q1a, ld2(o + ea_o)); add2(q1b, ld2(o + eb_o));
+        }
         float z2a0 = 0.0f, z2a1 = 0.0f, z2b0 = 0.0f, z2b1 = 0.0f;
         float zsa0 = 0.0f, zsa1 = 0.0f, zsb0 = 0.0f, zsb1 = 0.0f;   // NORM (see sweep_body)
         float acc_rr = 0.0f, acc_bb = 0.0f, acc_rr2 = 0.0f, acc_bb2 = 0.0f;   // one pair of sums per ROW, as sweep_body keeps them
@@ -196,10 +240,18 @@ __device__ __forceinline__ void lean_body2(const BulkArgs& a, const BulkMaps& al
             bb = vb ? lds4(pb + ob + C::TX) : zero4();
             hva = ph[o0];
             hvb = ph[o0 + 4];
+            if (PRO) {
+                add2(ym, Em); add2(yp, Ep);
+                hva += Ha; hvb += Hb;      // (only the first and the last lane use them)
+                add2(zpa, (gzs & 1) ? Aa : Ea); add2(zpb, (gzs & 1) ? Ab : Eb);
+                gzs = (gzs + 1 == nz) ? 0 : gzs + 1;
+            }
         };
         owna = lds4(pp + o0);
         ownb = lds4(pp + o0 + C::TX);
+        if (PRO) { fetch_parents(true); add2(owna, Ea); add2(ownb, Eb); }
         load_step();
+        if (PRO) cta_sync();   // step 0 stores corrected float4s into rows other warps have just read
 
         // The last warp owns one row only (phase-B row 14, the ring row) and also updates the ring-1
         // CELLS x0-1 and x0+TX of all 15 rows (phase B only; lane = 2 row + side), as sweep_body's edge
@@ -313,6 +365,7 @@ __device__ __forceinline__ void lean_body2(const BulkArgs& a, const BulkMaps& al
             oP = (oP == (R - 1) * C::P_PLANE) ? 0 : oP + C::P_PLANE;
             ob = (ob == (R - 1) * C::C_PLANE) ? 0 : ob + C::C_PLANE;
             if (++jb == R) { jb = 0; kpar ^= 1u; }
+            if (PRO && t + 1 < T) fetch_parents(false);
             if (t + 1 < T) load_step();
             fence_async_smem();  // order this thread's smem writes before later TMA overwrites
             cta_sync();
@@ -347,18 +400,60 @@ __device__ __forceinline__ void lean_body2(const BulkArgs& a, const BulkMaps& al
         const float D = diag6(wx, wx, wy, wy, wz, wz);
         int oM = 0, o0 = C::P_PLANE, oP = 2 * C::P_PLANE, jb = 0;
         uint32_t kpar = 0;
+        // PRO: parents of the edge cell and its six neighbours; the neighbour INSIDE the tile is a cell a
+        // main thread stores to during the step, so it is read in front of the barrier
+        const int ncx = nx >> 1, cplane = ncx * (ny >> 1);
+        const int in_off = side ? xm_off : xp_off;
+        const int c0 = wrapi(xs, nx) >> 1;                                   // coarse columns of the cell,
+        const int cin = wrapi(side ? xs - 1 : xs + 1, nx) >> 1;              // its neighbour inside the tile
+        const int cout = wrapi(side ? xs + 1 : xs - 1, nx) >> 1;             // and the one outside
+        const int r0 = (wrapi(eyl, ny) >> 1) * ncx, rl = (wrapi(eyl - 1, ny) >> 1) * ncx, rh = (wrapi(eyl + 1, ny) >> 1) * ncx;
+        int gzu = wrap1(z0 - 1, nz);   // wrapped plane index of step t
+        float xin = 0.0f;
+        if (PRO) {
+            mbar_wait(bars, 0);
+            xin = P[o0 + in_off];
+            cta_sync();   // (the main threads' barrier in front of step 0)
+        }
         for (int t = 0; t < T; ++t) {
             if (t + 1 < T) {   // the next plane's right-hand side, one step ahead
                 gz = (gz + 1 == nz) ? 0 : gz + 1;
                 bn = __ldg(bptr + (size_t)gz * plane);
             }
+            const bool upd = e_act && ((ecol0 ^ t) & 1) == fc;
+            float e_c0 = 0.f, e_in = 0.f, e_out = 0.f, e_yl = 0.f, e_yh = 0.f, e_zl = 0.f, e_zh = 0.f;
+            if (PRO && upd) {   // the seven parents, fetched before the wait for the plane
+                const int k0 = (gzu >> 1) * cplane;
+                const int kl = ((gzu == 0 ? nz - 1 : gzu - 1) >> 1) * cplane, kh = ((gzu + 1 == nz ? 0 : gzu + 1) >> 1) * cplane;
+                e_c0 = __ldg(a.e_c + k0 + r0 + c0);
+                e_in = __ldg(a.e_c + k0 + r0 + cin);
+                e_out = __ldg(a.e_c + k0 + r0 + cout);
+                e_yl = __ldg(a.e_c + k0 + rl + c0);
+                e_yh = __ldg(a.e_c + k0 + rh + c0);
+                e_zl = __ldg(a.e_c + kl + r0 + c0);
+                e_zh = __ldg(a.e_c + kh + r0 + c0);
+            }
             mbar_wait(bars + jb, kpar);
-            if (e_act && ((ecol0 ^ t) & 1) == fc) {
+            if (upd) {
                 float* P0 = P + o0;
-                const float pc = P0[pc_off];
-                const float Ap = apply7(pc, wx, wx, wy, wy, wz, wz, P0[xm_off], P0[xp_off], P0[pc_off - 4],
-                                        P0[pc_off + 4], P[oM + pc_off], P[oP + pc_off]);
-                P0[pc_off] = relax(pc, bc_, Ap, D, omega);
+                if (PRO) {
+                    const float pc = P0[pc_off] + e_c0;
+                    const float vin = xin + e_in;
+                    const float vout = P0[side ? xp_off : xm_off] + e_out;
+                    const float Ap = apply7(pc, wx, wx, wy, wy, wz, wz, side ? vin : vout, side ? vout : vin,
+                                            P0[pc_off - 4] + e_yl, P0[pc_off + 4] + e_yh,
+                                            P[oM + pc_off] + e_zl, P[oP + pc_off] + e_zh);
+                    P0[pc_off] = relax(pc, bc_, Ap, D, omega);
+                } else {
+                    const float pc = P0[pc_off];
+                    const float Ap = apply7(pc, wx, wx, wy, wy, wz, wz, P0[xm_off], P0[xp_off], P0[pc_off - 4],
+                                            P0[pc_off + 4], P[oM + pc_off], P[oP + pc_off]);
+                    P0[pc_off] = relax(pc, bc_, Ap, D, omega);
+                }
+            }
+            if (PRO && t + 1 < T) {   // the in-tile neighbour of the next step (plane u+1 has landed): still a source value
+                xin = P[oP + in_off];
+                gzu = gzu + 1 == nz ? 0 : gzu + 1;
             }
             fence_async_smem();
             cta_sync();

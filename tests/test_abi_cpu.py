@@ -110,7 +110,13 @@ def test_library_level_table_matches_golden_and_oracle(libpath):
         N = [s[0] * s[1] * s[2] for s in shapes]
         lower = 4 * (N[0] + 6 * N[0] + sum(6 * v for v in N[1:]) + sum(6 * v for v in N[tail:]))
         cluster_extra = 4 * sum(6 * v for v in N[:tail] if v <= 32768)
-        assert lower <= ws <= lower + cluster_extra + 256 * (7 * len(N) + 8)
+        # ... and one array as large as the largest TMA-fed level with 2x2x2 coarsening: the corrected
+        # copy of the non-lean tiles for the sweep that folds the prolongation in (uniform.cuh)
+        scratch = 4 * max([N[l] for l in range(min(tail, len(N) - 1))
+                           if shapes[l][0] >= 128 and shapes[l][0] % 128 == 0 and factors[l] == (2, 2, 2)] + [0])
+        assert lower <= ws <= lower + cluster_extra + scratch + 256 * (7 * len(N) + 9)
+        if shapes[0] == (1024, 1024, 1024):
+            assert ws >= lower + scratch
     # agreement with the oracle's rule on odd / mixed cases, both coarsening modes
     for n, bc in [((20, 20, 20), (1, 0, 0)), ((36, 20, 6), (0, 1, 0)), ((64, 4, 4), (1, 0, 0)), ((15, 9, 7), (1, 1, 1)),
                   ((64, 16, 1), (1, 0, 1)), ((128, 32, 1), (0, 0, 1))]:      # 2-D mode

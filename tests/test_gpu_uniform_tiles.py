@@ -106,6 +106,25 @@ def test_residual_restrict_and_vcycle_bit_identical(pair):
                            off.op_vcycle(p.clone(), b, omega=0.9375, symmetric=sym))
 
 
+def test_prolongation_folded_into_the_sweep_is_bit_identical_every_time(pair):
+    """With uniform bricks marked, the first post-smoothing sweep of a TMA-fed 2x2x2 level takes the
+    prolongation + correction along (lean tiles: parents added where source values enter registers;
+    other tiles: a corrected copy of their footprints) instead of running k_prolong_add4 first.  The
+    lean kernel stores corrected values into planes its neighbours read, so a missing barrier shows
+    as a run-to-run difference: every one of 25 cycles must give the bits of the separate pass."""
+    wl, on, off = pair
+    plan = on.describe_plan().split("\n")[0]
+    folded = "prolong=in-sweep" in plan
+    if wl.name in ("config4_spheres_128", "config1_tgv", "ones_256x64x32", "ones_128x64x64"):
+        assert folded, plan
+    assert "prolong=pass" in off.describe_plan().split("\n")[0]
+    p, b = _fields(wl, 55)
+    for sym in (False, True):
+        ref = off.op_vcycle(p.clone(), b, omega=0.875, symmetric=sym)
+        for _ in range(25 if folded else 2):
+            assert torch.equal(on.op_vcycle(p.clone(), b, omega=0.875, symmetric=sym), ref)
+
+
 @pytest.mark.parametrize("solver", [gmg.GMG_RBGS, gmg.GMG_PCG, gmg.PCG, gmg.GMG_CGS])
 def test_solves_bit_identical(pair, solver):
     wl, on, off = pair
