@@ -215,7 +215,7 @@ static void build_levels(gmg_ctx* c) {
             c->uni[l].brick = nullptr;
             c->uni[l].side_stream = c->uni[l].ev_fork = c->uni[l].ev_join = nullptr;
             c->uni[l].left_list = nullptr; c->uni[l].left_count = nullptr; c->uni[l].left_n = -1;
-            c->uni[l].scratch = nullptr;
+            c->uni[l].scratch = nullptr; c->uni[l].fold = 0;
             c->ubrick_n[l] = 0;
             c->uni_frac_sweep[l] = c->uni_frac_res[l] = 0.0;
             for (int d = 0; d < 3; ++d) C[d] *= c->g[l].c[d];
@@ -285,7 +285,7 @@ static void free_uniform(gmg_ctx* c) {
     for (int l = 0; l < GMG_MAX_LEVELS; ++l) {
         c->uni[l].brick = nullptr; c->ubrick_n[l] = 0;
         c->uni[l].left_list = nullptr; c->uni[l].left_count = nullptr; c->uni[l].left_n = -1;
-        c->uni[l].scratch = nullptr;
+        c->uni[l].scratch = nullptr; c->uni[l].fold = 0;
     }
 }
 static cudaError_t alloc_uniform(gmg_ctx* c) {
@@ -579,7 +579,15 @@ static void refresh_uniform_stats(gmg_ctx* c) {
     for (int l = 0; l < c->nlev; ++l) {
         c->uni_frac_sweep[l] = c->uni[l].brick ? (double)c->ucount_host[l] / (double)c->g[l].N : 0.0;
         c->uni_frac_res[l] = c->uni[l].brick ? (double)c->ucount_host[GMG_MAX_LEVELS + l] / (double)c->g[l].N : 0.0;
-        if (c->uni[l].left_list) c->uni[l].left_n = (int)lcnt[l];
+        if (c->uni[l].left_list) {
+            c->uni[l].left_n = (int)lcnt[l];
+            int ty = 0, zc = 0;
+            if (gmgf::bulk_sweep_tiling(c->g[l], &ty, &zc)) {
+                const long long tiles = (long long)(c->g[l].n[0] / 128) * ((c->g[l].n[1] + ty - 1) / ty) *
+                                        ((c->g[l].n[2] + zc - 1) / zc);
+                c->uni[l].fold = 2LL * c->uni[l].left_n <= tiles;
+            }
+        }
     }
 }
 

@@ -35,6 +35,9 @@ struct UniArgs {
     // a level-0-sized scratch array (workspace): the corrected iterate p + P e_c over the footprints of
     // the non-lean tiles, for the sweep that folds the prolongation in (sweep_lean2.cuh, PRO)
     float* scratch;
+    // host-side hint, kept across coefficient updates: at the last count at least half of the level's
+    // tiles were lean, so folding the prolongation into the sweep pays
+    int fold;
     // host side only: a side stream and two events with which a launcher runs the kernel of the
     // remaining (non-uniform) tiles beside the lean kernel; nullptr = one after the other
     void* side_stream;
