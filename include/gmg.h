@@ -102,6 +102,9 @@ typedef struct {
                           constants, every cell gets the same bits (SURVEY.md S8(d) "a lossless 'tile is
                           all L=1' flag ... honest only if reported as such": gmg_stats.uniform_fraction
                           and bytes_as_run report it).  0: every CTA loads its coefficients (1) */
+    int small_cg;      /* 1: GMG_GMG_CGS runs a whole smoothing (restart + nu CG iterations) of a level of
+                          at most 4096 cells as ONE single-CTA kernel instead of 4 launches per iteration;
+                          same arithmetic and the same summation order, every cell gets the same bits (1) */
 } gmg_params_t;
 
 /* Statistics of the last gmg_solve. */

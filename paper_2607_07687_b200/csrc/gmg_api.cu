@@ -358,6 +358,7 @@ extern "C" void gmg_default_params(gmg_params_t* p) {
     p->fast_path = 1; p->use_graph = 1; p->tma_min_cells = 1 << 20; p->cluster_tail = 1;
     p->fused_norm = 1;
     p->uniform_tiles = 1;
+    p->small_cg = 1;
 }
 
 extern "C" int gmg_create(gmg_ctx** out, int nx, int ny, int nz, const int bc[3]) {
@@ -723,22 +724,34 @@ static void cg_smooth(gmg_ctx* c, int l, float* x, const float* b, int m, cudaSt
     const LevelGeom& g = c->g[l];
     const float* L = c->lv[l].L;
     float *r = c->pcg_r, *d = c->pcg_d, *q = c->pcg_q, *sv = c->pcg_s;
+    int nmax = g.n[0] > g.n[1] ? g.n[0] : g.n[1];
+    if (g.n[2] > nmax) nmax = g.n[2];
+    // a step longer than 16 n_max^2 is a direction that drifted into the null space (reading O12)
+    const double alpha_cap = 16.0 * (double)nmax * (double)nmax;
+    // small levels: the whole smoothing in one single-CTA kernel (kernels_pcg4.cu), same bits
+    if (c->prm.small_cg && gmgk::cgs_small(g, L, x, b, m, alpha_cap, s)) {
+        c->n_launch += 1;
+        return;
+    }
+    // the control steps (begin / alpha / beta, stencil.cuh) ride on the reductions they follow
+    ReduceBuf rb_begin = rbuf(c), rb_alpha = rbuf(c), rb_beta = rbuf(c);
+    rb_begin.post = POST_CGS_BEGIN;
+    rb_begin.post_arg = alpha_cap;
+    rb_alpha.post = POST_CGS_ALPHA;
+    rb_beta.post = POST_CGS_BETA;
     gmgk::cgs_residual_sum(g, L, x, b, r, rbuf(c), s);
-    gmgk::cgs_start(g, L, r, d, rbuf(c), s);       // r -= mean; d = r/D; rho = r.d
-    gmgk::ctl_cgs_begin(c->sc, g, s);
-    c->n_launch += 3;
+    gmgk::cgs_start(g, L, r, d, rb_begin, s);      // r -= mean; d = r/D; rho = r.d; begin
+    c->n_launch += 2;
     for (int it = 0; it < m; ++it) {
         if (!(c->prm.fast_path && c->tma_ok[l] && (c->prm.tma_min_cells == 0 || g.N >= kBulkMatvecMinCells) &&
-              gmgf::matvec_dot_bulk(g, L, d, q, rbuf(c), RED_DQ, U(c, l), s)))
-            gmgk::matvec_dot(g, L, d, q, rbuf(c), RED_DQ, s);
-        gmgk::ctl_cgs_alpha(c->sc, s);
+              gmgf::matvec_dot_bulk(g, L, d, q, rb_alpha, RED_DQ, U(c, l), s)))
+            gmgk::matvec_dot(g, L, d, q, rb_alpha, RED_DQ, s);     // ... alpha
         gmgk::pcg_update_pr(g, L, x, r, d, q, nullptr, 0, rbuf(c), s);
-        c->n_launch += 3;
+        c->n_launch += 2;
         if (it == m - 1) break;
-        gmgk::jacobi_apply(g, L, r, sv, rbuf(c), RED_RS, s);
-        gmgk::ctl_cgs_beta(c->sc, s);
+        gmgk::jacobi_apply(g, L, r, sv, rb_beta, RED_RS, s);       // ... beta
         gmgk::pcg_update_d(g.N, d, sv, c->sc, 0, s);
-        c->n_launch += 3;
+        c->n_launch += 2;
     }
 }
 

@@ -99,7 +99,12 @@ struct ReduceBuf {
     double* partials;       // [2][GMG_REDUCE_MAX_BLOCKS] (a kernel reduces at most two sums)
     unsigned int* counter;  // ticket of the "last block finishes the sum" stage, self-resetting
     DevScalars* sc;
+    // a single-thread control step that rides on the reduction it follows (stencil.cuh,
+    // finish_reduction): the thread that writes the sums runs it, instead of a <<<1, 1>>> launch
+    int post;               // POST_NONE, or a step of the CG smoother
+    double post_arg;        // POST_CGS_BEGIN: the step-length cap of the level
 };
+enum { POST_NONE = 0, POST_CGS_BEGIN = 1, POST_CGS_ALPHA = 2, POST_CGS_BETA = 3 };
 #define GMG_REDUCE_MAX_BLOCKS 16384
 
 // ---- launchers (kernels_generic.cu) --------------------------------------------------------
@@ -185,9 +190,12 @@ void cgs_residual_sum(const LevelGeom& g, const float* L, const float* x, const 
                       ReduceBuf rb, cudaStream_t s);
 // r -= mean over active cells; d = r/D; red[RS] = r.d
 void cgs_start(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s);
-void ctl_cgs_begin(DevScalars* sc, const LevelGeom& g, cudaStream_t s);
-void ctl_cgs_alpha(DevScalars* sc, cudaStream_t s);
-void ctl_cgs_beta(DevScalars* sc, cudaStream_t s);
+// (the smoother's control steps -- begin, alpha, beta -- ride on cgs_start, the mat-vec and the
+// Jacobi kernel: ReduceBuf::post)
+// m iterations restarted from x (in place) on a level of at most 4096 cells with nx % 4 == 0, as one
+// single-CTA kernel; false = level not eligible (nothing enqueued)
+bool cgs_small(const LevelGeom& g, const float* L, float* x, const float* b, int m, double alpha_cap,
+               cudaStream_t s);
 void ctl_set_omega(DevScalars* sc, double omega, cudaStream_t s);
 
 }  // namespace gmgk

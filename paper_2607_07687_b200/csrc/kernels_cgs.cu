@@ -4,7 +4,8 @@
 // current iterate of a level.  The iteration itself reuses the PCG vector kernels
 // (kernels_reduce.cu / kernels_pcg4.cu / the TMA-fed mat-vec); this file holds what the restart
 // needs -- the residual with its sum over the active cells, the mean-free start r -= mean,
-// d = r/D, rho = r.d -- and the single-thread control kernels with the smoother's guards.
+// d = r/D, rho = r.d.  The single-thread control steps with the smoother's guards (stencil.cuh,
+// cgs_ctl_*) ride on the reductions they follow (ReduceBuf::post) instead of being launches.
 // Per-cell arithmetic in the one-cell and the float4 kernels is identical.
 #include "stencil.cuh"
 
@@ -85,54 +86,5 @@ void cgs_start(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf
     if (cgs_start4(g, L, r, d, rb, s)) return;
     k_cgs_start<<<cgs_blocks(g.N), kCT, 0, s>>>(g, L, r, d, rb);
 }
-
-// ---- control (single thread).  A is negative semi-definite: r.s and d.q are negative. -----------
-// after cgs_start: rho = rho0 = r.d ; nothing to do when rho is not < 0
-__global__ void k_ctl_cgs_begin(DevScalars* sc, double alpha_cap) {
-    const double rho = sc->red[RED_RS];
-    sc->cgs_alpha_cap = alpha_cap;
-    sc->rho_cg = rho;
-    sc->cgs_rho0 = rho;
-    sc->cgs_frozen = !(rho < 0.0);
-    sc->alpha = 0.0;
-    sc->beta = 0.0;
-}
-void ctl_cgs_begin(DevScalars* sc, const LevelGeom& g, cudaStream_t s) {
-    // a step longer than 16 n_max^2 is a direction that drifted into the null space (reading O12)
-    int nmax = g.n[0] > g.n[1] ? g.n[0] : g.n[1];
-    if (g.n[2] > nmax) nmax = g.n[2];
-    k_ctl_cgs_begin<<<1, 1, 0, s>>>(sc, 16.0 * (double)nmax * (double)nmax);
-}
-
-// after q = A d, red[DQ] = d.q : alpha = rho/(d.q); d.q not < 0 or alpha above the cap ends the
-// smoothing (alpha = 0 leaves x and r untouched for the remaining iterations)
-__global__ void k_ctl_cgs_alpha(DevScalars* sc) {
-    const double dq = sc->red[RED_DQ];
-    double alpha = 0.0;
-    bool stop = sc->cgs_frozen || !(dq < 0.0);
-    if (!stop) {
-        alpha = sc->rho_cg / dq;
-        stop = alpha > sc->cgs_alpha_cap;
-    }
-    if (stop) {
-        sc->cgs_frozen = 1;
-        alpha = 0.0;
-    }
-    sc->alpha = alpha;
-}
-void ctl_cgs_alpha(DevScalars* sc, cudaStream_t s) { k_ctl_cgs_alpha<<<1, 1, 0, s>>>(sc); }
-
-// after s = r/D, red[RS] = r.s : beta = rho'/rho ; freeze once |rho'| <= 1e-8 |rho0|
-__global__ void k_ctl_cgs_beta(DevScalars* sc) {
-    if (sc->cgs_frozen) {
-        sc->beta = 0.0;
-        return;
-    }
-    const double rho_new = sc->red[RED_RS];
-    sc->beta = rho_new / sc->rho_cg;
-    sc->rho_cg = rho_new;
-    if (!(fabs(rho_new) > GMG_CGS_FREEZE * fabs(sc->cgs_rho0))) sc->cgs_frozen = 1;
-}
-void ctl_cgs_beta(DevScalars* sc, cudaStream_t s) { k_ctl_cgs_beta<<<1, 1, 0, s>>>(sc); }
 
 }  // namespace gmgk

@@ -249,7 +249,180 @@ k_cgs_start4(LevelGeom g, const float* __restrict__ L, float* __restrict__ r, fl
     finish_reduction(acc, 0.0, false, rb, RED_RS, 0);
 }
 
+// ---- a whole smoothing of the CG smoother on a small level, one CTA ---------------------------------
+// On a level of at most 4096 cells the six kernels above are one or a few blocks each and a smoothing
+// of m iterations is 4 m launch-bound launches (GMG_GMG_CGS on the paper's Table-1 sizes: 185 per
+// cycle at 32 x 32 x 16).  k_cgs_small runs the restart and the m iterations in ONE CTA of B x 256
+// threads, B = the grid those kernels would have (1..4): thread t owns the float4 group t, keeps its
+// weights, x, r, d, q, s in registers and exchanges only the vector whose neighbours a stencil needs
+// (x at the restart, d in every iteration) through shared memory.  Same expressions per cell; the
+// sums follow finish_reduction's order (warp tree, the 8 warp sums of each 256-thread "block", the B
+// block sums in lanes 0..B-1 of one more tree), so every cell gets the bits of the multi-launch path.
+// The control steps (cgs_ctl_*) run on a DevScalars block in shared memory.
+static constexpr int kSmallMaxGroups = 1024;
+
+struct SmallSmem {
+    float v[4 * kSmallMaxGroups];   // the vector a stencil reads
+    double warp_part[32];
+    double part[4];
+    double total;
+    DevScalars sc;
+};
+
+// sum over the CTA in finish_reduction's order; every thread gets the result
+__device__ __forceinline__ double small_sum(double v, int B, SmallSmem& S) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    __syncthreads();
+    if (lane == 0) S.warp_part[wid] = v;
+    __syncthreads();
+    if ((wid & 7) == 0) {   // first warp of a 256-thread "block": its 8 warp sums
+        double t = (lane < 8) ? S.warp_part[wid + lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+        if (lane == 0) S.part[wid >> 3] = t;
+    }
+    __syncthreads();
+    if (wid == 0) {         // the "last block": the B partials in index order
+        double t = (lane < B) ? S.part[lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+        if (lane == 0) S.total = t;
+    }
+    __syncthreads();
+    return S.total;
+}
+
+__global__ void __launch_bounds__(1024)
+k_cgs_small(LevelGeom g, const float* __restrict__ L, float* __restrict__ x, const float* __restrict__ b, int m,
+            double alpha_cap) {
+    __shared__ SmallSmem S;
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const int sy = nx, sz = nx * ny;
+    const int groups = (int)(g.N >> 2);
+    const int B = (int)(blockDim.x >> 8);
+    const int t = threadIdx.x;
+    const bool act = t < groups;
+    const int c = 4 * t;
+    int i = 0, j = 0, k = 0;
+    W4 w;
+    w.xl = w.xh = w.yl = w.yh = w.zl = w.zh = splat4(0.0f);
+    float4 xv = splat4(0.0f), bv = xv;
+    if (act) {
+        unflat4(g, (unsigned int)t, i, j, k);
+        w = weights4(g, L, i, j, k, c);
+        xv = ldg4(x + c);
+        bv = ldg4(b + c);
+        *reinterpret_cast<float4*>(S.v + c) = xv;
+    }
+    // neighbour offsets in the shared vector (as the kernels above index global memory)
+    const int o_xm = (i == 0) ? c + (nx - 1) : c - 1, o_xp = (i + 4 == nx) ? c - (nx - 4) : c + 4;
+    const int o_yl = (j == 0) ? c + sy * (ny - 1) : c - sy, o_yh = (j == ny - 1) ? c - sy * (ny - 1) : c + sy;
+    const int o_zl = (k == 0) ? c + sz * (nz - 1) : c - sz, o_zh = (k == nz - 1) ? c - sz * (nz - 1) : c + sz;
+    auto A4 = [&](const float4 vc) {   // A v on the own group, v's neighbours from shared memory
+        const float vm = S.v[o_xm], vp = S.v[o_xp];
+        const float4 yl = *reinterpret_cast<const float4*>(S.v + o_yl), yh = *reinterpret_cast<const float4*>(S.v + o_yh);
+        const float4 zl = *reinterpret_cast<const float4*>(S.v + o_zl), zh = *reinterpret_cast<const float4*>(S.v + o_zh);
+        float4 o;
+        o.x = apply7(vc.x, w.xl.x, w.xh.x, w.yl.x, w.yh.x, w.zl.x, w.zh.x, vm, vc.y, yl.x, yh.x, zl.x, zh.x);
+        o.y = apply7(vc.y, w.xl.y, w.xh.y, w.yl.y, w.yh.y, w.zl.y, w.zh.y, vc.x, vc.z, yl.y, yh.y, zl.y, zh.y);
+        o.z = apply7(vc.z, w.xl.z, w.xh.z, w.yl.z, w.yh.z, w.zl.z, w.zh.z, vc.y, vc.w, yl.z, yh.z, zl.z, zh.z);
+        o.w = apply7(vc.w, w.xl.w, w.xh.w, w.yl.w, w.yh.w, w.zl.w, w.zh.w, vc.z, vp, yl.w, yh.w, zl.w, zh.w);
+        return o;
+    };
+    const float Dx = diag6(w.xl.x, w.xh.x, w.yl.x, w.yh.x, w.zl.x, w.zh.x);
+    const float Dy = diag6(w.xl.y, w.xh.y, w.yl.y, w.yh.y, w.zl.y, w.zh.y);
+    const float Dz = diag6(w.xl.z, w.xh.z, w.yl.z, w.yh.z, w.zl.z, w.zh.z);
+    const float Dw = diag6(w.xl.w, w.xh.w, w.yl.w, w.yh.w, w.zl.w, w.zh.w);
+    __syncthreads();
+    // ---- restart: r = b - A x on active cells (k_cgs_residual_sum4), its sum and the active count ----
+    float4 rv = splat4(0.0f);
+    double sum = 0.0, cnt = 0.0;
+    if (act) {
+        const float4 Ax = A4(xv);
+        const bool ax = Dx != 0.0f, ay = Dy != 0.0f, az = Dz != 0.0f, aw = Dw != 0.0f;
+        rv.x = ax ? bv.x - Ax.x : 0.0f;
+        rv.y = ay ? bv.y - Ax.y : 0.0f;
+        rv.z = az ? bv.z - Ax.z : 0.0f;
+        rv.w = aw ? bv.w - Ax.w : 0.0f;
+        sum += (double)rv.x + (double)rv.y + (double)rv.z + (double)rv.w;
+        cnt += (double)((int)ax + (int)ay + (int)az + (int)aw);
+    }
+    const double tsum = small_sum(sum, B, S);
+    const double tcnt = small_sum(cnt, B, S);
+    if (t == 0) { S.sc.red[RED_CGS_SUM] = tsum; S.sc.red[RED_CGS_CNT] = tcnt; }
+    __syncthreads();
+    // ---- mean-free start (k_cgs_start4): r -= mean; d = r/D; rho = r.d ----
+    const float mu = cgs_mean(&S.sc);
+    float4 dv = splat4(0.0f);
+    double acc = 0.0;
+    if (act) {
+        const float4 r0 = rv;
+        rv = splat4(0.0f);
+        if (Dx != 0.0f) { rv.x = r0.x - mu; dv.x = rv.x / Dx; }
+        if (Dy != 0.0f) { rv.y = r0.y - mu; dv.y = rv.y / Dy; }
+        if (Dz != 0.0f) { rv.z = r0.z - mu; dv.z = rv.z / Dz; }
+        if (Dw != 0.0f) { rv.w = r0.w - mu; dv.w = rv.w / Dw; }
+        acc += (double)rv.x * (double)dv.x + (double)rv.y * (double)dv.y + (double)rv.z * (double)dv.z +
+               (double)rv.w * (double)dv.w;
+    }
+    {
+        const double rho = small_sum(acc, B, S);
+        if (t == 0) { S.sc.red[RED_RS] = rho; cgs_ctl_begin(&S.sc, alpha_cap); }
+    }
+    for (int it = 0; it < m; ++it) {
+        // q = A d, d.q (k_matvec_dot4); alpha
+        if (act) *reinterpret_cast<float4*>(S.v + c) = dv;
+        __syncthreads();
+        float4 qv = splat4(0.0f);
+        acc = 0.0;
+        if (act) {
+            qv = A4(dv);
+            acc += (double)dv.x * (double)qv.x + (double)dv.y * (double)qv.y + (double)dv.z * (double)qv.z +
+                   (double)dv.w * (double)qv.w;
+        }
+        const double dq = small_sum(acc, B, S);
+        if (t == 0) { S.sc.red[RED_DQ] = dq; cgs_ctl_alpha(&S.sc); }
+        __syncthreads();
+        // x += alpha d; r -= alpha q (k_pcg_update_pr4)
+        const float alpha = (float)S.sc.alpha;
+        xv.x = fmaf(alpha, dv.x, xv.x); xv.y = fmaf(alpha, dv.y, xv.y);
+        xv.z = fmaf(alpha, dv.z, xv.z); xv.w = fmaf(alpha, dv.w, xv.w);
+        rv.x = fmaf(-alpha, qv.x, rv.x); rv.y = fmaf(-alpha, qv.y, rv.y);
+        rv.z = fmaf(-alpha, qv.z, rv.z); rv.w = fmaf(-alpha, qv.w, rv.w);
+        if (it == m - 1) break;
+        // s = r/D, r.s (k_jacobi_apply4); beta; d = s + beta d (k_pcg_update_d4)
+        float4 sv;
+        sv.x = (Dx != 0.0f) ? rv.x / Dx : 0.0f;
+        sv.y = (Dy != 0.0f) ? rv.y / Dy : 0.0f;
+        sv.z = (Dz != 0.0f) ? rv.z / Dz : 0.0f;
+        sv.w = (Dw != 0.0f) ? rv.w / Dw : 0.0f;
+        acc = act ? (double)rv.x * (double)sv.x + (double)rv.y * (double)sv.y + (double)rv.z * (double)sv.z +
+                        (double)rv.w * (double)sv.w
+                  : 0.0;
+        const double rs = small_sum(acc, B, S);
+        if (t == 0) { S.sc.red[RED_RS] = rs; cgs_ctl_beta(&S.sc); }
+        __syncthreads();
+        const float beta = (float)S.sc.beta;
+        dv.x = fmaf(beta, dv.x, sv.x); dv.y = fmaf(beta, dv.y, sv.y);
+        dv.z = fmaf(beta, dv.z, sv.z); dv.w = fmaf(beta, dv.w, sv.w);
+    }
+    if (act) *reinterpret_cast<float4*>(x + c) = xv;
+}
+
 static inline bool al16(const void* p) { return (reinterpret_cast<size_t>(p) & 15) == 0; }
+
+bool cgs_small(const LevelGeom& g, const float* L, float* x, const float* b, int m, double alpha_cap,
+               cudaStream_t s) {
+    const long long groups = g.N >> 2;
+    // (x extents of 128 and more may take the TMA-fed mat-vec, whose sums run in another order)
+    if (g.n[0] % 4 != 0 || g.n[0] >= 128 || groups > kSmallMaxGroups || m <= 0 || !al16(L) || !al16(x) || !al16(b))
+        return false;
+    const int B = (int)((groups + kPT - 1) / kPT);
+    k_cgs_small<<<1, B * kPT, 0, s>>>(g, L, x, b, m, alpha_cap);
+    return true;
+}
 
 bool matvec_dot4(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot,
                  cudaStream_t s) {

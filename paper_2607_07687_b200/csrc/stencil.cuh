@@ -122,8 +122,48 @@ __device__ __forceinline__ double block_sum(double v) {
     return t;
 }
 
+// ---- control steps of the CG smoother (reading O12; S9b), run by the one thread that has
+// just written the sum they depend on.  A is negative semi-definite: r.s and d.q are negative. ------
+// after the mean-free start: rho = rho0 = r.d; nothing to do when rho is not < 0
+__device__ __forceinline__ void cgs_ctl_begin(DevScalars* sc, double alpha_cap) {
+    const double rho = sc->red[RED_RS];
+    sc->cgs_alpha_cap = alpha_cap;
+    sc->rho_cg = rho;
+    sc->cgs_rho0 = rho;
+    sc->cgs_frozen = !(rho < 0.0);
+    sc->alpha = 0.0;
+    sc->beta = 0.0;
+}
+// after q = A d, red[DQ] = d.q: alpha = rho/(d.q); d.q not < 0 or alpha above the cap ends the
+// smoothing (alpha = 0 leaves x and r untouched for the remaining iterations)
+__device__ __forceinline__ void cgs_ctl_alpha(DevScalars* sc) {
+    const double dq = sc->red[RED_DQ];
+    double alpha = 0.0;
+    bool stop = sc->cgs_frozen || !(dq < 0.0);
+    if (!stop) {
+        alpha = sc->rho_cg / dq;
+        stop = alpha > sc->cgs_alpha_cap;
+    }
+    if (stop) {
+        sc->cgs_frozen = 1;
+        alpha = 0.0;
+    }
+    sc->alpha = alpha;
+}
+// after s = r/D, red[RS] = r.s: beta = rho'/rho; freeze once |rho'| <= 1e-8 |rho0|
+__device__ __forceinline__ void cgs_ctl_beta(DevScalars* sc) {
+    if (sc->cgs_frozen) {
+        sc->beta = 0.0;
+        return;
+    }
+    const double rho_new = sc->red[RED_RS];
+    sc->beta = rho_new / sc->rho_cg;
+    sc->rho_cg = rho_new;
+    if (!(fabs(rho_new) > GMG_CGS_FREEZE * fabs(sc->cgs_rho0))) sc->cgs_frozen = 1;
+}
+
 // Finishes up to two sums: every block deposits its partial(s); the last block adds them in
-// index order and writes red[slot0] (and red[slot1]).
+// index order and writes red[slot0] (and red[slot1]), then runs the control step rb.post, if any.
 __device__ __forceinline__ void finish_reduction(double v0, double v1, bool two, ReduceBuf rb,
                                                  int slot0, int slot1) {
     __shared__ bool is_last;
@@ -150,6 +190,9 @@ __device__ __forceinline__ void finish_reduction(double v0, double v1, bool two,
         rb.sc->red[slot0] = s0;
         if (two) rb.sc->red[slot1] = s1;
         *rb.counter = 0u;
+        if (rb.post == POST_CGS_BEGIN) cgs_ctl_begin(rb.sc, rb.post_arg);
+        else if (rb.post == POST_CGS_ALPHA) cgs_ctl_alpha(rb.sc);
+        else if (rb.post == POST_CGS_BETA) cgs_ctl_beta(rb.sc);
     }
 }
 

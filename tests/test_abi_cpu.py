@@ -50,15 +50,15 @@ def test_library_contains_sm100a_code(libpath):
 
 
 def test_struct_sizes_match_header(libpath):
-    """Params / Stats mirror the C structs (16 x 4 bytes; Stats has 8-byte alignment)."""
+    """Params / Stats mirror the C structs (17 x 4 bytes; Stats has 8-byte alignment)."""
     from paper_2607_07687_b200 import gmg
-    assert C.sizeof(gmg.Params) == 64
+    assert C.sizeof(gmg.Params) == 68
     assert C.sizeof(gmg.Stats) == 4 * 4 + 6 * 8 + 8 + 8 + 3 * 8
     p = gmg.Params()
     gmg.lib.gmg_default_params(C.byref(p))
     assert (p.nu_pre, p.nu_post, p.nu_coarse, p.n_min) == (2, 2, 32, 4)
     assert (p.omega0, p.omega_min, p.omega_down, p.omega_up) == (1.0, 0.5, 0.125, 0.03125)
-    assert (p.fast_path, p.use_graph, p.cluster_tail, p.fused_norm, p.uniform_tiles) == (1, 1, 1, 1, 1)
+    assert (p.fast_path, p.use_graph, p.cluster_tail, p.fused_norm, p.uniform_tiles, p.small_cg) == (1, 1, 1, 1, 1, 1)
 
 
 def test_null_arguments_are_rejected_without_a_gpu(libpath):

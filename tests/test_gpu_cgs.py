@@ -140,3 +140,38 @@ def test_cgs_survives_an_incompatible_right_hand_side():
         assert rel_l2_demeaned(out, ref["p"], act) <= TOL_P
     finally:
         g.close()
+
+
+@pytest.mark.parametrize("n,bc", [((32, 32, 16), (0, 0, 0)), ((16, 16, 16), (1, 0, 1)), ((64, 64, 32), (1, 1, 1)),
+                                  ((40, 24, 8), (1, 0, 1)), ((128, 128, 64), (1, 1, 1))])
+def test_single_cta_smoothing_gives_the_bits_of_the_multi_launch_path(n, bc):
+    """`small_cg` (include/gmg.h): on levels of at most 4096 cells a whole smoothing is ONE kernel that
+    keeps the multi-launch kernels' expressions and summation order.  Every level and iteration count
+    through the hook, one whole cycle, and a solve: identical bits with the switch on and off."""
+    wl = random_workload(n, bc, seed=sum(n))
+    on, off = make_gpu(wl, small_cg=1), make_gpu(wl, small_cg=0)
+    rng = np.random.default_rng(9)
+    try:
+        small = 0
+        for lev in range(on.num_levels()):
+            (nx, ny, nz), _ = on.level_shape(lev)
+            small += int(nx * ny * nz <= 4096 and nx % 4 == 0)
+            x0 = dev(rng.standard_normal((nz, ny, nx)))
+            b = dev(rng.standard_normal((nz, ny, nx)))
+            for m in (1, 2, 5, 32):
+                a = on.op_cg_smooth(lev, x0.clone(), b, m)
+                c = off.op_cg_smooth(lev, x0.clone(), b, m)
+                assert torch.equal(a, c), (n, lev, m, float((a - c).abs().max()))
+        assert small >= 1, "the case must reach a level the single-CTA kernel takes"
+        p, z = dev(rng.standard_normal(wl.z.shape)), dev(wl.z)
+        assert torch.equal(on.op_vcycle_cgs(p.clone(), z), off.op_vcycle_cgs(p.clone(), z))
+        out = []
+        for g in (on, off):
+            x = torch.zeros(wl.z.shape, dtype=torch.float32, device="cuda")
+            rc = g.solve(x, z, tol=1e-5, maxiter=60, solver=gmg.GMG_CGS)
+            out.append((rc, g.stats()["iterations"], x, g.stats()["kernel_launches"]))
+        assert out[0][:2] == out[1][:2] and torch.equal(out[0][2], out[1][2])
+        assert out[0][3] < out[1][3]          # fewer launches
+    finally:
+        on.close()
+        off.close()
