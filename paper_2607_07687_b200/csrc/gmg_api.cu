@@ -62,6 +62,7 @@ struct GraphSlot {
     double* hist = nullptr;
     long long n_pre = 0, n_body = 0, n_post = 0;  // kernel launches per section
     int left_n[GMG_MAX_LEVELS];   // lengths of the remaining-tile lists the launch grids were sized with
+    int fold[GMG_MAX_LEVELS];     // ... and whether the prolongation rode on the first post-sweep
 };
 
 struct gmg_ctx {
@@ -1007,7 +1008,10 @@ static int build_graph(gmg_ctx* c, GraphSlot& slot, int solver, float* p, const 
     CUDA_TRY(c, cudaGraphInstantiate(&slot.exec, graph, 0));
     slot.p = p; slot.z = z; slot.solver = solver; slot.tol = tol; slot.maxiter = maxiter;
     slot.hist = c->hist;
-    for (int l = 0; l < GMG_MAX_LEVELS; ++l) slot.left_n[l] = l < c->nlev ? c->uni[l].left_n : -1;
+    for (int l = 0; l < GMG_MAX_LEVELS; ++l) {
+        slot.left_n[l] = l < c->nlev ? c->uni[l].left_n : -1;
+        slot.fold[l] = l < c->nlev ? c->uni[l].fold : 0;
+    }
     return GMG_OK;
 }
 
@@ -1062,7 +1066,8 @@ extern "C" int gmg_solve(gmg_ctx* c, float* p, const float* z, float tol, int ma
     if (c->prm.use_graph) {
         GraphSlot& slot = c->slots[solver];
         bool same_lists = true;   // the launch grids in the graph were sized with these list lengths
-        for (int l = 0; l < c->nlev; ++l) same_lists = same_lists && slot.left_n[l] == c->uni[l].left_n;
+        for (int l = 0; l < c->nlev; ++l)
+            same_lists = same_lists && slot.left_n[l] == c->uni[l].left_n && slot.fold[l] == c->uni[l].fold;
         if (!slot.exec || slot.p != p || slot.z != z || slot.tol != tol || slot.maxiter != maxiter ||
             slot.hist != c->hist || !same_lists) {
             rc = build_graph(c, slot, solver, p, z, tol, maxiter);

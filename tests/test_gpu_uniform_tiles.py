@@ -185,3 +185,38 @@ def test_coarse_level_constants_and_a_moving_body():
     finally:
         on.close()
         off.close()
+
+
+def test_pressure_steps_with_a_moving_body_bit_identical():
+    """gmg_pressure_step does not read the tile counts back between the coefficient update and the
+    solve: the kernels of the remaining tiles (k_rb_sweep_bulk, k_prolong_tiles) launch the whole grid
+    and bound themselves by the device-side list length, and the fold hint is the one of the last
+    count.  Four steps with a body that moves, warm-started: u, p and the cycle counts of every step
+    are those of the run without uniform tiles."""
+    n, bc = (256, 128, 64), (0, 0, 0)
+    fields = [_ones_with_bodies(n, bc, 20 + s, nblobs=1) for s in range(4)]
+    rng = np.random.default_rng(21)
+    u0 = rng.standard_normal((3, n[2], n[1], n[0])).astype(np.float32)
+    runs = []
+    for uni in (1, 0):
+        g = gmg.GMG(n, bc, tma_min_cells=0, uniform_tiles=uni)
+        try:
+            p = torch.zeros((n[2], n[1], n[0]), dtype=torch.float32, device="cuda")
+            L = dev(fields[0].L)
+            out = []
+            for s, wl in enumerate(fields):
+                L.copy_(dev(wl.L))              # the body moves: the same array, rewritten in place
+                u = dev(u0 * (1.0 + 0.1 * s))
+                rc = g.pressure_step(L, u, p, tol=1e-5, maxiter=60)
+                torch.cuda.synchronize()
+                st = g.stats()
+                out.append((rc, st["iterations"], u.clone(), p.clone(), st["uniform_fraction"]))
+            if uni:
+                assert out[-1][4] > 0.5, out[-1][4]
+                assert "prolong=in-sweep" in g.describe_plan().split("\n")[0]
+            runs.append(out)
+        finally:
+            g.close()
+    for a, b in zip(*runs):
+        assert a[:2] == b[:2] and a[0] == gmg.OK
+        assert torch.equal(a[2], b[2]) and torch.equal(a[3], b[3])
