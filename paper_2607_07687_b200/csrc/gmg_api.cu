@@ -907,24 +907,26 @@ static void pcg_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStream
 }
 static void pcg_body(gmg_ctx* c, float* p, int gmg_precond, LoopCtl lc, cudaStream_t s) {
     const long long N = c->g[0].N;
+    // beta and alpha (stencil.cuh, pcg_ctl_*) ride on the reductions they follow
+    ReduceBuf rb_beta = rbuf(c), rb_alpha = rbuf(c);
+    rb_beta.post = POST_PCG_BETA;
+    rb_alpha.post = POST_PCG_ALPHA;
     if (!gmg_precond) {
-        gmgk::jacobi_apply(c->g[0], c->lv[0].L, c->pcg_r, c->pcg_s, rbuf(c), RED_RS, s);
+        gmgk::jacobi_apply(c->g[0], c->lv[0].L, c->pcg_r, c->pcg_s, rb_beta, RED_RS, s);
         c->n_launch += 1;
     } else {
         gmgk::fill(c->pcg_s, N, 0.0f, s);
         enqueue_vcycle(c, c->pcg_s, c->pcg_r, &c->sc->omega_one, 1, s);
-        gmgk::dot(N, c->pcg_r, c->pcg_s, rbuf(c), RED_RS, s);
+        gmgk::dot(N, c->pcg_r, c->pcg_s, rb_beta, RED_RS, s);
         c->n_launch += 2;
     }
-    gmgk::ctl_pcg_beta(c->sc, s);
     gmgk::pcg_update_d(N, c->pcg_d, c->pcg_s, c->sc, 0, s);
     if (!(c->prm.fast_path && c->tma_ok[0] && (c->prm.tma_min_cells == 0 || c->g[0].N >= kBulkMatvecMinCells) &&
-          gmgf::matvec_dot_bulk(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rbuf(c), RED_DQ, U(c, 0), s)))
-        gmgk::matvec_dot(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rbuf(c), RED_DQ, s);
-    gmgk::ctl_pcg_alpha(c->sc, s);
+          gmgf::matvec_dot_bulk(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rb_alpha, RED_DQ, U(c, 0), s)))
+        gmgk::matvec_dot(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rb_alpha, RED_DQ, s);
     gmgk::pcg_update_pr(c->g[0], c->lv[0].L, p, c->pcg_r, c->pcg_d, c->pcg_q, nullptr, 0, rbuf(c), s);
     gmgk::ctl_pcg_check(c->sc, c->hist, lc.cond, lc.use_cond, s);
-    c->n_launch += 6;
+    c->n_launch += 4;
 }
 static void pcg_post(gmg_ctx* c, float* p, const float* z, cudaStream_t s) {
     // true residual at exit (the recursive one drove the test)

@@ -101,10 +101,10 @@ struct ReduceBuf {
     DevScalars* sc;
     // a single-thread control step that rides on the reduction it follows (stencil.cuh,
     // finish_reduction): the thread that writes the sums runs it, instead of a <<<1, 1>>> launch
-    int post;               // POST_NONE, or a step of the CG smoother
+    int post;               // POST_NONE, a step of the CG smoother, or alpha / beta of the (GMG-)PCG solver
     double post_arg;        // POST_CGS_BEGIN: the step-length cap of the level
 };
-enum { POST_NONE = 0, POST_CGS_BEGIN = 1, POST_CGS_ALPHA = 2, POST_CGS_BETA = 3 };
+enum { POST_NONE = 0, POST_CGS_BEGIN = 1, POST_CGS_ALPHA = 2, POST_CGS_BETA = 3, POST_PCG_ALPHA = 4, POST_PCG_BETA = 5 };
 #define GMG_REDUCE_MAX_BLOCKS 16384
 
 // ---- launchers (kernels_generic.cu) --------------------------------------------------------
@@ -178,8 +178,7 @@ void ctl_begin(DevScalars* sc, double* hist, double* omegas, cudaGraphConditiona
                int use_cond, cudaStream_t s);
 void ctl_rbgs_cycle_end(DevScalars* sc, double* hist, double* omegas,
                         cudaGraphConditionalHandle cond, int use_cond, cudaStream_t s);
-void ctl_pcg_beta(DevScalars* sc, cudaStream_t s);
-void ctl_pcg_alpha(DevScalars* sc, cudaStream_t s);
+// (alpha and beta of the PCG solvers ride on the mat-vec and on the r.s reduction: ReduceBuf::post)
 void ctl_pcg_check(DevScalars* sc, double* hist, cudaGraphConditionalHandle cond, int use_cond,
                    cudaStream_t s);
 void ctl_set_hook_omega(DevScalars* sc, float omega, cudaStream_t s);

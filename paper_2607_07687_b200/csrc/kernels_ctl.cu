@@ -143,26 +143,6 @@ void ctl_rbgs_cycle_end(DevScalars* sc, double* hist, double* omegas,
     k_ctl_rbgs_cycle_end<<<1, 1, 0, s>>>(sc, hist, omegas, cond, use_cond);
 }
 
-// PCG: after s = M^-1 r and red[RS] = r.s :  beta = rho'/rho (0 on the first iteration).
-__global__ void k_ctl_pcg_beta(DevScalars* sc) {
-    const double rho_new = sc->red[RED_RS];
-    sc->beta = (sc->iter == 0) ? 0.0 : rho_new / sc->rho_cg;
-    sc->rho_cg = rho_new;
-}
-void ctl_pcg_beta(DevScalars* sc, cudaStream_t s) { k_ctl_pcg_beta<<<1, 1, 0, s>>>(sc); }
-
-// PCG: after q = A d and red[DQ] = d.q :  alpha = rho/(d.q); breakdown if d.q == 0.
-__global__ void k_ctl_pcg_alpha(DevScalars* sc) {
-    const double dq = sc->red[RED_DQ];
-    if (dq == 0.0) {
-        sc->alpha = 0.0;  // the update kernels then leave p and r unchanged
-        sc->status = GMG_EBREAKDOWN;
-    } else {
-        sc->alpha = sc->rho_cg / dq;
-    }
-}
-void ctl_pcg_alpha(DevScalars* sc, cudaStream_t s) { k_ctl_pcg_alpha<<<1, 1, 0, s>>>(sc); }
-
 // PCG: after p, r updates and red[RR] = r.r (recursive residual drives the test).
 __global__ void k_ctl_pcg_check(DevScalars* sc, double* hist, cudaGraphConditionalHandle cond,
                                 int use_cond) {

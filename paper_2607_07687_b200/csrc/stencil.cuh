@@ -162,6 +162,24 @@ __device__ __forceinline__ void cgs_ctl_beta(DevScalars* sc) {
     if (!(fabs(rho_new) > GMG_CGS_FREEZE * fabs(sc->cgs_rho0))) sc->cgs_frozen = 1;
 }
 
+// ---- (GMG-)PCG solver (reading O10): the same arrangement --------------------------------------
+// after s = M^-1 r and red[RS] = r.s: beta = rho'/rho (0 on the first iteration)
+__device__ __forceinline__ void pcg_ctl_beta(DevScalars* sc) {
+    const double rho_new = sc->red[RED_RS];
+    sc->beta = (sc->iter == 0) ? 0.0 : rho_new / sc->rho_cg;
+    sc->rho_cg = rho_new;
+}
+// after q = A d and red[DQ] = d.q: alpha = rho/(d.q); breakdown if d.q == 0
+__device__ __forceinline__ void pcg_ctl_alpha(DevScalars* sc) {
+    const double dq = sc->red[RED_DQ];
+    if (dq == 0.0) {
+        sc->alpha = 0.0;  // the update kernels then leave p and r unchanged
+        sc->status = GMG_EBREAKDOWN;
+    } else {
+        sc->alpha = sc->rho_cg / dq;
+    }
+}
+
 // Finishes up to two sums: every block deposits its partial(s); the last block adds them in
 // index order and writes red[slot0] (and red[slot1]), then runs the control step rb.post, if any.
 __device__ __forceinline__ void finish_reduction(double v0, double v1, bool two, ReduceBuf rb,
@@ -193,6 +211,8 @@ __device__ __forceinline__ void finish_reduction(double v0, double v1, bool two,
         if (rb.post == POST_CGS_BEGIN) cgs_ctl_begin(rb.sc, rb.post_arg);
         else if (rb.post == POST_CGS_ALPHA) cgs_ctl_alpha(rb.sc);
         else if (rb.post == POST_CGS_BETA) cgs_ctl_beta(rb.sc);
+        else if (rb.post == POST_PCG_ALPHA) pcg_ctl_alpha(rb.sc);
+        else if (rb.post == POST_PCG_BETA) pcg_ctl_beta(rb.sc);
     }
 }
 
