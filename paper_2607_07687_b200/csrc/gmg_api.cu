@@ -146,7 +146,7 @@ static inline const gmgf::UniArgs& U(const gmg_ctx* c, int l) { return c->uni[l]
 // The float4 / TMA paths read caller arrays 16 bytes at a time (gmg.h "Alignment").
 static inline bool al16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
 #define MUST_LAUNCH(c, call) do { if (!(call)) (c)->enqueue_fail = true; } while (0)
-static inline ReduceBuf rbuf(gmg_ctx* c) { return ReduceBuf{c->partials, c->counter, c->sc}; }
+static inline ReduceBuf rbuf(gmg_ctx* c) { return ReduceBuf{c->partials, c->counter, c->sc, POST_NONE, 0.0}; }
 
 // ---- level table: reading O4 ("downsamples every dimension independently") ------
 static void build_levels(gmg_ctx* c) {

@@ -535,7 +535,7 @@ void residual_restrict(const LevelGeom& g, const float* L, const float* p, const
     if (allow_tma && residual_restrict_bulk(g, L, p, b, b_c, p_c, uni, s)) return;
     ResArgs a;
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = b_c; a.p_c = p_c;
-    a.rb = ReduceBuf{nullptr, nullptr, nullptr};
+    a.rb = ReduceBuf{nullptr, nullptr, nullptr, POST_NONE, 0.0};
     a.slot = 0;
     if (g.n[0] >= 128) launch_res<Res128, 0>(a, s);
     else if (g.n[0] >= 64) launch_res<Res64, 0>(a, s);

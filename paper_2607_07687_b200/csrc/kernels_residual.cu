@@ -463,7 +463,7 @@ bool residual_restrict_bulk(const LevelGeom& g, const float* L, const float* p, 
     ResBulkArgs a;
     a.uni = uni;
     a.g = g; a.L = L; a.p = p; a.b = b; a.b_c = b_c; a.p_c = p_c;
-    a.rb = ReduceBuf{nullptr, nullptr, nullptr};
+    a.rb = ReduceBuf{nullptr, nullptr, nullptr, POST_NONE, 0.0};
     a.slot = 0;
     a.slot2 = 0;
     a.run_flag = nullptr;

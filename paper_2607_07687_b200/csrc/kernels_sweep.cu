@@ -951,7 +951,7 @@ static bool rb_sweep_bulk_launch(const LevelGeom& g, const float* L, const float
     a.e_c = e_c;
     a.g = g; a.L = L; a.src = src; a.dst = dst; a.b = b; a.omega = omega;
     a.first_colour = first_colour;
-    a.rb = norm ? *norm : ReduceBuf{nullptr, nullptr, nullptr};
+    a.rb = norm ? *norm : ReduceBuf{nullptr, nullptr, nullptr, POST_NONE, 0.0};
     a.slot_rr = slot_rr; a.slot_ref = slot_ref;
     a.run_flag = run_flag;
     a.uni = uni;
