@@ -234,7 +234,10 @@ k_uniform_cells(LevelGeom g, const unsigned char* __restrict__ brick, int TXc, i
     using namespace gmgf;
     const int tiles_x = g.n[0] / TXc, tiles_y = (g.n[1] + TYc - 1) / TYc, nzc = (g.n[2] + zchunk - 1) / zchunk;
     const long long total = (long long)tiles_x * tiles_y * nzc;
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    // one WARP per tile: the lanes share the bricks of its footprint (a few hundred byte loads that
+    // one thread would issue one after the other: 38 instead of 6 us per pass at 1024^3)
+    const int lane = threadIdx.x & 31;
+    const long long t = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     if (t >= total) return;
     const int tx = (int)(t % tiles_x), ty = (int)((t / tiles_x) % tiles_y), zc = (int)(t / ((long long)tiles_x * tiles_y));
     const int x0 = tx * TXc, y0 = ty * TYc, z0 = zc * zchunk, z1 = min(g.n[2], z0 + zchunk), ny = g.n[1];
@@ -245,20 +248,20 @@ k_uniform_cells(LevelGeom g, const unsigned char* __restrict__ brick, int TXc, i
     } else {
         boxfed = (y0 >= 1) && (y0 + TYc + 1 <= ny);
     }
-    if (!boxfed || !ub_box_uniform(g, brick, x0 - 2, x0 + TXc + 1, y0 - 2, y0 + yhi, z0 - 2, z1 + 1)) {
+    if (!boxfed || !ub_box_uniform_warp(g, brick, x0 - 2, x0 + TXc + 1, y0 - 2, y0 + yhi, z0 - 2, z1 + 1, lane)) {
         // not lean: onto the list of remaining tiles (any order: tiles are independent)
-        if (left_list) left_list[atomicAdd(left_count, 1u)] = (int)t;
+        if (left_list && lane == 0) left_list[atomicAdd(left_count, 1u)] = (int)t;
         return;
     }
     const int rows = min(TYc, ny - y0);
-    atomicAdd(out, (unsigned long long)TXc * rows * (z1 - z0));
+    if (lane == 0) atomicAdd(out, (unsigned long long)TXc * rows * (z1 - z0));
 }
 
 void uniform_cells(const LevelGeom& g, const unsigned char* brick, int TXc, int TYc, int yhi, int zchunk, int rule,
                    unsigned long long* out, int* left_list, unsigned int* left_count, cudaStream_t s) {
     const int tiles_x = g.n[0] / TXc, tiles_y = (g.n[1] + TYc - 1) / TYc, nzc = (g.n[2] + zchunk - 1) / zchunk;
     const long long total = (long long)tiles_x * tiles_y * nzc;
-    k_uniform_cells<<<(unsigned int)((total + 127) / 128), 128, 0, s>>>(g, brick, TXc, TYc, yhi, zchunk, rule, out, left_list, left_count);
+    k_uniform_cells<<<(unsigned int)((total + 3) / 4), 128, 0, s>>>(g, brick, TXc, TYc, yhi, zchunk, rule, out, left_list, left_count);
 }
 
 }  // namespace gmgk
