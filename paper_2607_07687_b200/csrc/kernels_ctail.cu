@@ -85,60 +85,104 @@ struct CLevel {  // one level as this CTA sees it
     float *W, *p, *b, *r;
 };
 
-// Neighbours of the local cell l of a distributed level: x/y as local indices (12 bits each),
-// z as shared::cluster addresses of p (the neighbouring slab when the plane is a slab boundary).
+// Neighbours of the local cell l of a distributed level, two words per cell so that the four slots
+// of a thread stay in registers (a cluster barrier invalidates L1, spilled slots would come back
+// from L2 after every half-sweep): x/y neighbours as local indices (12 bits each), the colour, and
+// one flag per z direction: the neighbouring plane lies in ANOTHER CTA's slab.  A slab is whole
+// planes, so only its first and its last plane look across; the other z accesses are plain
+// shared-memory loads at l -+ plane.
 struct CSlot {
-    uint32_t x, y, zm, zp;  // x = xm | xp << 12 | colour << 30 (colour 3 = no cell); y = ym | yp << 12
+    uint32_t x, y;  // x = xm | xp << 12 | zm remote << 24 | zp remote << 25 | colour << 30 (3 = no cell); y = ym | yp << 12
     __device__ __forceinline__ int colour() const { return (int)(x >> 30); }
 };
 
-__device__ __forceinline__ CSlot make_slot(const CLevel& L, int l) {
-    CSlot s;
-    s.x = 3u << 30;
-    s.y = s.zm = s.zp = 0;
-    if (l >= L.per) return s;
-    const int nx = L.g.n[0], ny = L.g.n[1], nz = L.g.n[2], plane = nx * ny;
-    const int c = L.c0 + l;
-    const int k = c / plane, rem = c - k * plane, j = rem / nx, i = rem - j * nx;
-    const int xm = (i == 0) ? l + (nx - 1) : l - 1;
-    const int xp = (i == nx - 1) ? l - (nx - 1) : l + 1;
-    const int ym = (j == 0) ? l + (plane - nx) : l - nx;
-    const int yp = (j == ny - 1) ? l - (plane - nx) : l + nx;
-    s.x = (uint32_t)xm | ((uint32_t)xp << 12) | ((uint32_t)((i + j + k) & 1) << 30);
-    s.y = (uint32_t)ym | ((uint32_t)yp << 12);
-    const int czm = (k == 0) ? c + (nz - 1) * plane : c - plane;
-    const int czp = (k == nz - 1) ? c - (nz - 1) * plane : c + plane;
-    const int rm = czm / L.per, rp = czp / L.per;
-    const uint32_t pa = saddr(L.p);
-    s.zm = map_rank(pa + 4u * (uint32_t)(czm - rm * L.per), rm);
-    s.zp = map_rank(pa + 4u * (uint32_t)(czp - rp * L.per), rp);
-    return s;
+// What the z accesses of a level need besides the slot
+struct CZ {
+    int plane, wrap;      // wrap = per - plane: from the first plane of a slab to the last of the one below
+    uint32_t pa;          // shared address of p
+    int rm, rp;           // ranks of the slabs below and above (periodic; across a wall the weight is zero)
+};
+
+__device__ __forceinline__ CZ make_cz(const CLevel& L, int rank) {
+    CZ z;
+    z.plane = L.g.n[0] * L.g.n[1];
+    z.wrap = L.per - z.plane;
+    z.pa = saddr(L.p);
+    z.rm = (rank + kCR - 1) % kCR;
+    z.rp = (rank + 1) % kCR;
+    return z;
 }
 
-__device__ __forceinline__ Cell slot_cell(const CLevel& L, const CSlot& s, int l) {
+// Visits the cells tid, tid + T, tid + 2T, ... of the slab with their global (i, j, k): one division
+// pair for the first cell, then (i, j, k) advance by T cells with carries.
+template <class F>
+__device__ __forceinline__ void for_slab_cells(const CLevel& L, F f) {
+    const int nx = L.g.n[0], ny = L.g.n[1], plane = nx * ny;
+    const int di = kTailThreads % nx, dj = (kTailThreads / nx) % ny, dk = kTailThreads / plane;
+    const int c = L.c0 + (int)threadIdx.x;
+    int k = c / plane;
+    const int rem = c - k * plane;
+    int j = rem / nx, i = rem - j * nx;
+#pragma unroll
+    for (int m = 0; m < kCSlots; ++m) {
+        const int l = (int)threadIdx.x + m * kTailThreads;
+        f(m, l, l < L.per, i, j, k);
+        i += di;
+        if (i >= nx) { i -= nx; ++j; }
+        j += dj;
+        if (j >= ny) { j -= ny; ++k; }
+        k += dk;
+    }
+}
+
+__device__ __forceinline__ void make_slots_dist(const CLevel& L, int rank, CSlot (&s)[kCSlots]) {
+    const int nx = L.g.n[0], ny = L.g.n[1], plane = nx * ny;
+    const int zs = L.g.n[2] / kCR;                 // planes per slab (per = zs * plane)
+    for_slab_cells(L, [&](int m, int l, bool in, int i, int j, int k) {
+        CSlot q;
+        q.x = 3u << 30;
+        q.y = 0;
+        if (in) {
+            const int xm = (i == 0) ? l + (nx - 1) : l - 1;
+            const int xp = (i == nx - 1) ? l - (nx - 1) : l + 1;
+            const int ym = (j == 0) ? l + (plane - nx) : l - nx;
+            const int yp = (j == ny - 1) ? l - (plane - nx) : l + nx;
+            const int kl = k - rank * zs;          // plane index inside the slab
+            q.x = (uint32_t)xm | ((uint32_t)xp << 12) | ((uint32_t)(kl == 0) << 24) | ((uint32_t)(kl == zs - 1) << 25) |
+                  ((uint32_t)((i + j + k) & 1) << 30);
+            q.y = (uint32_t)ym | ((uint32_t)yp << 12);
+        }
+        s[m] = q;
+    });
+}
+
+__device__ __forceinline__ Cell slot_cell(const CLevel& L, const CZ& z, const CSlot& s, int l) {
     const int per = L.per;
     const float* W = L.W;
     const float w0 = W[l], w1 = W[per + l], w2 = W[2 * per + l], w3 = W[3 * per + l], w4 = W[4 * per + l],
                 w5 = W[5 * per + l];
     const float* p = L.p;
+    // below / above: the same column one plane away -- in the neighbouring slab its last / first plane
+    const float pzm = (s.x & (1u << 24)) ? ld_cluster(map_rank(z.pa + 4u * (uint32_t)(l + z.wrap), z.rm)) : p[l - z.plane];
+    const float pzp = (s.x & (1u << 25)) ? ld_cluster(map_rank(z.pa + 4u * (uint32_t)(l - z.wrap), z.rp)) : p[l + z.plane];
     Cell r;
     r.pc = p[l];
     r.Ap = apply7(r.pc, w0, w1, w2, w3, w4, w5, p[s.x & 0xfffu], p[(s.x >> 12) & 0xfffu], p[s.y & 0xfffu],
-                  p[s.y >> 12], ld_cluster(s.zm), ld_cluster(s.zp));
+                  p[s.y >> 12], pzm, pzp);
     r.D = diag6(w0, w1, w2, w3, w4, w5);
     return r;
 }
 
 // `count` red-black sweeps on a distributed level; every colour half-sweep ends in a cluster barrier.
-__device__ __forceinline__ void dist_sweeps(const CLevel& L, const CSlot (&s)[kCSlots], float omega, int count,
-                                            int first) {
+__device__ __forceinline__ void dist_sweeps(const CLevel& L, const CZ& z, const CSlot (&s)[kCSlots], float omega,
+                                            int count, int first) {
     for (int h = 0; h < 2 * count; ++h) {
         const int colour = (h & 1) ? 1 - first : first;
 #pragma unroll
         for (int m = 0; m < kCSlots; ++m) {
             if (s[m].colour() != colour) continue;
             const int l = threadIdx.x + m * kTailThreads;
-            const Cell c = slot_cell(L, s[m], l);
+            const Cell c = slot_cell(L, z, s[m], l);
             L.p[l] = relax(c.pc, L.b[l], c.Ap, c.D, omega);
         }
         cluster_sync();
@@ -150,7 +194,7 @@ __device__ __forceinline__ void level_sweeps(const CLevel& L, const CSlot (&s)[k
                                              int count, int first) {
     if (count <= 0) return;
     if (L.dist) {
-        dist_sweeps(L, s, omega, count, first);
+        dist_sweeps(L, make_cz(L, rank), s, omega, count, first);
     } else {
         if (rank == 0) {
             int T = ((int)L.g.N + 31) / 32 * 32;
@@ -201,9 +245,14 @@ __global__ void __cluster_dims__(kCR, 1, 1) __launch_bounds__(kTailThreads, 1) k
 
     CSlot s[kCSlots];
     auto make_slots = [&](const CLevel& L) {
+        if (L.dist) {
+            make_slots_dist(L, rank, s);
+        } else {   // small level: no slots
 #pragma unroll
-        for (int m = 0; m < kCSlots; ++m) {
-            s[m] = make_slot(L, L.dist ? tid + m * kTailThreads : L.per);  // small level: no slots
+            for (int m = 0; m < kCSlots; ++m) {
+                s[m].x = 3u << 30;
+                s[m].y = 0;
+            }
         }
     };
 
@@ -214,11 +263,12 @@ __global__ void __cluster_dims__(kCR, 1, 1) __launch_bounds__(kTailThreads, 1) k
         level_sweeps(L, s, rank, omega, a.t.nu1, 0);
         // residual of the cells held here (0 on inactive cells)
         if (L.dist) {
+            const CZ cz_res = make_cz(L, rank);
 #pragma unroll
             for (int m = 0; m < kCSlots; ++m) {
                 if (s[m].colour() > 1) continue;
                 const int l = tid + m * kTailThreads;
-                const Cell c = slot_cell(L, s[m], l);
+                const Cell c = slot_cell(L, cz_res, s[m], l);
                 L.r[l] = (c.D != 0.0f) ? L.b[l] - c.Ap : 0.0f;
             }
         } else if (rank == 0) {
@@ -238,11 +288,20 @@ __global__ void __cluster_dims__(kCR, 1, 1) __launch_bounds__(kTailThreads, 1) k
             for (int l = tid; l < Lc.per; l += kTailThreads) {
                 const int u = Lc.c0 + l;
                 const int row = u / ncx, I = u - row * ncx, K = row / ncy, J = row - K * ncy;
-                Lc.b[l] = restrict_tree(cx, cy, cz, [&](int e, int bb, int aa) {
-                    const int f = (cx * I + e) + L.g.n[0] * ((cy * J + bb) + L.g.n[1] * (cz * K + aa));
-                    const int fr = L.dist ? f / L.per : 0;
-                    return ld_cluster(map_rank(ra + 4u * (uint32_t)(f - fr * L.per), fr));
-                });
+                if (Lc.dist) {
+                    // both levels cut into slabs: a coarse slab's children are this CTA's fine slab
+                    // (planes cz K .. cz K + cz - 1 with K in the coarse slab): plain shared-memory loads
+                    Lc.b[l] = restrict_tree(cx, cy, cz, [&](int e, int bb, int aa) {
+                        const int f = (cx * I + e) + L.g.n[0] * ((cy * J + bb) + L.g.n[1] * (cz * K + aa));
+                        return L.r[f - L.c0];
+                    });
+                } else {
+                    Lc.b[l] = restrict_tree(cx, cy, cz, [&](int e, int bb, int aa) {
+                        const int f = (cx * I + e) + L.g.n[0] * ((cy * J + bb) + L.g.n[1] * (cz * K + aa));
+                        const int fr = L.dist ? f / L.per : 0;
+                        return ld_cluster(map_rank(ra + 4u * (uint32_t)(f - fr * L.per), fr));
+                    });
+                }
                 Lc.p[l] = 0.0f;
             }
         }
@@ -262,16 +321,24 @@ __global__ void __cluster_dims__(kCR, 1, 1) __launch_bounds__(kTailThreads, 1) k
     // ---- up leg -----------------------------------------------------------------------------------
     for (int t = last - 1; t >= 0; --t) {
         const CLevel L = level(t), Lc = level(t + 1);
-        if (holds(L)) {
+        if (L.dist) {
+            // factors are 1 or 2.  With the coarse level cut into slabs too, the parents of this
+            // slab are the CTA's own coarse slab.
+            const int sx = L.g.c[0] >> 1, sy = L.g.c[1] >> 1, sz = L.g.c[2] >> 1;
+            const int ncx = L.g.n[0] >> sx, ncy = L.g.n[1] >> sy;
+            const uint32_t pa = saddr(Lc.p);
+            for_slab_cells(L, [&](int, int l, bool in, int i, int j, int k) {
+                if (!in) return;
+                const int parent = (i >> sx) + ncx * ((j >> sy) + ncy * (k >> sz));
+                L.p[l] += Lc.dist ? Lc.p[parent - Lc.c0] : ld_cluster(map_rank(pa + 4u * (uint32_t)parent, 0));
+            });
+        } else if (rank == 0) {
             const int nx = L.g.n[0], ny = L.g.n[1];
             const int ncx = nx / L.g.c[0], ncy = ny / L.g.c[1];
-            const uint32_t pa = saddr(Lc.p);
             for (int l = tid; l < L.per; l += kTailThreads) {
-                const int c = L.c0 + l;
-                const int row = c / nx, i = c - row * nx, k = row / ny, j = row - k * ny;
+                const int row = l / nx, i = l - row * nx, k = row / ny, j = row - k * ny;
                 const int parent = (i / L.g.c[0]) + ncx * ((j / L.g.c[1]) + ncy * (k / L.g.c[2]));
-                const int pr = Lc.dist ? parent / Lc.per : 0;
-                L.p[l] += ld_cluster(map_rank(pa + 4u * (uint32_t)(parent - pr * Lc.per), pr));
+                L.p[l] += Lc.p[parent];   // both levels live here
             }
         }
         cluster_sync();
