@@ -704,7 +704,7 @@ k_rb_sweep_bulk(const BulkArgs a, const __grid_constant__ BulkMaps maps) {
 
 // The lean path as a kernel of its own: the box-fed tiles whose footprint is uniform; every other
 // tile of the grid returns at once (k_rb_sweep_bulk takes those).  Without coefficient rings a CTA
-// needs 88 KB of shared memory and 64 registers per thread, so TWO CTAs share an SM and one fills
+// needs 102 KB of shared memory and 96-128 registers per thread, so TWO CTAs share an SM and one fills
 // the other's barrier and latency gaps (issue slots 44 % -> 69 % busy).
 template <class C, int NORM = 0>
 __global__ void __launch_bounds__(Lean2Threads<(NORM != 0)>::value, 2)

@@ -8,7 +8,7 @@
 // (source values) for phase B, in plane u-1 (its own phase-B results of the step before) for phase C --
 // and carries plane u+1 into the next step as "own": 8 instead of 18 float4 loads per 8 cells.  Eight
 // main warps cover the 15 phase-B rows of a 128 x 13 tile (the last thread row has one row only), one
-// edge warp the two ring-1 columns: 288 threads, two CTAs per SM, up to 112 registers, operands of
+// edge warp the two ring-1 columns: 288 threads, two CTAs per SM, 96 registers (a CTA's 9 warps are allocated as 10), operands of
 // the next step loaded in front of the barrier as in sweep_body.  Same update_pair_* calls on the same
 // operands: bit-identical to sweep_body (tests).  Included by kernels_sweep.cu.
 #pragma once
