@@ -32,7 +32,7 @@
 
 namespace gmgf {
 // LEAN_: the layout of the kernel that runs ONLY the lean path (uniform.cuh): no coefficient rings,
-// 88 KB instead of 190 KB, so that two CTAs share an SM.
+// 102 KB instead of 190 KB, so that two CTAs share an SM.
 template <int TY_, int PD_, bool LEAN_ = false>
 struct BulkCfg {
     static constexpr int TX = 128, TY = TY_, PD = PD_;
