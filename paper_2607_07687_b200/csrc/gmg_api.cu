@@ -627,6 +627,21 @@ extern "C" int gmg_level_coeffs(gmg_ctx* c, int lev, float* L_out_dev, void* str
 // e_c != nullptr: the coarse correction P e_c is added to p first (fused into the first sweep
 // on the fast path, a separate kernel otherwise).
 // skip_first: the first fused sweep p -> q of this call has already been run (fused_norm path).
+// Kernels one TMA-fed sweep of level l launches beyond the first: with uniform bricks marked the lean
+// tiles and the remaining tiles are two kernels (one when either set is known to be empty), and a
+// sweep that folds the prolongation in copies the footprints of the remaining tiles first.
+static int sweep_extra_launches(const gmg_ctx* c, int l, bool with_pro) {
+    if (!(c->fast_sweep[l] && c->tma_ok[l] && gmgf::tma_shape_ok(c->g[l]))) return 0;
+    const gmgf::UniArgs& u = U(c, l);
+    if (!u.brick) return 0;
+    int ty = 0, zc = 0;
+    if (!gmgf::bulk_sweep_tiling(c->g[l], &ty, &zc)) return 0;
+    const long long tiles = (long long)(c->g[l].n[0] / 128) * ((c->g[l].n[1] + ty - 1) / ty) * ((c->g[l].n[2] + zc - 1) / zc);
+    if (u.left_list && u.left_n == tiles) return 0;   // no lean tile: one kernel over the whole grid
+    if (u.left_n == 0) return 0;                      // every tile lean
+    return with_pro ? 2 : 1;
+}
+
 static void smooth(gmg_ctx* c, int l, float* p, const float* b, const float* omega, int nsweeps,
                    int first_colour, const float* e_c, cudaStream_t s, int skip_first = 0) {
     const LevelGeom& g = c->g[l];
@@ -635,7 +650,6 @@ static void smooth(gmg_ctx* c, int l, float* p, const float* b, const float* ome
         if (gmgf::sweep_fuses_prolong(g, U(c, l))) {
             // uniform bricks: the first sweep takes the correction along (lean tiles on the fly, the
             // others through a corrected copy of their footprints): e_c stays
-            c->n_launch += 1;
         } else {
             // in front of the general TMA-fed sweep the correction is cheaper as its own streaming pass
             gmgf::prolong_add4(g, e_c, p, s);
@@ -649,10 +663,10 @@ static void smooth(gmg_ctx* c, int l, float* p, const float* b, const float* ome
         for (int i = 0; i < pairs; ++i) {
             if (!(i == 0 && skip_first)) {
                 gmgf::rb_sweep(g, c->lv[l].L, p, q, b, omega, first_colour, (i == 0) ? e_c : nullptr, c->tma_ok[l], U(c, l), s);
-                c->n_launch += 1;
+                c->n_launch += 1 + sweep_extra_launches(c, l, i == 0 && e_c != nullptr);
             }
             gmgf::rb_sweep(g, c->lv[l].L, q, p, b, omega, first_colour, nullptr, c->tma_ok[l], U(c, l), s);
-            c->n_launch += 1;
+            c->n_launch += 1 + sweep_extra_launches(c, l, false);
         }
         done = 2 * pairs;
         e_c = nullptr;
@@ -855,7 +869,7 @@ static void rbgs_pre(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStrea
     if (!cgs && fused_norm_active(c)) {
         first_sweep_with_norm(c, p, z, &c->sc->omega_f, true, nullptr, s);
         gmgk::ctl_begin(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
-        c->n_launch += 2;
+        c->n_launch += 2 + sweep_extra_launches(c, 0, false);
         return;
     }
     // reference norm ||z|| over active cells and initial residual norm: one fused pass on big levels
@@ -875,7 +889,7 @@ static void rbgs_body(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStre
         const bool pred = predict_active(c);
         if (pred) {   // after a failed "last cycle" prediction the first sweep is still to run
             MUST_LAUNCH(c, gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->need_first, U(c, 0), s));
-            c->n_launch += 1;
+            c->n_launch += 1 + sweep_extra_launches(c, 0, false);
         }
         enqueue_vcycle(c, p, z, &c->sc->omega_f, 0, s, 1);             // its first sweep already ran
         if (pred) {   // expected to be the last cycle: the plain norm pass
@@ -886,7 +900,7 @@ static void rbgs_body(gmg_ctx* c, float* p, const float* z, LoopCtl lc, cudaStre
         first_sweep_with_norm(c, p, z, &c->sc->omega_spec_f, false, pred ? &c->sc->run_s1n : nullptr, s);
         gmgk::ctl_rbgs_cycle_end(c->sc, c->hist, c->omegas, lc.cond, lc.use_cond, s);
         MUST_LAUNCH(c, gmgf::rb_sweep_if(c->g[0], c->lv[0].L, p, c->lv[0].q, z, &c->sc->omega_f, 0, &c->sc->redo_first, U(c, 0), s));
-        c->n_launch += 3;
+        c->n_launch += 3 + 2 * sweep_extra_launches(c, 0, false);   // (gated launches count: they are launches)
         return;
     }
     if (cgs) enqueue_vcycle_cgs(c, p, z, s);
