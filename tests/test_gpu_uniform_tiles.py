@@ -220,3 +220,26 @@ def test_pressure_steps_with_a_moving_body_bit_identical():
     for a, b in zip(*runs):
         assert a[:2] == b[:2] and a[0] == gmg.OK
         assert torch.equal(a[2], b[2]) and torch.equal(a[3], b[3])
+
+
+@pytest.mark.parametrize("nu_pre,nu_post", [(1, 3), (3, 2), (2, 1), (4, 4), (0, 2)])
+def test_other_sweep_counts_bit_identical(nu_pre, nu_post):
+    """Odd and larger sweep counts take other routes through smooth(): pairs of fused sweeps, a last
+    sweep as two half-sweeps, the prolongation folded in only where a pair follows it."""
+    wl = _ones_with_bodies((256, 128, 64), (0, 0, 0), 6, nblobs=1)
+    on = make_gpu(wl, tma_min_cells=0, uniform_tiles=1, nu_pre=nu_pre, nu_post=nu_post)
+    off = make_gpu(wl, tma_min_cells=0, uniform_tiles=0, nu_pre=nu_pre, nu_post=nu_post)
+    try:
+        p, b = _fields(wl, 66)
+        for sym in (False, True):
+            assert torch.equal(on.op_vcycle(p.clone(), b, omega=0.9375, symmetric=sym),
+                               off.op_vcycle(p.clone(), b, omega=0.9375, symmetric=sym))
+        out = []
+        for g in (on, off):
+            x = torch.zeros(wl.z.shape, dtype=torch.float32, device="cuda")
+            rc = g.solve(x, dev(wl.z), tol=1e-5, maxiter=80)
+            out.append((rc, g.stats()["iterations"], x))
+        assert out[0][:2] == out[1][:2] and torch.equal(out[0][2], out[1][2])
+    finally:
+        on.close()
+        off.close()
