@@ -138,6 +138,7 @@ struct gmg_ctx {
 // Jacobi-PCG: 5.2 vs 5.7 ms per solve), whatever tma_min_cells says for the sweeps -- unless it is
 // 0 ("whenever the shape allows": the tests force the TMA path on small grids that way).
 static const long long kBulkMatvecMinCells = 4LL << 20;
+static const long long kLeanVectorMinCells = 8LL << 20;   // (tma_min_cells = 0 forces both, for the tests)
 
 static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 // behind the brick flags: [2][levels] u64 lean-cell counts, [levels] u32 remaining-tile list lengths
@@ -734,6 +735,14 @@ static void enqueue_vcycle(gmg_ctx* c, float* p0, const float* b0, const float* 
 // m Jacobi-PCG iterations on A^l x = b restarted from x.  The four CG vectors are the level-0
 // sized PCG vectors of the workspace on EVERY level: the CG state does not survive the visit to
 // the coarser levels (the post-smoothing restarts), so the levels can share them.
+// The float4 vector kernels of the CG iterations (kernels_pcg4.cu) skip the coefficient loads of the
+// groups whose faces all carry the level's constants -- where the level streams from DRAM.  On an
+// L2-resident level the brick look-up in front of the loads only adds latency (256 x 96 x 96: PCG
+// 22.3 -> 24.3 ms), so it stays off there.
+static const gmgf::UniArgs* lean_vectors(const gmg_ctx* c, int l) {
+    return (c->uni[l].brick && (c->prm.tma_min_cells == 0 || c->g[l].N >= kLeanVectorMinCells)) ? &c->uni[l] : nullptr;
+}
+
 static void cg_smooth(gmg_ctx* c, int l, float* x, const float* b, int m, cudaStream_t s) {
     if (m <= 0) return;
     const LevelGeom& g = c->g[l];
@@ -754,17 +763,18 @@ static void cg_smooth(gmg_ctx* c, int l, float* x, const float* b, int m, cudaSt
     rb_begin.post_arg = alpha_cap;
     rb_alpha.post = POST_CGS_ALPHA;
     rb_beta.post = POST_CGS_BETA;
-    gmgk::cgs_residual_sum(g, L, x, b, r, rbuf(c), s);
-    gmgk::cgs_start(g, L, r, d, rb_begin, s);      // r -= mean; d = r/D; rho = r.d; begin
+    const gmgf::UniArgs* ul = lean_vectors(c, l);   // lean path of the float4 kernels
+    gmgk::cgs_residual_sum(g, L, x, b, r, rbuf(c), s, ul);
+    gmgk::cgs_start(g, L, r, d, rb_begin, s, ul);  // r -= mean; d = r/D; rho = r.d; begin
     c->n_launch += 2;
     for (int it = 0; it < m; ++it) {
         if (!(c->prm.fast_path && c->tma_ok[l] && (c->prm.tma_min_cells == 0 || g.N >= kBulkMatvecMinCells) &&
               gmgf::matvec_dot_bulk(g, L, d, q, rb_alpha, RED_DQ, U(c, l), s)))
-            gmgk::matvec_dot(g, L, d, q, rb_alpha, RED_DQ, s);     // ... alpha
+            gmgk::matvec_dot(g, L, d, q, rb_alpha, RED_DQ, s, ul);     // ... alpha
         gmgk::pcg_update_pr(g, L, x, r, d, q, nullptr, 0, rbuf(c), s);
         c->n_launch += 2;
         if (it == m - 1) break;
-        gmgk::jacobi_apply(g, L, r, sv, rb_beta, RED_RS, s);       // ... beta
+        gmgk::jacobi_apply(g, L, r, sv, rb_beta, RED_RS, s, ul);   // ... beta
         gmgk::pcg_update_d(g.N, d, sv, c->sc, 0, s);
         c->n_launch += 2;
     }
@@ -926,7 +936,7 @@ static void pcg_body(gmg_ctx* c, float* p, int gmg_precond, LoopCtl lc, cudaStre
     rb_beta.post = POST_PCG_BETA;
     rb_alpha.post = POST_PCG_ALPHA;
     if (!gmg_precond) {
-        gmgk::jacobi_apply(c->g[0], c->lv[0].L, c->pcg_r, c->pcg_s, rb_beta, RED_RS, s);
+        gmgk::jacobi_apply(c->g[0], c->lv[0].L, c->pcg_r, c->pcg_s, rb_beta, RED_RS, s, lean_vectors(c, 0));
         c->n_launch += 1;
     } else {
         gmgk::fill(c->pcg_s, N, 0.0f, s);
@@ -937,7 +947,7 @@ static void pcg_body(gmg_ctx* c, float* p, int gmg_precond, LoopCtl lc, cudaStre
     gmgk::pcg_update_d(N, c->pcg_d, c->pcg_s, c->sc, 0, s);
     if (!(c->prm.fast_path && c->tma_ok[0] && (c->prm.tma_min_cells == 0 || c->g[0].N >= kBulkMatvecMinCells) &&
           gmgf::matvec_dot_bulk(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rb_alpha, RED_DQ, U(c, 0), s)))
-        gmgk::matvec_dot(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rb_alpha, RED_DQ, s);
+        gmgk::matvec_dot(c->g[0], c->lv[0].L, c->pcg_d, c->pcg_q, rb_alpha, RED_DQ, s, lean_vectors(c, 0));
     gmgk::pcg_update_pr(c->g[0], c->lv[0].L, p, c->pcg_r, c->pcg_d, c->pcg_q, nullptr, 0, rbuf(c), s);
     gmgk::ctl_pcg_check(c->sc, c->hist, lc.cond, lc.use_cond, s);
     c->n_launch += 4;

@@ -160,15 +160,17 @@ void norm2(long long N, const float* r, ReduceBuf rb, int slot, cudaStream_t s);
 void dot(long long N, const float* a, const float* b, ReduceBuf rb, int slot, cudaStream_t s);
 
 // PCG pieces
+// (uni: uniform bricks of the level, uniform.cuh -- the float4 kernels then skip the coefficient loads
+// of the groups whose faces all carry the level's constants; nullptr = load everything)
 void matvec_dot(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb,
-                int slot, cudaStream_t s);              // q = A d ; red[slot] = d.q
+                int slot, cudaStream_t s, const gmgf::UniArgs* uni = nullptr);   // q = A d ; red[slot] = d.q
 void pcg_update_pr(const LevelGeom& g, const float* L, float* p, float* r, const float* d,
                    const float* q, float* s_out, int jacobi, ReduceBuf rb, cudaStream_t st);
 // p += alpha d; r -= alpha q; red[RR] = r.r; if jacobi: s = r/D, red[RS] = r.s
 void pcg_update_d(long long N, float* d, const float* s_in, const DevScalars* sc, int first,
                   cudaStream_t st);                      // d = s + beta d   (first: d = s)
 void jacobi_apply(const LevelGeom& g, const float* L, const float* r, float* s_out, ReduceBuf rb,
-                  int slot, cudaStream_t st);            // s = r/D ; red[slot] = r.s
+                  int slot, cudaStream_t st, const gmgf::UniArgs* uni = nullptr);   // s = r/D ; red[slot] = r.s
 
 // on-device iteration control (single-thread kernels, kernels_ctl.cu).  `cond` is the WHILE
 // node's conditional handle; use_cond = 0 outside a graph.
@@ -186,9 +188,10 @@ void ctl_set_hook_omega(DevScalars* sc, float omega, cudaStream_t s);
 // CG smoother of the paper's GMG-PCG (kernels_cgs.cu, reading O12)
 // r = b - A x (0 on inactive cells); red[CGS_SUM] = sum r, red[CGS_CNT] = number of active cells
 void cgs_residual_sum(const LevelGeom& g, const float* L, const float* x, const float* b, float* r,
-                      ReduceBuf rb, cudaStream_t s);
+                      ReduceBuf rb, cudaStream_t s, const gmgf::UniArgs* uni = nullptr);
 // r -= mean over active cells; d = r/D; red[RS] = r.d
-void cgs_start(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s);
+void cgs_start(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s,
+               const gmgf::UniArgs* uni = nullptr);
 // (the smoother's control steps -- begin, alpha, beta -- ride on cgs_start, the mat-vec and the
 // Jacobi kernel: ReduceBuf::post)
 // m iterations restarted from x (in place) on a level of at most 4096 cells with nx % 4 == 0, as one

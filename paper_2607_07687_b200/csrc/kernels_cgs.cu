@@ -16,8 +16,9 @@ static constexpr int kCT = 256;
 
 // float4 versions (kernels_pcg4.cu); false = shape or alignment not eligible
 bool cgs_residual_sum4(const LevelGeom& g, const float* L, const float* x, const float* b, float* r,
-                       ReduceBuf rb, cudaStream_t s);
-bool cgs_start4(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s);
+                       ReduceBuf rb, cudaStream_t s, const gmgf::UniArgs* uni);
+bool cgs_start4(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s,
+                const gmgf::UniArgs* uni);
 
 static inline unsigned int cgs_blocks(long long N) {
     long long b = (N + (long long)kCT * 8 - 1) / ((long long)kCT * 8);
@@ -54,8 +55,8 @@ k_cgs_residual_sum(LevelGeom g, const float* __restrict__ L, const float* __rest
 }
 
 void cgs_residual_sum(const LevelGeom& g, const float* L, const float* x, const float* b, float* r,
-                      ReduceBuf rb, cudaStream_t s) {
-    if (cgs_residual_sum4(g, L, x, b, r, rb, s)) return;
+                      ReduceBuf rb, cudaStream_t s, const gmgf::UniArgs* uni) {
+    if (cgs_residual_sum4(g, L, x, b, r, rb, s, uni)) return;
     k_cgs_residual_sum<<<cgs_blocks(g.N), kCT, 0, s>>>(g, L, x, b, r, rb);
 }
 
@@ -82,8 +83,9 @@ k_cgs_start(LevelGeom g, const float* __restrict__ L, float* __restrict__ r, flo
     finish_reduction(acc, 0.0, false, rb, RED_RS, 0);
 }
 
-void cgs_start(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s) {
-    if (cgs_start4(g, L, r, d, rb, s)) return;
+void cgs_start(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s,
+               const gmgf::UniArgs* uni) {
+    if (cgs_start4(g, L, r, d, rb, s, uni)) return;
     k_cgs_start<<<cgs_blocks(g.N), kCT, 0, s>>>(g, L, r, d, rb);
 }
 

@@ -4,6 +4,7 @@
 // (same apply7 / diag6 argument order); only the order in which the FP64 partial sums are
 // accumulated differs.  The launchers there dispatch here when nx % 4 == 0.
 #include "stencil.cuh"
+#include "uniform.cuh"
 
 namespace gmgk {
 using namespace gmgd;
@@ -60,6 +61,48 @@ __device__ __forceinline__ W4 weights4(const LevelGeom& g, const float* __restri
     return w;
 }
 
+// Uniform bricks (uniform.cuh) in the float4 kernels: where every brick that holds one of the faces of
+// a group is marked and none of them is a wall face, the six weights are the level's constants and
+// the three coefficient arrays are not loaded (12 of the 20-24 B/cell of these passes); the same
+// diag6 / apply7 run on the constants, so every cell gets the same bits.
+struct UniK {
+    const unsigned char* brick;   // nullptr: disabled
+    float ux, uy, uz;
+};
+static inline UniK unik(const gmgf::UniArgs* u) {
+    UniK k;
+    k.brick = u ? u->brick : nullptr;
+    k.ux = u ? u->ux : 0.0f;
+    k.uy = u ? u->uy : 0.0f;
+    k.uz = u ? u->uz : 0.0f;
+    return k;
+}
+__device__ __forceinline__ bool group_uniform(const LevelGeom& g, const UniK& u, int i, int j, int k) {
+    if (!u.brick) return false;
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    if ((g.bc[0] && (i == 0 || i + 4 == nx)) || (g.bc[1] && (j == 0 || j == ny - 1)) ||
+        (g.bc[2] && (k == 0 || k == nz - 1)))
+        return false;   // wall faces carry 0, not the constant
+    const int nbx = gmgf::ub_count(nx, gmgf::kUBX), nby = gmgf::ub_count(ny, gmgf::kUBY);
+    const int bx = i / gmgf::kUBX, by = j / gmgf::kUBY, bz = k / gmgf::kUBZ;
+    const int i4 = (i + 4 == nx) ? 0 : i + 4, j1 = (j == ny - 1) ? 0 : j + 1, k1 = (k == nz - 1) ? 0 : k + 1;
+    const unsigned char* row = u.brick + ((size_t)bz * nby + by) * nbx;
+    return __ldg(row + bx) && __ldg(row + i4 / gmgf::kUBX) &&
+           __ldg(u.brick + ((size_t)bz * nby + j1 / gmgf::kUBY) * nbx + bx) &&
+           __ldg(u.brick + ((size_t)(k1 / gmgf::kUBZ) * nby + by) * nbx + bx);
+}
+__device__ __forceinline__ W4 weights4_uni(const LevelGeom& g, const float* __restrict__ L, const UniK& u, int i, int j,
+                                           int k, long long c) {
+    if (group_uniform(g, u, i, j, k)) {
+        W4 w;
+        w.xl = w.xh = splat4(u.ux);
+        w.yl = w.yh = splat4(u.uy);
+        w.zl = w.zh = splat4(u.uz);
+        return w;
+    }
+    return weights4(g, L, i, j, k, c);
+}
+
 // group index -> (i, j, k); 32-bit arithmetic (a level has fewer than 2^31 cells)
 __device__ __forceinline__ void unflat4(const LevelGeom& g, unsigned int t, int& i, int& j, int& k) {
     const unsigned int nx4 = (unsigned int)g.n[0] >> 2, ny = (unsigned int)g.n[1];
@@ -73,7 +116,7 @@ __device__ __forceinline__ void unflat4(const LevelGeom& g, unsigned int t, int&
 // q = A d on every cell ; red[slot] = d.q
 __global__ void __launch_bounds__(kPT)
 k_matvec_dot4(LevelGeom g, const float* __restrict__ L, const float* __restrict__ d, float* __restrict__ q,
-              ReduceBuf rb, int slot) {
+              ReduceBuf rb, int slot, UniK uni) {
     const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
     const long long sy = nx, sz = (long long)nx * ny;
     const unsigned int groups = (unsigned int)(g.N >> 2);
@@ -82,7 +125,7 @@ k_matvec_dot4(LevelGeom g, const float* __restrict__ L, const float* __restrict_
         int i, j, k;
         unflat4(g, t, i, j, k);
         const long long c = 4LL * t;
-        const W4 w = weights4(g, L, i, j, k, c);
+        const W4 w = weights4_uni(g, L, uni, i, j, k, c);
         const float4 dc = ldg4(d + c);
         const float dxm = __ldg(d + ((i == 0) ? c + (nx - 1) : c - 1));
         const float dxp = __ldg(d + ((i + 4 == nx) ? c - (nx - 4) : c + 4));
@@ -105,14 +148,14 @@ k_matvec_dot4(LevelGeom g, const float* __restrict__ L, const float* __restrict_
 // s = r / D on active cells, 0 elsewhere (Jacobi) ; red[slot] = r.s
 __global__ void __launch_bounds__(kPT)
 k_jacobi_apply4(LevelGeom g, const float* __restrict__ L, const float* __restrict__ r, float* __restrict__ s_out,
-                ReduceBuf rb, int slot) {
+                ReduceBuf rb, int slot, UniK uni) {
     const unsigned int groups = (unsigned int)(g.N >> 2);
     double acc = 0.0;
     for (unsigned int t = blockIdx.x * kPT + threadIdx.x; t < groups; t += gridDim.x * kPT) {
         int i, j, k;
         unflat4(g, t, i, j, k);
         const long long c = 4LL * t;
-        const W4 w = weights4(g, L, i, j, k, c);
+        const W4 w = weights4_uni(g, L, uni, i, j, k, c);
         const float4 rv = ldg4(r + c);
         const float Dx = diag6(w.xl.x, w.xh.x, w.yl.x, w.yh.x, w.zl.x, w.zh.x);
         const float Dy = diag6(w.xl.y, w.xh.y, w.yl.y, w.yh.y, w.zl.y, w.zh.y);
@@ -181,7 +224,7 @@ k_dot4(long long groups, const float4* __restrict__ a, const float4* __restrict_
 // r = b - A x on active cells, 0 elsewhere ; red[CGS_SUM] = sum r ; red[CGS_CNT] = #active
 __global__ void __launch_bounds__(kPT)
 k_cgs_residual_sum4(LevelGeom g, const float* __restrict__ L, const float* __restrict__ x,
-                    const float* __restrict__ b, float* __restrict__ r, ReduceBuf rb) {
+                    const float* __restrict__ b, float* __restrict__ r, ReduceBuf rb, UniK uni) {
     const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
     const long long sy = nx, sz = (long long)nx * ny;
     const unsigned int groups = (unsigned int)(g.N >> 2);
@@ -190,7 +233,7 @@ k_cgs_residual_sum4(LevelGeom g, const float* __restrict__ L, const float* __res
         int i, j, k;
         unflat4(g, t, i, j, k);
         const long long c = 4LL * t;
-        const W4 w = weights4(g, L, i, j, k, c);
+        const W4 w = weights4_uni(g, L, uni, i, j, k, c);
         const float4 xc = ldg4(x + c);
         const float xm = __ldg(x + ((i == 0) ? c + (nx - 1) : c - 1));
         const float xp = __ldg(x + ((i + 4 == nx) ? c - (nx - 4) : c + 4));
@@ -222,7 +265,7 @@ k_cgs_residual_sum4(LevelGeom g, const float* __restrict__ L, const float* __res
 // active cells: r -= mean ; d = r/D ; inactive: d = 0 ; red[RS] = r.d
 __global__ void __launch_bounds__(kPT)
 k_cgs_start4(LevelGeom g, const float* __restrict__ L, float* __restrict__ r, float* __restrict__ d,
-             ReduceBuf rb) {
+             ReduceBuf rb, UniK uni) {
     const unsigned int groups = (unsigned int)(g.N >> 2);
     const float mu = cgs_mean(rb.sc);
     double acc = 0.0;
@@ -230,7 +273,7 @@ k_cgs_start4(LevelGeom g, const float* __restrict__ L, float* __restrict__ r, fl
         int i, j, k;
         unflat4(g, t, i, j, k);
         const long long c = 4LL * t;
-        const W4 w = weights4(g, L, i, j, k, c);
+        const W4 w = weights4_uni(g, L, uni, i, j, k, c);
         const float4 r0 = *reinterpret_cast<const float4*>(r + c);
         const float Dx = diag6(w.xl.x, w.xh.x, w.yl.x, w.yh.x, w.zl.x, w.zh.x);
         const float Dy = diag6(w.xl.y, w.xh.y, w.yl.y, w.yh.y, w.zl.y, w.zh.y);
@@ -425,15 +468,15 @@ bool cgs_small(const LevelGeom& g, const float* L, float* x, const float* b, int
 }
 
 bool matvec_dot4(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot,
-                 cudaStream_t s) {
+                 cudaStream_t s, const gmgf::UniArgs* uni) {
     if (g.n[0] % 4 != 0 || !al16(L) || !al16(d) || !al16(q)) return false;
-    k_matvec_dot4<<<blocks_plane(g), kPT, 0, s>>>(g, L, d, q, rb, slot);
+    k_matvec_dot4<<<blocks_plane(g), kPT, 0, s>>>(g, L, d, q, rb, slot, unik(uni));
     return true;
 }
 bool jacobi_apply4(const LevelGeom& g, const float* L, const float* r, float* s_out, ReduceBuf rb, int slot,
-                   cudaStream_t st) {
+                   cudaStream_t st, const gmgf::UniArgs* uni) {
     if (g.n[0] % 4 != 0 || !al16(L) || !al16(r) || !al16(s_out)) return false;
-    k_jacobi_apply4<<<blocks_plane(g), kPT, 0, st>>>(g, L, r, s_out, rb, slot);
+    k_jacobi_apply4<<<blocks_plane(g), kPT, 0, st>>>(g, L, r, s_out, rb, slot, unik(uni));
     return true;
 }
 bool pcg_update_pr4(long long N, float* p, float* r, const float* d, const float* q, ReduceBuf rb,
@@ -452,14 +495,15 @@ bool pcg_update_d4(long long N, float* d, const float* s_in, const DevScalars* s
     return true;
 }
 bool cgs_residual_sum4(const LevelGeom& g, const float* L, const float* x, const float* b, float* r,
-                       ReduceBuf rb, cudaStream_t s) {
+                       ReduceBuf rb, cudaStream_t s, const gmgf::UniArgs* uni) {
     if (g.n[0] % 4 != 0 || !al16(L) || !al16(x) || !al16(b) || !al16(r)) return false;
-    k_cgs_residual_sum4<<<blocks_plane(g), kPT, 0, s>>>(g, L, x, b, r, rb);
+    k_cgs_residual_sum4<<<blocks_plane(g), kPT, 0, s>>>(g, L, x, b, r, rb, unik(uni));
     return true;
 }
-bool cgs_start4(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s) {
+bool cgs_start4(const LevelGeom& g, const float* L, float* r, float* d, ReduceBuf rb, cudaStream_t s,
+                const gmgf::UniArgs* uni) {
     if (g.n[0] % 4 != 0 || !al16(L) || !al16(r) || !al16(d)) return false;
-    k_cgs_start4<<<blocks_plane(g), kPT, 0, s>>>(g, L, r, d, rb);
+    k_cgs_start4<<<blocks_plane(g), kPT, 0, s>>>(g, L, r, d, rb, unik(uni));
     return true;
 }
 bool dot4(long long N, const float* a, const float* b, ReduceBuf rb, int slot, cudaStream_t s) {

@@ -16,8 +16,10 @@ using namespace gmgd;
 static constexpr int kRT = 256;  // threads per reduction block
 
 // float4 versions (kernels_pcg4.cu); false = shape or alignment not eligible
-bool matvec_dot4(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot, cudaStream_t s);
-bool jacobi_apply4(const LevelGeom& g, const float* L, const float* r, float* s_out, ReduceBuf rb, int slot, cudaStream_t st);
+bool matvec_dot4(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb, int slot, cudaStream_t s,
+                 const gmgf::UniArgs* uni);
+bool jacobi_apply4(const LevelGeom& g, const float* L, const float* r, float* s_out, ReduceBuf rb, int slot, cudaStream_t st,
+                   const gmgf::UniArgs* uni);
 bool pcg_update_pr4(long long N, float* p, float* r, const float* d, const float* q, ReduceBuf rb, cudaStream_t st);
 bool pcg_update_d4(long long N, float* d, const float* s_in, const DevScalars* sc, cudaStream_t st);
 bool dot4(long long N, const float* a, const float* b, ReduceBuf rb, int slot, cudaStream_t s);
@@ -131,8 +133,8 @@ k_matvec_dot(LevelGeom g, const float* __restrict__ L, const float* __restrict__
 }
 
 void matvec_dot(const LevelGeom& g, const float* L, const float* d, float* q, ReduceBuf rb,
-                int slot, cudaStream_t s) {
-    if (matvec_dot4(g, L, d, q, rb, slot, s)) return;
+                int slot, cudaStream_t s, const gmgf::UniArgs* uni) {
+    if (matvec_dot4(g, L, d, q, rb, slot, s, uni)) return;
     k_matvec_dot<<<reduce_blocks(g.N), kRT, 0, s>>>(g, L, d, q, rb, slot);
 }
 
@@ -195,8 +197,8 @@ k_jacobi_apply(LevelGeom g, const float* __restrict__ L, const float* __restrict
 }
 
 void jacobi_apply(const LevelGeom& g, const float* L, const float* r, float* s_out, ReduceBuf rb,
-                  int slot, cudaStream_t st) {
-    if (jacobi_apply4(g, L, r, s_out, rb, slot, st)) return;
+                  int slot, cudaStream_t st, const gmgf::UniArgs* uni) {
+    if (jacobi_apply4(g, L, r, s_out, rb, slot, st, uni)) return;
     k_jacobi_apply<<<reduce_blocks(g.N), kRT, 0, st>>>(g, L, r, s_out, rb, slot);
 }
 
